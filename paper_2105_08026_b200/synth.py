@@ -1,0 +1,150 @@
+"""Seeded synthetic inputs for the five BASELINE.json configs (C0..C4).
+
+This module serves BOTH the CUDA path and the oracle and therefore holds none of the method's
+arithmetic (no log-density, no RAM step, no Philox stream of the sampler): it only simulates
+catalogs with the shape of the paper's workloads -- one latent per object, heteroscedastic Gaussian
+member likelihoods, volume-uniform distances, flux-limited thinning -- with
+BASELINE.json's parameter values.  The paper's own simulated catalogs are not available; these
+stand in for them.  Random numbers: numpy's Philox bit generator, keyed by the
+config's seed, so every call is reproducible on any machine.
+"""
+from dataclasses import dataclass
+
+import numpy as np
+
+M_NORMAL1D, M_THINNED_SCHECHTER1D, M_BINORMAL2D, M_LINREG_ME1D = 0, 1, 2, 3
+F64, F32_STATE_F64_REDUCE = 0, 1
+
+
+@dataclass(frozen=True)
+class RunConfig:
+    name: str
+    model: int
+    precision: int
+    n_objects: int
+    n_iter: int
+    burn_in: int
+    thin: int
+    target_accept_chi: float
+    target_accept_theta: float
+    keep_chi_moments: bool
+    seed: int
+
+
+# BASELINE.json "configs" 0..4 (burn-in / thinning where BASELINE is silent: DESIGN.md section 7)
+CONFIGS = {
+    "C0": RunConfig("C0", M_NORMAL1D, F64, 1_000, 2_000, 500, 1, 0.44, 0.234, True, 0),
+    "C1": RunConfig("C1", M_THINNED_SCHECHTER1D, F64, 100_000, 5_000, 1_000, 1, 0.44, 0.234, False, 1),
+    "C2": RunConfig("C2", M_THINNED_SCHECHTER1D, F64, 300_000, 10_000, 2_000, 10, 0.44, 0.234, True, 2),
+    "C3": RunConfig("C3", M_BINORMAL2D, F64, 1_000_000, 5_000, 1_000, 1, 0.234, 0.234, False, 3),
+    "C4": RunConfig("C4", M_LINREG_ME1D, F32_STATE_F64_REDUCE, 10_000_000, 2_000, 500, 1, 0.44, 0.234, False, 4),
+}
+
+# constants of the thinned point-process configs: {F_lim, sigma_F, x_lo, x_hi, r_min, r_max}
+SCHECHTER_CONSTS = np.array([1e-3, 1e-4, np.log(1e-4), np.log(30.0), 1.0, 10.0 ** (1.0 / 3.0)])
+SCHECHTER_TRUTH = (-1.2, 0.0)   # (alpha, x* = log L*)
+
+
+def _rng(seed):
+    return np.random.Generator(np.random.Philox(key=int(seed)))
+
+
+def _round_f32(cols):
+    return [c.astype(np.float32).astype(np.float64) for c in cols]
+
+
+def make_normal1d(n, seed=0, fp32=False):
+    """C0: sigma_i ~ U(0.5,1.5); chi_i ~ N(0,1); y_i = chi_i + sigma_i eps."""
+    g = _rng(seed)
+    sigma = g.uniform(0.5, 1.5, n)
+    chi = g.standard_normal(n)
+    y = chi + sigma * g.standard_normal(n)
+    cols = [y, sigma]
+    if fp32:
+        cols = _round_f32(cols)
+    sd = float(np.std(cols[0])) if n > 1 else 1.0
+    return dict(model=M_NORMAL1D, cols=cols, consts=None, chi_true=chi[None, :],
+                theta_true=np.array([0.0, 0.0]),
+                theta0=np.array([float(np.mean(cols[0])) if n else 0.0, np.log(max(sd, 1e-3))]))
+
+
+def make_thinned_schechter1d(n, seed=1):
+    """C1/C2: latent x = ln L from the density prop. to exp((alpha+1)x - e^x) on [x_lo, x_hi] (inverse CDF
+    on a 200,001-point grid), V ~ U(1,10), r = V^(1/3), F = e^x/(4 pi r^2), Fhat = F + sigma_F eps, kept iff
+    Fhat > F_lim.  Columns: Fhat_i and g_i = 1/(4 pi r_i^2)."""
+    g = _rng(seed)
+    F_lim, sig_F, x_lo, x_hi, r_min, r_max = SCHECHTER_CONSTS
+    alpha, xstar = SCHECHTER_TRUTH
+    grid = np.linspace(x_lo, x_hi, 200_001)
+    dens = np.exp((alpha + 1.0) * (grid - xstar) - np.exp(grid - xstar))
+    cdf = np.concatenate([[0.0], np.cumsum(0.5 * (dens[1:] + dens[:-1]) * np.diff(grid))])
+    Z = cdf[-1]
+    cdf /= Z
+    xs, Fh, gs = [], [], []
+    kept, drawn = 0, 0
+    while kept < n:
+        m = max(4096, int(1.2 * (n - kept) / 0.15))
+        x = np.interp(g.uniform(size=m), cdf, grid)
+        r = g.uniform(r_min ** 3, r_max ** 3, m) ** (1.0 / 3.0)
+        gi = 1.0 / (4.0 * np.pi * r * r)
+        Fhat = np.exp(x) * gi + sig_F * g.standard_normal(m)
+        ok = np.flatnonzero(Fhat > F_lim)
+        if kept + ok.size >= n:          # stop at exactly n detections; count the candidates used
+            ok = ok[: n - kept]
+            drawn += int(ok[-1]) + 1 if ok.size else 0
+        else:
+            drawn += m
+        kept += ok.size
+        xs.append(x[ok]); Fh.append(Fhat[ok]); gs.append(gi[ok])
+    x, Fhat, gi = np.concatenate(xs), np.concatenate(Fh), np.concatenate(gs)
+    a_true = float(np.log(max(drawn, 1) / Z))       # amplitude whose expected population count = candidates drawn
+    return dict(model=M_THINNED_SCHECHTER1D, cols=[Fhat, gi], consts=SCHECHTER_CONSTS.copy(),
+                chi_true=x[None, :], theta_true=np.array([alpha, xstar, a_true]),
+                theta0=np.array([alpha + 0.05, xstar + 0.05, a_true + 0.05]),
+                detected_fraction=n / max(drawn, 1))
+
+
+def make_binormal2d(n, seed=3, fp32=False):
+    """C3: chi ~ N2(m, Sigma), m=(0,0.5), sds (1, e^-0.5), rho=0.3; per-axis sigma ~ U(0.05,0.3)."""
+    g = _rng(seed)
+    m = np.array([0.0, 0.5]); lam = np.array([0.0, -0.5]); rho = 0.3
+    s = g.uniform(0.05, 0.3, (2, n))
+    e = g.standard_normal((2, n))
+    chi = np.empty((2, n))
+    chi[0] = m[0] + np.exp(lam[0]) * e[0]
+    chi[1] = m[1] + np.exp(lam[1]) * (rho * e[0] + np.sqrt(1 - rho * rho) * e[1])
+    y = chi + s * g.standard_normal((2, n))
+    cols = [y[0], y[1], s[0], s[1]]
+    if fp32:
+        cols = _round_f32(cols)
+    th = np.array([m[0], m[1], lam[0], lam[1], np.arctanh(rho)])
+    return dict(model=M_BINORMAL2D, cols=cols, consts=None, chi_true=chi, theta_true=th,
+                theta0=th + np.array([0.05, -0.05, 0.05, 0.05, -0.05]))
+
+
+def make_linreg_me1d(n, seed=4, fp32=True):
+    """C4: z ~ U(0,3); chi ~ N(1 - 0.5 z, 0.3^2); sigma = exp(ln 0.2 + 0.5 eps); y = chi + sigma eps'."""
+    g = _rng(seed)
+    z = g.uniform(0.0, 3.0, n)
+    chi = 1.0 - 0.5 * z + 0.3 * g.standard_normal(n)
+    sigma = np.exp(np.log(0.2) + 0.5 * g.standard_normal(n))
+    y = chi + sigma * g.standard_normal(n)
+    cols = [y, sigma, z]
+    if fp32:
+        cols = _round_f32(cols)
+    th = np.array([1.0, -0.5, np.log(0.3)])
+    return dict(model=M_LINREG_ME1D, cols=cols, consts=None, chi_true=chi[None, :], theta_true=th,
+                theta0=th + np.array([0.02, -0.02, 0.05]))
+
+
+def make_inputs(config_name, n_objects=None):
+    """Inputs of config C0..C4; n_objects overrides N (reduced-size parity cases keep the recipe)."""
+    c = CONFIGS[config_name]
+    n = c.n_objects if n_objects is None else int(n_objects)
+    if c.model == M_NORMAL1D:
+        return make_normal1d(n, c.seed)
+    if c.model == M_THINNED_SCHECHTER1D:
+        return make_thinned_schechter1d(n, c.seed)
+    if c.model == M_BINORMAL2D:
+        return make_binormal2d(n, c.seed)
+    return make_linreg_me1d(n, c.seed, fp32=(c.precision == F32_STATE_F64_REDUCE))

@@ -1,0 +1,338 @@
+"""Pins P6-P14 of the oracle as a SAMPLER: the stationary law of the plate updates against conjugate closed
+forms (M0, M2, M3) and brute-force grid integration (M1); the theta chain against exact grids of the marginal
+posterior (M0, M3), the paper's Eq. 4.3-4.4 (M1) and an independent numpy sampler (M2); moments and trace
+bookkeeping.  All comparisons within 4 Monte Carlo standard errors (batch means) plus a small floor."""
+import numpy as np
+import pytest
+from scipy import stats
+
+from mcmc_util import mcse_batch_means, mean_and_var_with_mcse
+from oracle import api as O
+from paper_2105_08026_b200 import synth
+
+
+def _collect_chi(s, n_iter):
+    out = np.empty((n_iter, s.p, s.N))
+    for t in range(n_iter):
+        s.step()
+        out[t] = s.get_state()["chi"]
+    return out
+
+
+def _assert_within(est, mcse, truth, k=4.0, floor=0.0, what=""):
+    err = np.abs(np.asarray(est) - np.asarray(truth))
+    bound = k * np.asarray(mcse) + floor
+    assert np.all(err <= bound), f"{what}: max excess {np.max(err / bound):.2f}x of the {k}-MCSE bound"
+
+
+# Per-object tests make ~100 comparisons with a 30-batch standard error each (t_29 tails): a single 4-sigma
+# excursion is then a few-percent event, so those use 5 MCSE per comparison AND require the z-scores as a
+# set to look standard normal (rms < 1.5), which is the sharper test: a real error shifts them all.
+K_MANY = 5.0
+
+
+def _assert_z_rms(z, what=""):
+    z = np.asarray(z)
+    assert np.sqrt(np.mean(z ** 2)) < 1.5, f"{what}: rms z-score {np.sqrt(np.mean(z ** 2)):.2f}"
+
+
+# ---------------------------------------------------------------- plate stationary laws (theta frozen)
+def test_plate_stationary_law_normal1d_and_moments_bookkeeping():
+    """P6 + P14: chi_i | theta, y_i ~ N((y/s^2 + mu/tau^2) v^2, v^2), v^2 = 1/(1/s^2 + 1/tau^2)."""
+    n, burn, T = 40, 1500, 24000
+    inp = synth.make_normal1d(n, seed=31)
+    theta = np.array([0.2, -0.1])
+    s = O.Sampler(0, n, seed=31, target_accept_chi=0.44, freeze_theta=True, keep_chi_moments=True)
+    s.set_data(inp["cols"]); s.set_init(theta)
+    s.run(burn, burn_in=burn)
+    assert s.get_chi_moments()[2] == 0
+    chain = np.empty((T, n))
+    for t in range(T):
+        s.step(burn_in=burn)
+        chain[t] = s.get_state()["chi"][0]
+    y, sig = inp["cols"]
+    tau = np.exp(theta[1])
+    v2 = 1 / (1 / sig ** 2 + 1 / tau ** 2)
+    m = (y / sig ** 2 + theta[0] / tau ** 2) * v2
+    mean, mse, var, vse = mean_and_var_with_mcse(chain)
+    _assert_within(mean, mse, m, k=K_MANY, what="conditional mean")
+    _assert_within(var, vse, v2, k=K_MANY, floor=1e-4, what="conditional variance")
+    _assert_z_rms(np.concatenate([(mean - m) / mse, (var - v2) / vse]), "normal1d plate law")
+    # P14: on-line (Welford) moments == two-pass moments of the stored chain
+    om, ov, cnt = s.get_chi_moments()
+    assert cnt == T
+    np.testing.assert_allclose(om[0], chain.mean(0), rtol=1e-12, atol=1e-13)
+    np.testing.assert_allclose(ov[0], chain.var(0, ddof=1), rtol=1e-11)
+
+
+def test_plate_stationary_law_linreg_fp64_and_fp32():
+    """P6 for M3 (mean a + b z_i), in both precisions of the oracle."""
+    n, burn, T = 30, 1500, 20000
+    inp = synth.make_linreg_me1d(n, seed=32, fp32=True)
+    theta = np.array([1.0, -0.5, np.log(0.3)])
+    y, sig, z = inp["cols"]
+    tau = np.exp(theta[2])
+    v2 = 1 / (1 / sig ** 2 + 1 / tau ** 2)
+    m = (y / sig ** 2 + (theta[0] + theta[1] * z) / tau ** 2) * v2
+    for prec, floor in ((O.F64, 0.0), (O.F32_STATE_F64_REDUCE, 2e-5)):
+        s = O.Sampler(3, n, seed=32, precision=prec, target_accept_chi=0.44, freeze_theta=True)
+        s.set_data(inp["cols"]); s.set_init(theta)
+        s.run(burn)
+        chain = _collect_chi(s, T)[:, 0, :]
+        mean, mse, var, vse = mean_and_var_with_mcse(chain)
+        _assert_within(mean, mse, m, k=K_MANY, floor=floor, what=f"mean prec={prec}")
+        _assert_within(var, vse, v2, k=K_MANY, floor=1e-4 * v2.max() + floor, what=f"var prec={prec}")
+        _assert_z_rms(np.concatenate([(mean - m) / (mse + floor), (var - v2) / (vse + floor)]), f"linreg prec={prec}")
+
+
+def test_plate_stationary_law_binormal2d():
+    """P7: bivariate normal with precision Sigma_pop^-1 + diag(1/s^2)."""
+    n, burn, T = 24, 3000, 30000
+    inp = synth.make_binormal2d(n, seed=33)
+    th = inp["theta_true"]
+    s = O.Sampler(2, n, seed=33, target_accept_chi=0.234, freeze_theta=True)
+    s.set_data(inp["cols"]); s.set_init(th)
+    s.run(burn)
+    chain = _collect_chi(s, T)                                   # (T, 2, n)
+    sd = np.exp(th[2:4]); rho = np.tanh(th[4])
+    Sp = np.array([[sd[0] ** 2, rho * sd[0] * sd[1]], [rho * sd[0] * sd[1], sd[1] ** 2]])
+    Pp = np.linalg.inv(Sp)
+    y1, y2, s1, s2 = inp["cols"]
+    zs = []
+    for i in range(n):
+        P = Pp + np.diag([1 / s1[i] ** 2, 1 / s2[i] ** 2])
+        C = np.linalg.inv(P)
+        mu = C @ (Pp @ th[:2] + np.array([y1[i] / s1[i] ** 2, y2[i] / s2[i] ** 2]))
+        x = chain[:, :, i]
+        mean, mse, var, vse = mean_and_var_with_mcse(x)
+        _assert_within(mean, mse, mu, k=K_MANY, what=f"mean obj {i}")
+        _assert_within(var, vse, np.diag(C), k=K_MANY, floor=1e-4 * np.diag(C).max(), what=f"var obj {i}")
+        xc = (x[:, 0] - mu[0]) * (x[:, 1] - mu[1])
+        cse = mcse_batch_means(xc)
+        _assert_within(xc.mean(), cse, C[0, 1], k=K_MANY, floor=1e-4 * abs(C[0, 0]), what=f"cov obj {i}")
+        zs += list((mean - mu) / mse) + list((var - np.diag(C)) / vse) + [(xc.mean() - C[0, 1]) / cse[0]]
+    _assert_z_rms(zs, "binormal plate law")
+
+
+def test_plate_stationary_law_schechter_against_grid():
+    """P8: brute-force grid integration of exp(l_i + f) on [x_lo, x_hi] at fixed theta (named by north_star)."""
+    n, burn, T = 16, 3000, 30000
+    inp = synth.make_thinned_schechter1d(n, seed=34)
+    th = inp["theta_true"]
+    c = inp["consts"]
+    s = O.Sampler(1, n, seed=34, target_accept_chi=0.44, freeze_theta=True)
+    s.set_data(inp["cols"]); s.set_model_consts(c); s.set_init(th)
+    s.run(burn)
+    chain = _collect_chi(s, T)[:, 0, :]
+    Fh, g = inp["cols"]
+    grid = np.linspace(c[2], c[3], 1_200_001)
+    zs = []
+    for i in range(n):
+        logd = stats.norm.logpdf(Fh[i], g[i] * np.exp(grid), c[1]) + (th[0] + 1) * (grid - th[1]) - np.exp(grid - th[1])
+        w = np.exp(logd - logd.max())
+        w /= w.sum()
+        m = (w * grid).sum()
+        v = (w * (grid - m) ** 2).sum()
+        mean, mse, var, vse = mean_and_var_with_mcse(chain[:, i])
+        _assert_within(mean, mse, m, k=K_MANY, floor=1e-6, what=f"mean obj {i}")
+        _assert_within(var, vse, v, k=K_MANY, floor=1e-3 * v, what=f"var obj {i}")
+        zs += [(mean[0] - m) / mse[0], (var[0] - v) / vse[0]]
+    _assert_z_rms(zs, "schechter plate law")
+    assert np.all(chain >= c[2]) and np.all(chain <= c[3])
+
+
+# ---------------------------------------------------------------- theta posteriors (full Gibbs cycle)
+def _grid_moments(logpost, axes):
+    w = np.exp(logpost - logpost.max())
+    w /= w.sum()
+    means, sds = [], []
+    for k, ax in enumerate(axes):
+        wk = w.sum(tuple(j for j in range(len(axes)) if j != k))
+        m = (wk * ax).sum()
+        means.append(m)
+        sds.append(np.sqrt((wk * (ax - m) ** 2).sum()))
+    return np.array(means), np.array(sds)
+
+
+def test_theta_posterior_normal1d_against_marginal_grid():
+    """P9: integrating chi out, y_i ~ N(mu, s_i^2 + tau^2); exact 2-D grid over (mu, log tau), flat prior."""
+    n, burn, T = 200, 4000, 50000
+    inp = synth.make_normal1d(n, seed=35)
+    s = O.Sampler(0, n, seed=35, target_accept_chi=0.44, target_accept_theta=0.234)
+    s.set_data(inp["cols"]); s.set_init(inp["theta0"])
+    s.run(burn + T, burn_in=burn, thin=1)
+    tr = s.get_theta_trace()
+    assert tr.shape == (T, 2)
+    y, sig = inp["cols"]
+    mu = np.linspace(-0.6, 0.6, 401); lam = np.linspace(-1.0, 0.6, 401)
+    V = sig[None, None, :] ** 2 + np.exp(2 * lam)[None, :, None]
+    lp = (-0.5 * np.log(V) - 0.5 * (y[None, None, :] - mu[:, None, None]) ** 2 / V).sum(-1)
+    gm, gs = _grid_moments(lp, [mu, lam])
+    mean, mse, var, vse = mean_and_var_with_mcse(tr)
+    _assert_within(mean, mse, gm, floor=1e-4, what="theta mean")
+    _assert_within(var, vse, gs ** 2, floor=1e-3 * gs.max() ** 2, what="theta variance")
+    st = s.get_stats()
+    assert 0.1 < st["theta_accepts"] / st["theta_proposals"] < 0.4      # RAM on theta homes in on 0.234
+
+
+@pytest.mark.parametrize("prec", [O.F64, O.F32_STATE_F64_REDUCE])
+def test_theta_posterior_linreg_against_marginal_grid(prec):
+    """P12 (M3): y_i ~ N(a + b z_i, s_i^2 + tau^2); exact 3-D grid; both precisions of the oracle."""
+    n, burn, T = 150, 5000, 50000
+    inp = synth.make_linreg_me1d(n, seed=36, fp32=True)
+    s = O.Sampler(3, n, seed=36, precision=prec, target_accept_chi=0.44)
+    s.set_data(inp["cols"]); s.set_init(inp["theta0"])
+    s.run(burn + T, burn_in=burn)
+    tr = s.get_theta_trace()
+    y, sig, z = inp["cols"]
+    m0, s0 = tr.mean(0), tr.std(0)
+    axes = [np.linspace(m0[k] - 6 * s0[k], m0[k] + 6 * s0[k], 81) for k in range(3)]
+    A, B, Lm = np.meshgrid(*axes, indexing="ij")
+    lp = np.zeros_like(A)
+    for i in range(n):
+        V = sig[i] ** 2 + np.exp(2 * Lm)
+        lp += -0.5 * np.log(V) - 0.5 * (y[i] - A - B * z[i]) ** 2 / V
+    gm, gs = _grid_moments(lp, axes)
+    mean, mse, var, vse = mean_and_var_with_mcse(tr)
+    _assert_within(mean, mse, gm, floor=2e-4, what="theta mean")
+    _assert_within(var, vse, gs ** 2, floor=2e-3 * gs.max() ** 2, what="theta variance")
+
+
+def test_theta_posterior_binormal_against_independent_sampler():
+    """P12 (M2): plain random-walk MH (numpy) on the closed-form MARGINAL likelihood
+    y_i ~ N2(m, Sigma_pop + diag(s_i^2)) -- a different algorithm on a different (chi-free) target."""
+    n, burn, T = 200, 6000, 50000
+    inp = synth.make_binormal2d(n, seed=37)
+    s = O.Sampler(2, n, seed=37, target_accept_chi=0.234)
+    s.set_data(inp["cols"]); s.set_init(inp["theta0"])
+    s.run(burn + T, burn_in=burn)
+    tr = s.get_theta_trace()
+    y1, y2, s1, s2 = inp["cols"]
+
+    def marg(th):
+        sd1, sd2, rho = np.exp(th[2]), np.exp(th[3]), np.tanh(th[4])
+        a = sd1 ** 2 + s1 ** 2; d = sd2 ** 2 + s2 ** 2; b = rho * sd1 * sd2
+        det = a * d - b * b
+        r1, r2 = y1 - th[0], y2 - th[1]
+        return (-0.5 * np.log(det) - 0.5 * (d * r1 * r1 - 2 * b * r1 * r2 + a * r2 * r2) / det).sum()
+
+    g = np.random.default_rng(0)
+    step = np.linalg.cholesky(np.cov(tr.T) * (2.38 ** 2 / 5))
+    cur = tr.mean(0); lc = marg(cur)
+    ref = np.empty((60000, 5))
+    for t in range(ref.shape[0]):
+        prop = cur + step @ g.normal(size=5)
+        lpn = marg(prop)
+        if np.log(g.uniform()) < lpn - lc:
+            cur, lc = prop, lpn
+        ref[t] = cur
+    ref = ref[5000:]
+    m1, e1, v1, ve1 = mean_and_var_with_mcse(tr)
+    m2, e2, v2, ve2 = mean_and_var_with_mcse(ref)
+    _assert_within(m1, np.hypot(e1, e2), m2, floor=2e-4, what="theta mean")
+    _assert_within(v1, np.hypot(ve1, ve2), v2, floor=2e-3 * v2.max(), what="theta variance")
+
+
+def test_theta_posterior_schechter_against_eq_4_3():
+    """P11: marginalising the log-flat amplitude out of the Poisson form gives the paper's likelihood
+    L(zeta) = prod_i int dx mu(x, r_i; zeta) l_i(x), mu = phi h / int int eta h phi (Eq. 4.3-4.4).
+    The (alpha, x*) marginals of the 3-parameter chain must match a direct grid of that expression, written
+    here in numpy from the equations (its own quadrature, its own densities)."""
+    n, burn, T = 120, 6000, 60000
+    inp = synth.make_thinned_schechter1d(n, seed=38)
+    c = inp["consts"]
+    F_lim, sigF, x_lo, x_hi, r_min, r_max = c
+    s = O.Sampler(1, n, seed=38, target_accept_chi=0.44)
+    s.set_data(inp["cols"]); s.set_model_consts(c); s.set_init(inp["theta0"])
+    s.run(burn + T, burn_in=burn)
+    tr = s.get_theta_trace()
+    Fh, g = inp["cols"]
+
+    # selection integral on the test's own tensor grid (trapezoid in x on a fine grid, Gauss-Legendre in r)
+    xr, wr = np.polynomial.legendre.leggauss(200)
+    r = 0.5 * (r_max - r_min) * xr + 0.5 * (r_max + r_min); w_r = 0.5 * (r_max - r_min) * wr
+    xg = np.linspace(x_lo, x_hi, 6001)
+    F = np.exp(xg)[:, None] / (4 * np.pi * r[None, :] ** 2)
+    G = (w_r * 3 * r ** 2 / (r_max ** 3 - r_min ** 3) * stats.norm.cdf((F - F_lim) / sigF)).sum(1)
+    # per-object local grids around the flux estimate
+    xc = np.log(Fh / g)
+    half = 12 * sigF / Fh + 1e-3
+    loc = xc[:, None] + half[:, None] * np.linspace(-1, 1, 801)[None, :]
+    loc = np.clip(loc, x_lo, x_hi)
+    lik = np.exp(stats.norm.logpdf(Fh[:, None], g[:, None] * np.exp(loc), sigF) - stats.norm.logpdf(0, 0, sigF))
+    dloc = np.gradient(loc, axis=1)
+
+    m0, s0 = tr[:, :2].mean(0), tr[:, :2].std(0)
+    al = np.linspace(max(m0[0] - 5 * s0[0], -1.999), min(m0[0] + 5 * s0[0], -1e-3), 61)
+    xs = np.linspace(m0[1] - 5 * s0[1], m0[1] + 5 * s0[1], 61)
+    lp = np.empty((al.size, xs.size))
+    for i, a_ in enumerate(al):
+        for j, x_ in enumerate(xs):
+            phi = lambda x: np.exp((a_ + 1) * (x - x_) - np.exp(x - x_))
+            I = np.trapezoid(phi(xg) * G, xg)
+            num = (phi(loc) * lik * dloc).sum(1)
+            lp[i, j] = np.log(num).sum() - n * np.log(I) - np.log(1 + a_ * a_)
+    gm, gs = _grid_moments(lp, [al, xs])
+    mean, mse, var, vse = mean_and_var_with_mcse(tr[:, :2])
+    _assert_within(mean, mse, gm, floor=2e-3 * gs.max(), what="(alpha, x*) mean")
+    _assert_within(var, vse, gs ** 2, floor=0.02 * gs.max() ** 2, what="(alpha, x*) variance")
+    # P10: given (alpha, x*), A ~ Gamma(N, rate I): E[a | rest] = digamma(N) - log I  => check the chain average
+    from scipy.special import digamma
+    I_chain = np.array([-s.theta_only([t_[0], t_[1], 0.0]) for t_ in tr[::50]])
+    want = (digamma(n) - np.log(I_chain)).mean()
+    assert tr[:, 2].mean() == pytest.approx(want, abs=4 * mcse_batch_means(tr[:, 2])[0] + 5e-3)
+
+
+def test_trace_thinning_and_resume_bookkeeping():
+    n = 50
+    inp = synth.make_normal1d(n, seed=39)
+    a = O.Sampler(0, n, seed=39, keep_chi_moments=True)
+    a.set_data(inp["cols"]); a.set_init(inp["theta0"])
+    a.run(100, burn_in=40, thin=7)
+    tr = a.get_theta_trace()
+    assert tr.shape == (8, 2)                                   # t = 47, 54, ..., 96
+    # same run in three resumed pieces gives the identical chain (counter-based streams: nothing to save)
+    b = O.Sampler(0, n, seed=39, keep_chi_moments=True)
+    b.set_data(inp["cols"]); b.set_init(inp["theta0"])
+    b.run(33, burn_in=40, thin=7); b.run(30, burn_in=40, thin=7); b.run(37, burn_in=40, thin=7)
+    assert np.array_equal(b.get_theta_trace(), tr)
+    sa, sb = a.get_state(), b.get_state()
+    for k in ("chi", "L", "theta", "L_theta"):
+        assert np.array_equal(sa[k], sb[k])
+    assert sa["t"] == sb["t"] == 100 and a.get_chi_moments()[2] == 60
+    # a different seed gives a different chain; set_state/get_state round-trip restarts it exactly
+    c = O.Sampler(0, n, seed=39)
+    c.set_data(inp["cols"]); c.set_init(inp["theta0"])
+    c.run(10)
+    snap = c.get_state()
+    c.run(5); after = c.get_state()
+    c.set_state(snap["chi"], snap["L"], snap["theta"], snap["L_theta"], snap["t"])
+    c.run(5)
+    assert np.array_equal(c.get_state()["chi"], after["chi"]) and np.array_equal(c.get_state()["theta"], after["theta"])
+
+
+def test_population_sums_in_taps():
+    """P13: S = sum a_i and Delta = sum (b_i - a_i) of the taps equal math.fsum of the per-object values, and the
+    theta decision uses log r = Delta + T' - T + prior' - prior."""
+    import math
+    n = 3000
+    inp = synth.make_thinned_schechter1d(n, seed=40)
+    s = O.Sampler(1, n, seed=40, target_accept_chi=0.44)
+    s.set_data(inp["cols"]); s.set_model_consts(inp["consts"]); s.set_init(inp["theta0"])
+    s.run(5)
+    th = s.get_state()["theta"].copy()
+    tp = s.step(taps=True)
+    assert tp["S"] == pytest.approx(math.fsum(tp["a"]), rel=1e-15)
+    assert tp["Delta"] == pytest.approx(math.fsum(tp["b"] - tp["a"]), rel=1e-13, abs=1e-12)
+    assert tp["T_cur"] == s.theta_only(th) and tp["T_prop"] == s.theta_only(tp["theta_prop"])
+    want = tp["Delta"] + (tp["T_prop"] - tp["T_cur"]) + (O.logprior(1, tp["theta_prop"]) - O.logprior(1, th))
+    assert tp["log_r"] == pytest.approx(want, rel=1e-14)
+    assert tp["alpha_theta"] == pytest.approx(min(1.0, np.exp(tp["log_r"])), rel=1e-14)
+    assert tp["accepted_theta"] == int(tp["u_theta"] < tp["alpha_theta"])
+    assert tp["u_theta"] == O.uniform_f64(40, O.KIND_THETA, 0, 6, 0)
+    new = s.get_state()["theta"]
+    assert np.array_equal(new, tp["theta_prop"] if tp["accepted_theta"] else th)
+    # b_i is the population density at the NEW chi under theta'
+    chi = s.get_state()["chi"][0]
+    i = 11
+    assert tp["b"][i] == O.logpop(1, [chi[i]], [0, 0], tp["theta_prop"], inp["consts"])
