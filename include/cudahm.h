@@ -1,0 +1,160 @@
+/*
+ * cudahm.h -- C ABI of the B200-native plate-level RAM Metropolis-within-Gibbs sampler.
+ *
+ * What it computes (citations are /root/reference/PAPER.md line numbers, arXiv 2105.08026):
+ *   The Metropolis-within-Gibbs cycle of Eq. 2.4-2.5 for a single-plate
+ *   hierarchical model (Eq. 2.3).  Per Gibbs iteration t, for every object i:
+ *     1. propose  chi' = chi_i + L_i z,  z ~ N(0, I_p)                   (RAM step 1)
+ *     2. accept with probability alpha = min{1, pi(chi')/pi(chi_i)},
+ *        pi = l_i(.) f(.; theta)                                         (RAM step 2)
+ *     3. L_i <- chol(L_i (I + eta_n (alpha - alpha_*) z z^T/|z|^2) L_i^T),
+ *        eta_n = n^(-2/3)                                                (RAM step 3, Eq. 2.6)
+ *   fused, in the same pass, with the population sums  S = sum_i log f(chi_i; theta)  and
+ *   Delta = sum_i [log f(chi_i; theta') - log f(chi_i; theta)]  that the Metropolis-Hastings step
+ *   on theta consumes, then the theta decision itself (RAM on theta), running
+ *   chi moments and a thinned theta trace.  Models are compiled in (the counterpart of the two
+ *   user functions of PAPER.md:144, :391); their definitions are in DESIGN.md section 3.
+ *
+ * Conventions
+ *   - Every function returns a CUDAHM_* status (0 = OK) and never throws; cudahm_last_error()
+ *     returns a message for the last failure on that handle (or the global one if the handle is NULL).
+ *   - DEVICE MEMORY IS OWNED BY THE CALLER: allocate cudahm_workspace_bytes(cfg) bytes (256-byte
+ *     aligned), pass it to cudahm_create; the library sub-allocates all of its state there and never
+ *     allocates device memory on the hot path.  The workspace must outlive the handle.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All device work
+ *     is enqueued on it.  cudahm_run returns once the work is enqueued (THETA_DEVICE_TAIL, THETA_GRAPH)
+ *     or complete (THETA_HOST); every getter synchronises the stream first.
+ *   - "T" below is the state precision: double for CUDAHM_F64, float for CUDAHM_F32_STATE_F64_REDUCE.
+ *   - Per-object arrays are structure-of-arrays: chi[j*N + i] = component j of object i; L is the
+ *     packed lower triangle row-major ((0,0),(1,0),(1,1)): L[k*N + i] = packed entry k of object i.
+ *   - theta, L_theta (packed lower triangle of the theta proposal factor), traces and moments are fp64.
+ *   - There is no CPU fallback: without a CUDA device every call that needs one fails with CUDAHM_E_CUDA.
+ */
+#ifndef CUDAHM_H
+#define CUDAHM_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cudahm_sampler cudahm_sampler;   /* opaque; created/destroyed only by the library */
+
+enum { CUDAHM_OK = 0, CUDAHM_E_INVALID = -1, CUDAHM_E_STATE = -2, CUDAHM_E_CUDA = -3,
+       CUDAHM_E_WORKSPACE = -4, CUDAHM_E_UNSUPPORTED = -5, CUDAHM_E_NONFINITE = -6 };
+
+/* compiled-in models: (p, dtheta, data columns, model constants) */
+enum { CUDAHM_M_NORMAL1D = 0,            /* (1, 2, {y, sigma}, 0)            theta = (mu, log tau)              */
+       CUDAHM_M_THINNED_SCHECHTER1D = 1, /* (1, 3, {Fhat, g=1/(4 pi r^2)}, 6) theta = (alpha, log L*, log A)     */
+       CUDAHM_M_BINORMAL2D = 2,          /* (2, 5, {y1, y2, s1, s2}, 0)      theta = (m1, m2, l1, l2, zeta)      */
+       CUDAHM_M_LINREG_ME1D = 3 };       /* (1, 3, {y, sigma, z}, 0)         theta = (a, b, log tau)            */
+enum { CUDAHM_F64 = 0, CUDAHM_F32_STATE_F64_REDUCE = 1 };
+/* where the theta Metropolis-Hastings step runs (PAPER.md:142 puts it on the host) */
+enum { CUDAHM_THETA_HOST = 0,         /* one sweep launch + one sync per iteration; theta step in host C++     */
+       CUDAHM_THETA_GRAPH = 1,        /* {sweep kernel, 1-block tail kernel} per iteration, CUDA-Graph batches */
+       CUDAHM_THETA_DEVICE_TAIL = 2 };/* one persistent cooperative kernel, one grid barrier per iteration     */
+
+typedef struct {
+  uint32_t struct_size;          /* sizeof(cudahm_config), checked                                          */
+  int32_t  model;                /* CUDAHM_M_*                                                              */
+  int32_t  precision;            /* CUDAHM_F64 | CUDAHM_F32_STATE_F64_REDUCE                                */
+  int32_t  theta_mode;           /* CUDAHM_THETA_*                                                          */
+  int64_t  n_objects;            /* N >= 0                                                                  */
+  int32_t  p, dtheta, n_data_cols; /* must match the compiled-in model, else CUDAHM_E_INVALID               */
+  int32_t  freeze_theta;         /* 1: skip the theta step (theta held fixed)                               */
+  uint64_t seed;                 /* Philox4x32-10 key                                                       */
+  double   target_accept_chi;    /* alpha_* of the plate RAM; paper default 0.4              */
+  double   target_accept_theta;  /* alpha_* of the theta RAM (paper-silent; reading R7)           */
+  double   eta_exponent;         /* eta_n = n^(-eta_exponent); paper: 2/3                    */
+  double   init_scale_chi;       /* S_1 = init_scale_chi * I; paper: identity                */
+  int32_t  keep_chi_moments;     /* 1: running mean / variance of every chi component after burn-in         */
+  int32_t  block_threads;        /* 0 = default; else 256, 512 or 1024                                      */
+  int32_t  blocks_per_sm;        /* 0 = as many as fit; else an upper limit                                 */
+  int32_t  reserved;             /* must be 0                                                               */
+  int64_t  max_trace_rows;       /* capacity of the on-device thinned theta trace (rows of dtheta doubles)   */
+} cudahm_config;
+
+typedef struct {
+  int64_t iterations;            /* Gibbs iterations done (t)                                               */
+  int64_t chi_accepts;           /* accepted plate proposals over all objects and iterations                */
+  int64_t chi_proposals;
+  int64_t theta_accepts;
+  int64_t theta_proposals;
+  int64_t nonfinite;             /* plate proposals whose log target ratio was NaN (rejected, alpha = 0)    */
+  int64_t moment_samples;        /* post-burn-in iterations accumulated into the chi moments                */
+  int64_t trace_rows;
+  int64_t gpu_launches;          /* kernels launched by this handle so far                                  */
+  int32_t grid_blocks, block_threads;   /* launch configuration of the sweep                               */
+  double  last_run_ms;           /* device time of the last cudahm_run (CUDA events on the stream)          */
+} cudahm_stats;
+
+/* Per-iteration taps of cudahm_debug_step; HOST pointers, each may be NULL.  Values are widened to double. */
+typedef struct {
+  double* chi_prop;    /* p*N    chi' = chi + L z                                                           */
+  double* pi_cur;      /* N      log l_i(chi) + log f(chi; theta)                                           */
+  double* pi_prop;     /* N      same at chi'                                                               */
+  double* alpha;       /* N      min{1, pi(chi')/pi(chi)}                                                   */
+  double* u;           /* N      accept uniform                                                             */
+  int32_t* accepted;   /* N      1 iff u < alpha                                                            */
+  double* L_new;       /* ntri*N updated factor                                                             */
+  double* a;           /* N      log f(chi_new; theta)                                                      */
+  double* b;           /* N      log f(chi_new; theta')                                                     */
+  double  theta_prop[8];
+  double  S, Delta, T_cur, T_prop, lp_cur, lp_prop, log_r, alpha_theta, u_theta;
+  int32_t accepted_theta;
+  int32_t pad_;
+} cudahm_taps;
+
+/* Model dimensions: (p, dtheta, n_data_cols, n_consts).  CUDAHM_E_INVALID for an unknown model. */
+int cudahm_model_dims(int model, int* p, int* dtheta, int* n_data_cols, int* n_consts);
+
+/* Bytes of device workspace the configuration needs (0 if cfg is invalid). */
+size_t cudahm_workspace_bytes(const cudahm_config* cfg);
+
+/* Create a sampler inside the caller's device workspace.  CUDAHM_E_WORKSPACE if `bytes` is too small or the
+ * pointer is not 256-byte aligned; CUDAHM_E_UNSUPPORTED for a (model, precision) pair that is not compiled in
+ * (compiled in: every model in F64; NORMAL1D and LINREG_ME1D in F32_STATE_F64_REDUCE). */
+int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size_t bytes, void* cuda_stream,
+                  cudahm_sampler** out);
+void cudahm_destroy(cudahm_sampler* s);
+
+/* Copy the n_cols data columns (arrays of N values of type T, host or device) into the workspace; the caller's
+ * buffers may be freed afterwards.  Member likelihoods l_i are built from them. */
+int cudahm_set_data(cudahm_sampler* s, const void* const* cols, int n_cols, int cols_on_device);
+
+/* Model constants (host doubles).  THINNED_SCHECHTER1D: {F_lim, sigma_F, x_lo, x_hi, r_min, r_max}; builds the
+ * 1,024-point selection-integral table (Eq. 4.4 denominator).  Other models take n = 0. */
+int cudahm_set_model_consts(cudahm_sampler* s, const double* v, int n);
+
+/* Initial state: chi0 (p*N values of type T, host or device per chi0_on_device; NULL = the model's default
+ * X_1, reading R6), theta0 (dtheta host doubles), theta_chol0 (packed lower triangle, host doubles;
+ * NULL = 0.1 * I).  Resets t = 0, L_i = init_scale_chi * I, the trace, the moments and the counters.
+ * CUDAHM_E_STATE before set_data (and set_model_consts where the model has constants). */
+int cudahm_set_init(cudahm_sampler* s, const void* chi0_or_null, int chi0_on_device, const double* theta0,
+                    const double* theta_chol0_or_null);
+
+/* Run n_iter more Gibbs iterations (resumable: continues from the current iteration index t).  Moments are
+ * accumulated for t > burn_in, the trace takes theta whenever t > burn_in and (t - burn_in) % thin == 0.
+ * CUDAHM_E_INVALID if the trace would overflow max_trace_rows. */
+int cudahm_run(cudahm_sampler* s, int64_t n_iter, int64_t burn_in, int32_t thin);
+
+/* One iteration through the non-persistent sweep + tail kernels with per-object taps (test instrument). */
+int cudahm_debug_step(cudahm_sampler* s, int64_t burn_in, int32_t thin, cudahm_taps* taps);
+
+/* out: row-major n_rows x dtheta host doubles.  out == NULL just reports n_rows. */
+int cudahm_get_theta_trace(cudahm_sampler* s, double* out, int64_t cap_rows, int64_t* n_rows);
+/* mean, var: p*N host doubles (SoA); var is the sample variance (divisor n_samples - 1). */
+int cudahm_get_chi_moments(cudahm_sampler* s, double* mean, double* var, int64_t cap_objects, int64_t* n_samples);
+int cudahm_get_stats(cudahm_sampler* s, cudahm_stats* out);
+/* chi, L: host arrays of T (p*N, ntri*N); theta, L_theta: host doubles; any pointer may be NULL. */
+int cudahm_get_state(cudahm_sampler* s, void* chi, void* L, double* theta, double* L_theta, int64_t* t);
+int cudahm_set_state(cudahm_sampler* s, const void* chi, const void* L, const double* theta,
+                     const double* L_theta, int64_t t);
+/* Block until everything enqueued on the sampler's stream is done; reports asynchronous CUDA errors. */
+int cudahm_sync(cudahm_sampler* s);
+const char* cudahm_last_error(const cudahm_sampler* s_or_null);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

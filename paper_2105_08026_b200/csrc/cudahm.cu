@@ -1,0 +1,699 @@
+// cudahm.cu -- host side of the C ABI declared in include/cudahm.h: argument checks, workspace layout,
+// kernel dispatch and the three theta-step drivers (device tail / CUDA graph / host).  No CPU fallback:
+// every step of the path runs in the kernels of kernels.cuh.
+#include "cudahm.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "kernels.cuh"
+
+using namespace hm;
+
+namespace {
+
+thread_local std::string g_err;
+
+struct Layout {
+  size_t chi, L, data, mom_mean, mom_M2, mom_var, slots, bar, iter, trace, totals, qx, qex, qW, total;
+};
+
+constexpr int MAX_BLOCKS = 148 * 8 * 2;   // upper bound on the cooperative grid (slots capacity)
+
+inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+struct KernelSet {
+  const void* persistent;
+  const void* sweep;
+  const void* sweep_tap;
+  const void* init_state;
+};
+
+template <int MODEL, class T, int BLOCK>
+KernelSet make_set() {
+  KernelSet k;
+  k.persistent = (const void*)k_persistent<MODEL, T, BLOCK>;
+  k.sweep = (const void*)k_sweep<MODEL, T, BLOCK, false>;
+  k.sweep_tap = (const void*)k_sweep<MODEL, T, BLOCK, true>;
+  k.init_state = (const void*)k_init_state<MODEL, T>;
+  return k;
+}
+
+template <int MODEL, class T>
+bool pick_block(int block, KernelSet* k) {
+  switch (block) {
+    case 256:  *k = make_set<MODEL, T, 256>(); return true;
+    case 512:  *k = make_set<MODEL, T, 512>(); return true;
+    case 1024: *k = make_set<MODEL, T, 1024>(); return true;
+  }
+  return false;
+}
+
+bool pick_kernels(int model, int precision, int block, KernelSet* k) {
+  if (precision == CUDAHM_F64) {
+    switch (model) {
+      case M_NORMAL1D:            return pick_block<M_NORMAL1D, double>(block, k);
+      case M_THINNED_SCHECHTER1D: return pick_block<M_THINNED_SCHECHTER1D, double>(block, k);
+      case M_BINORMAL2D:          return pick_block<M_BINORMAL2D, double>(block, k);
+      case M_LINREG_ME1D:         return pick_block<M_LINREG_ME1D, double>(block, k);
+    }
+  } else if (precision == CUDAHM_F32_STATE_F64_REDUCE) {
+    switch (model) {
+      case M_NORMAL1D:    return pick_block<M_NORMAL1D, float>(block, k);
+      case M_LINREG_ME1D: return pick_block<M_LINREG_ME1D, float>(block, k);
+    }
+  }
+  return false;
+}
+
+}  // namespace
+
+struct cudahm_sampler {
+  cudahm_config cfg{};
+  Params P{};
+  Layout lay{};
+  KernelSet ks{};
+  cudaStream_t stream = nullptr;
+  char* ws = nullptr;
+  int p = 0, dtheta = 0, ncols = 0, nconsts = 0, ntri = 0, ntri_theta = 0;
+  size_t tsize = 8;
+  bool have_data = false, have_consts = false, have_init = false;
+  int num_sms = 0, grid = 1, block = 512, vec = 2;
+  long long t_done = 0;             // iterations completed (host mirror)
+  long long launches = 0;
+  Iter* h_iter = nullptr;           // pinned host copy of the iteration state
+  double* h_totals = nullptr;       // pinned
+  bool host_iter_valid = false;     // THETA_HOST: h_iter is authoritative between runs
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  bool timed = false;
+  // CUDA-graph cache (THETA_GRAPH)
+  cudaGraphExec_t gexec = nullptr;
+  long long g_burn = -1; int g_thin = -1; int g_iters = 0;
+  std::string err;
+};
+
+namespace {
+
+int fail(cudahm_sampler* s, int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  g_err = buf;
+  if (s) s->err = buf;
+  return code;
+}
+
+#define CU_TRY(s, call)                                                                      \
+  do {                                                                                       \
+    cudaError_t e_ = (call);                                                                 \
+    if (e_ != cudaSuccess) return fail(s, CUDAHM_E_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+  } while (0)
+
+bool valid_config(const cudahm_config* c, int* p, int* dt, int* nc, int* nk) {
+  if (!c || c->struct_size != sizeof(cudahm_config)) return false;
+  if (!model_dims(c->model, p, dt, nc, nk)) return false;
+  if (c->p != *p || c->dtheta != *dt || c->n_data_cols != *nc) return false;
+  if (c->n_objects < 0 || c->max_trace_rows < 0 || c->reserved != 0) return false;
+  if (c->precision != CUDAHM_F64 && c->precision != CUDAHM_F32_STATE_F64_REDUCE) return false;
+  if (c->theta_mode < CUDAHM_THETA_HOST || c->theta_mode > CUDAHM_THETA_DEVICE_TAIL) return false;
+  if (!(c->target_accept_chi > 0.0 && c->target_accept_chi < 1.0)) return false;
+  if (!(c->target_accept_theta > 0.0 && c->target_accept_theta < 1.0)) return false;
+  if (!(c->eta_exponent > 0.0 && c->eta_exponent <= 1.0) || !(c->init_scale_chi > 0.0)) return false;
+  if (c->block_threads != 0 && c->block_threads != 256 && c->block_threads != 512 && c->block_threads != 1024)
+    return false;
+  if (c->blocks_per_sm < 0) return false;
+  return true;
+}
+
+Layout make_layout(const cudahm_config& c, int p, int ncols, int dtheta) {
+  const size_t ts = c.precision == CUDAHM_F64 ? 8 : 4;
+  const size_t Npad = (size_t)((c.n_objects + 31) / 32 * 32);
+  const int ntri = p * (p + 1) / 2;
+  Layout l{};
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t at = o; o = align_up(o + bytes); return at; };
+  l.chi = take((size_t)p * Npad * ts);
+  l.L = take((size_t)ntri * Npad * ts);
+  l.data = take((size_t)ncols * Npad * ts);
+  const size_t mom = c.keep_chi_moments ? (size_t)p * Npad * 8 : 0;
+  l.mom_mean = take(mom); l.mom_M2 = take(mom); l.mom_var = take(mom);
+  l.slots = take((size_t)2 * MAX_BLOCKS * NPART * 8);
+  l.bar = take(256);
+  l.iter = take(sizeof(Iter));
+  l.trace = take((size_t)c.max_trace_rows * dtheta * 8);
+  l.totals = take(NPART * 8);
+  l.qx = take(NQUAD * 8); l.qex = take(NQUAD * 8); l.qW = take(NQUAD * 8);
+  l.total = o;
+  return l;
+}
+
+}  // namespace
+
+// ----------------------------------------------------------------------------------------------------
+extern "C" int cudahm_model_dims(int model, int* p, int* dtheta, int* n_data_cols, int* n_consts) {
+  int a, b, c, d;
+  if (!model_dims(model, &a, &b, &c, &d)) return fail(nullptr, CUDAHM_E_INVALID, "unknown model %d", model);
+  if (p) *p = a;
+  if (dtheta) *dtheta = b;
+  if (n_data_cols) *n_data_cols = c;
+  if (n_consts) *n_consts = d;
+  return CUDAHM_OK;
+}
+
+extern "C" size_t cudahm_workspace_bytes(const cudahm_config* cfg) {
+  int p, dt, nc, nk;
+  if (!valid_config(cfg, &p, &dt, &nc, &nk)) return 0;
+  return make_layout(*cfg, p, nc, dt).total;
+}
+
+extern "C" const char* cudahm_last_error(const cudahm_sampler* s) { return s ? s->err.c_str() : g_err.c_str(); }
+
+extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size_t bytes, void* cuda_stream,
+                             cudahm_sampler** out) {
+  if (!out) return fail(nullptr, CUDAHM_E_INVALID, "out is NULL");
+  *out = nullptr;
+  int p, dt, nc, nk;
+  if (!valid_config(cfg, &p, &dt, &nc, &nk)) return fail(nullptr, CUDAHM_E_INVALID, "invalid cudahm_config");
+  const int block = cfg->block_threads ? cfg->block_threads : 512;
+  KernelSet ks;
+  if (!pick_kernels(cfg->model, cfg->precision, block, &ks))
+    return fail(nullptr, CUDAHM_E_UNSUPPORTED, "model %d is not compiled in for precision %d", cfg->model, cfg->precision);
+  const Layout lay = make_layout(*cfg, p, nc, dt);
+  if (!dev_workspace || bytes < lay.total || ((uintptr_t)dev_workspace & 255u))
+    return fail(nullptr, CUDAHM_E_WORKSPACE, "workspace must be 256-byte aligned and >= %zu bytes (got %zu)", lay.total, bytes);
+  int dev = 0, sms = 0, coop = 0;
+  CU_TRY(nullptr, cudaGetDevice(&dev));
+  CU_TRY(nullptr, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  CU_TRY(nullptr, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev));
+  if (!coop) return fail(nullptr, CUDAHM_E_CUDA, "device does not support cooperative launches");
+
+  cudahm_sampler* s = new cudahm_sampler();
+  s->cfg = *cfg; s->lay = lay; s->ks = ks; s->stream = (cudaStream_t)cuda_stream; s->ws = (char*)dev_workspace;
+  s->p = p; s->dtheta = dt; s->ncols = nc; s->nconsts = nk; s->ntri = p * (p + 1) / 2; s->ntri_theta = dt * (dt + 1) / 2;
+  s->tsize = cfg->precision == CUDAHM_F64 ? 8 : 4;
+  s->vec = cfg->precision == CUDAHM_F64 ? 2 : 4;
+  s->num_sms = sms; s->block = block;
+  s->have_consts = (nk == 0);
+
+  int per_sm = 0;
+  cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ks.persistent, block, 0);
+  if (e != cudaSuccess || per_sm < 1) { delete s; return fail(nullptr, CUDAHM_E_CUDA, "occupancy query failed: %s", cudaGetErrorString(e)); }
+  if (cfg->blocks_per_sm > 0) per_sm = std::min(per_sm, (int)cfg->blocks_per_sm);
+  long long need = (cfg->n_objects + (long long)s->vec * block - 1) / ((long long)s->vec * block);
+  s->grid = (int)std::max(1LL, std::min<long long>((long long)sms * per_sm, need));
+  s->grid = std::min(s->grid, MAX_BLOCKS);
+
+  Params& P = s->P;
+  P.N = cfg->n_objects; P.Npad = (cfg->n_objects + 31) / 32 * 32;
+  P.chi = s->ws + lay.chi; P.L = s->ws + lay.L; P.data = s->ws + lay.data;
+  P.mom_mean = cfg->keep_chi_moments ? (double*)(s->ws + lay.mom_mean) : nullptr;
+  P.mom_M2 = cfg->keep_chi_moments ? (double*)(s->ws + lay.mom_M2) : nullptr;
+  P.slots = (double*)(s->ws + lay.slots); P.bar = (unsigned*)(s->ws + lay.bar);
+  P.iter = (Iter*)(s->ws + lay.iter); P.trace = (double*)(s->ws + lay.trace); P.totals = (double*)(s->ws + lay.totals);
+  P.qx = (double*)(s->ws + lay.qx); P.qex = (double*)(s->ws + lay.qex); P.qW = (double*)(s->ws + lay.qW);
+  for (int k = 0; k < 8; ++k) P.mc[k] = 0.0;
+  P.astar_chi = cfg->target_accept_chi;
+  P.max_blocks = MAX_BLOCKS;
+  P.tail = TailCfg{cfg->model, dt, cfg->freeze_theta ? 1 : 0, cfg->keep_chi_moments ? 1 : 0, cfg->seed,
+                   cfg->target_accept_theta, cfg->eta_exponent, 0, cfg->max_trace_rows, 1, 0};
+  P.taps = DevTaps{};
+
+  if (cudaMemsetAsync(s->ws, 0, lay.total, s->stream) != cudaSuccess ||
+      cudaHostAlloc((void**)&s->h_iter, sizeof(Iter), cudaHostAllocDefault) != cudaSuccess ||
+      cudaHostAlloc((void**)&s->h_totals, NPART * sizeof(double), cudaHostAllocDefault) != cudaSuccess ||
+      cudaEventCreate(&s->ev0) != cudaSuccess || cudaEventCreate(&s->ev1) != cudaSuccess) {
+    const char* m = cudaGetErrorString(cudaGetLastError());
+    cudahm_destroy(s);
+    return fail(nullptr, CUDAHM_E_CUDA, "create: %s", m);
+  }
+  std::memset(s->h_iter, 0, sizeof(Iter));
+  *out = s;
+  return CUDAHM_OK;
+}
+
+extern "C" void cudahm_destroy(cudahm_sampler* s) {
+  if (!s) return;
+  cudaStreamSynchronize(s->stream);
+  if (s->gexec) cudaGraphExecDestroy(s->gexec);
+  if (s->h_iter) cudaFreeHost(s->h_iter);
+  if (s->h_totals) cudaFreeHost(s->h_totals);
+  if (s->ev0) cudaEventDestroy(s->ev0);
+  if (s->ev1) cudaEventDestroy(s->ev1);
+  delete s;
+}
+
+extern "C" int cudahm_sync(cudahm_sampler* s) {
+  if (!s) return fail(nullptr, CUDAHM_E_INVALID, "NULL handle");
+  CU_TRY(s, cudaStreamSynchronize(s->stream));
+  CU_TRY(s, cudaGetLastError());
+  return CUDAHM_OK;
+}
+
+extern "C" int cudahm_set_data(cudahm_sampler* s, const void* const* cols, int n_cols, int cols_on_device) {
+  if (!s || !cols) return fail(s, CUDAHM_E_INVALID, "set_data: NULL argument");
+  if (n_cols != s->ncols) return fail(s, CUDAHM_E_INVALID, "set_data: model takes %d columns, got %d", s->ncols, n_cols);
+  const long long N = s->P.N, Npad = s->P.Npad;
+  const cudaMemcpyKind kind = cols_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  for (int c = 0; c < n_cols; ++c) {
+    if (!cols[c] && N > 0) return fail(s, CUDAHM_E_INVALID, "set_data: column %d is NULL", c);
+    if (N > 0) CU_TRY(s, cudaMemcpyAsync((char*)s->P.data + (size_t)c * Npad * s->tsize, cols[c], (size_t)N * s->tsize, kind, s->stream));
+  }
+  // Gaussian error columns sigma -> 1/(2 sigma^2)
+  int first = -1, last = -1;
+  switch (s->cfg.model) {
+    case M_NORMAL1D: case M_LINREG_ME1D: first = last = 1; break;
+    case M_BINORMAL2D: first = 2; last = 3; break;
+    default: break;
+  }
+  if (N > 0) {
+    const int tb = 256; const unsigned nb = (unsigned)((N + tb - 1) / tb);
+    for (int c = first; c >= 0 && c <= last; ++c) {
+      if (s->tsize == 8) k_sigma_to_h<double><<<nb, tb, 0, s->stream>>>((double*)s->P.data + (size_t)c * Npad, N);
+      else k_sigma_to_h<float><<<nb, tb, 0, s->stream>>>((float*)s->P.data + (size_t)c * Npad, N);
+      s->launches++;
+    }
+    CU_TRY(s, cudaGetLastError());
+  }
+  if (!cols_on_device) CU_TRY(s, cudaStreamSynchronize(s->stream));   // caller may free host buffers on return
+  s->have_data = true; s->have_init = false;
+  return CUDAHM_OK;
+}
+
+namespace {
+// Gauss-Legendre rule on [a,b]: Newton on P_n from the Chebyshev-like guess; weights 2/((1-x^2) P_n'^2).
+void gl_rule(int n, double a, double b, std::vector<double>& x, std::vector<double>& w) {
+  x.assign(n, 0.0); w.assign(n, 0.0);
+  const long double PI = 3.141592653589793238462643383279502884L;
+  const long double half = 0.5L * ((long double)b - (long double)a), mid = 0.5L * ((long double)b + (long double)a);
+  for (int i = 0; i < (n + 1) / 2; ++i) {
+    long double t = cosl(PI * (4 * i + 3) / (4.0L * n + 2.0L)), d = 1.0L;
+    for (int it = 0; it < 64; ++it) {
+      long double pm = 1.0L, pc = t;
+      for (int k = 1; k < n; ++k) { const long double pn = ((2 * k + 1) * t * pc - k * pm) / (k + 1); pm = pc; pc = pn; }
+      d = n * (pm - t * pc) / (1.0L - t * t);
+      const long double step = pc / d;
+      t -= step;
+      if (fabsl(step) < 1e-19L) {
+        pm = 1.0L; pc = t;
+        for (int k = 1; k < n; ++k) { const long double pn = ((2 * k + 1) * t * pc - k * pm) / (k + 1); pm = pc; pc = pn; }
+        d = n * (pm - t * pc) / (1.0L - t * t);
+        break;
+      }
+    }
+    const long double wt = 2.0L / ((1.0L - t * t) * d * d);
+    x[n - 1 - i] = (double)(mid + half * t); x[i] = (double)(mid - half * t);
+    w[n - 1 - i] = w[i] = (double)(half * wt);
+  }
+}
+}  // namespace
+
+extern "C" int cudahm_set_model_consts(cudahm_sampler* s, const double* v, int n) {
+  if (!s) return fail(s, CUDAHM_E_INVALID, "NULL handle");
+  if (n != s->nconsts || (n > 0 && !v)) return fail(s, CUDAHM_E_INVALID, "model takes %d constants, got %d", s->nconsts, n);
+  if (n == 0) { s->have_consts = true; return CUDAHM_OK; }
+  // THINNED_SCHECHTER1D: {F_lim, sigma_F, x_lo, x_hi, r_min, r_max}
+  if (!(v[MC_SIGF] > 0.0 && v[MC_XHI] > v[MC_XLO] && v[MC_RMAX] > v[MC_RMIN] && v[MC_RMIN] > 0.0))
+    return fail(s, CUDAHM_E_INVALID, "model constants out of range");
+  for (int k = 0; k < 6; ++k) s->P.mc[k] = v[k];
+  s->P.mc[MC_INV2S2] = 0.5 / (v[MC_SIGF] * v[MC_SIGF]);
+  // selection table: W_k = w_k * G(x_k), G(x) = int h(r) Phi((e^x/(4 pi r^2) - F_lim)/sigma_F) dr
+  std::vector<double> xk, wk, rj, wj, ex(NQUAD), W(NQUAD);
+  gl_rule(NQUAD, v[MC_XLO], v[MC_XHI], xk, wk);
+  gl_rule(256, v[MC_RMIN], v[MC_RMAX], rj, wj);
+  const double vol3 = (v[MC_RMAX] * v[MC_RMAX] * v[MC_RMAX] - v[MC_RMIN] * v[MC_RMIN] * v[MC_RMIN]) / 3.0;
+  const double inv_s2 = 1.0 / (v[MC_SIGF] * std::sqrt(2.0));
+  for (int k = 0; k < NQUAD; ++k) {
+    ex[k] = std::exp(xk[k]);
+    long double G = 0.0L;
+    for (int j = 0; j < 256; ++j) {
+      const double r2 = rj[j] * rj[j];
+      const double F = ex[k] / (4.0 * M_PI * r2);
+      G += (long double)(wj[j] * r2 * 0.5 * std::erfc((v[MC_FLIM] - F) * inv_s2));
+    }
+    W[k] = wk[k] * (double)(G / vol3);
+  }
+  CU_TRY(s, cudaMemcpyAsync((void*)s->P.qx, xk.data(), NQUAD * 8, cudaMemcpyHostToDevice, s->stream));
+  CU_TRY(s, cudaMemcpyAsync((void*)s->P.qex, ex.data(), NQUAD * 8, cudaMemcpyHostToDevice, s->stream));
+  CU_TRY(s, cudaMemcpyAsync((void*)s->P.qW, W.data(), NQUAD * 8, cudaMemcpyHostToDevice, s->stream));
+  CU_TRY(s, cudaStreamSynchronize(s->stream));
+  s->have_consts = true; s->have_init = false;
+  return CUDAHM_OK;
+}
+
+// ----------------------------------------------------------------------------------------------------
+namespace {
+
+int launch(cudahm_sampler* s, const void* fn, int grid, int block, void** args, bool cooperative) {
+  cudaError_t e = cooperative ? cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(block), args, 0, s->stream)
+                              : cudaLaunchKernel(fn, dim3(grid), dim3(block), args, 0, s->stream);
+  if (e != cudaSuccess) return fail(s, CUDAHM_E_CUDA, "kernel launch: %s", cudaGetErrorString(e));
+  s->launches++;
+  return CUDAHM_OK;
+}
+
+// upload a raw Iter (theta, L_theta, counters, t) and let the device derive the rest (k_init_iter)
+int upload_and_init_iter(cudahm_sampler* s, const Iter& raw) {
+  *s->h_iter = raw;
+  CU_TRY(s, cudaMemcpyAsync(s->P.iter, s->h_iter, sizeof(Iter), cudaMemcpyHostToDevice, s->stream));
+  Params P = s->P;
+  void* args[] = {&P};
+  int rc = launch(s, (const void*)k_init_iter, 1, 256, args, false);
+  if (rc) return rc;
+  CU_TRY(s, cudaMemcpyAsync(s->h_iter, s->P.iter, sizeof(Iter), cudaMemcpyDeviceToHost, s->stream));
+  CU_TRY(s, cudaStreamSynchronize(s->stream));
+  s->host_iter_valid = true;
+  return CUDAHM_OK;
+}
+
+int fetch_iter(cudahm_sampler* s) {   // device -> h_iter (no-op in host mode, where h_iter is authoritative)
+  CU_TRY(s, cudaStreamSynchronize(s->stream));
+  if (s->cfg.theta_mode == CUDAHM_THETA_HOST && s->host_iter_valid) return CUDAHM_OK;
+  CU_TRY(s, cudaMemcpy(s->h_iter, s->P.iter, sizeof(Iter), cudaMemcpyDeviceToHost));
+  return CUDAHM_OK;
+}
+
+}  // namespace
+
+extern "C" int cudahm_set_init(cudahm_sampler* s, const void* chi0, int chi0_on_device, const double* theta0,
+                               const double* theta_chol0) {
+  if (!s || !theta0) return fail(s, CUDAHM_E_INVALID, "set_init: NULL argument");
+  if (!s->have_data || !s->have_consts) return fail(s, CUDAHM_E_STATE, "set_init before set_data / set_model_consts");
+  const long long N = s->P.N, Npad = s->P.Npad;
+  if (chi0 && N > 0) {
+    const cudaMemcpyKind kind = chi0_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    for (int j = 0; j < s->p; ++j)
+      CU_TRY(s, cudaMemcpyAsync((char*)s->P.chi + (size_t)j * Npad * s->tsize, (const char*)chi0 + (size_t)j * N * s->tsize,
+                                (size_t)N * s->tsize, kind, s->stream));
+  }
+  if (N > 0) {
+    Params P = s->P;
+    const void* raw = s->P.data;
+    int have = chi0 ? 1 : 0;
+    double sc64 = s->cfg.init_scale_chi; float sc32 = (float)sc64;
+    void* args[] = {&P, &raw, &have, s->tsize == 8 ? (void*)&sc64 : (void*)&sc32};
+    int rc = launch(s, s->ks.init_state, (int)((N + 255) / 256), 256, args, false);
+    if (rc) return rc;
+  }
+  if (s->lay.trace != s->lay.totals)
+    CU_TRY(s, cudaMemsetAsync(s->P.trace, 0, (size_t)s->cfg.max_trace_rows * s->dtheta * 8, s->stream));
+  Iter raw;
+  std::memset(&raw, 0, sizeof raw);
+  for (int r = 0; r < s->dtheta; ++r) raw.theta[r] = theta0[r];
+  if (theta_chol0) for (int k = 0; k < s->ntri_theta; ++k) raw.Lth[k] = theta_chol0[k];
+  else for (int r = 0; r < s->dtheta; ++r) raw.Lth[tri(r, r)] = 0.1;
+  raw.t = 1;
+  s->t_done = 0;
+  int rc = upload_and_init_iter(s, raw);
+  if (rc) return rc;
+  s->have_init = true;
+  return CUDAHM_OK;
+}
+
+namespace {
+
+// THETA_DEVICE_TAIL: cooperative persistent launches of at most max_it iterations each
+int run_device_tail(cudahm_sampler* s, long long n_iter) {
+  const long long max_it = (long long)(0x7fffffffLL / std::max(1, s->grid));
+  while (n_iter > 0) {
+    long long k = std::min(n_iter, max_it);
+    CU_TRY(s, cudaMemsetAsync(s->P.bar, 0, sizeof(unsigned), s->stream));
+    Params P = s->P;
+    void* args[] = {&P, &k};
+    int rc = launch(s, s->ks.persistent, s->grid, s->block, args, true);
+    if (rc) return rc;
+    n_iter -= k;
+  }
+  return CUDAHM_OK;
+}
+
+int enqueue_graph_iteration(cudahm_sampler* s) {
+  Params P = s->P;
+  void* a1[] = {&P};
+  int rc = launch(s, s->ks.sweep, s->grid, s->block, a1, false);
+  if (rc) return rc;
+  int nb = s->grid, flags = TAIL_REDUCE | TAIL_DECIDE | TAIL_PREPARE;
+  void* a2[] = {&P, &nb, &flags};
+  return launch(s, (const void*)k_tail, 1, 32, a2, false);
+}
+
+// THETA_GRAPH: {sweep, tail} x GRAPH_ITERS captured once per (burn_in, thin), replayed; remainder launched directly
+int run_graph(cudahm_sampler* s, long long n_iter) {
+  constexpr int GRAPH_ITERS = 50;
+  if (n_iter >= GRAPH_ITERS) {
+    if (!s->gexec || s->g_burn != s->P.tail.burn_in || s->g_thin != s->P.tail.thin) {
+      if (s->gexec) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }
+      cudaStream_t cap;
+      CU_TRY(s, cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+      cudaStream_t user = s->stream;
+      s->stream = cap;
+      const long long before = s->launches;
+      cudaGraph_t g = nullptr;
+      cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+      int rc = CUDAHM_OK;
+      if (e == cudaSuccess) {
+        for (int k = 0; k < GRAPH_ITERS && rc == CUDAHM_OK; ++k) rc = enqueue_graph_iteration(s);
+        e = cudaStreamEndCapture(cap, &g);
+      }
+      s->stream = user;
+      s->launches = before;
+      if (rc == CUDAHM_OK && e == cudaSuccess) e = cudaGraphInstantiate(&s->gexec, g, 0);
+      if (g) cudaGraphDestroy(g);
+      cudaStreamDestroy(cap);
+      if (rc) return rc;
+      if (e != cudaSuccess) return fail(s, CUDAHM_E_CUDA, "graph capture: %s", cudaGetErrorString(e));
+      s->g_burn = s->P.tail.burn_in; s->g_thin = s->P.tail.thin; s->g_iters = GRAPH_ITERS;
+    }
+    while (n_iter >= GRAPH_ITERS) {
+      CU_TRY(s, cudaGraphLaunch(s->gexec, s->stream));
+      s->launches += 2 * GRAPH_ITERS;
+      n_iter -= GRAPH_ITERS;
+    }
+  }
+  for (; n_iter > 0; --n_iter) { int rc = enqueue_graph_iteration(s); if (rc) return rc; }
+  return CUDAHM_OK;
+}
+
+// THETA_HOST (the paper's split): sweep + reduction on the device, theta step in host C++
+int run_host(cudahm_sampler* s, long long n_iter) {
+  Iter& it = *s->h_iter;
+  for (long long k = 0; k < n_iter; ++k) {
+    Params P = s->P;
+    void* a1[] = {&P};
+    int rc = launch(s, s->ks.sweep, s->grid, s->block, a1, false);
+    if (rc) return rc;
+    int nb = s->grid, flags = TAIL_REDUCE;
+    void* a2[] = {&P, &nb, &flags};
+    rc = launch(s, (const void*)k_tail, 1, 32, a2, false);
+    if (rc) return rc;
+    CU_TRY(s, cudaMemcpyAsync(s->h_totals, s->P.totals, NPART * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    CU_TRY(s, cudaStreamSynchronize(s->stream));
+    tail_decide(it, s->P.tail, s->h_totals);
+    if (it.trace_write)
+      CU_TRY(s, cudaMemcpyAsync(s->P.trace + (it.trace_rows - 1) * s->dtheta, it.theta, s->dtheta * sizeof(double),
+                                cudaMemcpyHostToDevice, s->stream));
+    prepare_iteration(it, s->P.tail, it.t + 1);
+    CU_TRY(s, cudaMemcpyAsync(s->P.iter, s->h_iter, sizeof(Iter), cudaMemcpyHostToDevice, s->stream));
+    // h_iter is pinned and reused next iteration: the copy must have left before we overwrite it
+    CU_TRY(s, cudaStreamSynchronize(s->stream));
+  }
+  return CUDAHM_OK;
+}
+
+}  // namespace
+
+extern "C" int cudahm_run(cudahm_sampler* s, int64_t n_iter, int64_t burn_in, int32_t thin) {
+  if (!s) return fail(s, CUDAHM_E_INVALID, "NULL handle");
+  if (!s->have_init) return fail(s, CUDAHM_E_STATE, "run before set_init");
+  if (n_iter < 0 || burn_in < 0 || thin < 1) return fail(s, CUDAHM_E_INVALID, "run: bad n_iter/burn_in/thin");
+  if (s->t_done + n_iter >= 0xffffffffLL) return fail(s, CUDAHM_E_INVALID, "iteration index exceeds the 32-bit stream counter");
+  // trace capacity
+  {
+    int rc = fetch_iter(s); if (rc) return rc;
+    const long long t1 = s->t_done + n_iter;
+    const long long lo = std::max<long long>(s->t_done, burn_in);
+    const long long rows = t1 > lo ? (t1 - burn_in) / thin - (lo - burn_in) / thin : 0;
+    if (s->h_iter->trace_rows + rows > s->cfg.max_trace_rows)
+      return fail(s, CUDAHM_E_INVALID, "theta trace would need %lld rows, capacity %lld", s->h_iter->trace_rows + rows,
+                  (long long)s->cfg.max_trace_rows);
+  }
+  s->P.tail.burn_in = burn_in; s->P.tail.thin = thin;
+  if (n_iter == 0) return CUDAHM_OK;
+  CU_TRY(s, cudaEventRecord(s->ev0, s->stream));
+  int rc;
+  switch (s->cfg.theta_mode) {
+    case CUDAHM_THETA_DEVICE_TAIL: rc = run_device_tail(s, n_iter); break;
+    case CUDAHM_THETA_GRAPH:       rc = run_graph(s, n_iter); break;
+    default:                       rc = run_host(s, n_iter); break;
+  }
+  if (rc) return rc;
+  CU_TRY(s, cudaEventRecord(s->ev1, s->stream));
+  s->timed = true;
+  s->t_done += n_iter;
+  return CUDAHM_OK;
+}
+
+// ----------------------------------------------------------------------------------------------------
+extern "C" int cudahm_debug_step(cudahm_sampler* s, int64_t burn_in, int32_t thin, cudahm_taps* taps) {
+  if (!s || !taps) return fail(s, CUDAHM_E_INVALID, "debug_step: NULL argument");
+  if (!s->have_init) return fail(s, CUDAHM_E_STATE, "debug_step before set_init");
+  if (burn_in < 0 || thin < 1) return fail(s, CUDAHM_E_INVALID, "debug_step: bad burn_in/thin");
+  int rc = fetch_iter(s); if (rc) return rc;
+  if (s->cfg.theta_mode == CUDAHM_THETA_HOST)   // make the device copy current
+    CU_TRY(s, cudaMemcpy(s->P.iter, s->h_iter, sizeof(Iter), cudaMemcpyHostToDevice));
+  const long long t = s->h_iter->t;
+  if (t > burn_in && ((t - burn_in) % thin) == 0 && s->h_iter->trace_rows + 1 > s->cfg.max_trace_rows)
+    return fail(s, CUDAHM_E_INVALID, "theta trace is full");
+  s->P.tail.burn_in = burn_in; s->P.tail.thin = thin;
+  const size_t N = (size_t)s->P.N;
+  // tap scratch is test instrumentation, not the hot path: allocated here, freed below
+  const size_t nd = (size_t)(s->p + s->ntri + 6) * N;
+  double* dbuf = nullptr; int* ibuf = nullptr;
+  if (N > 0) {
+    CU_TRY(s, cudaMalloc((void**)&dbuf, nd * sizeof(double)));
+    if (cudaMalloc((void**)&ibuf, N * sizeof(int)) != cudaSuccess) { cudaFree(dbuf); return fail(s, CUDAHM_E_CUDA, "cudaMalloc taps"); }
+  }
+  Params P = s->P;
+  double* q = dbuf;
+  P.taps.chi_prop = q; q += (size_t)s->p * N;
+  P.taps.L_new = q; q += (size_t)s->ntri * N;
+  P.taps.pi_cur = q; q += N; P.taps.pi_prop = q; q += N; P.taps.alpha = q; q += N;
+  P.taps.u = q; q += N; P.taps.a = q; q += N; P.taps.b = q; q += N;
+  P.taps.accepted = ibuf;
+  void* a1[] = {&P};
+  rc = launch(s, s->ks.sweep_tap, s->grid, s->block, a1, false);
+  int nb = s->grid, flags = TAIL_REDUCE | TAIL_DECIDE;
+  void* a2[] = {&P, &nb, &flags};
+  if (!rc) rc = launch(s, (const void*)k_tail, 1, 32, a2, false);
+  cudaError_t e = cudaSuccess;
+  if (!rc) e = cudaMemcpyAsync(s->h_iter, s->P.iter, sizeof(Iter), cudaMemcpyDeviceToHost, s->stream);
+  if (!rc && e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  if (!rc && e == cudaSuccess) {
+    const Iter& it = *s->h_iter;
+    for (int r = 0; r < 8; ++r) taps->theta_prop[r] = r < s->dtheta ? it.thetaP[r] : 0.0;
+    taps->S = it.S; taps->Delta = it.Delta; taps->T_cur = it.T_cur_used; taps->T_prop = it.T_prop;
+    taps->lp_cur = it.lp_cur_used; taps->lp_prop = it.lp_prop; taps->log_r = it.log_r;
+    taps->alpha_theta = it.alpha_theta; taps->u_theta = it.u_theta; taps->accepted_theta = it.accepted_theta;
+    struct { double* dst; const double* src; size_t n; } cp[] = {
+        {taps->chi_prop, P.taps.chi_prop, (size_t)s->p * N}, {taps->L_new, P.taps.L_new, (size_t)s->ntri * N},
+        {taps->pi_cur, P.taps.pi_cur, N}, {taps->pi_prop, P.taps.pi_prop, N}, {taps->alpha, P.taps.alpha, N},
+        {taps->u, P.taps.u, N}, {taps->a, P.taps.a, N}, {taps->b, P.taps.b, N}};
+    for (auto& c : cp)
+      if (c.dst && c.n && e == cudaSuccess) e = cudaMemcpy(c.dst, c.src, c.n * sizeof(double), cudaMemcpyDeviceToHost);
+    if (taps->accepted && N && e == cudaSuccess) e = cudaMemcpy(taps->accepted, ibuf, N * sizeof(int), cudaMemcpyDeviceToHost);
+  }
+  // prepare the next iteration (device prepares in the device modes, the host in host mode)
+  if (!rc && e == cudaSuccess) {
+    if (s->cfg.theta_mode == CUDAHM_THETA_HOST) {
+      prepare_iteration(*s->h_iter, s->P.tail, s->h_iter->t + 1);
+      e = cudaMemcpy(s->P.iter, s->h_iter, sizeof(Iter), cudaMemcpyHostToDevice);
+    } else {
+      // the tail kernel decided without preparing: it.t is still the decided iteration
+      Iter tmp = *s->h_iter; tmp.t += 1;
+      e = cudaMemcpy(s->P.iter, &tmp, sizeof(Iter), cudaMemcpyHostToDevice);
+      int fl = TAIL_PREPARE;
+      void* a3[] = {&P, &nb, &fl};
+      if (e == cudaSuccess) rc = launch(s, (const void*)k_tail, 1, 32, a3, false);
+      if (!rc) e = cudaStreamSynchronize(s->stream);
+    }
+  }
+  if (dbuf) cudaFree(dbuf);
+  if (ibuf) cudaFree(ibuf);
+  if (rc) return rc;
+  if (e != cudaSuccess) return fail(s, CUDAHM_E_CUDA, "debug_step: %s", cudaGetErrorString(e));
+  s->t_done += 1;
+  return CUDAHM_OK;
+}
+
+extern "C" int cudahm_get_theta_trace(cudahm_sampler* s, double* out, int64_t cap_rows, int64_t* n_rows) {
+  if (!s || !n_rows) return fail(s, CUDAHM_E_INVALID, "get_theta_trace: NULL argument");
+  if (!s->have_init) return fail(s, CUDAHM_E_STATE, "get_theta_trace before set_init");
+  int rc = fetch_iter(s); if (rc) return rc;
+  const long long rows = s->h_iter->trace_rows;
+  *n_rows = rows;
+  if (!out) return CUDAHM_OK;
+  if (cap_rows < rows) return fail(s, CUDAHM_E_INVALID, "trace has %lld rows, capacity %lld", rows, (long long)cap_rows);
+  if (rows > 0) CU_TRY(s, cudaMemcpy(out, s->P.trace, (size_t)rows * s->dtheta * 8, cudaMemcpyDeviceToHost));
+  return CUDAHM_OK;
+}
+
+extern "C" int cudahm_get_chi_moments(cudahm_sampler* s, double* mean, double* var, int64_t cap_objects, int64_t* n_samples) {
+  if (!s || !n_samples) return fail(s, CUDAHM_E_INVALID, "get_chi_moments: NULL argument");
+  if (!s->have_init) return fail(s, CUDAHM_E_STATE, "get_chi_moments before set_init");
+  if (!s->cfg.keep_chi_moments) return fail(s, CUDAHM_E_STATE, "keep_chi_moments was not set");
+  int rc = fetch_iter(s); if (rc) return rc;
+  const long long cnt = s->h_iter->mom_count, N = s->P.N, Npad = s->P.Npad;
+  *n_samples = cnt;
+  if (cap_objects < N) return fail(s, CUDAHM_E_INVALID, "moments need room for %lld objects", N);
+  double* dvar = (double*)(s->ws + s->lay.mom_var);
+  if (var && N > 0) {
+    const long long n = (long long)s->p * Npad;
+    const double inv = cnt > 1 ? 1.0 / (double)(cnt - 1) : 0.0;
+    k_finalize_moments<<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(s->P.mom_M2, dvar, n, inv);
+    s->launches++;
+    CU_TRY(s, cudaGetLastError());
+    CU_TRY(s, cudaStreamSynchronize(s->stream));
+  }
+  for (int j = 0; j < s->p && N > 0; ++j) {
+    if (mean) CU_TRY(s, cudaMemcpy(mean + (size_t)j * N, s->P.mom_mean + (size_t)j * Npad, (size_t)N * 8, cudaMemcpyDeviceToHost));
+    if (var) CU_TRY(s, cudaMemcpy(var + (size_t)j * N, dvar + (size_t)j * Npad, (size_t)N * 8, cudaMemcpyDeviceToHost));
+  }
+  return CUDAHM_OK;
+}
+
+extern "C" int cudahm_get_stats(cudahm_sampler* s, cudahm_stats* out) {
+  if (!s || !out) return fail(s, CUDAHM_E_INVALID, "get_stats: NULL argument");
+  std::memset(out, 0, sizeof *out);
+  out->grid_blocks = s->grid; out->block_threads = s->block; out->gpu_launches = s->launches;
+  if (!s->have_init) return CUDAHM_OK;
+  int rc = fetch_iter(s); if (rc) return rc;
+  const Iter& it = *s->h_iter;
+  out->iterations = it.t - 1;
+  out->chi_accepts = (int64_t)it.chi_acc; out->chi_proposals = (it.t - 1) * s->P.N;
+  out->theta_accepts = (int64_t)it.theta_acc; out->theta_proposals = (int64_t)it.theta_prop_n;
+  out->nonfinite = (int64_t)it.nonfinite; out->moment_samples = it.mom_count; out->trace_rows = it.trace_rows;
+  if (s->timed) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, s->ev0, s->ev1) == cudaSuccess) out->last_run_ms = ms;
+  }
+  return CUDAHM_OK;
+}
+
+extern "C" int cudahm_get_state(cudahm_sampler* s, void* chi, void* L, double* theta, double* L_theta, int64_t* t) {
+  if (!s) return fail(s, CUDAHM_E_INVALID, "NULL handle");
+  if (!s->have_init) return fail(s, CUDAHM_E_STATE, "get_state before set_init");
+  int rc = fetch_iter(s); if (rc) return rc;
+  const size_t N = (size_t)s->P.N, Npad = (size_t)s->P.Npad, ts = s->tsize;
+  for (int j = 0; j < s->p && chi && N; ++j)
+    CU_TRY(s, cudaMemcpy((char*)chi + j * N * ts, (char*)s->P.chi + j * Npad * ts, N * ts, cudaMemcpyDeviceToHost));
+  for (int k = 0; k < s->ntri && L && N; ++k)
+    CU_TRY(s, cudaMemcpy((char*)L + k * N * ts, (char*)s->P.L + k * Npad * ts, N * ts, cudaMemcpyDeviceToHost));
+  if (theta) std::copy(s->h_iter->theta, s->h_iter->theta + s->dtheta, theta);
+  if (L_theta) std::copy(s->h_iter->Lth, s->h_iter->Lth + s->ntri_theta, L_theta);
+  if (t) *t = s->h_iter->t - 1;
+  return CUDAHM_OK;
+}
+
+extern "C" int cudahm_set_state(cudahm_sampler* s, const void* chi, const void* L, const double* theta,
+                                const double* L_theta, int64_t t) {
+  if (!s || t < 0) return fail(s, CUDAHM_E_INVALID, "set_state: bad argument");
+  if (!s->have_init) return fail(s, CUDAHM_E_STATE, "set_state before set_init");
+  int rc = fetch_iter(s); if (rc) return rc;
+  const size_t N = (size_t)s->P.N, Npad = (size_t)s->P.Npad, ts = s->tsize;
+  for (int j = 0; j < s->p && chi && N; ++j)
+    CU_TRY(s, cudaMemcpy((char*)s->P.chi + j * Npad * ts, (const char*)chi + j * N * ts, N * ts, cudaMemcpyHostToDevice));
+  for (int k = 0; k < s->ntri && L && N; ++k)
+    CU_TRY(s, cudaMemcpy((char*)s->P.L + k * Npad * ts, (const char*)L + k * N * ts, N * ts, cudaMemcpyHostToDevice));
+  Iter raw = *s->h_iter;
+  if (theta) std::copy(theta, theta + s->dtheta, raw.theta);
+  if (L_theta) std::copy(L_theta, L_theta + s->ntri_theta, raw.Lth);
+  raw.t = t + 1;
+  s->t_done = t;
+  return upload_and_init_iter(s, raw);
+}

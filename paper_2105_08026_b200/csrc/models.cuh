@@ -1,0 +1,153 @@
+// models.cuh -- compiled-in models of the CUDA path: the counterpart of the paper's two user functions
+// (member log-likelihood log l_i(chi); population log-density log f(chi; theta), PAPER.md:80;
+// see PAPER.md:144, :391) plus the theta prior.  Definitions: DESIGN.md section 3.
+//
+// Layout choices made for the kernels (not part of the model):
+//   - every theta-only transcendental (exp(-2 lambda), exp(-x*), log cosh zeta ...) is hoisted into a small
+//     table ThetaK computed once per iteration by the theta tail, for theta and for theta';
+//   - Gaussian error columns are stored as h = 1/(2 sigma^2) so the sweep has no division;
+//   - M1 evaluates e^chi once per point and shares it between the flux likelihood and the population term.
+#pragma once
+#include <cmath>
+#include <cstdint>
+#include "philox.cuh"
+
+namespace hm {
+
+enum : int { M_NORMAL1D = 0, M_THINNED_SCHECHTER1D = 1, M_BINORMAL2D = 2, M_LINREG_ME1D = 3 };
+enum : int { MC_FLIM = 0, MC_SIGF = 1, MC_XLO = 2, MC_XHI = 3, MC_RMIN = 4, MC_RMAX = 5, MC_INV2S2 = 6 };
+constexpr int NQUAD = 1024;   // selection-integral nodes (BASELINE.json configs[1])
+
+template <int MODEL> struct ModelDims;
+template <> struct ModelDims<M_NORMAL1D>            { static constexpr int p = 1, dtheta = 2, ncols = 2, nconsts = 0; };
+template <> struct ModelDims<M_THINNED_SCHECHTER1D> { static constexpr int p = 1, dtheta = 3, ncols = 2, nconsts = 6; };
+template <> struct ModelDims<M_BINORMAL2D>          { static constexpr int p = 2, dtheta = 5, ncols = 4, nconsts = 0; };
+template <> struct ModelDims<M_LINREG_ME1D>         { static constexpr int p = 1, dtheta = 3, ncols = 3, nconsts = 0; };
+
+inline bool model_dims(int model, int* p, int* dtheta, int* ncols, int* nconsts) {
+  switch (model) {
+    case M_NORMAL1D:            *p = 1; *dtheta = 2; *ncols = 2; *nconsts = 0; return true;
+    case M_THINNED_SCHECHTER1D: *p = 1; *dtheta = 3; *ncols = 2; *nconsts = 6; return true;
+    case M_BINORMAL2D:          *p = 2; *dtheta = 5; *ncols = 4; *nconsts = 0; return true;
+    case M_LINREG_ME1D:         *p = 1; *dtheta = 3; *ncols = 3; *nconsts = 0; return true;
+  }
+  return false;
+}
+
+// theta-derived constants, fp64
+struct ThetaK { double v[8]; };
+
+HM_HD ThetaK theta_consts(int model, const double* th) {
+  ThetaK k;
+#pragma unroll
+  for (int j = 0; j < 8; ++j) k.v[j] = 0.0;
+  switch (model) {
+    case M_NORMAL1D:            // (mu, lambda): f = -lambda - (chi - mu)^2 * [e^(-2 lambda)/2]
+      k.v[0] = th[0]; k.v[1] = th[1]; k.v[2] = 0.5 * exp(-2.0 * th[1]);
+      break;
+    case M_LINREG_ME1D:         // (a, b, lambda): f = -lambda - (chi - a - b z)^2 * [e^(-2 lambda)/2]
+      k.v[0] = th[0]; k.v[1] = th[1]; k.v[2] = th[2]; k.v[3] = 0.5 * exp(-2.0 * th[2]);
+      break;
+    case M_THINNED_SCHECHTER1D: // (alpha, x*, a): f = a + (alpha+1)(chi - x*) - e^chi e^(-x*)
+      k.v[0] = th[0] + 1.0; k.v[1] = th[1]; k.v[2] = th[2]; k.v[3] = exp(-th[1]);
+      break;
+    case M_BINORMAL2D: {        // (m1, m2, l1, l2, zeta): f = c0 - h (u1^2 - 2 rho u1 u2 + u2^2)
+      const double ch = cosh(th[4]);
+      k.v[0] = th[0]; k.v[1] = th[1]; k.v[2] = exp(-th[2]); k.v[3] = exp(-th[3]);
+      k.v[4] = -th[2] - th[3] + log(ch); k.v[5] = 0.5 * ch * ch; k.v[6] = tanh(th[4]);
+      break;
+    }
+  }
+  return k;
+}
+
+// log prior: flat on a wide box; M1 slope: truncated Cauchy of Eq. 5.4
+HM_HD double log_prior(int model, const double* th) {
+  const double ninf = -INFINITY;
+  switch (model) {
+    case M_NORMAL1D:
+      return (fabs(th[0]) <= 1e3 && fabs(th[1]) <= 10.0) ? 0.0 : ninf;
+    case M_LINREG_ME1D:
+      return (fabs(th[0]) <= 1e3 && fabs(th[1]) <= 1e3 && fabs(th[2]) <= 10.0) ? 0.0 : ninf;
+    case M_BINORMAL2D:
+      return (fabs(th[0]) <= 1e3 && fabs(th[1]) <= 1e3 && fabs(th[2]) <= 10.0 && fabs(th[3]) <= 10.0 &&
+              fabs(th[4]) <= 10.0) ? 0.0 : ninf;
+    case M_THINNED_SCHECHTER1D:
+      return (th[0] > -2.0 && th[0] < 0.0 && fabs(th[1]) <= 20.0 && fabs(th[2]) <= 50.0)
+                 ? -log1p(th[0] * th[0]) : ninf;
+  }
+  return ninf;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// Plate-side evaluation.  T = state precision.  D = stored data columns of the object (h = 1/(2 sigma^2)).
+// K<T> = ThetaK narrowed to T.  A "point" caches what the target and the population terms share.
+template <class T> struct KT { T v[7]; };
+template <class T> HM_HD KT<T> narrow(const ThetaK& k) {
+  KT<T> r;
+#pragma unroll
+  for (int j = 0; j < 7; ++j) r.v[j] = (T)k.v[j];
+  return r;
+}
+
+__device__ __forceinline__ double hm_exp(double x) { return exp(x); }
+__device__ __forceinline__ float hm_exp(float x) { return expf(x); }
+
+template <int MODEL, class T> struct Plate;
+
+template <class T> struct Plate<M_NORMAL1D, T> {
+  struct Pt { T x; };
+  __device__ __forceinline__ static Pt point(const T* chi) { return Pt{chi[0]}; }
+  // log l_i + log f(.; theta)
+  __device__ __forceinline__ static T target(const Pt& q, const T* d, const KT<T>& k, const T*) {
+    const T r = d[0] - q.x, s = q.x - k.v[0];
+    return -(r * r) * d[1] - k.v[1] - (s * s) * k.v[2];
+  }
+  __device__ __forceinline__ static double pop(const Pt& q, const T*, const ThetaK& k) {
+    const double s = (double)q.x - k.v[0];
+    return -k.v[1] - (s * s) * k.v[2];
+  }
+};
+
+template <class T> struct Plate<M_LINREG_ME1D, T> {
+  struct Pt { T x; };
+  __device__ __forceinline__ static Pt point(const T* chi) { return Pt{chi[0]}; }
+  __device__ __forceinline__ static T target(const Pt& q, const T* d, const KT<T>& k, const T*) {
+    const T r = d[0] - q.x, s = q.x - k.v[0] - k.v[1] * d[2];
+    return -(r * r) * d[1] - k.v[2] - (s * s) * k.v[3];
+  }
+  __device__ __forceinline__ static double pop(const Pt& q, const T* d, const ThetaK& k) {
+    const double s = (double)q.x - k.v[0] - k.v[1] * (double)d[2];
+    return -k.v[2] - (s * s) * k.v[3];
+  }
+};
+
+template <class T> struct Plate<M_THINNED_SCHECHTER1D, T> {
+  struct Pt { T x, ex; };
+  __device__ __forceinline__ static Pt point(const T* chi) { return Pt{chi[0], hm_exp(chi[0])}; }
+  // mc = {F_lim, sigma_F, x_lo, x_hi, r_min, r_max, 1/(2 sigma_F^2)} narrowed to T
+  __device__ __forceinline__ static T target(const Pt& q, const T* d, const KT<T>& k, const T* mc) {
+    if (!(q.x >= mc[MC_XLO] && q.x <= mc[MC_XHI])) return -INFINITY;
+    const T r = d[0] - d[1] * q.ex;
+    return -(r * r) * mc[MC_INV2S2] + k.v[2] + k.v[0] * (q.x - k.v[1]) - q.ex * k.v[3];
+  }
+  __device__ __forceinline__ static double pop(const Pt& q, const T*, const ThetaK& k) {
+    return k.v[2] + k.v[0] * ((double)q.x - k.v[1]) - (double)q.ex * k.v[3];
+  }
+};
+
+template <class T> struct Plate<M_BINORMAL2D, T> {
+  struct Pt { T x1, x2; };
+  __device__ __forceinline__ static Pt point(const T* chi) { return Pt{chi[0], chi[1]}; }
+  __device__ __forceinline__ static T target(const Pt& q, const T* d, const KT<T>& k, const T*) {
+    const T r1 = d[0] - q.x1, r2 = d[1] - q.x2;
+    const T u1 = (q.x1 - k.v[0]) * k.v[2], u2 = (q.x2 - k.v[1]) * k.v[3];
+    return -(r1 * r1) * d[2] - (r2 * r2) * d[3] + k.v[4] - k.v[5] * (u1 * u1 - T(2) * k.v[6] * u1 * u2 + u2 * u2);
+  }
+  __device__ __forceinline__ static double pop(const Pt& q, const T*, const ThetaK& k) {
+    const double u1 = ((double)q.x1 - k.v[0]) * k.v[2], u2 = ((double)q.x2 - k.v[1]) * k.v[3];
+    return k.v[4] - k.v[5] * (u1 * u1 - 2.0 * k.v[6] * u1 * u2 + u2 * u2);
+  }
+};
+
+}  // namespace hm

@@ -1,0 +1,75 @@
+// philox.cuh -- counter-based Philox4x32-10 streams of the CUDA path (host + device).
+//
+// Replaces the PRNG library of the paper (PAPER.md:65 fn. 2, :142) with streams keyed by
+// (seed, object, iteration, draw) so any thread can produce any variate with no RNG state in HBM
+// (DESIGN.md section 4).  Shares nothing with oracle/.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#define HM_HD __host__ __device__ __forceinline__
+
+namespace hm {
+
+enum : int { KIND_PLATE = 0, KIND_THETA = 1 };
+
+struct U4 { uint32_t x, y, z, w; };
+
+HM_HD uint32_t mulhi32(uint32_t a, uint32_t b) {
+#ifdef __CUDA_ARCH__
+  return __umulhi(a, b);
+#else
+  return (uint32_t)(((uint64_t)a * (uint64_t)b) >> 32);
+#endif
+}
+
+// 10 rounds of the Philox-4x32 S-P network; the key schedule is a Weyl sequence.
+HM_HD U4 philox4x32_10(U4 c, uint32_t k0, uint32_t k1) {
+  constexpr uint32_t PM0 = 0xD2511F53u, PM1 = 0xCD9E8D57u, PW0 = 0x9E3779B9u, PW1 = 0xBB67AE85u;
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint32_t h0 = mulhi32(PM0, c.x), l0 = PM0 * c.x;
+    const uint32_t h1 = mulhi32(PM1, c.z), l1 = PM1 * c.z;
+    c = U4{h1 ^ c.y ^ k0, l1, h0 ^ c.w ^ k1, l0};
+    k0 += PW0; k1 += PW1;
+  }
+  return c;
+}
+
+// counter = (object lo, kind<<24 | object bits 32..55, iteration, draw); key = seed words
+HM_HD U4 stream(uint64_t seed, int kind, uint64_t obj, uint32_t t, uint32_t d) {
+  U4 c{(uint32_t)obj, ((uint32_t)kind << 24) | ((uint32_t)(obj >> 32) & 0xffffffu), t, d};
+  return philox4x32_10(c, (uint32_t)seed, (uint32_t)(seed >> 32));
+}
+
+// (52 random bits + 1/2) * 2^-52: exact, in [2^-53, 1 - 2^-53]
+HM_HD double u01(uint32_t a, uint32_t b) {
+  const uint64_t k = ((uint64_t)(a >> 6) << 26) | (uint64_t)(b >> 6);
+  return ((double)(int64_t)k + 0.5) * 0x1.0p-52;
+}
+// (23 random bits + 1/2) * 2^-23: exact in fp32
+HM_HD float u01f(uint32_t a) { return ((float)(a >> 9) + 0.5f) * 0x1.0p-23f; }
+
+// Box-Muller pair from one Philox call (fp64): u1 from (x,y), u2 from (z,w).
+// Returns radius and the unit vector (cos, sin)(2 pi u2): z = rad * (c, s) and z/|z| = (c, s).
+HM_HD void box_muller(const U4& r, double* rad, double* c, double* s) {
+  const double u1 = u01(r.x, r.y), u2 = u01(r.z, r.w);
+  *rad = sqrt(-2.0 * log(u1));
+#ifdef __CUDA_ARCH__
+  sincospi(2.0 * u2, s, c);
+#else
+  sincos(6.283185307179586476925286766559 * u2, s, c);
+#endif
+}
+
+// n fp64 standard normals of stream (seed, kind, obj, t): pair k comes from draw d = 1 + k
+HM_HD void normals(uint64_t seed, int kind, uint64_t obj, uint32_t t, int n, double* z) {
+  for (int k = 0; 2 * k < n; ++k) {
+    double rad, c, s;
+    box_muller(stream(seed, kind, obj, t, 1u + (uint32_t)k), &rad, &c, &s);
+    z[2 * k] = rad * c;
+    if (2 * k + 1 < n) z[2 * k + 1] = rad * s;
+  }
+}
+
+}  // namespace hm
