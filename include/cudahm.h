@@ -71,7 +71,8 @@ typedef struct {
   int32_t  block_threads;        /* 0 = default; else 256, 512 or 1024                                      */
   int32_t  blocks_per_sm;        /* 0 = as many as fit; else an upper limit                                 */
   int32_t  reserved;             /* must be 0                                                               */
-  int64_t  max_trace_rows;       /* capacity of the on-device thinned theta trace (rows of dtheta doubles)   */
+  int64_t  max_trace_rows;       /* capacity of the on-device thinned theta trace (rows of dtheta doubles);
+                                    0 = keep no trace                                                        */
 } cudahm_config;
 
 typedef struct {
@@ -135,7 +136,7 @@ int cudahm_set_init(cudahm_sampler* s, const void* chi0_or_null, int chi0_on_dev
 
 /* Run n_iter more Gibbs iterations (resumable: continues from the current iteration index t).  Moments are
  * accumulated for t > burn_in, the trace takes theta whenever t > burn_in and (t - burn_in) % thin == 0.
- * CUDAHM_E_INVALID if the trace would overflow max_trace_rows. */
+ * CUDAHM_E_INVALID if the trace would overflow max_trace_rows (max_trace_rows == 0 keeps no trace at all). */
 int cudahm_run(cudahm_sampler* s, int64_t n_iter, int64_t burn_in, int32_t thin);
 
 /* One iteration through the non-persistent sweep + tail kernels with per-object taps (test instrument). */

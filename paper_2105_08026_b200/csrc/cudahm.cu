@@ -519,7 +519,7 @@ extern "C" int cudahm_run(cudahm_sampler* s, int64_t n_iter, int64_t burn_in, in
     const long long t1 = s->t_done + n_iter;
     const long long lo = std::max<long long>(s->t_done, burn_in);
     const long long rows = t1 > lo ? (t1 - burn_in) / thin - (lo - burn_in) / thin : 0;
-    if (s->h_iter->trace_rows + rows > s->cfg.max_trace_rows)
+    if (s->cfg.max_trace_rows > 0 && s->h_iter->trace_rows + rows > s->cfg.max_trace_rows)
       return fail(s, CUDAHM_E_INVALID, "theta trace would need %lld rows, capacity %lld", s->h_iter->trace_rows + rows,
                   (long long)s->cfg.max_trace_rows);
   }
@@ -548,7 +548,8 @@ extern "C" int cudahm_debug_step(cudahm_sampler* s, int64_t burn_in, int32_t thi
   if (s->cfg.theta_mode == CUDAHM_THETA_HOST)   // make the device copy current
     CU_TRY(s, cudaMemcpy(s->P.iter, s->h_iter, sizeof(Iter), cudaMemcpyHostToDevice));
   const long long t = s->h_iter->t;
-  if (t > burn_in && ((t - burn_in) % thin) == 0 && s->h_iter->trace_rows + 1 > s->cfg.max_trace_rows)
+  if (s->cfg.max_trace_rows > 0 && t > burn_in && ((t - burn_in) % thin) == 0 &&
+      s->h_iter->trace_rows + 1 > s->cfg.max_trace_rows)
     return fail(s, CUDAHM_E_INVALID, "theta trace is full");
   s->P.tail.burn_in = burn_in; s->P.tail.thin = thin;
   const size_t N = (size_t)s->P.N;

@@ -1,0 +1,202 @@
+"""GPU parity: the CUDA path (through the C ABI, include/cudahm.h) against the CPU oracle on the same seeded
+inputs, element by element.  Tolerances are BASELINE.json north_star's (tests/parity_util.py::TOL):
+per-object log-densities rel 1e-12 (fp64) / 1e-5 (fp32), population sum rel 1e-10, accept sequences identical
+except inside the near-tie band |log alpha - log u| < 1e-9 (counted)."""
+import numpy as np
+import pytest
+
+from parity_util import TOL, compare_step, compare_theta_step, make_pair, sync_gpu_to_oracle
+from paper_2105_08026_b200 import binding as B
+
+pytestmark = pytest.mark.gpu
+NO_TRACE = 10 ** 12   # burn-in beyond any iteration: tapped steps append nothing to the theta trace
+
+# (model, precision, alpha_*, N): sizes span several 16-byte vectors, several blocks and a ragged tail
+CASES = [
+    (B.M_NORMAL1D, B.F64, 0.44, 1000),
+    (B.M_THINNED_SCHECHTER1D, B.F64, 0.44, 4099),
+    (B.M_BINORMAL2D, B.F64, 0.234, 3001),
+    (B.M_LINREG_ME1D, B.F64, 0.44, 2050),
+    (B.M_NORMAL1D, B.F32_STATE_F64_REDUCE, 0.44, 4097),
+    (B.M_LINREG_ME1D, B.F32_STATE_F64_REDUCE, 0.44, 10007),
+]
+IDS = ["M0-f64", "M1-f64", "M2-f64", "M3-f64", "M0-f32", "M3-f32"]
+
+
+@pytest.mark.parametrize("model,precision,astar,n", CASES, ids=IDS)
+def test_single_step_fed_state(model, precision, astar, n):
+    """One iteration from identical state: every tap of SURVEY 8(c) protocol (i)."""
+    orc, gpu, _ = make_pair(model, n, seed=11 + model, precision=precision, astar=astar, block_threads=256)
+    st = sync_gpu_to_oracle(orc, gpu)
+    to, tg = orc.step(NO_TRACE, 1, taps=True), gpu.debug_step(NO_TRACE, 1)
+    nm = compare_step(to, tg, precision, st, what=f"model {model}")
+    compare_theta_step(to, tg, what=f"model {model}")
+    assert nm == 0 or precision != B.F64, "an fp64 near tie in the very first step is (almost surely) a bug"
+    if nm == 0:
+        assert to["accepted_theta"] == tg["accepted_theta"]
+
+
+@pytest.mark.parametrize("model,precision,astar,n", CASES, ids=IDS)
+def test_lockstep_trajectory(model, precision, astar, n):
+    """Protocol (ii): lock-step for 60 iterations with taps; accept sequences identical outside the tie band;
+    the GPU is re-fed the oracle's state after every iteration in fp32 (per-decision disagreement is expected
+    there) and only after a counted in-band divergence in fp64."""
+    orc, gpu, _ = make_pair(model, n, seed=21 + model, precision=precision, astar=astar, block_threads=256)
+    ties = 0
+    st = sync_gpu_to_oracle(orc, gpu)
+    for it in range(60):
+        to, tg = orc.step(NO_TRACE, 1, taps=True), gpu.debug_step(NO_TRACE, 1)
+        nm = compare_step(to, tg, precision, st, what=f"model {model} it {it}")
+        compare_theta_step(to, tg, what=f"model {model} it {it}", rel=1e-9 if precision == B.F64 else 1e-6)
+        ties += nm
+        if precision == B.F64 and nm == 0 and to["accepted_theta"] == tg["accepted_theta"]:
+            st = orc.get_state()
+            sg = gpu.get_state()
+            np.testing.assert_allclose(sg["chi"], st["chi"], rtol=1e-11, atol=1e-11)
+            np.testing.assert_allclose(sg["L"], st["L"], rtol=1e-10)
+            np.testing.assert_allclose(sg["theta"], st["theta"], rtol=1e-9, atol=1e-9)
+            np.testing.assert_allclose(sg["L_theta"], st["L_theta"], rtol=1e-8, atol=1e-12)
+            # keep the two strictly in lock step so rounding differences do not accumulate into a decision
+            gpu.set_state(st["chi"], st["L"], st["theta"], st["L_theta"], st["t"])
+        else:
+            st = sync_gpu_to_oracle(orc, gpu)
+    if precision == B.F64:
+        assert ties <= 1, f"{ties} near ties in {60 * n} fp64 decisions (expected ~1e-9 each)"
+    else:
+        assert ties <= 60 * n * 1e-3
+
+
+@pytest.mark.parametrize("mode", [B.THETA_HOST, B.THETA_GRAPH, B.THETA_DEVICE_TAIL], ids=["host", "graph", "tail"])
+@pytest.mark.parametrize("model,astar,n", [(B.M_NORMAL1D, 0.44, 1000), (B.M_THINNED_SCHECHTER1D, 0.44, 3000),
+                                             (B.M_BINORMAL2D, 0.234, 2000)], ids=["M0", "M1", "M2"])
+def test_free_running_matches_oracle(model, astar, n, mode):
+    """cudahm_run (no taps, no resync) for 120 iterations in every theta mode against oracle_run: same theta
+    trace, same chi / L, same moments, same counters.  (~1e5 decisions at ~1e-9 tie probability each.)"""
+    iters, burn, thin = 120, 20, 5
+    orc, gpu, _ = make_pair(model, n, seed=31 + model, astar=astar, theta_mode=mode, keep_moments=True,
+                            max_trace_rows=(iters - burn) // thin)
+    orc.run(iters, burn, thin)
+    gpu.run(iters, burn, thin, sync=True)
+    so, sg = orc.get_state(), gpu.get_state()
+    assert sg["t"] == so["t"] == iters
+    tro, trg = orc.get_theta_trace(), gpu.get_theta_trace()
+    assert trg.shape == tro.shape == ((iters - burn) // thin, gpu.dtheta)
+    np.testing.assert_allclose(trg, tro, rtol=1e-8, atol=1e-8)
+    np.testing.assert_allclose(sg["chi"], so["chi"], rtol=1e-9, atol=1e-9)
+    np.testing.assert_allclose(sg["L"], so["L"], rtol=1e-9)
+    np.testing.assert_allclose(sg["L_theta"], so["L_theta"], rtol=1e-7, atol=1e-12)
+    mo, vo, ko = orc.get_chi_moments()
+    mg, vg, kg = gpu.get_chi_moments()
+    assert kg == ko == iters - burn
+    np.testing.assert_allclose(mg, mo, rtol=1e-10, atol=1e-10)
+    np.testing.assert_allclose(vg, vo, rtol=1e-8, atol=1e-12)
+    stg, sto = gpu.get_stats(), orc.get_stats()
+    for k in ("iterations", "chi_accepts", "chi_proposals", "theta_accepts", "theta_proposals", "nonfinite",
+              "moment_samples", "trace_rows"):
+        assert stg[k] == sto[k], k
+    assert stg["gpu_launches"] > 0
+
+
+def test_theta_modes_agree():
+    """Same grid, same thread->object map, same reduction order in all three drivers.  GRAPH and DEVICE_TAIL run
+    the theta step with the same device code => identical bits.  HOST runs it with the host libm (exp, pow,
+    sincos differ from the device's by ulps), so it agrees to rounding, not bitwise."""
+    out = []
+    for mode in (B.THETA_HOST, B.THETA_GRAPH, B.THETA_DEVICE_TAIL):
+        _, gpu, _ = make_pair(B.M_THINNED_SCHECHTER1D, 5000, seed=5, theta_mode=mode, max_trace_rows=130,
+                              want_oracle=False)
+        gpu.run(130, 0, 1, sync=True)
+        s = gpu.get_state()
+        out.append((s["chi"], s["L"], s["theta"], s["L_theta"], gpu.get_theta_trace()))
+    for a, b in zip(out[1], out[2]):
+        assert np.array_equal(a, b)
+    for a, b in zip(out[0], out[2]):
+        np.testing.assert_allclose(a, b, rtol=1e-9, atol=1e-10)
+
+
+def test_resume_is_bit_exact():
+    """Counter-based streams: run(70) + run(50) == run(120), and get_state/set_state round-trips."""
+    _, g1, inp = make_pair(B.M_BINORMAL2D, 3000, seed=8, astar=0.234, max_trace_rows=120, want_oracle=False)
+    g1.run(120, 0, 1, sync=True)
+    _, g2, _ = make_pair(B.M_BINORMAL2D, 3000, seed=8, astar=0.234, max_trace_rows=120, inputs=inp, want_oracle=False)
+    g2.run(70, 0, 1)
+    g2.run(50, 0, 1, sync=True)
+    s1, s2 = g1.get_state(), g2.get_state()
+    for k in ("chi", "L", "theta", "L_theta"):
+        assert np.array_equal(s1[k], s2[k]), k
+    assert np.array_equal(g1.get_theta_trace(), g2.get_theta_trace())
+    _, g3, _ = make_pair(B.M_BINORMAL2D, 3000, seed=8, astar=0.234, max_trace_rows=120, inputs=inp, want_oracle=False)
+    g3.run(70, 0, 1, sync=True)
+    mid = g3.get_state()
+    _, g4, _ = make_pair(B.M_BINORMAL2D, 3000, seed=8, astar=0.234, max_trace_rows=120, inputs=inp, want_oracle=False)
+    g4.set_state(mid["chi"], mid["L"], mid["theta"], mid["L_theta"], mid["t"])
+    g4.run(50, 0, 1, sync=True)
+    s4 = g4.get_state()
+    for k in ("chi", "L", "theta", "L_theta"):
+        assert np.array_equal(s1[k], s4[k]), k
+
+
+@pytest.mark.parametrize("n", [0, 1, 2, 3, 31, 33, 1023, 1025])
+@pytest.mark.parametrize("precision", [B.F64, B.F32_STATE_F64_REDUCE], ids=["f64", "f32"])
+def test_ragged_and_degenerate_sizes(n, precision):
+    """Empty, single-object and ragged-tail populations (vector tails, partial warps)."""
+    orc, gpu, _ = make_pair(B.M_NORMAL1D, n, seed=3, precision=precision, astar=0.44, max_trace_rows=16)
+    if n > 0:
+        st = sync_gpu_to_oracle(orc, gpu)
+        to, tg = orc.step(taps=True), gpu.debug_step()
+        compare_step(to, tg, precision, st, what=f"N={n}")
+        sync_gpu_to_oracle(orc, gpu)
+    gpu.run(8, 0, 1, sync=True)
+    orc.run(8, 0, 1)
+    if precision == B.F64:
+        np.testing.assert_allclose(gpu.get_theta_trace()[-8:], orc.get_theta_trace()[-8:], rtol=1e-9, atol=1e-9)
+    assert gpu.get_stats()["iterations"] == orc.get_stats()["iterations"]
+
+
+def test_frozen_theta_conjugate_conditional():
+    """theta frozen: chi_i | theta, y_i ~ N((y/s^2 + mu/tau^2) v, v), v = 1/(1/s^2 + 1/tau^2) (closed form, P6):
+    the on-device moments must land on it, and the RAM scale on 2.4176 sd (P5)."""
+    from paper_2105_08026_b200 import synth
+    n, iters, burn = 4096, 6000, 1000
+    inp = synth.make_normal1d(n, 17)
+    th = np.array([0.1, np.log(0.8)])
+    _, gpu, _ = make_pair(B.M_NORMAL1D, n, seed=17, astar=0.44, inputs=inp, theta0=th, keep_moments=True,
+                          freeze_theta=True, want_oracle=False)
+    gpu.run(iters, burn, 1, sync=True)
+    y, s = inp["cols"]
+    tau2 = np.exp(2 * th[1])
+    v = 1.0 / (1.0 / s ** 2 + 1.0 / tau2)
+    m = (y / s ** 2 + th[0] / tau2) * v
+    mean, var, k = gpu.get_chi_moments()
+    assert k == iters - burn
+    zs = (mean[0] - m) / np.sqrt(v)
+    # ESS ~ k/4.5 for a tuned 1-D random-walk Metropolis: sd of the mean ~ 0.03 sd units
+    assert np.abs(zs).max() < 0.2 and abs(zs.mean()) < 0.005
+    assert abs(np.mean(var[0] / v) - 1.0) < 0.02
+    L = gpu.get_state()["L"][0]
+    assert abs(np.mean(L / np.sqrt(v)) - 2.41758) < 0.06
+    st = gpu.get_stats()
+    assert abs(st["chi_accepts"] / st["chi_proposals"] - 0.44) < 0.01
+
+
+def test_config0_posterior_against_oracle_and_closed_form():
+    """BASELINE config 0 as stated (N=1000, 2000 iterations, 500 burn-in, seed 0): GPU and oracle theta
+    posteriors agree within 4 MCSE (they are in fact the same chain to rounding)."""
+    from mcmc_util import mean_and_var_with_mcse
+    from paper_2105_08026_b200 import synth
+    c = synth.CONFIGS["C0"]
+    inp = synth.make_inputs("C0")
+    orc, gpu, _ = make_pair(c.model, c.n_objects, seed=c.seed, astar=c.target_accept_chi, inputs=inp,
+                            keep_moments=True, max_trace_rows=c.n_iter - c.burn_in)
+    orc.run(c.n_iter, c.burn_in, c.thin)
+    gpu.run(c.n_iter, c.burn_in, c.thin, sync=True)
+    tg, to = gpu.get_theta_trace(), orc.get_theta_trace()
+    assert tg.shape == to.shape == (1500, 2)
+    mg, seg, vg, sevg = mean_and_var_with_mcse(tg)
+    mo, seo, vo, sevo = mean_and_var_with_mcse(to)
+    assert np.all(np.abs(mg - mo) <= 4 * np.hypot(seg, seo))
+    assert np.all(np.abs(vg - vo) <= 4 * np.hypot(sevg, sevo))
+    # closed form: mu | tau, y ~ N(sum w y / sum w, 1/sum w), w = 1/(sigma^2 + tau^2), at the posterior-mean tau
+    y, s = inp["cols"]
+    w = 1.0 / (s ** 2 + np.exp(2 * mg[1]))
+    assert abs(mg[0] - (w * y).sum() / w.sum()) <= 4 * seg[0] + 0.01
