@@ -20,10 +20,11 @@ namespace {
 thread_local std::string g_err;
 
 struct Layout {
-  size_t chi, L, data, mom_mean, mom_M2, mom_var, slots, bar, iter, trace, totals, qx, qex, qW, total;
+  size_t chi, L, data, mom_mean, mom_M2, mom_var, slots, mbox, blk_cnt, iter, trace, totals, qx, qex, qW, total;
 };
 
-constexpr int MAX_BLOCKS = 148 * 8 * 2;   // upper bound on the cooperative grid (slots capacity)
+constexpr int MAX_BLOCKS = 148 * 8 * 2;   // upper bound on the grid (slots capacity)
+constexpr int MAX_PGRID = 320;            // upper bound on the persistent grid (mailboxes grow with its square)
 
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
@@ -91,6 +92,8 @@ struct cudahm_sampler {
   bool host_iter_valid = false;     // THETA_HOST: h_iter is authoritative between runs
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   bool timed = false;
+  unsigned epoch = 1;               // next mailbox epoch of the persistent kernel
+  double h_lp_prop_before = 0.0;    // log prior at theta' of the iteration debug_step is about to decide
   // CUDA-graph cache (THETA_GRAPH)
   cudaGraphExec_t gexec = nullptr;
   long long g_burn = -1; int g_thin = -1; int g_iters = 0;
@@ -144,8 +147,9 @@ Layout make_layout(const cudahm_config& c, int p, int ncols, int dtheta) {
   l.data = take((size_t)ncols * Npad * ts);
   const size_t mom = c.keep_chi_moments ? (size_t)p * Npad * 8 : 0;
   l.mom_mean = take(mom); l.mom_M2 = take(mom); l.mom_var = take(mom);
-  l.slots = take((size_t)2 * MAX_BLOCKS * NPART * 8);
-  l.bar = take(256);
+  l.slots = take((size_t)MAX_BLOCKS * NPART * 8);
+  l.mbox = take((size_t)2 * MAX_PGRID * MAX_PGRID * 4 * 8);
+  l.blk_cnt = take((size_t)MAX_BLOCKS * 2 * 8);
   l.iter = take(sizeof(Iter));
   l.trace = take((size_t)c.max_trace_rows * dtheta * 8);
   l.totals = take(NPART * 8);
@@ -209,13 +213,15 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
   long long need = (cfg->n_objects + (long long)s->vec * block - 1) / ((long long)s->vec * block);
   s->grid = (int)std::max(1LL, std::min<long long>((long long)sms * per_sm, need));
   s->grid = std::min(s->grid, MAX_BLOCKS);
+  if (cfg->theta_mode == CUDAHM_THETA_DEVICE_TAIL && s->grid > MAX_PGRID) s->grid = std::max(1, MAX_PGRID / sms) * sms;
 
   Params& P = s->P;
   P.N = cfg->n_objects; P.Npad = (cfg->n_objects + 31) / 32 * 32;
   P.chi = s->ws + lay.chi; P.L = s->ws + lay.L; P.data = s->ws + lay.data;
   P.mom_mean = cfg->keep_chi_moments ? (double*)(s->ws + lay.mom_mean) : nullptr;
   P.mom_M2 = cfg->keep_chi_moments ? (double*)(s->ws + lay.mom_M2) : nullptr;
-  P.slots = (double*)(s->ws + lay.slots); P.bar = (unsigned*)(s->ws + lay.bar);
+  P.slots = (double*)(s->ws + lay.slots); P.mbox = (unsigned long long*)(s->ws + lay.mbox);
+  P.blk_cnt = (unsigned long long*)(s->ws + lay.blk_cnt);
   P.iter = (Iter*)(s->ws + lay.iter); P.trace = (double*)(s->ws + lay.trace); P.totals = (double*)(s->ws + lay.totals);
   P.qx = (double*)(s->ws + lay.qx); P.qex = (double*)(s->ws + lay.qex); P.qW = (double*)(s->ws + lay.qW);
   for (int k = 0; k < 8; ++k) P.mc[k] = 0.0;
@@ -403,6 +409,7 @@ extern "C" int cudahm_set_init(cudahm_sampler* s, const void* chi0, int chi0_on_
   }
   if (s->lay.trace != s->lay.totals)
     CU_TRY(s, cudaMemsetAsync(s->P.trace, 0, (size_t)s->cfg.max_trace_rows * s->dtheta * 8, s->stream));
+  CU_TRY(s, cudaMemsetAsync(s->P.blk_cnt, 0, (size_t)MAX_BLOCKS * 2 * 8, s->stream));
   Iter raw;
   std::memset(&raw, 0, sizeof raw);
   for (int r = 0; r < s->dtheta; ++r) raw.theta[r] = theta0[r];
@@ -420,12 +427,13 @@ namespace {
 
 // THETA_DEVICE_TAIL: cooperative persistent launches of at most max_it iterations each
 int run_device_tail(cudahm_sampler* s, long long n_iter) {
-  const long long max_it = (long long)(0x7fffffffLL / std::max(1, s->grid));
+  const long long max_it = 0x3fffffffLL;
   while (n_iter > 0) {
     long long k = std::min(n_iter, max_it);
-    CU_TRY(s, cudaMemsetAsync(s->P.bar, 0, sizeof(unsigned), s->stream));
     Params P = s->P;
-    void* args[] = {&P, &k};
+    unsigned epoch0 = s->epoch;            // epochs never repeat over the sampler's lifetime (0 = never written)
+    s->epoch += (unsigned)k;
+    void* args[] = {&P, &k, &epoch0};
     int rc = launch(s, s->ks.persistent, s->grid, s->block, args, true);
     if (rc) return rc;
     n_iter -= k;
@@ -438,9 +446,9 @@ int enqueue_graph_iteration(cudahm_sampler* s) {
   void* a1[] = {&P};
   int rc = launch(s, s->ks.sweep, s->grid, s->block, a1, false);
   if (rc) return rc;
-  int nb = s->grid, flags = TAIL_REDUCE | TAIL_DECIDE | TAIL_PREPARE;
+  int nb = s->grid, flags = TAIL_DECIDE;
   void* a2[] = {&P, &nb, &flags};
-  return launch(s, (const void*)k_tail, 1, 32, a2, false);
+  return launch(s, (const void*)k_tail, 1, TAIL_THREADS, a2, false);
 }
 
 // THETA_GRAPH: {sweep, tail} x GRAPH_ITERS captured once per (burn_in, thin), replayed; remainder launched directly
@@ -490,7 +498,7 @@ int run_host(cudahm_sampler* s, long long n_iter) {
     if (rc) return rc;
     int nb = s->grid, flags = TAIL_REDUCE;
     void* a2[] = {&P, &nb, &flags};
-    rc = launch(s, (const void*)k_tail, 1, 32, a2, false);
+    rc = launch(s, (const void*)k_tail, 1, TAIL_THREADS, a2, false);
     if (rc) return rc;
     CU_TRY(s, cudaMemcpyAsync(s->h_totals, s->P.totals, NPART * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
     CU_TRY(s, cudaStreamSynchronize(s->stream));
@@ -548,6 +556,7 @@ extern "C" int cudahm_debug_step(cudahm_sampler* s, int64_t burn_in, int32_t thi
   if (s->cfg.theta_mode == CUDAHM_THETA_HOST)   // make the device copy current
     CU_TRY(s, cudaMemcpy(s->P.iter, s->h_iter, sizeof(Iter), cudaMemcpyHostToDevice));
   const long long t = s->h_iter->t;
+  s->h_lp_prop_before = s->h_iter->lp_prop;
   if (s->cfg.max_trace_rows > 0 && t > burn_in && ((t - burn_in) % thin) == 0 &&
       s->h_iter->trace_rows + 1 > s->cfg.max_trace_rows)
     return fail(s, CUDAHM_E_INVALID, "theta trace is full");
@@ -569,17 +578,17 @@ extern "C" int cudahm_debug_step(cudahm_sampler* s, int64_t burn_in, int32_t thi
   P.taps.accepted = ibuf;
   void* a1[] = {&P};
   rc = launch(s, s->ks.sweep_tap, s->grid, s->block, a1, false);
-  int nb = s->grid, flags = TAIL_REDUCE | TAIL_DECIDE;
+  int nb = s->grid, flags = TAIL_REDUCE | TAIL_DECIDE;     // the device tail decides t and prepares t + 1
   void* a2[] = {&P, &nb, &flags};
-  if (!rc) rc = launch(s, (const void*)k_tail, 1, 32, a2, false);
+  if (!rc) rc = launch(s, (const void*)k_tail, 1, TAIL_THREADS, a2, false);
   cudaError_t e = cudaSuccess;
   if (!rc) e = cudaMemcpyAsync(s->h_iter, s->P.iter, sizeof(Iter), cudaMemcpyDeviceToHost, s->stream);
   if (!rc && e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
   if (!rc && e == cudaSuccess) {
     const Iter& it = *s->h_iter;
-    for (int r = 0; r < 8; ++r) taps->theta_prop[r] = r < s->dtheta ? it.thetaP[r] : 0.0;
+    for (int r = 0; r < 8; ++r) taps->theta_prop[r] = r < s->dtheta ? it.tap_thetaP[r] : 0.0;
     taps->S = it.S; taps->Delta = it.Delta; taps->T_cur = it.T_cur_used; taps->T_prop = it.T_prop;
-    taps->lp_cur = it.lp_cur_used; taps->lp_prop = it.lp_prop; taps->log_r = it.log_r;
+    taps->lp_cur = it.lp_cur_used; taps->lp_prop = s->h_lp_prop_before; taps->log_r = it.log_r;
     taps->alpha_theta = it.alpha_theta; taps->u_theta = it.u_theta; taps->accepted_theta = it.accepted_theta;
     struct { double* dst; const double* src; size_t n; } cp[] = {
         {taps->chi_prop, P.taps.chi_prop, (size_t)s->p * N}, {taps->L_new, P.taps.L_new, (size_t)s->ntri * N},
@@ -588,21 +597,6 @@ extern "C" int cudahm_debug_step(cudahm_sampler* s, int64_t burn_in, int32_t thi
     for (auto& c : cp)
       if (c.dst && c.n && e == cudaSuccess) e = cudaMemcpy(c.dst, c.src, c.n * sizeof(double), cudaMemcpyDeviceToHost);
     if (taps->accepted && N && e == cudaSuccess) e = cudaMemcpy(taps->accepted, ibuf, N * sizeof(int), cudaMemcpyDeviceToHost);
-  }
-  // prepare the next iteration (device prepares in the device modes, the host in host mode)
-  if (!rc && e == cudaSuccess) {
-    if (s->cfg.theta_mode == CUDAHM_THETA_HOST) {
-      prepare_iteration(*s->h_iter, s->P.tail, s->h_iter->t + 1);
-      e = cudaMemcpy(s->P.iter, s->h_iter, sizeof(Iter), cudaMemcpyHostToDevice);
-    } else {
-      // the tail kernel decided without preparing: it.t is still the decided iteration
-      Iter tmp = *s->h_iter; tmp.t += 1;
-      e = cudaMemcpy(s->P.iter, &tmp, sizeof(Iter), cudaMemcpyHostToDevice);
-      int fl = TAIL_PREPARE;
-      void* a3[] = {&P, &nb, &fl};
-      if (e == cudaSuccess) rc = launch(s, (const void*)k_tail, 1, 32, a3, false);
-      if (!rc) e = cudaStreamSynchronize(s->stream);
-    }
   }
   if (dbuf) cudaFree(dbuf);
   if (ibuf) cudaFree(ibuf);
@@ -656,9 +650,13 @@ extern "C" int cudahm_get_stats(cudahm_sampler* s, cudahm_stats* out) {
   int rc = fetch_iter(s); if (rc) return rc;
   const Iter& it = *s->h_iter;
   out->iterations = it.t - 1;
-  out->chi_accepts = (int64_t)it.chi_acc; out->chi_proposals = (it.t - 1) * s->P.N;
+  std::vector<unsigned long long> bc((size_t)2 * MAX_BLOCKS);
+  CU_TRY(s, cudaMemcpy(bc.data(), s->P.blk_cnt, bc.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+  unsigned long long acc = it.chi_acc, nonf = it.nonfinite;
+  for (int b = 0; b < MAX_BLOCKS; ++b) { acc += bc[2 * b]; nonf += bc[2 * b + 1]; }
+  out->chi_accepts = (int64_t)acc; out->chi_proposals = (it.t - 1) * s->P.N;
   out->theta_accepts = (int64_t)it.theta_acc; out->theta_proposals = (int64_t)it.theta_prop_n;
-  out->nonfinite = (int64_t)it.nonfinite; out->moment_samples = it.mom_count; out->trace_rows = it.trace_rows;
+  out->nonfinite = (int64_t)nonf; out->moment_samples = it.mom_count; out->trace_rows = it.trace_rows;
   if (s->timed) {
     float ms = 0.f;
     if (cudaEventElapsedTime(&ms, s->ev0, s->ev1) == cudaSuccess) out->last_run_ms = ms;

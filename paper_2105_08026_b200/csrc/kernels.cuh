@@ -22,8 +22,9 @@ struct Params {
   void* data;                    // T [ncols][Npad], Gaussian error columns stored as 1/(2 sigma^2)
   double* mom_mean;              // [p][Npad]   Welford mean
   double* mom_M2;                // [p][Npad]   Welford sum of squared deviations
-  double* slots;                 // [2][max_blocks][NPART] per-block partials, double-buffered by iteration parity
-  unsigned* bar;                 // grid barrier arrival counter
+  double* slots;                 // [max_blocks][NPART] per-block partials of k_sweep (THETA_GRAPH / HOST / debug_step)
+  unsigned long long* mbox;      // [2][G][2][G][2] flagged mailboxes of k_persistent (G = its grid <= MAX_PGRID)
+  unsigned long long* blk_cnt;   // [max_blocks][2] accepted / non-finite plate proposals counted by k_persistent
   Iter* iter;                    // prepared iteration state (global copy)
   double* trace;                 // [max_trace_rows][dtheta]
   double* totals;                // [NPART] reduced totals (host mode reads them)
@@ -101,7 +102,7 @@ __device__ __forceinline__ void sweep(const Params& P, const Iter& it, double* p
   T mcT[7];
 #pragma unroll
   for (int j = 0; j < 7; ++j) mcT[j] = (T)P.mc[j];
-  const T eta = (T)it.eta, astar = (T)P.astar_chi;
+  const T eta = (T)it.dr[it.t % 3].eta, astar = (T)P.astar_chi;
   const bool do_mom = P.tail.keep_moments && it.t > P.tail.burn_in;
   const double inv_k = 1.0 / (double)(it.mom_count + 1);
 
@@ -209,59 +210,142 @@ __device__ __forceinline__ void sweep(const Params& P, const Iter& it, double* p
   part[0] = accS; part[1] = accD; part[2] = tq; part[3] = nacc; part[4] = nnan;
 }
 
-// Deterministic block reduction: shuffle tree inside each warp, then warp 0 over the per-warp results.
-// Returns the block totals in part[] of thread 0.  red: shared [32][NPART].
-__device__ __forceinline__ void block_reduce(double* part, double (*red)[NPART]) {
+// Deterministic block reduction of NQ quantities: shuffle tree inside each warp, then warp 0 over the per-warp
+// results.  Returns the block totals in v[] of thread 0.  red: shared [32][NPART].
+template <int NQ>
+__device__ __forceinline__ void block_reduce(double* v, double (*red)[NPART]) {
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
 #pragma unroll
-  for (int q = 0; q < NPART; ++q) {
+  for (int o = 16; o > 0; o >>= 1) {
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) part[q] += __shfl_down_sync(0xffffffffu, part[q], o);
+    for (int q = 0; q < NQ; ++q) v[q] += __shfl_down_sync(0xffffffffu, v[q], o);
   }
   if (lane == 0) {
 #pragma unroll
-    for (int q = 0; q < NPART; ++q) red[wid][q] = part[q];
+    for (int q = 0; q < NQ; ++q) red[wid][q] = v[q];
   }
   __syncthreads();
   if (wid == 0) {
+    double w[NQ];
 #pragma unroll
-    for (int q = 0; q < NPART; ++q) {
-      double v = lane < nw ? red[lane][q] : 0.0;
+    for (int q = 0; q < NQ; ++q) w[q] = lane < nw ? red[lane][q] : 0.0;
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
-      part[q] = v;
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+      for (int q = 0; q < NQ; ++q) w[q] += __shfl_down_sync(0xffffffffu, w[q], o);
     }
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) v[q] = w[q];
   }
 }
 
-// Fixed-order sum of the per-block slots by warp 0: lane l adds blocks l, l+32, ... in order, then a tree.
-__device__ __forceinline__ void slots_reduce(const double* slots, int nblocks, double* tot) {
-  const int lane = threadIdx.x & 31;
-  double v[NPART];
+// Same tree, but EVERY warp redoes the second stage, so every thread of the block ends up with the totals
+// (no broadcast barrier before the mailbox push).
+template <int NQ>
+__device__ __forceinline__ void block_reduce_all(double* v, double (*red)[NPART]) {
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
 #pragma unroll
-  for (int q = 0; q < NPART; ++q) v[q] = 0.0;
-  for (int g = lane; g < nblocks; g += 32) {
+  for (int o = 16; o > 0; o >>= 1) {
 #pragma unroll
-    for (int q = 0; q < NPART; ++q) v[q] += __ldcg(slots + (size_t)g * NPART + q);
+    for (int q = 0; q < NQ; ++q) v[q] += __shfl_down_sync(0xffffffffu, v[q], o);
   }
+  if (lane == 0) {
 #pragma unroll
-  for (int q = 0; q < NPART; ++q) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v[q] += __shfl_down_sync(0xffffffffu, v[q], o);
-    tot[q] = v[q];
-  }
-}
-
-// Grid barrier for the co-resident (cooperative) grid: one release-add per block, one acquire-poll.
-__device__ __forceinline__ void grid_barrier(unsigned* bar, unsigned target) {
-  if (threadIdx.x == 0) {
-    asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(bar) : "memory");
-    unsigned v;
-    do {
-      asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
-    } while (v < target);
+    for (int q = 0; q < NQ; ++q) red[wid][q] = v[q];
   }
   __syncthreads();
+#pragma unroll
+  for (int q = 0; q < NQ; ++q) v[q] = lane < nw ? red[lane][q] : 0.0;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) v[q] += __shfl_down_sync(0xffffffffu, v[q], o);
+  }
+#pragma unroll
+  for (int q = 0; q < NQ; ++q) v[q] = __shfl_sync(0xffffffffu, v[q], 0);
+}
+
+// Fixed-order sum over blocks by warp 0: lane l adds blocks l, l+32, ... in order, then a shuffle tree; the
+// result is broadcast to every lane.  Both slot formats below use exactly this order, so the persistent
+// kernel and the k_sweep + k_tail pair produce the same bits.
+template <int NQ>
+__device__ __forceinline__ void lanes_to_total(double* v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) v[q] += __shfl_down_sync(0xffffffffu, v[q], o);
+  }
+#pragma unroll
+  for (int q = 0; q < NQ; ++q) v[q] = __shfl_sync(0xffffffffu, v[q], 0);
+}
+
+// plain slots [nblocks][NPART] written by k_sweep (a kernel boundary orders them)
+__device__ __forceinline__ void slots_reduce(const double* slots, int nblocks, double* tot) {
+  const int lane = threadIdx.x & 31;
+#pragma unroll
+  for (int q = 0; q < NPART; ++q) tot[q] = 0.0;
+  for (int g = lane; g < nblocks; g += 32) {
+#pragma unroll
+    for (int q = 0; q < NPART; ++q) tot[q] += __ldcg(slots + (size_t)g * NPART + q);
+  }
+  lanes_to_total<NPART>(tot);
+}
+
+// Per-iteration exchange of the persistent kernel: the grid-wide reduction AND the barrier in one round trip.
+// Every block has a private mailbox with one slot per block; a block PUSHES its two partials (Delta, Tq) into
+// its slot of every mailbox (thread r writes to reader r: one 16-byte store per thread and value), and warp 0
+// of a block polls only its own mailbox.  No line is ever polled by more than one SM, so nothing queues at L2
+// (an all-read-all layout measured 4 us from last publish to visibility; profiles/r01b).  A slot holds, per
+// value, two 8-byte words {epoch << 32 | 32 data bits}: an 8-byte store is single-copy atomic, so a reader that
+// sees the right epoch in a word has that word's data -- no fence, no arrival counter, no second read.  Mailboxes
+// alternate by iteration parity: a block can be at most one iteration ahead of the slowest reader (it needs
+// everybody's slot of iteration k to get past k).  Epochs increase over the sampler's lifetime.
+//   mbox layout: [parity][reader][value 0..1][writer][2 words]
+__device__ __forceinline__ void mbox_push(unsigned long long* mbox_parity, int G, int writer, unsigned epoch, double a, double b) {
+  const unsigned long long e = (unsigned long long)epoch << 32;
+  const unsigned long long ua = (unsigned long long)__double_as_longlong(a), ub = (unsigned long long)__double_as_longlong(b);
+  const unsigned long long a0 = e | (ua & 0xffffffffull), a1 = e | (ua >> 32), b0 = e | (ub & 0xffffffffull), b1 = e | (ub >> 32);
+  for (int r = threadIdx.x; r < G; r += blockDim.x) {
+    unsigned long long* box = mbox_parity + (size_t)r * 4 * G;
+    asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(box + 2 * writer), "l"(a0), "l"(a1) : "memory");
+    asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(box + 2 * G + 2 * writer), "l"(b0), "l"(b1) : "memory");
+  }
+}
+// Collect (warp 0): lane l owns writers l, l+32, ...; up to LL_BATCH of them are polled TOGETHER (independent
+// loads in flight: one L2 round trip once everything has arrived), then added in ascending order.
+constexpr int LL_BATCH = 5;   // ceil(148 / 32): the whole one-block-per-SM grid in one batch
+__device__ __forceinline__ void mbox_collect(const unsigned long long* box, int G, unsigned epoch, double* tot2) {
+  const int lane = threadIdx.x & 31;
+  tot2[0] = 0.0; tot2[1] = 0.0;
+  for (int g0 = lane; g0 < G; g0 += 32 * LL_BATCH) {
+    unsigned long long w[LL_BATCH][4];
+    bool ok;
+    do {
+      ok = true;
+#pragma unroll
+      for (int j = 0; j < LL_BATCH; ++j) {
+        const int g = g0 + 32 * j;
+        if (g < G) {
+          asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(w[j][0]), "=l"(w[j][1]) : "l"(box + 2 * g) : "memory");
+          asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(w[j][2]), "=l"(w[j][3]) : "l"(box + 2 * G + 2 * g) : "memory");
+        }
+      }
+#pragma unroll
+      for (int j = 0; j < LL_BATCH; ++j) {
+        if (g0 + 32 * j < G)
+          ok = ok && (unsigned)(w[j][0] >> 32) == epoch && (unsigned)(w[j][1] >> 32) == epoch &&
+               (unsigned)(w[j][2] >> 32) == epoch && (unsigned)(w[j][3] >> 32) == epoch;
+      }
+    } while (!ok);
+#pragma unroll
+    for (int j = 0; j < LL_BATCH; ++j) {
+      if (g0 + 32 * j < G) {
+        tot2[0] += __longlong_as_double((long long)((w[j][0] & 0xffffffffull) | (w[j][1] << 32)));
+        tot2[1] += __longlong_as_double((long long)((w[j][2] & 0xffffffffull) | (w[j][3] << 32)));
+      }
+    }
+  }
+  lanes_to_total<2>(tot2);
 }
 
 __device__ __forceinline__ void copy_iter(Iter* dst, const Iter* src) {
@@ -273,39 +357,70 @@ __device__ __forceinline__ void copy_iter(Iter* dst, const Iter* src) {
 static_assert(sizeof(Iter) % sizeof(double) == 0, "Iter is copied as doubles");
 
 // ---------------------------------------------------------------------------------------------------
-// THETA_DEVICE_TAIL: the whole Gibbs loop in one cooperative launch.  Per iteration: sweep -> per-block
-// slot -> ONE grid barrier -> every block reduces all slots in the same fixed order and thread 0 takes the
-// identical theta decision (no second barrier; slots are double-buffered by iteration parity so a fast
-// block's iteration t+1 write cannot race a slow block's iteration t read).
+// THETA_DEVICE_TAIL: the whole Gibbs loop in one cooperative launch (co-residency of all blocks is what the
+// flag exchange needs).  Per iteration: sweep -> block partials -> flagged slot -> warp 0 of EVERY block collects
+// all slots in the same fixed order -> block-parallel theta tail (identical in every block) -> next sweep.
+// One grid-wide round trip per iteration.  Accept / non-finite counters stay in registers until the launch ends.
 template <int MODEL, class T, int BLOCK>
-__global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const long long n_iter) {
+__global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const long long n_iter, const unsigned epoch0) {
   __shared__ Iter it;
   __shared__ double red[32][NPART];
   copy_iter(&it, P.iter);
   __syncthreads();
   const int G = (int)gridDim.x;
+  double cnt[2] = {0.0, 0.0};
+#ifdef HM_PHASE_TIMING
+  long long ph[5] = {0, 0, 0, 0, 0};
+#define HM_STAMP(i) { const long long now_ = clock64(); ph[i] += now_ - last_; last_ = now_; }
+#else
+#define HM_STAMP(i)
+#endif
   for (long long k = 0; k < n_iter; ++k) {
+#ifdef HM_PHASE_TIMING
+    long long last_ = clock64();
+    unsigned long long g0_, g1_, g2_, g3_;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g0_));
+#endif
     double part[NPART];
     sweep<MODEL, T, false>(P, it, part);
-    block_reduce(part, red);
-    double* slots = P.slots + (size_t)(k & 1) * P.max_blocks * NPART;
-    if (threadIdx.x == 0) {
-#pragma unroll
-      for (int q = 0; q < NPART; ++q) __stcg(slots + (size_t)blockIdx.x * NPART + q, part[q]);
-    }
-    grid_barrier(P.bar, (unsigned)(k + 1) * (unsigned)G);
+    HM_STAMP(0)
+    cnt[0] += part[3]; cnt[1] += part[4];
+    double dq[2] = {part[1], part[2]};
+    block_reduce_all<2>(dq, red);
+    unsigned long long* mb = P.mbox + (size_t)(k & 1) * 4 * G * G;
+    const unsigned epoch = epoch0 + (unsigned)k;
+    mbox_push(mb, G, (int)blockIdx.x, epoch, dq[0], dq[1]);
+    HM_STAMP(1)
+#ifdef HM_PHASE_TIMING
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1_));
+#endif
+    double tot[NPART] = {0.0, 0.0, 0.0, 0.0, 0.0};
     if (threadIdx.x < 32) {
-      double tot[NPART];
-      slots_reduce(slots, G, tot);
-      if (threadIdx.x == 0) {
-        tail_decide(it, P.tail, tot);
-        if (blockIdx.x == 0 && it.trace_write) {
-          for (int j = 0; j < P.tail.dtheta; ++j) P.trace[(it.trace_rows - 1) * P.tail.dtheta + j] = it.theta[j];
-        }
-        prepare_iteration(it, P.tail, it.t + 1);
-      }
+      double t2[2];
+      mbox_collect(mb + (size_t)blockIdx.x * 4 * G, G, epoch, t2);
+      tot[1] = t2[0]; tot[2] = t2[1];
     }
-    __syncthreads();
+    HM_STAMP(2)
+#ifdef HM_PHASE_TIMING
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g2_));
+#endif
+    tail_block(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr);
+    HM_STAMP(3)
+#ifdef HM_PHASE_TIMING
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g3_));
+    if (threadIdx.x == 0 && k == n_iter - 2)
+      printf("GT %d %llu %llu %llu %llu\n", (int)blockIdx.x, g0_, g1_, g2_, g3_);
+#endif
+  }
+#ifdef HM_PHASE_TIMING
+  if (threadIdx.x == 0 && (blockIdx.x == 0 || blockIdx.x == gridDim.x - 1))
+    printf("block %d: cycles/iter sweep %.0f reduce+publish %.0f collect %.0f tail %.0f\n", (int)blockIdx.x,
+           (double)ph[0] / n_iter, (double)ph[1] / n_iter, (double)ph[2] / n_iter, (double)ph[3] / n_iter);
+#endif
+  block_reduce<2>(cnt, red);
+  if (threadIdx.x == 0) {
+    P.blk_cnt[2 * blockIdx.x] += (unsigned long long)cnt[0];
+    P.blk_cnt[2 * blockIdx.x + 1] += (unsigned long long)cnt[1];
   }
   if (blockIdx.x == 0) copy_iter(P.iter, &it);
 }
@@ -319,38 +434,33 @@ __global__ void __launch_bounds__(BLOCK, 1) k_sweep(const Params P) {
   __syncthreads();
   double part[NPART];
   sweep<MODEL, T, TAP>(P, it, part);
-  block_reduce(part, red);
+  block_reduce<NPART>(part, red);
   if (threadIdx.x == 0) {
 #pragma unroll
     for (int q = 0; q < NPART; ++q) P.slots[(size_t)blockIdx.x * NPART + q] = part[q];
   }
 }
 
-// 1-warp tail: reduce the slots; optionally decide; optionally prepare the next iteration.
-enum : int { TAIL_REDUCE = 1, TAIL_DECIDE = 2, TAIL_PREPARE = 4 };
-__global__ void __launch_bounds__(32, 1) k_tail(const Params P, const int nblocks, const int flags) {
+// Tail kernel: reduce the slots (TAIL_REDUCE: also publish the totals for the host); TAIL_DECIDE: the
+// block-parallel theta tail, which decides iteration t and prepares t + 1.
+enum : int { TAIL_REDUCE = 1, TAIL_DECIDE = 2 };
+constexpr int TAIL_THREADS = 128;
+__global__ void __launch_bounds__(TAIL_THREADS, 1) k_tail(const Params P, const int nblocks, const int flags) {
   __shared__ Iter it;
   copy_iter(&it, P.iter);
-  __syncwarp();
-  double tot[NPART];
-  if (flags & TAIL_REDUCE) {
+  __syncthreads();
+  double tot[NPART] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  if (threadIdx.x < 32) {
     slots_reduce(P.slots, nblocks, tot);
-    if (threadIdx.x == 0) {
+    if ((flags & TAIL_REDUCE) && threadIdx.x == 0) {
 #pragma unroll
       for (int q = 0; q < NPART; ++q) P.totals[q] = tot[q];
     }
   }
-  if (threadIdx.x == 0) {
-    if (flags & TAIL_DECIDE) {
-      tail_decide(it, P.tail, tot);
-      if (it.trace_write) {
-        for (int j = 0; j < P.tail.dtheta; ++j) P.trace[(it.trace_rows - 1) * P.tail.dtheta + j] = it.theta[j];
-      }
-    }
-    if (flags & TAIL_PREPARE) prepare_iteration(it, P.tail, (flags & TAIL_DECIDE) ? it.t + 1 : it.t);
+  if (flags & TAIL_DECIDE) {
+    tail_block(it, P.tail, tot, P.trace);
+    copy_iter(P.iter, &it);
   }
-  __syncwarp();
-  if (flags & (TAIL_DECIDE | TAIL_PREPARE)) copy_iter(P.iter, &it);
 }
 
 // After set_init / set_state: derive kc, log prior and T(theta) for the uploaded theta, then prepare it.t.
@@ -365,11 +475,11 @@ __global__ void __launch_bounds__(256, 1) k_init_iter(const Params P) {
     for (int k = threadIdx.x; k < NQUAD; k += blockDim.x)
       part[2] += P.qW[k] * exp(kc.v[0] * (P.qx[k] - kc.v[1]) - P.qex[k] * kc.v[3]);
   }
-  block_reduce(part, red);
+  block_reduce<NPART>(part, red);
   if (threadIdx.x == 0) {
     it.kc = kc;
     it.lp_cur = log_prior(P.tail.model, it.theta);
-    it.T_cur = (P.tail.model == M_THINNED_SCHECHTER1D) ? -exp(kc.v[2]) * part[2] : 0.0;
+    it.T_cur = (P.tail.model == M_THINNED_SCHECHTER1D) ? -kc.v[4] * part[2] : 0.0;
     prepare_iteration(it, P.tail, it.t);
   }
   __syncthreads();

@@ -37,27 +37,33 @@ inline bool model_dims(int model, int* p, int* dtheta, int* ncols, int* nconsts)
 // theta-derived constants, fp64
 struct ThetaK { double v[8]; };
 
+// theta_consts in three independent parts (disjoint entries of k) so that the block-parallel tail can give each
+// part to its own warp; part 0 carries the bulk, parts 1 and 2 only exist for M2's cosh/log and tanh.
+HM_HD void theta_consts_part(int model, int part, const double* th, ThetaK& k) {
+  switch (model) {
+    case M_NORMAL1D:            // (mu, lambda): f = -lambda - (chi - mu)^2 * [e^(-2 lambda)/2]
+      if (part == 0) { k.v[0] = th[0]; k.v[1] = th[1]; k.v[2] = 0.5 * exp(-2.0 * th[1]); }
+      break;
+    case M_LINREG_ME1D:         // (a, b, lambda): f = -lambda - (chi - a - b z)^2 * [e^(-2 lambda)/2]
+      if (part == 0) { k.v[0] = th[0]; k.v[1] = th[1]; k.v[2] = th[2]; k.v[3] = 0.5 * exp(-2.0 * th[2]); }
+      break;
+    case M_THINNED_SCHECHTER1D: // (alpha, x*, a): f = a + (alpha+1)(chi - x*) - e^chi e^(-x*);  v[4] = A = e^a
+      if (part == 0) { k.v[0] = th[0] + 1.0; k.v[1] = th[1]; k.v[2] = th[2]; k.v[3] = exp(-th[1]); }
+      if (part == 1) k.v[4] = exp(th[2]);
+      break;
+    case M_BINORMAL2D:          // (m1, m2, l1, l2, zeta): f = c0 - h (u1^2 - 2 rho u1 u2 + u2^2)
+      if (part == 0) { k.v[0] = th[0]; k.v[1] = th[1]; k.v[2] = exp(-th[2]); k.v[3] = exp(-th[3]); }
+      if (part == 1) { const double ch = cosh(th[4]); k.v[4] = -th[2] - th[3] + log(ch); k.v[5] = 0.5 * ch * ch; }
+      if (part == 2) k.v[6] = tanh(th[4]);
+      break;
+  }
+}
+
 HM_HD ThetaK theta_consts(int model, const double* th) {
   ThetaK k;
 #pragma unroll
   for (int j = 0; j < 8; ++j) k.v[j] = 0.0;
-  switch (model) {
-    case M_NORMAL1D:            // (mu, lambda): f = -lambda - (chi - mu)^2 * [e^(-2 lambda)/2]
-      k.v[0] = th[0]; k.v[1] = th[1]; k.v[2] = 0.5 * exp(-2.0 * th[1]);
-      break;
-    case M_LINREG_ME1D:         // (a, b, lambda): f = -lambda - (chi - a - b z)^2 * [e^(-2 lambda)/2]
-      k.v[0] = th[0]; k.v[1] = th[1]; k.v[2] = th[2]; k.v[3] = 0.5 * exp(-2.0 * th[2]);
-      break;
-    case M_THINNED_SCHECHTER1D: // (alpha, x*, a): f = a + (alpha+1)(chi - x*) - e^chi e^(-x*)
-      k.v[0] = th[0] + 1.0; k.v[1] = th[1]; k.v[2] = th[2]; k.v[3] = exp(-th[1]);
-      break;
-    case M_BINORMAL2D: {        // (m1, m2, l1, l2, zeta): f = c0 - h (u1^2 - 2 rho u1 u2 + u2^2)
-      const double ch = cosh(th[4]);
-      k.v[0] = th[0]; k.v[1] = th[1]; k.v[2] = exp(-th[2]); k.v[3] = exp(-th[3]);
-      k.v[4] = -th[2] - th[3] + log(ch); k.v[5] = 0.5 * ch * ch; k.v[6] = tanh(th[4]);
-      break;
-    }
-  }
+  for (int part = 0; part < 3; ++part) theta_consts_part(model, part, th, k);
   return k;
 }
 

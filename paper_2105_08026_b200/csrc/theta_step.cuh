@@ -1,8 +1,13 @@
 // theta_step.cuh -- the theta Metropolis-Hastings tail (PAPER.md:108 Eq. 2.5, :142), host + device.
 //
-// The same two functions run (a) on thread 0 of every block of the persistent kernel, redundantly and
-// bit-identically (THETA_DEVICE_TAIL), (b) in the 1-block tail kernel (THETA_GRAPH, debug_step), and
-// (c) on the host (THETA_HOST, the paper's own split).  DESIGN.md section 8.3.
+// Two implementations of the same arithmetic:
+//   (a) serial, __host__ __device__: `prepare_iteration` + `tail_decide`.  Used on the host (THETA_HOST, the
+//       paper's own split) and once per set_init / set_state on the device (k_init_iter).
+//   (b) block-parallel, device only: `tail_block`.  Used by the persistent kernel (every block, redundantly and
+//       bit-identically) and by k_tail (THETA_GRAPH, debug_step).  The serial chain of (a) costs ~4.4 us per
+//       iteration on one thread (profiles/r01a); (b) takes everything that does not depend on the decision off
+//       the critical path (draws are made two iterations ahead while warp 0 waits for the other blocks'
+//       partials) and spreads the rest over lanes and warps.
 #pragma once
 #include "models.cuh"
 
@@ -12,16 +17,25 @@ constexpr int MAXD = 8;                       // max dtheta
 constexpr int MAXTRI = MAXD * (MAXD + 1) / 2;
 constexpr int NPART = 5;                      // per-block partials: S, Delta, Tq, n_accept, n_nonfinite
 
-// Iteration state: lives in global memory between launches, in shared memory inside the persistent kernel.
+// Decision-independent quantities of one iteration t; ring slot t % 3 of Iter::dr.
+struct Draws {
+  double z[MAXD];       // z_theta ~ N(0, I)                       (theta Philox stream, draws 1..)
+  double uh[MAXD];      // z / |z|
+  double Pc[MAXD + 1];  // Pc[j] = sum_{k<j} uh_k^2
+  double eta;           // eta_n = n^(-eta_exp), n = t + 1         (X_1, S_1 are initial values)
+  double u;             // accept uniform of the theta step        (theta Philox stream, draw 0)
+};
+
+// Iteration state: lives in global memory between launches, in shared memory inside the kernels.
 struct Iter {
-  double theta[MAXD], thetaP[MAXD];   // theta and the pre-drawn proposal theta' of iteration t
+  double theta[MAXD], thetaP[MAXD];   // theta and the pre-drawn proposal theta' of the PREPARED iteration t
   double Lth[MAXTRI];                 // packed lower-triangular proposal factor of the theta RAM
-  double z[MAXD];                     // z_theta of iteration t (needed again by the RAM update)
+  double W[MAXTRI];                   // W[tri(i,j)] = sum_{k=j+1..i} Lth[i,k] uh_k for iteration t
+  Draws dr[3];                        // slots t%3 (iteration t) and (t+1)%3 are valid; (t+2)%3 is scratch
   ThetaK kc, kp;                      // theta-derived constants at theta / theta'
   double T_cur, lp_cur, lp_prop;      // theta-only term and log prior at theta; log prior at theta'
-  double eta;                         // eta_n of iteration t, n = t + 1
   // taps of the last decision (debug_step / host mode read them)
-  double S, Delta, T_prop, log_r, alpha_theta, u_theta, T_cur_used, lp_cur_used;
+  double S, Delta, T_prop, log_r, alpha_theta, u_theta, T_cur_used, lp_cur_used, tap_thetaP[MAXD];
   long long t;                        // the PREPARED iteration (1-based): t-1 iterations are complete
   long long mom_count, trace_rows;
   unsigned long long chi_acc, theta_acc, theta_prop_n, nonfinite;
@@ -37,44 +51,62 @@ struct TailCfg {
 };
 
 HM_HD int tri(int r, int c) { return r * (r + 1) / 2 + c; }
+HM_HD int tri_row(int e) { int r = 0; while ((r + 1) * (r + 2) / 2 <= e) ++r; return r; }
 
+// ---------------------------------------------------------------------------------------------------
 // RAM step 3 (Eq. 2.6) for general p as a rank-one update in closed form:
 //   chol(I + c u u^T) = K,  K_jj = sqrt(s_{j+1}/s_j),  K_ij = c u_i u_j / sqrt(s_j s_{j+1}) (i > j),
-//   s_j = 1 + c sum_{k<j} u_k^2;  then L <- L K, which is lower-triangular with positive diagonal and
-//   satisfies (L K)(L K)^T = L (I + c u u^T) L^T, hence is THE left Cholesky factor.
-//   1 + c >= 1 - alpha_* > 0, so every s_j > 0.
-HM_HD void ram_update_general(int p, double* L, const double* z, double c) {
-  double n2 = 0.0;
-  for (int j = 0; j < p; ++j) n2 += z[j] * z[j];
-  const double rn = 1.0 / sqrt(n2);
-  double u[MAXD], rs[MAXD + 1], Kd[MAXD], g[MAXD];
-  double s = 1.0;
-  rs[0] = 1.0;
-  for (int j = 0; j < p; ++j) { u[j] = z[j] * rn; s += c * u[j] * u[j]; rs[j + 1] = sqrt(s); }
-  for (int j = 0; j < p; ++j) { Kd[j] = rs[j + 1] / rs[j]; g[j] = c * u[j] / (rs[j] * rs[j + 1]); }
-  for (int i = 0; i < p; ++i) {
-    double w = 0.0;                               // sum_{k=j+1..i} L_ik u_k
-    for (int j = i; j >= 0; --j) {
-      const double lij = L[tri(i, j)];
-      L[tri(i, j)] = lij * Kd[j] + g[j] * w;
-      w += lij * u[j];
-    }
-  }
+//   s_j = 1 + c sum_{k<j} u_k^2;  then L <- L K, lower-triangular with positive diagonal, and
+//   (L K)(L K)^T = L (I + c u u^T) L^T, hence THE left Cholesky factor.
+//   1 + c >= 1 - alpha_* > 0, so every s_j > 0.  Entry-wise:
+//   (L K)_ij = L_ij Kd_j + g_j W_ij,  Kd_j = rs_{j+1}/rs_j,  g_j = c u_j/(rs_j rs_{j+1}),  rs_j = sqrt(s_j),
+//   W_ij = sum_{k=j+1..i} L_ik u_k (does not depend on c: precomputed off the critical path).
+HM_HD void ram_coeffs(int j, double c, const Draws& d, double* Kd, double* g) {
+  const double rs0 = sqrt(1.0 + c * d.Pc[j]), rs1 = sqrt(1.0 + c * d.Pc[j + 1]);
+  *Kd = rs1 / rs0;
+  *g = c * d.uh[j] / (rs0 * rs1);
 }
 
-// Everything about iteration t that does not depend on the sweep: eta_n, the theta proposal
-// theta' = theta + L_theta z (drawn BEFORE the sweep so one pass evaluates f at theta and theta'), its
-// derived constants and prior.
+HM_HD void make_draws(Draws& d, const TailCfg& c, long long t) {
+  d.eta = pow((double)(t + 1), -c.eta_exp);
+  for (int j = 0; j < MAXD; ++j) { d.z[j] = 0.0; d.uh[j] = 0.0; }
+  for (int j = 0; j <= MAXD; ++j) d.Pc[j] = 0.0;
+  d.u = 0.0;
+  if (c.freeze_theta) return;
+  normals(c.seed, KIND_THETA, 0ull, (uint32_t)t, c.dtheta, d.z);
+  double n2 = 0.0;
+  for (int j = 0; j < c.dtheta; ++j) n2 += d.z[j] * d.z[j];
+  const double rn = 1.0 / sqrt(n2);
+  double s = 0.0;
+  for (int j = 0; j < c.dtheta; ++j) { d.uh[j] = d.z[j] * rn; d.Pc[j] = s; s += d.uh[j] * d.uh[j]; }
+  d.Pc[c.dtheta] = s;
+  const U4 r = stream(c.seed, KIND_THETA, 0ull, (uint32_t)t, 0u);
+  d.u = u01(r.x, r.y);
+}
+
+HM_HD double make_W_entry(const Iter& it, const Draws& d, int i, int j) {
+  double w = 0.0;
+  for (int k = i; k > j; --k) w += it.Lth[tri(i, k)] * d.uh[k];
+  return w;
+}
+
+HM_HD double propose_entry(const Iter& it, const Draws& d, int r) {
+  double s = it.theta[r];
+  for (int k = 0; k <= r; ++k) s += it.Lth[tri(r, k)] * d.z[k];
+  return s;
+}
+
+// (a) serial: everything about iteration t that does not depend on its sweep.  theta' = theta + L_theta z is
+// drawn BEFORE the sweep so one pass evaluates f at theta and theta' (reading R7).
 HM_HD void prepare_iteration(Iter& it, const TailCfg& c, long long t) {
   it.t = t;
-  it.eta = pow((double)(t + 1), -c.eta_exp);                 // RAM iteration n = t + 1 (X_1, S_1 are initial values)
+  Draws& d = it.dr[t % 3];
+  make_draws(d, c, t);
+  make_draws(it.dr[(t + 1) % 3], c, t + 1);
   if (!c.freeze_theta) {
-    normals(c.seed, KIND_THETA, 0ull, (uint32_t)t, c.dtheta, it.z);
-    for (int r = 0; r < c.dtheta; ++r) {
-      double s = it.theta[r];
-      for (int k = 0; k <= r; ++k) s += it.Lth[tri(r, k)] * it.z[k];
-      it.thetaP[r] = s;
-    }
+    for (int r = 0; r < c.dtheta; ++r) it.thetaP[r] = propose_entry(it, d, r);
+    for (int i = 0; i < c.dtheta; ++i)
+      for (int j = 0; j <= i; ++j) it.W[tri(i, j)] = make_W_entry(it, d, i, j);
     it.kp = theta_consts(c.model, it.thetaP);
     it.lp_prop = log_prior(c.model, it.thetaP);
   } else {
@@ -84,38 +116,29 @@ HM_HD void prepare_iteration(Iter& it, const TailCfg& c, long long t) {
   }
 }
 
-// The theta decision of iteration it.t from the reduced sweep totals tot[NPART] = {S, Delta, Tq, nacc, nnan}.
-// Sets it.trace_write when the (new) theta has to be appended to the thinned trace at row it.trace_rows - 1.
-HM_HD void tail_decide(Iter& it, const TailCfg& c, const double* tot) {
-  it.S = tot[0];
-  it.Delta = tot[1];
-  it.chi_acc += (unsigned long long)tot[3];
-  it.nonfinite += (unsigned long long)tot[4];
-  it.accepted_theta = 0;
-  it.T_prop = 0.0; it.log_r = 0.0; it.alpha_theta = 0.0; it.u_theta = 0.0;
-  it.T_cur_used = it.T_cur; it.lp_cur_used = it.lp_cur;
-  if (!c.freeze_theta) {
-    double la;
-    if (it.lp_prop == -INFINITY) {
-      it.log_r = -INFINITY; la = -INFINITY;
-    } else {
-      // M1: T(theta') = -A' sum_k W_k phi(x_k; theta') -- minus the expected detected count (Eq. 4.4 denominator)
-      it.T_prop = (c.model == M_THINNED_SCHECHTER1D) ? -exp(it.kp.v[2]) * tot[2] : 0.0;
-      it.log_r = it.Delta + (it.T_prop - it.T_cur) + (it.lp_prop - it.lp_cur);
-      la = (it.log_r != it.log_r) ? -INFINITY : fmin(0.0, it.log_r);
-    }
-    it.alpha_theta = exp(la);
-    const U4 r = stream(c.seed, KIND_THETA, 0ull, (uint32_t)it.t, 0u);
-    it.u_theta = u01(r.x, r.y);
-    it.theta_prop_n += 1;
-    if (it.u_theta < it.alpha_theta) {
-      it.accepted_theta = 1;
-      it.theta_acc += 1;
-      for (int r2 = 0; r2 < c.dtheta; ++r2) it.theta[r2] = it.thetaP[r2];
-      it.kc = it.kp; it.T_cur = it.T_prop; it.lp_cur = it.lp_prop;
-    }
-    ram_update_general(c.dtheta, it.Lth, it.z, it.eta * (it.alpha_theta - c.astar_theta));
+// The acceptance part shared by (a) and (b): log r, alpha, accept flag.  tq = sum_k W_k phi(x_k; theta').
+HM_HD void decide_scalars(const Iter& it, const TailCfg& c, const Draws& d, double Delta, double tq, double* T_prop,
+                          double* log_r, double* alpha, int* acc) {
+  double la;
+  *T_prop = 0.0;
+  if (it.lp_prop == -INFINITY) {
+    *log_r = -INFINITY; la = -INFINITY;
+  } else {
+    // M1: T(theta') = -A' sum_k W_k phi(x_k; theta'): minus the expected detected count (Eq. 4.4 denominator)
+    *T_prop = (c.model == M_THINNED_SCHECHTER1D) ? -it.kp.v[4] * tq : 0.0;
+    *log_r = Delta + (*T_prop - it.T_cur) + (it.lp_prop - it.lp_cur);
+    la = (*log_r != *log_r) ? -INFINITY : fmin(0.0, *log_r);
   }
+  *alpha = exp(la);
+  *acc = d.u < *alpha ? 1 : 0;
+}
+
+// bookkeeping shared by (a) and (b), one thread: counters, moments count, trace row
+HM_HD void decide_bookkeeping(Iter& it, const TailCfg& c, double S, double Delta, double nacc, double nnan) {
+  it.S = S;
+  it.Delta = Delta;
+  it.chi_acc += (unsigned long long)nacc;
+  it.nonfinite += (unsigned long long)nnan;
   if (c.keep_moments && it.t > c.burn_in) it.mom_count += 1;
   it.trace_write = 0;
   if (it.t > c.burn_in && ((it.t - c.burn_in) % c.thin) == 0 && it.trace_rows < c.max_trace_rows) {
@@ -123,5 +146,139 @@ HM_HD void tail_decide(Iter& it, const TailCfg& c, const double* tot) {
     it.trace_write = 1;
   }
 }
+
+// (a) serial: the theta decision of iteration it.t from the reduced sweep totals {S, Delta, Tq, nacc, nnan}.
+// Sets it.trace_write when the (new) theta has to be appended to the thinned trace at row it.trace_rows - 1.
+HM_HD void tail_decide(Iter& it, const TailCfg& c, const double* tot) {
+  const Draws& d = it.dr[it.t % 3];
+  it.accepted_theta = 0;
+  it.T_prop = 0.0; it.log_r = 0.0; it.alpha_theta = 0.0; it.u_theta = 0.0;
+  it.T_cur_used = it.T_cur; it.lp_cur_used = it.lp_cur;
+  for (int r = 0; r < MAXD; ++r) it.tap_thetaP[r] = it.thetaP[r];
+  if (!c.freeze_theta) {
+    int acc;
+    decide_scalars(it, c, d, tot[1], tot[2], &it.T_prop, &it.log_r, &it.alpha_theta, &acc);
+    it.u_theta = d.u;
+    it.theta_prop_n += 1;
+    if (acc) {
+      it.accepted_theta = 1;
+      it.theta_acc += 1;
+      for (int r = 0; r < c.dtheta; ++r) it.theta[r] = it.thetaP[r];
+      it.kc = it.kp; it.T_cur = it.T_prop; it.lp_cur = it.lp_prop;
+    }
+    const double cc = d.eta * (it.alpha_theta - c.astar_theta);
+    for (int j = 0; j < c.dtheta; ++j) {
+      double Kd, g;
+      ram_coeffs(j, cc, d, &Kd, &g);
+      for (int i = j; i < c.dtheta; ++i) it.Lth[tri(i, j)] = it.Lth[tri(i, j)] * Kd + g * it.W[tri(i, j)];
+    }
+  }
+  decide_bookkeeping(it, c, tot[0], tot[1], tot[3], tot[4]);
+}
+
+#ifdef __CUDACC__
+// ---------------------------------------------------------------------------------------------------
+// (b) block-parallel tail (device).  Called by ALL threads of a block with >= 4 warps; `it` is in shared
+// memory.  tot = {S, Delta, Tq, nacc, nnan}, valid in every lane of warp 0 (S, nacc, nnan feed only the tap and
+// the counters: the persistent kernel passes zeros and counts locally).  Decides iteration t = it.t, prepares
+// iteration t + 1 and makes the draws of iteration t + 2.  Two block barriers.
+//
+//   phase B   warp 0:  decision scalars (all lanes redundantly) -> RAM coefficients (lane j) -> new L_theta
+//                      (lane e) -> theta, theta' of t+1 (lane r) -> kc <- kp on accept (lane v), bookkeeping.
+//             warp 1:  z, uh, Pc of iteration t+2 (Box-Muller pair per lane);  warp 2: eta of t+2;
+//             warp 3:  accept uniform of t+2.      None of these depends on the decision, so they run
+//                      while warp 0 is still waiting for the other blocks' partials.
+//   phase C   warp 0..2: the parts of theta_consts(theta'); warp 3: log prior(theta'); warp 1 (after its
+//             part): W of iteration t+1 (lane e).
+__device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const double* tot, double* trace_or_null) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int dt = c.dtheta, nt = dt * (dt + 1) / 2;
+  const long long t = it.t;
+  const Draws& d0 = it.dr[t % 3];
+  const Draws& d1 = it.dr[(t + 1) % 3];
+  Draws& d2 = it.dr[(t + 2) % 3];
+
+  if (warp == 0) {
+    if (!c.freeze_theta) {
+      double T_prop, log_r, alpha;
+      int acc;
+      decide_scalars(it, c, d0, tot[1], tot[2], &T_prop, &log_r, &alpha, &acc);
+      const double cc = d0.eta * (alpha - c.astar_theta);
+      double Kd = 1.0, g = 0.0;
+      if (lane < dt) ram_coeffs(lane, cc, d0, &Kd, &g);
+      const int e = lane < nt ? lane : 0;
+      const int ei = tri_row(e), ej = e - ei * (ei + 1) / 2;
+      const double Kd_j = __shfl_sync(0xffffffffu, Kd, ej), g_j = __shfl_sync(0xffffffffu, g, ej);
+      const double l_new = it.Lth[e] * Kd_j + g_j * it.W[e];
+      const double th_old = lane < dt ? it.theta[lane] : 0.0, thp_old = lane < dt ? it.thetaP[lane] : 0.0;
+      const double kpv = lane < 8 ? it.kp.v[lane] : 0.0;
+      __syncwarp();
+      if (lane < nt) it.Lth[e] = l_new;
+      if (lane < MAXD) it.tap_thetaP[lane] = lane < dt ? thp_old : 0.0;
+      if (lane < dt) it.theta[lane] = acc ? thp_old : th_old;
+      if (lane < 8 && acc) it.kc.v[lane] = kpv;
+      __syncwarp();
+      if (lane < dt) it.thetaP[lane] = propose_entry(it, d1, lane);
+      if (lane == 0) {
+        it.T_cur_used = it.T_cur; it.lp_cur_used = it.lp_cur;
+        it.T_prop = T_prop; it.log_r = log_r; it.alpha_theta = alpha; it.u_theta = d0.u;
+        it.accepted_theta = acc;
+        it.theta_prop_n += 1;
+        if (acc) { it.theta_acc += 1; it.T_cur = T_prop; it.lp_cur = it.lp_prop; }
+      }
+    } else if (lane == 0) {
+      it.accepted_theta = 0;
+      it.T_prop = 0.0; it.log_r = 0.0; it.alpha_theta = 0.0; it.u_theta = 0.0;
+      it.T_cur_used = it.T_cur; it.lp_cur_used = it.lp_cur;
+    }
+    if (lane == 0) decide_bookkeeping(it, c, tot[0], tot[1], tot[3], tot[4]);
+    __syncwarp();
+    if (trace_or_null && it.trace_write && lane < dt) trace_or_null[(it.trace_rows - 1) * dt + lane] = it.theta[lane];
+  } else if (warp == 1) {
+    if (!c.freeze_theta) {
+      if (2 * lane < dt) {
+        double rad, cs, sn;
+        box_muller(stream(c.seed, KIND_THETA, 0ull, (uint32_t)(t + 2), 1u + (uint32_t)lane), &rad, &cs, &sn);
+        d2.z[2 * lane] = rad * cs;
+        if (2 * lane + 1 < dt) d2.z[2 * lane + 1] = rad * sn;
+      }
+      __syncwarp();
+      if (lane == 0) {
+        double n2 = 0.0;
+        for (int j = 0; j < dt; ++j) n2 += d2.z[j] * d2.z[j];
+        const double rn = 1.0 / sqrt(n2);
+        double s = 0.0;
+        for (int j = 0; j < dt; ++j) { d2.uh[j] = d2.z[j] * rn; d2.Pc[j] = s; s += d2.uh[j] * d2.uh[j]; }
+        d2.Pc[dt] = s;
+      }
+    }
+  } else if (warp == 2) {
+    if (lane == 0) d2.eta = pow((double)(t + 3), -c.eta_exp);
+  } else if (warp == 3) {
+    if (lane == 0 && !c.freeze_theta) {
+      const U4 r = stream(c.seed, KIND_THETA, 0ull, (uint32_t)(t + 2), 0u);
+      d2.u = u01(r.x, r.y);
+    }
+  }
+  __syncthreads();
+  if (!c.freeze_theta) {
+    if (warp < 3) {
+      if (lane == 0) theta_consts_part(c.model, warp, it.thetaP, it.kp);
+      if (warp == 1 && lane < nt) {
+        const int ei = tri_row(lane), ej = lane - ei * (ei + 1) / 2;
+        it.W[lane] = make_W_entry(it, d1, ei, ej);
+      }
+    } else if (warp == 3) {
+      if (lane == 0) it.lp_prop = log_prior(c.model, it.thetaP);
+    }
+  } else if (threadIdx.x < 8) {
+    it.kp.v[threadIdx.x] = it.kc.v[threadIdx.x];
+    if (threadIdx.x < dt) it.thetaP[threadIdx.x] = it.theta[threadIdx.x];
+    if (threadIdx.x == 0) it.lp_prop = it.lp_cur;
+  }
+  if (threadIdx.x == 0) it.t = t + 1;
+  __syncthreads();
+}
+#endif
 
 }  // namespace hm
