@@ -16,6 +16,7 @@ OK, E_INVALID, E_STATE, E_CUDA, E_WORKSPACE, E_UNSUPPORTED, E_NONFINITE = 0, -1,
 M_NORMAL1D, M_THINNED_SCHECHTER1D, M_BINORMAL2D, M_LINREG_ME1D = 0, 1, 2, 3
 F64, F32_STATE_F64_REDUCE = 0, 1
 THETA_HOST, THETA_GRAPH, THETA_DEVICE_TAIL = 0, 1, 2
+FLAG_STREAMING_ONLY = 1
 FLOOR_LAUNCH, FLOOR_GRAPH, FLOOR_GRID_BARRIER, FLOOR_HOST_SYNC = 0, 1, 2, 3
 
 EXPORTS = ["cudahm_model_dims", "cudahm_workspace_bytes", "cudahm_create", "cudahm_destroy", "cudahm_set_data",
@@ -33,7 +34,7 @@ class Config(C.Structure):
                 ("n_data_cols", C.c_int32), ("freeze_theta", C.c_int32), ("seed", C.c_uint64),
                 ("target_accept_chi", C.c_double), ("target_accept_theta", C.c_double),
                 ("eta_exponent", C.c_double), ("init_scale_chi", C.c_double), ("keep_chi_moments", C.c_int32),
-                ("block_threads", C.c_int32), ("blocks_per_sm", C.c_int32), ("reserved", C.c_int32),
+                ("block_threads", C.c_int32), ("blocks_per_sm", C.c_int32), ("flags", C.c_int32),
                 ("max_trace_rows", C.c_int64)]
 
 
@@ -111,11 +112,11 @@ def model_dims(model):
 
 def make_config(model, n_objects, seed=0, precision=F64, theta_mode=THETA_DEVICE_TAIL, target_accept_chi=0.4,
                 target_accept_theta=0.234, eta_exponent=2.0 / 3.0, init_scale_chi=1.0, freeze_theta=False,
-                keep_chi_moments=False, max_trace_rows=0, block_threads=0, blocks_per_sm=0):
+                keep_chi_moments=False, max_trace_rows=0, block_threads=0, blocks_per_sm=0, flags=0):
     d = model_dims(model)
     return Config(C.sizeof(Config), model, precision, theta_mode, int(n_objects), d["p"], d["dtheta"], d["n_cols"],
                   int(freeze_theta), seed, target_accept_chi, target_accept_theta, eta_exponent, init_scale_chi,
-                  int(keep_chi_moments), block_threads, blocks_per_sm, 0, int(max_trace_rows))
+                  int(keep_chi_moments), block_threads, blocks_per_sm, int(flags), int(max_trace_rows))
 
 
 def workspace_bytes(cfg):

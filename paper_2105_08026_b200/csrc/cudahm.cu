@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "kernels.cuh"
+#include "resident.cuh"
 
 using namespace hm;
 
@@ -55,6 +56,18 @@ bool pick_block(int block, KernelSet* k) {
   return false;
 }
 
+// on-chip variant (resident.cuh): fp64, p = 1 models; n_values = shared-memory doubles per object
+const void* pick_resident(int model, int precision, int keep_moments, int* n_values) {
+  if (precision != CUDAHM_F64) return nullptr;
+  const int mom = keep_moments ? 2 : 0;
+  switch (model) {
+    case M_NORMAL1D:            *n_values = ResValues<M_NORMAL1D>::n_base + mom; return (const void*)k_resident<M_NORMAL1D>;
+    case M_THINNED_SCHECHTER1D: *n_values = ResValues<M_THINNED_SCHECHTER1D>::n_base + mom; return (const void*)k_resident<M_THINNED_SCHECHTER1D>;
+    case M_LINREG_ME1D:         *n_values = ResValues<M_LINREG_ME1D>::n_base + mom; return (const void*)k_resident<M_LINREG_ME1D>;
+  }
+  return nullptr;
+}
+
 bool pick_kernels(int model, int precision, int block, KernelSet* k) {
   if (precision == CUDAHM_F64) {
     switch (model) {
@@ -93,6 +106,9 @@ struct cudahm_sampler {
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   bool timed = false;
   unsigned epoch = 1;               // next mailbox epoch of the persistent kernel
+  const void* res_kernel = nullptr; // on-chip persistent kernel (resident.cuh) when the population fits, else NULL
+  int res_R = 0; size_t res_smem = 0;
+  int sweep_grid = 1, sweep_block = 512;   // launch shape of k_sweep (THETA_GRAPH / HOST / debug_step)
   double h_lp_prop_before = 0.0;    // log prior at theta' of the iteration debug_step is about to decide
   // CUDA-graph cache (THETA_GRAPH)
   cudaGraphExec_t gexec = nullptr;
@@ -123,7 +139,7 @@ bool valid_config(const cudahm_config* c, int* p, int* dt, int* nc, int* nk) {
   if (!c || c->struct_size != sizeof(cudahm_config)) return false;
   if (!model_dims(c->model, p, dt, nc, nk)) return false;
   if (c->p != *p || c->dtheta != *dt || c->n_data_cols != *nc) return false;
-  if (c->n_objects < 0 || c->max_trace_rows < 0 || c->reserved != 0) return false;
+  if (c->n_objects < 0 || c->max_trace_rows < 0 || (c->flags & ~CUDAHM_FLAG_STREAMING_ONLY) != 0) return false;
   if (c->precision != CUDAHM_F64 && c->precision != CUDAHM_F32_STATE_F64_REDUCE) return false;
   if (c->theta_mode < CUDAHM_THETA_HOST || c->theta_mode > CUDAHM_THETA_DEVICE_TAIL) return false;
   if (!(c->target_accept_chi > 0.0 && c->target_accept_chi < 1.0)) return false;
@@ -214,6 +230,24 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
   s->grid = (int)std::max(1LL, std::min<long long>((long long)sms * per_sm, need));
   s->grid = std::min(s->grid, MAX_BLOCKS);
   if (cfg->theta_mode == CUDAHM_THETA_DEVICE_TAIL && s->grid > MAX_PGRID) s->grid = std::max(1, MAX_PGRID / sms) * sms;
+  s->sweep_grid = s->grid; s->sweep_block = block;
+  // on-chip variant: every object stays in the shared memory of its block for the whole launch
+  if (cfg->theta_mode == CUDAHM_THETA_DEVICE_TAIL && !(cfg->flags & CUDAHM_FLAG_STREAMING_ONLY) && cfg->n_objects > 0) {
+    int nv = 0;
+    const void* rk = pick_resident(cfg->model, cfg->precision, cfg->keep_chi_moments, &nv);
+    if (rk) {
+      const long long g = std::min<long long>(sms, (cfg->n_objects + RES_S - 1) / RES_S);
+      const long long R = (cfg->n_objects + g * RES_S - 1) / (g * RES_S);
+      const size_t bytes = (size_t)nv * R * RES_S * sizeof(double);
+      if (bytes <= (size_t)RES_MAX_SMEM &&
+          cudaFuncSetAttribute(rk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) == cudaSuccess) {
+        s->res_kernel = rk; s->res_R = (int)R; s->res_smem = bytes;
+        s->grid = (int)g; s->block = RES_THREADS;
+      } else {
+        cudaGetLastError();
+      }
+    }
+  }
 
   Params& P = s->P;
   P.N = cfg->n_objects; P.Npad = (cfg->n_objects + 31) / 32 * 32;
@@ -433,8 +467,17 @@ int run_device_tail(cudahm_sampler* s, long long n_iter) {
     Params P = s->P;
     unsigned epoch0 = s->epoch;            // epochs never repeat over the sampler's lifetime (0 = never written)
     s->epoch += (unsigned)k;
-    void* args[] = {&P, &k, &epoch0};
-    int rc = launch(s, s->ks.persistent, s->grid, s->block, args, true);
+    int R = s->res_R;
+    void* args[] = {&P, &k, &epoch0, &R};
+    int rc;
+    if (s->res_kernel) {
+      cudaError_t e = cudaLaunchCooperativeKernel(s->res_kernel, dim3(s->grid), dim3(RES_THREADS), args, s->res_smem, s->stream);
+      if (e != cudaSuccess) return fail(s, CUDAHM_E_CUDA, "resident kernel launch: %s", cudaGetErrorString(e));
+      s->launches++;
+      rc = CUDAHM_OK;
+    } else {
+      rc = launch(s, s->ks.persistent, s->grid, s->block, args, true);
+    }
     if (rc) return rc;
     n_iter -= k;
   }
@@ -444,9 +487,9 @@ int run_device_tail(cudahm_sampler* s, long long n_iter) {
 int enqueue_graph_iteration(cudahm_sampler* s) {
   Params P = s->P;
   void* a1[] = {&P};
-  int rc = launch(s, s->ks.sweep, s->grid, s->block, a1, false);
+  int rc = launch(s, s->ks.sweep, s->sweep_grid, s->sweep_block, a1, false);
   if (rc) return rc;
-  int nb = s->grid, flags = TAIL_DECIDE;
+  int nb = s->sweep_grid, flags = TAIL_DECIDE;
   void* a2[] = {&P, &nb, &flags};
   return launch(s, (const void*)k_tail, 1, TAIL_THREADS, a2, false);
 }
@@ -494,9 +537,9 @@ int run_host(cudahm_sampler* s, long long n_iter) {
   for (long long k = 0; k < n_iter; ++k) {
     Params P = s->P;
     void* a1[] = {&P};
-    int rc = launch(s, s->ks.sweep, s->grid, s->block, a1, false);
+    int rc = launch(s, s->ks.sweep, s->sweep_grid, s->sweep_block, a1, false);
     if (rc) return rc;
-    int nb = s->grid, flags = TAIL_REDUCE;
+    int nb = s->sweep_grid, flags = TAIL_REDUCE;
     void* a2[] = {&P, &nb, &flags};
     rc = launch(s, (const void*)k_tail, 1, TAIL_THREADS, a2, false);
     if (rc) return rc;
@@ -577,8 +620,8 @@ extern "C" int cudahm_debug_step(cudahm_sampler* s, int64_t burn_in, int32_t thi
   P.taps.u = q; q += N; P.taps.a = q; q += N; P.taps.b = q; q += N;
   P.taps.accepted = ibuf;
   void* a1[] = {&P};
-  rc = launch(s, s->ks.sweep_tap, s->grid, s->block, a1, false);
-  int nb = s->grid, flags = TAIL_REDUCE | TAIL_DECIDE;     // the device tail decides t and prepares t + 1
+  rc = launch(s, s->ks.sweep_tap, s->sweep_grid, s->sweep_block, a1, false);
+  int nb = s->sweep_grid, flags = TAIL_REDUCE | TAIL_DECIDE;     // the device tail decides t and prepares t + 1
   void* a2[] = {&P, &nb, &flags};
   if (!rc) rc = launch(s, (const void*)k_tail, 1, TAIL_THREADS, a2, false);
   cudaError_t e = cudaSuccess;

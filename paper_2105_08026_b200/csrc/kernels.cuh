@@ -301,11 +301,12 @@ __device__ __forceinline__ void slots_reduce(const double* slots, int nblocks, d
 // alternate by iteration parity: a block can be at most one iteration ahead of the slowest reader (it needs
 // everybody's slot of iteration k to get past k).  Epochs increase over the sampler's lifetime.
 //   mbox layout: [parity][reader][value 0..1][writer][2 words]
-__device__ __forceinline__ void mbox_push(unsigned long long* mbox_parity, int G, int writer, unsigned epoch, double a, double b) {
+__device__ __forceinline__ void mbox_push(unsigned long long* mbox_parity, int G, int writer, unsigned epoch, double a, double b,
+                                          int first, int stride) {
   const unsigned long long e = (unsigned long long)epoch << 32;
   const unsigned long long ua = (unsigned long long)__double_as_longlong(a), ub = (unsigned long long)__double_as_longlong(b);
   const unsigned long long a0 = e | (ua & 0xffffffffull), a1 = e | (ua >> 32), b0 = e | (ub & 0xffffffffull), b1 = e | (ub >> 32);
-  for (int r = threadIdx.x; r < G; r += blockDim.x) {
+  for (int r = first; r < G; r += stride) {
     unsigned long long* box = mbox_parity + (size_t)r * 4 * G;
     asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(box + 2 * writer), "l"(a0), "l"(a1) : "memory");
     asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(box + 2 * G + 2 * writer), "l"(b0), "l"(b1) : "memory");
@@ -389,7 +390,7 @@ __global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const l
     block_reduce_all<2>(dq, red);
     unsigned long long* mb = P.mbox + (size_t)(k & 1) * 4 * G * G;
     const unsigned epoch = epoch0 + (unsigned)k;
-    mbox_push(mb, G, (int)blockIdx.x, epoch, dq[0], dq[1]);
+    mbox_push(mb, G, (int)blockIdx.x, epoch, dq[0], dq[1], (int)threadIdx.x, (int)blockDim.x);
     HM_STAMP(1)
 #ifdef HM_PHASE_TIMING
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1_));
@@ -404,7 +405,7 @@ __global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const l
 #ifdef HM_PHASE_TIMING
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g2_));
 #endif
-    tail_block(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr);
+    tail_block(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, (int)(threadIdx.x >> 5), SyncAll());
     HM_STAMP(3)
 #ifdef HM_PHASE_TIMING
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g3_));
@@ -458,7 +459,7 @@ __global__ void __launch_bounds__(TAIL_THREADS, 1) k_tail(const Params P, const 
     }
   }
   if (flags & TAIL_DECIDE) {
-    tail_block(it, P.tail, tot, P.trace);
+    tail_block(it, P.tail, tot, P.trace, (int)(threadIdx.x >> 5), SyncAll());
     copy_iter(P.iter, &it);
   }
 }

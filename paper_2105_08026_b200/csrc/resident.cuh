@@ -1,0 +1,208 @@
+// resident.cuh -- the on-chip variant of the persistent Gibbs kernel for populations that fit in shared memory
+// (fp64, p = 1: BASELINE configs C0, C1, C2).  DESIGN.md section 8.5.
+//
+// At N = 3e5 an iteration moves 24 MB (3.7 us at HBM peak) and the exchange + theta tail is a serial chain of
+// ~4 us that no amount of bandwidth shortens (profiles/r01b).  This kernel removes both from the critical path:
+//   - every object lives in the shared memory of the block that owns it for the whole launch (chi, L, data,
+//     moments, e^chi): HBM/L2 are touched at launch start and end only;
+//   - the sweep is split into a theta-INDEPENDENT front (Philox draws, Box-Muller, chi' = chi + L z, e^chi') and
+//     a theta-dependent back (log targets, accept, RAM update, population terms, moments).  Sweep warps run
+//     back(t) -> hand their partials to the tail warps -> front(t+1) while 4 dedicated tail warps do the
+//     grid-wide exchange and the theta step of iteration t; the sweep warps only wait for theta_{t+1} if the
+//     tail is still running when their front is done.
+// Same arithmetic per object as kernels.cuh::sweep (same Plate<> functors, same draws); only the order in which
+// block partials are added differs (fixed, so still deterministic).
+#pragma once
+#include "kernels.cuh"
+
+namespace hm {
+
+constexpr int RES_SW = 16;                          // sweep warps per block
+constexpr int RES_S = RES_SW * 32;                  // sweep threads per block
+constexpr int RES_TW = 4;                           // tail warps per block (tail_block needs exactly 4)
+constexpr int RES_THREADS = RES_S + RES_TW * 32;    // 640
+constexpr int RES_MAX_SMEM = 200 * 1024;            // dynamic shared memory the kernel may ask for
+
+// per-object values kept in shared memory: [value][slot r][sweep thread]
+template <int MODEL> struct ResValues {
+  static constexpr int ncols = ModelDims<MODEL>::ncols;
+  static constexpr bool m1 = MODEL == M_THINNED_SCHECHTER1D;
+  static constexpr int V_CHI = 0, V_L = 1, V_D = 2, V_XP = 2 + ncols, V_U = 3 + ncols, V_E = 4 + ncols, V_EP = 5 + ncols;
+  static constexpr int n_base = 4 + ncols + (m1 ? 2 : 0);   // + 2 (mean, M2) when moments are kept
+};
+
+__device__ __forceinline__ void bar_sync(const int id, const int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void bar_arrive(const int id, const int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+enum : int { BAR_PARTIALS = 1, BAR_THETA = 2, BAR_TAIL = 3 };
+
+template <int MODEL>
+__global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, const long long n_iter, const unsigned epoch0,
+                                                             const int R) {
+  using T = double;
+  using V = ResValues<MODEL>;
+  using PL = Plate<MODEL, T>;
+  constexpr int ncols = V::ncols;
+  extern __shared__ double sm[];
+  __shared__ Iter it;
+  __shared__ double red[2][RES_SW][2];
+  __shared__ unsigned long long cnt_sm[2];
+  const int tid = (int)threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const bool is_tail = warp >= RES_SW;
+  const int G = (int)gridDim.x;
+  const long long N = P.N, Npad = P.Npad;
+  const int RS = R * RES_S;
+  const bool keep_mom = P.tail.keep_moments != 0;
+  const int V_MEAN = V::n_base, V_M2 = V::n_base + 1;
+  const long long obj0 = (long long)blockIdx.x * RS + tid;      // slot r of this thread is object obj0 + r*RES_S
+  T* const chi = static_cast<T*>(P.chi);
+  T* const Lm = static_cast<T*>(P.L);
+  const T* const dat = static_cast<const T*>(P.data);
+#define HM_AT(v, r) sm[(size_t)(v) * RS + (r) * RES_S + tid]
+
+  copy_iter(&it, P.iter);
+  if (tid < 2) cnt_sm[tid] = 0ull;
+  if (!is_tail) {
+    for (int r = 0; r < R; ++r) {
+      const long long i = obj0 + (long long)r * RES_S;
+      if (i < N) {
+        const T x = chi[i];
+        HM_AT(V::V_CHI, r) = x;
+        HM_AT(V::V_L, r) = Lm[i];
+#pragma unroll
+        for (int c = 0; c < ncols; ++c) HM_AT(V::V_D + c, r) = __ldg(dat + c * Npad + i);
+        if (V::m1) HM_AT(V::V_E, r) = hm_exp(x);
+        if (keep_mom) { HM_AT(V_MEAN, r) = P.mom_mean[i]; HM_AT(V_M2, r) = P.mom_M2[i]; }
+      }
+    }
+  }
+  __syncthreads();
+  const long long t0 = it.t;
+
+  if (!is_tail) {
+    // theta-independent half of the update of iteration t: draws, proposal, e^chi'
+    auto front = [&](const uint32_t t) {
+      for (int r = 0; r < R; ++r) {
+        const long long i = obj0 + (long long)r * RES_S;
+        if (i < N) {
+          T z[2] = {0.0, 0.0}, cs, sn, u;
+          plate_draws<1>(P.tail.seed, i, t, z, &cs, &sn, &u);
+          const T xp = HM_AT(V::V_CHI, r) + HM_AT(V::V_L, r) * z[0];
+          HM_AT(V::V_XP, r) = xp;
+          HM_AT(V::V_U, r) = u;
+          if (V::m1) HM_AT(V::V_EP, r) = hm_exp(xp);
+        }
+      }
+    };
+    T mcT[7];
+#pragma unroll
+    for (int j = 0; j < 7; ++j) mcT[j] = (T)P.mc[j];
+    const T astar = (T)P.astar_chi;
+    double nacc = 0.0, nnan = 0.0;
+
+    front((uint32_t)t0);
+    for (long long k = 0; k < n_iter; ++k) {
+      const long long t = t0 + k;
+      if (k > 0) bar_sync(BAR_THETA, RES_THREADS);          // theta_t, theta'_t are in `it`
+      // theta-dependent half: targets, accept, RAM update, population terms, moments
+      const ThetaK kc = it.kc, kp = it.kp;
+      const KT<T> kT = narrow<T>(kc);
+      const T eta = (T)it.dr[t % 3].eta;
+      const bool do_mom = keep_mom && t > P.tail.burn_in;
+      const double inv_k = 1.0 / (double)(it.mom_count + 1);
+      double v[2] = {0.0, 0.0};
+      for (int r = 0; r < R; ++r) {
+        const long long i = obj0 + (long long)r * RES_S;
+        if (i < N) {
+          T di[ncols];
+#pragma unroll
+          for (int c = 0; c < ncols; ++c) di[c] = HM_AT(V::V_D + c, r);
+          const T xi = HM_AT(V::V_CHI, r), yi = HM_AT(V::V_XP, r), l = HM_AT(V::V_L, r), u = HM_AT(V::V_U, r);
+          typename PL::Pt qc, qp;
+          if constexpr (V::m1) { qc = typename PL::Pt{xi, HM_AT(V::V_E, r)}; qp = typename PL::Pt{yi, HM_AT(V::V_EP, r)}; }
+          else { qc = PL::point(&xi); qp = PL::point(&yi); }
+          const T pc = PL::target(qc, di, kT, mcT), pp = PL::target(qp, di, kT, mcT);
+          const T diff = pp - pc;
+          const bool bad = diff != diff;
+          const T la = bad ? T(-INFINITY) : (diff < T(0) ? diff : T(0));
+          const T alpha = hm_exp(la);
+          const bool acc = u < alpha;
+          const typename PL::Pt qn = acc ? qp : qc;
+          const T ln = l * hm_sqrt(T(1) + eta * (alpha - astar));
+          const double a = PL::pop(qn, di, kc), b = PL::pop(qn, di, kp);
+          v[0] += b - a;
+          nacc += acc ? 1.0 : 0.0; nnan += bad ? 1.0 : 0.0;
+          HM_AT(V::V_CHI, r) = qn.x;
+          HM_AT(V::V_L, r) = ln;
+          if constexpr (V::m1) HM_AT(V::V_E, r) = qn.ex;
+          if (do_mom) {
+            const double xv = (double)qn.x, m0 = HM_AT(V_MEAN, r);
+            const double dl = xv - m0, m1 = m0 + dl * inv_k;
+            HM_AT(V_MEAN, r) = m1;
+            HM_AT(V_M2, r) += dl * (xv - m1);
+          }
+        }
+      }
+      if (V::m1 && !P.tail.freeze_theta) {          // this thread's terms of the selection integral at theta'
+        for (int q = (int)blockIdx.x + G * tid; q < NQUAD; q += G * RES_S)
+          v[1] += P.qW[q] * exp(kp.v[0] * (P.qx[q] - kp.v[1]) - P.qex[q] * kp.v[3]);
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        v[0] += __shfl_down_sync(0xffffffffu, v[0], o);
+        v[1] += __shfl_down_sync(0xffffffffu, v[1], o);
+      }
+      if (lane == 0) { red[k & 1][warp][0] = v[0]; red[k & 1][warp][1] = v[1]; }
+      __threadfence_block();
+      bar_arrive(BAR_PARTIALS, RES_THREADS);                 // hand the partials to the tail warps, do not wait
+      if (k + 1 < n_iter) front((uint32_t)(t + 1));          // overlaps the exchange and the theta step
+    }
+    bar_sync(BAR_THETA, RES_THREADS);                        // the last tail has finished
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      nacc += __shfl_down_sync(0xffffffffu, nacc, o);
+      nnan += __shfl_down_sync(0xffffffffu, nnan, o);
+    }
+    if (lane == 0) {
+      atomicAdd(&cnt_sm[0], (unsigned long long)nacc);
+      atomicAdd(&cnt_sm[1], (unsigned long long)nnan);
+    }
+    for (int r = 0; r < R; ++r) {
+      const long long i = obj0 + (long long)r * RES_S;
+      if (i < N) {
+        chi[i] = HM_AT(V::V_CHI, r);
+        Lm[i] = HM_AT(V::V_L, r);
+        if (keep_mom) { P.mom_mean[i] = HM_AT(V_MEAN, r); P.mom_M2[i] = HM_AT(V_M2, r); }
+      }
+    }
+  } else {
+    const int tw = warp - RES_SW, ttid = tid - RES_S;
+    for (long long k = 0; k < n_iter; ++k) {
+      bar_sync(BAR_PARTIALS, RES_THREADS);                   // the block's 16 warp partials of iteration t0 + k
+      double dq[2];
+      dq[0] = lane < RES_SW ? red[k & 1][lane][0] : 0.0;
+      dq[1] = lane < RES_SW ? red[k & 1][lane][1] : 0.0;
+      lanes_to_total<2>(dq);
+      unsigned long long* mb = P.mbox + (size_t)(k & 1) * 4 * G * G;
+      const unsigned epoch = epoch0 + (unsigned)k;
+      mbox_push(mb, G, (int)blockIdx.x, epoch, dq[0], dq[1], ttid, RES_TW * 32);
+      double tot[NPART] = {0.0, 0.0, 0.0, 0.0, 0.0};
+      if (tw == 0) {
+        double t2[2];
+        mbox_collect(mb + (size_t)blockIdx.x * 4 * G, G, epoch, t2);
+        tot[1] = t2[0]; tot[2] = t2[1];
+      }
+      tail_block(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, tw, SyncNamed<BAR_TAIL, RES_TW * 32>());
+      __threadfence_block();
+      bar_arrive(BAR_THETA, RES_THREADS);
+    }
+  }
+#undef HM_AT
+  __syncthreads();
+  if (tid == 0) {
+    P.blk_cnt[2 * blockIdx.x] += cnt_sm[0];
+    P.blk_cnt[2 * blockIdx.x + 1] += cnt_sm[1];
+  }
+  if (blockIdx.x == 0) copy_iter(P.iter, &it);
+}
+
+}  // namespace hm

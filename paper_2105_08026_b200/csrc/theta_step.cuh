@@ -62,9 +62,14 @@ HM_HD int tri_row(int e) { int r = 0; while ((r + 1) * (r + 2) / 2 <= e) ++r; re
 //   (L K)_ij = L_ij Kd_j + g_j W_ij,  Kd_j = rs_{j+1}/rs_j,  g_j = c u_j/(rs_j rs_{j+1}),  rs_j = sqrt(s_j),
 //   W_ij = sum_{k=j+1..i} L_ik u_k (does not depend on c: precomputed off the critical path).
 HM_HD void ram_coeffs(int j, double c, const Draws& d, double* Kd, double* g) {
-  const double rs0 = sqrt(1.0 + c * d.Pc[j]), rs1 = sqrt(1.0 + c * d.Pc[j + 1]);
-  *Kd = rs1 / rs0;
-  *g = c * d.uh[j] / (rs0 * rs1);
+  const double s0 = 1.0 + c * d.Pc[j], s1 = 1.0 + c * d.Pc[j + 1];
+#ifdef __CUDA_ARCH__
+  const double r = rsqrt(s0 * s1);          // one reciprocal square root instead of two roots and two divisions
+#else
+  const double r = 1.0 / sqrt(s0 * s1);
+#endif
+  *Kd = s1 * r;                             // sqrt(s1/s0)
+  *g = c * d.uh[j] * r;                     // c u_j / sqrt(s0 s1)
 }
 
 HM_HD void make_draws(Draws& d, const TailCfg& c, long long t) {
@@ -133,12 +138,15 @@ HM_HD void decide_scalars(const Iter& it, const TailCfg& c, const Draws& d, doub
   *acc = d.u < *alpha ? 1 : 0;
 }
 
-// bookkeeping shared by (a) and (b), one thread: counters, moments count, trace row
-HM_HD void decide_bookkeeping(Iter& it, const TailCfg& c, double S, double Delta, double nacc, double nnan) {
+// bookkeeping shared by (a) and (b): taps and counters fed by the sweep totals ...
+HM_HD void decide_counters(Iter& it, double S, double Delta, double nacc, double nnan) {
   it.S = S;
   it.Delta = Delta;
   it.chi_acc += (unsigned long long)nacc;
   it.nonfinite += (unsigned long long)nnan;
+}
+// ... and the moments count / trace row of iteration it.t (independent of the decision)
+HM_HD void decide_schedule(Iter& it, const TailCfg& c) {
   if (c.keep_moments && it.t > c.burn_in) it.mom_count += 1;
   it.trace_write = 0;
   if (it.t > c.burn_in && ((it.t - c.burn_in) % c.thin) == 0 && it.trace_rows < c.max_trace_rows) {
@@ -173,30 +181,40 @@ HM_HD void tail_decide(Iter& it, const TailCfg& c, const double* tot) {
       for (int i = j; i < c.dtheta; ++i) it.Lth[tri(i, j)] = it.Lth[tri(i, j)] * Kd + g * it.W[tri(i, j)];
     }
   }
-  decide_bookkeeping(it, c, tot[0], tot[1], tot[3], tot[4]);
+  decide_counters(it, tot[0], tot[1], tot[3], tot[4]);
+  decide_schedule(it, c);
 }
 
 #ifdef __CUDACC__
 // ---------------------------------------------------------------------------------------------------
-// (b) block-parallel tail (device).  Called by ALL threads of a block with >= 4 warps; `it` is in shared
-// memory.  tot = {S, Delta, Tq, nacc, nnan}, valid in every lane of warp 0 (S, nacc, nnan feed only the tap and
-// the counters: the persistent kernel passes zeros and counts locally).  Decides iteration t = it.t, prepares
-// iteration t + 1 and makes the draws of iteration t + 2.  Two block barriers.
+// (b) block-parallel tail (device).  Called by 4 warps (`warp` = 0..3 among them; `sync` = a barrier over exactly
+// those 128 threads); `it` is in shared memory.  tot = {S, Delta, Tq, nacc, nnan}, valid in every lane of warp 0
+// (S, nacc, nnan feed only the tap and the counters: the persistent kernels pass zeros and count locally).
+// Decides iteration t = it.t, prepares iteration t + 1 and makes the draws of iteration t + 2.
 //
 //   phase B   warp 0:  decision scalars (all lanes redundantly) -> RAM coefficients (lane j) -> new L_theta
-//                      (lane e) -> theta, theta' of t+1 (lane r) -> kc <- kp on accept (lane v), bookkeeping.
-//             warp 1:  z, uh, Pc of iteration t+2 (Box-Muller pair per lane);  warp 2: eta of t+2;
-//             warp 3:  accept uniform of t+2.      None of these depends on the decision, so they run
-//                      while warp 0 is still waiting for the other blocks' partials.
-//   phase C   warp 0..2: the parts of theta_consts(theta'); warp 3: log prior(theta'); warp 1 (after its
-//             part): W of iteration t+1 (lane e).
-__device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const double* tot, double* trace_or_null) {
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+//                      (lane e) -> theta, theta' of t+1 (lane r) -> kc <- kp on accept (lane v).
+//             warp 1:  z, uh, Pc of iteration t+2 (Box-Muller pair per lane);  warp 2: eta of t+2, moments /
+//             trace schedule of t;  warp 3: accept uniform of t+2.  None of these depends on the decision, so
+//             they run while warp 0 is still waiting for the other blocks' partials.
+//   phase C   warp 0..2: the parts of theta_consts(theta'); warp 3: log prior(theta'); warp 1 also W of t+1
+//             (lane e); warp 2 also the trace row.
+struct SyncAll { __device__ __forceinline__ void operator()() const { __syncthreads(); } };
+template <int ID, int THREADS>
+struct SyncNamed {
+  __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, %1;" ::"n"(ID), "n"(THREADS) : "memory"); }
+};
+
+template <class Sync>
+__device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const double* tot, double* trace_or_null,
+                                           const int warp, const Sync sync) {
+  const int lane = threadIdx.x & 31;
   const int dt = c.dtheta, nt = dt * (dt + 1) / 2;
   const long long t = it.t;
-  const Draws& d0 = it.dr[t % 3];
-  const Draws& d1 = it.dr[(t + 1) % 3];
-  Draws& d2 = it.dr[(t + 2) % 3];
+  const int r0 = (int)(t % 3), r1 = r0 == 2 ? 0 : r0 + 1, r2 = r1 == 2 ? 0 : r1 + 1;
+  const Draws& d0 = it.dr[r0];
+  const Draws& d1 = it.dr[r1];
+  Draws& d2 = it.dr[r2];
 
   if (warp == 0) {
     if (!c.freeze_theta) {
@@ -231,9 +249,7 @@ __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const dou
       it.T_prop = 0.0; it.log_r = 0.0; it.alpha_theta = 0.0; it.u_theta = 0.0;
       it.T_cur_used = it.T_cur; it.lp_cur_used = it.lp_cur;
     }
-    if (lane == 0) decide_bookkeeping(it, c, tot[0], tot[1], tot[3], tot[4]);
-    __syncwarp();
-    if (trace_or_null && it.trace_write && lane < dt) trace_or_null[(it.trace_rows - 1) * dt + lane] = it.theta[lane];
+    if (lane == 1) decide_counters(it, tot[0], tot[1], tot[3], tot[4]);
   } else if (warp == 1) {
     if (!c.freeze_theta) {
       if (2 * lane < dt) {
@@ -253,14 +269,17 @@ __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const dou
       }
     }
   } else if (warp == 2) {
-    if (lane == 0) d2.eta = pow((double)(t + 3), -c.eta_exp);
+    if (lane == 0) {
+      d2.eta = pow((double)(t + 3), -c.eta_exp);
+      decide_schedule(it, c);
+    }
   } else if (warp == 3) {
     if (lane == 0 && !c.freeze_theta) {
       const U4 r = stream(c.seed, KIND_THETA, 0ull, (uint32_t)(t + 2), 0u);
       d2.u = u01(r.x, r.y);
     }
   }
-  __syncthreads();
+  sync();
   if (!c.freeze_theta) {
     if (warp < 3) {
       if (lane == 0) theta_consts_part(c.model, warp, it.thetaP, it.kp);
@@ -271,13 +290,15 @@ __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const dou
     } else if (warp == 3) {
       if (lane == 0) it.lp_prop = log_prior(c.model, it.thetaP);
     }
-  } else if (threadIdx.x < 8) {
-    it.kp.v[threadIdx.x] = it.kc.v[threadIdx.x];
-    if (threadIdx.x < dt) it.thetaP[threadIdx.x] = it.theta[threadIdx.x];
-    if (threadIdx.x == 0) it.lp_prop = it.lp_cur;
+  } else if (warp == 0 && lane < 8) {
+    it.kp.v[lane] = it.kc.v[lane];
+    if (lane < dt) it.thetaP[lane] = it.theta[lane];
+    if (lane == 0) it.lp_prop = it.lp_cur;
   }
-  if (threadIdx.x == 0) it.t = t + 1;
-  __syncthreads();
+  if (warp == 2 && trace_or_null && it.trace_write && lane < dt)
+    trace_or_null[(it.trace_rows - 1) * dt + lane] = it.theta[lane];
+  if (warp == 3 && lane == 1) it.t = t + 1;
+  sync();
 }
 #endif
 
