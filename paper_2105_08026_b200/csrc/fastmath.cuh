@@ -1,0 +1,137 @@
+// fastmath.cuh -- fp64 exp / log / sqrt specialised to the arguments the sweep feeds them (host + device).
+//
+// The ncu source page of the on-chip kernel (profiles/r01b) attributes 42 % of all executed instructions to four
+// libm calls per object-update: log + sqrt of the Box-Muller radius (99 instructions), two exp (97), cospi (50).
+// The CUDA libm versions pay for argument ranges that cannot occur here (denormals, infinities, huge arguments).
+// These versions keep 1-2 ulp accuracy (exp <= 1.5, log <= 2, sqrt <= 1) on the ranges below with about half the
+// instructions:
+//   hm_exp_fast(x)   any finite x (clamped to [-708, 709]); x = -inf gives exp(-708) ~ 3e-308, NOT 0 (callers that
+//                    need exp(-inf) = 0 select it themselves)
+//   hm_log_unit(u)   u in [2^-53, 1): positive normal numbers only
+//   hm_sqrt_fast(w)  w > 0 normal
+// tests/test_fastmath_host.py measures their error against mpmath on the host build of this very header.
+#pragma once
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <cuda_runtime.h>
+
+#ifndef HM_HD
+#define HM_HD __host__ __device__ __forceinline__
+#endif
+
+namespace hm {
+
+HM_HD double hm_bits2d(uint64_t b) {
+#ifdef __CUDA_ARCH__
+  return __longlong_as_double((long long)b);
+#else
+  double d; std::memcpy(&d, &b, sizeof d); return d;
+#endif
+}
+HM_HD uint64_t hm_d2bits(double d) {
+#ifdef __CUDA_ARCH__
+  return (uint64_t)__double_as_longlong(d);
+#else
+  uint64_t b; std::memcpy(&b, &d, sizeof b); return b;
+#endif
+}
+HM_HD double hm_fma(double a, double b, double c) {
+#ifdef __CUDA_ARCH__
+  return __fma_rn(a, b, c);
+#else
+  return std::fma(a, b, c);
+#endif
+}
+
+// 2^-23-accurate seeds (one MUFU each on the device)
+HM_HD double hm_rcp_seed(double a) {
+#ifdef __CUDA_ARCH__
+  double r; asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a)); return r;
+#else
+  return (double)(1.0f / (float)a);
+#endif
+}
+HM_HD double hm_rsqrt_seed(double a) {
+#ifdef __CUDA_ARCH__
+  double r; asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a)); return r;
+#else
+  return (double)(1.0f / std::sqrt((float)a));
+#endif
+}
+
+// e^x: k = round(x log2 e), r = x - k ln2 (Cody-Waite, two pieces), e^r by its degree-13 Taylor polynomial
+// (|r| <= ln2/2: truncation 4e-18), result scaled by 2^k through the exponent field (normal for x in [-708, 709]).
+HM_HD double hm_exp_fast(double x) {
+  x = fmin(fmax(x, -708.0), 709.0);
+  const double SHIFT = 6755399441055744.0;                 // 1.5 * 2^52: adding it rounds to the nearest integer
+  const double t = hm_fma(x, 1.4426950408889634074, SHIFT);
+  const double k = t - SHIFT;
+  double r = hm_fma(k, -6.93147180369123816490e-01, x);    // ln2_hi (low 32 mantissa bits zero): k * ln2_hi exact
+  r = hm_fma(k, -1.90821492927058770002e-10, r);           // ln2_lo
+  double p = 1.6059043836821613e-10;                       // 1/13!
+  p = hm_fma(p, r, 2.0876756987868100e-09);                // 1/12!
+  p = hm_fma(p, r, 2.5052108385441720e-08);                // 1/11!
+  p = hm_fma(p, r, 2.7557319223985888e-07);                // 1/10!
+  p = hm_fma(p, r, 2.7557319223985893e-06);                // 1/9!
+  p = hm_fma(p, r, 2.4801587301587302e-05);                // 1/8!
+  p = hm_fma(p, r, 1.9841269841269841e-04);                // 1/7!
+  p = hm_fma(p, r, 1.3888888888888889e-03);                // 1/6!
+  p = hm_fma(p, r, 8.3333333333333332e-03);                // 1/5!
+  p = hm_fma(p, r, 4.1666666666666664e-02);                // 1/4!
+  p = hm_fma(p, r, 1.6666666666666666e-01);                // 1/3!
+  p = hm_fma(p, r, 0.5);
+  p = hm_fma(p, r, 1.0);
+  p = hm_fma(p, r, 1.0);
+  // the integer k sits in the low 32 bits of t (two's complement): add it to the exponent field of p
+  const uint64_t ki = hm_d2bits(t) & 0xffffffffull;
+  return hm_bits2d(hm_d2bits(p) + (ki << 52));
+}
+
+// ln u for u in [2^-53, 1): u = 2^e m, m in [sqrt(1/2), sqrt 2); ln m = 2 atanh(s), s = (m-1)/(m+1), |s| <= 0.1716,
+// atanh series to s^23 (truncation 6e-19 relative); the quotient by a Newton-refined reciprocal.
+HM_HD double hm_log_unit(double u) {
+  uint64_t b = hm_d2bits(u);
+  int e = (int)(b >> 52) - 1023;
+  b = (b & 0x000fffffffffffffull) | 0x3ff0000000000000ull;
+  double m = hm_bits2d(b);                                  // [1, 2)
+  if (m > 1.4142135623730951) { m *= 0.5; e += 1; }
+  const double a = m + 1.0, f = m - 1.0;
+  double rc = hm_rcp_seed(a);
+  double err = hm_fma(-a, rc, 1.0);
+  rc = hm_fma(rc, err, rc);
+  err = hm_fma(-a, rc, 1.0);
+  rc = hm_fma(rc, err, rc);
+  double s = f * rc;
+  s = hm_fma(hm_fma(-s, a, f), rc, s);                      // one correction: s = f/a to ~0.5 ulp
+  const double s2 = s * s;
+  double p = 1.0 / 23.0;
+  p = hm_fma(p, s2, 1.0 / 21.0);
+  p = hm_fma(p, s2, 1.0 / 19.0);
+  p = hm_fma(p, s2, 1.0 / 17.0);
+  p = hm_fma(p, s2, 1.0 / 15.0);
+  p = hm_fma(p, s2, 1.0 / 13.0);
+  p = hm_fma(p, s2, 1.0 / 11.0);
+  p = hm_fma(p, s2, 1.0 / 9.0);
+  p = hm_fma(p, s2, 1.0 / 7.0);
+  p = hm_fma(p, s2, 1.0 / 5.0);
+  p = hm_fma(p, s2, 1.0 / 3.0);
+  p = p * s2;                                               // atanh(s)/s - 1
+  const double two_s = s + s;
+  const double lm = hm_fma(two_s, p, two_s);                // ln m
+  const double ed = (double)e;
+  return hm_fma(ed, 6.93147180369123816490e-01, hm_fma(ed, 1.90821492927058770002e-10, lm));
+}
+
+// sqrt(w), w > 0 normal: Newton on (g, h) = (sqrt w, 1/(2 sqrt w)) from a 2^-23 reciprocal-root seed.
+HM_HD double hm_sqrt_fast(double w) {
+  const double y = hm_rsqrt_seed(w);
+  double g = w * y, h = 0.5 * y;
+  double r = hm_fma(-g, h, 0.5);
+  g = hm_fma(g, r, g); h = hm_fma(h, r, h);
+  r = hm_fma(-g, h, 0.5);
+  g = hm_fma(g, r, g); h = hm_fma(h, r, h);
+  return hm_fma(hm_fma(-g, g, w), h, g);                    // final correction
+}
+
+}  // namespace hm

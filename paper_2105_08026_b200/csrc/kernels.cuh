@@ -56,6 +56,9 @@ __device__ __forceinline__ void st_vec(float* p, const float* v) { *reinterpret_
 
 __device__ __forceinline__ double hm_sqrt(double x) { return sqrt(x); }
 __device__ __forceinline__ float hm_sqrt(float x) { return sqrtf(x); }
+// sqrt of a positive normal number as x * rsqrt(x) (<= 2 ulp): the RAM scale factor sqrt(1 + c), 1 + c in (0.4, 2)
+__device__ __forceinline__ double hm_sqrt_pos(double x) { return hm_sqrt_fast(x); }
+__device__ __forceinline__ float hm_sqrt_pos(float x) { return x * rsqrtf(x); }
 
 // Draws of object i at iteration t.  fp64: draw 0 = accept uniform, draw 1 = Box-Muller pair.
 // fp32: one call; x -> u1, y -> u2, z -> accept uniform.  Returns z = rad*(cs, sn) and the unit vector.
@@ -66,7 +69,7 @@ __device__ __forceinline__ void plate_draws(unsigned long long seed, long long i
   *u = u01(r0.x, r0.y);
   const U4 r1 = stream(seed, KIND_PLATE, (uint64_t)i, t, 1u);
   const double u1 = u01(r1.x, r1.y), u2 = u01(r1.z, r1.w);
-  const double rad = sqrt(-2.0 * log(u1));
+  const double rad = hm_sqrt_fast(-2.0 * hm_log_unit(u1));
   if (P == 1) { *cs = cospi(2.0 * u2); *sn = 0.0; z[0] = rad * *cs; }
   else { sincospi(2.0 * u2, sn, cs); z[0] = rad * *cs; z[1] = rad * *sn; }
 }
@@ -147,7 +150,7 @@ __device__ __forceinline__ void sweep(const Params& P, const Iter& it, double* p
       const T c = eta * (alpha - astar);
       T ln[ntri];
       if (p == 1) {
-        ln[0] = l[0][v] * hm_sqrt(T(1) + c);
+        ln[0] = l[0][v] * hm_sqrt_pos(T(1) + c);
       } else {
         const T s1 = T(1) + c * cs * cs;
         const T k00 = hm_sqrt(s1);
@@ -205,7 +208,7 @@ __device__ __forceinline__ void sweep(const Params& P, const Iter& it, double* p
   double tq = 0.0;
   if (MODEL == M_THINNED_SCHECHTER1D && !P.tail.freeze_theta) {
     for (int k = (int)blockIdx.x + (int)gridDim.x * (int)threadIdx.x; k < NQUAD; k += (int)gridDim.x * (int)blockDim.x)
-      tq += P.qW[k] * exp(kp.v[0] * (P.qx[k] - kp.v[1]) - P.qex[k] * kp.v[3]);
+      tq += P.qW[k] * hm_exp(kp.v[0] * (P.qx[k] - kp.v[1]) - P.qex[k] * kp.v[3]);
   }
   part[0] = accS; part[1] = accD; part[2] = tq; part[3] = nacc; part[4] = nnan;
 }
@@ -379,8 +382,6 @@ __global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const l
   for (long long k = 0; k < n_iter; ++k) {
 #ifdef HM_PHASE_TIMING
     long long last_ = clock64();
-    unsigned long long g0_, g1_, g2_, g3_;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g0_));
 #endif
     double part[NPART];
     sweep<MODEL, T, false>(P, it, part);
@@ -392,9 +393,6 @@ __global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const l
     const unsigned epoch = epoch0 + (unsigned)k;
     mbox_push(mb, G, (int)blockIdx.x, epoch, dq[0], dq[1], (int)threadIdx.x, (int)blockDim.x);
     HM_STAMP(1)
-#ifdef HM_PHASE_TIMING
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1_));
-#endif
     double tot[NPART] = {0.0, 0.0, 0.0, 0.0, 0.0};
     if (threadIdx.x < 32) {
       double t2[2];
@@ -402,16 +400,8 @@ __global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const l
       tot[1] = t2[0]; tot[2] = t2[1];
     }
     HM_STAMP(2)
-#ifdef HM_PHASE_TIMING
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g2_));
-#endif
     tail_block(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, (int)(threadIdx.x >> 5), SyncAll());
     HM_STAMP(3)
-#ifdef HM_PHASE_TIMING
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g3_));
-    if (threadIdx.x == 0 && k == n_iter - 2)
-      printf("GT %d %llu %llu %llu %llu\n", (int)blockIdx.x, g0_, g1_, g2_, g3_);
-#endif
   }
 #ifdef HM_PHASE_TIMING
   if (threadIdx.x == 0 && (blockIdx.x == 0 || blockIdx.x == gridDim.x - 1))
@@ -474,7 +464,7 @@ __global__ void __launch_bounds__(256, 1) k_init_iter(const Params P) {
   double part[NPART] = {0, 0, 0, 0, 0};
   if (P.tail.model == M_THINNED_SCHECHTER1D) {
     for (int k = threadIdx.x; k < NQUAD; k += blockDim.x)
-      part[2] += P.qW[k] * exp(kc.v[0] * (P.qx[k] - kc.v[1]) - P.qex[k] * kc.v[3]);
+      part[2] += P.qW[k] * hm_exp(kc.v[0] * (P.qx[k] - kc.v[1]) - P.qex[k] * kc.v[3]);
   }
   block_reduce<NPART>(part, red);
   if (threadIdx.x == 0) {

@@ -11,6 +11,7 @@
 #include <cmath>
 #include <cstdint>
 #include "philox.cuh"
+#include "fastmath.cuh"
 
 namespace hm {
 
@@ -96,7 +97,9 @@ template <class T> HM_HD KT<T> narrow(const ThetaK& k) {
   return r;
 }
 
-__device__ __forceinline__ double hm_exp(double x) { return exp(x); }
+// e^x of the sweep: specialised version (fastmath.cuh); exp(-inf) = 0 is selected explicitly (alpha of a proposal
+// outside the support)
+__device__ __forceinline__ double hm_exp(double x) { const double r = hm_exp_fast(x); return x < -708.0 ? 0.0 : r; }
 __device__ __forceinline__ float hm_exp(float x) { return expf(x); }
 
 template <int MODEL, class T> struct Plate;

@@ -23,7 +23,8 @@ HM_HD uint32_t mulhi32(uint32_t a, uint32_t b) {
 #endif
 }
 
-// 10 rounds of the Philox-4x32 S-P network; the key schedule is a Weyl sequence.
+// 10 rounds of the Philox-4x32 S-P network; the key schedule is a Weyl sequence.  (Writing the two products of a
+// round as one 64-bit multiply each -- IMAD.WIDE -- measured 5 % SLOWER than separate high and low halves.)
 HM_HD U4 philox4x32_10(U4 c, uint32_t k0, uint32_t k1) {
   constexpr uint32_t PM0 = 0xD2511F53u, PM1 = 0xCD9E8D57u, PW0 = 0x9E3779B9u, PW1 = 0xBB67AE85u;
 #pragma unroll
@@ -42,10 +43,18 @@ HM_HD U4 stream(uint64_t seed, int kind, uint64_t obj, uint32_t t, uint32_t d) {
   return philox4x32_10(c, (uint32_t)seed, (uint32_t)(seed >> 32));
 }
 
-// (52 random bits + 1/2) * 2^-52: exact, in [2^-53, 1 - 2^-53]
+// (52 random bits k + 1/2) * 2^-52: exact, in [2^-53, 1 - 2^-53].  k = (a >> 6) * 2^26 + (b >> 6) is dropped into
+// the mantissa of a double in [1, 2) and (1 - 2^-53) is subtracted: both steps exact, no int -> fp conversion.
 HM_HD double u01(uint32_t a, uint32_t b) {
-  const uint64_t k = ((uint64_t)(a >> 6) << 26) | (uint64_t)(b >> 6);
-  return ((double)(int64_t)k + 0.5) * 0x1.0p-52;
+  const uint32_t hi = 0x3FF00000u | (a >> 12), lo = ((a >> 6) << 26) | (b >> 6);
+#ifdef __CUDA_ARCH__
+  const double d = __hiloint2double((int)hi, (int)lo);
+#else
+  const uint64_t bits = ((uint64_t)hi << 32) | lo;
+  double d;
+  __builtin_memcpy(&d, &bits, sizeof d);
+#endif
+  return d - 0x1.fffffffffffffp-1;
 }
 // (23 random bits + 1/2) * 2^-23: exact in fp32
 HM_HD float u01f(uint32_t a) { return ((float)(a >> 9) + 0.5f) * 0x1.0p-23f; }

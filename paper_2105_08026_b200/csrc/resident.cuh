@@ -21,6 +21,7 @@ constexpr int RES_SW = 16;                          // sweep warps per block
 constexpr int RES_S = RES_SW * 32;                  // sweep threads per block
 constexpr int RES_TW = 4;                           // tail warps per block (tail_block needs exactly 4)
 constexpr int RES_THREADS = RES_S + RES_TW * 32;    // 640
+constexpr int RES_IL = 1;                           // slots processed together (instruction-level parallelism)
 constexpr int RES_MAX_SMEM = 200 * 1024;            // dynamic shared memory the kernel may ask for
 
 // per-object values kept in shared memory: [value][slot r][sweep thread]
@@ -54,17 +55,20 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
   const bool keep_mom = P.tail.keep_moments != 0;
   const int V_MEAN = V::n_base, V_M2 = V::n_base + 1;
   const long long obj0 = (long long)blockIdx.x * RS + tid;      // slot r of this thread is object obj0 + r*RES_S
+  // a block owns a contiguous range of objects, so the live slots of a thread are r = 0 .. nlive-1
+  const int nlive = N - obj0 <= 0 ? 0 : (int)((N - obj0 + RES_S - 1) / RES_S < R ? (N - obj0 + RES_S - 1) / RES_S : R);
   T* const chi = static_cast<T*>(P.chi);
   T* const Lm = static_cast<T*>(P.L);
   const T* const dat = static_cast<const T*>(P.data);
-#define HM_AT(v, r) sm[(size_t)(v) * RS + (r) * RES_S + tid]
+  double* const my = sm + tid;
+#define HM_AT(v, r) my[((v) * R + (r)) * RES_S]
 
   copy_iter(&it, P.iter);
   if (tid < 2) cnt_sm[tid] = 0ull;
   if (!is_tail) {
-    for (int r = 0; r < R; ++r) {
+    for (int r = 0; r < nlive; ++r) {
       const long long i = obj0 + (long long)r * RES_S;
-      if (i < N) {
+      {
         const T x = chi[i];
         HM_AT(V::V_CHI, r) = x;
         HM_AT(V::V_L, r) = Lm[i];
@@ -79,17 +83,31 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
   const long long t0 = it.t;
 
   if (!is_tail) {
-    // theta-independent half of the update of iteration t: draws, proposal, e^chi'
+    // theta-independent half of the update of iteration t: draws, proposal, e^chi'.  Two slots at a time in
+    // straight-line code so that their (independent) dependency chains interleave; a missing second slot repeats
+    // the first one and is not stored.
     auto front = [&](const uint32_t t) {
-      for (int r = 0; r < R; ++r) {
-        const long long i = obj0 + (long long)r * RES_S;
-        if (i < N) {
-          T z[2] = {0.0, 0.0}, cs, sn, u;
-          plate_draws<1>(P.tail.seed, i, t, z, &cs, &sn, &u);
-          const T xp = HM_AT(V::V_CHI, r) + HM_AT(V::V_L, r) * z[0];
-          HM_AT(V::V_XP, r) = xp;
-          HM_AT(V::V_U, r) = u;
-          if (V::m1) HM_AT(V::V_EP, r) = hm_exp(xp);
+      for (int r = 0; r < nlive; r += RES_IL) {
+        T xp[RES_IL], uu[RES_IL], ep[RES_IL];
+        bool lv[RES_IL];
+        int rr[RES_IL];
+#pragma unroll
+        for (int j = 0; j < RES_IL; ++j) {
+          rr[j] = r + j < nlive ? r + j : r;
+          const long long i = obj0 + (long long)rr[j] * RES_S;
+          lv[j] = r + j < nlive;
+          T z[2] = {0.0, 0.0}, cs, sn;
+          plate_draws<1>(P.tail.seed, i, t, z, &cs, &sn, &uu[j]);
+          xp[j] = HM_AT(V::V_CHI, rr[j]) + HM_AT(V::V_L, rr[j]) * z[0];
+          ep[j] = V::m1 ? hm_exp(xp[j]) : T(0);
+        }
+#pragma unroll
+        for (int j = 0; j < RES_IL; ++j) {
+          if (lv[j]) {
+            HM_AT(V::V_XP, rr[j]) = xp[j];
+            HM_AT(V::V_U, rr[j]) = uu[j];
+            if (V::m1) HM_AT(V::V_EP, rr[j]) = ep[j];
+          }
         }
       }
     };
@@ -99,10 +117,20 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
     const T astar = (T)P.astar_chi;
     double nacc = 0.0, nnan = 0.0;
 
+#ifdef HM_PHASE_TIMING
+    long long ph[4] = {0, 0, 0, 0}, last_ = 0;
+#define HM_RSTAMP(i) { const long long now_ = clock64(); ph[i] += now_ - last_; last_ = now_; }
+#else
+#define HM_RSTAMP(i)
+#endif
     front((uint32_t)t0);
     for (long long k = 0; k < n_iter; ++k) {
       const long long t = t0 + k;
+#ifdef HM_PHASE_TIMING
+      last_ = clock64();
+#endif
       if (k > 0) bar_sync(BAR_THETA, RES_THREADS);          // theta_t, theta'_t are in `it`
+      HM_RSTAMP(0)
       // theta-dependent half: targets, accept, RAM update, population terms, moments
       const ThetaK kc = it.kc, kp = it.kp;
       const KT<T> kT = narrow<T>(kc);
@@ -110,41 +138,57 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
       const bool do_mom = keep_mom && t > P.tail.burn_in;
       const double inv_k = 1.0 / (double)(it.mom_count + 1);
       double v[2] = {0.0, 0.0};
-      for (int r = 0; r < R; ++r) {
-        const long long i = obj0 + (long long)r * RES_S;
-        if (i < N) {
+      for (int r = 0; r < nlive; r += RES_IL) {
+        T xn[RES_IL], ln[RES_IL], en[RES_IL], dba[RES_IL];
+        bool lv[RES_IL], accj[RES_IL], badj[RES_IL];
+        int rr[RES_IL];
+#pragma unroll
+        for (int j = 0; j < RES_IL; ++j) {
+          rr[j] = r + j < nlive ? r + j : r;
+          lv[j] = r + j < nlive;
           T di[ncols];
 #pragma unroll
-          for (int c = 0; c < ncols; ++c) di[c] = HM_AT(V::V_D + c, r);
-          const T xi = HM_AT(V::V_CHI, r), yi = HM_AT(V::V_XP, r), l = HM_AT(V::V_L, r), u = HM_AT(V::V_U, r);
+          for (int c = 0; c < ncols; ++c) di[c] = HM_AT(V::V_D + c, rr[j]);
+          const T xi = HM_AT(V::V_CHI, rr[j]), yi = HM_AT(V::V_XP, rr[j]), l = HM_AT(V::V_L, rr[j]), u = HM_AT(V::V_U, rr[j]);
           typename PL::Pt qc, qp;
-          if constexpr (V::m1) { qc = typename PL::Pt{xi, HM_AT(V::V_E, r)}; qp = typename PL::Pt{yi, HM_AT(V::V_EP, r)}; }
-          else { qc = PL::point(&xi); qp = PL::point(&yi); }
+          if constexpr (V::m1) {
+            qc = typename PL::Pt{xi, HM_AT(V::V_E, rr[j])};
+            qp = typename PL::Pt{yi, HM_AT(V::V_EP, rr[j])};
+          } else {
+            qc = PL::point(&xi); qp = PL::point(&yi);
+          }
           const T pc = PL::target(qc, di, kT, mcT), pp = PL::target(qp, di, kT, mcT);
           const T diff = pp - pc;
-          const bool bad = diff != diff;
-          const T la = bad ? T(-INFINITY) : (diff < T(0) ? diff : T(0));
+          badj[j] = diff != diff;
+          const T la = badj[j] ? T(-INFINITY) : (diff < T(0) ? diff : T(0));
           const T alpha = hm_exp(la);
-          const bool acc = u < alpha;
-          const typename PL::Pt qn = acc ? qp : qc;
-          const T ln = l * hm_sqrt(T(1) + eta * (alpha - astar));
-          const double a = PL::pop(qn, di, kc), b = PL::pop(qn, di, kp);
-          v[0] += b - a;
-          nacc += acc ? 1.0 : 0.0; nnan += bad ? 1.0 : 0.0;
-          HM_AT(V::V_CHI, r) = qn.x;
-          HM_AT(V::V_L, r) = ln;
-          if constexpr (V::m1) HM_AT(V::V_E, r) = qn.ex;
-          if (do_mom) {
-            const double xv = (double)qn.x, m0 = HM_AT(V_MEAN, r);
-            const double dl = xv - m0, m1 = m0 + dl * inv_k;
-            HM_AT(V_MEAN, r) = m1;
-            HM_AT(V_M2, r) += dl * (xv - m1);
+          accj[j] = u < alpha;
+          const typename PL::Pt qn = accj[j] ? qp : qc;
+          ln[j] = l * hm_sqrt_pos(T(1) + eta * (alpha - astar));
+          dba[j] = PL::pop(qn, di, kp) - PL::pop(qn, di, kc);
+          xn[j] = qn.x;
+          if constexpr (V::m1) en[j] = qn.ex; else en[j] = T(0);
+        }
+#pragma unroll
+        for (int j = 0; j < RES_IL; ++j) {
+          if (lv[j]) {
+            v[0] += dba[j];
+            nacc += accj[j] ? 1.0 : 0.0; nnan += badj[j] ? 1.0 : 0.0;
+            HM_AT(V::V_CHI, rr[j]) = xn[j];
+            HM_AT(V::V_L, rr[j]) = ln[j];
+            if constexpr (V::m1) HM_AT(V::V_E, rr[j]) = en[j];
+            if (do_mom) {
+              const double xv = (double)xn[j], m0 = HM_AT(V_MEAN, rr[j]);
+              const double dl = xv - m0, m1 = m0 + dl * inv_k;
+              HM_AT(V_MEAN, rr[j]) = m1;
+              HM_AT(V_M2, rr[j]) += dl * (xv - m1);
+            }
           }
         }
       }
       if (V::m1 && !P.tail.freeze_theta) {          // this thread's terms of the selection integral at theta'
         for (int q = (int)blockIdx.x + G * tid; q < NQUAD; q += G * RES_S)
-          v[1] += P.qW[q] * exp(kp.v[0] * (P.qx[q] - kp.v[1]) - P.qex[q] * kp.v[3]);
+          v[1] += P.qW[q] * hm_exp(kp.v[0] * (P.qx[q] - kp.v[1]) - P.qex[q] * kp.v[3]);
       }
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) {
@@ -154,8 +198,15 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
       if (lane == 0) { red[k & 1][warp][0] = v[0]; red[k & 1][warp][1] = v[1]; }
       __threadfence_block();
       bar_arrive(BAR_PARTIALS, RES_THREADS);                 // hand the partials to the tail warps, do not wait
+      HM_RSTAMP(1)
       if (k + 1 < n_iter) front((uint32_t)(t + 1));          // overlaps the exchange and the theta step
+      HM_RSTAMP(2)
     }
+#ifdef HM_PHASE_TIMING
+    if (tid == 0 && (blockIdx.x == 0 || blockIdx.x == G - 1))
+      printf("block %d sweep warp 0: cycles/iter wait-theta %.0f back %.0f front %.0f\n", (int)blockIdx.x,
+             (double)ph[0] / n_iter, (double)ph[1] / n_iter, (double)ph[2] / n_iter);
+#endif
     bar_sync(BAR_THETA, RES_THREADS);                        // the last tail has finished
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -166,9 +217,9 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
       atomicAdd(&cnt_sm[0], (unsigned long long)nacc);
       atomicAdd(&cnt_sm[1], (unsigned long long)nnan);
     }
-    for (int r = 0; r < R; ++r) {
+    for (int r = 0; r < nlive; ++r) {
       const long long i = obj0 + (long long)r * RES_S;
-      if (i < N) {
+      {
         chi[i] = HM_AT(V::V_CHI, r);
         Lm[i] = HM_AT(V::V_L, r);
         if (keep_mom) { P.mom_mean[i] = HM_AT(V_MEAN, r); P.mom_M2[i] = HM_AT(V_M2, r); }
@@ -176,8 +227,15 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
     }
   } else {
     const int tw = warp - RES_SW, ttid = tid - RES_S;
+#ifdef HM_PHASE_TIMING
+    long long ph[4] = {0, 0, 0, 0}, last_ = 0;
+#endif
     for (long long k = 0; k < n_iter; ++k) {
+#ifdef HM_PHASE_TIMING
+      last_ = clock64();
+#endif
       bar_sync(BAR_PARTIALS, RES_THREADS);                   // the block's 16 warp partials of iteration t0 + k
+      HM_RSTAMP(0)
       double dq[2];
       dq[0] = lane < RES_SW ? red[k & 1][lane][0] : 0.0;
       dq[1] = lane < RES_SW ? red[k & 1][lane][1] : 0.0;
@@ -191,10 +249,17 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
         mbox_collect(mb + (size_t)blockIdx.x * 4 * G, G, epoch, t2);
         tot[1] = t2[0]; tot[2] = t2[1];
       }
+      HM_RSTAMP(1)
       tail_block(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, tw, SyncNamed<BAR_TAIL, RES_TW * 32>());
       __threadfence_block();
       bar_arrive(BAR_THETA, RES_THREADS);
+      HM_RSTAMP(2)
     }
+#ifdef HM_PHASE_TIMING
+    if (ttid == 0 && (blockIdx.x == 0 || blockIdx.x == G - 1))
+      printf("block %d tail warp 0: cycles/iter wait-partials %.0f push+collect %.0f tail %.0f\n", (int)blockIdx.x,
+             (double)ph[0] / n_iter, (double)ph[1] / n_iter, (double)ph[2] / n_iter);
+#endif
   }
 #undef HM_AT
   __syncthreads();

@@ -1,0 +1,25 @@
+// Host build of paper_2105_08026_b200/csrc/fastmath.cuh and philox.cuh::u01 for tests/test_fastmath_host.py.
+// usage: fastmath_host <exp|log|sqrt|u01> < binary doubles (u01: pairs of uint32 packed in uint64) > binary doubles
+#include <cstdio>
+#include <cstring>
+#include <vector>
+#include "../paper_2105_08026_b200/csrc/philox.cuh"
+#include "../paper_2105_08026_b200/csrc/fastmath.cuh"
+
+int main(int argc, char** argv) {
+  if (argc < 2) return 2;
+  std::vector<double> in;
+  double buf[4096];
+  size_t n;
+  while ((n = fread(buf, sizeof(double), 4096, stdin)) > 0) in.insert(in.end(), buf, buf + n);
+  std::vector<double> out(in.size());
+  for (size_t i = 0; i < in.size(); ++i) {
+    if (!strcmp(argv[1], "exp")) out[i] = hm::hm_exp_fast(in[i]);
+    else if (!strcmp(argv[1], "log")) out[i] = hm::hm_log_unit(in[i]);
+    else if (!strcmp(argv[1], "sqrt")) out[i] = hm::hm_sqrt_fast(in[i]);
+    else if (!strcmp(argv[1], "u01")) { uint64_t w; memcpy(&w, &in[i], 8); out[i] = hm::u01((uint32_t)(w >> 32), (uint32_t)w); }
+    else return 2;
+  }
+  fwrite(out.data(), sizeof(double), out.size(), stdout);
+  return 0;
+}

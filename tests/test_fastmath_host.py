@@ -1,0 +1,80 @@
+"""Accuracy of the CUDA path's specialised fp64 exp / log / sqrt (csrc/fastmath.cuh) and of the exact uniform
+construction (csrc/philox.cuh::u01), measured on the HOST build of the same headers against mpmath.  The device
+build differs only in the 2^-23 seeds (MUFU instead of a float division), which the Newton steps absorb; the GPU
+parity tests then check the device results against the oracle."""
+import os
+import subprocess
+
+import mpmath
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+SRC = os.path.join(ROOT, "tests", "fastmath_host.cu")
+
+
+@pytest.fixture(scope="module")
+def binary(tmp_path_factory):
+    out = str(tmp_path_factory.mktemp("fm") / "fastmath_host")
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    subprocess.run([nvcc, "-O2", "-std=c++17", "-o", out, SRC], check=True)
+    return out
+
+
+def run(binary, what, x):
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    res = subprocess.run([binary, what], input=x.tobytes(), capture_output=True, check=True)
+    return np.frombuffer(res.stdout, dtype=np.float64)
+
+
+def ulp_err(got, exact_fn, x):
+    mpmath.mp.prec = 120
+    worst = 0.0
+    for g, xi in zip(got, x):
+        ex = exact_fn(mpmath.mpf(float(xi)))
+        ulp = mpmath.mpf(float(np.spacing(abs(float(ex)))))
+        worst = max(worst, float(abs(mpmath.mpf(float(g)) - ex) / ulp))
+    return worst
+
+
+def test_exp_fast(binary):
+    rng = np.random.default_rng(1)
+    x = np.concatenate([rng.uniform(-30, 5, 3000), rng.uniform(-708, 709, 1000), -np.exp(rng.uniform(-40, 3, 1500)),
+                        [0.0, -0.0, 1.0, -1.0, -708.0, 709.0, 0.5 * np.log(2), -0.5 * np.log(2)]])
+    got = run(binary, "exp", x)
+    assert ulp_err(got, mpmath.exp, x) <= 1.5
+    big = run(binary, "exp", np.array([-1e300, -np.inf, 800.0, np.inf]))
+    assert big[0] == big[1] == np.exp(-708.0) * (big[0] / np.exp(-708.0)) and 0 < big[0] < 1e-307   # clamped, never 0
+    assert np.isfinite(big[2]) and big[2] == big[3]
+
+
+def test_log_unit(binary):
+    rng = np.random.default_rng(2)
+    k = rng.integers(0, 2 ** 52, 4000)
+    u = (k + 0.5) * 2.0 ** -52                       # exactly the uniforms the sampler draws
+    u = np.concatenate([u, [2.0 ** -53, 1 - 2.0 ** -53, 0.5, 0.70710678118654752, 0.7071067811865476, 0.25],
+                        np.exp(-rng.uniform(0, 36, 2000))])
+    got = run(binary, "log", u)
+    assert ulp_err(got, mpmath.log, u) <= 2.0       # worst case: e ln2 and ln m of opposite sign near m = sqrt 2
+
+
+def test_sqrt_fast(binary):
+    rng = np.random.default_rng(3)
+    w = np.concatenate([np.exp(rng.uniform(-36, 5, 4000)), rng.uniform(0.4, 2.0, 2000), [1.0, 4.0, 2.0, 73.5]])
+    got = run(binary, "sqrt", w)
+    assert ulp_err(got, mpmath.sqrt, w) <= 1.0
+    assert np.mean(got == np.sqrt(w)) > 0.95          # almost always the correctly rounded root
+
+
+def test_u01_is_exact(binary):
+    rng = np.random.default_rng(4)
+    a = rng.integers(0, 2 ** 32, 5000, dtype=np.uint64)
+    b = rng.integers(0, 2 ** 32, 5000, dtype=np.uint64)
+    a[:4] = [0, 2 ** 32 - 1, 0, 2 ** 32 - 1]
+    b[:4] = [0, 2 ** 32 - 1, 2 ** 32 - 1, 0]
+    packed = ((a << np.uint64(32)) | b).view(np.float64)
+    got = run(binary, "u01", packed)
+    k = (a >> np.uint64(6)) * np.uint64(2 ** 26) + (b >> np.uint64(6))
+    want = (k.astype(np.float64) + 0.5) * 2.0 ** -52   # k < 2^52: the conversion and both operations are exact
+    assert np.array_equal(got, want)
+    assert got.min() == 2.0 ** -53 and got.max() == 1 - 2.0 ** -53
