@@ -7,7 +7,7 @@
 // instructions:
 //   hm_exp_fast(x)   any finite x (clamped to [-708, 709]); x = -inf gives exp(-708) ~ 3e-308, NOT 0 (callers that
 //                    need exp(-inf) = 0 select it themselves)
-//   hm_log_unit(u)   u in [2^-53, 1): positive normal numbers only
+//   hm_log_pos(x)    positive normal numbers only (the Box-Muller uniforms u in [2^-53, 1); 1 + alpha^2 of the prior)
 //   hm_sqrt_fast(w)  w > 0 normal
 // tests/test_fastmath_host.py measures their error against mpmath on the host build of this very header.
 #pragma once
@@ -88,9 +88,9 @@ HM_HD double hm_exp_fast(double x) {
   return hm_bits2d(hm_d2bits(p) + (ki << 52));
 }
 
-// ln u for u in [2^-53, 1): u = 2^e m, m in [sqrt(1/2), sqrt 2); ln m = 2 atanh(s), s = (m-1)/(m+1), |s| <= 0.1716,
+// ln u for positive normal u: u = 2^e m, m in [sqrt(1/2), sqrt 2); ln m = 2 atanh(s), s = (m-1)/(m+1), |s| <= 0.1716,
 // atanh series to s^23 (truncation 6e-19 relative); the quotient by a Newton-refined reciprocal.
-HM_HD double hm_log_unit(double u) {
+HM_HD double hm_log_pos(double u) {
   uint64_t b = hm_d2bits(u);
   int e = (int)(b >> 52) - 1023;
   b = (b & 0x000fffffffffffffull) | 0x3ff0000000000000ull;
@@ -123,6 +123,8 @@ HM_HD double hm_log_unit(double u) {
   return hm_fma(ed, 6.93147180369123816490e-01, hm_fma(ed, 1.90821492927058770002e-10, lm));
 }
 
+HM_HD double hm_log_unit(double u) { return hm_log_pos(u); }   // u in [2^-53, 1)
+
 // sqrt(w), w > 0 normal: Newton on (g, h) = (sqrt w, 1/(2 sqrt w)) from a 2^-23 reciprocal-root seed.
 HM_HD double hm_sqrt_fast(double w) {
   const double y = hm_rsqrt_seed(w);
@@ -132,6 +134,24 @@ HM_HD double hm_sqrt_fast(double w) {
   r = hm_fma(-g, h, 0.5);
   g = hm_fma(g, r, g); h = hm_fma(h, r, h);
   return hm_fma(hm_fma(-g, g, w), h, g);                    // final correction
+}
+
+// exp / log of the theta tail: the specialised versions on the device (the tail is a serial chain on the critical
+// path of every iteration), libm on the host (THETA_HOST).
+HM_HD double hm_exp_any(double x) {
+#ifdef __CUDA_ARCH__
+  const double r = hm_exp_fast(x);
+  return x < -708.0 ? 0.0 : (x != x ? x : r);
+#else
+  return std::exp(x);
+#endif
+}
+HM_HD double hm_log_any_pos(double x) {
+#ifdef __CUDA_ARCH__
+  return hm_log_pos(x);
+#else
+  return std::log(x);
+#endif
 }
 
 }  // namespace hm

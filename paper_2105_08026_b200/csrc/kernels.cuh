@@ -450,6 +450,7 @@ __global__ void __launch_bounds__(TAIL_THREADS, 1) k_tail(const Params P, const 
   }
   if (flags & TAIL_DECIDE) {
     tail_block(it, P.tail, tot, P.trace, (int)(threadIdx.x >> 5), SyncAll());
+    __syncthreads();
     copy_iter(P.iter, &it);
   }
 }

@@ -43,17 +43,17 @@ struct ThetaK { double v[8]; };
 HM_HD void theta_consts_part(int model, int part, const double* th, ThetaK& k) {
   switch (model) {
     case M_NORMAL1D:            // (mu, lambda): f = -lambda - (chi - mu)^2 * [e^(-2 lambda)/2]
-      if (part == 0) { k.v[0] = th[0]; k.v[1] = th[1]; k.v[2] = 0.5 * exp(-2.0 * th[1]); }
+      if (part == 0) { k.v[0] = th[0]; k.v[1] = th[1]; k.v[2] = 0.5 * hm_exp_any(-2.0 * th[1]); }
       break;
     case M_LINREG_ME1D:         // (a, b, lambda): f = -lambda - (chi - a - b z)^2 * [e^(-2 lambda)/2]
-      if (part == 0) { k.v[0] = th[0]; k.v[1] = th[1]; k.v[2] = th[2]; k.v[3] = 0.5 * exp(-2.0 * th[2]); }
+      if (part == 0) { k.v[0] = th[0]; k.v[1] = th[1]; k.v[2] = th[2]; k.v[3] = 0.5 * hm_exp_any(-2.0 * th[2]); }
       break;
     case M_THINNED_SCHECHTER1D: // (alpha, x*, a): f = a + (alpha+1)(chi - x*) - e^chi e^(-x*);  v[4] = A = e^a
-      if (part == 0) { k.v[0] = th[0] + 1.0; k.v[1] = th[1]; k.v[2] = th[2]; k.v[3] = exp(-th[1]); }
-      if (part == 1) k.v[4] = exp(th[2]);
+      if (part == 0) { k.v[0] = th[0] + 1.0; k.v[1] = th[1]; k.v[2] = th[2]; k.v[3] = hm_exp_any(-th[1]); }
+      if (part == 1) k.v[4] = hm_exp_any(th[2]);
       break;
     case M_BINORMAL2D:          // (m1, m2, l1, l2, zeta): f = c0 - h (u1^2 - 2 rho u1 u2 + u2^2)
-      if (part == 0) { k.v[0] = th[0]; k.v[1] = th[1]; k.v[2] = exp(-th[2]); k.v[3] = exp(-th[3]); }
+      if (part == 0) { k.v[0] = th[0]; k.v[1] = th[1]; k.v[2] = hm_exp_any(-th[2]); k.v[3] = hm_exp_any(-th[3]); }
       if (part == 1) { const double ch = cosh(th[4]); k.v[4] = -th[2] - th[3] + log(ch); k.v[5] = 0.5 * ch * ch; }
       if (part == 2) k.v[6] = tanh(th[4]);
       break;
@@ -81,7 +81,7 @@ HM_HD double log_prior(int model, const double* th) {
               fabs(th[4]) <= 10.0) ? 0.0 : ninf;
     case M_THINNED_SCHECHTER1D:
       return (th[0] > -2.0 && th[0] < 0.0 && fabs(th[1]) <= 20.0 && fabs(th[2]) <= 50.0)
-                 ? -log1p(th[0] * th[0]) : ninf;
+                 ? -hm_log_any_pos(1.0 + th[0] * th[0]) : ninf;
   }
   return ninf;
 }

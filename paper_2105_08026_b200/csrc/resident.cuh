@@ -17,10 +17,13 @@
 
 namespace hm {
 
-constexpr int RES_SW = 16;                          // sweep warps per block
+#ifndef HM_RES_SW
+#define HM_RES_SW 16
+#endif
+constexpr int RES_SW = HM_RES_SW;                   // sweep warps per block
 constexpr int RES_S = RES_SW * 32;                  // sweep threads per block
 constexpr int RES_TW = 4;                           // tail warps per block (tail_block needs exactly 4)
-constexpr int RES_THREADS = RES_S + RES_TW * 32;    // 640
+constexpr int RES_THREADS = RES_S + RES_TW * 32;    // 640 with 16 sweep warps
 constexpr int RES_IL = 1;                           // slots processed together (instruction-level parallelism)
 constexpr int RES_MAX_SMEM = 200 * 1024;            // dynamic shared memory the kernel may ask for
 

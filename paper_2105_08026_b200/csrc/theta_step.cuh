@@ -34,6 +34,7 @@ struct Iter {
   Draws dr[3];                        // slots t%3 (iteration t) and (t+1)%3 are valid; (t+2)%3 is scratch
   ThetaK kc, kp;                      // theta-derived constants at theta / theta'
   double T_cur, lp_cur, lp_prop;      // theta-only term and log prior at theta; log prior at theta'
+  double lp_prop_next;                // staging slot of the block-parallel tail
   // taps of the last decision (debug_step / host mode read them)
   double S, Delta, T_prop, log_r, alpha_theta, u_theta, T_cur_used, lp_cur_used, tap_thetaP[MAXD];
   long long t;                        // the PREPARED iteration (1-based): t-1 iterations are complete
@@ -134,7 +135,7 @@ HM_HD void decide_scalars(const Iter& it, const TailCfg& c, const Draws& d, doub
     *log_r = Delta + (*T_prop - it.T_cur) + (it.lp_prop - it.lp_cur);
     la = (*log_r != *log_r) ? -INFINITY : fmin(0.0, *log_r);
   }
-  *alpha = exp(la);
+  *alpha = hm_exp_any(la);
   *acc = d.u < *alpha ? 1 : 0;
 }
 
@@ -215,11 +216,16 @@ __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const dou
   const Draws& d0 = it.dr[r0];
   const Draws& d1 = it.dr[r1];
   Draws& d2 = it.dr[r2];
+#ifdef HM_PHASE_TIMING
+  const long long tc0_ = clock64();
+  long long tc1_ = 0, tc2_ = 0, tc3_ = 0;
+#endif
 
+  // decision scalars stay in warp 0's registers until phase C, where the taps are written (off the critical path)
+  double T_prop = 0.0, log_r = 0.0, alpha = 0.0;
+  int acc = 0;
   if (warp == 0) {
     if (!c.freeze_theta) {
-      double T_prop, log_r, alpha;
-      int acc;
       decide_scalars(it, c, d0, tot[1], tot[2], &T_prop, &log_r, &alpha, &acc);
       const double cc = d0.eta * (alpha - c.astar_theta);
       double Kd = 1.0, g = 0.0;
@@ -237,19 +243,10 @@ __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const dou
       if (lane < 8 && acc) it.kc.v[lane] = kpv;
       __syncwarp();
       if (lane < dt) it.thetaP[lane] = propose_entry(it, d1, lane);
-      if (lane == 0) {
-        it.T_cur_used = it.T_cur; it.lp_cur_used = it.lp_cur;
-        it.T_prop = T_prop; it.log_r = log_r; it.alpha_theta = alpha; it.u_theta = d0.u;
-        it.accepted_theta = acc;
-        it.theta_prop_n += 1;
-        if (acc) { it.theta_acc += 1; it.T_cur = T_prop; it.lp_cur = it.lp_prop; }
-      }
-    } else if (lane == 0) {
-      it.accepted_theta = 0;
-      it.T_prop = 0.0; it.log_r = 0.0; it.alpha_theta = 0.0; it.u_theta = 0.0;
-      it.T_cur_used = it.T_cur; it.lp_cur_used = it.lp_cur;
     }
-    if (lane == 1) decide_counters(it, tot[0], tot[1], tot[3], tot[4]);
+#ifdef HM_PHASE_TIMING
+    tc1_ = clock64();
+#endif
   } else if (warp == 1) {
     if (!c.freeze_theta) {
       if (2 * lane < dt) {
@@ -280,25 +277,50 @@ __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const dou
     }
   }
   sync();
+#ifdef HM_PHASE_TIMING
+  tc2_ = clock64();
+#endif
   if (!c.freeze_theta) {
-    if (warp < 3) {
-      if (lane == 0) theta_consts_part(c.model, warp, it.thetaP, it.kp);
-      if (warp == 1 && lane < nt) {
-        const int ei = tri_row(lane), ej = lane - ei * (ei + 1) / 2;
-        it.W[lane] = make_W_entry(it, d1, ei, ej);
+    if (warp >= 1) {
+      if (lane == 0) theta_consts_part(c.model, warp - 1, it.thetaP, it.kp);
+      if (warp == 1 && lane >= 1 && lane <= nt) {
+        const int e = lane - 1, ei = tri_row(e), ej = e - ei * (ei + 1) / 2;
+        it.W[e] = make_W_entry(it, d1, ei, ej);
       }
-    } else if (warp == 3) {
-      if (lane == 0) it.lp_prop = log_prior(c.model, it.thetaP);
+      if (warp == 3 && lane == 0) it.lp_prop_next = log_prior(c.model, it.thetaP);
+    } else if (lane == 0) {               // warp 0: taps and acceptance bookkeeping of the decision just taken
+      it.T_cur_used = it.T_cur; it.lp_cur_used = it.lp_cur;
+      it.T_prop = T_prop; it.log_r = log_r; it.alpha_theta = alpha; it.u_theta = d0.u;
+      it.accepted_theta = acc;
+      it.theta_prop_n += 1;
+      if (acc) { it.theta_acc += 1; it.T_cur = T_prop; it.lp_cur = it.lp_prop; }
+      decide_counters(it, tot[0], tot[1], tot[3], tot[4]);
     }
-  } else if (warp == 0 && lane < 8) {
-    it.kp.v[lane] = it.kc.v[lane];
+  } else if (warp == 0) {
+    if (lane < 8) it.kp.v[lane] = it.kc.v[lane];
     if (lane < dt) it.thetaP[lane] = it.theta[lane];
-    if (lane == 0) it.lp_prop = it.lp_cur;
+    if (lane == 0) {
+      it.lp_prop_next = it.lp_cur;
+      it.accepted_theta = 0;
+      it.T_prop = 0.0; it.log_r = 0.0; it.alpha_theta = 0.0; it.u_theta = 0.0;
+      it.T_cur_used = it.T_cur; it.lp_cur_used = it.lp_cur;
+      decide_counters(it, tot[0], tot[1], tot[3], tot[4]);
+    }
   }
   if (warp == 2 && trace_or_null && it.trace_write && lane < dt)
     trace_or_null[(it.trace_rows - 1) * dt + lane] = it.theta[lane];
   if (warp == 3 && lane == 1) it.t = t + 1;
+#ifdef HM_PHASE_TIMING
+  tc3_ = clock64();
+#endif
   sync();
+  // warp 0 read it.lp_prop (the decided iteration's) during phase C, so the next one is moved in only now; the
+  // next reader is the decision of iteration t + 1, at least one block barrier away
+  if (warp == 3 && lane == 0) it.lp_prop = it.lp_prop_next;
+#ifdef HM_PHASE_TIMING
+  if (warp == 0 && lane == 0 && blockIdx.x == 0 && (t % 100) == 0)
+    printf("tail t=%lld: decide %lld  wait-sync1 %lld  phaseC %lld  sync2 %lld\n", t, tc1_ - tc0_, tc2_ - tc1_, tc3_ - tc2_, clock64() - tc3_);
+#endif
 }
 #endif
 

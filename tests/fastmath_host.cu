@@ -15,7 +15,7 @@ int main(int argc, char** argv) {
   std::vector<double> out(in.size());
   for (size_t i = 0; i < in.size(); ++i) {
     if (!strcmp(argv[1], "exp")) out[i] = hm::hm_exp_fast(in[i]);
-    else if (!strcmp(argv[1], "log")) out[i] = hm::hm_log_unit(in[i]);
+    else if (!strcmp(argv[1], "log")) out[i] = hm::hm_log_pos(in[i]);
     else if (!strcmp(argv[1], "sqrt")) out[i] = hm::hm_sqrt_fast(in[i]);
     else if (!strcmp(argv[1], "u01")) { uint64_t w; memcpy(&w, &in[i], 8); out[i] = hm::u01((uint32_t)(w >> 32), (uint32_t)w); }
     else return 2;

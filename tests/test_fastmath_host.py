@@ -48,12 +48,12 @@ def test_exp_fast(binary):
     assert np.isfinite(big[2]) and big[2] == big[3]
 
 
-def test_log_unit(binary):
+def test_log_pos(binary):
     rng = np.random.default_rng(2)
     k = rng.integers(0, 2 ** 52, 4000)
     u = (k + 0.5) * 2.0 ** -52                       # exactly the uniforms the sampler draws
     u = np.concatenate([u, [2.0 ** -53, 1 - 2.0 ** -53, 0.5, 0.70710678118654752, 0.7071067811865476, 0.25],
-                        np.exp(-rng.uniform(0, 36, 2000))])
+                        np.exp(-rng.uniform(0, 36, 2000)), rng.uniform(1.0, 5.0, 1000), [1.0, 2.0, 1e300, 3e-308]])
     got = run(binary, "log", u)
     assert ulp_err(got, mpmath.log, u) <= 2.0       # worst case: e ln2 and ln m of opposite sign near m = sqrt 2
 
