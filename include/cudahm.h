@@ -56,7 +56,9 @@ enum { CUDAHM_THETA_HOST = 0,         /* one sweep launch + one sync per iterati
 
 /* cudahm_config.flags: THETA_DEVICE_TAIL keeps a population that fits in shared memory on chip for the whole run
  * (fp64, p = 1 models); this flag forces the HBM-streaming persistent kernel instead. */
-enum { CUDAHM_FLAG_STREAMING_ONLY = 1 };
+enum { CUDAHM_FLAG_STREAMING_ONLY = 1,
+       CUDAHM_FLAG_TMA_STAGING = 2 };  /* stream through TMA-staged shared-memory tiles (stream_tma.cuh) instead of
+                                          plain vector loads; measured slower on C3 / C4, kept as an option          */
 
 typedef struct {
   uint32_t struct_size;          /* sizeof(cudahm_config), checked                                          */
@@ -74,7 +76,7 @@ typedef struct {
   int32_t  keep_chi_moments;     /* 1: running mean / variance of every chi component after burn-in         */
   int32_t  block_threads;        /* 0 = default; else 256, 512 or 1024                                      */
   int32_t  blocks_per_sm;        /* 0 = as many as fit; else an upper limit                                 */
-  int32_t  flags;                /* 0, or CUDAHM_FLAG_STREAMING_ONLY                                        */
+  int32_t  flags;                /* 0, or CUDAHM_FLAG_* ORed                                                */
   int64_t  max_trace_rows;       /* capacity of the on-device thinned theta trace (rows of dtheta doubles);
                                     0 = keep no trace                                                        */
 } cudahm_config;

@@ -75,6 +75,10 @@ def lib():
         fp = C.POINTER(C.c_float)
         L.oracle_draws_f32.argtypes = [C.c_uint64, C.c_int, C.c_uint64, C.c_uint32, fp, fp]
         L.oracle_draws_f32.restype = None
+        L.oracle_plate_draws_f64.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_int, _dp, _dp]
+        L.oracle_plate_draws_f64.restype = None
+        L.oracle_plate_draws_f32.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_int, fp, fp]
+        L.oracle_plate_draws_f32.restype = None
         L.oracle_loglik.argtypes = [C.c_int, _dp, _dp, _dp]
         L.oracle_loglik.restype = C.c_double
         L.oracle_logpop.argtypes = [C.c_int, _dp, _dp, _dp, _dp]
@@ -250,6 +254,21 @@ def draws_f32(seed, kind, obj, t):
     u = C.c_float()
     lib().oracle_draws_f32(seed, kind, obj, t, z, C.byref(u))
     return np.float32(z[0]), np.float32(z[1]), np.float32(u.value)
+
+
+def plate_draws_f64(seed, i, t, p):
+    """(z[0..p-1], accept uniform) of object i at iteration t."""
+    z = np.zeros(max(p, 2))
+    u = C.c_double()
+    lib().oracle_plate_draws_f64(seed, i, t, p, _d(z), C.byref(u))
+    return z[:p].copy(), u.value
+
+
+def plate_draws_f32(seed, i, t, p):
+    z = (C.c_float * 2)()
+    u = C.c_float()
+    lib().oracle_plate_draws_f32(seed, i, t, p, z, C.byref(u))
+    return np.array([z[k] for k in range(p)], dtype=np.float32), np.float32(u.value)
 
 
 def loglik(model, chi, data_i, consts=None):

@@ -102,6 +102,9 @@ void   oracle_stream_words(uint64_t seed, int kind, uint64_t obj, uint32_t t, ui
 double oracle_uniform_f64(uint64_t seed, int kind, uint64_t obj, uint32_t t, uint32_t d);
 void   oracle_normals_f64(uint64_t seed, int kind, uint64_t obj, uint32_t t, int n, double* z);
 void   oracle_draws_f32(uint64_t seed, int kind, uint64_t obj, uint32_t t, float* z2, float* u);
+/* the p normals and the accept uniform of object i at iteration t (objects draw in pairs: oracle/rng.hpp) */
+void   oracle_plate_draws_f64(uint64_t seed, uint64_t i, uint32_t t, int p, double* z, double* u);
+void   oracle_plate_draws_f32(uint64_t seed, uint64_t i, uint32_t t, int p, float* z, float* u);
 double oracle_loglik(int model, const double* chi, const double* data_i, const double* consts);
 double oracle_logpop(int model, const double* chi, const double* data_i, const double* theta,
                      const double* consts);

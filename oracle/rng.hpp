@@ -85,4 +85,43 @@ inline void draws_f32(uint64_t seed, int kind, uint64_t obj, uint32_t t, float z
   *u = u01_f32(r.w[2]);
 }
 
+// ---- plate-level draws of object i at iteration t --------------------------------
+// Objects are taken in PAIRS m = i >> 1, h = i & 1, so that one Philox call and one Box-Muller evaluation
+// serve two objects (both branches of Box-Muller are independent N(0,1) variates; nothing is discarded).
+//   fp64  accept uniform: draw 0 of PAIR m -- words (w0,w1) for h = 0, (w2,w3) for h = 1.
+//         p = 1 normal:   draw 1 of PAIR m -- u1 from (w0,w1), u2 from (w2,w3), radius sqrt(-2 ln u1);
+//                         z = radius cos(2 pi u2) for h = 0, radius sin(2 pi u2) for h = 1.
+//         p >= 2 normals: per OBJECT, draws 1+k of object i exactly as normals_f64.
+//   fp32  p = 1: ONE call per pair, draw 0 of PAIR m: w0 -> u1, w1 -> u2, z = cos / sin branch for h = 0 / 1,
+//                accept uniform from w2 (h = 0) / w3 (h = 1).
+//         p = 2: per OBJECT as draws_f32.
+inline void plate_draws_f64(uint64_t seed, uint64_t i, uint32_t t, int p, double* z, double* u) {
+  const double two_pi = 6.283185307179586476925286766559;
+  const uint64_t m = i >> 1;
+  const int h = (int)(i & 1);
+  const Words a = stream_words(seed, 0 /* PLATE */, m, t, 0u);
+  *u = h ? u01_f64(a.w[2], a.w[3]) : u01_f64(a.w[0], a.w[1]);
+  if (p == 1) {
+    const Words b = stream_words(seed, 0, m, t, 1u);
+    const double u1 = u01_f64(b.w[0], b.w[1]);
+    const double u2 = u01_f64(b.w[2], b.w[3]);
+    const double rad = std::sqrt(-2.0 * std::log(u1));
+    z[0] = h ? rad * std::sin(two_pi * u2) : rad * std::cos(two_pi * u2);
+  } else {
+    normals_f64(seed, 0, i, t, p, z);
+  }
+}
+inline void plate_draws_f32(uint64_t seed, uint64_t i, uint32_t t, int p, float* z, float* u) {
+  if (p != 1) { draws_f32(seed, 0, i, t, z, u); return; }
+  const float two_pi = 6.283185307179586476925286766559f;
+  const uint64_t m = i >> 1;
+  const int h = (int)(i & 1);
+  const Words r = stream_words(seed, 0, m, t, 0u);
+  const float u1 = u01_f32(r.w[0]);
+  const float u2 = u01_f32(r.w[1]);
+  const float rad = std::sqrt(-2.0f * std::log(u1));
+  z[0] = h ? rad * std::sin(two_pi * u2) : rad * std::cos(two_pi * u2);
+  *u = u01_f32(h ? r.w[3] : r.w[2]);
+}
+
 }  // namespace oracle

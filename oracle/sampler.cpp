@@ -174,13 +174,13 @@ struct Impl : Base {
       for (int k = 0; k < nt; ++k) l[k] = L[(size_t)k * N + i];
       for (int c = 0; c < nc; ++c) d[c] = data[(size_t)c * N + i];
       if (sizeof(T) == 8) {
-        double zz[2] = {0, 0};
-        normals_f64(cfg.seed, ORACLE_KIND_PLATE, (uint64_t)i, tcur, p, zz);
+        double zz[2] = {0, 0}, uu = 0;
+        plate_draws_f64(cfg.seed, (uint64_t)i, tcur, p, zz, &uu);
         z[0] = (T)zz[0]; z[1] = (T)zz[1];
-        u = (T)accept_uniform_f64(cfg.seed, ORACLE_KIND_PLATE, (uint64_t)i, tcur);
+        u = (T)uu;
       } else {
-        float zf[2], uf;
-        draws_f32(cfg.seed, ORACLE_KIND_PLATE, (uint64_t)i, tcur, zf, &uf);
+        float zf[2] = {0.0f, 0.0f}, uf;
+        plate_draws_f32(cfg.seed, (uint64_t)i, tcur, p, zf, &uf);
         z[0] = (T)zf[0]; z[1] = (T)zf[1]; u = (T)uf;
         if (p == 1) z[1] = T(0);
       }
@@ -431,6 +431,12 @@ void oracle_normals_f64(uint64_t seed, int kind, uint64_t obj, uint32_t t, int n
 }
 void oracle_draws_f32(uint64_t seed, int kind, uint64_t obj, uint32_t t, float* z2, float* u) {
   draws_f32(seed, kind, obj, t, z2, u);
+}
+void oracle_plate_draws_f64(uint64_t seed, uint64_t i, uint32_t t, int p, double* z, double* u) {
+  plate_draws_f64(seed, i, t, p, z, u);
+}
+void oracle_plate_draws_f32(uint64_t seed, uint64_t i, uint32_t t, int p, float* z, float* u) {
+  plate_draws_f32(seed, i, t, p, z, u);
 }
 double oracle_loglik(int model, const double* chi, const double* d, const double* consts) {
   return loglik<double>(model, chi, d, consts);

@@ -16,7 +16,7 @@ OK, E_INVALID, E_STATE, E_CUDA, E_WORKSPACE, E_UNSUPPORTED, E_NONFINITE = 0, -1,
 M_NORMAL1D, M_THINNED_SCHECHTER1D, M_BINORMAL2D, M_LINREG_ME1D = 0, 1, 2, 3
 F64, F32_STATE_F64_REDUCE = 0, 1
 THETA_HOST, THETA_GRAPH, THETA_DEVICE_TAIL = 0, 1, 2
-FLAG_STREAMING_ONLY = 1
+FLAG_STREAMING_ONLY, FLAG_TMA_STAGING = 1, 2
 FLOOR_LAUNCH, FLOOR_GRAPH, FLOOR_GRID_BARRIER, FLOOR_HOST_SYNC = 0, 1, 2, 3
 
 EXPORTS = ["cudahm_model_dims", "cudahm_workspace_bytes", "cudahm_create", "cudahm_destroy", "cudahm_set_data",

@@ -13,6 +13,7 @@
 
 #include "kernels.cuh"
 #include "resident.cuh"
+#include "stream_tma.cuh"
 
 using namespace hm;
 
@@ -31,6 +32,8 @@ inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct KernelSet {
   const void* persistent;
+  const void* persistent_tma;
+  size_t tma_stage_bytes;
   const void* sweep;
   const void* sweep_tap;
   const void* init_state;
@@ -40,6 +43,8 @@ template <int MODEL, class T, int BLOCK>
 KernelSet make_set() {
   KernelSet k;
   k.persistent = (const void*)k_persistent<MODEL, T, BLOCK>;
+  k.persistent_tma = (const void*)k_persistent_tma<MODEL, T, BLOCK>;
+  k.tma_stage_bytes = (size_t)(ModelDims<MODEL>::p * (ModelDims<MODEL>::p + 3) / 2 + ModelDims<MODEL>::ncols) * (BLOCK - 32) * 16;
   k.sweep = (const void*)k_sweep<MODEL, T, BLOCK, false>;
   k.sweep_tap = (const void*)k_sweep<MODEL, T, BLOCK, true>;
   k.init_state = (const void*)k_init_state<MODEL, T>;
@@ -109,6 +114,7 @@ struct cudahm_sampler {
   const void* res_kernel = nullptr; // on-chip persistent kernel (resident.cuh) when the population fits, else NULL
   int res_R = 0; size_t res_smem = 0;
   int sweep_grid = 1, sweep_block = 512;   // launch shape of k_sweep (THETA_GRAPH / HOST / debug_step)
+  int tma_stages = 0; size_t tma_smem = 0;   // > 0: the streaming persistent kernel is k_persistent_tma
   double h_lp_prop_before = 0.0;    // log prior at theta' of the iteration debug_step is about to decide
   // CUDA-graph cache (THETA_GRAPH)
   cudaGraphExec_t gexec = nullptr;
@@ -139,7 +145,7 @@ bool valid_config(const cudahm_config* c, int* p, int* dt, int* nc, int* nk) {
   if (!c || c->struct_size != sizeof(cudahm_config)) return false;
   if (!model_dims(c->model, p, dt, nc, nk)) return false;
   if (c->p != *p || c->dtheta != *dt || c->n_data_cols != *nc) return false;
-  if (c->n_objects < 0 || c->max_trace_rows < 0 || (c->flags & ~CUDAHM_FLAG_STREAMING_ONLY) != 0) return false;
+  if (c->n_objects < 0 || c->max_trace_rows < 0 || (c->flags & ~(CUDAHM_FLAG_STREAMING_ONLY | CUDAHM_FLAG_TMA_STAGING)) != 0) return false;
   if (c->precision != CUDAHM_F64 && c->precision != CUDAHM_F32_STATE_F64_REDUCE) return false;
   if (c->theta_mode < CUDAHM_THETA_HOST || c->theta_mode > CUDAHM_THETA_DEVICE_TAIL) return false;
   if (!(c->target_accept_chi > 0.0 && c->target_accept_chi < 1.0)) return false;
@@ -231,13 +237,26 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
   s->grid = std::min(s->grid, MAX_BLOCKS);
   if (cfg->theta_mode == CUDAHM_THETA_DEVICE_TAIL && s->grid > MAX_PGRID) s->grid = std::max(1, MAX_PGRID / sms) * sms;
   s->sweep_grid = s->grid; s->sweep_block = block;
+  // HBM-streaming variant with TMA-staged loads (stream_tma.cuh), opt-in: measured 10-30 % slower than plain vector
+  // loads on C3 / C4 (the sweep is issue-bound, not latency-bound, and the producer warp costs a sweep warp)
+  if (cfg->theta_mode == CUDAHM_THETA_DEVICE_TAIL && (cfg->flags & CUDAHM_FLAG_TMA_STAGING) && block <= 512) {
+    int stages = (int)std::min<size_t>(TMA_MAX_STAGES, (size_t)(200 * 1024) / ks.tma_stage_bytes);
+    if (stages >= 2 && cudaFuncSetAttribute(ks.persistent_tma, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                            (int)(stages * ks.tma_stage_bytes)) == cudaSuccess) {
+      s->tma_stages = stages; s->tma_smem = stages * ks.tma_stage_bytes;
+      const long long tiles = (cfg->n_objects + (long long)s->vec * (block - 32) - 1) / ((long long)s->vec * (block - 32));
+      s->grid = (int)std::max(1LL, std::min<long long>(sms, tiles));
+    } else {
+      cudaGetLastError();
+    }
+  }
   // on-chip variant: every object stays in the shared memory of its block for the whole launch
   if (cfg->theta_mode == CUDAHM_THETA_DEVICE_TAIL && !(cfg->flags & CUDAHM_FLAG_STREAMING_ONLY) && cfg->n_objects > 0) {
     int nv = 0;
     const void* rk = pick_resident(cfg->model, cfg->precision, cfg->keep_chi_moments, &nv);
     if (rk) {
       const long long g = std::min<long long>(sms, (cfg->n_objects + RES_S - 1) / RES_S);
-      const long long R = (cfg->n_objects + g * RES_S - 1) / (g * RES_S);
+      const long long R = 2 * ((cfg->n_objects + 2 * g * RES_S - 1) / (2 * g * RES_S));   // slots per thread, in pairs
       const size_t bytes = (size_t)nv * R * RES_S * sizeof(double);
       if (bytes <= (size_t)RES_MAX_SMEM &&
           cudaFuncSetAttribute(rk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) == cudaSuccess) {
@@ -473,6 +492,13 @@ int run_device_tail(cudahm_sampler* s, long long n_iter) {
     if (s->res_kernel) {
       cudaError_t e = cudaLaunchCooperativeKernel(s->res_kernel, dim3(s->grid), dim3(RES_THREADS), args, s->res_smem, s->stream);
       if (e != cudaSuccess) return fail(s, CUDAHM_E_CUDA, "resident kernel launch: %s", cudaGetErrorString(e));
+      s->launches++;
+      rc = CUDAHM_OK;
+    } else if (s->tma_stages > 0) {
+      int st = s->tma_stages;
+      void* targs[] = {&P, &k, &epoch0, &st};
+      cudaError_t e = cudaLaunchCooperativeKernel(s->ks.persistent_tma, dim3(s->grid), dim3(s->block), targs, s->tma_smem, s->stream);
+      if (e != cudaSuccess) return fail(s, CUDAHM_E_CUDA, "streaming kernel launch: %s", cudaGetErrorString(e));
       s->launches++;
       rc = CUDAHM_OK;
     } else {

@@ -60,33 +60,195 @@ __device__ __forceinline__ float hm_sqrt(float x) { return sqrtf(x); }
 __device__ __forceinline__ double hm_sqrt_pos(double x) { return hm_sqrt_fast(x); }
 __device__ __forceinline__ float hm_sqrt_pos(float x) { return x * rsqrtf(x); }
 
-// Draws of object i at iteration t.  fp64: draw 0 = accept uniform, draw 1 = Box-Muller pair.
-// fp32: one call; x -> u1, y -> u2, z -> accept uniform.  Returns z = rad*(cs, sn) and the unit vector.
+// Plate-level draws.  Objects draw in PAIRS m = i >> 1 so that one Philox call and one
+// Box-Muller evaluation serve two objects (both Box-Muller branches are independent N(0,1); nothing is wasted):
+//   fp64  accept uniforms: draw 0 of pair m -- (x,y) for the even object, (z,w) for the odd one;
+//         p = 1 normals:   draw 1 of pair m -- cos branch for the even object, sin branch for the odd one;
+//         p = 2 normals:   per object, draw 1 of object i; z = rad*(cs, sn), unit vector (cs, sn).
+//   fp32  p = 1: one call per pair (draw 0 of pair m): x -> u1, y -> u2, cos / sin branch, accept uniforms z / w.
+// i0 is the even object of the pair.  z[h][k]: normal k of object i0 + h.
 template <int P>
-__device__ __forceinline__ void plate_draws(unsigned long long seed, long long i, uint32_t t, double* z, double* cs,
-                                            double* sn, double* u) {
-  const U4 r0 = stream(seed, KIND_PLATE, (uint64_t)i, t, 0u);
-  *u = u01(r0.x, r0.y);
-  const U4 r1 = stream(seed, KIND_PLATE, (uint64_t)i, t, 1u);
-  const double u1 = u01(r1.x, r1.y), u2 = u01(r1.z, r1.w);
-  const double rad = hm_sqrt_fast(-2.0 * hm_log_unit(u1));
-  if (P == 1) { *cs = cospi(2.0 * u2); *sn = 0.0; z[0] = rad * *cs; }
-  else { sincospi(2.0 * u2, sn, cs); z[0] = rad * *cs; z[1] = rad * *sn; }
+__device__ __forceinline__ void pair_draws(unsigned long long seed, long long i0, uint32_t t, double (*z)[2], double* cs,
+                                           double* sn, double* u) {
+  const uint64_t m = (uint64_t)i0 >> 1;
+  const U4 a = stream(seed, KIND_PLATE, m, t, 0u);
+  u[0] = u01(a.x, a.y); u[1] = u01(a.z, a.w);
+  if (P == 1) {
+    const U4 b = stream(seed, KIND_PLATE, m, t, 1u);
+    const double u1 = u01(b.x, b.y), u2 = u01(b.z, b.w);
+    const double rad = hm_sqrt_fast(-2.0 * hm_log_unit(u1));
+    double s_, c_;
+    sincospi(2.0 * u2, &s_, &c_);
+    z[0][0] = rad * c_; z[1][0] = rad * s_;
+    z[0][1] = 0.0; z[1][1] = 0.0;
+    cs[0] = cs[1] = 0.0; sn[0] = sn[1] = 0.0;      // the unit vector is not needed for p = 1
+  } else {
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const U4 b = stream(seed, KIND_PLATE, (uint64_t)(i0 + h), t, 1u);
+      const double u1 = u01(b.x, b.y), u2 = u01(b.z, b.w);
+      const double rad = hm_sqrt_fast(-2.0 * hm_log_unit(u1));
+      sincospi(2.0 * u2, &sn[h], &cs[h]);
+      z[h][0] = rad * cs[h]; z[h][1] = rad * sn[h];
+    }
+  }
 }
 template <int P>
-__device__ __forceinline__ void plate_draws(unsigned long long seed, long long i, uint32_t t, float* z, float* cs,
-                                            float* sn, float* u) {
-  const U4 r = stream(seed, KIND_PLATE, (uint64_t)i, t, 0u);
-  const float u1 = u01f(r.x), u2 = u01f(r.y);
-  *u = u01f(r.z);
-  const float rad = sqrtf(-2.0f * logf(u1));
-  if (P == 1) { *cs = cospif(2.0f * u2); *sn = 0.0f; z[0] = rad * *cs; }
-  else { sincospif(2.0f * u2, sn, cs); z[0] = rad * *cs; z[1] = rad * *sn; }
+__device__ __forceinline__ void pair_draws(unsigned long long seed, long long i0, uint32_t t, float (*z)[2], float* cs,
+                                           float* sn, float* u) {
+  if (P == 1) {
+    const U4 r = stream(seed, KIND_PLATE, (uint64_t)i0 >> 1, t, 0u);
+    const float u1 = u01f(r.x), u2 = u01f(r.y);
+    u[0] = u01f(r.z); u[1] = u01f(r.w);
+    const float rad = hm_sqrt_pos(-2.0f * logf(u1));
+    float s_, c_;
+    sincospif(2.0f * u2, &s_, &c_);
+    z[0][0] = rad * c_; z[1][0] = rad * s_;
+    z[0][1] = 0.0f; z[1][1] = 0.0f;
+    cs[0] = cs[1] = 0.0f; sn[0] = sn[1] = 0.0f;
+  } else {
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {                  // per object: x -> u1, y -> u2, z -> accept uniform
+      const U4 r = stream(seed, KIND_PLATE, (uint64_t)(i0 + h), t, 0u);
+      const float u1 = u01f(r.x), u2 = u01f(r.y);
+      u[h] = u01f(r.z);
+      const float rad = hm_sqrt_pos(-2.0f * logf(u1));
+      sincospif(2.0f * u2, &sn[h], &cs[h]);
+      z[h][0] = rad * cs[h]; z[h][1] = rad * sn[h];
+    }
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------
 // The sweep.  Fixed thread -> object map: at step k the thread with global index gid owns the VEC
 // consecutive objects starting at VEC*(k*nthreads + gid): unit-stride 16-byte loads/stores per column.
+
+// per-iteration constants of the sweep, in registers
+template <class T> struct SweepCtx {
+  uint32_t t;
+  ThetaK kc, kp;
+  KT<T> kT;
+  T mcT[7];
+  T eta, astar;
+  bool do_mom;
+  double inv_k;
+};
+template <class T>
+__device__ __forceinline__ SweepCtx<T> make_ctx(const Params& P, const Iter& it) {
+  SweepCtx<T> c;
+  c.t = (uint32_t)it.t;
+  c.kc = it.kc; c.kp = it.kp;
+  c.kT = narrow<T>(c.kc);
+#pragma unroll
+  for (int j = 0; j < 7; ++j) c.mcT[j] = (T)P.mc[j];
+  c.eta = (T)it.dr[it.t % 3].eta; c.astar = (T)P.astar_chi;
+  c.do_mom = P.tail.keep_moments && it.t > P.tail.burn_in;
+  c.inv_k = 1.0 / (double)(it.mom_count + 1);
+  return c;
+}
+
+// RAM steps 1-3 + population terms + moments for the VEC objects base .. base+VEC-1 held in x, l (updated in
+// place; the caller stores them) and d.  acc = {S, Delta, n_accept, n_nonfinite} of this thread.
+template <int MODEL, class T, bool TAP>
+__device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c, const long long base,
+                                           T (*x)[VecOf<T>::n], T (*l)[VecOf<T>::n], const T (*d)[VecOf<T>::n], double* sum) {
+  constexpr int p = ModelDims<MODEL>::p, ntri = p * (p + 1) / 2, ncols = ModelDims<MODEL>::ncols;
+  constexpr int VEC = VecOf<T>::n;
+  T zz[VEC][2], csv[VEC], snv[VEC], uu[VEC];
+#pragma unroll
+  for (int v = 0; v < VEC; v += 2) pair_draws<p>(P.tail.seed, base + v, c.t, &zz[v], &csv[v], &snv[v], &uu[v]);
+#pragma unroll
+  for (int v = 0; v < VEC; ++v) {
+    const long long i = base + v;
+    const bool live = i < P.N;
+    T xi[p], di[ncols];
+    const T cs = csv[v], sn = snv[v], u = uu[v];
+    const T* z = zz[v];
+#pragma unroll
+    for (int j = 0; j < p; ++j) xi[j] = x[j][v];
+#pragma unroll
+    for (int q = 0; q < ncols; ++q) di[q] = d[q][v];
+    // step 1: chi' = chi + L z
+    T yi[p];
+    yi[0] = xi[0] + l[0][v] * z[0];
+    if (p == 2) yi[1] = xi[1] + l[1][v] * z[0] + l[2][v] * z[1];
+    // step 2: alpha = min{1, pi(chi')/pi(chi)}
+    using PL = Plate<MODEL, T>;
+    const typename PL::Pt qc = PL::point(xi), qp = PL::point(yi);
+    const T pc = PL::target(qc, di, c.kT, c.mcT), pp = PL::target(qp, di, c.kT, c.mcT);
+    const T diff = pp - pc;
+    const bool bad = diff != diff;
+    const T la = bad ? T(-INFINITY) : (diff < T(0) ? diff : T(0));
+    const T alpha = hm_exp(la);
+    const bool acc = u < alpha;
+    const typename PL::Pt qn = acc ? qp : qc;
+#pragma unroll
+    for (int j = 0; j < p; ++j) x[j][v] = acc ? yi[j] : xi[j];
+    // step 3: L <- L chol(I + c uu^T), u = z/|z| = (cs, sn)
+    const T cc = c.eta * (alpha - c.astar);
+    T ln[ntri];
+    if (p == 1) {
+      ln[0] = l[0][v] * hm_sqrt_pos(T(1) + cc);
+    } else {
+      const T s1 = T(1) + cc * cs * cs;
+      const T k00 = hm_sqrt(s1);
+      const T k10 = cc * cs * sn / k00;
+      const T k11 = hm_sqrt((T(1) + cc) / s1);
+      ln[0] = l[0][v] * k00;
+      ln[1] = l[1][v] * k00 + l[2][v] * k10;
+      ln[2] = l[2][v] * k11;
+    }
+    // population terms at the new chi, fp64
+    const double a = PL::pop(qn, di, c.kc), b = PL::pop(qn, di, c.kp);
+    if (live) {
+#pragma unroll
+      for (int k = 0; k < ntri; ++k) l[k][v] = ln[k];
+      sum[0] += a; sum[1] += b - a;
+      sum[2] += acc ? 1.0 : 0.0; sum[3] += bad ? 1.0 : 0.0;
+      if (c.do_mom) {
+#pragma unroll
+        for (int j = 0; j < p; ++j) {
+          const long long q = j * P.Npad + i;
+          const double xv = (double)x[j][v];
+          const double m0 = P.mom_mean[q];
+          const double dl = xv - m0;
+          const double m1 = m0 + dl * c.inv_k;
+          P.mom_mean[q] = m1;
+          P.mom_M2[q] += dl * (xv - m1);
+        }
+      }
+      if (TAP) {
+        const DevTaps& tp = P.taps;
+#pragma unroll
+        for (int j = 0; j < p; ++j) if (tp.chi_prop) tp.chi_prop[j * P.N + i] = (double)yi[j];
+        if (tp.pi_cur) tp.pi_cur[i] = (double)pc;
+        if (tp.pi_prop) tp.pi_prop[i] = (double)pp;
+        if (tp.alpha) tp.alpha[i] = (double)alpha;
+        if (tp.u) tp.u[i] = (double)u;
+        if (tp.accepted) tp.accepted[i] = acc ? 1 : 0;
+#pragma unroll
+        for (int k = 0; k < ntri; ++k) if (tp.L_new) tp.L_new[k * P.N + i] = (double)ln[k];
+        if (tp.a) tp.a[i] = a;
+        if (tp.b) tp.b[i] = b;
+      }
+    } else {
+#pragma unroll
+      for (int j = 0; j < p; ++j) x[j][v] = xi[j];
+    }
+  }
+}
+
+// selection-integral slice (M1): term k belongs to block k % gridDim.x, thread k / gridDim.x
+template <int MODEL>
+__device__ __forceinline__ double selection_slice(const Params& P, const ThetaK& kp, const int sweep_threads) {
+  double tq = 0.0;
+  if (MODEL == M_THINNED_SCHECHTER1D && !P.tail.freeze_theta) {
+    for (int k = (int)blockIdx.x + (int)gridDim.x * (int)threadIdx.x; k < NQUAD; k += (int)gridDim.x * sweep_threads)
+      tq += P.qW[k] * hm_exp(kp.v[0] * (P.qx[k] - kp.v[1]) - P.qex[k] * kp.v[3]);
+  }
+  return tq;
+}
+
 // part[NPART] receives this thread's partial sums in ascending object order.
 template <int MODEL, class T, bool TAP>
 __device__ __forceinline__ void sweep(const Params& P, const Iter& it, double* part) {
@@ -98,19 +260,8 @@ __device__ __forceinline__ void sweep(const Params& P, const Iter& it, double* p
   T* const chi = static_cast<T*>(P.chi);
   T* const Lm = static_cast<T*>(P.L);
   const T* const dat = static_cast<const T*>(P.data);
-
-  const uint32_t t = (uint32_t)it.t;
-  const ThetaK kc = it.kc, kp = it.kp;
-  const KT<T> kT = narrow<T>(kc);
-  T mcT[7];
-#pragma unroll
-  for (int j = 0; j < 7; ++j) mcT[j] = (T)P.mc[j];
-  const T eta = (T)it.dr[it.t % 3].eta, astar = (T)P.astar_chi;
-  const bool do_mom = P.tail.keep_moments && it.t > P.tail.burn_in;
-  const double inv_k = 1.0 / (double)(it.mom_count + 1);
-
-  double accS = 0.0, accD = 0.0, nacc = 0.0, nnan = 0.0;
-
+  const SweepCtx<T> c = make_ctx<T>(P, it);
+  double acc[4] = {0.0, 0.0, 0.0, 0.0};
   for (long long base = (long long)VEC * gid; base < N; base += (long long)VEC * nthreads) {
     T x[p][VEC], l[ntri][VEC], d[ncols][VEC];
 #pragma unroll
@@ -118,99 +269,14 @@ __device__ __forceinline__ void sweep(const Params& P, const Iter& it, double* p
 #pragma unroll
     for (int k = 0; k < ntri; ++k) ld_vec<T>(Lm + k * Npad + base, l[k], false);
 #pragma unroll
-    for (int c = 0; c < ncols; ++c) ld_vec<T>(dat + c * Npad + base, d[c], true);
-
-#pragma unroll
-    for (int v = 0; v < VEC; ++v) {
-      const long long i = base + v;
-      const bool live = i < N;
-      T xi[p], di[ncols], z[2] = {T(0), T(0)}, cs, sn, u;
-#pragma unroll
-      for (int j = 0; j < p; ++j) xi[j] = x[j][v];
-#pragma unroll
-      for (int c = 0; c < ncols; ++c) di[c] = d[c][v];
-      plate_draws<p>(P.tail.seed, i, t, z, &cs, &sn, &u);
-      // step 1: chi' = chi + L z
-      T yi[p];
-      yi[0] = xi[0] + l[0][v] * z[0];
-      if (p == 2) yi[1] = xi[1] + l[1][v] * z[0] + l[2][v] * z[1];
-      // step 2: alpha = min{1, pi(chi')/pi(chi)}
-      using PL = Plate<MODEL, T>;
-      const typename PL::Pt qc = PL::point(xi), qp = PL::point(yi);
-      const T pc = PL::target(qc, di, kT, mcT), pp = PL::target(qp, di, kT, mcT);
-      const T diff = pp - pc;
-      const bool bad = diff != diff;
-      const T la = bad ? T(-INFINITY) : (diff < T(0) ? diff : T(0));
-      const T alpha = hm_exp(la);
-      const bool acc = u < alpha;
-      const typename PL::Pt qn = acc ? qp : qc;
-#pragma unroll
-      for (int j = 0; j < p; ++j) x[j][v] = acc ? yi[j] : xi[j];
-      // step 3: L <- L chol(I + c uu^T), u = z/|z| = (cs, sn)
-      const T c = eta * (alpha - astar);
-      T ln[ntri];
-      if (p == 1) {
-        ln[0] = l[0][v] * hm_sqrt_pos(T(1) + c);
-      } else {
-        const T s1 = T(1) + c * cs * cs;
-        const T k00 = hm_sqrt(s1);
-        const T k10 = c * cs * sn / k00;
-        const T k11 = hm_sqrt((T(1) + c) / s1);
-        ln[0] = l[0][v] * k00;
-        ln[1] = l[1][v] * k00 + l[2][v] * k10;
-        ln[2] = l[2][v] * k11;
-      }
-      // population terms at the new chi, fp64
-      const double a = PL::pop(qn, di, kc), b = PL::pop(qn, di, kp);
-      if (live) {
-#pragma unroll
-        for (int k = 0; k < ntri; ++k) l[k][v] = ln[k];
-        accS += a; accD += b - a;
-        nacc += acc ? 1.0 : 0.0; nnan += bad ? 1.0 : 0.0;
-        if (do_mom) {
-#pragma unroll
-          for (int j = 0; j < p; ++j) {
-            const long long q = j * Npad + i;
-            const double xv = (double)x[j][v];
-            const double m0 = P.mom_mean[q];
-            const double dl = xv - m0;
-            const double m1 = m0 + dl * inv_k;
-            P.mom_mean[q] = m1;
-            P.mom_M2[q] += dl * (xv - m1);
-          }
-        }
-        if (TAP) {
-          const DevTaps& tp = P.taps;
-#pragma unroll
-          for (int j = 0; j < p; ++j) if (tp.chi_prop) tp.chi_prop[j * N + i] = (double)yi[j];
-          if (tp.pi_cur) tp.pi_cur[i] = (double)pc;
-          if (tp.pi_prop) tp.pi_prop[i] = (double)pp;
-          if (tp.alpha) tp.alpha[i] = (double)alpha;
-          if (tp.u) tp.u[i] = (double)u;
-          if (tp.accepted) tp.accepted[i] = acc ? 1 : 0;
-#pragma unroll
-          for (int k = 0; k < ntri; ++k) if (tp.L_new) tp.L_new[k * N + i] = (double)ln[k];
-          if (tp.a) tp.a[i] = a;
-          if (tp.b) tp.b[i] = b;
-        }
-      } else {
-#pragma unroll
-        for (int j = 0; j < p; ++j) x[j][v] = xi[j];
-      }
-    }
+    for (int cc = 0; cc < ncols; ++cc) ld_vec<T>(dat + cc * Npad + base, d[cc], true);
+    update_vec<MODEL, T, TAP>(P, c, base, x, l, d, acc);
 #pragma unroll
     for (int j = 0; j < p; ++j) st_vec(chi + j * Npad + base, x[j]);
 #pragma unroll
     for (int k = 0; k < ntri; ++k) st_vec(Lm + k * Npad + base, l[k]);
   }
-
-  // selection-integral slice (M1): term k belongs to block k % gridDim.x, thread k / gridDim.x
-  double tq = 0.0;
-  if (MODEL == M_THINNED_SCHECHTER1D && !P.tail.freeze_theta) {
-    for (int k = (int)blockIdx.x + (int)gridDim.x * (int)threadIdx.x; k < NQUAD; k += (int)gridDim.x * (int)blockDim.x)
-      tq += P.qW[k] * hm_exp(kp.v[0] * (P.qx[k] - kp.v[1]) - P.qex[k] * kp.v[3]);
-  }
-  part[0] = accS; part[1] = accD; part[2] = tq; part[3] = nacc; part[4] = nnan;
+  part[0] = acc[0]; part[1] = acc[1]; part[2] = selection_slice<MODEL>(P, c.kp, (int)blockDim.x); part[3] = acc[2]; part[4] = acc[3];
 }
 
 // Deterministic block reduction of NQ quantities: shuffle tree inside each warp, then warp 0 over the per-warp

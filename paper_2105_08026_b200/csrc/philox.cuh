@@ -56,8 +56,18 @@ HM_HD double u01(uint32_t a, uint32_t b) {
 #endif
   return d - 0x1.fffffffffffffp-1;
 }
-// (23 random bits + 1/2) * 2^-23: exact in fp32
-HM_HD float u01f(uint32_t a) { return ((float)(a >> 9) + 0.5f) * 0x1.0p-23f; }
+// (23 random bits k + 1/2) * 2^-23: exact in fp32; k goes into the mantissa of a float in [1, 2), then 1 - 2^-24 is
+// subtracted (both steps exact, no int -> fp conversion)
+HM_HD float u01f(uint32_t a) {
+  const uint32_t bits = 0x3f800000u | (a >> 9);
+#ifdef __CUDA_ARCH__
+  return __uint_as_float(bits) - 0x1.fffffep-1f;
+#else
+  float f;
+  __builtin_memcpy(&f, &bits, sizeof f);
+  return f - 0x1.fffffep-1f;
+#endif
+}
 
 // Box-Muller pair from one Philox call (fp64): u1 from (x,y), u2 from (z,w).
 // Returns radius and the unit vector (cos, sin)(2 pi u2): z = rad * (c, s) and z/|z| = (c, s).

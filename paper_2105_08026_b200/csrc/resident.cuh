@@ -57,9 +57,12 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
   const int RS = R * RES_S;
   const bool keep_mom = P.tail.keep_moments != 0;
   const int V_MEAN = V::n_base, V_M2 = V::n_base + 1;
-  const long long obj0 = (long long)blockIdx.x * RS + tid;      // slot r of this thread is object obj0 + r*RES_S
-  // a block owns a contiguous range of objects, so the live slots of a thread are r = 0 .. nlive-1
-  const int nlive = N - obj0 <= 0 ? 0 : (int)((N - obj0 + RES_S - 1) / RES_S < R ? (N - obj0 + RES_S - 1) / RES_S : R);
+  // A block owns the contiguous objects [blockIdx.x * RS, (blockIdx.x + 1) * RS); a thread owns adjacent PAIRS of
+  // them (objects draw in pairs, kernels.cuh::pair_draws): slot r = 2a + h is object obj0 + 2 a RES_S + h.  R is even.
+  const long long obj0 = (long long)blockIdx.x * RS + 2 * tid;
+#define HM_OBJ(r) (obj0 + (long long)((r) >> 1) * (2 * RES_S) + ((r) & 1))
+  int nlive = 0;                                                  // HM_OBJ increases with r: live slots are 0 .. nlive-1
+  for (int r = 0; r < R; ++r) nlive += HM_OBJ(r) < N ? 1 : 0;
   T* const chi = static_cast<T*>(P.chi);
   T* const Lm = static_cast<T*>(P.L);
   const T* const dat = static_cast<const T*>(P.data);
@@ -70,7 +73,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
   if (tid < 2) cnt_sm[tid] = 0ull;
   if (!is_tail) {
     for (int r = 0; r < nlive; ++r) {
-      const long long i = obj0 + (long long)r * RES_S;
+      const long long i = HM_OBJ(r);
       {
         const T x = chi[i];
         HM_AT(V::V_CHI, r) = x;
@@ -86,30 +89,18 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
   const long long t0 = it.t;
 
   if (!is_tail) {
-    // theta-independent half of the update of iteration t: draws, proposal, e^chi'.  Two slots at a time in
-    // straight-line code so that their (independent) dependency chains interleave; a missing second slot repeats
-    // the first one and is not stored.
+    // theta-independent half of the update of iteration t: pair draws, proposals, e^chi'
     auto front = [&](const uint32_t t) {
-      for (int r = 0; r < nlive; r += RES_IL) {
-        T xp[RES_IL], uu[RES_IL], ep[RES_IL];
-        bool lv[RES_IL];
-        int rr[RES_IL];
+      for (int r = 0; r < nlive; r += 2) {
+        T z[2][2], cs[2], sn[2], u[2];
+        pair_draws<1>(P.tail.seed, HM_OBJ(r), t, z, cs, sn, u);
 #pragma unroll
-        for (int j = 0; j < RES_IL; ++j) {
-          rr[j] = r + j < nlive ? r + j : r;
-          const long long i = obj0 + (long long)rr[j] * RES_S;
-          lv[j] = r + j < nlive;
-          T z[2] = {0.0, 0.0}, cs, sn;
-          plate_draws<1>(P.tail.seed, i, t, z, &cs, &sn, &uu[j]);
-          xp[j] = HM_AT(V::V_CHI, rr[j]) + HM_AT(V::V_L, rr[j]) * z[0];
-          ep[j] = V::m1 ? hm_exp(xp[j]) : T(0);
-        }
-#pragma unroll
-        for (int j = 0; j < RES_IL; ++j) {
-          if (lv[j]) {
-            HM_AT(V::V_XP, rr[j]) = xp[j];
-            HM_AT(V::V_U, rr[j]) = uu[j];
-            if (V::m1) HM_AT(V::V_EP, rr[j]) = ep[j];
+        for (int h = 0; h < 2; ++h) {
+          if (r + h < nlive) {
+            const T xp = HM_AT(V::V_CHI, r + h) + HM_AT(V::V_L, r + h) * z[h][0];
+            HM_AT(V::V_XP, r + h) = xp;
+            HM_AT(V::V_U, r + h) = u[h];
+            if (V::m1) HM_AT(V::V_EP, r + h) = hm_exp(xp);
           }
         }
       }
@@ -221,7 +212,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
       atomicAdd(&cnt_sm[1], (unsigned long long)nnan);
     }
     for (int r = 0; r < nlive; ++r) {
-      const long long i = obj0 + (long long)r * RES_S;
+      const long long i = HM_OBJ(r);
       {
         chi[i] = HM_AT(V::V_CHI, r);
         Lm[i] = HM_AT(V::V_L, r);
@@ -265,6 +256,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
 #endif
   }
 #undef HM_AT
+#undef HM_OBJ
   __syncthreads();
   if (tid == 0) {
     P.blk_cnt[2 * blockIdx.x] += cnt_sm[0];

@@ -99,12 +99,14 @@ def test_free_running_matches_oracle(model, astar, n, mode):
 
 def test_theta_modes_agree():
     """Same grid, same thread->object map, same reduction order in the three streaming drivers.  GRAPH and the
-    streaming DEVICE_TAIL kernel run the theta step with the same device code => identical bits.  HOST runs it
-    with the host libm (exp, pow, sincos differ from the device's by ulps) and the on-chip DEVICE_TAIL kernel
-    (resident.cuh) adds the block partials in another fixed order: both agree to rounding, not bitwise."""
+    plain-load streaming DEVICE_TAIL kernel run the theta step with the same device code => identical bits.  HOST
+    runs it with the host libm (exp, pow, sincos differ from the device's by ulps); the on-chip kernel
+    (resident.cuh) and the TMA-staged streaming kernel (stream_tma.cuh) own objects in other fixed orders: they
+    agree to rounding, not bitwise."""
     out = []
-    for mode, flags in ((B.THETA_HOST, 0), (B.THETA_GRAPH, 0), (B.THETA_DEVICE_TAIL, B.FLAG_STREAMING_ONLY),
-                        (B.THETA_DEVICE_TAIL, 0)):
+    for mode, flags in ((B.THETA_HOST, 0), (B.THETA_GRAPH, 0),
+                        (B.THETA_DEVICE_TAIL, B.FLAG_STREAMING_ONLY),
+                        (B.THETA_DEVICE_TAIL, 0), (B.THETA_DEVICE_TAIL, B.FLAG_STREAMING_ONLY | B.FLAG_TMA_STAGING)):
         _, gpu, _ = make_pair(B.M_THINNED_SCHECHTER1D, 5000, seed=5, theta_mode=mode, max_trace_rows=130,
                               want_oracle=False, flags=flags)
         gpu.run(130, 0, 1, sync=True)
@@ -112,19 +114,20 @@ def test_theta_modes_agree():
         out.append((s["chi"], s["L"], s["theta"], s["L_theta"], gpu.get_theta_trace()))
     for a, b in zip(out[1], out[2]):
         assert np.array_equal(a, b)
-    for other in (out[0], out[3]):
+    for other in (out[0], out[3], out[4]):
         for a, b in zip(other, out[2]):
             np.testing.assert_allclose(a, b, rtol=1e-9, atol=1e-10)
 
 
+@pytest.mark.parametrize("flags", [B.FLAG_STREAMING_ONLY | B.FLAG_TMA_STAGING, B.FLAG_STREAMING_ONLY], ids=["tma", "ldg"])
 @pytest.mark.parametrize("model,astar,n", [(B.M_NORMAL1D, 0.44, 1000), (B.M_THINNED_SCHECHTER1D, 0.44, 3000),
-                                             (B.M_LINREG_ME1D, 0.44, 70001)], ids=["M0", "M1", "M3"])
-def test_streaming_persistent_kernel_matches_oracle(model, astar, n):
+                                             (B.M_LINREG_ME1D, 0.44, 150001)], ids=["M0", "M1", "M3"])
+def test_streaming_persistent_kernel_matches_oracle(model, astar, n, flags):
     """The HBM-streaming persistent kernel (what C3 / C4 and any population too large for shared memory run),
     forced on the small fp64 p=1 cases that would otherwise take the on-chip kernel."""
     iters, burn, thin = 100, 20, 5
     orc, gpu, _ = make_pair(model, n, seed=41 + model, astar=astar, keep_moments=True, precision=B.F64,
-                            max_trace_rows=(iters - burn) // thin, flags=B.FLAG_STREAMING_ONLY)
+                            max_trace_rows=(iters - burn) // thin, flags=flags)
     orc.run(iters, burn, thin)
     gpu.run(iters, burn, thin, sync=True)
     so, sg = orc.get_state(), gpu.get_state()

@@ -143,10 +143,10 @@ def test_accept_rule_and_alpha_definition():
     np.testing.assert_allclose(tp["alpha"], np.minimum(1.0, np.exp(tp["pi_prop"] - tp["pi_cur"])), rtol=1e-14)
     assert np.array_equal(tp["accepted"], (tp["u"] < tp["alpha"]).astype(np.int32))
     assert 0 < tp["accepted"].sum() < n
-    z = np.array([O.normals_f64(25, O.KIND_PLATE, i, 21, 1)[0] for i in range(n)])
+    draws = [O.plate_draws_f64(25, i, 21, 1) for i in range(n)]      # pinned in test_oracle_rng.py
+    z = np.array([d[0][0] for d in draws])
     np.testing.assert_allclose(tp["chi_prop"][0], before["chi"][0] + before["L"][0] * z, rtol=1e-15)
-    u = np.array([O.uniform_f64(25, O.KIND_PLATE, i, 21, 0) for i in range(n)])
-    assert np.array_equal(tp["u"], u)
+    assert np.array_equal(tp["u"], np.array([d[1] for d in draws]))
     np.testing.assert_array_equal(after["chi"][0], np.where(tp["accepted"] == 1, tp["chi_prop"][0], before["chi"][0]))
     # pi is l_i * f: check against the separately pinned log-densities
     i = 7

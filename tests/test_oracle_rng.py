@@ -126,6 +126,77 @@ def test_normals_are_a_function_of_the_documented_words():
     assert abs(z5[4] - float(mp.sqrt(-2 * mp.log(u1)) * mp.cos(2 * mp.pi * u2))) < 1e-14
 
 
+def _u52(wa, wb):
+    import mpmath as mp
+    return mp.mpf(2 * (((wa >> 6) << 26) | (wb >> 6)) + 1) / mp.mpf(2) ** 53
+
+
+def test_plate_draws_f64_are_the_documented_function_of_the_pair_words():
+    """objects draw in pairs m = i >> 1.  Accept uniform: draw 0 of pair m, words (w0,w1) for
+    the even object and (w2,w3) for the odd one.  p = 1 normal: draw 1 of pair m, cos branch for the even object,
+    sin branch for the odd one.  p = 2 normals: per object, draws 1.. of object i.  Evaluated with mpmath."""
+    import mpmath as mp
+    mp.mp.dps = 40
+    for i, t in ((0, 1), (1, 1), (17, 9), (299_998, 10_000), (299_999, 10_000), (2 ** 33 + 5, 3)):
+        m, h = i >> 1, i & 1
+        a = O.stream_words(9, O.KIND_PLATE, m, t, 0)
+        b = O.stream_words(9, O.KIND_PLATE, m, t, 1)
+        z, u = O.plate_draws_f64(9, i, t, 1)
+        assert u == float(_u52(a[2], a[3]) if h else _u52(a[0], a[1]))
+        u1, u2 = _u52(b[0], b[1]), _u52(b[2], b[3])
+        r = mp.sqrt(-2 * mp.log(u1))
+        want = r * (mp.sin(2 * mp.pi * u2) if h else mp.cos(2 * mp.pi * u2))
+        assert abs(z[0] - float(want)) < 1e-14 * max(1.0, abs(z[0]))
+        # p = 2: uniform as above, normals are the per-object Box-Muller pair
+        z2, u_2 = O.plate_draws_f64(9, i, t, 2)
+        assert u_2 == u
+        assert np.array_equal(z2, O.normals_f64(9, O.KIND_PLATE, i, t, 2))
+
+
+def test_plate_draws_follow_their_laws_and_pairs_are_independent():
+    n = 60_000
+    d = [O.plate_draws_f64(13, i, 5, 1) for i in range(n)]
+    z = np.array([x[0][0] for x in d]); u = np.array([x[1] for x in d])
+    assert abs(z.mean()) < 4 / np.sqrt(n) and abs(z.var() - 1) < 4 * np.sqrt(2 / n)
+    assert stats.kstest(z, "norm").pvalue > 1e-3 and stats.kstest(u, "uniform").pvalue > 1e-3
+    assert 0 < u.min() and u.max() < 1
+    ze, zo, ue, uo = z[0::2], z[1::2], u[0::2], u[1::2]
+    assert abs(np.corrcoef(ze, zo)[0, 1]) < 4 / np.sqrt(n / 2)
+    assert abs(np.corrcoef(ue, uo)[0, 1]) < 4 / np.sqrt(n / 2)
+    assert abs(np.corrcoef(ze, ue)[0, 1]) < 4 / np.sqrt(n / 2)
+    # joint law of a pair: radius^2 ~ chi^2_2 and the angle uniform (full independence of the two normals)
+    assert stats.kstest(ze ** 2 + zo ** 2, "chi2", args=(2,)).pvalue > 1e-3
+    assert stats.kstest((np.arctan2(zo, ze) / (2 * np.pi)) % 1.0, "uniform").pvalue > 1e-3
+    # consecutive iterations of one object are independent draws
+    zt = np.array([O.plate_draws_f64(13, 7, t, 1)[0][0] for t in range(1, 20001)])
+    assert abs(np.corrcoef(zt[:-1], zt[1:])[0, 1]) < 4 / np.sqrt(zt.size)
+    assert stats.kstest(zt, "norm").pvalue > 1e-3
+
+
+def test_plate_draws_f32():
+    n = 40_000
+    zs, us = np.empty(n, np.float32), np.empty(n, np.float32)
+    for i in range(n):
+        z, u = O.plate_draws_f32(11, i, 7, 1)
+        zs[i] = z[0]; us[i] = u
+    for i in (10, 11):
+        w = O.stream_words(11, O.KIND_PLATE, i >> 1, 7, 0)
+        assert us[i] == np.float32(((w[3 if i & 1 else 2] >> 9) + 0.5) * 2.0 ** -23)
+        u1 = ((w[0] >> 9) + 0.5) * 2.0 ** -23
+        u2 = ((w[1] >> 9) + 0.5) * 2.0 ** -23
+        trig = np.sin if i & 1 else np.cos
+        assert abs(float(zs[i]) - np.sqrt(-2 * np.log(u1)) * trig(2 * np.pi * u2)) < 1e-5
+    assert 0 < us.min() and us.max() < 1
+    assert stats.kstest(us.astype(np.float64), "uniform").pvalue > 1e-3
+    assert stats.kstest(zs.astype(np.float64), "norm").pvalue > 1e-3
+    assert abs(np.corrcoef(zs[0::2], zs[1::2])[0, 1]) < 4.0 / np.sqrt(n / 2)
+    assert abs(np.corrcoef(us[0::2], us[1::2])[0, 1]) < 4.0 / np.sqrt(n / 2)
+    # p = 2 keeps the per-object layout
+    z2, u2_ = O.plate_draws_f32(11, 5, 7, 2)
+    z0, z1, u = O.draws_f32(11, O.KIND_PLATE, 5, 7)
+    assert z2[0] == z0 and z2[1] == z1 and u2_ == u
+
+
 def test_draws_f32():
     n = 40_000
     zs, us = np.empty((n, 2), np.float32), np.empty(n, np.float32)
