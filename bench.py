@@ -35,6 +35,11 @@ UNIT = "updates/s"
 # data read; + running-moment read+write (fp64 mean and M2 per component) once past burn-in
 ALG_BYTES = {"C0": (48, 32), "C1": (48, 32), "C2": (48, 32), "C3": (112, 64), "C4": (28, 32)}
 MODES = {"host": 0, "graph": 1, "tail": 2}
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel PER GIBBS ITERATION, from the committed
+# `ncu --set full` captures (profiles/r01d_resident_C2_ncu.md: 14.57 MB + 0.27 MB over 300 iterations;
+# profiles/r01d_persistent_C4_ncu.md: 5.947 GB + 2.373 GB over 30 iterations); scaled to the K iterations one timed
+# launch runs.  C2 keeps its state in shared memory, so its DRAM traffic is ~0.2 % of the algorithmic bytes.
+NCU_DRAM_BYTES_PER_ITER = {"C2": (14.569984e6 + 271.104e3) / 300, "C4": (5.947117e9 + 2.373307e9) / 30}
 
 
 def parse_args():
@@ -223,14 +228,17 @@ def time_e2e(cfg_name, args, device, rank):
     return dict(sec=sec, n=n, iters=W + K, h2d=h2d, d2h=d2h)
 
 
-def roofline_entry(cfg_name, c, n, K, W, ms, peak, peak_src):
+def roofline_entry(cfg_name, c, n, K, W, ms, peak, peak_src, kernel=None):
     base, mom = ALG_BYTES[cfg_name]
     per_obj = base + (mom if c.keep_chi_moments else 0)     # the timed iterations are all past burn-in
     bytes_per_iter = per_obj * n
     achieved = bytes_per_iter * K / (ms * 1e-3) / 1e9
+    per_iter = NCU_DRAM_BYTES_PER_ITER.get(cfg_name) if n == c.n_objects else None
     return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-            "traffic": None, "peak_source": peak_src, "alg_bytes_per_object_iter": per_obj,
-            "alg_bytes_per_iter": bytes_per_iter, "us_per_iter": ms * 1e3 / K}
+            "traffic": None if per_iter is None else per_iter * K, "peak_source": peak_src, "kernel": kernel,
+            "launches_timed": 1, "iterations_per_launch": K, "alg_bytes_per_object_iter": per_obj,
+            "alg_bytes_per_iter": bytes_per_iter, "alg_bytes_per_launch": bytes_per_iter * K,
+            "us_per_iter": ms * 1e3 / K}
 
 
 # ----------------------------------------------------------------------------------------------------------
@@ -352,18 +360,21 @@ def main():
                    "burn_in": W, "thin": c.thin, "chi_moments": bool(c.keep_chi_moments),
                    "theta_mode": args.theta_mode, "parallelism": "replicas only" if world > 1 else "1 gpu",
                    "grid": [r["stats"]["grid_blocks"], r["stats"]["block_threads"]],
-                   "l2": ("inputs larger than L2" if n * (sum(ALG_BYTES[args.config])) > 126e6 else
-                          "working set smaller than L2 and L2-resident BY DESIGN: the sampler iterates K times over "
-                          "the same state inside one persistent launch, so no flush between iterations is "
-                          "possible or meaningful; roofline.frac may exceed 1 (see roofline_cold for the "
-                          "flushed single-sweep figure)")},
+                   "l2": ("inputs larger than L2: every iteration streams the whole state through HBM"
+                          if n * ALG_BYTES[args.config][0] > 126e6 else
+                          "state resident ON CHIP by design: the sampler iterates K times over the same objects "
+                          "inside one persistent launch and keeps them in shared memory, so there is nothing to "
+                          "flush between iterations; roofline.achieved divides the ALGORITHMIC bytes by the time "
+                          "(roofline.traffic is what actually reached DRAM); other_configs holds the HBM-streaming "
+                          "configs C3 / C4, whose inputs are larger than L2")},
         "gibbs_iters_per_s": K * world / (ms * 1e-3),
         "e2e": {"value": e_value, "unit": UNIT, "h2d_bytes_per_step": e["h2d"] / e["iters"],
                 "d2h_bytes_per_step": e["d2h"] / e["iters"], "seconds": e_ms * 1e-3,
                 "what": "set_data(host cols, H2D) + set_init + run(W+K) + get_theta_trace + get_chi_moments (D2H)"},
         "gpu_launches": int(r["launches"]),
         "clocks": r["clocks"],
-        "roofline": roofline_entry(args.config, c, n, K, W, r["ms"], peak, peak_src),
+        "roofline": roofline_entry(args.config, c, n, K, W, r["ms"], peak, peak_src,
+                                   "k_resident" if r["stats"]["block_threads"] == 640 else "k_persistent"),
         "accept": {"chi": r["stats"]["chi_accepts"] / max(1, r["stats"]["chi_proposals"]),
                    "theta": r["stats"]["theta_accepts"] / max(1, r["stats"]["theta_proposals"])},
         "theta_mean": [float(x) for x in r["trace"].mean(0)] if len(r["trace"]) else None,
@@ -406,7 +417,7 @@ def extras(args, device, peak, peak_src, n):
         a = copy.copy(args)
         a.steps, a.warmup, a.n_objects = k, w, 0
         r = time_gpu(cfg_name, a, device, 0, 1, lambda: None, with_clocks=False)
-        rf = roofline_entry(cfg_name, r["cfg"], r["n"], k, w, r["ms"], peak, peak_src)
+        rf = roofline_entry(cfg_name, r["cfg"], r["n"], k, w, r["ms"], peak, peak_src, "k_persistent")
         side[cfg_name] = {"n_objects": r["n"], "steps": k, "warmup": w, "updates_per_s": r["n"] * k / (r["ms"] * 1e-3),
                           "gibbs_iters_per_s": k / (r["ms"] * 1e-3), "roofline": rf,
                           "grid": [r["stats"]["grid_blocks"], r["stats"]["block_threads"]]}

@@ -112,7 +112,7 @@ struct cudahm_sampler {
   bool timed = false;
   unsigned epoch = 1;               // next mailbox epoch of the persistent kernel
   const void* res_kernel = nullptr; // on-chip persistent kernel (resident.cuh) when the population fits, else NULL
-  int res_R = 0; size_t res_smem = 0;
+  int res_R = 0, res_OB = 0; size_t res_smem = 0;
   int sweep_grid = 1, sweep_block = 512;   // launch shape of k_sweep (THETA_GRAPH / HOST / debug_step)
   int tma_stages = 0; size_t tma_smem = 0;   // > 0: the streaming persistent kernel is k_persistent_tma
   double h_lp_prop_before = 0.0;    // log prior at theta' of the iteration debug_step is about to decide
@@ -255,12 +255,13 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
     int nv = 0;
     const void* rk = pick_resident(cfg->model, cfg->precision, cfg->keep_chi_moments, &nv);
     if (rk) {
-      const long long g = std::min<long long>(sms, (cfg->n_objects + RES_S - 1) / RES_S);
-      const long long R = 2 * ((cfg->n_objects + 2 * g * RES_S - 1) / (2 * g * RES_S));   // slots per thread, in pairs
+      const long long g = std::min<long long>(sms, (cfg->n_objects + 63) / 64);          // >= one warp of pairs per block
+      const long long OB = 2 * ((cfg->n_objects + 2 * g - 1) / (2 * g));                   // objects per block (even)
+      const long long R = 2 * ((OB + 2 * RES_S - 1) / (2 * RES_S));                        // slots per thread, in pairs
       const size_t bytes = (size_t)nv * R * RES_S * sizeof(double);
       if (bytes <= (size_t)RES_MAX_SMEM &&
           cudaFuncSetAttribute(rk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) == cudaSuccess) {
-        s->res_kernel = rk; s->res_R = (int)R; s->res_smem = bytes;
+        s->res_kernel = rk; s->res_R = (int)R; s->res_OB = (int)OB; s->res_smem = bytes;
         s->grid = (int)g; s->block = RES_THREADS;
       } else {
         cudaGetLastError();
@@ -486,8 +487,8 @@ int run_device_tail(cudahm_sampler* s, long long n_iter) {
     Params P = s->P;
     unsigned epoch0 = s->epoch;            // epochs never repeat over the sampler's lifetime (0 = never written)
     s->epoch += (unsigned)k;
-    int R = s->res_R;
-    void* args[] = {&P, &k, &epoch0, &R};
+    int R = s->res_R, OB = s->res_OB;
+    void* args[] = {&P, &k, &epoch0, &R, &OB};
     int rc;
     if (s->res_kernel) {
       cudaError_t e = cudaLaunchCooperativeKernel(s->res_kernel, dim3(s->grid), dim3(RES_THREADS), args, s->res_smem, s->stream);

@@ -41,7 +41,7 @@ enum : int { BAR_PARTIALS = 1, BAR_THETA = 2, BAR_TAIL = 3 };
 
 template <int MODEL>
 __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, const long long n_iter, const unsigned epoch0,
-                                                             const int R) {
+                                                             const int R, const int OB) {
   using T = double;
   using V = ResValues<MODEL>;
   using PL = Plate<MODEL, T>;
@@ -54,15 +54,16 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
   const bool is_tail = warp >= RES_SW;
   const int G = (int)gridDim.x;
   const long long N = P.N, Npad = P.Npad;
-  const int RS = R * RES_S;
   const bool keep_mom = P.tail.keep_moments != 0;
   const int V_MEAN = V::n_base, V_M2 = V::n_base + 1;
-  // A block owns the contiguous objects [blockIdx.x * RS, (blockIdx.x + 1) * RS); a thread owns adjacent PAIRS of
-  // them (objects draw in pairs, kernels.cuh::pair_draws): slot r = 2a + h is object obj0 + 2 a RES_S + h.  R is even.
-  const long long obj0 = (long long)blockIdx.x * RS + 2 * tid;
+  // A block owns the OB (even) contiguous objects [blockIdx.x * OB, (blockIdx.x + 1) * OB), so the population is
+  // spread evenly over the grid; a thread owns adjacent PAIRS of them (objects draw in pairs,
+  // kernels.cuh::pair_draws): slot r = 2a + h is object obj0 + 2 a RES_S + h.  R = 2 ceil(OB / (2 RES_S)).
+  const long long obj0 = (long long)blockIdx.x * OB + 2 * tid;
+  const long long obj_end = (long long)(blockIdx.x + 1) * OB < N ? (long long)(blockIdx.x + 1) * OB : N;
 #define HM_OBJ(r) (obj0 + (long long)((r) >> 1) * (2 * RES_S) + ((r) & 1))
   int nlive = 0;                                                  // HM_OBJ increases with r: live slots are 0 .. nlive-1
-  for (int r = 0; r < R; ++r) nlive += HM_OBJ(r) < N ? 1 : 0;
+  for (int r = 0; r < R; ++r) nlive += HM_OBJ(r) < obj_end ? 1 : 0;
   T* const chi = static_cast<T*>(P.chi);
   T* const Lm = static_cast<T*>(P.L);
   const T* const dat = static_cast<const T*>(P.data);
