@@ -24,7 +24,6 @@ constexpr int RES_SW = HM_RES_SW;                   // sweep warps per block
 constexpr int RES_S = RES_SW * 32;                  // sweep threads per block
 constexpr int RES_TW = 4;                           // tail warps per block (tail_block needs exactly 4)
 constexpr int RES_THREADS = RES_S + RES_TW * 32;    // 640 with 16 sweep warps
-constexpr int RES_IL = 1;                           // slots processed together (instruction-level parallelism)
 constexpr int RES_MAX_SMEM = 200 * 1024;            // dynamic shared memory the kernel may ask for
 
 // per-object values kept in shared memory: [value][slot r][sweep thread]
@@ -37,7 +36,7 @@ template <int MODEL> struct ResValues {
 
 __device__ __forceinline__ void bar_sync(const int id, const int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 __device__ __forceinline__ void bar_arrive(const int id, const int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
-enum : int { BAR_PARTIALS = 1, BAR_THETA = 2, BAR_TAIL = 3 };
+enum : int { BAR_PARTIALS = 1, BAR_THETA = 2, BAR_TAIL = 3, BAR_THETAP = 4 };
 
 template <int MODEL>
 __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, const long long n_iter, const unsigned epoch0,
@@ -124,62 +123,58 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
 #ifdef HM_PHASE_TIMING
       last_ = clock64();
 #endif
-      if (k > 0) bar_sync(BAR_THETA, RES_THREADS);          // theta_t, theta'_t are in `it`
+      if (k > 0) bar_sync(BAR_THETA, RES_THREADS);          // theta_t and everything derived from it are in `it`
       HM_RSTAMP(0)
-      // theta-dependent half: targets, accept, RAM update, population terms, moments
-      const ThetaK kc = it.kc, kp = it.kp;
+      // back, part 1 (needs theta_t only): targets, accept, RAM update, new chi, moments
+      const ThetaK kc = it.kc;
       const KT<T> kT = narrow<T>(kc);
       const T eta = (T)it.dr[t % 3].eta;
       const bool do_mom = keep_mom && t > P.tail.burn_in;
       const double inv_k = 1.0 / (double)(it.mom_count + 1);
+      for (int r = 0; r < nlive; ++r) {
+        T di[ncols];
+#pragma unroll
+        for (int c = 0; c < ncols; ++c) di[c] = HM_AT(V::V_D + c, r);
+        const T xi = HM_AT(V::V_CHI, r), yi = HM_AT(V::V_XP, r), l = HM_AT(V::V_L, r), u = HM_AT(V::V_U, r);
+        typename PL::Pt qc, qp;
+        if constexpr (V::m1) {
+          qc = typename PL::Pt{xi, HM_AT(V::V_E, r)};
+          qp = typename PL::Pt{yi, HM_AT(V::V_EP, r)};
+        } else {
+          qc = PL::point(&xi); qp = PL::point(&yi);
+        }
+        const T pc = PL::target(qc, di, kT, mcT), pp = PL::target(qp, di, kT, mcT);
+        const T diff = pp - pc;
+        const bool bad = diff != diff;
+        const T la = bad ? T(-INFINITY) : (diff < T(0) ? diff : T(0));
+        const T alpha = hm_exp(la);
+        const bool acc = u < alpha;
+        nacc += acc ? 1.0 : 0.0; nnan += bad ? 1.0 : 0.0;
+        HM_AT(V::V_L, r) = l * hm_sqrt_pos(T(1) + eta * (alpha - astar));
+        if (acc) {
+          HM_AT(V::V_CHI, r) = yi;
+          if constexpr (V::m1) HM_AT(V::V_E, r) = qp.ex;
+        }
+        if (do_mom) {
+          const double xv = (double)(acc ? yi : xi), m0 = HM_AT(V_MEAN, r);
+          const double dl = xv - m0, m1 = m0 + dl * inv_k;
+          HM_AT(V_MEAN, r) = m1;
+          HM_AT(V_M2, r) += dl * (xv - m1);
+        }
+      }
+      // back, part 2 (needs theta'_t, which the tail finishes a little later): population terms and the
+      // selection-integral slice
+      if (k > 0) bar_sync(BAR_THETAP, RES_THREADS);
+      const ThetaK kp = it.kp;
       double v[2] = {0.0, 0.0};
-      for (int r = 0; r < nlive; r += RES_IL) {
-        T xn[RES_IL], ln[RES_IL], en[RES_IL], dba[RES_IL];
-        bool lv[RES_IL], accj[RES_IL], badj[RES_IL];
-        int rr[RES_IL];
+      for (int r = 0; r < nlive; ++r) {
+        T di[ncols];
 #pragma unroll
-        for (int j = 0; j < RES_IL; ++j) {
-          rr[j] = r + j < nlive ? r + j : r;
-          lv[j] = r + j < nlive;
-          T di[ncols];
-#pragma unroll
-          for (int c = 0; c < ncols; ++c) di[c] = HM_AT(V::V_D + c, rr[j]);
-          const T xi = HM_AT(V::V_CHI, rr[j]), yi = HM_AT(V::V_XP, rr[j]), l = HM_AT(V::V_L, rr[j]), u = HM_AT(V::V_U, rr[j]);
-          typename PL::Pt qc, qp;
-          if constexpr (V::m1) {
-            qc = typename PL::Pt{xi, HM_AT(V::V_E, rr[j])};
-            qp = typename PL::Pt{yi, HM_AT(V::V_EP, rr[j])};
-          } else {
-            qc = PL::point(&xi); qp = PL::point(&yi);
-          }
-          const T pc = PL::target(qc, di, kT, mcT), pp = PL::target(qp, di, kT, mcT);
-          const T diff = pp - pc;
-          badj[j] = diff != diff;
-          const T la = badj[j] ? T(-INFINITY) : (diff < T(0) ? diff : T(0));
-          const T alpha = hm_exp(la);
-          accj[j] = u < alpha;
-          const typename PL::Pt qn = accj[j] ? qp : qc;
-          ln[j] = l * hm_sqrt_pos(T(1) + eta * (alpha - astar));
-          dba[j] = PL::pop(qn, di, kp) - PL::pop(qn, di, kc);
-          xn[j] = qn.x;
-          if constexpr (V::m1) en[j] = qn.ex; else en[j] = T(0);
-        }
-#pragma unroll
-        for (int j = 0; j < RES_IL; ++j) {
-          if (lv[j]) {
-            v[0] += dba[j];
-            nacc += accj[j] ? 1.0 : 0.0; nnan += badj[j] ? 1.0 : 0.0;
-            HM_AT(V::V_CHI, rr[j]) = xn[j];
-            HM_AT(V::V_L, rr[j]) = ln[j];
-            if constexpr (V::m1) HM_AT(V::V_E, rr[j]) = en[j];
-            if (do_mom) {
-              const double xv = (double)xn[j], m0 = HM_AT(V_MEAN, rr[j]);
-              const double dl = xv - m0, m1 = m0 + dl * inv_k;
-              HM_AT(V_MEAN, rr[j]) = m1;
-              HM_AT(V_M2, rr[j]) += dl * (xv - m1);
-            }
-          }
-        }
+        for (int c = 0; c < ncols; ++c) di[c] = HM_AT(V::V_D + c, r);
+        const T xn = HM_AT(V::V_CHI, r);
+        typename PL::Pt qn;
+        if constexpr (V::m1) qn = typename PL::Pt{xn, HM_AT(V::V_E, r)}; else qn = PL::point(&xn);
+        v[0] += PL::pop(qn, di, kp) - PL::pop(qn, di, kc);
       }
       if (V::m1 && !P.tail.freeze_theta) {          // this thread's terms of the selection integral at theta'
         for (int q = (int)blockIdx.x + G * tid; q < NQUAD; q += G * RES_S)
@@ -203,6 +198,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
              (double)ph[0] / n_iter, (double)ph[1] / n_iter, (double)ph[2] / n_iter);
 #endif
     bar_sync(BAR_THETA, RES_THREADS);                        // the last tail has finished
+    bar_sync(BAR_THETAP, RES_THREADS);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
       nacc += __shfl_down_sync(0xffffffffu, nacc, o);
@@ -245,9 +241,10 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
         tot[1] = t2[0]; tot[2] = t2[1];
       }
       HM_RSTAMP(1)
-      tail_block(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, tw, SyncNamed<BAR_TAIL, RES_TW * 32>());
+      tail_block(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, tw, SyncNamed<BAR_TAIL, RES_TW * 32>(),
+                 ArriveNamed<BAR_THETA, RES_THREADS>());      // theta_{t+1} is signalled after the decision phase ...
       __threadfence_block();
-      bar_arrive(BAR_THETA, RES_THREADS);
+      bar_arrive(BAR_THETAP, RES_THREADS);                   // ... theta'_{t+1} and its constants when the tail is done
       HM_RSTAMP(2)
     }
 #ifdef HM_PHASE_TIMING

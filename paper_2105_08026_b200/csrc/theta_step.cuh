@@ -206,9 +206,20 @@ struct SyncNamed {
   __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, %1;" ::"n"(ID), "n"(THREADS) : "memory"); }
 };
 
-template <class Sync>
+struct NoSignal { __device__ __forceinline__ void operator()() const {} };
+template <int ID, int THREADS>
+struct ArriveNamed {
+  __device__ __forceinline__ void operator()() const {
+    __threadfence_block();
+    asm volatile("bar.arrive %0, %1;" ::"n"(ID), "n"(THREADS) : "memory");
+  }
+};
+
+// `decided` is called by all four warps right after the decision phase: theta, kc, eta, the moments count and
+// L_theta of iteration t + 1 are final from there on (theta', kp, the prior and W only when tail_block returns).
+template <class Sync, class Decided = NoSignal>
 __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const double* tot, double* trace_or_null,
-                                           const int warp, const Sync sync) {
+                                           const int warp, const Sync sync, const Decided decided = Decided()) {
   const int lane = threadIdx.x & 31;
   const int dt = c.dtheta, nt = dt * (dt + 1) / 2;
   const long long t = it.t;
@@ -277,6 +288,7 @@ __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const dou
     }
   }
   sync();
+  decided();
 #ifdef HM_PHASE_TIMING
   tc2_ = clock64();
 #endif
