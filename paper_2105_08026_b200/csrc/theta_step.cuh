@@ -215,8 +215,9 @@ struct ArriveNamed {
   }
 };
 
-// `decided` is called by all four warps right after the decision phase: theta, kc, eta, the moments count and
-// L_theta of iteration t + 1 are final from there on (theta', kp, the prior and W only when tail_block returns).
+// `decided` is called once by every thread of the four warps as soon as what the next sweep's targets need is
+// final: kc (theta_{t+1}'s constants: the accept decision only, NOT the RAM update of L_theta), the moments count
+// and eta of iteration t + 1.  theta', kp, the prior, L_theta and W are final only when tail_block returns.
 template <class Sync, class Decided = NoSignal>
 __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const double* tot, double* trace_or_null,
                                            const int warp, const Sync sync, const Decided decided = Decided()) {
@@ -238,6 +239,9 @@ __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const dou
   if (warp == 0) {
     if (!c.freeze_theta) {
       decide_scalars(it, c, d0, tot[1], tot[2], &T_prop, &log_r, &alpha, &acc);
+      const double kpv = lane < 8 ? it.kp.v[lane] : 0.0;
+      if (lane < 8 && acc) it.kc.v[lane] = kpv;          // theta_{t+1}'s constants: all the next sweep's targets need
+      decided();
       const double cc = d0.eta * (alpha - c.astar_theta);
       double Kd = 1.0, g = 0.0;
       if (lane < dt) ram_coeffs(lane, cc, d0, &Kd, &g);
@@ -246,19 +250,20 @@ __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const dou
       const double Kd_j = __shfl_sync(0xffffffffu, Kd, ej), g_j = __shfl_sync(0xffffffffu, g, ej);
       const double l_new = it.Lth[e] * Kd_j + g_j * it.W[e];
       const double th_old = lane < dt ? it.theta[lane] : 0.0, thp_old = lane < dt ? it.thetaP[lane] : 0.0;
-      const double kpv = lane < 8 ? it.kp.v[lane] : 0.0;
       __syncwarp();
       if (lane < nt) it.Lth[e] = l_new;
       if (lane < MAXD) it.tap_thetaP[lane] = lane < dt ? thp_old : 0.0;
       if (lane < dt) it.theta[lane] = acc ? thp_old : th_old;
-      if (lane < 8 && acc) it.kc.v[lane] = kpv;
       __syncwarp();
       if (lane < dt) it.thetaP[lane] = propose_entry(it, d1, lane);
+    } else {
+      decided();
     }
 #ifdef HM_PHASE_TIMING
     tc1_ = clock64();
 #endif
   } else if (warp == 1) {
+    decided();
     if (!c.freeze_theta) {
       if (2 * lane < dt) {
         double rad, cs, sn;
@@ -277,18 +282,17 @@ __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const dou
       }
     }
   } else if (warp == 2) {
-    if (lane == 0) {
-      d2.eta = pow((double)(t + 3), -c.eta_exp);
-      decide_schedule(it, c);
-    }
+    if (lane == 0) decide_schedule(it, c);               // moments count of t + 1: the next sweep reads it
+    decided();
+    if (lane == 0) d2.eta = pow((double)(t + 3), -c.eta_exp);
   } else if (warp == 3) {
+    decided();
     if (lane == 0 && !c.freeze_theta) {
       const U4 r = stream(c.seed, KIND_THETA, 0ull, (uint32_t)(t + 2), 0u);
       d2.u = u01(r.x, r.y);
     }
   }
   sync();
-  decided();
 #ifdef HM_PHASE_TIMING
   tc2_ = clock64();
 #endif
