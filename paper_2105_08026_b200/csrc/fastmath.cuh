@@ -60,32 +60,46 @@ HM_HD double hm_rsqrt_seed(double a) {
 #endif
 }
 
-// e^x: k = round(x log2 e), r = x - k ln2 (Cody-Waite, two pieces), e^r by its degree-13 Taylor polynomial
-// (|r| <= ln2/2: truncation 4e-18), result scaled by 2^k through the exponent field (normal for x in [-708, 709]).
-HM_HD double hm_exp_fast(double x) {
-  x = fmin(fmax(x, -708.0), 709.0);
+// e^x = 2^k T[j] e^r with n = 64 k + j = round(64 x / ln2), r = x - n ln2/64 (Cody-Waite, two pieces, |r| <= ln2/128),
+// T[j] = 2^(j/64) from a 64-entry (hi, lo) table (1 KB, stays in L1) and e^r - 1 by its degree-6 Taylor polynomial
+// (truncation 3e-20).  The result is scaled by 2^k through the exponent field (normal for x in [-708, 709]).
+// Half the polynomial of a table-free version, and -- what matters more here -- half the fp64 immediates.
+#include "exp_table.inc"
+struct hm_d2 { double hi, lo; };
+#ifdef __CUDACC__
+__device__ const hm_d2 hm_exp2_tab_dev[64] = {HM_EXP2_TABLE};
+#endif
+static const hm_d2 hm_exp2_tab_host[64] = {HM_EXP2_TABLE};
+
+// hm_exp_core: NO argument check -- finite garbage (or inf / NaN) outside [-708, 709]; for callers that discard the
+// result there anyway (a proposal outside the model's support, alpha of a log ratio below -708).
+HM_HD double hm_exp_core(double x) {
   const double SHIFT = 6755399441055744.0;                 // 1.5 * 2^52: adding it rounds to the nearest integer
-  const double t = hm_fma(x, 1.4426950408889634074, SHIFT);
-  const double k = t - SHIFT;
-  double r = hm_fma(k, -6.93147180369123816490e-01, x);    // ln2_hi (low 32 mantissa bits zero): k * ln2_hi exact
-  r = hm_fma(k, -1.90821492927058770002e-10, r);           // ln2_lo
-  double p = 1.6059043836821613e-10;                       // 1/13!
-  p = hm_fma(p, r, 2.0876756987868100e-09);                // 1/12!
-  p = hm_fma(p, r, 2.5052108385441720e-08);                // 1/11!
-  p = hm_fma(p, r, 2.7557319223985888e-07);                // 1/10!
-  p = hm_fma(p, r, 2.7557319223985893e-06);                // 1/9!
-  p = hm_fma(p, r, 2.4801587301587302e-05);                // 1/8!
-  p = hm_fma(p, r, 1.9841269841269841e-04);                // 1/7!
-  p = hm_fma(p, r, 1.3888888888888889e-03);                // 1/6!
+  const double t = hm_fma(x, HM_64_LN2, SHIFT);
+  const double nf = t - SHIFT;
+  double r = hm_fma(nf, -HM_LN2_64_HI, x);                 // HM_LN2_64_HI has 32 significant bits: exact product
+  r = hm_fma(nf, -HM_LN2_64_LO, r);
+  const int n = (int)(uint32_t)(hm_d2bits(t) & 0xffffffffull);   // the integer sits in the low word of t
+  const int j = n & 63, k = n >> 6;
+#ifdef __CUDA_ARCH__
+  const double2 tj = __ldg(reinterpret_cast<const double2*>(hm_exp2_tab_dev) + j);
+  const double thi = tj.x, tlo = tj.y;
+#else
+  const double thi = hm_exp2_tab_host[j].hi, tlo = hm_exp2_tab_host[j].lo;
+#endif
+  double p = 1.3888888888888889e-03;                       // 1/6!
   p = hm_fma(p, r, 8.3333333333333332e-03);                // 1/5!
   p = hm_fma(p, r, 4.1666666666666664e-02);                // 1/4!
   p = hm_fma(p, r, 1.6666666666666666e-01);                // 1/3!
   p = hm_fma(p, r, 0.5);
-  p = hm_fma(p, r, 1.0);
-  p = hm_fma(p, r, 1.0);
-  // the integer k sits in the low 32 bits of t (two's complement): add it to the exponent field of p
-  const uint64_t ki = hm_d2bits(t) & 0xffffffffull;
-  return hm_bits2d(hm_d2bits(p) + (ki << 52));
+  p = p * r;
+  p = hm_fma(p, r, r);                                     // e^r - 1
+  const double y = thi + hm_fma(thi, p, tlo);              // T[j] e^r
+  return hm_bits2d(hm_d2bits(y) + ((uint64_t)(int64_t)k << 52));
+}
+HM_HD double hm_exp_fast(double x) {
+  x = x < -708.0 ? -708.0 : (x > 709.0 ? 709.0 : x);       // (fmin / fmax cost 7 instructions each: NaN handling)
+  return hm_exp_core(x);
 }
 
 // ln u for positive normal u: u = 2^e m, m in [sqrt(1/2), sqrt 2); ln m = 2 atanh(s), s = (m-1)/(m+1), |s| <= 0.1716,
@@ -141,7 +155,7 @@ HM_HD double hm_sqrt_fast(double w) {
 HM_HD double hm_exp_any(double x) {
 #ifdef __CUDA_ARCH__
   const double r = hm_exp_fast(x);
-  return x < -708.0 ? 0.0 : (x != x ? x : r);
+  return x < -708.0 ? 0.0 : r;
 #else
   return std::exp(x);
 #endif

@@ -179,7 +179,7 @@ __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c
     const T diff = pp - pc;
     const bool bad = diff != diff;
     const T la = bad ? T(-INFINITY) : (diff < T(0) ? diff : T(0));
-    const T alpha = hm_exp(la);
+    const T alpha = hm_exp_nonpos(la);
     const bool acc = u < alpha;
     const typename PL::Pt qn = acc ? qp : qc;
 #pragma unroll

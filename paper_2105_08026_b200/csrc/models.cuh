@@ -100,6 +100,16 @@ template <class T> HM_HD KT<T> narrow(const ThetaK& k) {
 // e^x of the sweep: specialised version (fastmath.cuh); exp(-inf) = 0 is selected explicitly (alpha of a proposal
 // outside the support)
 __device__ __forceinline__ double hm_exp(double x) { const double r = hm_exp_fast(x); return x < -708.0 ? 0.0 : r; }
+// alpha = e^la for la <= 0 (or -inf): one compare serves the clamp and the exact zero
+__device__ __forceinline__ double hm_exp_nonpos(double la) {
+  const bool tiny = la < -708.0;
+  const double r = hm_exp_core(tiny ? -708.0 : la);
+  return tiny ? 0.0 : r;
+}
+__device__ __forceinline__ float hm_exp_nonpos(float la) { return expf(la); }
+// e^x of a model point whose target is -inf outside a bounded support: no argument check at all
+__device__ __forceinline__ double hm_exp_point(double x) { return hm_exp_core(x); }
+__device__ __forceinline__ float hm_exp_point(float x) { return expf(x); }
 __device__ __forceinline__ float hm_exp(float x) { return expf(x); }
 
 template <int MODEL, class T> struct Plate;
@@ -133,7 +143,7 @@ template <class T> struct Plate<M_LINREG_ME1D, T> {
 
 template <class T> struct Plate<M_THINNED_SCHECHTER1D, T> {
   struct Pt { T x, ex; };
-  __device__ __forceinline__ static Pt point(const T* chi) { return Pt{chi[0], hm_exp(chi[0])}; }
+  __device__ __forceinline__ static Pt point(const T* chi) { return Pt{chi[0], hm_exp_point(chi[0])}; }
   // mc = {F_lim, sigma_F, x_lo, x_hi, r_min, r_max, 1/(2 sigma_F^2)} narrowed to T
   __device__ __forceinline__ static T target(const Pt& q, const T* d, const KT<T>& k, const T* mc) {
     if (!(q.x >= mc[MC_XLO] && q.x <= mc[MC_XHI])) return -INFINITY;

@@ -100,7 +100,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
             const T xp = HM_AT(V::V_CHI, r + h) + HM_AT(V::V_L, r + h) * z[h][0];
             HM_AT(V::V_XP, r + h) = xp;
             HM_AT(V::V_U, r + h) = u[h];
-            if (V::m1) HM_AT(V::V_EP, r + h) = hm_exp(xp);
+            if (V::m1) HM_AT(V::V_EP, r + h) = hm_exp_point(xp);
           }
         }
       }
@@ -147,7 +147,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
         const T diff = pp - pc;
         const bool bad = diff != diff;
         const T la = bad ? T(-INFINITY) : (diff < T(0) ? diff : T(0));
-        const T alpha = hm_exp(la);
+        const T alpha = hm_exp_nonpos(la);
         const bool acc = u < alpha;
         nacc += acc ? 1.0 : 0.0; nnan += bad ? 1.0 : 0.0;
         HM_AT(V::V_L, r) = l * hm_sqrt_pos(T(1) + eta * (alpha - astar));
