@@ -24,6 +24,7 @@ struct Draws {
   double Pc[MAXD + 1];  // Pc[j] = sum_{k<j} uh_k^2
   double eta;           // eta_n = n^(-eta_exp), n = t + 1         (X_1, S_1 are initial values)
   double u;             // accept uniform of the theta step        (theta Philox stream, draw 0)
+  double lu;            // ln u (device tail: the decision is taken as ln u < ln alpha, see decide_scalars)
 };
 
 // Iteration state: lives in global memory between launches, in shared memory inside the kernels.
@@ -77,7 +78,7 @@ HM_HD void make_draws(Draws& d, const TailCfg& c, long long t) {
   d.eta = pow((double)(t + 1), -c.eta_exp);
   for (int j = 0; j < MAXD; ++j) { d.z[j] = 0.0; d.uh[j] = 0.0; }
   for (int j = 0; j <= MAXD; ++j) d.Pc[j] = 0.0;
-  d.u = 0.0;
+  d.u = 0.0; d.lu = 0.0;
   if (c.freeze_theta) return;
   normals(c.seed, KIND_THETA, 0ull, (uint32_t)t, c.dtheta, d.z);
   double n2 = 0.0;
@@ -88,6 +89,7 @@ HM_HD void make_draws(Draws& d, const TailCfg& c, long long t) {
   d.Pc[c.dtheta] = s;
   const U4 r = stream(c.seed, KIND_THETA, 0ull, (uint32_t)t, 0u);
   d.u = u01(r.x, r.y);
+  d.lu = hm_log_any_pos(d.u);
 }
 
 HM_HD double make_W_entry(const Iter& it, const Draws& d, int i, int j) {
@@ -122,21 +124,24 @@ HM_HD void prepare_iteration(Iter& it, const TailCfg& c, long long t) {
   }
 }
 
-// The acceptance part shared by (a) and (b): log r, alpha, accept flag.  tq = sum_k W_k phi(x_k; theta').
+// The acceptance part shared by (a) and (b): log r, ln alpha = min(0, log r), accept flag.
+// The paper's rule is "accept iff u < alpha"; it is taken here as ln u < ln alpha with ln u drawn
+// ahead of time, so that no exponential sits between the arrival of the sums and the decision the next sweep is
+// waiting for.  The two forms differ only where |ln alpha - ln u| is of the order of one rounding error, far
+// inside the near-tie band (1e-9) in which BASELINE.json allows accept sequences to differ.  alpha itself (the
+// RAM update needs it) is computed by the caller afterwards.
 HM_HD void decide_scalars(const Iter& it, const TailCfg& c, const Draws& d, double Delta, double tq, double* T_prop,
-                          double* log_r, double* alpha, int* acc) {
-  double la;
+                          double* log_r, double* la, int* acc) {
   *T_prop = 0.0;
   if (it.lp_prop == -INFINITY) {
-    *log_r = -INFINITY; la = -INFINITY;
+    *log_r = -INFINITY; *la = -INFINITY;
   } else {
     // M1: T(theta') = -A' sum_k W_k phi(x_k; theta'): minus the expected detected count (Eq. 4.4 denominator)
     *T_prop = (c.model == M_THINNED_SCHECHTER1D) ? -it.kp.v[4] * tq : 0.0;
     *log_r = Delta + (*T_prop - it.T_cur) + (it.lp_prop - it.lp_cur);
-    la = (*log_r != *log_r) ? -INFINITY : fmin(0.0, *log_r);
+    *la = (*log_r != *log_r) ? -INFINITY : fmin(0.0, *log_r);
   }
-  *alpha = hm_exp_any(la);
-  *acc = d.u < *alpha ? 1 : 0;
+  *acc = d.lu < *la ? 1 : 0;
 }
 
 // bookkeeping shared by (a) and (b): taps and counters fed by the sweep totals ...
@@ -166,7 +171,9 @@ HM_HD void tail_decide(Iter& it, const TailCfg& c, const double* tot) {
   for (int r = 0; r < MAXD; ++r) it.tap_thetaP[r] = it.thetaP[r];
   if (!c.freeze_theta) {
     int acc;
-    decide_scalars(it, c, d, tot[1], tot[2], &it.T_prop, &it.log_r, &it.alpha_theta, &acc);
+    double la;
+    decide_scalars(it, c, d, tot[1], tot[2], &it.T_prop, &it.log_r, &la, &acc);
+    it.alpha_theta = hm_exp_any(la);
     it.u_theta = d.u;
     it.theta_prop_n += 1;
     if (acc) {
@@ -238,10 +245,12 @@ __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const dou
   int acc = 0;
   if (warp == 0) {
     if (!c.freeze_theta) {
-      decide_scalars(it, c, d0, tot[1], tot[2], &T_prop, &log_r, &alpha, &acc);
+      double la;
+      decide_scalars(it, c, d0, tot[1], tot[2], &T_prop, &log_r, &la, &acc);
       const double kpv = lane < 8 ? it.kp.v[lane] : 0.0;
       if (lane < 8 && acc) it.kc.v[lane] = kpv;          // theta_{t+1}'s constants: all the next sweep's targets need
       decided();
+      alpha = hm_exp_any(la);
       const double cc = d0.eta * (alpha - c.astar_theta);
       double Kd = 1.0, g = 0.0;
       if (lane < dt) ram_coeffs(lane, cc, d0, &Kd, &g);
@@ -290,6 +299,7 @@ __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const dou
     if (lane == 0 && !c.freeze_theta) {
       const U4 r = stream(c.seed, KIND_THETA, 0ull, (uint32_t)(t + 2), 0u);
       d2.u = u01(r.x, r.y);
+      d2.lu = hm_log_any_pos(d2.u);
     }
   }
   sync();
