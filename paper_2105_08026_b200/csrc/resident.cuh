@@ -24,6 +24,10 @@ constexpr int RES_SW = HM_RES_SW;                   // sweep warps per block
 constexpr int RES_S = RES_SW * 32;                  // sweep threads per block
 constexpr int RES_TW = 4;                           // tail warps per block (tail_block needs exactly 4)
 constexpr int RES_THREADS = RES_S + RES_TW * 32;    // 640 with 16 sweep warps
+#ifndef HM_RES_IL
+#define HM_RES_IL 2
+#endif
+constexpr int RES_IL = HM_RES_IL;                   // slots of the back processed together (instruction-level parallelism)
 constexpr int RES_MAX_SMEM = 200 * 1024;            // dynamic shared memory the kernel may ask for
 
 // per-object values kept in shared memory: [value][slot r][sweep thread]
@@ -112,7 +116,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
     double nacc = 0.0, nnan = 0.0;
 
 #ifdef HM_PHASE_TIMING
-    long long ph[4] = {0, 0, 0, 0}, last_ = 0;
+    long long ph[6] = {0, 0, 0, 0, 0, 0}, last_ = 0;
 #define HM_RSTAMP(i) { const long long now_ = clock64(); ph[i] += now_ - last_; last_ = now_; }
 #else
 #define HM_RSTAMP(i)
@@ -131,40 +135,64 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
       const T eta = (T)it.dr[t % 3].eta;
       const bool do_mom = keep_mom && t > P.tail.burn_in;
       const double inv_k = 1.0 / (double)(it.mom_count + 1);
-      for (int r = 0; r < nlive; ++r) {
-        T di[ncols];
+      // RES_IL slots at a time in straight-line code: the back sits on the critical path of the iteration (the
+      // exchange cannot start before it ends) and one slot is a single dependent chain of fp64 operations, so with
+      // 4 warps per scheduler it is latency-bound; independent slots interleave.  A slot past nlive repeats the
+      // last live one and is not stored.
+      for (int r = 0; r < nlive; r += RES_IL) {
+        T xi[RES_IL], yi[RES_IL], la[RES_IL], lnew[RES_IL], exq[RES_IL];
+        bool acc[RES_IL], bad[RES_IL];
+        int rr[RES_IL];
 #pragma unroll
-        for (int c = 0; c < ncols; ++c) di[c] = HM_AT(V::V_D + c, r);
-        const T xi = HM_AT(V::V_CHI, r), yi = HM_AT(V::V_XP, r), l = HM_AT(V::V_L, r), u = HM_AT(V::V_U, r);
-        typename PL::Pt qc, qp;
-        if constexpr (V::m1) {
-          qc = typename PL::Pt{xi, HM_AT(V::V_E, r)};
-          qp = typename PL::Pt{yi, HM_AT(V::V_EP, r)};
-        } else {
-          qc = PL::point(&xi); qp = PL::point(&yi);
+        for (int j = 0; j < RES_IL; ++j) {
+          rr[j] = r + j < nlive ? r + j : nlive - 1;
+          T di[ncols];
+#pragma unroll
+          for (int c = 0; c < ncols; ++c) di[c] = HM_AT(V::V_D + c, rr[j]);
+          xi[j] = HM_AT(V::V_CHI, rr[j]); yi[j] = HM_AT(V::V_XP, rr[j]);
+          typename PL::Pt qc, qp;
+          if constexpr (V::m1) {
+            qc = typename PL::Pt{xi[j], HM_AT(V::V_E, rr[j])};
+            qp = typename PL::Pt{yi[j], HM_AT(V::V_EP, rr[j])};
+            exq[j] = qp.ex;
+          } else {
+            qc = PL::point(&xi[j]); qp = PL::point(&yi[j]);
+            exq[j] = T(0);
+          }
+          const T pc = PL::target(qc, di, kT, mcT), pp = PL::target(qp, di, kT, mcT);
+          const T diff = pp - pc;
+          bad[j] = diff != diff;
+          la[j] = bad[j] ? T(-INFINITY) : (diff < T(0) ? diff : T(0));
         }
-        const T pc = PL::target(qc, di, kT, mcT), pp = PL::target(qp, di, kT, mcT);
-        const T diff = pp - pc;
-        const bool bad = diff != diff;
-        const T la = bad ? T(-INFINITY) : (diff < T(0) ? diff : T(0));
-        const T alpha = hm_exp_nonpos(la);
-        const bool acc = u < alpha;
-        nacc += acc ? 1.0 : 0.0; nnan += bad ? 1.0 : 0.0;
-        HM_AT(V::V_L, r) = l * hm_sqrt_pos(T(1) + eta * (alpha - astar));
-        if (acc) {
-          HM_AT(V::V_CHI, r) = yi;
-          if constexpr (V::m1) HM_AT(V::V_E, r) = qp.ex;
+#pragma unroll
+        for (int j = 0; j < RES_IL; ++j) {
+          const T alpha = hm_exp_nonpos(la[j]);
+          acc[j] = HM_AT(V::V_U, rr[j]) < alpha;
+          lnew[j] = HM_AT(V::V_L, rr[j]) * hm_sqrt_pos(T(1) + eta * (alpha - astar));
         }
-        if (do_mom) {
-          const double xv = (double)(acc ? yi : xi), m0 = HM_AT(V_MEAN, r);
-          const double dl = xv - m0, m1 = m0 + dl * inv_k;
-          HM_AT(V_MEAN, r) = m1;
-          HM_AT(V_M2, r) += dl * (xv - m1);
+#pragma unroll
+        for (int j = 0; j < RES_IL; ++j) {
+          if (r + j < nlive) {
+            nacc += acc[j] ? 1.0 : 0.0; nnan += bad[j] ? 1.0 : 0.0;
+            HM_AT(V::V_L, rr[j]) = lnew[j];
+            if (acc[j]) {
+              HM_AT(V::V_CHI, rr[j]) = yi[j];
+              if constexpr (V::m1) HM_AT(V::V_E, rr[j]) = exq[j];
+            }
+            if (do_mom) {
+              const double xv = (double)(acc[j] ? yi[j] : xi[j]), m0 = HM_AT(V_MEAN, rr[j]);
+              const double dl = xv - m0, m1 = m0 + dl * inv_k;
+              HM_AT(V_MEAN, rr[j]) = m1;
+              HM_AT(V_M2, rr[j]) += dl * (xv - m1);
+            }
+          }
         }
       }
       // back, part 2 (needs theta'_t, which the tail finishes a little later): population terms and the
       // selection-integral slice
+      HM_RSTAMP(3)
       if (k > 0) bar_sync(BAR_THETAP, RES_THREADS);
+      HM_RSTAMP(4)
       const ThetaK kp = it.kp;
       double v[2] = {0.0, 0.0};
       for (int r = 0; r < nlive; ++r) {
@@ -190,12 +218,16 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
       bar_arrive(BAR_PARTIALS, RES_THREADS);                 // hand the partials to the tail warps, do not wait
       HM_RSTAMP(1)
       if (k + 1 < n_iter) front((uint32_t)(t + 1));          // overlaps the exchange and the theta step
+#ifdef HM_SWEEP_DELAY
+      { const long long t_ = clock64(); while (clock64() - t_ < HM_SWEEP_DELAY) {} }
+#endif
       HM_RSTAMP(2)
     }
 #ifdef HM_PHASE_TIMING
     if (tid == 0 && (blockIdx.x == 0 || blockIdx.x == G - 1))
-      printf("block %d sweep warp 0: cycles/iter wait-theta %.0f back %.0f front %.0f\n", (int)blockIdx.x,
-             (double)ph[0] / n_iter, (double)ph[1] / n_iter, (double)ph[2] / n_iter);
+      printf("block %d sweep warp 0: cycles/iter wait-theta %.0f back1 %.0f wait-theta' %.0f back2+reduce %.0f front %.0f\n",
+             (int)blockIdx.x, (double)ph[0] / n_iter, (double)ph[3] / n_iter, (double)ph[4] / n_iter,
+             (double)ph[1] / n_iter, (double)ph[2] / n_iter);
 #endif
     bar_sync(BAR_THETA, RES_THREADS);                        // the last tail has finished
     bar_sync(BAR_THETAP, RES_THREADS);
@@ -241,6 +273,9 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
         tot[1] = t2[0]; tot[2] = t2[1];
       }
       HM_RSTAMP(1)
+#ifdef HM_TAIL_DELAY      /* scratch experiment: is the tail on the critical path? */
+      { const long long t_ = clock64(); while (clock64() - t_ < HM_TAIL_DELAY) {} }
+#endif
       tail_block(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, tw, SyncNamed<BAR_TAIL, RES_TW * 32>(),
                  ArriveNamed<BAR_THETA, RES_THREADS>());      // theta_{t+1} is signalled after the decision phase ...
       __threadfence_block();
