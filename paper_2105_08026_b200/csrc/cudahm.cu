@@ -170,7 +170,7 @@ Layout make_layout(const cudahm_config& c, int p, int ncols, int dtheta) {
   const size_t mom = c.keep_chi_moments ? (size_t)p * Npad * 8 : 0;
   l.mom_mean = take(mom); l.mom_M2 = take(mom); l.mom_var = take(mom);
   l.slots = take((size_t)MAX_BLOCKS * NPART * 8);
-  l.mbox = take((size_t)2 * MAX_PGRID * MAX_PGRID * 4 * 8);
+  l.mbox = take((size_t)2 * MAX_PGRID * MAX_PGRID * 2 * MBOX_NV * 8);
   l.blk_cnt = take((size_t)MAX_BLOCKS * 2 * 8);
   l.iter = take(sizeof(Iter));
   l.trace = take((size_t)c.max_trace_rows * dtheta * 8);

@@ -369,26 +369,37 @@ __device__ __forceinline__ void slots_reduce(const double* slots, int nblocks, d
 // sees the right epoch in a word has that word's data -- no fence, no arrival counter, no second read.  Mailboxes
 // alternate by iteration parity: a block can be at most one iteration ahead of the slowest reader (it needs
 // everybody's slot of iteration k to get past k).  Epochs increase over the sampler's lifetime.
-//   mbox layout: [parity][reader][value 0..1][writer][2 words]
-__device__ __forceinline__ void mbox_push(unsigned long long* mbox_parity, int G, int writer, unsigned epoch, double a, double b,
+//   mbox layout: [parity][reader][value 0..MBOX_NV-1][writer][2 words]; a kernel uses the first NV values
+constexpr int MBOX_NV = 3;
+__device__ __forceinline__ size_t mbox_parity_words(int G) { return (size_t)2 * MBOX_NV * G * G; }
+__device__ __forceinline__ size_t mbox_reader_words(int G) { return (size_t)2 * MBOX_NV * G; }
+template <int NV>
+__device__ __forceinline__ void mbox_push(unsigned long long* mbox_parity, int G, int writer, unsigned epoch, const double* val,
                                           int first, int stride) {
   const unsigned long long e = (unsigned long long)epoch << 32;
-  const unsigned long long ua = (unsigned long long)__double_as_longlong(a), ub = (unsigned long long)__double_as_longlong(b);
-  const unsigned long long a0 = e | (ua & 0xffffffffull), a1 = e | (ua >> 32), b0 = e | (ub & 0xffffffffull), b1 = e | (ub >> 32);
+  unsigned long long w0[NV], w1[NV];
+#pragma unroll
+  for (int q = 0; q < NV; ++q) {
+    const unsigned long long u = (unsigned long long)__double_as_longlong(val[q]);
+    w0[q] = e | (u & 0xffffffffull); w1[q] = e | (u >> 32);
+  }
   for (int r = first; r < G; r += stride) {
-    unsigned long long* box = mbox_parity + (size_t)r * 4 * G;
-    asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(box + 2 * writer), "l"(a0), "l"(a1) : "memory");
-    asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(box + 2 * G + 2 * writer), "l"(b0), "l"(b1) : "memory");
+    unsigned long long* box = mbox_parity + (size_t)r * mbox_reader_words(G);
+#pragma unroll
+    for (int q = 0; q < NV; ++q)
+      asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1, %2};" ::"l"(box + 2 * q * G + 2 * writer), "l"(w0[q]), "l"(w1[q]) : "memory");
   }
 }
 // Collect (warp 0): lane l owns writers l, l+32, ...; up to LL_BATCH of them are polled TOGETHER (independent
 // loads in flight: one L2 round trip once everything has arrived), then added in ascending order.
 constexpr int LL_BATCH = 5;   // ceil(148 / 32): the whole one-block-per-SM grid in one batch
-__device__ __forceinline__ void mbox_collect(const unsigned long long* box, int G, unsigned epoch, double* tot2) {
+template <int NV>
+__device__ __forceinline__ void mbox_collect(const unsigned long long* box, int G, unsigned epoch, double* tot) {
   const int lane = threadIdx.x & 31;
-  tot2[0] = 0.0; tot2[1] = 0.0;
+#pragma unroll
+  for (int q = 0; q < NV; ++q) tot[q] = 0.0;
   for (int g0 = lane; g0 < G; g0 += 32 * LL_BATCH) {
-    unsigned long long w[LL_BATCH][4];
+    unsigned long long w[LL_BATCH][2 * NV];
     bool ok;
     do {
       ok = true;
@@ -396,26 +407,29 @@ __device__ __forceinline__ void mbox_collect(const unsigned long long* box, int 
       for (int j = 0; j < LL_BATCH; ++j) {
         const int g = g0 + 32 * j;
         if (g < G) {
-          asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(w[j][0]), "=l"(w[j][1]) : "l"(box + 2 * g) : "memory");
-          asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(w[j][2]), "=l"(w[j][3]) : "l"(box + 2 * G + 2 * g) : "memory");
+#pragma unroll
+          for (int q = 0; q < NV; ++q)
+            asm volatile("ld.relaxed.gpu.global.v2.u64 {%0, %1}, [%2];" : "=l"(w[j][2 * q]), "=l"(w[j][2 * q + 1]) : "l"(box + 2 * q * G + 2 * g) : "memory");
         }
       }
 #pragma unroll
       for (int j = 0; j < LL_BATCH; ++j) {
-        if (g0 + 32 * j < G)
-          ok = ok && (unsigned)(w[j][0] >> 32) == epoch && (unsigned)(w[j][1] >> 32) == epoch &&
-               (unsigned)(w[j][2] >> 32) == epoch && (unsigned)(w[j][3] >> 32) == epoch;
+        if (g0 + 32 * j < G) {
+#pragma unroll
+          for (int q = 0; q < 2 * NV; ++q) ok = ok && (unsigned)(w[j][q] >> 32) == epoch;
+        }
       }
     } while (!ok);
 #pragma unroll
     for (int j = 0; j < LL_BATCH; ++j) {
       if (g0 + 32 * j < G) {
-        tot2[0] += __longlong_as_double((long long)((w[j][0] & 0xffffffffull) | (w[j][1] << 32)));
-        tot2[1] += __longlong_as_double((long long)((w[j][2] & 0xffffffffull) | (w[j][3] << 32)));
+#pragma unroll
+        for (int q = 0; q < NV; ++q)
+          tot[q] += __longlong_as_double((long long)((w[j][2 * q] & 0xffffffffull) | (w[j][2 * q + 1] << 32)));
       }
     }
   }
-  lanes_to_total<2>(tot2);
+  lanes_to_total<NV>(tot);
 }
 
 __device__ __forceinline__ void copy_iter(Iter* dst, const Iter* src) {
@@ -455,14 +469,15 @@ __global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const l
     cnt[0] += part[3]; cnt[1] += part[4];
     double dq[2] = {part[1], part[2]};
     block_reduce_all<2>(dq, red);
-    unsigned long long* mb = P.mbox + (size_t)(k & 1) * 4 * G * G;
+    constexpr int NVX = MODEL == M_THINNED_SCHECHTER1D ? 2 : 1;   // only M1 has a selection-integral slice to exchange
+    unsigned long long* mb = P.mbox + (size_t)(k & 1) * mbox_parity_words(G);
     const unsigned epoch = epoch0 + (unsigned)k;
-    mbox_push(mb, G, (int)blockIdx.x, epoch, dq[0], dq[1], (int)threadIdx.x, (int)blockDim.x);
+    mbox_push<NVX>(mb, G, (int)blockIdx.x, epoch, dq, (int)threadIdx.x, (int)blockDim.x);
     HM_STAMP(1)
     double tot[NPART] = {0.0, 0.0, 0.0, 0.0, 0.0};
     if (threadIdx.x < 32) {
-      double t2[2];
-      mbox_collect(mb + (size_t)blockIdx.x * 4 * G, G, epoch, t2);
+      double t2[2] = {0.0, 0.0};
+      mbox_collect<NVX>(mb + (size_t)blockIdx.x * mbox_reader_words(G), G, epoch, t2);
       tot[1] = t2[0]; tot[2] = t2[1];
     }
     HM_STAMP(2)

@@ -51,8 +51,10 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
   constexpr int ncols = V::ncols;
   extern __shared__ double sm[];
   __shared__ Iter it;
-  __shared__ double red[2][RES_SW][2];
+  __shared__ double red[2][RES_SW][1];
   __shared__ unsigned long long cnt_sm[2];
+  __shared__ double qtab[V::m1 ? 3 : 1][V::m1 ? NQUAD : 1];   // M1: quadrature weights W_k, nodes x_k, e^{x_k}
+  __shared__ double tq_warp[RES_TW];     // M1: the tail warps' partial sums of the selection integral at theta'
   const int tid = (int)threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const bool is_tail = warp >= RES_SW;
   const int G = (int)gridDim.x;
@@ -188,8 +190,9 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
           }
         }
       }
-      // back, part 2 (needs theta'_t, which the tail finishes a little later): population terms and the
-      // selection-integral slice
+      // back, part 2 (needs theta'_t, which the tail finishes a little later): population terms.  (M1's selection
+      // integral at theta' is computed by the tail warps, see below: every value less in the exchange is worth more
+      // than the arithmetic it saves -- a third mailbox value measured +0.7 us per iteration.)
       HM_RSTAMP(3)
       if (k > 0) bar_sync(BAR_THETAP, RES_THREADS);
       HM_RSTAMP(4)
@@ -204,16 +207,9 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
         if constexpr (V::m1) qn = typename PL::Pt{xn, HM_AT(V::V_E, r)}; else qn = PL::point(&xn);
         v[0] += PL::pop(qn, di, kp) - PL::pop(qn, di, kc);
       }
-      if (V::m1 && !P.tail.freeze_theta) {          // this thread's terms of the selection integral at theta'
-        for (int q = (int)blockIdx.x + G * tid; q < NQUAD; q += G * RES_S)
-          v[1] += P.qW[q] * hm_exp(kp.v[0] * (P.qx[q] - kp.v[1]) - P.qex[q] * kp.v[3]);
-      }
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) {
-        v[0] += __shfl_down_sync(0xffffffffu, v[0], o);
-        v[1] += __shfl_down_sync(0xffffffffu, v[1], o);
-      }
-      if (lane == 0) { red[k & 1][warp][0] = v[0]; red[k & 1][warp][1] = v[1]; }
+      for (int o = 16; o > 0; o >>= 1) v[0] += __shfl_down_sync(0xffffffffu, v[0], o);
+      if (lane == 0) red[k & 1][warp][0] = v[0];
       __threadfence_block();
       bar_arrive(BAR_PARTIALS, RES_THREADS);                 // hand the partials to the tail warps, do not wait
       HM_RSTAMP(1)
@@ -250,6 +246,33 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
     }
   } else {
     const int tw = warp - RES_SW, ttid = tid - RES_S;
+    // M1: T(theta') needs sum_k W_k phi(x_k; theta') over the 1,024 quadrature nodes.  Every block computes the
+    // whole sum itself on its tail warps right after theta' is known -- while the sweep warps are busy with the
+    // next back -- in a fixed order: all blocks hold the same bits and only ONE value per block (Delta) has to be
+    // exchanged.  Node tables in shared memory (24 KB), loaded once per launch.
+    constexpr int QPT = NQUAD / (RES_TW * 32);
+    static_assert(NQUAD % (RES_TW * 32) == 0, "quadrature nodes must divide over the tail threads");
+    if constexpr (V::m1) {
+      for (int q = ttid; q < NQUAD; q += RES_TW * 32) { qtab[0][q] = P.qW[q]; qtab[1][q] = P.qx[q]; qtab[2][q] = P.qex[q]; }
+    }
+    auto selection_full = [&]() {
+      if constexpr (V::m1) {
+        if (!P.tail.freeze_theta) {
+          const double k0 = it.kp.v[0], k1 = it.kp.v[1], k3 = it.kp.v[3];
+          double s_ = 0.0;
+#pragma unroll
+          for (int m = 0; m < QPT; ++m) {
+            const int q = ttid + m * RES_TW * 32;
+            s_ += qtab[0][q] * hm_exp(k0 * (qtab[1][q] - k1) - qtab[2][q] * k3);
+          }
+#pragma unroll
+          for (int o = 16; o > 0; o >>= 1) s_ += __shfl_down_sync(0xffffffffu, s_, o);
+          if (lane == 0) tq_warp[tw] = s_;
+        }
+        bar_sync(BAR_TAIL, RES_TW * 32);
+      }
+    };
+    selection_full();
 #ifdef HM_PHASE_TIMING
     long long ph[4] = {0, 0, 0, 0}, last_ = 0;
 #endif
@@ -259,18 +282,18 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
 #endif
       bar_sync(BAR_PARTIALS, RES_THREADS);                   // the block's 16 warp partials of iteration t0 + k
       HM_RSTAMP(0)
-      double dq[2];
+      double dq[1];
       dq[0] = lane < RES_SW ? red[k & 1][lane][0] : 0.0;
-      dq[1] = lane < RES_SW ? red[k & 1][lane][1] : 0.0;
-      lanes_to_total<2>(dq);
-      unsigned long long* mb = P.mbox + (size_t)(k & 1) * 4 * G * G;
+      lanes_to_total<1>(dq);
+      unsigned long long* mb = P.mbox + (size_t)(k & 1) * mbox_parity_words(G);
       const unsigned epoch = epoch0 + (unsigned)k;
-      mbox_push(mb, G, (int)blockIdx.x, epoch, dq[0], dq[1], ttid, RES_TW * 32);
+      mbox_push<1>(mb, G, (int)blockIdx.x, epoch, dq, ttid, RES_TW * 32);
       double tot[NPART] = {0.0, 0.0, 0.0, 0.0, 0.0};
       if (tw == 0) {
-        double t2[2];
-        mbox_collect(mb + (size_t)blockIdx.x * 4 * G, G, epoch, t2);
-        tot[1] = t2[0]; tot[2] = t2[1];
+        double t1[1];
+        mbox_collect<1>(mb + (size_t)blockIdx.x * mbox_reader_words(G), G, epoch, t1);
+        tot[1] = t1[0];
+        if constexpr (V::m1) tot[2] = ((tq_warp[0] + tq_warp[1]) + tq_warp[2]) + tq_warp[3];
       }
       HM_RSTAMP(1)
 #ifdef HM_TAIL_DELAY      /* scratch experiment: is the tail on the critical path? */
@@ -280,6 +303,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
                  ArriveNamed<BAR_THETA, RES_THREADS>());      // theta_{t+1} is signalled after the decision phase ...
       __threadfence_block();
       bar_arrive(BAR_THETAP, RES_THREADS);                   // ... theta'_{t+1} and its constants when the tail is done
+      selection_full();                                      // M1: for the NEXT decision; off the critical path
       HM_RSTAMP(2)
     }
 #ifdef HM_PHASE_TIMING

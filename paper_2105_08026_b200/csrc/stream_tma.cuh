@@ -144,13 +144,14 @@ __global__ void __launch_bounds__(BLOCK_ALL, 1) k_persistent_tma(const Params P,
     if (producer && lane == 0 && k + 1 < n_iter) {       // ... before the async proxy re-reads them for iteration k+1:
       for (int j = 0; j < n_pre; ++j) request(j, q + j); //     requested now, they land during the exchange and the tail
     }
-    unsigned long long* mb = P.mbox + (size_t)(k & 1) * 4 * G * G;
+    constexpr int NVX = MODEL == M_THINNED_SCHECHTER1D ? 2 : 1;   // only M1 has a selection-integral slice to exchange
+    unsigned long long* mb = P.mbox + (size_t)(k & 1) * mbox_parity_words(G);
     const unsigned epoch = epoch0 + (unsigned)k;
-    mbox_push(mb, G, (int)blockIdx.x, epoch, dq[0], dq[1], tid, BLOCK_ALL);
+    mbox_push<NVX>(mb, G, (int)blockIdx.x, epoch, dq, tid, BLOCK_ALL);
     double tot[NPART] = {0.0, 0.0, 0.0, 0.0, 0.0};
     if (tid < 32) {
-      double t2[2];
-      mbox_collect(mb + (size_t)blockIdx.x * 4 * G, G, epoch, t2);
+      double t2[2] = {0.0, 0.0};
+      mbox_collect<NVX>(mb + (size_t)blockIdx.x * mbox_reader_words(G), G, epoch, t2);
       tot[1] = t2[0]; tot[2] = t2[1];
     }
     tail_block(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, tid >> 5, SyncAll());
