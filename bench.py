@@ -36,10 +36,10 @@ UNIT = "updates/s"
 ALG_BYTES = {"C0": (48, 32), "C1": (48, 32), "C2": (48, 32), "C3": (112, 64), "C4": (28, 32)}
 MODES = {"host": 0, "graph": 1, "tail": 2}
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel PER GIBBS ITERATION, from the committed
-# `ncu --set full` captures (profiles/r01d_resident_C2_ncu.md: 14.57 MB + 0.27 MB over 300 iterations;
-# profiles/r01d_persistent_C4_ncu.md: 5.947 GB + 2.373 GB over 30 iterations); scaled to the K iterations one timed
+# `ncu --set full` captures (profiles/r01f_resident_C2_ncu.md: 14.60 MB + 0.075 MB over 300 iterations;
+# profiles/r01f_persistent_C4_ncu.md: 5.940 GB + 2.363 GB over 30 iterations); scaled to the K iterations one timed
 # launch runs.  C2 keeps its state in shared memory, so its DRAM traffic is ~0.2 % of the algorithmic bytes.
-NCU_DRAM_BYTES_PER_ITER = {"C2": (14.569984e6 + 271.104e3) / 300, "C4": (5.947117e9 + 2.373307e9) / 30}
+NCU_DRAM_BYTES_PER_ITER = {"C2": (14.599424e6 + 75.008e3) / 300, "C4": (5.940074e9 + 2.362765e9) / 30}
 
 
 def parse_args():
