@@ -9,7 +9,7 @@ import numpy as np
 
 from . import build as _build
 
-M_NORMAL1D, M_THINNED_SCHECHTER1D, M_BINORMAL2D, M_LINREG_ME1D = 0, 1, 2, 3
+M_NORMAL1D, M_THINNED_SCHECHTER1D, M_BINORMAL2D, M_LINREG_ME1D, M_BB1_FLUXNOISE1D = 0, 1, 2, 3, 4
 F64, F32_STATE_F64_REDUCE = 0, 1
 KIND_PLATE, KIND_THETA = 0, 1
 
@@ -93,6 +93,10 @@ def lib():
         L.oracle_ram_update.restype = None
         L.oracle_gauss_legendre.argtypes = [C.c_int, C.c_double, C.c_double, _dp, _dp]
         L.oracle_gauss_legendre.restype = None
+        L.oracle_bb1_log_norm.argtypes = [C.c_double] * 3
+        L.oracle_bb1_log_norm.restype = C.c_double
+        L.oracle_bb1_selection_integral_2d.argtypes = [_dp, _dp]
+        L.oracle_bb1_selection_integral_2d.restype = C.c_double
         L.oracle_sum.argtypes = [_dp, C.c_int64]
         L.oracle_sum.restype = C.c_double
         _lib = L
@@ -314,6 +318,14 @@ def gauss_legendre(n, a, b):
     x, w = np.empty(n), np.empty(n)
     lib().oracle_gauss_legendre(n, a, b, _d(x), _d(w))
     return x, w
+
+
+def bb1_log_norm(beta, l, u):
+    return lib().oracle_bb1_log_norm(beta, l, u)
+
+
+def bb1_selection_integral_2d(theta, consts):
+    return lib().oracle_bb1_selection_integral_2d(_d(_arr(theta)), _d(_arr(consts)))
 
 
 def osum(v):

@@ -1,4 +1,4 @@
-// oracle/models.hpp -- the four compiled-in models, written out plainly.  TEST INFRASTRUCTURE ONLY.
+// oracle/models.hpp -- the five compiled-in models, written out plainly.  TEST INFRASTRUCTURE ONLY.
 //
 // The paper asks the user for two functions: the member log-likelihood
 // log l_i(chi) and the population log-density log f(chi; theta);
@@ -12,7 +12,7 @@
 
 namespace oracle {
 
-enum Model { M_NORMAL1D = 0, M_THINNED_SCHECHTER1D = 1, M_BINORMAL2D = 2, M_LINREG_ME1D = 3 };
+enum Model { M_NORMAL1D = 0, M_THINNED_SCHECHTER1D = 1, M_BINORMAL2D = 2, M_LINREG_ME1D = 3, M_BB1_FLUXNOISE1D = 4 };
 
 struct Dims { int p, dtheta, n_cols, n_consts; };
 inline bool model_dims(int model, Dims* d) {
@@ -21,12 +21,28 @@ inline bool model_dims(int model, Dims* d) {
     case M_THINNED_SCHECHTER1D: *d = {1, 3, 2, 6}; return true;   // cols Fhat, g=1/(4 pi r^2); theta (alpha, x*, a)
     case M_BINORMAL2D:          *d = {2, 5, 4, 0}; return true;   // cols y1,y2,s1,s2;       theta (m1,m2,l1,l2,zeta)
     case M_LINREG_ME1D:         *d = {1, 3, 3, 0}; return true;   // cols y, sigma, z;       theta (a, b, log tau)
+    case M_BB1_FLUXNOISE1D:     *d = {1, 3, 2, 7}; return true;   // cols Fhat, g=1/(4 pi r^2); theta (beta, ln l, ln u)
   }
   return false;
 }
 
 // consts of M1: {F_lim, sigma_F, x_lo, x_hi, r_min, r_max}
 enum { C_FLIM = 0, C_SIGF = 1, C_XLO = 2, C_XHI = 3, C_RMIN = 4, C_RMAX = 5 };
+// consts of M4 (the paper's case study): {sigma_0, alpha (the noise slope of Eq. 5.8), x_lo, x_hi,
+// r_min, r_max, F_th}; x_lo .. r_max sit at the same indices as in M1
+enum { B_SIG0 = 0, B_ANOISE = 1, B_FTH = 6 };
+
+// log C(beta, u, l), the BB1 normaliser of PAPER.md:429 (Eq. C.3):
+//   C = 1 / (Gamma(beta+1) (1 - (1 + u/l)^-(beta+1)))   (beta > -2, beta != -1),     C = 1/log(1 + u/l)  (beta = -1).
+// For -2 < beta < -1 both factors are negative, the product is positive; near beta = -1 each factor keeps its
+// relative accuracy (lgamma; expm1/log1p), so the 0 x inf product is harmless.
+inline double bb1_log_norm(double beta, double l, double u) {
+  const double b1 = beta + 1.0;
+  const double A = std::log1p(u / l);
+  if (b1 == 0.0) return -std::log(A);
+  const double q = -std::expm1(-b1 * A);              // 1 - (1 + u/l)^-(beta+1)
+  return -(std::lgamma(b1) + std::log(std::fabs(q)));
+}
 
 // ---- member log-likelihood  log l_i(chi) ------------------------------------------------------
 template <class T>
@@ -44,6 +60,15 @@ inline T loglik(int model, const T* chi, const T* d, const T* consts) {
     case M_BINORMAL2D: {                        // independent Gaussian errors per axis
       const T r1 = d[0] - chi[0], r2 = d[1] - chi[1];
       return -T(0.5) * ((r1 * r1) / (d[2] * d[2]) + (r2 * r2) / (d[3] * d[3]));
+    }
+    case M_BB1_FLUXNOISE1D: {
+      // Fhat ~ N(F, sigma(F)^2), sigma(F)^2 = sigma_0^2 + (alpha F)^2 (Eq. 5.8), F = L/(4 pi r^2),
+      // L = e^chi; the member likelihood is the sampling density as a function of F -- the g(n_obs; F) choice
+      // of PAPER.md:298-321 (Eq. 5.6), NOT Gaussian in F: the 1/sigma(F) factor stays.
+      const T F = d[1] * std::exp(chi[0]);
+      const T s2 = consts[B_SIG0] * consts[B_SIG0] + (consts[B_ANOISE] * F) * (consts[B_ANOISE] * F);
+      const T r = d[0] - F;
+      return -T(0.5) * std::log(s2) - (r * r) / (T(2) * s2);
     }
   }
   return std::numeric_limits<T>::quiet_NaN();
@@ -73,6 +98,15 @@ inline T logpop(int model, const T* chi, const T* d, const T* th, const T* const
       const T rho = std::tanh(th[4]);
       return -th[2] - th[3] + std::log(ch) - ch * ch * (u1 * u1 - T(2) * rho * u1 * u2 + u2 * u2) / T(2);
     }
+    case M_BB1_FLUXNOISE1D: {
+      // BB1 luminosity PDF, PAPER.md:256 (Eq. 5.1) = :423 (Eq. C.2), as a density in x = ln L (Jacobian L):
+      //   L f(L) = C (L/u)^(beta+1) (1 - e^(-L/l)) e^(-L/u),   theta = (beta, ln l, ln u);
+      // truncated to [x_lo, x_hi] (large L "formally excluded by truncation").
+      if (!(chi[0] >= consts[C_XLO] && chi[0] <= consts[C_XHI])) return -std::numeric_limits<T>::infinity();
+      const T Lum = std::exp(chi[0]), l = std::exp(th[1]), u = std::exp(th[2]);
+      const T logC = (T)bb1_log_norm((double)th[0], (double)l, (double)u);
+      return logC + (th[0] + T(1)) * (chi[0] - th[2]) + std::log(-std::expm1(-Lum / l)) - Lum / u;
+    }
   }
   return std::numeric_limits<T>::quiet_NaN();
 }
@@ -96,6 +130,13 @@ inline double logprior(int model, const double* th) {
     case M_THINNED_SCHECHTER1D:
       if (!(th[0] > -2.0 && th[0] < 0.0 && std::fabs(th[1]) <= 20.0 && std::fabs(th[2]) <= 50.0)) return ninf;
       return -std::log(1.0 + th[0] * th[0]);
+    case M_BB1_FLUXNOISE1D:
+      // PAPER.md:277-290 (Eq. 5.3-5.5): truncated Cauchy in beta on (-2, 0), log-flat in u, flat in l on l < u
+      // (p(l|u) = 1/u).  As a density in the sampled coordinates (beta, ln l, ln u) that is
+      // l / (u (1 + beta^2)) -- Eq. 5.5 as printed (reading R17); box |ln l|, |ln u| <= 30 keeps it proper.
+      if (!(th[0] > -2.0 && th[0] < 0.0 && th[1] < th[2] && std::fabs(th[1]) <= 30.0 && std::fabs(th[2]) <= 30.0))
+        return ninf;
+      return th[1] - th[2] - std::log(1.0 + th[0] * th[0]);
   }
   return ninf;
 }
@@ -141,6 +182,65 @@ inline void gauss_legendre(int n, double a, double b, double* x, double* w) {
 // G itself by a 256-point rule in r (BASELINE.json configs[1]; reading R9).
 struct SelectionTable {
   std::vector<double> xk, Wk;
+  // M4: eta(F) = Phi((F - F_th)/sigma(F)) with the flux-dependent sigma of Eq. 5.8 (Eq. 5.10).  eta does
+  // not depend on theta, so the paper's 2-D cubature again factorises: G(x) is tabulated once.
+  // Inner rule: 512-point Gauss-Legendre in q = ln r on [ln r_min, ln r_max] (h(r) dr = 3 e^(3q) dq/(rmax^3 - rmin^3));
+  // the detection edge has a fixed width (1/(2 nu) ~ 0.1) in q wherever it falls, which a rule in r would not resolve
+  // at small L.  selection_integral_2d() below is the same tensor-product rule written as the plain double sum.
+  static double eta_bb1(double F, const double* c) {
+    const double sg = std::sqrt(c[B_SIG0] * c[B_SIG0] + (c[B_ANOISE] * F) * (c[B_ANOISE] * F));
+    return 0.5 * std::erfc(-((F - c[B_FTH]) / sg) / 1.4142135623730950488016887242097);
+  }
+  void build_bb1(const double* c) {
+    const int NX = 1024, NQ = 512;
+    const double four_pi = 12.566370614359172953850573533118;
+    xk.assign(NX, 0.0); Wk.assign(NX, 0.0);
+    std::vector<double> wx(NX), qj(NQ), wq(NQ);
+    gauss_legendre(NX, c[C_XLO], c[C_XHI], xk.data(), wx.data());
+    gauss_legendre(NQ, std::log(c[C_RMIN]), std::log(c[C_RMAX]), qj.data(), wq.data());
+    const double vol = c[C_RMAX] * c[C_RMAX] * c[C_RMAX] - c[C_RMIN] * c[C_RMIN] * c[C_RMIN];
+    for (int k = 0; k < NX; ++k) {
+      long double G = 0.0L;
+      for (int j = 0; j < NQ; ++j) {
+        const double r = std::exp(qj[j]);
+        const double F = std::exp(xk[k]) / (four_pi * r * r);
+        G += (long double)(wq[j] * (3.0 * r * r * r / vol) * eta_bb1(F, c));
+      }
+      Wk[k] = wx[k] * (double)G;
+    }
+  }
+  // I(theta) = int dx rho(x; theta) G(x), the denominator of Eq. 4.4; T(theta) = -N log I(theta) is the
+  // theta-only term of log L = sum_i [log rho(x_i) + log l_i] - N log I   (Eq. 4.3 with mu = h rho / I).
+  double bb1_integral(const double* th, const double* c) const {
+    long double acc = 0.0L;
+    double x[1], d[2] = {0.0, 0.0};
+    for (size_t k = 0; k < xk.size(); ++k) {
+      x[0] = xk[k];
+      acc += (long double)(Wk[k] * std::exp(logpop<double>(M_BB1_FLUXNOISE1D, x, d, th, c)));
+    }
+    return (double)acc;
+  }
+  // the same integral as the plain 2-D tensor-product cubature, nothing tabulated (slow; pins the table route)
+  static double selection_integral_2d(const double* th, const double* c) {
+    const int NX = 1024, NQ = 512;
+    const double four_pi = 12.566370614359172953850573533118;
+    std::vector<double> xs(NX), wx(NX), qj(NQ), wq(NQ);
+    gauss_legendre(NX, c[C_XLO], c[C_XHI], xs.data(), wx.data());
+    gauss_legendre(NQ, std::log(c[C_RMIN]), std::log(c[C_RMAX]), qj.data(), wq.data());
+    const double vol = c[C_RMAX] * c[C_RMAX] * c[C_RMAX] - c[C_RMIN] * c[C_RMIN] * c[C_RMIN];
+    long double acc = 0.0L;
+    double x[1], d[2] = {0.0, 0.0};
+    for (int k = 0; k < NX; ++k) {
+      x[0] = xs[k];
+      const double rho = std::exp(logpop<double>(M_BB1_FLUXNOISE1D, x, d, th, c));
+      for (int j = 0; j < NQ; ++j) {
+        const double r = std::exp(qj[j]);
+        const double F = std::exp(xs[k]) / (four_pi * r * r);
+        acc += (long double)(wx[k] * wq[j] * rho * (3.0 * r * r * r / vol) * eta_bb1(F, c));
+      }
+    }
+    return (double)acc;
+  }
   void build(const double* c) {
     const int NX = 1024, NR = 256;
     const double four_pi = 12.566370614359172953850573533118;

@@ -8,6 +8,7 @@
  *   - theta Metropolis-Hastings step with the population
  *     log-posterior sum
  *   - thinned latent point process likelihood               PAPER.md:228-236 (Eq. 4.3, 4.4)
+ *   - BB1 luminosity PDF, priors, flux noise, detection     PAPER.md:256-333 (Eq. 5.1-5.10), :423-450 (Eq. C.2-C.6)
  * It shares no code, header, table or constant with paper_2105_08026_b200/csrc (the CUDA path).
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may
  * load it.  All pointers are HOST pointers.  All arrays are structure-of-arrays:
@@ -28,7 +29,8 @@ typedef struct oracle_sampler oracle_sampler;
 
 enum { ORACLE_OK = 0, ORACLE_E_INVALID = -1, ORACLE_E_STATE = -2, ORACLE_E_UNSUPPORTED = -5 };
 /* models: */
-enum { ORACLE_M_NORMAL1D = 0, ORACLE_M_THINNED_SCHECHTER1D = 1, ORACLE_M_BINORMAL2D = 2, ORACLE_M_LINREG_ME1D = 3 };
+enum { ORACLE_M_NORMAL1D = 0, ORACLE_M_THINNED_SCHECHTER1D = 1, ORACLE_M_BINORMAL2D = 2, ORACLE_M_LINREG_ME1D = 3,
+       ORACLE_M_BB1_FLUXNOISE1D = 4 /* the paper's case study: BB1 population, flux-dependent noise */ };
 enum { ORACLE_F64 = 0, ORACLE_F32_STATE_F64_REDUCE = 1 };
 /* Philox stream kinds */
 enum { ORACLE_KIND_PLATE = 0, ORACLE_KIND_THETA = 1 };
@@ -114,6 +116,10 @@ float  oracle_logpop_f32(int model, const float* chi, const float* data_i, const
 double oracle_logprior(int model, const double* theta);
 void   oracle_ram_update(int p, const double* L_packed, const double* z, double c, double* L_out);
 void   oracle_gauss_legendre(int n, double a, double b, double* x, double* w);
+/* M4: log C(beta, u, l) of PAPER.md:429 (Eq. C.3); the selection integral (Eq. 4.4 denominator) as the plain
+ * 1,024 x 512 tensor-product cubature, nothing tabulated.  consts = {sigma_0, alpha, x_lo, x_hi, r_min, r_max, F_th} */
+double oracle_bb1_log_norm(double beta, double l, double u);
+double oracle_bb1_selection_integral_2d(const double* theta, const double* consts);
 double oracle_sum(const double* v, int64_t n);
 
 #ifdef __cplusplus

@@ -70,7 +70,10 @@ struct Base {
   virtual int get_state(double* chi, double* L, double* th, double* Lth, int64_t* tt) = 0;
   virtual int set_state(const double* chi, const double* L, const double* th, const double* Lth, int64_t tt) = 0;
   double theta_only(const double* th) const {
-    return cfg.model == M_THINNED_SCHECHTER1D ? table.theta_only(th) : 0.0;
+    if (cfg.model == M_THINNED_SCHECHTER1D) return table.theta_only(th);
+    // M4: log L = sum_i [log rho(x_i; theta) + log l_i(x_i)] - N log I(theta)   (Eq. 4.3-4.4)
+    if (cfg.model == M_BB1_FLUXNOISE1D) return -(double)cfg.n_objects * std::log(table.bb1_integral(th, consts.data()));
+    return 0.0;
   }
 };
 
@@ -97,7 +100,7 @@ struct Impl : Base {
     for (int64_t i = 0; i < N; ++i) {
       if (chi0) {
         for (int j = 0; j < p; ++j) chi[(size_t)j * N + i] = (T)chi0[(size_t)j * N + i];
-      } else if (cfg.model == M_THINNED_SCHECHTER1D) {
+      } else if (cfg.model == M_THINNED_SCHECHTER1D || cfg.model == M_BB1_FLUXNOISE1D) {
         // X_1 with pi(X_1) > 0: the flux estimate inverted, clamped to the support
         double x = std::log((double)data[i] / (double)data[(size_t)N + i]);
         x = std::min(std::max(x, consts[C_XLO]), consts[C_XHI]);
@@ -333,6 +336,7 @@ int oracle_set_model_consts(oracle_sampler* s, const double* v, int n) {
     f->consts_T.assign(v, v + n);
   }
   if (b->cfg.model == M_THINNED_SCHECHTER1D) b->table.build(b->consts.data());
+  if (b->cfg.model == M_BB1_FLUXNOISE1D) b->table.build_bb1(b->consts.data());
   b->have_consts = true;
   return ORACLE_OK;
 }
@@ -456,6 +460,10 @@ void oracle_ram_update(int p, const double* L_packed, const double* z, double c,
   ram_update<double>(p, L_packed, z, c, L_out);
 }
 void oracle_gauss_legendre(int n, double a, double b, double* x, double* w) { gauss_legendre(n, a, b, x, w); }
+double oracle_bb1_log_norm(double beta, double l, double u) { return bb1_log_norm(beta, l, u); }
+double oracle_bb1_selection_integral_2d(const double* theta, const double* consts) {
+  return SelectionTable::selection_integral_2d(theta, consts);
+}
 double oracle_sum(const double* v, int64_t n) {
   long double acc = 0.0L;
   for (int64_t i = 0; i < n; ++i) acc += (long double)v[i];

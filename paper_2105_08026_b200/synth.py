@@ -1,4 +1,4 @@
-"""Seeded synthetic inputs for the five BASELINE.json configs (C0..C4).
+"""Seeded synthetic inputs for the five BASELINE.json configs (C0..C4) and the paper's BB1 case study (C5).
 
 This module serves BOTH the CUDA path and the oracle and therefore holds none of the method's
 arithmetic (no log-density, no RAM step, no Philox stream of the sampler): it only simulates
@@ -12,7 +12,7 @@ from dataclasses import dataclass
 
 import numpy as np
 
-M_NORMAL1D, M_THINNED_SCHECHTER1D, M_BINORMAL2D, M_LINREG_ME1D = 0, 1, 2, 3
+M_NORMAL1D, M_THINNED_SCHECHTER1D, M_BINORMAL2D, M_LINREG_ME1D, M_BB1_FLUXNOISE1D = 0, 1, 2, 3, 4
 F64, F32_STATE_F64_REDUCE = 0, 1
 
 
@@ -38,11 +38,26 @@ CONFIGS = {
     "C2": RunConfig("C2", M_THINNED_SCHECHTER1D, F64, 300_000, 10_000, 2_000, 10, 0.44, 0.234, True, 2),
     "C3": RunConfig("C3", M_BINORMAL2D, F64, 1_000_000, 5_000, 1_000, 1, 0.234, 0.234, False, 3),
     "C4": RunConfig("C4", M_LINREG_ME1D, F32_STATE_F64_REDUCE, 10_000_000, 2_000, 500, 1, 0.44, 0.234, False, 4),
+    # the paper's own case study (Table 5.1): BB1 population, N = 1e5
+    "C5": RunConfig("C5", M_BB1_FLUXNOISE1D, F64, 100_000, 5_000, 1_000, 1, 0.44, 0.234, False, 5),
 }
 
 # constants of the thinned point-process configs: {F_lim, sigma_F, x_lo, x_hi, r_min, r_max}
 SCHECHTER_CONSTS = np.array([1e-3, 1e-4, np.log(1e-4), np.log(30.0), 1.0, 10.0 ** (1.0 / 3.0)])
 SCHECHTER_TRUTH = (-1.2, 0.0)   # (alpha, x* = log L*)
+
+
+# BB1 case study.  Units: luminosity in 1e10 L_sun (u_true = 1, l_true = 0.01), distance in
+# Gpc (r_max = 1), flux in (1e10 L_sun)/Gpc^2, so F_fid = u/(4 pi r_max^2) = 1/(4 pi) (Eq. 5.2).
+# nu = 5, alpha = 0.01.  The printed sigma_0 and F_th are inconsistent with "L = 20 u at r_max is
+# just detectable" (reading R18); the text's statement is kept: F_th = 20 F_fid, and sigma_0 follows from
+# F_th = nu sigma(F_th), i.e. sigma_0 = F_th sqrt(1 - nu^2 alpha^2)/nu (Eq. 5.9 with the nu^2 restored).
+BB1_TRUTH = (-1.5, np.log(0.01), 0.0)          # (beta, ln l, ln u)           PAPER.md:262, Table 5.1
+BB1_NU, BB1_ALPHA_NOISE = 5.0, 1e-2
+BB1_FTH = 20.0 / (4.0 * np.pi)
+BB1_SIGMA0 = BB1_FTH * np.sqrt(1.0 - (BB1_NU * BB1_ALPHA_NOISE) ** 2) / BB1_NU
+# constants of the model: {sigma_0, alpha, x_lo, x_hi, r_min, r_max, F_th}
+BB1_CONSTS = np.array([BB1_SIGMA0, BB1_ALPHA_NOISE, np.log(1e-5), np.log(30.0), 1e-4, 1.0, BB1_FTH])
 
 
 def _rng(seed):
@@ -104,6 +119,50 @@ def make_thinned_schechter1d(n, seed=1):
                 detected_fraction=n / max(drawn, 1))
 
 
+def make_bb1_fluxnoise1d(n, seed=5, truth=BB1_TRUTH):
+    """C5, the paper's case study: L ~ BB1(beta, l, u) (Eq. 5.1), r uniform in volume on
+    [r_min, r_max], F = L/(4 pi r^2), Fhat = F + sigma(F) eps with sigma(F)^2 = sigma_0^2 + (alpha F)^2 (Eq. 5.8), kept
+    iff Fhat > F_th.  Only ~1e-3 of the population is detectable, so candidates are drawn where detection is
+    possible at all: r <= R(x) = min(r_max, 3 r_det(x)), r_det = sqrt(L/(4 pi F_th)) (beyond 3 r_det the flux is below
+    F_th/9, 40 sigma under the threshold), and x = ln L from the BB1 density times the probability of r <= R(x).
+    That is the full process conditioned on an event every detection satisfies (up to Phi(-40))."""
+    g = _rng(seed)
+    sig0, a_n, x_lo, x_hi, r_min, r_max, F_th = BB1_CONSTS
+    beta, ll, lu = truth
+    grid = np.linspace(x_lo, x_hi, 400_001)
+    Lum = np.exp(grid)
+    dens = np.exp((beta + 1.0) * (grid - lu) - Lum / np.exp(lu)) * -np.expm1(-Lum / np.exp(ll))   # L f(L) / C
+    R3 = np.minimum(r_max, 3.0 * np.sqrt(Lum / (4.0 * np.pi * F_th))) ** 3
+    vfrac = np.clip((R3 - r_min ** 3) / (r_max ** 3 - r_min ** 3), 0.0, 1.0)
+    w = dens * vfrac
+    cdf = np.concatenate([[0.0], np.cumsum(0.5 * (w[1:] + w[:-1]) * np.diff(grid))])
+    reach = cdf[-1] / np.trapezoid(dens, grid)          # share of the population drawn from at all
+    cdf /= cdf[-1]
+    xs, Fh, gs = [], [], []
+    kept, drawn = 0, 0
+    while kept < n:
+        m = max(4096, int(1.2 * (n - kept) / 0.03))
+        x = np.interp(g.uniform(size=m), cdf, grid)
+        Rx = np.minimum(r_max, 3.0 * np.sqrt(np.exp(x) / (4.0 * np.pi * F_th)))
+        r = (r_min ** 3 + g.uniform(size=m) * np.maximum(Rx ** 3 - r_min ** 3, 0.0)) ** (1.0 / 3.0)
+        gi = 1.0 / (4.0 * np.pi * r * r)
+        F = np.exp(x) * gi
+        Fhat = F + np.sqrt(sig0 ** 2 + (a_n * F) ** 2) * g.standard_normal(m)
+        ok = np.flatnonzero(Fhat > F_th)
+        if kept + ok.size >= n:
+            ok = ok[: n - kept]
+            drawn += int(ok[-1]) + 1 if ok.size else 0
+        else:
+            drawn += m
+        kept += ok.size
+        xs.append(x[ok]); Fh.append(Fhat[ok]); gs.append(gi[ok])
+    x, Fhat, gi = np.concatenate(xs), np.concatenate(Fh), np.concatenate(gs)
+    th = np.array([beta, ll, lu])
+    return dict(model=M_BB1_FLUXNOISE1D, cols=[Fhat, gi], consts=BB1_CONSTS.copy(), chi_true=x[None, :],
+                theta_true=th, theta0=th + np.array([0.03, 0.1, 0.03]),
+                detected_fraction=reach * n / max(drawn, 1))
+
+
 def make_binormal2d(n, seed=3, fp32=False):
     """C3: chi ~ N2(m, Sigma), m=(0,0.5), sds (1, e^-0.5), rho=0.3; per-axis sigma ~ U(0.05,0.3)."""
     g = _rng(seed)
@@ -138,7 +197,7 @@ def make_linreg_me1d(n, seed=4, fp32=True):
 
 
 def make_inputs(config_name, n_objects=None):
-    """Inputs of config C0..C4; n_objects overrides N (reduced-size parity cases keep the recipe)."""
+    """Inputs of config C0..C5; n_objects overrides N (reduced-size parity cases keep the recipe)."""
     c = CONFIGS[config_name]
     n = c.n_objects if n_objects is None else int(n_objects)
     if c.model == M_NORMAL1D:
@@ -147,4 +206,6 @@ def make_inputs(config_name, n_objects=None):
         return make_thinned_schechter1d(n, c.seed)
     if c.model == M_BINORMAL2D:
         return make_binormal2d(n, c.seed)
+    if c.model == M_BB1_FLUXNOISE1D:
+        return make_bb1_fluxnoise1d(n, c.seed)
     return make_linreg_me1d(n, c.seed, fp32=(c.precision == F32_STATE_F64_REDUCE))
