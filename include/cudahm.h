@@ -47,7 +47,11 @@ enum { CUDAHM_OK = 0, CUDAHM_E_INVALID = -1, CUDAHM_E_STATE = -2, CUDAHM_E_CUDA 
 enum { CUDAHM_M_NORMAL1D = 0,            /* (1, 2, {y, sigma}, 0)            theta = (mu, log tau)              */
        CUDAHM_M_THINNED_SCHECHTER1D = 1, /* (1, 3, {Fhat, g=1/(4 pi r^2)}, 6) theta = (alpha, log L*, log A)     */
        CUDAHM_M_BINORMAL2D = 2,          /* (2, 5, {y1, y2, s1, s2}, 0)      theta = (m1, m2, l1, l2, zeta)      */
-       CUDAHM_M_LINREG_ME1D = 3 };       /* (1, 3, {y, sigma, z}, 0)         theta = (a, b, log tau)            */
+       CUDAHM_M_LINREG_ME1D = 3,         /* (1, 3, {y, sigma, z}, 0)         theta = (a, b, log tau)            */
+       /* the paper's case study: BB1 luminosity PDF (Eq. 5.1 / C.2-C.3) in x = ln L, member
+        * likelihood = sampling density of Fhat in F with sigma(F)^2 = sigma_0^2 + (alpha F)^2 (Eq. 5.6, 5.8), prior of
+        * Eq. 5.5, selection term -N log I(theta) of Eq. 4.3-4.4 with eta of Eq. 5.10                              */
+       CUDAHM_M_BB1_FLUXNOISE1D = 4 };   /* (1, 3, {Fhat, g=1/(4 pi r^2)}, 7) theta = (beta, log l, log u)       */
 enum { CUDAHM_F64 = 0, CUDAHM_F32_STATE_F64_REDUCE = 1 };
 /* where the theta Metropolis-Hastings step runs (PAPER.md:142 puts it on the host) */
 enum { CUDAHM_THETA_HOST = 0,         /* one sweep launch + one sync per iteration; theta step in host C++     */
@@ -129,8 +133,9 @@ void cudahm_destroy(cudahm_sampler* s);
  * buffers may be freed afterwards.  Member likelihoods l_i are built from them. */
 int cudahm_set_data(cudahm_sampler* s, const void* const* cols, int n_cols, int cols_on_device);
 
-/* Model constants (host doubles).  THINNED_SCHECHTER1D: {F_lim, sigma_F, x_lo, x_hi, r_min, r_max}; builds the
- * 1,024-point selection-integral table (Eq. 4.4 denominator).  Other models take n = 0. */
+/* Model constants (host doubles).  THINNED_SCHECHTER1D: {F_lim, sigma_F, x_lo, x_hi, r_min, r_max};
+ * BB1_FLUXNOISE1D: {sigma_0, alpha, x_lo, x_hi, r_min, r_max, F_th} (Eq. 5.8-5.10).  Builds the 1,024-point
+ * selection-integral table (Eq. 4.4 denominator).  Other models take n = 0. */
 int cudahm_set_model_consts(cudahm_sampler* s, const double* v, int n);
 
 /* Initial state: chi0 (p*N values of type T, host or device per chi0_on_device; NULL = the model's default

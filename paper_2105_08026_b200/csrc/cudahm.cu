@@ -69,6 +69,7 @@ const void* pick_resident(int model, int precision, int keep_moments, int* n_val
     case M_NORMAL1D:            *n_values = ResValues<M_NORMAL1D>::n_base + mom; return (const void*)k_resident<M_NORMAL1D>;
     case M_THINNED_SCHECHTER1D: *n_values = ResValues<M_THINNED_SCHECHTER1D>::n_base + mom; return (const void*)k_resident<M_THINNED_SCHECHTER1D>;
     case M_LINREG_ME1D:         *n_values = ResValues<M_LINREG_ME1D>::n_base + mom; return (const void*)k_resident<M_LINREG_ME1D>;
+    case M_BB1_FLUXNOISE1D:     *n_values = ResValues<M_BB1_FLUXNOISE1D>::n_base + mom; return (const void*)k_resident<M_BB1_FLUXNOISE1D>;
   }
   return nullptr;
 }
@@ -80,6 +81,7 @@ bool pick_kernels(int model, int precision, int block, KernelSet* k) {
       case M_THINNED_SCHECHTER1D: return pick_block<M_THINNED_SCHECHTER1D, double>(block, k);
       case M_BINORMAL2D:          return pick_block<M_BINORMAL2D, double>(block, k);
       case M_LINREG_ME1D:         return pick_block<M_LINREG_ME1D, double>(block, k);
+      case M_BB1_FLUXNOISE1D:     return pick_block<M_BB1_FLUXNOISE1D, double>(block, k);
     }
   } else if (precision == CUDAHM_F32_STATE_F64_REDUCE) {
     switch (model) {
@@ -282,7 +284,7 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
   P.astar_chi = cfg->target_accept_chi;
   P.max_blocks = MAX_BLOCKS;
   P.tail = TailCfg{cfg->model, dt, cfg->freeze_theta ? 1 : 0, cfg->keep_chi_moments ? 1 : 0, cfg->seed,
-                   cfg->target_accept_theta, cfg->eta_exponent, 0, cfg->max_trace_rows, 1, 0};
+                   cfg->target_accept_theta, cfg->eta_exponent, 0, cfg->max_trace_rows, 1, 0, (double)cfg->n_objects};
   P.taps = DevTaps{};
 
   if (cudaMemsetAsync(s->ws, 0, lay.total, s->stream) != cudaSuccess ||
@@ -378,26 +380,51 @@ extern "C" int cudahm_set_model_consts(cudahm_sampler* s, const double* v, int n
   if (!s) return fail(s, CUDAHM_E_INVALID, "NULL handle");
   if (n != s->nconsts || (n > 0 && !v)) return fail(s, CUDAHM_E_INVALID, "model takes %d constants, got %d", s->nconsts, n);
   if (n == 0) { s->have_consts = true; return CUDAHM_OK; }
-  // THINNED_SCHECHTER1D: {F_lim, sigma_F, x_lo, x_hi, r_min, r_max}
-  if (!(v[MC_SIGF] > 0.0 && v[MC_XHI] > v[MC_XLO] && v[MC_RMAX] > v[MC_RMIN] && v[MC_RMIN] > 0.0))
-    return fail(s, CUDAHM_E_INVALID, "model constants out of range");
-  for (int k = 0; k < 6; ++k) s->P.mc[k] = v[k];
-  s->P.mc[MC_INV2S2] = 0.5 / (v[MC_SIGF] * v[MC_SIGF]);
-  // selection table: W_k = w_k * G(x_k), G(x) = int h(r) Phi((e^x/(4 pi r^2) - F_lim)/sigma_F) dr
   std::vector<double> xk, wk, rj, wj, ex(NQUAD), W(NQUAD);
-  gl_rule(NQUAD, v[MC_XLO], v[MC_XHI], xk, wk);
-  gl_rule(256, v[MC_RMIN], v[MC_RMAX], rj, wj);
-  const double vol3 = (v[MC_RMAX] * v[MC_RMAX] * v[MC_RMAX] - v[MC_RMIN] * v[MC_RMIN] * v[MC_RMIN]) / 3.0;
-  const double inv_s2 = 1.0 / (v[MC_SIGF] * std::sqrt(2.0));
-  for (int k = 0; k < NQUAD; ++k) {
-    ex[k] = std::exp(xk[k]);
-    long double G = 0.0L;
-    for (int j = 0; j < 256; ++j) {
-      const double r2 = rj[j] * rj[j];
-      const double F = ex[k] / (4.0 * M_PI * r2);
-      G += (long double)(wj[j] * r2 * 0.5 * std::erfc((v[MC_FLIM] - F) * inv_s2));
+  if (s->cfg.model == M_THINNED_SCHECHTER1D) {
+    // THINNED_SCHECHTER1D: {F_lim, sigma_F, x_lo, x_hi, r_min, r_max}
+    if (!(v[MC_SIGF] > 0.0 && v[MC_XHI] > v[MC_XLO] && v[MC_RMAX] > v[MC_RMIN] && v[MC_RMIN] > 0.0))
+      return fail(s, CUDAHM_E_INVALID, "model constants out of range");
+    for (int k = 0; k < 6; ++k) s->P.mc[k] = v[k];
+    s->P.mc[MC_INV2S2] = 0.5 / (v[MC_SIGF] * v[MC_SIGF]);
+    // selection table: W_k = w_k * G(x_k), G(x) = int h(r) Phi((e^x/(4 pi r^2) - F_lim)/sigma_F) dr
+    gl_rule(NQUAD, v[MC_XLO], v[MC_XHI], xk, wk);
+    gl_rule(256, v[MC_RMIN], v[MC_RMAX], rj, wj);
+    const double vol3 = (v[MC_RMAX] * v[MC_RMAX] * v[MC_RMAX] - v[MC_RMIN] * v[MC_RMIN] * v[MC_RMIN]) / 3.0;
+    const double inv_s2 = 1.0 / (v[MC_SIGF] * std::sqrt(2.0));
+    for (int k = 0; k < NQUAD; ++k) {
+      ex[k] = std::exp(xk[k]);
+      long double G = 0.0L;
+      for (int j = 0; j < 256; ++j) {
+        const double r2 = rj[j] * rj[j];
+        const double F = ex[k] / (4.0 * M_PI * r2);
+        G += (long double)(wj[j] * r2 * 0.5 * std::erfc((v[MC_FLIM] - F) * inv_s2));
+      }
+      W[k] = wk[k] * (double)(G / vol3);
     }
-    W[k] = wk[k] * (double)(G / vol3);
+  } else {
+    // BB1_FLUXNOISE1D: {sigma_0, alpha, x_lo, x_hi, r_min, r_max, F_th}.  eta(F) = Phi((F - F_th)/sigma(F)) with the
+    // flux-dependent sigma of Eq. 5.8 does not depend on theta, so the 2-D cubature the paper
+    // redoes for every proposal factorises here too: G(x) = int h(r) eta(e^x/(4 pi r^2)) dr is tabulated
+    // once, by a 512-point rule in q = ln r (the detection edge has a fixed width in q wherever it falls).
+    if (!(v[0] > 0.0 && v[1] >= 0.0 && v[MC_XHI] > v[MC_XLO] && v[MC_RMAX] > v[MC_RMIN] && v[MC_RMIN] > 0.0 && v[MB_FTH] > 0.0))
+      return fail(s, CUDAHM_E_INVALID, "model constants out of range");
+    for (int k = 0; k < 7; ++k) s->P.mc[k] = v[k];
+    s->P.mc[MB_S0SQ] = v[0] * v[0]; s->P.mc[MB_A2] = v[1] * v[1];
+    constexpr int NQR = 512;
+    gl_rule(NQUAD, v[MC_XLO], v[MC_XHI], xk, wk);
+    gl_rule(NQR, std::log(v[MC_RMIN]), std::log(v[MC_RMAX]), rj, wj);
+    const double vol3 = (v[MC_RMAX] * v[MC_RMAX] * v[MC_RMAX] - v[MC_RMIN] * v[MC_RMIN] * v[MC_RMIN]) / 3.0;
+    for (int k = 0; k < NQUAD; ++k) {
+      ex[k] = std::exp(xk[k]);
+      long double G = 0.0L;
+      for (int j = 0; j < NQR; ++j) {
+        const double F = ex[k] * std::exp(-2.0 * rj[j]) / (4.0 * M_PI);
+        const double sg = std::sqrt(s->P.mc[MB_S0SQ] + s->P.mc[MB_A2] * F * F);
+        G += (long double)(wj[j] * std::exp(3.0 * rj[j]) * 0.5 * std::erfc((v[MB_FTH] - F) / (sg * std::sqrt(2.0))));
+      }
+      W[k] = wk[k] * (double)(G / vol3);
+    }
   }
   CU_TRY(s, cudaMemcpyAsync((void*)s->P.qx, xk.data(), NQUAD * 8, cudaMemcpyHostToDevice, s->stream));
   CU_TRY(s, cudaMemcpyAsync((void*)s->P.qex, ex.data(), NQUAD * 8, cudaMemcpyHostToDevice, s->stream));

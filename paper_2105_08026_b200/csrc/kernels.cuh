@@ -242,9 +242,9 @@ __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c
 template <int MODEL>
 __device__ __forceinline__ double selection_slice(const Params& P, const ThetaK& kp, const int sweep_threads) {
   double tq = 0.0;
-  if (MODEL == M_THINNED_SCHECHTER1D && !P.tail.freeze_theta) {
+  if (has_selection(MODEL) && !P.tail.freeze_theta) {
     for (int k = (int)blockIdx.x + (int)gridDim.x * (int)threadIdx.x; k < NQUAD; k += (int)gridDim.x * sweep_threads)
-      tq += P.qW[k] * hm_exp(kp.v[0] * (P.qx[k] - kp.v[1]) - P.qex[k] * kp.v[3]);
+      tq += selection_term<MODEL>(kp, P.qW[k], P.qx[k], P.qex[k]);
   }
   return tq;
 }
@@ -469,7 +469,7 @@ __global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const l
     cnt[0] += part[3]; cnt[1] += part[4];
     double dq[2] = {part[1], part[2]};
     block_reduce_all<2>(dq, red);
-    constexpr int NVX = MODEL == M_THINNED_SCHECHTER1D ? 2 : 1;   // only M1 has a selection-integral slice to exchange
+    constexpr int NVX = has_selection(MODEL) ? 2 : 1;   // only M1 / M4 have a selection-integral slice to exchange
     unsigned long long* mb = P.mbox + (size_t)(k & 1) * mbox_parity_words(G);
     const unsigned epoch = epoch0 + (unsigned)k;
     mbox_push<NVX>(mb, G, (int)blockIdx.x, epoch, dq, (int)threadIdx.x, (int)blockDim.x);
@@ -544,15 +544,15 @@ __global__ void __launch_bounds__(256, 1) k_init_iter(const Params P) {
   __syncthreads();
   const ThetaK kc = theta_consts(P.tail.model, it.theta);
   double part[NPART] = {0, 0, 0, 0, 0};
-  if (P.tail.model == M_THINNED_SCHECHTER1D) {
+  if (has_selection(P.tail.model)) {
     for (int k = threadIdx.x; k < NQUAD; k += blockDim.x)
-      part[2] += P.qW[k] * hm_exp(kc.v[0] * (P.qx[k] - kc.v[1]) - P.qex[k] * kc.v[3]);
+      part[2] += selection_term_rt(P.tail.model, kc, P.qW[k], P.qx[k], P.qex[k]);
   }
   block_reduce<NPART>(part, red);
   if (threadIdx.x == 0) {
     it.kc = kc;
     it.lp_cur = log_prior(P.tail.model, it.theta);
-    it.T_cur = (P.tail.model == M_THINNED_SCHECHTER1D) ? -kc.v[4] * part[2] : 0.0;
+    it.T_cur = has_selection(P.tail.model) ? theta_only_from_sum(P.tail.model, kc, part[2], P.tail.n_objects) : 0.0;
     prepare_iteration(it, P.tail, it.t);
   }
   __syncthreads();
@@ -577,7 +577,7 @@ __global__ void k_init_state(const Params P, const T* raw, const int have_chi0, 
   T* chi = static_cast<T*>(P.chi);
   T* Lm = static_cast<T*>(P.L);
   if (!have_chi0) {
-    if (MODEL == M_THINNED_SCHECHTER1D) {
+    if (has_selection(MODEL)) {
       double x = log((double)raw[i] / (double)raw[P.Npad + i]);
       x = fmin(fmax(x, P.mc[MC_XLO]), P.mc[MC_XHI]);
       chi[i] = (T)x;

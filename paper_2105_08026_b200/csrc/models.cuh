@@ -15,8 +15,10 @@
 
 namespace hm {
 
-enum : int { M_NORMAL1D = 0, M_THINNED_SCHECHTER1D = 1, M_BINORMAL2D = 2, M_LINREG_ME1D = 3 };
+enum : int { M_NORMAL1D = 0, M_THINNED_SCHECHTER1D = 1, M_BINORMAL2D = 2, M_LINREG_ME1D = 3, M_BB1_FLUXNOISE1D = 4 };
 enum : int { MC_FLIM = 0, MC_SIGF = 1, MC_XLO = 2, MC_XHI = 3, MC_RMIN = 4, MC_RMAX = 5, MC_INV2S2 = 6 };
+// M4 keeps sigma_0^2 and alpha^2 (Eq. 5.8) where M1 keeps F_lim and sigma_F; the threshold goes to slot 6
+enum : int { MB_S0SQ = 0, MB_A2 = 1, MB_FTH = 6 };
 constexpr int NQUAD = 1024;   // selection-integral nodes (BASELINE.json configs[1])
 
 template <int MODEL> struct ModelDims;
@@ -24,6 +26,11 @@ template <> struct ModelDims<M_NORMAL1D>            { static constexpr int p = 1
 template <> struct ModelDims<M_THINNED_SCHECHTER1D> { static constexpr int p = 1, dtheta = 3, ncols = 2, nconsts = 6; };
 template <> struct ModelDims<M_BINORMAL2D>          { static constexpr int p = 2, dtheta = 5, ncols = 4, nconsts = 0; };
 template <> struct ModelDims<M_LINREG_ME1D>         { static constexpr int p = 1, dtheta = 3, ncols = 3, nconsts = 0; };
+template <> struct ModelDims<M_BB1_FLUXNOISE1D>     { static constexpr int p = 1, dtheta = 3, ncols = 2, nconsts = 7; };
+
+// models whose likelihood carries a theta-only selection term (the denominator of Eq. 4.4) summed over
+// the NQUAD nodes, whose latent is x = ln L with flux columns (Fhat, g = 1/(4 pi r^2)) and a bounded support
+HM_HD constexpr bool has_selection(int model) { return model == M_THINNED_SCHECHTER1D || model == M_BB1_FLUXNOISE1D; }
 
 inline bool model_dims(int model, int* p, int* dtheta, int* ncols, int* nconsts) {
   switch (model) {
@@ -31,6 +38,7 @@ inline bool model_dims(int model, int* p, int* dtheta, int* ncols, int* nconsts)
     case M_THINNED_SCHECHTER1D: *p = 1; *dtheta = 3; *ncols = 2; *nconsts = 6; return true;
     case M_BINORMAL2D:          *p = 2; *dtheta = 5; *ncols = 4; *nconsts = 0; return true;
     case M_LINREG_ME1D:         *p = 1; *dtheta = 3; *ncols = 3; *nconsts = 0; return true;
+    case M_BB1_FLUXNOISE1D:     *p = 1; *dtheta = 3; *ncols = 2; *nconsts = 7; return true;
   }
   return false;
 }
@@ -57,7 +65,30 @@ HM_HD void theta_consts_part(int model, int part, const double* th, ThetaK& k) {
       if (part == 1) { const double ch = cosh(th[4]); k.v[4] = -th[2] - th[3] + log(ch); k.v[5] = 0.5 * ch * ch; }
       if (part == 2) k.v[6] = tanh(th[4]);
       break;
+    case M_BB1_FLUXNOISE1D:
+      // (beta, ln l, ln u): f = log C + (beta+1)(x - ln u) + log(1 - e^(-L/l)) - L/u   (Eq. 5.1 in x = ln L), with
+      // log C = -(log|Gamma(beta+1)| + log|1 - (1 + u/l)^-(beta+1)|)   (Eq. C.3; both factors negative for beta < -1).
+      // v[5] + v[6] = -log C; the plate functor folds them into its additive constant.
+      if (part == 0) { k.v[0] = th[0] + 1.0; k.v[1] = th[2]; k.v[3] = hm_exp_any(-th[1]); k.v[4] = hm_exp_any(-th[2]); }
+      if (part == 1) k.v[5] = (th[0] + 1.0 == 0.0) ? 0.0 : lgamma(th[0] + 1.0);
+      if (part == 2) {
+        const double A = log1p(exp(th[2] - th[1]));                       // log(1 + u/l)
+        k.v[6] = (th[0] + 1.0 == 0.0) ? log(A) : log(fabs(expm1(-(th[0] + 1.0) * A)));
+      }
+      break;
   }
+}
+
+// theta-only term T(theta) from the node sum  sum_k W_k rho(x_k; theta):
+//   M1: minus the expected detected count, -A sum;   M4: -N log sum  (Eq. 4.3 with mu = h rho / I, Eq. 4.4)
+HM_HD double theta_only_from_sum(int model, const ThetaK& k, double tq, double n_objects) {
+  if (model == M_THINNED_SCHECHTER1D) return -k.v[4] * tq;
+#ifdef __CUDA_ARCH__
+  if (model == M_BB1_FLUXNOISE1D) return -n_objects * hm_log_pos(tq);
+#else
+  if (model == M_BB1_FLUXNOISE1D) return -n_objects * std::log(tq);
+#endif
+  return 0.0;
 }
 
 HM_HD ThetaK theta_consts(int model, const double* th) {
@@ -82,6 +113,9 @@ HM_HD double log_prior(int model, const double* th) {
     case M_THINNED_SCHECHTER1D:
       return (th[0] > -2.0 && th[0] < 0.0 && fabs(th[1]) <= 20.0 && fabs(th[2]) <= 50.0)
                  ? -hm_log_any_pos(1.0 + th[0] * th[0]) : ninf;
+    case M_BB1_FLUXNOISE1D:     // Eq. 5.5 as a density in (beta, ln l, ln u): l / (u (1 + beta^2)), l < u
+      return (th[0] > -2.0 && th[0] < 0.0 && th[1] < th[2] && fabs(th[1]) <= 30.0 && fabs(th[2]) <= 30.0)
+                 ? th[1] - th[2] - hm_log_any_pos(1.0 + th[0] * th[0]) : ninf;
   }
   return ninf;
 }
@@ -154,6 +188,59 @@ template <class T> struct Plate<M_THINNED_SCHECHTER1D, T> {
     return k.v[2] + k.v[0] * ((double)q.x - k.v[1]) - (double)q.ex * k.v[3];
   }
 };
+
+// 1 - e^(-t), t >= 0, with full relative accuracy at small t (L << l)
+__device__ __forceinline__ double hm_one_minus_exp_neg(double t) { return -expm1(-t); }
+__device__ __forceinline__ float hm_one_minus_exp_neg(float t) { return -expm1f(-t); }
+// 1/a for positive normal a: MUFU seed + two Newton steps (~1 ulp)
+__device__ __forceinline__ double hm_rcp_pos(double a) {
+  double r = hm_rcp_seed(a);
+  double e = hm_fma(-a, r, 1.0);
+  r = hm_fma(r, e, r);
+  e = hm_fma(-a, r, 1.0);
+  r = hm_fma(r, e, r);
+  e = hm_fma(-a, r, 1.0);
+  return hm_fma(r, e, r);
+}
+__device__ __forceinline__ float hm_rcp_pos(float a) { return 1.0f / a; }
+__device__ __forceinline__ double hm_log_point(double x) { return hm_log_pos(x); }
+__device__ __forceinline__ float hm_log_point(float x) { return logf(x); }
+
+// M4, the paper's case study: BB1 population in x = ln L, member likelihood = the sampling density
+// of Fhat as a function of F with sigma(F)^2 = sigma_0^2 + (alpha F)^2 (Eq. 5.6, 5.8).
+template <class T> struct Plate<M_BB1_FLUXNOISE1D, T> {
+  struct Pt { T x, ex; };
+  __device__ __forceinline__ static Pt point(const T* chi) { return Pt{chi[0], hm_exp_point(chi[0])}; }
+  // mc = {sigma_0^2, alpha^2, x_lo, x_hi, r_min, r_max, F_th} narrowed to T
+  __device__ __forceinline__ static T target(const Pt& q, const T* d, const KT<T>& k, const T* mc) {
+    if (!(q.x >= mc[MC_XLO] && q.x <= mc[MC_XHI])) return -INFINITY;
+    const T F = d[1] * q.ex, r = d[0] - F;
+    const T inv = hm_rcp_pos(mc[MB_S0SQ] + mc[MB_A2] * F * F);          // 1/sigma(F)^2
+    const T w = hm_one_minus_exp_neg(q.ex * k.v[3]);                     // 1 - e^(-L/l)
+    const T c0 = -(k.v[5] + k.v[6]) - k.v[0] * k.v[1];
+    // -log sigma(F) + log(1 - e^(-L/l)) in one logarithm
+    return T(0.5) * hm_log_point(w * w * inv) - T(0.5) * (r * r) * inv + c0 + k.v[0] * q.x - q.ex * k.v[4];
+  }
+  __device__ __forceinline__ static double pop(const Pt& q, const T*, const ThetaK& k) {
+    const double c0 = -(k.v[5] + k.v[6]) - k.v[0] * k.v[1];
+    return c0 + k.v[0] * (double)q.x + hm_log_pos(hm_one_minus_exp_neg((double)q.ex * k.v[3])) - (double)q.ex * k.v[4];
+  }
+};
+
+// one node of the selection sum: W_k rho(x_k; theta) from the node's x_k and e^(x_k)
+template <int MODEL>
+__device__ __forceinline__ double selection_term(const ThetaK& k, double W, double x, double ex) {
+  if (MODEL == M_THINNED_SCHECHTER1D) return W * hm_exp(k.v[0] * (x - k.v[1]) - ex * k.v[3]);
+  if (MODEL == M_BB1_FLUXNOISE1D) {
+    const double c0 = -(k.v[5] + k.v[6]) - k.v[0] * k.v[1];
+    return W * hm_exp(c0 + k.v[0] * x - ex * k.v[4]) * hm_one_minus_exp_neg(ex * k.v[3]);
+  }
+  return 0.0;
+}
+__device__ __forceinline__ double selection_term_rt(int model, const ThetaK& k, double W, double x, double ex) {
+  return model == M_THINNED_SCHECHTER1D ? selection_term<M_THINNED_SCHECHTER1D>(k, W, x, ex)
+                                        : selection_term<M_BB1_FLUXNOISE1D>(k, W, x, ex);
+}
 
 template <class T> struct Plate<M_BINORMAL2D, T> {
   struct Pt { T x1, x2; };

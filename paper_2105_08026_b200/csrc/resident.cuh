@@ -33,7 +33,7 @@ constexpr int RES_MAX_SMEM = 200 * 1024;            // dynamic shared memory the
 // per-object values kept in shared memory: [value][slot r][sweep thread]
 template <int MODEL> struct ResValues {
   static constexpr int ncols = ModelDims<MODEL>::ncols;
-  static constexpr bool m1 = MODEL == M_THINNED_SCHECHTER1D;
+  static constexpr bool m1 = has_selection(MODEL);     // M1 / M4: e^chi cached next to chi, selection sum on the tail warps
   static constexpr int V_CHI = 0, V_L = 1, V_D = 2, V_XP = 2 + ncols, V_U = 3 + ncols, V_E = 4 + ncols, V_EP = 5 + ncols;
   static constexpr int n_base = 4 + ncols + (m1 ? 2 : 0);   // + 2 (mean, M2) when moments are kept
 };
@@ -258,12 +258,12 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
     auto selection_full = [&]() {
       if constexpr (V::m1) {
         if (!P.tail.freeze_theta) {
-          const double k0 = it.kp.v[0], k1 = it.kp.v[1], k3 = it.kp.v[3];
+          const ThetaK kq = it.kp;
           double s_ = 0.0;
 #pragma unroll
           for (int m = 0; m < QPT; ++m) {
             const int q = ttid + m * RES_TW * 32;
-            s_ += qtab[0][q] * hm_exp(k0 * (qtab[1][q] - k1) - qtab[2][q] * k3);
+            s_ += selection_term<MODEL>(kq, qtab[0][q], qtab[1][q], qtab[2][q]);
           }
 #pragma unroll
           for (int o = 16; o > 0; o >>= 1) s_ += __shfl_down_sync(0xffffffffu, s_, o);

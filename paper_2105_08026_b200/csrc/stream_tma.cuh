@@ -144,7 +144,7 @@ __global__ void __launch_bounds__(BLOCK_ALL, 1) k_persistent_tma(const Params P,
     if (producer && lane == 0 && k + 1 < n_iter) {       // ... before the async proxy re-reads them for iteration k+1:
       for (int j = 0; j < n_pre; ++j) request(j, q + j); //     requested now, they land during the exchange and the tail
     }
-    constexpr int NVX = MODEL == M_THINNED_SCHECHTER1D ? 2 : 1;   // only M1 has a selection-integral slice to exchange
+    constexpr int NVX = has_selection(MODEL) ? 2 : 1;   // only M1 / M4 have a selection-integral slice to exchange
     unsigned long long* mb = P.mbox + (size_t)(k & 1) * mbox_parity_words(G);
     const unsigned epoch = epoch0 + (unsigned)k;
     mbox_push<NVX>(mb, G, (int)blockIdx.x, epoch, dq, tid, BLOCK_ALL);

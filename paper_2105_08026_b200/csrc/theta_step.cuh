@@ -50,6 +50,7 @@ struct TailCfg {
   double astar_theta, eta_exp;
   long long burn_in, max_trace_rows;
   int thin, pad_;
+  double n_objects;     // N of the selection term -N log I(theta) (M4)
 };
 
 HM_HD int tri(int r, int c) { return r * (r + 1) / 2 + c; }
@@ -137,7 +138,8 @@ HM_HD void decide_scalars(const Iter& it, const TailCfg& c, const Draws& d, doub
     *log_r = -INFINITY; *la = -INFINITY;
   } else {
     // M1: T(theta') = -A' sum_k W_k phi(x_k; theta'): minus the expected detected count (Eq. 4.4 denominator)
-    *T_prop = (c.model == M_THINNED_SCHECHTER1D) ? -it.kp.v[4] * tq : 0.0;
+    // M4: T(theta') = -N log sum_k W_k rho(x_k; theta')   (Eq. 4.3-4.4)
+    *T_prop = theta_only_from_sum(c.model, it.kp, tq, c.n_objects);
     *log_r = Delta + (*T_prop - it.T_cur) + (it.lp_prop - it.lp_cur);
     *la = (*log_r != *log_r) ? -INFINITY : fmin(0.0, *log_r);
   }

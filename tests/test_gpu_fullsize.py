@@ -51,6 +51,22 @@ def test_c2_full_size_free_running():
     assert st["theta_accepts"] == sto["theta_accepts"]
 
 
+def test_c5_full_size_free_running():
+    """C5, the paper's case study (BB1 population, N = 1e5) in the on-chip kernel; 12 iterations."""
+    c, orc, gpu = _pair("C5")
+    orc.run(12, 0, 1)
+    gpu.run(12, 0, 1, sync=True)
+    st = gpu.get_stats()
+    assert st["block_threads"] == 640
+    so, sg = orc.get_state(), gpu.get_state()
+    np.testing.assert_allclose(gpu.get_theta_trace(), orc.get_theta_trace(), rtol=1e-9, atol=1e-9)
+    np.testing.assert_allclose(sg["chi"], so["chi"], rtol=1e-9, atol=1e-9)
+    np.testing.assert_allclose(sg["L"], so["L"], rtol=1e-9)
+    np.testing.assert_allclose(sg["L_theta"], so["L_theta"], rtol=1e-8, atol=1e-12)
+    sto = orc.get_stats()
+    assert st["chi_accepts"] == sto["chi_accepts"] and st["theta_accepts"] == sto["theta_accepts"]
+
+
 def test_c3_full_size_free_running():
     """C3 as benched: N = 1e6, 2-D latent, streaming persistent kernel (148 x 512); 8 iterations."""
     c, orc, gpu = _pair("C3")
