@@ -7,7 +7,7 @@ chi moments on device, theta chain thinned by 10) -- the configuration BASELINE.
 `--warmup W` iterations run untimed as burn-in, then EXACTLY `--steps K` post-burn-in iterations are timed with
 CUDA events on the sampler's stream, bracketed by barrier + synchronize; rank 0 prints ONE JSON line.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C0..C4] [--theta-mode tail|graph|host]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C0..C5] [--theta-mode tail|graph|host]
     python bench.py --impl reference ...      # the CPU oracle, as it stands, on the same config / metric
 
 Multi-GPU: the path does not shard without a per-iteration exchange (the theta step needs the global sum), and
@@ -33,7 +33,7 @@ METRIC = "plate_ram_updates_per_s"
 UNIT = "updates/s"
 # algorithmic bytes per object per iteration: state read+write and
 # data read; + running-moment read+write (fp64 mean and M2 per component) once past burn-in
-ALG_BYTES = {"C0": (48, 32), "C1": (48, 32), "C2": (48, 32), "C3": (112, 64), "C4": (28, 32)}
+ALG_BYTES = {"C0": (48, 32), "C1": (48, 32), "C2": (48, 32), "C3": (112, 64), "C4": (28, 32), "C5": (48, 32)}
 MODES = {"host": 0, "graph": 1, "tail": 2}
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel PER GIBBS ITERATION, from the committed
 # `ncu --set full` captures (profiles/r01f_resident_C2_ncu.md: 14.60 MB + 0.075 MB over 300 iterations;
@@ -144,6 +144,8 @@ def make_workload(cfg_name, n_override=0, seed_offset=0):
         inp = synth.make_thinned_schechter1d(n, c.seed + seed_offset)
     elif c.model == synth.M_BINORMAL2D:
         inp = synth.make_binormal2d(n, c.seed + seed_offset)
+    elif c.model == synth.M_BB1_FLUXNOISE1D:
+        inp = synth.make_bb1_fluxnoise1d(n, c.seed + seed_offset)
     else:
         inp = synth.make_linreg_me1d(n, c.seed + seed_offset, fp32=(c.precision == synth.F32_STATE_F64_REDUCE))
     return c, n, inp
@@ -356,7 +358,7 @@ def main():
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64" if c.precision == synth.F64 else "f32 state / f64 reductions", "data": "synthetic",
         "config": {"workload": f"{args.config}: BASELINE.json configs[{int(args.config[1])}]", "n_objects": n,
-                   "model": ["normal1d", "thinned_schechter1d", "binormal2d", "linreg_me1d"][c.model],
+                   "model": ["normal1d", "thinned_schechter1d", "binormal2d", "linreg_me1d", "bb1_fluxnoise1d"][c.model],
                    "burn_in": W, "thin": c.thin, "chi_moments": bool(c.keep_chi_moments),
                    "theta_mode": args.theta_mode, "parallelism": "replicas only" if world > 1 else "1 gpu",
                    "grid": [r["stats"]["grid_blocks"], r["stats"]["block_threads"]],
@@ -411,13 +413,15 @@ def extras(args, device, peak, peak_src, n):
                     "gpu_launches": int(r["launches"])}
     out["other_theta_modes"] = modes
     side = {}
-    for cfg_name, k, w in (("C3", 600, 200), ("C4", 300, 100)):
+    # C3 / C4: the HBM-streaming configs; C5: the paper's own case study (BB1 population, N = 1e5)
+    for cfg_name, k, w in (("C3", 600, 200), ("C4", 300, 100), ("C5", 3000, 1000)):
         if cfg_name == args.config:
             continue
         a = copy.copy(args)
         a.steps, a.warmup, a.n_objects = k, w, 0
         r = time_gpu(cfg_name, a, device, 0, 1, lambda: None, with_clocks=False)
-        rf = roofline_entry(cfg_name, r["cfg"], r["n"], k, w, r["ms"], peak, peak_src, "k_persistent")
+        kern = "k_resident" if r["stats"]["block_threads"] == 640 else "k_persistent"
+        rf = roofline_entry(cfg_name, r["cfg"], r["n"], k, w, r["ms"], peak, peak_src, kern)
         side[cfg_name] = {"n_objects": r["n"], "steps": k, "warmup": w, "updates_per_s": r["n"] * k / (r["ms"] * 1e-3),
                           "gibbs_iters_per_s": k / (r["ms"] * 1e-3), "roofline": rf,
                           "grid": [r["stats"]["grid_blocks"], r["stats"]["block_threads"]]}

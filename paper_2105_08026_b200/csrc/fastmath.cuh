@@ -97,6 +97,36 @@ HM_HD double hm_exp_core(double x) {
   const double y = thi + hm_fma(thi, p, tlo);              // T[j] e^r
   return hm_bits2d(hm_d2bits(y) + ((uint64_t)(int64_t)k << 52));
 }
+// e^x - 1 for x in [-708, 0] with full RELATIVE accuracy also at small |x| (1 - e^(-L/l) of the BB1 density at L << l):
+// the same reduction as hm_exp_core; e^x - 1 = (s - 1) + s (e^r - 1) + 2^k T_lo with s = 2^k T_hi[j] in (0, 1]:
+// s - 1 is exact for s >= 1/2 (Sterbenz) and, for |x| <= ln2/128, s = 1 and the result is the polynomial itself.
+HM_HD double hm_expm1_nonpos(double x) {
+  x = x < -708.0 ? -708.0 : x;
+  const double SHIFT = 6755399441055744.0;
+  const double t = hm_fma(x, HM_64_LN2, SHIFT);
+  const double nf = t - SHIFT;
+  double r = hm_fma(nf, -HM_LN2_64_HI, x);
+  r = hm_fma(nf, -HM_LN2_64_LO, r);
+  const int n = (int)(uint32_t)(hm_d2bits(t) & 0xffffffffull);
+  const int j = n & 63, k = n >> 6;
+#ifdef __CUDA_ARCH__
+  const double2 tj = __ldg(reinterpret_cast<const double2*>(hm_exp2_tab_dev) + j);
+  const double thi = tj.x, tlo = tj.y;
+#else
+  const double thi = hm_exp2_tab_host[j].hi, tlo = hm_exp2_tab_host[j].lo;
+#endif
+  double p = 1.3888888888888889e-03;
+  p = hm_fma(p, r, 8.3333333333333332e-03);
+  p = hm_fma(p, r, 4.1666666666666664e-02);
+  p = hm_fma(p, r, 1.6666666666666666e-01);
+  p = hm_fma(p, r, 0.5);
+  p = p * r;
+  p = hm_fma(p, r, r);                                     // e^r - 1
+  const double scale = hm_bits2d((uint64_t)(int64_t)(k + 1023) << 52);   // 2^k, k in [-1022, 0]
+  const double sh = thi * scale;                           // exact (power of two)
+  return (sh - 1.0) + hm_fma(sh, p, tlo * scale);
+}
+
 HM_HD double hm_exp_fast(double x) {
   x = x < -708.0 ? -708.0 : (x > 709.0 ? 709.0 : x);       // (fmin / fmax cost 7 instructions each: NaN handling)
   return hm_exp_core(x);

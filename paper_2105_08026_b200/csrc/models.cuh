@@ -70,11 +70,26 @@ HM_HD void theta_consts_part(int model, int part, const double* th, ThetaK& k) {
       // log C = -(log|Gamma(beta+1)| + log|1 - (1 + u/l)^-(beta+1)|)   (Eq. C.3; both factors negative for beta < -1).
       // v[5] + v[6] = -log C; the plate functor folds them into its additive constant.
       if (part == 0) { k.v[0] = th[0] + 1.0; k.v[1] = th[2]; k.v[3] = hm_exp_any(-th[1]); k.v[4] = hm_exp_any(-th[2]); }
+#ifdef __CUDA_ARCH__
+      // device: the tail is a serial chain on the critical path of every iteration.  log|Gamma(b)| for -1 < b < 1 by the
+      // recurrence Gamma(b) = Gamma(b + 2)/(b (b + 1)) (lgamma on (1, 3) is a short polynomial; the reflection formula
+      // libm takes for b < 0 costs several hundred instructions), lean exp / log elsewhere.
+      if (part == 1) {
+        const double b1 = th[0] + 1.0;
+        k.v[5] = (b1 == 0.0) ? 0.0 : lgamma(b1 + 2.0) - hm_log_pos(fabs(b1 * (b1 + 1.0)));
+      }
+      if (part == 2) {
+        const double b1 = th[0] + 1.0;
+        const double A = hm_log_pos(1.0 + hm_exp_fast(th[2] - th[1]));      // log(1 + u/l); u/l >= 1 inside the prior
+        k.v[6] = (b1 == 0.0) ? hm_log_pos(A) : hm_log_pos(fabs(expm1(-b1 * A)));
+      }
+#else
       if (part == 1) k.v[5] = (th[0] + 1.0 == 0.0) ? 0.0 : lgamma(th[0] + 1.0);
       if (part == 2) {
         const double A = log1p(exp(th[2] - th[1]));                       // log(1 + u/l)
         k.v[6] = (th[0] + 1.0 == 0.0) ? log(A) : log(fabs(expm1(-(th[0] + 1.0) * A)));
       }
+#endif
       break;
   }
 }
@@ -190,7 +205,7 @@ template <class T> struct Plate<M_THINNED_SCHECHTER1D, T> {
 };
 
 // 1 - e^(-t), t >= 0, with full relative accuracy at small t (L << l)
-__device__ __forceinline__ double hm_one_minus_exp_neg(double t) { return -expm1(-t); }
+__device__ __forceinline__ double hm_one_minus_exp_neg(double t) { return -hm_expm1_nonpos(-t); }
 __device__ __forceinline__ float hm_one_minus_exp_neg(float t) { return -expm1f(-t); }
 // 1/a for positive normal a: MUFU seed + two Newton steps (~1 ulp)
 __device__ __forceinline__ double hm_rcp_pos(double a) {

@@ -48,6 +48,17 @@ def test_exp_fast(binary):
     assert np.isfinite(big[2]) and big[2] == big[3]
 
 
+def test_expm1_nonpos(binary):
+    """1 - e^(-L/l) of the BB1 density needs e^x - 1 with full relative accuracy from x ~ -1e-9 to -700."""
+    rng = np.random.default_rng(5)
+    x = -np.concatenate([np.exp(rng.uniform(-45, 6.5, 5000)), rng.uniform(0, 0.05, 1500), rng.uniform(0, 2.0, 1500),
+                         [0.0, np.log(2) / 128, np.log(2) / 64, 0.5 * np.log(2), np.log(2), 1e-300, 708.0]])
+    got = run(binary, "expm1", x)
+    assert ulp_err(got, mpmath.expm1, x) <= 2.5
+    assert got[-7] == 0.0 and np.all(got <= 0.0) and np.all(got >= -1.0)
+    assert run(binary, "expm1", np.array([-1e4, -np.inf]))[0] == -1.0
+
+
 def test_log_pos(binary):
     rng = np.random.default_rng(2)
     k = rng.integers(0, 2 ** 52, 4000)
