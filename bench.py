@@ -42,6 +42,12 @@ MODES = {"host": 0, "graph": 1, "tail": 2}
 NCU_DRAM_BYTES_PER_ITER = {"C2": (14.599424e6 + 75.008e3) / 300, "C4": (5.940074e9 + 2.362765e9) / 30}
 
 
+def workload_label(name):
+    if name == "C5":
+        return "C5: the paper's own case study (PAPER.md section 5.3, Table 5.1: BB1 population, N = 1e5); not a BASELINE.json config"
+    return f"{name}: BASELINE.json configs[{int(name[1])}]"
+
+
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -311,7 +317,7 @@ def run_reference(args, rank):
             "warmup": W, "ms_per_step": sec_k * 1e3 / K, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64" if c.precision == synth.F64 else "f32 state / f64 reductions",
             "data": "synthetic",
-            "config": {"workload": f"{args.config}: BASELINE.json configs[{int(args.config[1])}]", "n_objects": n_full,
+            "config": {"workload": workload_label(args.config), "n_objects": n_full,
                        "sample_objects": n_s},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -357,7 +363,7 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64" if c.precision == synth.F64 else "f32 state / f64 reductions", "data": "synthetic",
-        "config": {"workload": f"{args.config}: BASELINE.json configs[{int(args.config[1])}]", "n_objects": n,
+        "config": {"workload": workload_label(args.config), "n_objects": n,
                    "model": ["normal1d", "thinned_schechter1d", "binormal2d", "linreg_me1d", "bb1_fluxnoise1d"][c.model],
                    "burn_in": W, "thin": c.thin, "chi_moments": bool(c.keep_chi_moments),
                    "theta_mode": args.theta_mode, "parallelism": "replicas only" if world > 1 else "1 gpu",

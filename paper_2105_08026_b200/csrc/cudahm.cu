@@ -645,6 +645,16 @@ extern "C" int cudahm_run(cudahm_sampler* s, int64_t n_iter, int64_t burn_in, in
 }
 
 // ----------------------------------------------------------------------------------------------------
+namespace {
+// log C(beta, u, l), the BB1 normaliser of PAPER.md:429 (Eq. C.3): C = 1/(Gamma(b)(1 - (1 + u/l)^-b)), b = beta + 1 (both
+// factors negative for b < 0); 1/log(1 + u/l) at b = 0.  Host only: the kernels work with rho/C (models.cuh).
+double bb1_log_norm(const double* th) {
+  const double b = th[0] + 1.0, A = std::log1p(std::exp(th[2] - th[1]));
+  if (b == 0.0) return -std::log(A);
+  return -(std::lgamma(b) + std::log(std::fabs(std::expm1(-b * A))));
+}
+}  // namespace
+
 extern "C" int cudahm_debug_step(cudahm_sampler* s, int64_t burn_in, int32_t thin, cudahm_taps* taps) {
   if (!s || !taps) return fail(s, CUDAHM_E_INVALID, "debug_step: NULL argument");
   if (!s->have_init) return fail(s, CUDAHM_E_STATE, "debug_step before set_init");
@@ -673,6 +683,11 @@ extern "C" int cudahm_debug_step(cudahm_sampler* s, int64_t burn_in, int32_t thi
   P.taps.pi_cur = q; q += N; P.taps.pi_prop = q; q += N; P.taps.alpha = q; q += N;
   P.taps.u = q; q += N; P.taps.a = q; q += N; P.taps.b = q; q += N;
   P.taps.accepted = ibuf;
+  // constants the kernels drop (they cancel in every ratio): added back so the taps read in the paper's convention
+  double lc = 0.0, lcp = 0.0;
+  if (s->cfg.model == M_BB1_FLUXNOISE1D) { lc = bb1_log_norm(s->h_iter->theta); lcp = bb1_log_norm(s->h_iter->thetaP); }
+  P.taps.shift_c = lc; P.taps.shift_p = lcp;
+  const bool prop_in_support = s->h_iter->lp_prop != -INFINITY;
   void* a1[] = {&P};
   rc = launch(s, s->ks.sweep_tap, s->sweep_grid, s->sweep_block, a1, false);
   int nb = s->sweep_grid, flags = TAIL_REDUCE | TAIL_DECIDE;     // the device tail decides t and prepares t + 1
@@ -684,7 +699,9 @@ extern "C" int cudahm_debug_step(cudahm_sampler* s, int64_t burn_in, int32_t thi
   if (!rc && e == cudaSuccess) {
     const Iter& it = *s->h_iter;
     for (int r = 0; r < 8; ++r) taps->theta_prop[r] = r < s->dtheta ? it.tap_thetaP[r] : 0.0;
-    taps->S = it.S; taps->Delta = it.Delta; taps->T_cur = it.T_cur_used; taps->T_prop = it.T_prop;
+    const double Nd = (double)s->P.N;
+    taps->S = it.S + Nd * lc; taps->Delta = it.Delta + Nd * (lcp - lc);
+    taps->T_cur = it.T_cur_used - Nd * lc; taps->T_prop = it.T_prop - (prop_in_support ? Nd * lcp : 0.0);
     taps->lp_cur = it.lp_cur_used; taps->lp_prop = s->h_lp_prop_before; taps->log_r = it.log_r;
     taps->alpha_theta = it.alpha_theta; taps->u_theta = it.u_theta; taps->accepted_theta = it.accepted_theta;
     struct { double* dst; const double* src; size_t n; } cp[] = {

@@ -13,6 +13,9 @@ namespace hm {
 struct DevTaps {
   double *chi_prop, *pi_cur, *pi_prop, *alpha, *u, *L_new, *a, *b;
   int* accepted;
+  // additive constants the kernels drop because they cancel in every ratio (M4: log C(theta), log C(theta')); the taps
+  // add them back so that they read in the paper's convention
+  double shift_c, shift_p;
 };
 
 struct Params {
@@ -221,15 +224,15 @@ __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c
         const DevTaps& tp = P.taps;
 #pragma unroll
         for (int j = 0; j < p; ++j) if (tp.chi_prop) tp.chi_prop[j * P.N + i] = (double)yi[j];
-        if (tp.pi_cur) tp.pi_cur[i] = (double)pc;
-        if (tp.pi_prop) tp.pi_prop[i] = (double)pp;
+        if (tp.pi_cur) tp.pi_cur[i] = (double)pc + tp.shift_c;
+        if (tp.pi_prop) tp.pi_prop[i] = (double)pp + tp.shift_c;
         if (tp.alpha) tp.alpha[i] = (double)alpha;
         if (tp.u) tp.u[i] = (double)u;
         if (tp.accepted) tp.accepted[i] = acc ? 1 : 0;
 #pragma unroll
         for (int k = 0; k < ntri; ++k) if (tp.L_new) tp.L_new[k * P.N + i] = (double)ln[k];
-        if (tp.a) tp.a[i] = a;
-        if (tp.b) tp.b[i] = b;
+        if (tp.a) tp.a[i] = a + tp.shift_c;
+        if (tp.b) tp.b[i] = b + tp.shift_p;
       }
     } else {
 #pragma unroll

@@ -66,36 +66,18 @@ HM_HD void theta_consts_part(int model, int part, const double* th, ThetaK& k) {
       if (part == 2) k.v[6] = tanh(th[4]);
       break;
     case M_BB1_FLUXNOISE1D:
-      // (beta, ln l, ln u): f = log C + (beta+1)(x - ln u) + log(1 - e^(-L/l)) - L/u   (Eq. 5.1 in x = ln L), with
-      // log C = -(log|Gamma(beta+1)| + log|1 - (1 + u/l)^-(beta+1)|)   (Eq. C.3; both factors negative for beta < -1).
-      // v[5] + v[6] = -log C; the plate functor folds them into its additive constant.
+      // (beta, ln l, ln u): f = log C + (beta+1)(x - ln u) + log(1 - e^(-L/l)) - L/u   (Eq. 5.1 in x = ln L).
+      // The normaliser C(beta, u, l) of Eq. C.3 multiplies both rho(x_i; theta) and the selection integral I(theta) of
+      // Eq. 4.4, so it cancels in mu = h rho / I and in every Metropolis ratio: the device works with the SHAPE
+      // rho/C throughout (no lgamma / expm1 / log1p chain on the critical path of the theta step) and the taps of
+      // cudahm_debug_step add log C back on the host (cudahm.cu::bb1_log_norm), so they read in the paper's convention.
       if (part == 0) { k.v[0] = th[0] + 1.0; k.v[1] = th[2]; k.v[3] = hm_exp_any(-th[1]); k.v[4] = hm_exp_any(-th[2]); }
-#ifdef __CUDA_ARCH__
-      // device: the tail is a serial chain on the critical path of every iteration.  log|Gamma(b)| for -1 < b < 1 by the
-      // recurrence Gamma(b) = Gamma(b + 2)/(b (b + 1)) (lgamma on (1, 3) is a short polynomial; the reflection formula
-      // libm takes for b < 0 costs several hundred instructions), lean exp / log elsewhere.
-      if (part == 1) {
-        const double b1 = th[0] + 1.0;
-        k.v[5] = (b1 == 0.0) ? 0.0 : lgamma(b1 + 2.0) - hm_log_pos(fabs(b1 * (b1 + 1.0)));
-      }
-      if (part == 2) {
-        const double b1 = th[0] + 1.0;
-        const double A = hm_log_pos(1.0 + hm_exp_fast(th[2] - th[1]));      // log(1 + u/l); u/l >= 1 inside the prior
-        k.v[6] = (b1 == 0.0) ? hm_log_pos(A) : hm_log_pos(fabs(expm1(-b1 * A)));
-      }
-#else
-      if (part == 1) k.v[5] = (th[0] + 1.0 == 0.0) ? 0.0 : lgamma(th[0] + 1.0);
-      if (part == 2) {
-        const double A = log1p(exp(th[2] - th[1]));                       // log(1 + u/l)
-        k.v[6] = (th[0] + 1.0 == 0.0) ? log(A) : log(fabs(expm1(-(th[0] + 1.0) * A)));
-      }
-#endif
       break;
   }
 }
 
 // theta-only term T(theta) from the node sum  sum_k W_k rho(x_k; theta):
-//   M1: minus the expected detected count, -A sum;   M4: -N log sum  (Eq. 4.3 with mu = h rho / I, Eq. 4.4)
+//   M1: minus the expected detected count, -A sum;   M4: -N log sum  (Eq. 4.3 with mu = h rho / I, Eq. 4.4; rho/C)
 HM_HD double theta_only_from_sum(int model, const ThetaK& k, double tq, double n_objects) {
   if (model == M_THINNED_SCHECHTER1D) return -k.v[4] * tq;
 #ifdef __CUDA_ARCH__
@@ -232,12 +214,12 @@ template <class T> struct Plate<M_BB1_FLUXNOISE1D, T> {
     const T F = d[1] * q.ex, r = d[0] - F;
     const T inv = hm_rcp_pos(mc[MB_S0SQ] + mc[MB_A2] * F * F);          // 1/sigma(F)^2
     const T w = hm_one_minus_exp_neg(q.ex * k.v[3]);                     // 1 - e^(-L/l)
-    const T c0 = -(k.v[5] + k.v[6]) - k.v[0] * k.v[1];
+    const T c0 = -k.v[0] * k.v[1];
     // -log sigma(F) + log(1 - e^(-L/l)) in one logarithm
     return T(0.5) * hm_log_point(w * w * inv) - T(0.5) * (r * r) * inv + c0 + k.v[0] * q.x - q.ex * k.v[4];
   }
   __device__ __forceinline__ static double pop(const Pt& q, const T*, const ThetaK& k) {
-    const double c0 = -(k.v[5] + k.v[6]) - k.v[0] * k.v[1];
+    const double c0 = -k.v[0] * k.v[1];
     return c0 + k.v[0] * (double)q.x + hm_log_pos(hm_one_minus_exp_neg((double)q.ex * k.v[3])) - (double)q.ex * k.v[4];
   }
 };
@@ -247,8 +229,7 @@ template <int MODEL>
 __device__ __forceinline__ double selection_term(const ThetaK& k, double W, double x, double ex) {
   if (MODEL == M_THINNED_SCHECHTER1D) return W * hm_exp(k.v[0] * (x - k.v[1]) - ex * k.v[3]);
   if (MODEL == M_BB1_FLUXNOISE1D) {
-    const double c0 = -(k.v[5] + k.v[6]) - k.v[0] * k.v[1];
-    return W * hm_exp(c0 + k.v[0] * x - ex * k.v[4]) * hm_one_minus_exp_neg(ex * k.v[3]);
+    return W * hm_exp(k.v[0] * (x - k.v[1]) - ex * k.v[4]) * hm_one_minus_exp_neg(ex * k.v[3]);
   }
   return 0.0;
 }
