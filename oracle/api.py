@@ -10,6 +10,7 @@ import numpy as np
 from . import build as _build
 
 M_NORMAL1D, M_THINNED_SCHECHTER1D, M_BINORMAL2D, M_LINREG_ME1D, M_BB1_FLUXNOISE1D = 0, 1, 2, 3, 4
+M_NORMAL3D_KNOWNCOV = 5
 F64, F32_STATE_F64_REDUCE = 0, 1
 KIND_PLATE, KIND_THETA = 0, 1
 

@@ -1,4 +1,4 @@
-// oracle/models.hpp -- the five compiled-in models, written out plainly.  TEST INFRASTRUCTURE ONLY.
+// oracle/models.hpp -- the six compiled-in models, written out plainly.  TEST INFRASTRUCTURE ONLY.
 //
 // The paper asks the user for two functions: the member log-likelihood
 // log l_i(chi) and the population log-density log f(chi; theta);
@@ -12,7 +12,8 @@
 
 namespace oracle {
 
-enum Model { M_NORMAL1D = 0, M_THINNED_SCHECHTER1D = 1, M_BINORMAL2D = 2, M_LINREG_ME1D = 3, M_BB1_FLUXNOISE1D = 4 };
+enum Model { M_NORMAL1D = 0, M_THINNED_SCHECHTER1D = 1, M_BINORMAL2D = 2, M_LINREG_ME1D = 3, M_BB1_FLUXNOISE1D = 4,
+             M_NORMAL3D_KNOWNCOV = 5 };
 
 struct Dims { int p, dtheta, n_cols, n_consts; };
 inline bool model_dims(int model, Dims* d) {
@@ -22,6 +23,7 @@ inline bool model_dims(int model, Dims* d) {
     case M_BINORMAL2D:          *d = {2, 5, 4, 0}; return true;   // cols y1,y2,s1,s2;       theta (m1,m2,l1,l2,zeta)
     case M_LINREG_ME1D:         *d = {1, 3, 3, 0}; return true;   // cols y, sigma, z;       theta (a, b, log tau)
     case M_BB1_FLUXNOISE1D:     *d = {1, 3, 2, 7}; return true;   // cols Fhat, g=1/(4 pi r^2); theta (beta, ln l, ln u)
+    case M_NORMAL3D_KNOWNCOV:   *d = {3, 3, 3, 9}; return true;   // cols y1, y2, y3;        theta = mu (3)
   }
   return false;
 }
@@ -31,6 +33,10 @@ enum { C_FLIM = 0, C_SIGF = 1, C_XLO = 2, C_XHI = 3, C_RMIN = 4, C_RMAX = 5 };
 // consts of M4 (the paper's case study): {sigma_0, alpha (the noise slope of Eq. 5.8), x_lo, x_hi,
 // r_min, r_max, F_th}; x_lo .. r_max sit at the same indices as in M1
 enum { B_SIG0 = 0, B_ANOISE = 1, B_FTH = 6 };
+
+// consts of M5 (the normal-normal benchmark of PAPER.md:146-166, Eq. 3.1-3.4): {sigma_1, sigma_2, sigma_3, then the
+// packed lower triangle of C_pop: C11, C21, C22, C31, C32, C33}; C_pop and sigma_j are KNOWN, theta = mu
+enum { N3_SIG = 0, N3_COV = 3 };
 
 // log C(beta, u, l), the BB1 normaliser of PAPER.md:429 (Eq. C.3):
 //   C = 1 / (Gamma(beta+1) (1 - (1 + u/l)^-(beta+1)))   (beta > -2, beta != -1),     C = 1/log(1 + u/l)  (beta = -1).
@@ -60,6 +66,11 @@ inline T loglik(int model, const T* chi, const T* d, const T* consts) {
     case M_BINORMAL2D: {                        // independent Gaussian errors per axis
       const T r1 = d[0] - chi[0], r2 = d[1] - chi[1];
       return -T(0.5) * ((r1 * r1) / (d[2] * d[2]) + (r2 * r2) / (d[3] * d[3]));
+    }
+    case M_NORMAL3D_KNOWNCOV: {                 // y_ij ~ N(chi_ij, sigma_j^2), j = 1..3   (Eq. 3.2, sigma_j of :164)
+      T s = T(0);
+      for (int j = 0; j < 3; ++j) { const T r = d[j] - chi[j]; s += (r * r) / (consts[N3_SIG + j] * consts[N3_SIG + j]); }
+      return -T(0.5) * s;
     }
     case M_BB1_FLUXNOISE1D: {
       // Fhat ~ N(F, sigma(F)^2), sigma(F)^2 = sigma_0^2 + (alpha F)^2 (Eq. 5.8), F = L/(4 pi r^2),
@@ -98,6 +109,26 @@ inline T logpop(int model, const T* chi, const T* d, const T* th, const T* const
       const T rho = std::tanh(th[4]);
       return -th[2] - th[3] + std::log(ch) - ch * ch * (u1 * u1 - T(2) * rho * u1 * u2 + u2 * u2) / T(2);
     }
+    case M_NORMAL3D_KNOWNCOV: {
+      // chi ~ N(mu, C_pop) (Eq. 3.1), C_pop known: log f = -1/2 (chi - mu)^T C_pop^-1 (chi - mu) + const.
+      // Plain route: factor C_pop = G G^T (Cholesky), solve G w = chi - mu, then -1/2 w^T w.
+      T G[3][3] = {};
+      const T* Cp = consts + N3_COV;
+      for (int r = 0; r < 3; ++r)
+        for (int k = 0; k <= r; ++k) {
+          T a = Cp[r * (r + 1) / 2 + k];
+          for (int m = 0; m < k; ++m) a -= G[r][m] * G[k][m];
+          G[r][k] = (r == k) ? std::sqrt(a) : a / G[k][k];
+        }
+      T w[3], q = T(0);
+      for (int r = 0; r < 3; ++r) {
+        T a = chi[r] - th[r];
+        for (int m = 0; m < r; ++m) a -= G[r][m] * w[m];
+        w[r] = a / G[r][r];
+        q += w[r] * w[r];
+      }
+      return -T(0.5) * q;
+    }
     case M_BB1_FLUXNOISE1D: {
       // BB1 luminosity PDF, PAPER.md:256 (Eq. 5.1) = :423 (Eq. C.2), as a density in x = ln L (Jacobian L):
       //   L f(L) = C (L/u)^(beta+1) (1 - e^(-L/l)) e^(-L/u),   theta = (beta, ln l, ln u);
@@ -130,6 +161,9 @@ inline double logprior(int model, const double* th) {
     case M_THINNED_SCHECHTER1D:
       if (!(th[0] > -2.0 && th[0] < 0.0 && std::fabs(th[1]) <= 20.0 && std::fabs(th[2]) <= 50.0)) return ninf;
       return -std::log(1.0 + th[0] * th[0]);
+    case M_NORMAL3D_KNOWNCOV:                   // "uniform hyperpriors", on a wide box so they are proper
+      if (!(std::fabs(th[0]) <= 1e3 && std::fabs(th[1]) <= 1e3 && std::fabs(th[2]) <= 1e3)) return ninf;
+      return 0.0;
     case M_BB1_FLUXNOISE1D:
       // PAPER.md:277-290 (Eq. 5.3-5.5): truncated Cauchy in beta on (-2, 0), log-flat in u, flat in l on l < u
       // (p(l|u) = 1/u).  As a density in the sampled coordinates (beta, ln l, ln u) that is

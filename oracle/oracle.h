@@ -30,7 +30,8 @@ typedef struct oracle_sampler oracle_sampler;
 enum { ORACLE_OK = 0, ORACLE_E_INVALID = -1, ORACLE_E_STATE = -2, ORACLE_E_UNSUPPORTED = -5 };
 /* models: */
 enum { ORACLE_M_NORMAL1D = 0, ORACLE_M_THINNED_SCHECHTER1D = 1, ORACLE_M_BINORMAL2D = 2, ORACLE_M_LINREG_ME1D = 3,
-       ORACLE_M_BB1_FLUXNOISE1D = 4 /* the paper's case study: BB1 population, flux-dependent noise */ };
+       ORACLE_M_BB1_FLUXNOISE1D = 4, /* the paper's case study: BB1 population, flux-dependent noise */
+       ORACLE_M_NORMAL3D_KNOWNCOV = 5 /* the normal-normal benchmark: 3-vector latents, known C_pop */ };
 enum { ORACLE_F64 = 0, ORACLE_F32_STATE_F64_REDUCE = 1 };
 /* Philox stream kinds */
 enum { ORACLE_KIND_PLATE = 0, ORACLE_KIND_THETA = 1 };

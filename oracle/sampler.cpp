@@ -172,14 +172,14 @@ struct Impl : Base {
     // O3/O4: plate sweep in index order
     long double S = 0.0L, Delta = 0.0L;
     for (int64_t i = 0; i < N; ++i) {
-      T x[2], y[2], z[2] = {T(0), T(0)}, l[3], d[4], u;
+      T x[8], y[8], z[8] = {}, l[36], d[16], u;
       for (int j = 0; j < p; ++j) x[j] = chi[(size_t)j * N + i];
       for (int k = 0; k < nt; ++k) l[k] = L[(size_t)k * N + i];
       for (int c = 0; c < nc; ++c) d[c] = data[(size_t)c * N + i];
       if (sizeof(T) == 8) {
-        double zz[2] = {0, 0}, uu = 0;
+        double zz[8] = {}, uu = 0;
         plate_draws_f64(cfg.seed, (uint64_t)i, tcur, p, zz, &uu);
-        z[0] = (T)zz[0]; z[1] = (T)zz[1];
+        for (int j = 0; j < p; ++j) z[j] = (T)zz[j];
         u = (T)uu;
       } else {
         float zf[2] = {0.0f, 0.0f}, uf;
@@ -205,12 +205,12 @@ struct Impl : Base {
       if (acc) { for (int j = 0; j < p; ++j) x[j] = y[j]; stats.chi_accepts++; }
       stats.chi_proposals++;
       // step 3: S_n = chol(S (I + eta (alpha - alpha_*) U U^T/||U||^2) S^T)
-      T lnew[3];
+      T lnew[36];
       ram_update<T>(p, l, z, (T)eta * (alpha - (T)cfg.target_accept_chi), lnew);
       for (int j = 0; j < p; ++j) chi[(size_t)j * N + i] = x[j];
       for (int k = 0; k < nt; ++k) L[(size_t)k * N + i] = lnew[k];
       // population terms at the new chi, fp64 (log-posterior with the updated parameters)
-      double xd[2], dd[4];
+      double xd[8], dd[16];
       for (int j = 0; j < p; ++j) xd[j] = (double)x[j];
       for (int c = 0; c < nc; ++c) dd[c] = (double)d[c];
       const double a = logpop<double>(model, xd, dd, theta.data(), cD);
@@ -307,7 +307,7 @@ int oracle_create(const oracle_config* cfg, oracle_sampler** out) {
   if (!(cfg->target_accept_theta > 0 && cfg->target_accept_theta < 1)) return ORACLE_E_INVALID;
   std::unique_ptr<Base> b;
   if (cfg->precision == ORACLE_F64) b.reset(new Impl<double>());
-  else if (cfg->precision == ORACLE_F32_STATE_F64_REDUCE) b.reset(new Impl<float>());
+  else if (cfg->precision == ORACLE_F32_STATE_F64_REDUCE && d.p <= 2) b.reset(new Impl<float>());   // fp32 draws: p <= 2
   else return ORACLE_E_UNSUPPORTED;
   b->cfg = *cfg;
   b->dims = d;

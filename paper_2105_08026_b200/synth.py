@@ -12,7 +12,7 @@ from dataclasses import dataclass
 
 import numpy as np
 
-M_NORMAL1D, M_THINNED_SCHECHTER1D, M_BINORMAL2D, M_LINREG_ME1D, M_BB1_FLUXNOISE1D = 0, 1, 2, 3, 4
+M_NORMAL1D, M_THINNED_SCHECHTER1D, M_BINORMAL2D, M_LINREG_ME1D, M_BB1_FLUXNOISE1D, M_NORMAL3D_KNOWNCOV = 0, 1, 2, 3, 4, 5
 F64, F32_STATE_F64_REDUCE = 0, 1
 
 
@@ -40,6 +40,9 @@ CONFIGS = {
     "C4": RunConfig("C4", M_LINREG_ME1D, F32_STATE_F64_REDUCE, 10_000_000, 2_000, 500, 1, 0.44, 0.234, False, 4),
     # the paper's own case study (Table 5.1): BB1 population, N = 1e5
     "C5": RunConfig("C5", M_BB1_FLUXNOISE1D, F64, 100_000, 5_000, 1_000, 1, 0.44, 0.234, False, 5),
+    # the normal-normal benchmark of PAPER.md:146-188 (3-vector latents, known C_pop) at the
+    # largest population the paper ran (N = 3e4), p = 3 RAM with the general rank-one Cholesky update
+    "C6": RunConfig("C6", M_NORMAL3D_KNOWNCOV, F64, 30_000, 5_000, 1_000, 1, 0.234, 0.234, False, 6),
 }
 
 # constants of the thinned point-process configs: {F_lim, sigma_F, x_lo, x_hi, r_min, r_max}
@@ -58,6 +61,16 @@ BB1_FTH = 20.0 / (4.0 * np.pi)
 BB1_SIGMA0 = BB1_FTH * np.sqrt(1.0 - (BB1_NU * BB1_ALPHA_NOISE) ** 2) / BB1_NU
 # constants of the model: {sigma_0, alpha, x_lo, x_hi, r_min, r_max, F_th}
 BB1_CONSTS = np.array([BB1_SIGMA0, BB1_ALPHA_NOISE, np.log(1e-5), np.log(30.0), 1e-4, 1.0, BB1_FTH])
+
+
+# normal-normal benchmark (Eq. 3.3-3.4)
+NN3_MU = np.array([1.2, -0.4, 3.4])
+NN3_D = np.array([2.3, 0.45, 13.4])
+NN3_R = np.array([[1.0, 0.3, -0.5], [0.3, 1.0, 0.54], [-0.5, 0.54, 1.0]])
+NN3_SIGMA = np.array([1.2, 0.4, 0.24])
+NN3_CPOP = NN3_D[:, None] * NN3_R * NN3_D[None, :]
+# constants of the model: {sigma_1..3, packed lower triangle of C_pop}
+NN3_CONSTS = np.concatenate([NN3_SIGMA, NN3_CPOP[np.tril_indices(3)]])
 
 
 def _rng(seed):
@@ -163,6 +176,15 @@ def make_bb1_fluxnoise1d(n, seed=5, truth=BB1_TRUTH):
                 detected_fraction=reach * n / max(drawn, 1))
 
 
+def make_normal3d_knowncov(n, seed=6):
+    """C6, the normal-normal benchmark: chi_i ~ N3(mu, C_pop = D R D), y_ij = chi_ij + sigma_j eps."""
+    g = _rng(seed)
+    chi = NN3_MU[:, None] + np.linalg.cholesky(NN3_CPOP) @ g.standard_normal((3, n))
+    y = chi + NN3_SIGMA[:, None] * g.standard_normal((3, n))
+    return dict(model=M_NORMAL3D_KNOWNCOV, cols=[y[0].copy(), y[1].copy(), y[2].copy()], consts=NN3_CONSTS.copy(),
+                chi_true=chi, theta_true=NN3_MU.copy(), theta0=NN3_MU + np.array([0.05, -0.02, 0.2]))
+
+
 def make_binormal2d(n, seed=3, fp32=False):
     """C3: chi ~ N2(m, Sigma), m=(0,0.5), sds (1, e^-0.5), rho=0.3; per-axis sigma ~ U(0.05,0.3)."""
     g = _rng(seed)
@@ -197,7 +219,7 @@ def make_linreg_me1d(n, seed=4, fp32=True):
 
 
 def make_inputs(config_name, n_objects=None):
-    """Inputs of config C0..C5; n_objects overrides N (reduced-size parity cases keep the recipe)."""
+    """Inputs of config C0..C6; n_objects overrides N (reduced-size parity cases keep the recipe)."""
     c = CONFIGS[config_name]
     n = c.n_objects if n_objects is None else int(n_objects)
     if c.model == M_NORMAL1D:
@@ -208,4 +230,6 @@ def make_inputs(config_name, n_objects=None):
         return make_binormal2d(n, c.seed)
     if c.model == M_BB1_FLUXNOISE1D:
         return make_bb1_fluxnoise1d(n, c.seed)
+    if c.model == M_NORMAL3D_KNOWNCOV:
+        return make_normal3d_knowncov(n, c.seed)
     return make_linreg_me1d(n, c.seed, fp32=(c.precision == F32_STATE_F64_REDUCE))
