@@ -7,7 +7,7 @@ chi moments on device, theta chain thinned by 10) -- the configuration BASELINE.
 `--warmup W` iterations run untimed as burn-in, then EXACTLY `--steps K` post-burn-in iterations are timed with
 CUDA events on the sampler's stream, bracketed by barrier + synchronize; rank 0 prints ONE JSON line.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C0..C5] [--theta-mode tail|graph|host]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C0..C6] [--theta-mode tail|graph|host]
     python bench.py --impl reference ...      # the CPU oracle, as it stands, on the same config / metric
 
 Multi-GPU: the path does not shard without a per-iteration exchange (the theta step needs the global sum), and
@@ -33,7 +33,8 @@ METRIC = "plate_ram_updates_per_s"
 UNIT = "updates/s"
 # algorithmic bytes per object per iteration: state read+write and
 # data read; + running-moment read+write (fp64 mean and M2 per component) once past burn-in
-ALG_BYTES = {"C0": (48, 32), "C1": (48, 32), "C2": (48, 32), "C3": (112, 64), "C4": (28, 32), "C5": (48, 32)}
+ALG_BYTES = {"C0": (48, 32), "C1": (48, 32), "C2": (48, 32), "C3": (112, 64), "C4": (28, 32), "C5": (48, 32),
+             "C6": (240, 96)}     # p = 3: chi 3 + L 6 doubles read and written, 3 data doubles read
 MODES = {"host": 0, "graph": 1, "tail": 2}
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel PER GIBBS ITERATION, from the committed
 # `ncu --set full` captures (profiles/r01f_resident_C2_ncu.md: 14.60 MB + 0.075 MB over 300 iterations;
@@ -45,6 +46,8 @@ NCU_DRAM_BYTES_PER_ITER = {"C2": (14.599424e6 + 75.008e3) / 300, "C4": (5.940074
 def workload_label(name):
     if name == "C5":
         return "C5: the paper's own case study (PAPER.md section 5.3, Table 5.1: BB1 population, N = 1e5); not a BASELINE.json config"
+    if name == "C6":
+        return "C6: the paper's normal-normal benchmark (PAPER.md section 3: 3-vector latents, N = 3e4); not a BASELINE.json config"
     return f"{name}: BASELINE.json configs[{int(name[1])}]"
 
 
@@ -152,6 +155,8 @@ def make_workload(cfg_name, n_override=0, seed_offset=0):
         inp = synth.make_binormal2d(n, c.seed + seed_offset)
     elif c.model == synth.M_BB1_FLUXNOISE1D:
         inp = synth.make_bb1_fluxnoise1d(n, c.seed + seed_offset)
+    elif c.model == synth.M_NORMAL3D_KNOWNCOV:
+        inp = synth.make_normal3d_knowncov(n, c.seed + seed_offset)
     else:
         inp = synth.make_linreg_me1d(n, c.seed + seed_offset, fp32=(c.precision == synth.F32_STATE_F64_REDUCE))
     return c, n, inp
@@ -364,12 +369,16 @@ def main():
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64" if c.precision == synth.F64 else "f32 state / f64 reductions", "data": "synthetic",
         "config": {"workload": workload_label(args.config), "n_objects": n,
-                   "model": ["normal1d", "thinned_schechter1d", "binormal2d", "linreg_me1d", "bb1_fluxnoise1d"][c.model],
+                   "model": ["normal1d", "thinned_schechter1d", "binormal2d", "linreg_me1d", "bb1_fluxnoise1d", "normal3d_knowncov"][c.model],
                    "burn_in": W, "thin": c.thin, "chi_moments": bool(c.keep_chi_moments),
                    "theta_mode": args.theta_mode, "parallelism": "replicas only" if world > 1 else "1 gpu",
                    "grid": [r["stats"]["grid_blocks"], r["stats"]["block_threads"]],
                    "l2": ("inputs larger than L2: every iteration streams the whole state through HBM"
                           if n * ALG_BYTES[args.config][0] > 126e6 else
+                          "streaming persistent kernel on a working set SMALLER than L2 (the sampler iterates over the "
+                          "same objects inside one launch, so there is nothing to flush between iterations): the state "
+                          "is served from L2, roofline.achieved divides the ALGORITHMIC bytes by the time"
+                          if r["stats"]["block_threads"] != 640 else
                           "state resident ON CHIP by design: the sampler iterates K times over the same objects "
                           "inside one persistent launch and keeps them in shared memory, so there is nothing to "
                           "flush between iterations; roofline.achieved divides the ALGORITHMIC bytes by the time "
@@ -420,7 +429,7 @@ def extras(args, device, peak, peak_src, n):
     out["other_theta_modes"] = modes
     side = {}
     # C3 / C4: the HBM-streaming configs; C5: the paper's own case study (BB1 population, N = 1e5)
-    for cfg_name, k, w in (("C3", 600, 200), ("C4", 300, 100), ("C5", 3000, 1000)):
+    for cfg_name, k, w in (("C3", 600, 200), ("C4", 300, 100), ("C5", 3000, 1000), ("C6", 3000, 1000)):
         if cfg_name == args.config:
             continue
         a = copy.copy(args)

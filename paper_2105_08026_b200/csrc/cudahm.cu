@@ -82,6 +82,7 @@ bool pick_kernels(int model, int precision, int block, KernelSet* k) {
       case M_BINORMAL2D:          return pick_block<M_BINORMAL2D, double>(block, k);
       case M_LINREG_ME1D:         return pick_block<M_LINREG_ME1D, double>(block, k);
       case M_BB1_FLUXNOISE1D:     return pick_block<M_BB1_FLUXNOISE1D, double>(block, k);
+      case M_NORMAL3D_KNOWNCOV:   return pick_block<M_NORMAL3D_KNOWNCOV, double>(block, k);
     }
   } else if (precision == CUDAHM_F32_STATE_F64_REDUCE) {
     switch (model) {
@@ -280,7 +281,7 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
   P.blk_cnt = (unsigned long long*)(s->ws + lay.blk_cnt);
   P.iter = (Iter*)(s->ws + lay.iter); P.trace = (double*)(s->ws + lay.trace); P.totals = (double*)(s->ws + lay.totals);
   P.qx = (double*)(s->ws + lay.qx); P.qex = (double*)(s->ws + lay.qex); P.qW = (double*)(s->ws + lay.qW);
-  for (int k = 0; k < 8; ++k) P.mc[k] = 0.0;
+  for (int k = 0; k < MC_N; ++k) P.mc[k] = 0.0;
   P.astar_chi = cfg->target_accept_chi;
   P.max_blocks = MAX_BLOCKS;
   P.tail = TailCfg{cfg->model, dt, cfg->freeze_theta ? 1 : 0, cfg->keep_chi_moments ? 1 : 0, cfg->seed,
@@ -380,6 +381,21 @@ extern "C" int cudahm_set_model_consts(cudahm_sampler* s, const double* v, int n
   if (!s) return fail(s, CUDAHM_E_INVALID, "NULL handle");
   if (n != s->nconsts || (n > 0 && !v)) return fail(s, CUDAHM_E_INVALID, "model takes %d constants, got %d", s->nconsts, n);
   if (n == 0) { s->have_consts = true; return CUDAHM_OK; }
+  if (s->cfg.model == M_NORMAL3D_KNOWNCOV) {
+    // NORMAL3D_KNOWNCOV: {sigma_1..3, packed lower triangle of C_pop} (Eq. 3.3-3.4).  The kernels take
+    // h_j = 1/(2 sigma_j^2) and Q = packed lower triangle of C_pop^-1 with the diagonal halved (adjugate / determinant).
+    const double c11 = v[3], c21 = v[4], c22 = v[5], c31 = v[6], c32 = v[7], c33 = v[8];
+    const double a11 = c22 * c33 - c32 * c32, a21 = c31 * c32 - c21 * c33, a31 = c21 * c32 - c31 * c22;
+    const double a22 = c11 * c33 - c31 * c31, a32 = c31 * c21 - c11 * c32, a33 = c11 * c22 - c21 * c21;
+    const double det = c11 * a11 + c21 * a21 + c31 * a31;
+    if (!(v[0] > 0.0 && v[1] > 0.0 && v[2] > 0.0 && c11 > 0.0 && a33 > 0.0 && det > 0.0))
+      return fail(s, CUDAHM_E_INVALID, "model constants out of range (sigma_j > 0, C_pop positive definite)");
+    for (int j = 0; j < 3; ++j) s->P.mc[MN_H + j] = 0.5 / (v[j] * v[j]);
+    const double q[6] = {0.5 * a11 / det, a21 / det, 0.5 * a22 / det, a31 / det, a32 / det, 0.5 * a33 / det};
+    for (int j = 0; j < 6; ++j) s->P.mc[MN_Q + j] = q[j];
+    s->have_consts = true; s->have_init = false;
+    return CUDAHM_OK;
+  }
   std::vector<double> xk, wk, rj, wj, ex(NQUAD), W(NQUAD);
   if (s->cfg.model == M_THINNED_SCHECHTER1D) {
     // THINNED_SCHECHTER1D: {F_lim, sigma_F, x_lo, x_hi, r_min, r_max}

@@ -34,7 +34,7 @@ struct Params {
   const double* qx;              // [NQUAD] quadrature nodes x_k
   const double* qex;             // [NQUAD] e^{x_k}
   const double* qW;              // [NQUAD] W_k = w_k G(x_k)
-  double mc[8];                  // model constants (MC_*)
+  double mc[MC_N];               // model constants (MC_* / MB_* / MN_*)
   double astar_chi;
   int max_blocks, pad_;
   TailCfg tail;
@@ -60,6 +60,8 @@ __device__ __forceinline__ void st_vec(float* p, const float* v) { *reinterpret_
 __device__ __forceinline__ double hm_sqrt(double x) { return sqrt(x); }
 __device__ __forceinline__ float hm_sqrt(float x) { return sqrtf(x); }
 // sqrt of a positive normal number as x * rsqrt(x) (<= 2 ulp): the RAM scale factor sqrt(1 + c), 1 + c in (0.4, 2)
+__device__ __forceinline__ double hm_rsqrt(double x) { return rsqrt(x); }
+__device__ __forceinline__ float hm_rsqrt(float x) { return rsqrtf(x); }
 __device__ __forceinline__ double hm_sqrt_pos(double x) { return hm_sqrt_fast(x); }
 __device__ __forceinline__ float hm_sqrt_pos(float x) { return x * rsqrtf(x); }
 
@@ -70,8 +72,9 @@ __device__ __forceinline__ float hm_sqrt_pos(float x) { return x * rsqrtf(x); }
 //         p = 2 normals:   per object, draw 1 of object i; z = rad*(cs, sn), unit vector (cs, sn).
 //   fp32  p = 1: one call per pair (draw 0 of pair m): x -> u1, y -> u2, cos / sin branch, accept uniforms z / w.
 // i0 is the even object of the pair.  z[h][k]: normal k of object i0 + h.
-template <int P>
-__device__ __forceinline__ void pair_draws(unsigned long long seed, long long i0, uint32_t t, double (*z)[2], double* cs,
+//         p = 3 normals:   per object, draws 1 and 2 of object i: (z0, z1) and (z2, -).
+template <int P, int ZD>
+__device__ __forceinline__ void pair_draws(unsigned long long seed, long long i0, uint32_t t, double (*z)[ZD], double* cs,
                                            double* sn, double* u) {
   const uint64_t m = (uint64_t)i0 >> 1;
   const U4 a = stream(seed, KIND_PLATE, m, t, 0u);
@@ -93,12 +96,21 @@ __device__ __forceinline__ void pair_draws(unsigned long long seed, long long i0
       const double rad = hm_sqrt_fast(-2.0 * hm_log_unit(u1));
       sincospi(2.0 * u2, &sn[h], &cs[h]);
       z[h][0] = rad * cs[h]; z[h][1] = rad * sn[h];
+      if constexpr (P == 3) {
+        static_assert(P < 3 || ZD >= 3, "z needs room for the third normal");
+        const U4 b2 = stream(seed, KIND_PLATE, (uint64_t)(i0 + h), t, 2u);
+        const double v1 = u01(b2.x, b2.y), v2 = u01(b2.z, b2.w);
+        double s2_, c2_;
+        sincospi(2.0 * v2, &s2_, &c2_);
+        z[h][2] = hm_sqrt_fast(-2.0 * hm_log_unit(v1)) * c2_;
+      }
     }
   }
 }
-template <int P>
-__device__ __forceinline__ void pair_draws(unsigned long long seed, long long i0, uint32_t t, float (*z)[2], float* cs,
+template <int P, int ZD>
+__device__ __forceinline__ void pair_draws(unsigned long long seed, long long i0, uint32_t t, float (*z)[ZD], float* cs,
                                            float* sn, float* u) {
+  static_assert(P <= 2, "fp32 state: p <= 2");
   if (P == 1) {
     const U4 r = stream(seed, KIND_PLATE, (uint64_t)i0 >> 1, t, 0u);
     const float u1 = u01f(r.x), u2 = u01f(r.y);
@@ -131,7 +143,7 @@ template <class T> struct SweepCtx {
   uint32_t t;
   ThetaK kc, kp;
   KT<T> kT;
-  T mcT[7];
+  T mcT[MC_N];
   T eta, astar;
   bool do_mom;
   double inv_k;
@@ -143,7 +155,7 @@ __device__ __forceinline__ SweepCtx<T> make_ctx(const Params& P, const Iter& it)
   c.kc = it.kc; c.kp = it.kp;
   c.kT = narrow<T>(c.kc);
 #pragma unroll
-  for (int j = 0; j < 7; ++j) c.mcT[j] = (T)P.mc[j];
+  for (int j = 0; j < MC_N; ++j) c.mcT[j] = (T)P.mc[j];
   c.eta = (T)it.dr[it.t % 3].eta; c.astar = (T)P.astar_chi;
   c.do_mom = P.tail.keep_moments && it.t > P.tail.burn_in;
   c.inv_k = 1.0 / (double)(it.mom_count + 1);
@@ -157,7 +169,8 @@ __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c
                                            T (*x)[VecOf<T>::n], T (*l)[VecOf<T>::n], const T (*d)[VecOf<T>::n], double* sum) {
   constexpr int p = ModelDims<MODEL>::p, ntri = p * (p + 1) / 2, ncols = ModelDims<MODEL>::ncols;
   constexpr int VEC = VecOf<T>::n;
-  T zz[VEC][2], csv[VEC], snv[VEC], uu[VEC];
+  constexpr int ZD = p < 2 ? 2 : p;
+  T zz[VEC][ZD], csv[VEC], snv[VEC], uu[VEC];
 #pragma unroll
   for (int v = 0; v < VEC; v += 2) pair_draws<p>(P.tail.seed, base + v, c.t, &zz[v], &csv[v], &snv[v], &uu[v]);
 #pragma unroll
@@ -173,8 +186,13 @@ __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c
     for (int q = 0; q < ncols; ++q) di[q] = d[q][v];
     // step 1: chi' = chi + L z
     T yi[p];
-    yi[0] = xi[0] + l[0][v] * z[0];
-    if (p == 2) yi[1] = xi[1] + l[1][v] * z[0] + l[2][v] * z[1];
+#pragma unroll
+    for (int r = 0; r < p; ++r) {
+      T a_ = xi[r];
+#pragma unroll
+      for (int k = 0; k <= r; ++k) a_ += l[r * (r + 1) / 2 + k][v] * z[k];
+      yi[r] = a_;
+    }
     // step 2: alpha = min{1, pi(chi')/pi(chi)}
     using PL = Plate<MODEL, T>;
     const typename PL::Pt qc = PL::point(xi), qp = PL::point(yi);
@@ -190,8 +208,33 @@ __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c
     // step 3: L <- L chol(I + c uu^T), u = z/|z| = (cs, sn)
     const T cc = c.eta * (alpha - c.astar);
     T ln[ntri];
-    if (p == 1) {
+    if constexpr (p == 1) {
       ln[0] = l[0][v] * hm_sqrt_pos(T(1) + cc);
+    } else if constexpr (p >= 3) {
+      // general p, the rank-one update in closed form (theta_step.cuh::ram_coeffs): with u = z/|z| and
+      // s_j = 1 + c sum_{k<j} u_k^2:  K = chol(I + c u u^T) has K_jj = sqrt(s_{j+1}/s_j), K_ij = c u_i u_j/sqrt(s_j s_{j+1}),
+      // and (L K)_ij = L_ij K_jj + (c u_j/sqrt(s_j s_{j+1})) sum_{k=j+1..i} L_ik u_k -- the unique left factor of Eq. 2.6
+      T n2 = T(0);
+#pragma unroll
+      for (int j = 0; j < p; ++j) n2 += z[j] * z[j];
+      const T rn = hm_rsqrt(n2);
+      T uh[p], sj[p + 1];
+      T run = T(0);
+      sj[0] = T(1);
+#pragma unroll
+      for (int j = 0; j < p; ++j) { uh[j] = z[j] * rn; run += uh[j] * uh[j]; sj[j + 1] = T(1) + cc * run; }
+#pragma unroll
+      for (int j = 0; j < p; ++j) {
+        const T rr = hm_rsqrt(sj[j] * sj[j + 1]);
+        const T Kd = sj[j + 1] * rr, g = cc * uh[j] * rr;
+#pragma unroll
+        for (int i = j; i < p; ++i) {
+          T W = T(0);
+#pragma unroll
+          for (int k = j + 1; k <= i; ++k) W += l[i * (i + 1) / 2 + k][v] * uh[k];
+          ln[i * (i + 1) / 2 + j] = l[i * (i + 1) / 2 + j][v] * Kd + g * W;
+        }
+      }
     } else {
       const T s1 = T(1) + cc * cs * cs;
       const T k00 = hm_sqrt(s1);
@@ -202,7 +245,7 @@ __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c
       ln[2] = l[2][v] * k11;
     }
     // population terms at the new chi, fp64
-    const double a = PL::pop(qn, di, c.kc), b = PL::pop(qn, di, c.kp);
+    const double a = PL::pop(qn, di, c.kc, P.mc), b = PL::pop(qn, di, c.kp, P.mc);
     if (live) {
 #pragma unroll
       for (int k = 0; k < ntri; ++k) l[k][v] = ln[k];

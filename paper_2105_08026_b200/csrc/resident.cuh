@@ -111,9 +111,9 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
         }
       }
     };
-    T mcT[7];
+    T mcT[MC_N];
 #pragma unroll
-    for (int j = 0; j < 7; ++j) mcT[j] = (T)P.mc[j];
+    for (int j = 0; j < MC_N; ++j) mcT[j] = (T)P.mc[j];
     const T astar = (T)P.astar_chi;
     double nacc = 0.0, nnan = 0.0;
 
@@ -205,7 +205,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
         const T xn = HM_AT(V::V_CHI, r);
         typename PL::Pt qn;
         if constexpr (V::m1) qn = typename PL::Pt{xn, HM_AT(V::V_E, r)}; else qn = PL::point(&xn);
-        v[0] += PL::pop(qn, di, kp) - PL::pop(qn, di, kc);
+        v[0] += PL::pop(qn, di, kp, P.mc) - PL::pop(qn, di, kc, P.mc);
       }
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) v[0] += __shfl_down_sync(0xffffffffu, v[0], o);

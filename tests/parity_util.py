@@ -17,7 +17,8 @@ def make_pair(model, n, seed, precision=B.F64, theta_mode=B.THETA_DEVICE_TAIL, a
               want_oracle=True, flags=0):
     if inputs is None:
         maker = {0: synth.make_normal1d, 1: synth.make_thinned_schechter1d, 2: synth.make_binormal2d,
-                 3: synth.make_linreg_me1d, 4: synth.make_bb1_fluxnoise1d}[model]
+                 3: synth.make_linreg_me1d, 4: synth.make_bb1_fluxnoise1d,
+                 5: synth.make_normal3d_knowncov}[model]
         kw = dict(fp32=True) if (precision == B.F32_STATE_F64_REDUCE and model in (0, 3)) else {}
         if model == 3 and precision == B.F64:
             kw = dict(fp32=False)

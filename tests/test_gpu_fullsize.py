@@ -67,6 +67,21 @@ def test_c5_full_size_free_running():
     assert st["chi_accepts"] == sto["chi_accepts"] and st["theta_accepts"] == sto["theta_accepts"]
 
 
+def test_c6_full_size_free_running():
+    """C6, the normal-normal benchmark at the paper's largest population (N = 3e4, p = 3) in the
+    streaming persistent kernel; 40 iterations."""
+    c, orc, gpu = _pair("C6")
+    orc.run(40, 0, 1)
+    gpu.run(40, 0, 1, sync=True)
+    so, sg = orc.get_state(), gpu.get_state()
+    np.testing.assert_allclose(gpu.get_theta_trace(), orc.get_theta_trace(), rtol=1e-9, atol=1e-9)
+    np.testing.assert_allclose(sg["chi"], so["chi"], rtol=1e-9, atol=1e-9)
+    np.testing.assert_allclose(sg["L"], so["L"], rtol=1e-9, atol=1e-12)
+    np.testing.assert_allclose(sg["L_theta"], so["L_theta"], rtol=1e-8, atol=1e-12)
+    st, sto = gpu.get_stats(), orc.get_stats()
+    assert st["chi_accepts"] == sto["chi_accepts"] and st["theta_accepts"] == sto["theta_accepts"]
+
+
 def test_c3_full_size_free_running():
     """C3 as benched: N = 1e6, 2-D latent, streaming persistent kernel (148 x 512); 8 iterations."""
     c, orc, gpu = _pair("C3")

@@ -20,8 +20,9 @@ CASES = [
     (B.M_NORMAL1D, B.F32_STATE_F64_REDUCE, 0.44, 4097),
     (B.M_LINREG_ME1D, B.F32_STATE_F64_REDUCE, 0.44, 10007),
     (B.M_BB1_FLUXNOISE1D, B.F64, 0.44, 4099),
+    (B.M_NORMAL3D_KNOWNCOV, B.F64, 0.234, 3003),
 ]
-IDS = ["M0-f64", "M1-f64", "M2-f64", "M3-f64", "M0-f32", "M3-f32", "M4-f64"]
+IDS = ["M0-f64", "M1-f64", "M2-f64", "M3-f64", "M0-f32", "M3-f32", "M4-f64", "M5-f64"]
 
 
 @pytest.mark.parametrize("model,precision,astar,n", CASES, ids=IDS)
@@ -69,8 +70,9 @@ def test_lockstep_trajectory(model, precision, astar, n):
 
 @pytest.mark.parametrize("mode", [B.THETA_HOST, B.THETA_GRAPH, B.THETA_DEVICE_TAIL], ids=["host", "graph", "tail"])
 @pytest.mark.parametrize("model,astar,n", [(B.M_NORMAL1D, 0.44, 1000), (B.M_THINNED_SCHECHTER1D, 0.44, 3000),
-                                             (B.M_BINORMAL2D, 0.234, 2000), (B.M_BB1_FLUXNOISE1D, 0.44, 3000)],
-                         ids=["M0", "M1", "M2", "M4"])
+                                             (B.M_BINORMAL2D, 0.234, 2000), (B.M_BB1_FLUXNOISE1D, 0.44, 3000),
+                                             (B.M_NORMAL3D_KNOWNCOV, 0.234, 2001)],
+                         ids=["M0", "M1", "M2", "M4", "M5"])
 def test_free_running_matches_oracle(model, astar, n, mode):
     """cudahm_run (no taps, no resync) for 120 iterations in every theta mode against oracle_run: same theta
     trace, same chi / L, same moments, same counters.  (~1e5 decisions at ~1e-9 tie probability each.)"""
@@ -123,8 +125,9 @@ def test_theta_modes_agree():
 
 @pytest.mark.parametrize("flags", [B.FLAG_STREAMING_ONLY | B.FLAG_TMA_STAGING, B.FLAG_STREAMING_ONLY], ids=["tma", "ldg"])
 @pytest.mark.parametrize("model,astar,n", [(B.M_NORMAL1D, 0.44, 1000), (B.M_THINNED_SCHECHTER1D, 0.44, 3000),
-                                             (B.M_LINREG_ME1D, 0.44, 150001), (B.M_BB1_FLUXNOISE1D, 0.44, 3000)],
-                         ids=["M0", "M1", "M3", "M4"])
+                                             (B.M_LINREG_ME1D, 0.44, 150001), (B.M_BB1_FLUXNOISE1D, 0.44, 3000),
+                                             (B.M_NORMAL3D_KNOWNCOV, 0.234, 2001)],
+                         ids=["M0", "M1", "M3", "M4", "M5"])
 def test_streaming_persistent_kernel_matches_oracle(model, astar, n, flags):
     """The HBM-streaming persistent kernel (what C3 / C4 and any population too large for shared memory run),
     forced on the small fp64 p=1 cases that would otherwise take the on-chip kernel."""
