@@ -210,7 +210,13 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
   *out = nullptr;
   int p, dt, nc, nk;
   if (!valid_config(cfg, &p, &dt, &nc, &nk)) return fail(nullptr, CUDAHM_E_INVALID, "invalid cudahm_config");
-  const int block = cfg->block_threads ? cfg->block_threads : 512;
+  // default block: 512 threads; a population too small to give every SM a 512-thread block of 16-byte vectors takes
+  // 256-thread blocks instead (twice the SMs at work: the small configs are latency-bound, not bandwidth-bound)
+  int block = cfg->block_threads ? cfg->block_threads : 512;
+  if (!cfg->block_threads) {
+    const long long vec = cfg->precision == CUDAHM_F64 ? 2 : 4;
+    if ((cfg->n_objects + vec * 512 - 1) / (vec * 512) < 148) block = 256;
+  }
   KernelSet ks;
   if (!pick_kernels(cfg->model, cfg->precision, block, &ks))
     return fail(nullptr, CUDAHM_E_UNSUPPORTED, "model %d is not compiled in for precision %d", cfg->model, cfg->precision);
