@@ -86,6 +86,13 @@ typedef struct {
   int32_t  flags;                /* 0, or CUDAHM_FLAG_* ORed                                                */
   int64_t  max_trace_rows;       /* capacity of the on-device thinned theta trace (rows of dtheta doubles);
                                     0 = keep no trace                                                        */
+  /* advanced use.  Precisely measured predictors are read-only data columns (M3's z, the g
+   * column of M1 / M4), which is what PAPER.md:397-399 asks users to arrange by overriding the default kernels.  */
+  int64_t  adapt_until;          /* 0: the RAM adaptation never stops (it "decays with time"); else
+                                    eta_n = 0 for t > adapt_until: plate and theta proposal factors are frozen  */
+  double   prior_mean[8];        /* user prior on theta multiplying the model's default (the default */
+  double   prior_isd[8];         /* is uniform and can be overridden): independent normal factors
+                                    N(prior_mean[j], 1/prior_isd[j]^2) on theta[j]; prior_isd[j] = 0: no factor   */
 } cudahm_config;
 
 typedef struct {

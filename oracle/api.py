@@ -23,7 +23,8 @@ class Config(C.Structure):
                 ("seed", C.c_uint64), ("target_accept_chi", C.c_double),
                 ("target_accept_theta", C.c_double), ("eta_exponent", C.c_double),
                 ("init_scale_chi", C.c_double), ("freeze_theta", C.c_int32),
-                ("keep_chi_moments", C.c_int32)]
+                ("keep_chi_moments", C.c_int32), ("adapt_until", C.c_int64),
+                ("prior_mean", C.c_double * 8), ("prior_isd", C.c_double * 8)]
 
 
 class Taps(C.Structure):
@@ -128,14 +129,18 @@ class Sampler:
 
     def __init__(self, model, n_objects, seed=0, precision=F64, target_accept_chi=0.4,
                  target_accept_theta=0.234, eta_exponent=2.0 / 3.0, init_scale_chi=1.0,
-                 freeze_theta=False, keep_chi_moments=False):
+                 freeze_theta=False, keep_chi_moments=False, adapt_until=0, prior_mean=None, prior_sd=None):
         self.dims = model_dims(model)
         self.N = int(n_objects)
         self.p, self.dtheta = self.dims["p"], self.dims["dtheta"]
         self.ntri = self.p * (self.p + 1) // 2
         self.ntri_theta = self.dtheta * (self.dtheta + 1) // 2
         self.cfg = Config(model, precision, self.N, seed, target_accept_chi, target_accept_theta,
-                          eta_exponent, init_scale_chi, int(freeze_theta), int(keep_chi_moments))
+                          eta_exponent, init_scale_chi, int(freeze_theta), int(keep_chi_moments), int(adapt_until))
+        if prior_mean is not None:
+            for j, (m, sd) in enumerate(zip(prior_mean, prior_sd)):
+                self.cfg.prior_mean[j] = float(m)
+                self.cfg.prior_isd[j] = 0.0 if not np.isfinite(sd) else 1.0 / float(sd)
         self._h = C.c_void_p()
         _check(lib().oracle_create(C.byref(self.cfg), C.byref(self._h)), "create")
 

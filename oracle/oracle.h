@@ -47,6 +47,11 @@ typedef struct {
   double   init_scale_chi;      /* S_1 = init_scale_chi * I (paper: identity)              */
   int32_t  freeze_theta;        /* 1: skip the theta step entirely (theta held fixed)      */
   int32_t  keep_chi_moments;    /* 1: accumulate running mean / M2 of chi after burn-in    */
+  /* advanced use */
+  int64_t  adapt_until;         /* 0: RAM adaptation never stops ("decays with time"); else eta_n = 0
+                                   for iterations t > adapt_until (plate and theta factors frozen from then on)   */
+  double   prior_mean[8];       /* user prior on theta, multiplying the model's default (uniform):   */
+  double   prior_isd[8];        /* independent normal factors N(prior_mean_j, 1/prior_isd_j^2); isd_j = 0: none    */
 } oracle_config;
 
 /* Per-iteration taps (all optional: a NULL member is skipped).  Per-object arrays have N entries

@@ -69,6 +69,15 @@ struct Base {
   virtual int step(int64_t burn_in, int32_t thin, oracle_taps* taps) = 0;
   virtual int get_state(double* chi, double* L, double* th, double* Lth, int64_t* tt) = 0;
   virtual int set_state(const double* chi, const double* L, const double* th, const double* Lth, int64_t tt) = 0;
+  // user prior on theta ("To override this default prior ..."): independent normal factors
+  double user_prior(const double* th) const {
+    double s = 0.0;
+    for (int j = 0; j < dims.dtheta; ++j) {
+      const double r = (th[j] - cfg.prior_mean[j]) * cfg.prior_isd[j];
+      s += -0.5 * r * r;
+    }
+    return s;
+  }
   double theta_only(const double* th) const {
     if (cfg.model == M_THINNED_SCHECHTER1D) return table.theta_only(th);
     // M4: log L = sum_i [log rho(x_i; theta) + log l_i(x_i)] - N log I(theta)   (Eq. 4.3-4.4)
@@ -150,7 +159,8 @@ struct Impl : Base {
     // O1: this is RAM iteration n = t + 1 (X_1, S_1 are the initial values)
     const uint32_t tcur = (uint32_t)(t + 1);
     const double n_ram = (double)(t + 1) + 1.0;
-    const double eta = std::pow(n_ram, -cfg.eta_exponent);          // eta_n = n^(-2/3)
+    double eta = std::pow(n_ram, -cfg.eta_exponent);                // eta_n = n^(-2/3)
+    if (cfg.adapt_until > 0 && (t + 1) > cfg.adapt_until) eta = 0.0; // adaptation frozen: S_n = S_{n-1}
 
     // O2: theta proposal theta' = theta + L_theta z  (drawn before the sweep: it does not depend on chi)
     double zth[8] = {0}, thp[8] = {0};
@@ -246,8 +256,8 @@ struct Impl : Base {
     int acc_th = 0;
     if (!cfg.freeze_theta) {
       T_cur = theta_only(theta.data());
-      lp_cur = logprior(model, theta.data());
-      lp_prop = logprior(model, thp);
+      lp_cur = logprior(model, theta.data()) + user_prior(theta.data());
+      lp_prop = logprior(model, thp) + user_prior(thp);
       double la_th;
       if (lp_prop == ninf) { log_r = ninf; la_th = ninf; T_prop = 0; }
       else {

@@ -35,7 +35,8 @@ class Config(C.Structure):
                 ("target_accept_chi", C.c_double), ("target_accept_theta", C.c_double),
                 ("eta_exponent", C.c_double), ("init_scale_chi", C.c_double), ("keep_chi_moments", C.c_int32),
                 ("block_threads", C.c_int32), ("blocks_per_sm", C.c_int32), ("flags", C.c_int32),
-                ("max_trace_rows", C.c_int64)]
+                ("max_trace_rows", C.c_int64), ("adapt_until", C.c_int64),
+                ("prior_mean", C.c_double * 8), ("prior_isd", C.c_double * 8)]
 
 
 class Stats(C.Structure):
@@ -112,11 +113,17 @@ def model_dims(model):
 
 def make_config(model, n_objects, seed=0, precision=F64, theta_mode=THETA_DEVICE_TAIL, target_accept_chi=0.4,
                 target_accept_theta=0.234, eta_exponent=2.0 / 3.0, init_scale_chi=1.0, freeze_theta=False,
-                keep_chi_moments=False, max_trace_rows=0, block_threads=0, blocks_per_sm=0, flags=0):
+                keep_chi_moments=False, max_trace_rows=0, block_threads=0, blocks_per_sm=0, flags=0, adapt_until=0,
+                prior_mean=None, prior_sd=None):
     d = model_dims(model)
-    return Config(C.sizeof(Config), model, precision, theta_mode, int(n_objects), d["p"], d["dtheta"], d["n_cols"],
+    cfg = Config(C.sizeof(Config), model, precision, theta_mode, int(n_objects), d["p"], d["dtheta"], d["n_cols"],
                   int(freeze_theta), seed, target_accept_chi, target_accept_theta, eta_exponent, init_scale_chi,
-                  int(keep_chi_moments), block_threads, blocks_per_sm, int(flags), int(max_trace_rows))
+                  int(keep_chi_moments), block_threads, blocks_per_sm, int(flags), int(max_trace_rows), int(adapt_until))
+    if prior_mean is not None:          # user prior: independent normal factors on theta (sd = inf: none)
+        for j, (m, sd) in enumerate(zip(prior_mean, prior_sd)):
+            cfg.prior_mean[j] = float(m)
+            cfg.prior_isd[j] = 0.0 if not np.isfinite(sd) else 1.0 / float(sd)
+    return cfg
 
 
 def workspace_bytes(cfg):

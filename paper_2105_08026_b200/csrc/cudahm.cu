@@ -156,7 +156,9 @@ bool valid_config(const cudahm_config* c, int* p, int* dt, int* nc, int* nk) {
   if (!(c->eta_exponent > 0.0 && c->eta_exponent <= 1.0) || !(c->init_scale_chi > 0.0)) return false;
   if (c->block_threads != 0 && c->block_threads != 256 && c->block_threads != 512 && c->block_threads != 1024)
     return false;
-  if (c->blocks_per_sm < 0) return false;
+  if (c->blocks_per_sm < 0 || c->adapt_until < 0) return false;
+  for (int j = 0; j < 8; ++j)
+    if (!(c->prior_isd[j] >= 0.0) || !std::isfinite(c->prior_isd[j]) || !std::isfinite(c->prior_mean[j])) return false;
   return true;
 }
 
@@ -291,7 +293,9 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
   P.astar_chi = cfg->target_accept_chi;
   P.max_blocks = MAX_BLOCKS;
   P.tail = TailCfg{cfg->model, dt, cfg->freeze_theta ? 1 : 0, cfg->keep_chi_moments ? 1 : 0, cfg->seed,
-                   cfg->target_accept_theta, cfg->eta_exponent, 0, cfg->max_trace_rows, 1, 0, (double)cfg->n_objects};
+                   cfg->target_accept_theta, cfg->eta_exponent, 0, cfg->max_trace_rows, 1, 0, (double)cfg->n_objects,
+                   cfg->adapt_until, {}, {}};
+  for (int j = 0; j < MAXD; ++j) { P.tail.prior_mean[j] = cfg->prior_mean[j]; P.tail.prior_isd[j] = cfg->prior_isd[j]; }
   P.taps = DevTaps{};
 
   if (cudaMemsetAsync(s->ws, 0, lay.total, s->stream) != cudaSuccess ||

@@ -597,7 +597,7 @@ __global__ void __launch_bounds__(256, 1) k_init_iter(const Params P) {
   block_reduce<NPART>(part, red);
   if (threadIdx.x == 0) {
     it.kc = kc;
-    it.lp_cur = log_prior(P.tail.model, it.theta);
+    it.lp_cur = log_prior_full(P.tail, it.theta);
     it.T_cur = has_selection(P.tail.model) ? theta_only_from_sum(P.tail.model, kc, part[2], P.tail.n_objects) : 0.0;
     prepare_iteration(it, P.tail, it.t);
   }

@@ -51,7 +51,24 @@ struct TailCfg {
   long long burn_in, max_trace_rows;
   int thin, pad_;
   double n_objects;     // N of the selection term -N log I(theta) (M4)
+  long long adapt_until;             // 0: adapt forever; else eta_n = 0 for t > adapt_until
+  double prior_mean[MAXD], prior_isd[MAXD];   // user prior: independent normal factors on theta (isd = 0: none)
 };
+
+// eta_n of iteration t (n = t + 1: X_1, S_1 are the initial values); 0 once adaptation is frozen
+HM_HD double eta_of(const TailCfg& c, long long t) {
+  if (c.adapt_until > 0 && t > c.adapt_until) return 0.0;
+  return pow((double)(t + 1), -c.eta_exp);
+}
+// log prior = the model's default (uniform on a box; models.cuh) + the user's normal factors
+HM_HD double log_prior_full(const TailCfg& c, const double* th) {
+  double s = log_prior(c.model, th);
+  for (int j = 0; j < c.dtheta; ++j) {
+    const double r = (th[j] - c.prior_mean[j]) * c.prior_isd[j];
+    s += -0.5 * r * r;
+  }
+  return s;
+}
 
 HM_HD int tri(int r, int c) { return r * (r + 1) / 2 + c; }
 HM_HD int tri_row(int e) { int r = 0; while ((r + 1) * (r + 2) / 2 <= e) ++r; return r; }
@@ -76,7 +93,7 @@ HM_HD void ram_coeffs(int j, double c, const Draws& d, double* Kd, double* g) {
 }
 
 HM_HD void make_draws(Draws& d, const TailCfg& c, long long t) {
-  d.eta = pow((double)(t + 1), -c.eta_exp);
+  d.eta = eta_of(c, t);
   for (int j = 0; j < MAXD; ++j) { d.z[j] = 0.0; d.uh[j] = 0.0; }
   for (int j = 0; j <= MAXD; ++j) d.Pc[j] = 0.0;
   d.u = 0.0; d.lu = 0.0;
@@ -117,7 +134,7 @@ HM_HD void prepare_iteration(Iter& it, const TailCfg& c, long long t) {
     for (int i = 0; i < c.dtheta; ++i)
       for (int j = 0; j <= i; ++j) it.W[tri(i, j)] = make_W_entry(it, d, i, j);
     it.kp = theta_consts(c.model, it.thetaP);
-    it.lp_prop = log_prior(c.model, it.thetaP);
+    it.lp_prop = log_prior_full(c, it.thetaP);
   } else {
     for (int r = 0; r < c.dtheta; ++r) it.thetaP[r] = it.theta[r];
     it.kp = it.kc;
@@ -295,7 +312,7 @@ __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const dou
   } else if (warp == 2) {
     if (lane == 0) decide_schedule(it, c);               // moments count of t + 1: the next sweep reads it
     decided();
-    if (lane == 0) d2.eta = pow((double)(t + 3), -c.eta_exp);
+    if (lane == 0) d2.eta = eta_of(c, t + 2);
   } else if (warp == 3) {
     decided();
     if (lane == 0 && !c.freeze_theta) {
@@ -315,7 +332,7 @@ __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const dou
         const int e = lane - 1, ei = tri_row(e), ej = e - ei * (ei + 1) / 2;
         it.W[e] = make_W_entry(it, d1, ei, ej);
       }
-      if (warp == 3 && lane == 0) it.lp_prop_next = log_prior(c.model, it.thetaP);
+      if (warp == 3 && lane == 0) it.lp_prop_next = log_prior_full(c, it.thetaP);
     } else if (lane == 0) {               // warp 0: taps and acceptance bookkeeping of the decision just taken
       it.T_cur_used = it.T_cur; it.lp_cur_used = it.lp_cur;
       it.T_prop = T_prop; it.log_r = log_r; it.alpha_theta = alpha; it.u_theta = d0.u;

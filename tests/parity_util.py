@@ -14,7 +14,7 @@ TOL = {B.F64: dict(pi=1e-12, chi=1e-13, L=1e-12, pop=1e-12, tie=1e-9),
 
 def make_pair(model, n, seed, precision=B.F64, theta_mode=B.THETA_DEVICE_TAIL, astar=0.44, inputs=None, theta0=None,
               keep_moments=False, max_trace_rows=0, freeze_theta=False, block_threads=0, blocks_per_sm=0,
-              want_oracle=True, flags=0):
+              want_oracle=True, flags=0, adapt_until=0, prior_mean=None, prior_sd=None):
     if inputs is None:
         maker = {0: synth.make_normal1d, 1: synth.make_thinned_schechter1d, 2: synth.make_binormal2d,
                  3: synth.make_linreg_me1d, 4: synth.make_bb1_fluxnoise1d,
@@ -27,14 +27,16 @@ def make_pair(model, n, seed, precision=B.F64, theta_mode=B.THETA_DEVICE_TAIL, a
     orc = None
     if want_oracle:
         orc = O.Sampler(model, n, seed=seed, precision=precision, target_accept_chi=astar,
-                        keep_chi_moments=keep_moments, freeze_theta=freeze_theta)
+                        keep_chi_moments=keep_moments, freeze_theta=freeze_theta, adapt_until=adapt_until,
+                        prior_mean=prior_mean, prior_sd=prior_sd)
         orc.set_data(inputs["cols"])
         if inputs["consts"] is not None:
             orc.set_model_consts(inputs["consts"])
         orc.set_init(th0)
     gpu = B.Sampler(model, n, seed=seed, precision=precision, theta_mode=theta_mode, target_accept_chi=astar,
                     keep_chi_moments=keep_moments, max_trace_rows=max_trace_rows, freeze_theta=freeze_theta,
-                    block_threads=block_threads, blocks_per_sm=blocks_per_sm, flags=flags)
+                    block_threads=block_threads, blocks_per_sm=blocks_per_sm, flags=flags, adapt_until=adapt_until,
+                    prior_mean=prior_mean, prior_sd=prior_sd)
     gpu.set_data(inputs["cols"])
     if inputs["consts"] is not None:
         gpu.set_model_consts(inputs["consts"])

@@ -101,6 +101,39 @@ def test_free_running_matches_oracle(model, astar, n, mode):
     assert stg["gpu_launches"] > 0
 
 
+@pytest.mark.parametrize("mode", [B.THETA_HOST, B.THETA_GRAPH, B.THETA_DEVICE_TAIL], ids=["host", "graph", "tail"])
+@pytest.mark.parametrize("model,astar,n,flags", [(B.M_NORMAL1D, 0.44, 1500, 0), (B.M_BINORMAL2D, 0.234, 2000, 0),
+                                                   (B.M_NORMAL1D, 0.44, 1500, B.FLAG_STREAMING_ONLY)],
+                         ids=["M0", "M2", "M0-streaming"])
+def test_user_prior_and_adaptation_freeze_match_oracle(model, astar, n, flags, mode):
+    """The advanced-use hooks: a user prior on theta (normal factors on some components) and
+    adapt_until (eta_n = 0 from iteration 61 on), free-running against the oracle in every theta driver."""
+    iters, burn, thin, K = 120, 20, 5, 60
+    dt = 2 if model == B.M_NORMAL1D else 5
+    pm = [0.3, -0.2, 0.0, 0.0, 0.0][:dt]
+    psd = [0.05, np.inf, 0.1, np.inf, 0.2][:dt]
+    orc, gpu, _ = make_pair(model, n, seed=71 + model, astar=astar, theta_mode=mode, max_trace_rows=(iters - burn) // thin,
+                            adapt_until=K, prior_mean=pm, prior_sd=psd, flags=flags)
+    orc.run(K, burn, thin)
+    gpu.run(K, burn, thin, sync=True)
+    L_K, Lth_K = gpu.get_state()["L"].copy(), gpu.get_state()["L_theta"].copy()
+    np.testing.assert_allclose(L_K, orc.get_state()["L"], rtol=1e-9)
+    orc.run(iters - K, burn, thin)
+    gpu.run(iters - K, burn, thin, sync=True)
+    so, sg = orc.get_state(), gpu.get_state()
+    np.testing.assert_allclose(gpu.get_theta_trace(), orc.get_theta_trace(), rtol=1e-8, atol=1e-8)
+    np.testing.assert_allclose(sg["chi"], so["chi"], rtol=1e-9, atol=1e-9)
+    assert np.array_equal(sg["L"], L_K) and np.array_equal(sg["L_theta"], Lth_K)      # frozen: bit for bit on the device
+    np.testing.assert_allclose(sg["L"], so["L"], rtol=1e-9)
+    stg, sto = gpu.get_stats(), orc.get_stats()
+    assert stg["chi_accepts"] == sto["chi_accepts"] and stg["theta_accepts"] == sto["theta_accepts"]
+    # the prior is felt: lp taps differ from the default's zero
+    tg = gpu.debug_step(NO_TRACE, 1)
+    to = orc.step(NO_TRACE, 1, taps=True)
+    assert to["lp_cur"] != 0.0
+    compare_theta_step(to, tg, what="hooks")
+
+
 def test_theta_modes_agree():
     """Same grid, same thread->object map, same reduction order in the three streaming drivers.  GRAPH and the
     plain-load streaming DEVICE_TAIL kernel run the theta step with the same device code => identical bits.  HOST
