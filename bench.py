@@ -61,6 +61,9 @@ def parse_args():
     ap.add_argument("--theta-mode", default="tail", choices=sorted(MODES))
     ap.add_argument("--n-objects", type=int, default=0, help="override N (parity-size experiments)")
     ap.add_argument("--no-extras", action="store_true", help="skip cpu_baseline, floors and the side configs")
+    ap.add_argument("--sharded", action="store_true",
+                    help="ONE chain over a population of N objects PER GPU sharded by object range (SURVEY 8(e)): "
+                         "all-gather of five doubles per rank and iteration; default for --gpus > 1 is independent replicas")
     ap.add_argument("--block-threads", type=int, default=0)
     ap.add_argument("--blocks-per-sm", type=int, default=0)
     return ap.parse_args()
@@ -330,6 +333,61 @@ def run_reference(args, rank):
     print(json.dumps(line), flush=True)
 
 
+def run_sharded(args, device, rank, world, dist, barrier, peak, peak_src):
+    """ONE Metropolis-within-Gibbs chain over world x N objects, sharded by object range over the ranks (weak scaling:
+    N objects per GPU).  theta is replicated; per iteration every rank sweeps its shard (cudahm_shard_sweep), the ranks
+    all-gather their five totals over NCCL and sum them in rank order, and every rank takes the identical theta
+    decision (cudahm_shard_decide).  The host sits in the loop (launch + D2H + sync + all-gather per iteration), so
+    this pays for populations whose sweep takes much longer than that (~1e7 objects per GPU and up)."""
+    import torch
+    from paper_2105_08026_b200 import binding as B
+    from paper_2105_08026_b200 import sharded
+    c, n, inp = make_workload(args.config, args.n_objects, seed_offset=rank)   # each rank simulates its own shard
+    W, K = args.warmup, args.steps
+    stride = n + (n & 1)
+    th0 = torch.from_numpy(np.array(inp["theta0"], dtype=np.float64)).to(device)
+    if world > 1:
+        dist.broadcast(th0, 0)                                  # the initial theta must be the same everywhere
+    th0 = th0.cpu().numpy()
+    if c.model == synth.M_THINNED_SCHECHTER1D:
+        th0[2] += np.log(world)                                 # the amplitude counts the whole population
+    s = B.Sampler(c.model, n, device=device, seed=c.seed, precision=c.precision, theta_mode=B.THETA_HOST,
+                  target_accept_chi=c.target_accept_chi, target_accept_theta=c.target_accept_theta,
+                  keep_chi_moments=c.keep_chi_moments, max_trace_rows=trace_rows_needed(W + K, W, c.thin),
+                  object_offset=rank * stride, n_objects_total=world * stride)
+    s.set_data(inp["cols"])
+    if inp["consts"] is not None:
+        s.set_model_consts(inp["consts"])
+    s.set_init(th0)
+    drv = sharded.DistributedShard(s, dist, device) if world > 1 else sharded.LocalShards([s])
+    drv.run(W, W, c.thin)
+    l0 = s.get_stats()["gpu_launches"]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    torch.cuda.synchronize(device)
+    with torch.cuda.stream(s.stream):
+        e0.record(s.stream)
+        drv.run(K, W, c.thin)
+        e1.record(s.stream)
+    torch.cuda.synchronize(device)
+    barrier()
+    value, ms, _ = aggregate(e0.elapsed_time(e1), float(n) * K, dist if world > 1 else None)
+    st = s.get_stats()
+    if rank == 0:
+        rf = roofline_entry(args.config, c, n, K, W, ms, peak, peak_src, "k_sweep")
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64" if c.precision == synth.F64 else "f32 state / f64 reductions", "data": "synthetic",
+            "config": {"workload": workload_label(args.config), "n_objects_per_gpu": n, "n_objects_total": world * n,
+                       "parallelism": f"one chain sharded by object range over {world} gpu(s); all-gather of 5 doubles per rank and iteration",
+                       "theta_mode": "host", "grid": [st["grid_blocks"], st["block_threads"]]},
+            "gibbs_iters_per_s": K / (ms * 1e-3), "gpu_launches": int(st["gpu_launches"] - l0), "roofline": rf,
+            "accept": {"chi": st["chi_accepts"] / max(1, st["chi_proposals"]),
+                       "theta": st["theta_accepts"] / max(1, st["theta_proposals"])}}), flush=True)
+    s.close()
+
+
 # ----------------------------------------------------------------------------------------------------------
 def main():
     args = parse_args()
@@ -357,6 +415,11 @@ def main():
             dist.barrier()
 
     peak, peak_src = load_peaks()
+    if args.sharded:
+        run_sharded(args, device, rank, world, dist, barrier, peak, peak_src)
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
     W, K = args.warmup, args.steps
     r = time_gpu(args.config, args, device, rank, world, barrier)
     c, n = r["cfg"], r["n"]

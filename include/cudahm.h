@@ -93,6 +93,10 @@ typedef struct {
   double   prior_mean[8];        /* user prior on theta multiplying the model's default (the default */
   double   prior_isd[8];         /* is uniform and can be overridden): independent normal factors
                                     N(prior_mean[j], 1/prior_isd[j]^2) on theta[j]; prior_isd[j] = 0: no factor   */
+  /* sharding over several samplers / GPUs (cudahm_shard_sweep / cudahm_shard_decide below): this handle owns the
+   * objects [object_offset, object_offset + n_objects) of a population of n_objects_total                          */
+  int64_t  object_offset;        /* even, >= 0: global index of this handle's first object (keys its Philox streams) */
+  int64_t  n_objects_total;      /* 0 = n_objects (not sharded)                                                    */
 } cudahm_config;
 
 typedef struct {
@@ -160,6 +164,20 @@ int cudahm_set_init(cudahm_sampler* s, const void* chi0_or_null, int chi0_on_dev
  * accumulated for t > burn_in, the trace takes theta whenever t > burn_in and (t - burn_in) % thin == 0.
  * CUDAHM_E_INVALID if the trace would overflow max_trace_rows (max_trace_rows == 0 keeps no trace at all). */
 int cudahm_run(cudahm_sampler* s, int64_t n_iter, int64_t burn_in, int32_t thin);
+
+/* Sharded populations: objects are conditionally independent given theta (Eq. 2.4), so a
+ * population splits by object range over several handles (one per GPU); theta, L_theta and the theta Philox stream are
+ * replicated, and the only exchange per Gibbs iteration is the sum of the handles' totals.  THETA_HOST handles only
+ * (CUDAHM_E_UNSUPPORTED otherwise).
+ *   cudahm_shard_sweep:  one fused sweep over this handle's objects; totals[5] (host doubles) receives
+ *                        {S, Delta, Tq, n_accept, n_nonfinite} of THIS shard.  S, Delta, n_accept, n_nonfinite are to be
+ *                        summed over the shards (in a fixed order, so every rank holds the same bits); Tq (the selection
+ *                        sum of M1 / M4) is computed in full by every handle and must NOT be summed.
+ *   cudahm_shard_decide: the theta step of the iteration just swept from the GLOBAL totals, identical on every handle;
+ *                        prepares the next iteration.
+ * A handle with object_offset = 0 and n_objects_total = n_objects reproduces cudahm_run(THETA_HOST) bit for bit. */
+int cudahm_shard_sweep(cudahm_sampler* s, int64_t burn_in, int32_t thin, double* totals);
+int cudahm_shard_decide(cudahm_sampler* s, int64_t burn_in, int32_t thin, const double* totals_global);
 
 /* One iteration through the non-persistent sweep + tail kernels with per-object taps (test instrument). */
 int cudahm_debug_step(cudahm_sampler* s, int64_t burn_in, int32_t thin, cudahm_taps* taps);

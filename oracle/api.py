@@ -24,7 +24,8 @@ class Config(C.Structure):
                 ("target_accept_theta", C.c_double), ("eta_exponent", C.c_double),
                 ("init_scale_chi", C.c_double), ("freeze_theta", C.c_int32),
                 ("keep_chi_moments", C.c_int32), ("adapt_until", C.c_int64),
-                ("prior_mean", C.c_double * 8), ("prior_isd", C.c_double * 8)]
+                ("prior_mean", C.c_double * 8), ("prior_isd", C.c_double * 8),
+                ("object_offset", C.c_int64), ("n_objects_total", C.c_int64)]
 
 
 class Taps(C.Structure):
@@ -57,6 +58,8 @@ def lib():
         L.oracle_set_init.argtypes = [C.c_void_p, _dp, _dp, _dp]
         L.oracle_run.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_int32]
         L.oracle_step.argtypes = [C.c_void_p, C.c_int64, C.c_int32, C.POINTER(Taps)]
+        L.oracle_shard_sweep.argtypes = [C.c_void_p, C.c_int64, C.c_int32, _dp]
+        L.oracle_shard_decide.argtypes = [C.c_void_p, C.c_int64, C.c_int32, _dp]
         L.oracle_get_theta_trace.argtypes = [C.c_void_p, _dp, C.c_int64, C.POINTER(C.c_int64)]
         L.oracle_get_chi_moments.argtypes = [C.c_void_p, _dp, _dp, C.c_int64, C.POINTER(C.c_int64)]
         L.oracle_get_state.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp, C.POINTER(C.c_int64)]
@@ -129,7 +132,8 @@ class Sampler:
 
     def __init__(self, model, n_objects, seed=0, precision=F64, target_accept_chi=0.4,
                  target_accept_theta=0.234, eta_exponent=2.0 / 3.0, init_scale_chi=1.0,
-                 freeze_theta=False, keep_chi_moments=False, adapt_until=0, prior_mean=None, prior_sd=None):
+                 freeze_theta=False, keep_chi_moments=False, adapt_until=0, prior_mean=None, prior_sd=None,
+                 object_offset=0, n_objects_total=0):
         self.dims = model_dims(model)
         self.N = int(n_objects)
         self.p, self.dtheta = self.dims["p"], self.dims["dtheta"]
@@ -141,6 +145,7 @@ class Sampler:
             for j, (m, sd) in enumerate(zip(prior_mean, prior_sd)):
                 self.cfg.prior_mean[j] = float(m)
                 self.cfg.prior_isd[j] = 0.0 if not np.isfinite(sd) else 1.0 / float(sd)
+        self.cfg.object_offset, self.cfg.n_objects_total = int(object_offset), int(n_objects_total)
         self._h = C.c_void_p()
         _check(lib().oracle_create(C.byref(self.cfg), C.byref(self._h)), "create")
 
@@ -222,6 +227,15 @@ class Sampler:
         s = Stats()
         _check(lib().oracle_get_stats(self._h, C.byref(s)), "get_stats")
         return {k: getattr(s, k) for k, _ in Stats._fields_}
+
+    def shard_sweep(self, burn_in=0, thin=1):
+        tot = np.empty(5)
+        _check(lib().oracle_shard_sweep(self._h, burn_in, thin, _d(tot)), "shard_sweep")
+        return tot
+
+    def shard_decide(self, totals_global, burn_in=0, thin=1):
+        tot = _arr(totals_global)
+        _check(lib().oracle_shard_decide(self._h, burn_in, thin, _d(tot)), "shard_decide")
 
     def theta_only(self, theta):
         th, out = _arr(theta), C.c_double()

@@ -52,6 +52,9 @@ typedef struct {
                                    for iterations t > adapt_until (plate and theta factors frozen from then on)   */
   double   prior_mean[8];       /* user prior on theta, multiplying the model's default (uniform):   */
   double   prior_isd[8];        /* independent normal factors N(prior_mean_j, 1/prior_isd_j^2); isd_j = 0: none    */
+  /* sharded populations: this sampler owns objects [object_offset, object_offset + n_objects) of
+   * n_objects_total (0 = n_objects); object_offset even (objects draw in pairs) */
+  int64_t  object_offset, n_objects_total;
 } oracle_config;
 
 /* Per-iteration taps (all optional: a NULL member is skipped).  Per-object arrays have N entries
@@ -93,6 +96,10 @@ int  oracle_set_init(oracle_sampler* s, const double* chi0_or_null, const double
                      const double* theta_chol0_or_null);
 int  oracle_run(oracle_sampler* s, int64_t n_iter, int64_t burn_in, int32_t thin);
 int  oracle_step(oracle_sampler* s, int64_t burn_in, int32_t thin, oracle_taps* taps_or_null);
+/* the two halves of oracle_step for a sharded population: totals = {S, Delta, -, n_accept, n_nonfinite} of this shard;
+ * oracle_shard_decide takes them summed over all shards (objects are independent given theta) */
+int  oracle_shard_sweep(oracle_sampler* s, int64_t burn_in, int32_t thin, double* totals);
+int  oracle_shard_decide(oracle_sampler* s, int64_t burn_in, int32_t thin, const double* totals_global);
 int  oracle_get_theta_trace(oracle_sampler* s, double* out, int64_t cap_rows, int64_t* n_rows);
 int  oracle_get_chi_moments(oracle_sampler* s, double* mean, double* var, int64_t cap_objects,
                             int64_t* n_samples);

@@ -67,6 +67,8 @@ struct Base {
   virtual int set_data(const double* const* cols, int n_cols) = 0;
   virtual int set_init(const double* chi0, const double* theta0, const double* chol0) = 0;
   virtual int step(int64_t burn_in, int32_t thin, oracle_taps* taps) = 0;
+  virtual int sweep_part(int64_t burn_in, oracle_taps* taps, double* tot) = 0;
+  virtual int decide_part(int64_t burn_in, int32_t thin, oracle_taps* taps, const double* tot) = 0;
   virtual int get_state(double* chi, double* L, double* th, double* Lth, int64_t* tt) = 0;
   virtual int set_state(const double* chi, const double* L, const double* th, const double* Lth, int64_t tt) = 0;
   // user prior on theta ("To override this default prior ..."): independent normal factors
@@ -81,7 +83,8 @@ struct Base {
   double theta_only(const double* th) const {
     if (cfg.model == M_THINNED_SCHECHTER1D) return table.theta_only(th);
     // M4: log L = sum_i [log rho(x_i; theta) + log l_i(x_i)] - N log I(theta)   (Eq. 4.3-4.4)
-    if (cfg.model == M_BB1_FLUXNOISE1D) return -(double)cfg.n_objects * std::log(table.bb1_integral(th, consts.data()));
+    if (cfg.model == M_BB1_FLUXNOISE1D)
+      return -(double)(cfg.n_objects_total ? cfg.n_objects_total : cfg.n_objects) * std::log(table.bb1_integral(th, consts.data()));
     return 0.0;
   }
 };
@@ -149,21 +152,34 @@ struct Impl : Base {
     return ORACLE_OK;
   }
 
+  // one Gibbs iteration = the plate sweep (O1-O4, moments) followed by the theta decision (O5-O8).  The two halves are
+  // separate so that a sharded population can sum its shards' totals in between (oracle_shard_sweep / _decide).
+  double zth_[8] = {0}, thp_[8] = {0}, eta_ = 0.0;
+
   int step(int64_t burn_in, int32_t thin, oracle_taps* taps) override {
+    double tot[5];
+    int rc = sweep_part(burn_in, taps, tot);
+    if (rc != ORACLE_OK) return rc;
+    return decide_part(burn_in, thin, taps, tot);
+  }
+
+  int sweep_part(int64_t burn_in, oracle_taps* taps, double* tot) override {
     if (!have_init) return ORACLE_E_STATE;
     const int64_t N = cfg.n_objects;
     const int p = dims.p, dt = dims.dtheta, nc = dims.n_cols, nt = ntri(p);
     const int model = cfg.model;
-    const double ninf = -std::numeric_limits<double>::infinity();
 
     // O1: this is RAM iteration n = t + 1 (X_1, S_1 are the initial values)
     const uint32_t tcur = (uint32_t)(t + 1);
     const double n_ram = (double)(t + 1) + 1.0;
     double eta = std::pow(n_ram, -cfg.eta_exponent);                // eta_n = n^(-2/3)
     if (cfg.adapt_until > 0 && (t + 1) > cfg.adapt_until) eta = 0.0; // adaptation frozen: S_n = S_{n-1}
+    eta_ = eta;
 
     // O2: theta proposal theta' = theta + L_theta z  (drawn before the sweep: it does not depend on chi)
-    double zth[8] = {0}, thp[8] = {0};
+    double* zth = zth_;
+    double* thp = thp_;
+    for (int r = 0; r < 8; ++r) { zth[r] = 0.0; thp[r] = 0.0; }
     if (!cfg.freeze_theta) {
       normals_f64(cfg.seed, ORACLE_KIND_THETA, 0, tcur, dt, zth);
       for (int r = 0; r < dt; ++r) {
@@ -178,6 +194,7 @@ struct Impl : Base {
     for (int r = 0; r < dt; ++r) thT[r] = (T)theta[r];
     const T* cT = consts_T.empty() ? nullptr : consts_T.data();
     const double* cD = consts.empty() ? nullptr : consts.data();
+    int64_t n_acc = 0, n_nan = 0;
 
     // O3/O4: plate sweep in index order
     long double S = 0.0L, Delta = 0.0L;
@@ -188,12 +205,12 @@ struct Impl : Base {
       for (int c = 0; c < nc; ++c) d[c] = data[(size_t)c * N + i];
       if (sizeof(T) == 8) {
         double zz[8] = {}, uu = 0;
-        plate_draws_f64(cfg.seed, (uint64_t)i, tcur, p, zz, &uu);
+        plate_draws_f64(cfg.seed, (uint64_t)(cfg.object_offset + i), tcur, p, zz, &uu);
         for (int j = 0; j < p; ++j) z[j] = (T)zz[j];
         u = (T)uu;
       } else {
         float zf[2] = {0.0f, 0.0f}, uf;
-        plate_draws_f32(cfg.seed, (uint64_t)i, tcur, p, zf, &uf);
+        plate_draws_f32(cfg.seed, (uint64_t)(cfg.object_offset + i), tcur, p, zf, &uf);
         z[0] = (T)zf[0]; z[1] = (T)zf[1]; u = (T)uf;
         if (p == 1) z[1] = T(0);
       }
@@ -208,12 +225,11 @@ struct Impl : Base {
       const T pp = loglik<T>(model, y, d, cT) + logpop<T>(model, y, d, thT, cT);
       const T diff = pp - pc;
       T la;
-      if (std::isnan(diff)) { la = -std::numeric_limits<T>::infinity(); stats.nonfinite++; }
+      if (std::isnan(diff)) { la = -std::numeric_limits<T>::infinity(); n_nan++; }
       else la = std::min(T(0), diff);
       const T alpha = std::exp(la);
       const bool acc = (u < alpha);
-      if (acc) { for (int j = 0; j < p; ++j) x[j] = y[j]; stats.chi_accepts++; }
-      stats.chi_proposals++;
+      if (acc) { for (int j = 0; j < p; ++j) x[j] = y[j]; n_acc++; }
       // step 3: S_n = chol(S (I + eta (alpha - alpha_*) U U^T/||U||^2) S^T)
       T lnew[36];
       ram_update<T>(p, l, z, (T)eta * (alpha - (T)cfg.target_accept_chi), lnew);
@@ -224,7 +240,7 @@ struct Impl : Base {
       for (int j = 0; j < p; ++j) xd[j] = (double)x[j];
       for (int c = 0; c < nc; ++c) dd[c] = (double)d[c];
       const double a = logpop<double>(model, xd, dd, theta.data(), cD);
-      const double b = logpop<double>(model, xd, dd, thp, cD);
+      const double b = logpop<double>(model, xd, dd, thp_, cD);
       S += (long double)a;
       Delta += (long double)(b - a);
       if (taps) {
@@ -250,6 +266,24 @@ struct Impl : Base {
       }
     }
     if (cfg.keep_chi_moments && (t + 1) > burn_in) { mom_count++; stats.moment_samples = mom_count; }
+    tot[0] = (double)S; tot[1] = (double)Delta; tot[2] = 0.0; tot[3] = (double)n_acc; tot[4] = (double)n_nan;
+    return ORACLE_OK;
+  }
+
+  // tot = {S, Delta, -, n_accept, n_nonfinite} summed over the whole population (all shards)
+  int decide_part(int64_t burn_in, int32_t thin, oracle_taps* taps, const double* tot) override {
+    if (!have_init) return ORACLE_E_STATE;
+    const int dt = dims.dtheta;
+    const int model = cfg.model;
+    const double ninf = -std::numeric_limits<double>::infinity();
+    const uint32_t tcur = (uint32_t)(t + 1);
+    const double eta = eta_;
+    const double* zth = zth_;
+    const double* thp = thp_;
+    const double S = tot[0], Delta = tot[1];
+    stats.chi_accepts += (int64_t)tot[3];
+    stats.nonfinite += (int64_t)tot[4];
+    stats.chi_proposals += cfg.n_objects_total ? cfg.n_objects_total : cfg.n_objects;
 
     // O5-O7: theta decision and RAM update of L_theta
     double T_cur = 0, T_prop = 0, lp_cur = 0, lp_prop = 0, log_r = 0, alpha_th = 0, u_th = 0;
@@ -315,6 +349,7 @@ int oracle_create(const oracle_config* cfg, oracle_sampler** out) {
   if (!model_dims(cfg->model, &d) || cfg->n_objects < 0) return ORACLE_E_INVALID;
   if (!(cfg->target_accept_chi > 0 && cfg->target_accept_chi < 1)) return ORACLE_E_INVALID;
   if (!(cfg->target_accept_theta > 0 && cfg->target_accept_theta < 1)) return ORACLE_E_INVALID;
+  if (cfg->object_offset < 0 || (cfg->object_offset & 1) || cfg->n_objects_total < 0) return ORACLE_E_INVALID;
   std::unique_ptr<Base> b;
   if (cfg->precision == ORACLE_F64) b.reset(new Impl<double>());
   else if (cfg->precision == ORACLE_F32_STATE_F64_REDUCE && d.p <= 2) b.reset(new Impl<float>());   // fp32 draws: p <= 2
@@ -359,6 +394,15 @@ int oracle_set_init(oracle_sampler* s, const double* chi0, const double* theta0,
 int oracle_step(oracle_sampler* s, int64_t burn_in, int32_t thin, oracle_taps* taps) {
   if (!s || thin < 1 || burn_in < 0) return ORACLE_E_INVALID;
   return s->impl->step(burn_in, thin, taps);
+}
+
+int oracle_shard_sweep(oracle_sampler* s, int64_t burn_in, int32_t thin, double* totals) {
+  if (!s || !totals || thin < 1 || burn_in < 0) return ORACLE_E_INVALID;
+  return s->impl->sweep_part(burn_in, nullptr, totals);
+}
+int oracle_shard_decide(oracle_sampler* s, int64_t burn_in, int32_t thin, const double* totals_global) {
+  if (!s || !totals_global || thin < 1 || burn_in < 0) return ORACLE_E_INVALID;
+  return s->impl->decide_part(burn_in, thin, nullptr, totals_global);
 }
 
 int oracle_run(oracle_sampler* s, int64_t n_iter, int64_t burn_in, int32_t thin) {

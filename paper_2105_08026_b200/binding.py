@@ -22,7 +22,7 @@ FLOOR_LAUNCH, FLOOR_GRAPH, FLOOR_GRID_BARRIER, FLOOR_HOST_SYNC = 0, 1, 2, 3
 EXPORTS = ["cudahm_model_dims", "cudahm_workspace_bytes", "cudahm_create", "cudahm_destroy", "cudahm_set_data",
            "cudahm_set_model_consts", "cudahm_set_init", "cudahm_run", "cudahm_debug_step",
            "cudahm_get_theta_trace", "cudahm_get_chi_moments", "cudahm_get_stats", "cudahm_get_state",
-           "cudahm_set_state", "cudahm_sync", "cudahm_last_error", "cudahm_probe_floor", "cudahm_probe_fma_peak"]
+           "cudahm_set_state", "cudahm_sync", "cudahm_last_error", "cudahm_shard_sweep", "cudahm_shard_decide", "cudahm_probe_floor", "cudahm_probe_fma_peak"]
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int32)
@@ -36,7 +36,8 @@ class Config(C.Structure):
                 ("eta_exponent", C.c_double), ("init_scale_chi", C.c_double), ("keep_chi_moments", C.c_int32),
                 ("block_threads", C.c_int32), ("blocks_per_sm", C.c_int32), ("flags", C.c_int32),
                 ("max_trace_rows", C.c_int64), ("adapt_until", C.c_int64),
-                ("prior_mean", C.c_double * 8), ("prior_isd", C.c_double * 8)]
+                ("prior_mean", C.c_double * 8), ("prior_isd", C.c_double * 8),
+                ("object_offset", C.c_int64), ("n_objects_total", C.c_int64)]
 
 
 class Stats(C.Structure):
@@ -84,6 +85,8 @@ def load():
     L.cudahm_get_stats.argtypes = [vp, C.POINTER(Stats)]
     L.cudahm_get_state.argtypes = [vp, vp, vp, _dp, _dp, C.POINTER(C.c_int64)]
     L.cudahm_set_state.argtypes = [vp, vp, vp, _dp, _dp, C.c_int64]
+    L.cudahm_shard_sweep.argtypes = [vp, C.c_int64, C.c_int32, _dp]
+    L.cudahm_shard_decide.argtypes = [vp, C.c_int64, C.c_int32, _dp]
     L.cudahm_sync.argtypes = [vp]
     L.cudahm_last_error.argtypes = [vp]
     L.cudahm_last_error.restype = C.c_char_p
@@ -114,7 +117,7 @@ def model_dims(model):
 def make_config(model, n_objects, seed=0, precision=F64, theta_mode=THETA_DEVICE_TAIL, target_accept_chi=0.4,
                 target_accept_theta=0.234, eta_exponent=2.0 / 3.0, init_scale_chi=1.0, freeze_theta=False,
                 keep_chi_moments=False, max_trace_rows=0, block_threads=0, blocks_per_sm=0, flags=0, adapt_until=0,
-                prior_mean=None, prior_sd=None):
+                prior_mean=None, prior_sd=None, object_offset=0, n_objects_total=0):
     d = model_dims(model)
     cfg = Config(C.sizeof(Config), model, precision, theta_mode, int(n_objects), d["p"], d["dtheta"], d["n_cols"],
                   int(freeze_theta), seed, target_accept_chi, target_accept_theta, eta_exponent, init_scale_chi,
@@ -123,6 +126,7 @@ def make_config(model, n_objects, seed=0, precision=F64, theta_mode=THETA_DEVICE
         for j, (m, sd) in enumerate(zip(prior_mean, prior_sd)):
             cfg.prior_mean[j] = float(m)
             cfg.prior_isd[j] = 0.0 if not np.isfinite(sd) else 1.0 / float(sd)
+    cfg.object_offset, cfg.n_objects_total = int(object_offset), int(n_objects_total)
     return cfg
 
 
@@ -211,6 +215,19 @@ class Sampler:
     def sync(self):
         with self._dev():
             self._ck(self.lib.cudahm_sync(self._h))
+
+    def shard_sweep(self, burn_in=0, thin=1):
+        """One sweep over this handle's objects: {S, Delta, Tq, n_accept, n_nonfinite} of this shard (THETA_HOST)."""
+        tot = np.empty(5)
+        with self._dev():
+            self._ck(self.lib.cudahm_shard_sweep(self._h, burn_in, thin, _d(tot)))
+        return tot
+
+    def shard_decide(self, totals_global, burn_in=0, thin=1):
+        """The theta step of the iteration just swept, from the totals summed over all shards."""
+        tot = np.ascontiguousarray(totals_global, dtype=np.float64)
+        with self._dev():
+            self._ck(self.lib.cudahm_shard_decide(self._h, burn_in, thin, _d(tot)))
 
     def debug_step(self, burn_in=0, thin=1):
         N, p = self.N, self.p

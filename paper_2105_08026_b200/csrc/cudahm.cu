@@ -157,6 +157,8 @@ bool valid_config(const cudahm_config* c, int* p, int* dt, int* nc, int* nk) {
   if (c->block_threads != 0 && c->block_threads != 256 && c->block_threads != 512 && c->block_threads != 1024)
     return false;
   if (c->blocks_per_sm < 0 || c->adapt_until < 0) return false;
+  if (c->object_offset < 0 || (c->object_offset & 1) || c->n_objects_total < 0) return false;
+  if (c->n_objects_total != 0 && c->object_offset + c->n_objects > c->n_objects_total) return false;
   for (int j = 0; j < 8; ++j)
     if (!(c->prior_isd[j] >= 0.0) || !std::isfinite(c->prior_isd[j]) || !std::isfinite(c->prior_mean[j])) return false;
   return true;
@@ -293,8 +295,9 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
   P.astar_chi = cfg->target_accept_chi;
   P.max_blocks = MAX_BLOCKS;
   P.tail = TailCfg{cfg->model, dt, cfg->freeze_theta ? 1 : 0, cfg->keep_chi_moments ? 1 : 0, cfg->seed,
-                   cfg->target_accept_theta, cfg->eta_exponent, 0, cfg->max_trace_rows, 1, 0, (double)cfg->n_objects,
-                   cfg->adapt_until, {}, {}};
+                   cfg->target_accept_theta, cfg->eta_exponent, 0, cfg->max_trace_rows, 1, 0,
+                   (double)(cfg->n_objects_total ? cfg->n_objects_total : cfg->n_objects), cfg->adapt_until, {}, {}};
+  P.obj_offset = cfg->object_offset;
   for (int j = 0; j < MAXD; ++j) { P.tail.prior_mean[j] = cfg->prior_mean[j]; P.tail.prior_isd[j] = cfg->prior_isd[j]; }
   P.taps = DevTaps{};
 
@@ -611,28 +614,38 @@ int run_graph(cudahm_sampler* s, long long n_iter) {
   return CUDAHM_OK;
 }
 
-// THETA_HOST (the paper's split): sweep + reduction on the device, theta step in host C++
-int run_host(cudahm_sampler* s, long long n_iter) {
+// THETA_HOST (the paper's split): sweep + reduction on the device, theta step in host C++.
+// Two halves, so that a sharded population can put its exchange between them (cudahm_shard_sweep / _decide).
+int host_sweep(cudahm_sampler* s) {          // -> s->h_totals = {S, Delta, Tq, n_accept, n_nonfinite} of this handle
+  Params P = s->P;
+  void* a1[] = {&P};
+  int rc = launch(s, s->ks.sweep, s->sweep_grid, s->sweep_block, a1, false);
+  if (rc) return rc;
+  int nb = s->sweep_grid, flags = TAIL_REDUCE;
+  void* a2[] = {&P, &nb, &flags};
+  rc = launch(s, (const void*)k_tail, 1, TAIL_THREADS, a2, false);
+  if (rc) return rc;
+  CU_TRY(s, cudaMemcpyAsync(s->h_totals, s->P.totals, NPART * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+  CU_TRY(s, cudaStreamSynchronize(s->stream));
+  return CUDAHM_OK;
+}
+int host_decide(cudahm_sampler* s, const double* totals) {
   Iter& it = *s->h_iter;
+  tail_decide(it, s->P.tail, totals);
+  if (it.trace_write)
+    CU_TRY(s, cudaMemcpyAsync(s->P.trace + (it.trace_rows - 1) * s->dtheta, it.theta, s->dtheta * sizeof(double),
+                              cudaMemcpyHostToDevice, s->stream));
+  prepare_iteration(it, s->P.tail, it.t + 1);
+  CU_TRY(s, cudaMemcpyAsync(s->P.iter, s->h_iter, sizeof(Iter), cudaMemcpyHostToDevice, s->stream));
+  // h_iter is pinned and reused next iteration: the copy must have left before we overwrite it
+  CU_TRY(s, cudaStreamSynchronize(s->stream));
+  return CUDAHM_OK;
+}
+int run_host(cudahm_sampler* s, long long n_iter) {
   for (long long k = 0; k < n_iter; ++k) {
-    Params P = s->P;
-    void* a1[] = {&P};
-    int rc = launch(s, s->ks.sweep, s->sweep_grid, s->sweep_block, a1, false);
+    int rc = host_sweep(s);
+    if (!rc) rc = host_decide(s, s->h_totals);
     if (rc) return rc;
-    int nb = s->sweep_grid, flags = TAIL_REDUCE;
-    void* a2[] = {&P, &nb, &flags};
-    rc = launch(s, (const void*)k_tail, 1, TAIL_THREADS, a2, false);
-    if (rc) return rc;
-    CU_TRY(s, cudaMemcpyAsync(s->h_totals, s->P.totals, NPART * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
-    CU_TRY(s, cudaStreamSynchronize(s->stream));
-    tail_decide(it, s->P.tail, s->h_totals);
-    if (it.trace_write)
-      CU_TRY(s, cudaMemcpyAsync(s->P.trace + (it.trace_rows - 1) * s->dtheta, it.theta, s->dtheta * sizeof(double),
-                                cudaMemcpyHostToDevice, s->stream));
-    prepare_iteration(it, s->P.tail, it.t + 1);
-    CU_TRY(s, cudaMemcpyAsync(s->P.iter, s->h_iter, sizeof(Iter), cudaMemcpyHostToDevice, s->stream));
-    // h_iter is pinned and reused next iteration: the copy must have left before we overwrite it
-    CU_TRY(s, cudaStreamSynchronize(s->stream));
   }
   return CUDAHM_OK;
 }
@@ -667,6 +680,40 @@ extern "C" int cudahm_run(cudahm_sampler* s, int64_t n_iter, int64_t burn_in, in
   CU_TRY(s, cudaEventRecord(s->ev1, s->stream));
   s->timed = true;
   s->t_done += n_iter;
+  return CUDAHM_OK;
+}
+
+// Sharded populations: the two halves of one THETA_HOST iteration, with the caller's exchange in between.
+namespace {
+int shard_check(cudahm_sampler* s, int64_t burn_in, int32_t thin, const void* p) {
+  if (!s || !p) return fail(s, CUDAHM_E_INVALID, "shard: NULL argument");
+  if (!s->have_init) return fail(s, CUDAHM_E_STATE, "shard call before set_init");
+  if (s->cfg.theta_mode != CUDAHM_THETA_HOST) return fail(s, CUDAHM_E_UNSUPPORTED, "sharded stepping needs theta_mode = CUDAHM_THETA_HOST");
+  if (burn_in < 0 || thin < 1) return fail(s, CUDAHM_E_INVALID, "shard: bad burn_in/thin");
+  if (s->t_done + 1 >= 0xffffffffLL) return fail(s, CUDAHM_E_INVALID, "iteration index exceeds the 32-bit stream counter");
+  s->P.tail.burn_in = burn_in; s->P.tail.thin = thin;
+  return fetch_iter(s);
+}
+}  // namespace
+
+extern "C" int cudahm_shard_sweep(cudahm_sampler* s, int64_t burn_in, int32_t thin, double* totals) {
+  int rc = shard_check(s, burn_in, thin, totals);
+  if (rc) return rc;
+  rc = host_sweep(s);
+  if (rc) return rc;
+  for (int q = 0; q < NPART; ++q) totals[q] = s->h_totals[q];
+  return CUDAHM_OK;
+}
+
+extern "C" int cudahm_shard_decide(cudahm_sampler* s, int64_t burn_in, int32_t thin, const double* totals_global) {
+  int rc = shard_check(s, burn_in, thin, totals_global);
+  if (rc) return rc;
+  const long long t = s->h_iter->t;
+  if (s->cfg.max_trace_rows > 0 && t > burn_in && ((t - burn_in) % thin) == 0 && s->h_iter->trace_rows + 1 > s->cfg.max_trace_rows)
+    return fail(s, CUDAHM_E_INVALID, "theta trace is full");
+  rc = host_decide(s, totals_global);
+  if (rc) return rc;
+  s->t_done += 1;
   return CUDAHM_OK;
 }
 

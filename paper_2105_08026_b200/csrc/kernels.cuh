@@ -37,6 +37,7 @@ struct Params {
   double mc[MC_N];               // model constants (MC_* / MB_* / MN_*)
   double astar_chi;
   int max_blocks, pad_;
+  long long obj_offset;          // global index of object 0 (sharded populations; even): keys the plate Philox streams
   TailCfg tail;
   DevTaps taps;
 };
@@ -172,7 +173,7 @@ __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c
   constexpr int ZD = p < 2 ? 2 : p;
   T zz[VEC][ZD], csv[VEC], snv[VEC], uu[VEC];
 #pragma unroll
-  for (int v = 0; v < VEC; v += 2) pair_draws<p>(P.tail.seed, base + v, c.t, &zz[v], &csv[v], &snv[v], &uu[v]);
+  for (int v = 0; v < VEC; v += 2) pair_draws<p>(P.tail.seed, P.obj_offset + base + v, c.t, &zz[v], &csv[v], &snv[v], &uu[v]);
 #pragma unroll
   for (int v = 0; v < VEC; ++v) {
     const long long i = base + v;

@@ -134,6 +134,55 @@ def test_user_prior_and_adaptation_freeze_match_oracle(model, astar, n, flags, m
     compare_theta_step(to, tg, what="hooks")
 
 
+@pytest.mark.parametrize("model,astar,n", [(B.M_THINNED_SCHECHTER1D, 0.44, 4001), (B.M_BINORMAL2D, 0.234, 3000),
+                                             (B.M_BB1_FLUXNOISE1D, 0.44, 2500)], ids=["M1", "M2", "M4"])
+def test_sharded_population_matches_oracle(model, astar, n):
+    """the population split by object range over THREE handles (here on one GPU, launched one after the
+    other), theta replicated, the shards' totals summed in rank order between the sweep and the theta step
+    (cudahm_shard_sweep / cudahm_shard_decide) -- against the UNSHARDED oracle chain."""
+    from paper_2105_08026_b200 import sharded
+    iters, burn, thin = 100, 20, 5
+    orc, _, inp = make_pair(model, n, seed=81 + model, astar=astar, keep_moments=True, theta_mode=B.THETA_HOST)
+    orc.run(iters, burn, thin)
+    parts = []
+    for lo, hi in sharded.shard_ranges(n, 3):
+        g = B.Sampler(model, hi - lo, seed=81 + model, theta_mode=B.THETA_HOST, target_accept_chi=astar, keep_chi_moments=True,
+                      max_trace_rows=(iters - burn) // thin, object_offset=lo, n_objects_total=n)
+        g.set_data([c[lo:hi] for c in inp["cols"]])
+        if inp["consts"] is not None:
+            g.set_model_consts(inp["consts"])
+        g.set_init(inp["theta0"])
+        parts.append(g)
+    sharded.LocalShards(parts).run(iters, burn, thin)
+    for g in parts:
+        np.testing.assert_allclose(g.get_theta_trace(), orc.get_theta_trace(), rtol=1e-8, atol=1e-8)
+        assert np.array_equal(g.get_theta_trace(), parts[0].get_theta_trace())
+    so = orc.get_state()
+    np.testing.assert_allclose(np.concatenate([g.get_state()["chi"] for g in parts], axis=1), so["chi"], rtol=1e-9, atol=1e-9)
+    np.testing.assert_allclose(np.concatenate([g.get_state()["L"] for g in parts], axis=1), so["L"], rtol=1e-9)
+    np.testing.assert_allclose(np.concatenate([g.get_chi_moments()[0] for g in parts], axis=1), orc.get_chi_moments()[0],
+                               rtol=1e-10, atol=1e-10)
+    st, sto = parts[0].get_stats(), orc.get_stats()
+    assert st["chi_accepts"] == sto["chi_accepts"] and st["theta_accepts"] == sto["theta_accepts"] and st["iterations"] == iters
+
+
+def test_single_shard_is_the_host_mode_run_bit_for_bit():
+    from paper_2105_08026_b200 import sharded
+    _, a, inp = make_pair(B.M_THINNED_SCHECHTER1D, 3000, seed=9, theta_mode=B.THETA_HOST, max_trace_rows=60, want_oracle=False)
+    _, b, _ = make_pair(B.M_THINNED_SCHECHTER1D, 3000, seed=9, theta_mode=B.THETA_HOST, max_trace_rows=60, want_oracle=False,
+                        inputs=inp)
+    a.run(60, 0, 1, sync=True)
+    sharded.LocalShards([b]).run(60, 0, 1)
+    sa, sb = a.get_state(), b.get_state()
+    for k in ("chi", "L", "theta", "L_theta"):
+        assert np.array_equal(sa[k], sb[k]), k
+    assert np.array_equal(a.get_theta_trace(), b.get_theta_trace())
+    # device-tail handles refuse the call: sharded stepping is defined for THETA_HOST
+    _, c, _ = make_pair(B.M_NORMAL1D, 100, seed=1, want_oracle=False)
+    with pytest.raises(B.CudahmError):
+        c.shard_sweep()
+
+
 def test_theta_modes_agree():
     """Same grid, same thread->object map, same reduction order in the three streaming drivers.  GRAPH and the
     plain-load streaming DEVICE_TAIL kernel run the theta step with the same device code => identical bits.  HOST
