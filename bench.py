@@ -375,6 +375,7 @@ def run_sharded(args, device, rank, world, dist, barrier, peak, peak_src):
     st = s.get_stats()
     if rank == 0:
         rf = roofline_entry(args.config, c, n, K, W, ms, peak, peak_src, "k_sweep")
+        rf.update(launches_timed=K, iterations_per_launch=1, alg_bytes_per_launch=rf["alg_bytes_per_iter"], traffic=None)
         print(json.dumps({
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
