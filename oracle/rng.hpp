@@ -48,6 +48,10 @@ inline double u01_f64(uint32_t wa, uint32_t wb) {
   const uint64_t k = ((uint64_t)(wa >> 6) << 26) | (uint64_t)(wb >> 6);
   return ((double)k + 0.5) * 0x1.0p-52;
 }
+// 32 random bits + 1/2, scaled by 2^-32: a dyadic rational in [2^-33, 1-2^-33], exact in fp64.
+inline double u01_32(uint32_t w) {
+  return ((double)w + 0.5) * 0x1.0p-32;
+}
 // 23 random bits + 1/2, scaled by 2^-23: exact in fp32, never 0 or 1.
 inline float u01_f32(uint32_t w) {
   return ((float)(w >> 9) + 0.5f) * 0x1.0p-23f;
@@ -88,10 +92,12 @@ inline void draws_f32(uint64_t seed, int kind, uint64_t obj, uint32_t t, float z
 // ---- plate-level draws of object i at iteration t --------------------------------
 // Objects are taken in PAIRS m = i >> 1, h = i & 1, so that one Philox call and one Box-Muller evaluation
 // serve two objects (both branches of Box-Muller are independent N(0,1) variates; nothing is discarded).
-//   fp64  accept uniform: draw 0 of PAIR m -- words (w0,w1) for h = 0, (w2,w3) for h = 1.
-//         p = 1 normal:   draw 1 of PAIR m -- u1 from (w0,w1), u2 from (w2,w3), radius sqrt(-2 ln u1);
-//                         z = radius cos(2 pi u2) for h = 0, radius sin(2 pi u2) for h = 1.
-//         p >= 2 normals: per OBJECT, draws 1+k of object i exactly as normals_f64.
+//   fp64  p = 1: ONE call per pair, draw 0 of PAIR m, every word a 32-bit uniform u = (w + 1/2) 2^-32 (exact in fp64, in
+//                [2^-33, 1 - 2^-33]): w0 -> u1 (radius sqrt(-2 ln u1)), w1 -> u2 (angle), z = radius cos(2 pi u2) for
+//                h = 0, radius sin(2 pi u2) for h = 1; accept uniform from w2 (h = 0) / w3 (h = 1).  (The proposal stays
+//                symmetric -- all a Metropolis step needs -- with its radius capped at sqrt(66 ln 2) = 6.76.)
+//         p >= 2: accept uniform (52 bits): draw 0 of PAIR m -- words (w0,w1) for h = 0, (w2,w3) for h = 1;
+//                normals: per OBJECT, draws 1+k of object i exactly as normals_f64.
 //   fp32  p = 1: ONE call per pair, draw 0 of PAIR m: w0 -> u1, w1 -> u2, z = cos / sin branch for h = 0 / 1,
 //                accept uniform from w2 (h = 0) / w3 (h = 1).
 //         p = 2: per OBJECT as draws_f32.
@@ -100,14 +106,14 @@ inline void plate_draws_f64(uint64_t seed, uint64_t i, uint32_t t, int p, double
   const uint64_t m = i >> 1;
   const int h = (int)(i & 1);
   const Words a = stream_words(seed, 0 /* PLATE */, m, t, 0u);
-  *u = h ? u01_f64(a.w[2], a.w[3]) : u01_f64(a.w[0], a.w[1]);
   if (p == 1) {
-    const Words b = stream_words(seed, 0, m, t, 1u);
-    const double u1 = u01_f64(b.w[0], b.w[1]);
-    const double u2 = u01_f64(b.w[2], b.w[3]);
+    const double u1 = u01_32(a.w[0]);
+    const double u2 = u01_32(a.w[1]);
     const double rad = std::sqrt(-2.0 * std::log(u1));
     z[0] = h ? rad * std::sin(two_pi * u2) : rad * std::cos(two_pi * u2);
+    *u = u01_32(h ? a.w[3] : a.w[2]);
   } else {
+    *u = h ? u01_f64(a.w[2], a.w[3]) : u01_f64(a.w[0], a.w[1]);
     normals_f64(seed, 0, i, t, p, z);
   }
 }

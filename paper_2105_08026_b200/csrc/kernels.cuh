@@ -68,9 +68,10 @@ __device__ __forceinline__ float hm_sqrt_pos(float x) { return x * rsqrtf(x); }
 
 // Plate-level draws.  Objects draw in PAIRS m = i >> 1 so that one Philox call and one
 // Box-Muller evaluation serve two objects (both Box-Muller branches are independent N(0,1); nothing is wasted):
-//   fp64  accept uniforms: draw 0 of pair m -- (x,y) for the even object, (z,w) for the odd one;
-//         p = 1 normals:   draw 1 of pair m -- cos branch for the even object, sin branch for the odd one;
-//         p = 2 normals:   per object, draw 1 of object i; z = rad*(cs, sn), unit vector (cs, sn).
+//   fp64  p = 1: ONE call per pair (draw 0 of pair m), every word a 32-bit uniform (w + 1/2) 2^-32: x -> u1, y -> u2, cos /
+//                sin branch, accept uniforms z / w.  (Half the Philox work of 52-bit uniforms; the proposal stays symmetric.)
+//         p >= 2: accept uniforms (52 bits): draw 0 of pair m -- (x,y) for the even object, (z,w) for the odd one;
+//                normals: per object, draw 1 of object i; z = rad*(cs, sn), unit vector (cs, sn).
 //   fp32  p = 1: one call per pair (draw 0 of pair m): x -> u1, y -> u2, cos / sin branch, accept uniforms z / w.
 // i0 is the even object of the pair.  z[h][k]: normal k of object i0 + h.
 //         p = 3 normals:   per object, draws 1 and 2 of object i: (z0, z1) and (z2, -).
@@ -79,10 +80,9 @@ __device__ __forceinline__ void pair_draws(unsigned long long seed, long long i0
                                            double* sn, double* u) {
   const uint64_t m = (uint64_t)i0 >> 1;
   const U4 a = stream(seed, KIND_PLATE, m, t, 0u);
-  u[0] = u01(a.x, a.y); u[1] = u01(a.z, a.w);
   if (P == 1) {
-    const U4 b = stream(seed, KIND_PLATE, m, t, 1u);
-    const double u1 = u01(b.x, b.y), u2 = u01(b.z, b.w);
+    const double u1 = u01_32(a.x), u2 = u01_32(a.y);
+    u[0] = u01_32(a.z); u[1] = u01_32(a.w);
     const double rad = hm_sqrt_fast(-2.0 * hm_log_unit(u1));
     double s_, c_;
     sincospi(2.0 * u2, &s_, &c_);
@@ -90,6 +90,7 @@ __device__ __forceinline__ void pair_draws(unsigned long long seed, long long i0
     z[0][1] = 0.0; z[1][1] = 0.0;
     cs[0] = cs[1] = 0.0; sn[0] = sn[1] = 0.0;      // the unit vector is not needed for p = 1
   } else {
+    u[0] = u01(a.x, a.y); u[1] = u01(a.z, a.w);
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
       const U4 b = stream(seed, KIND_PLATE, (uint64_t)(i0 + h), t, 1u);

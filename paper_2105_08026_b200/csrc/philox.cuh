@@ -56,6 +56,19 @@ HM_HD double u01(uint32_t a, uint32_t b) {
 #endif
   return d - 0x1.fffffffffffffp-1;
 }
+// (32 random bits w + 1/2) * 2^-32: exact, in [2^-33, 1 - 2^-33].  w is dropped into the top of the mantissa of a double in
+// [1, 2) and (1 - 2^-33) is subtracted: both steps exact, no int -> fp conversion.
+HM_HD double u01_32(uint32_t w) {
+  const uint32_t hi = 0x3FF00000u | (w >> 12), lo = w << 20;
+#ifdef __CUDA_ARCH__
+  const double d = __hiloint2double((int)hi, (int)lo);
+#else
+  const uint64_t bits = ((uint64_t)hi << 32) | lo;
+  double d;
+  __builtin_memcpy(&d, &bits, sizeof d);
+#endif
+  return d - 0x1.ffffffffp-1;
+}
 // (23 random bits k + 1/2) * 2^-23: exact in fp32; k goes into the mantissa of a float in [1, 2), then 1 - 2^-24 is
 // subtracted (both steps exact, no int -> fp conversion)
 HM_HD float u01f(uint32_t a) {

@@ -89,3 +89,12 @@ def test_u01_is_exact(binary):
     want = (k.astype(np.float64) + 0.5) * 2.0 ** -52   # k < 2^52: the conversion and both operations are exact
     assert np.array_equal(got, want)
     assert got.min() == 2.0 ** -53 and got.max() == 1 - 2.0 ** -53
+
+
+def test_u01_32_is_exact(binary):
+    rng = np.random.default_rng(6)
+    w = rng.integers(0, 2 ** 32, 5000, dtype=np.uint64)
+    w[:3] = [0, 2 ** 32 - 1, 2 ** 31]
+    got = run(binary, "u32", w.view(np.float64))
+    assert np.array_equal(got, (w.astype(np.float64) + 0.5) * 2.0 ** -32)
+    assert got.min() == 2.0 ** -33 and got.max() == 1 - 2.0 ** -33

@@ -132,24 +132,25 @@ def _u52(wa, wb):
 
 
 def test_plate_draws_f64_are_the_documented_function_of_the_pair_words():
-    """objects draw in pairs m = i >> 1.  Accept uniform: draw 0 of pair m, words (w0,w1) for
-    the even object and (w2,w3) for the odd one.  p = 1 normal: draw 1 of pair m, cos branch for the even object,
-    sin branch for the odd one.  p = 2 normals: per object, draws 1.. of object i.  Evaluated with mpmath."""
+    """objects draw in pairs m = i >> 1.  p = 1: ONE call per pair (draw 0 of pair m), every word a
+    32-bit uniform (w + 1/2) 2^-32: w0 -> u1, w1 -> u2, cos branch for the even object, sin branch for the odd one,
+    accept uniform from w2 / w3.  p >= 2: 52-bit accept uniform from draw 0 of pair m, words (w0,w1) for the even object
+    and (w2,w3) for the odd one; normals per object, draws 1.. of object i.  Evaluated with mpmath."""
     import mpmath as mp
     mp.mp.dps = 40
     for i, t in ((0, 1), (1, 1), (17, 9), (299_998, 10_000), (299_999, 10_000), (2 ** 33 + 5, 3)):
         m, h = i >> 1, i & 1
         a = O.stream_words(9, O.KIND_PLATE, m, t, 0)
-        b = O.stream_words(9, O.KIND_PLATE, m, t, 1)
         z, u = O.plate_draws_f64(9, i, t, 1)
-        assert u == float(_u52(a[2], a[3]) if h else _u52(a[0], a[1]))
-        u1, u2 = _u52(b[0], b[1]), _u52(b[2], b[3])
+        u32 = lambda w: mp.mpf(2 * w + 1) / mp.mpf(2) ** 33
+        assert u == float(u32(a[3] if h else a[2])) and 2.0 ** -33 <= u <= 1 - 2.0 ** -33
+        u1, u2 = u32(a[0]), u32(a[1])
         r = mp.sqrt(-2 * mp.log(u1))
         want = r * (mp.sin(2 * mp.pi * u2) if h else mp.cos(2 * mp.pi * u2))
         assert abs(z[0] - float(want)) < 1e-14 * max(1.0, abs(z[0]))
         # p = 2: uniform as above, normals are the per-object Box-Muller pair
         z2, u_2 = O.plate_draws_f64(9, i, t, 2)
-        assert u_2 == u
+        assert u_2 == float(_u52(a[2], a[3]) if h else _u52(a[0], a[1]))
         assert np.array_equal(z2, O.normals_f64(9, O.KIND_PLATE, i, t, 2))
 
 
