@@ -16,7 +16,7 @@ from paper_2105_08026_b200 import synth  # noqa: E402
 
 def run(model, n, precision=B.F64, theta_mode=B.THETA_DEVICE_TAIL, flags=0, iters=6, astar=0.44):
     maker = {0: synth.make_normal1d, 1: synth.make_thinned_schechter1d, 2: synth.make_binormal2d,
-             3: synth.make_linreg_me1d}[model]
+             3: synth.make_linreg_me1d, 4: synth.make_bb1_fluxnoise1d, 5: synth.make_normal3d_knowncov}[model]
     kw = {}
     if model == 3:
         kw = dict(fp32=(precision != B.F64))
@@ -48,3 +48,5 @@ if __name__ == "__main__":
     run(B.M_BINORMAL2D, 2100, astar=0.234, flags=B.FLAG_TMA_STAGING)     # TMA-staged streaming kernel
     run(B.M_THINNED_SCHECHTER1D, 2500, theta_mode=B.THETA_GRAPH, iters=55)   # k_sweep + k_tail, graph replay
     run(B.M_NORMAL1D, 700, theta_mode=B.THETA_HOST)                      # host theta step
+    run(B.M_BB1_FLUXNOISE1D, 1900)                                       # on-chip kernel, BB1 case-study model
+    run(B.M_NORMAL3D_KNOWNCOV, 1500, astar=0.234)                        # streaming, p = 3 (general rank-one update)

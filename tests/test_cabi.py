@@ -41,6 +41,8 @@ def test_model_dims_and_workspace(lib):
     assert B.model_dims(B.M_THINNED_SCHECHTER1D) == dict(p=1, dtheta=3, n_cols=2, n_consts=6)
     assert B.model_dims(B.M_BINORMAL2D) == dict(p=2, dtheta=5, n_cols=4, n_consts=0)
     assert B.model_dims(B.M_LINREG_ME1D) == dict(p=1, dtheta=3, n_cols=3, n_consts=0)
+    assert B.model_dims(B.M_BB1_FLUXNOISE1D) == dict(p=1, dtheta=3, n_cols=2, n_consts=7)
+    assert B.model_dims(B.M_NORMAL3D_KNOWNCOV) == dict(p=3, dtheta=3, n_cols=3, n_consts=9)
     with pytest.raises(B.CudahmError):
         B.model_dims(99)
     small = B.workspace_bytes(B.make_config(B.M_BINORMAL2D, 1000))
@@ -64,6 +66,17 @@ def test_invalid_configs_are_refused(lib):
     assert B.workspace_bytes(bad) == 0
     bad = B.make_config(B.M_NORMAL1D, 10, block_threads=100)
     assert B.workspace_bytes(bad) == 0
+    # sharding: the offset must be even (objects draw in pairs) and the shard must lie inside the population
+    assert B.workspace_bytes(B.make_config(B.M_NORMAL1D, 10, object_offset=3, n_objects_total=100)) == 0
+    assert B.workspace_bytes(B.make_config(B.M_NORMAL1D, 10, object_offset=96, n_objects_total=100)) == 0
+    assert B.workspace_bytes(B.make_config(B.M_NORMAL1D, 10, object_offset=90, n_objects_total=100)) > 0
+    # hooks: a negative prior precision or a negative freeze iteration is refused
+    assert B.workspace_bytes(B.make_config(B.M_NORMAL1D, 10, prior_mean=[0.0, 0.0], prior_sd=[-1.0, 1.0])) == 0
+    assert B.workspace_bytes(B.make_config(B.M_NORMAL1D, 10, adapt_until=-1)) == 0
+    cfg = B.make_config(B.M_NORMAL3D_KNOWNCOV, 10, precision=B.F32_STATE_F64_REDUCE)
+    h = C.c_void_p()
+    assert lib.cudahm_create(C.byref(cfg), None, 0, None, C.byref(h)) == B.E_UNSUPPORTED
+    assert lib.cudahm_shard_sweep(None, 0, 1, None) == B.E_INVALID
     h = C.c_void_p()
     cfg = B.make_config(B.M_NORMAL1D, 10)
     assert lib.cudahm_create(C.byref(cfg), None, 0, None, C.byref(h)) == B.E_WORKSPACE

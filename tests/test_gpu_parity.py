@@ -270,6 +270,20 @@ def test_ragged_and_degenerate_sizes(n, precision):
     assert gpu.get_stats()["iterations"] == orc.get_stats()["iterations"]
 
 
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 63, 65, 513])
+def test_ragged_sizes_p3(n):
+    """The p = 3 path (general rank-one update, two Box-Muller pairs per object) on ragged and tiny populations."""
+    orc, gpu, _ = make_pair(B.M_NORMAL3D_KNOWNCOV, n, seed=4, astar=0.234, max_trace_rows=16)
+    st = sync_gpu_to_oracle(orc, gpu)
+    to, tg = orc.step(taps=True), gpu.debug_step()
+    compare_step(to, tg, B.F64, st, what=f"N={n}")
+    sync_gpu_to_oracle(orc, gpu)
+    gpu.run(8, 0, 1, sync=True)
+    orc.run(8, 0, 1)
+    np.testing.assert_allclose(gpu.get_theta_trace()[-8:], orc.get_theta_trace()[-8:], rtol=1e-9, atol=1e-9)
+    np.testing.assert_allclose(gpu.get_state()["L"], orc.get_state()["L"], rtol=1e-9, atol=1e-12)
+
+
 def test_frozen_theta_conjugate_conditional():
     """theta frozen: chi_i | theta, y_i ~ N((y/s^2 + mu/tau^2) v, v), v = 1/(1/s^2 + 1/tau^2) (closed form, P6):
     the on-device moments must land on it, and the RAM scale on 2.4176 sd (P5)."""
