@@ -55,7 +55,8 @@ def test_lockstep_trajectory(model, precision, astar, n):
             st = orc.get_state()
             sg = gpu.get_state()
             np.testing.assert_allclose(sg["chi"], st["chi"], rtol=1e-11, atol=1e-11)
-            np.testing.assert_allclose(sg["L"], st["L"], rtol=1e-10)
+            # an off-diagonal entry of L can nearly cancel: measure against the object's largest entry
+            assert np.all(np.abs(sg["L"] - st["L"]) <= 1e-10 * np.abs(st["L"]).max(0)), "L"
             np.testing.assert_allclose(sg["theta"], st["theta"], rtol=1e-9, atol=1e-9)
             np.testing.assert_allclose(sg["L_theta"], st["L_theta"], rtol=1e-8, atol=1e-12)
             # keep the two strictly in lock step so rounding differences do not accumulate into a decision
