@@ -184,6 +184,20 @@ def test_single_shard_is_the_host_mode_run_bit_for_bit():
         c.shard_sweep()
 
 
+def test_bench_sharded_leg_runs():
+    """`bench.py --sharded` (one shard on this box): the JSON line carries the metric, a positive rate and the launch
+    count of a host-driven loop (two kernels per iteration)."""
+    import json, os, subprocess, sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--sharded", "--config", "C0", "--steps", "40",
+                          "--warmup", "10"], capture_output=True, text=True, timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    assert line["metric"] == "plate_ram_updates_per_s" and line["value"] > 0 and line["n_gpus"] == 1
+    assert line["gpu_launches"] == 80 and line["config"]["theta_mode"] == "host"
+    assert 0.2 < line["accept"]["chi"] < 0.7
+
+
 def test_theta_modes_agree():
     """Same grid, same thread->object map, same reduction order in the three streaming drivers.  GRAPH and the
     plain-load streaming DEVICE_TAIL kernel run the theta step with the same device code => identical bits.  HOST
