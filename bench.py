@@ -67,6 +67,7 @@ def parse_args():
                          "all-gather of five doubles per rank and iteration; default for --gpus > 1 is independent replicas")
     ap.add_argument("--block-threads", type=int, default=0)
     ap.add_argument("--blocks-per-sm", type=int, default=0)
+    ap.add_argument("--flags", type=int, default=0, help="cudahm_config.flags (CUDAHM_FLAG_*), for experiments")
     return ap.parse_args()
 
 
@@ -171,7 +172,7 @@ def make_gpu_sampler(c, n, inp, args, seed, max_trace_rows, device, cols=None):
     s = B.Sampler(c.model, n, device=device, seed=seed, precision=c.precision, theta_mode=MODES[args.theta_mode],
                   target_accept_chi=c.target_accept_chi, target_accept_theta=c.target_accept_theta,
                   keep_chi_moments=c.keep_chi_moments, max_trace_rows=max_trace_rows,
-                  block_threads=args.block_threads, blocks_per_sm=args.blocks_per_sm)
+                  block_threads=args.block_threads, blocks_per_sm=args.blocks_per_sm, flags=getattr(args, "flags", 0))
     s.set_data(inp["cols"] if cols is None else cols)
     if inp["consts"] is not None:
         s.set_model_consts(inp["consts"])

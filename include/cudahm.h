@@ -66,6 +66,16 @@ enum { CUDAHM_THETA_HOST = 0,         /* one sweep launch + one sync per iterati
 enum { CUDAHM_FLAG_STREAMING_ONLY = 1,
        CUDAHM_FLAG_TMA_STAGING = 2 };  /* stream through TMA-staged shared-memory tiles (stream_tma.cuh) instead of
                                           plain vector loads; measured slower on C3 / C4, kept as an option          */
+/* bits 8-15 of flags: the streaming persistent kernel makes the plate draws (U_n ~ q) of each thread's
+ * first n steps of iteration t + 1 while the exchange and the theta step of iteration t are in flight; 0 in these
+ * bits = automatic, CUDAHM_FLAG_STAGE_STEPS(n) = exactly n (n = 0: off), clipped to what fits in shared memory.
+ * The chain is the same bit for bit whatever n is.                                                                */
+/* the streaming persistent kernel prefetches the columns of a thread's next step into L2 while it computes the current
+ * one, by default when state + data exceed the L2 cache (they then stream from HBM every iteration); these two force it */
+#define CUDAHM_FLAG_PREFETCH_OFF 4
+#define CUDAHM_FLAG_PREFETCH_ON 8
+#define CUDAHM_FLAG_STAGE_STEPS_MASK 0xff00
+#define CUDAHM_FLAG_STAGE_STEPS(n) ((((n) + 1) << 8) & CUDAHM_FLAG_STAGE_STEPS_MASK)
 
 typedef struct {
   uint32_t struct_size;          /* sizeof(cudahm_config), checked                                          */

@@ -17,6 +17,12 @@ M_NORMAL1D, M_THINNED_SCHECHTER1D, M_BINORMAL2D, M_LINREG_ME1D, M_BB1_FLUXNOISE1
 F64, F32_STATE_F64_REDUCE = 0, 1
 THETA_HOST, THETA_GRAPH, THETA_DEVICE_TAIL = 0, 1, 2
 FLAG_STREAMING_ONLY, FLAG_TMA_STAGING = 1, 2
+FLAG_PREFETCH_OFF, FLAG_PREFETCH_ON = 4, 8
+
+
+def flag_stage_steps(n):
+    """CUDAHM_FLAG_STAGE_STEPS(n): exactly n steps of plate draws staged ahead of the sweep (0 = off)."""
+    return ((int(n) + 1) << 8) & 0xff00
 FLOOR_LAUNCH, FLOOR_GRAPH, FLOOR_GRID_BARRIER, FLOOR_HOST_SYNC = 0, 1, 2, 3
 
 EXPORTS = ["cudahm_model_dims", "cudahm_workspace_bytes", "cudahm_create", "cudahm_destroy", "cudahm_set_data",

@@ -27,11 +27,15 @@ struct Layout {
 
 constexpr int MAX_BLOCKS = 148 * 8 * 2;   // upper bound on the grid (slots capacity)
 constexpr int MAX_PGRID = 320;            // upper bound on the persistent grid (mailboxes grow with its square)
+constexpr int STAGE_STEPS_AUTO = 2;       // staged steps of plate draws when the flags do not say
+constexpr size_t STAGE_MAX_SMEM = 192 * 1024;   // dynamic shared memory k_persistent may ask for
 
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct KernelSet {
-  const void* persistent;
+  const void* persistent;          // plain streaming persistent kernel
+  const void* persistent_ahead;    // the variant with staged draws / L2 prefetch
+  size_t stage_step_bytes;         // shared memory of one staged step of plate draws (DrawSet::NV x BLOCK values)
   const void* persistent_tma;
   size_t tma_stage_bytes;
   const void* sweep;
@@ -42,7 +46,9 @@ struct KernelSet {
 template <int MODEL, class T, int BLOCK>
 KernelSet make_set() {
   KernelSet k;
-  k.persistent = (const void*)k_persistent<MODEL, T, BLOCK>;
+  k.persistent = (const void*)k_persistent<MODEL, T, BLOCK, false>;
+  k.persistent_ahead = (const void*)k_persistent<MODEL, T, BLOCK, true>;
+  k.stage_step_bytes = (size_t)DrawSet<MODEL, T>::NV * BLOCK * sizeof(T);
   k.persistent_tma = (const void*)k_persistent_tma<MODEL, T, BLOCK>;
   k.tma_stage_bytes = (size_t)(ModelDims<MODEL>::p * (ModelDims<MODEL>::p + 3) / 2 + ModelDims<MODEL>::ncols) * (BLOCK - 32) * 16;
   k.sweep = (const void*)k_sweep<MODEL, T, BLOCK, false>;
@@ -118,6 +124,9 @@ struct cudahm_sampler {
   int res_R = 0, res_OB = 0; size_t res_smem = 0;
   int sweep_grid = 1, sweep_block = 512;   // launch shape of k_sweep (THETA_GRAPH / HOST / debug_step)
   int tma_stages = 0; size_t tma_smem = 0;   // > 0: the streaming persistent kernel is k_persistent_tma
+  bool ahead = false;                        // run k_persistent<.., AHEAD = true>
+  int prefetch = 0;                          // ... with L2 prefetch of the next step's columns
+  int n_stage = 0; size_t stage_smem = 0;    // k_persistent: steps of plate draws staged in shared memory ahead of the sweep
   double h_lp_prop_before = 0.0;    // log prior at theta' of the iteration debug_step is about to decide
   // CUDA-graph cache (THETA_GRAPH)
   cudaGraphExec_t gexec = nullptr;
@@ -148,7 +157,8 @@ bool valid_config(const cudahm_config* c, int* p, int* dt, int* nc, int* nk) {
   if (!c || c->struct_size != sizeof(cudahm_config)) return false;
   if (!model_dims(c->model, p, dt, nc, nk)) return false;
   if (c->p != *p || c->dtheta != *dt || c->n_data_cols != *nc) return false;
-  if (c->n_objects < 0 || c->max_trace_rows < 0 || (c->flags & ~(CUDAHM_FLAG_STREAMING_ONLY | CUDAHM_FLAG_TMA_STAGING)) != 0) return false;
+  if (c->n_objects < 0 || c->max_trace_rows < 0 || (c->flags & ~(CUDAHM_FLAG_STREAMING_ONLY | CUDAHM_FLAG_TMA_STAGING | CUDAHM_FLAG_STAGE_STEPS_MASK | CUDAHM_FLAG_PREFETCH_OFF |
+                                                              CUDAHM_FLAG_PREFETCH_ON)) != 0) return false;
   if (c->precision != CUDAHM_F64 && c->precision != CUDAHM_F32_STATE_F64_REDUCE) return false;
   if (c->theta_mode < CUDAHM_THETA_HOST || c->theta_mode > CUDAHM_THETA_DEVICE_TAIL) return false;
   if (!(c->target_accept_chi > 0.0 && c->target_accept_chi < 1.0)) return false;
@@ -250,6 +260,39 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
   s->grid = std::min(s->grid, MAX_BLOCKS);
   if (cfg->theta_mode == CUDAHM_THETA_DEVICE_TAIL && s->grid > MAX_PGRID) s->grid = std::max(1, MAX_PGRID / sms) * sms;
   s->sweep_grid = s->grid; s->sweep_block = block;
+  // The AHEAD variant of k_persistent:
+  // (i) a state + data set larger than L2 streams from HBM every iteration: the sweep prefetches the columns of its
+  //     next step into L2 while it computes the current one.  A set that L2 holds (C3: 72 MB) gains nothing;
+  // (ii) the plate draws of each thread's first n_stage steps of iteration t + 1 are made while the exchange and the
+  //     theta step of iteration t are in flight (they depend on (seed, object, t) only) and wait in shared memory.
+  //     Measured gains: p = 1 out of L2 -13 %, C6 (p = 3, one step) -10 %, C4 -0.5 %; C3 (p = 2: the fp64 draws of
+  //     one step take the idle warps as long as the whole exchange) loses 5 % to the plain kernel, which it keeps.
+  if (cfg->theta_mode == CUDAHM_THETA_DEVICE_TAIL && cfg->n_objects > 0) {
+    int l2 = 0;
+    cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev);
+    const size_t set_bytes = (size_t)(p + p * (p + 1) / 2 + nc) * (size_t)cfg->n_objects * s->tsize;
+    s->prefetch = (cfg->flags & CUDAHM_FLAG_PREFETCH_ON) ? 1 : (cfg->flags & CUDAHM_FLAG_PREFETCH_OFF) ? 0 : set_bytes > (size_t)l2;
+    const long long per_step = (long long)s->vec * block * s->grid;
+    const long long steps = (cfg->n_objects + per_step - 1) / per_step;
+    const int asked = (cfg->flags & CUDAHM_FLAG_STAGE_STEPS_MASK) >> 8;       // 0 = automatic, else steps + 1
+    long long ns = asked ? asked - 1 : (p == 2 && !s->prefetch ? 0 : STAGE_STEPS_AUTO);
+    ns = std::min<long long>(std::min(ns, steps), (long long)(STAGE_MAX_SMEM / ks.stage_step_bytes));
+    for (; ns > 0; --ns) {
+      const size_t bytes = (size_t)ns * ks.stage_step_bytes;
+      int fit = 0;
+      if (cudaFuncSetAttribute(ks.persistent_ahead, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) == cudaSuccess &&
+          cudaOccupancyMaxActiveBlocksPerMultiprocessor(&fit, ks.persistent_ahead, block, bytes) == cudaSuccess &&
+          (long long)fit * sms >= s->grid) break;
+      cudaGetLastError();
+    }
+    s->n_stage = (int)ns; s->stage_smem = (size_t)ns * ks.stage_step_bytes;
+    s->ahead = s->n_stage > 0 || s->prefetch;
+    if (s->ahead) {      // the grid must be co-resident for this variant too
+      int fit = 0;
+      if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&fit, ks.persistent_ahead, block, s->stage_smem) != cudaSuccess ||
+          (long long)fit * sms < s->grid) { cudaGetLastError(); s->ahead = false; s->n_stage = 0; s->stage_smem = 0; s->prefetch = 0; }
+    }
+  }
   // HBM-streaming variant with TMA-staged loads (stream_tma.cuh), opt-in: measured 10-30 % slower than plain vector
   // loads on C3 / C4 (the sweep is issue-bound, not latency-bound, and the producer warp costs a sweep warp)
   if (cfg->theta_mode == CUDAHM_THETA_DEVICE_TAIL && (cfg->flags & CUDAHM_FLAG_TMA_STAGING) && block <= 512) {
@@ -543,8 +586,9 @@ int run_device_tail(cudahm_sampler* s, long long n_iter) {
     Params P = s->P;
     unsigned epoch0 = s->epoch;            // epochs never repeat over the sampler's lifetime (0 = never written)
     s->epoch += (unsigned)k;
-    int R = s->res_R, OB = s->res_OB;
+    int R = s->res_R, OB = s->res_OB, ns = s->n_stage, pf = s->prefetch;
     void* args[] = {&P, &k, &epoch0, &R, &OB};
+    void* pargs[] = {&P, &k, &epoch0, &ns, &pf};
     int rc;
     if (s->res_kernel) {
       cudaError_t e = cudaLaunchCooperativeKernel(s->res_kernel, dim3(s->grid), dim3(RES_THREADS), args, s->res_smem, s->stream);
@@ -559,7 +603,14 @@ int run_device_tail(cudahm_sampler* s, long long n_iter) {
       s->launches++;
       rc = CUDAHM_OK;
     } else {
-      rc = launch(s, s->ks.persistent, s->grid, s->block, args, true);
+      // the shared-memory limit is a property of the function, shared by every handle of this model: set per launch
+      const void* fn = s->ahead ? s->ks.persistent_ahead : s->ks.persistent;
+      cudaError_t e = s->ahead ? cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->stage_smem) : cudaSuccess;
+      if (e == cudaSuccess)
+        e = cudaLaunchCooperativeKernel(fn, dim3(s->grid), dim3(s->block), pargs, s->ahead ? s->stage_smem : 0, s->stream);
+      if (e != cudaSuccess) return fail(s, CUDAHM_E_CUDA, "persistent kernel launch: %s", cudaGetErrorString(e));
+      s->launches++;
+      rc = CUDAHM_OK;
     }
     if (rc) return rc;
     n_iter -= k;

@@ -166,15 +166,54 @@ __device__ __forceinline__ SweepCtx<T> make_ctx(const Params& P, const Iter& it)
 
 // RAM steps 1-3 + population terms + moments for the VEC objects base .. base+VEC-1 held in x, l (updated in
 // place; the caller stores them) and d.  acc = {S, Delta, n_accept, n_nonfinite} of this thread.
+// The plate draws of the VEC objects one thread owns at one step (theta- and chi-independent: a function of
+// (seed, object, t) only, so they can be made ahead of the sweep -- k_persistent stages them in shared memory
+// while the exchange and the theta step are in flight).
+template <int MODEL, class T> struct DrawSet {
+  static constexpr int p = ModelDims<MODEL>::p, VEC = VecOf<T>::n, ZD = p < 2 ? 2 : p;
+  // values kept per object when staged: the p normals, the unit vector (p = 2 only) and the accept uniform
+  static constexpr int NZ = p, NU = (p == 2 ? 2 : 0), NV = VEC * (NZ + NU + 1);
+  T zz[VEC][ZD], csv[VEC], snv[VEC], uu[VEC];
+  __device__ __forceinline__ void make(const Params& P, const long long base, const uint32_t t) {
+#pragma unroll
+    for (int v = 0; v < VEC; v += 2) pair_draws<p>(P.tail.seed, P.obj_offset + base + v, t, &zz[v], &csv[v], &snv[v], &uu[v]);
+  }
+  // staged layout: value q of thread-slot j at st[q * stride + j] (unit stride across a warp: conflict-free)
+  __device__ __forceinline__ void put(T* st, const int stride) const {
+    int q = 0;
+#pragma unroll
+    for (int v = 0; v < VEC; ++v) {
+#pragma unroll
+      for (int k = 0; k < NZ; ++k) st[(q++) * stride] = zz[v][k];
+      if (NU) { st[(q++) * stride] = csv[v]; st[(q++) * stride] = snv[v]; }
+      st[(q++) * stride] = uu[v];
+    }
+  }
+  __device__ __forceinline__ void get(const T* st, const int stride) {
+    int q = 0;
+#pragma unroll
+    for (int v = 0; v < VEC; ++v) {
+#pragma unroll
+      for (int k = 0; k < ZD; ++k) zz[v][k] = T(0);
+#pragma unroll
+      for (int k = 0; k < NZ; ++k) zz[v][k] = st[(q++) * stride];
+      if (NU) { csv[v] = st[(q++) * stride]; snv[v] = st[(q++) * stride]; } else { csv[v] = T(0); snv[v] = T(0); }
+      uu[v] = st[(q++) * stride];
+    }
+  }
+};
+
 template <int MODEL, class T, bool TAP>
 __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c, const long long base,
-                                           T (*x)[VecOf<T>::n], T (*l)[VecOf<T>::n], const T (*d)[VecOf<T>::n], double* sum) {
+                                           T (*x)[VecOf<T>::n], T (*l)[VecOf<T>::n], const T (*d)[VecOf<T>::n], double* sum,
+                                           const DrawSet<MODEL, T>* staged = nullptr) {
   constexpr int p = ModelDims<MODEL>::p, ntri = p * (p + 1) / 2, ncols = ModelDims<MODEL>::ncols;
   constexpr int VEC = VecOf<T>::n;
-  constexpr int ZD = p < 2 ? 2 : p;
-  T zz[VEC][ZD], csv[VEC], snv[VEC], uu[VEC];
-#pragma unroll
-  for (int v = 0; v < VEC; v += 2) pair_draws<p>(P.tail.seed, P.obj_offset + base + v, c.t, &zz[v], &csv[v], &snv[v], &uu[v]);
+  DrawSet<MODEL, T> ds_;
+  if (!staged) ds_.make(P, base, c.t);
+  const DrawSet<MODEL, T>& ds = staged ? *staged : ds_;
+  const T (*zz)[DrawSet<MODEL, T>::ZD] = ds.zz;
+  const T* csv = ds.csv; const T* snv = ds.snv; const T* uu = ds.uu;
 #pragma unroll
   for (int v = 0; v < VEC; ++v) {
     const long long i = base + v;
@@ -297,34 +336,101 @@ __device__ __forceinline__ double selection_slice(const Params& P, const ThetaK&
   return tq;
 }
 
-// part[NPART] receives this thread's partial sums in ascending object order.
+// one step of the sweep: load the thread's VEC objects, update, store
 template <int MODEL, class T, bool TAP>
-__device__ __forceinline__ void sweep(const Params& P, const Iter& it, double* part) {
+__device__ __forceinline__ void sweep_step(const Params& P, const SweepCtx<T>& c, const long long base, double* acc,
+                                           const DrawSet<MODEL, T>* staged) {
   constexpr int p = ModelDims<MODEL>::p, ntri = p * (p + 1) / 2, ncols = ModelDims<MODEL>::ncols;
   constexpr int VEC = VecOf<T>::n;
-  const long long N = P.N, Npad = P.Npad;
-  const long long nthreads = (long long)gridDim.x * blockDim.x;
-  const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long Npad = P.Npad;
   T* const chi = static_cast<T*>(P.chi);
   T* const Lm = static_cast<T*>(P.L);
   const T* const dat = static_cast<const T*>(P.data);
+  T x[p][VEC], l[ntri][VEC], d[ncols][VEC];
+#pragma unroll
+  for (int j = 0; j < p; ++j) ld_vec<T>(chi + j * Npad + base, x[j], false);
+#pragma unroll
+  for (int k = 0; k < ntri; ++k) ld_vec<T>(Lm + k * Npad + base, l[k], false);
+#pragma unroll
+  for (int cc = 0; cc < ncols; ++cc) ld_vec<T>(dat + cc * Npad + base, d[cc], true);
+  update_vec<MODEL, T, TAP>(P, c, base, x, l, d, acc, staged);
+#pragma unroll
+  for (int j = 0; j < p; ++j) st_vec(chi + j * Npad + base, x[j]);
+#pragma unroll
+  for (int k = 0; k < ntri; ++k) st_vec(Lm + k * Npad + base, l[k]);
+}
+
+// L2 prefetch of the columns of the step that starts at object `base` (no registers held, unlike a load issued early)
+#ifndef HM_PREFETCH
+#define HM_PREFETCH 1
+#endif
+template <int MODEL, class T>
+__device__ __forceinline__ void prefetch_step(const Params& P, const long long base) {
+#if HM_PREFETCH
+  constexpr int p = ModelDims<MODEL>::p, ntri = p * (p + 1) / 2, ncols = ModelDims<MODEL>::ncols;
+  const long long Npad = P.Npad;
+  const T* const chi = static_cast<const T*>(P.chi);
+  const T* const Lm = static_cast<const T*>(P.L);
+  const T* const dat = static_cast<const T*>(P.data);
+#pragma unroll
+  for (int j = 0; j < p; ++j) asm volatile("prefetch.global.L2 [%0];" ::"l"(chi + j * Npad + base));
+#pragma unroll
+  for (int k = 0; k < ntri; ++k) asm volatile("prefetch.global.L2 [%0];" ::"l"(Lm + k * Npad + base));
+#pragma unroll
+  for (int cc = 0; cc < ncols; ++cc) asm volatile("prefetch.global.L2 [%0];" ::"l"(dat + cc * Npad + base));
+#endif
+}
+
+// part[NPART] receives this thread's partial sums in ascending object order.  stage / n_stage: the plate draws of
+// the thread's first n_stage steps, made ahead by stage_draws (k_persistent); the same values bit for bit.
+template <int MODEL, class T, bool TAP, bool AHEAD = false>
+__device__ __forceinline__ void sweep(const Params& P, const Iter& it, double* part, const T* stage = nullptr,
+                                      const int n_stage = 0, const bool prefetch = false) {
+  constexpr int VEC = VecOf<T>::n;
+  const long long N = P.N;
+  const long long nthreads = (long long)gridDim.x * blockDim.x;
+  const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const SweepCtx<T> c = make_ctx<T>(P, it);
   double acc[4] = {0.0, 0.0, 0.0, 0.0};
-  for (long long base = (long long)VEC * gid; base < N; base += (long long)VEC * nthreads) {
-    T x[p][VEC], l[ntri][VEC], d[ncols][VEC];
-#pragma unroll
-    for (int j = 0; j < p; ++j) ld_vec<T>(chi + j * Npad + base, x[j], false);
-#pragma unroll
-    for (int k = 0; k < ntri; ++k) ld_vec<T>(Lm + k * Npad + base, l[k], false);
-#pragma unroll
-    for (int cc = 0; cc < ncols; ++cc) ld_vec<T>(dat + cc * Npad + base, d[cc], true);
-    update_vec<MODEL, T, TAP>(P, c, base, x, l, d, acc);
-#pragma unroll
-    for (int j = 0; j < p; ++j) st_vec(chi + j * Npad + base, x[j]);
-#pragma unroll
-    for (int k = 0; k < ntri; ++k) st_vec(Lm + k * Npad + base, l[k]);
+  long long base = (long long)VEC * gid;
+  const long long stride = (long long)VEC * nthreads;
+  if constexpr (AHEAD) {
+    // while a step is computed the next one is on its way from HBM to L2 (after the last step: the first step of
+    // the next iteration, which then arrives during the exchange and the theta step)
+    const int B = (int)blockDim.x;
+    for (int s = 0; s < n_stage && base < N; ++s, base += stride) {
+      if (prefetch) prefetch_step<MODEL, T>(P, base + stride < N ? base + stride : (long long)VEC * gid);
+      DrawSet<MODEL, T> ds;
+      ds.get(stage + (size_t)s * DrawSet<MODEL, T>::NV * B + threadIdx.x, B);
+      sweep_step<MODEL, T, TAP>(P, c, base, acc, &ds);
+    }
+    for (; base < N; base += stride) {
+      if (prefetch) prefetch_step<MODEL, T>(P, base + stride < N ? base + stride : (long long)VEC * gid);
+      sweep_step<MODEL, T, TAP>(P, c, base, acc, nullptr);
+    }
+  } else {
+    for (; base < N; base += stride) sweep_step<MODEL, T, TAP>(P, c, base, acc, nullptr);
   }
   part[0] = acc[0]; part[1] = acc[1]; part[2] = selection_slice<MODEL>(P, c.kp, (int)blockDim.x); part[3] = acc[2]; part[4] = acc[3];
+}
+
+// Stage the plate draws of iteration t for the first n_stage steps of every thread of this block.  Called by the
+// `nworkers` threads with worker index w = 0 .. nworkers-1 (the warps that do not run the theta tail).
+template <int MODEL, class T>
+__device__ __forceinline__ void stage_draws(const Params& P, const uint32_t t, T* stage, const int n_stage, const int w,
+                                            const int nworkers) {
+  constexpr int VEC = VecOf<T>::n;
+  const int B = (int)blockDim.x;
+  const long long nthreads = (long long)gridDim.x * B;
+  for (int idx = w; idx < n_stage * B; idx += nworkers) {
+    const int s = idx / B, j = idx - s * B;
+    const long long base = (long long)VEC * ((long long)s * nthreads + (long long)blockIdx.x * B + j);
+    if (base < P.N) {
+      DrawSet<MODEL, T> ds;
+      ds.make(P, base, t);
+      ds.put(stage + (size_t)s * DrawSet<MODEL, T>::NV * B + j, B);
+    }
+  }
 }
 
 // Deterministic block reduction of NQ quantities: shuffle tree inside each warp, then warp 0 over the per-warp
@@ -493,12 +599,24 @@ static_assert(sizeof(Iter) % sizeof(double) == 0, "Iter is copied as doubles");
 // flag exchange needs).  Per iteration: sweep -> block partials -> flagged slot -> warp 0 of EVERY block collects
 // all slots in the same fixed order -> block-parallel theta tail (identical in every block) -> next sweep.
 // One grid-wide round trip per iteration.  Accept / non-finite counters stay in registers until the launch ends.
-template <int MODEL, class T, int BLOCK>
-__global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const long long n_iter, const unsigned epoch0) {
+// AHEAD: the variant that works ahead of the exchange -- plate draws of the next iteration staged in shared memory by
+// the warps that do not run the theta tail, next step's columns prefetched into L2.  The plain variant
+// is kept for the populations that gain nothing from either (p = 2 out of L2: C3).  Same chain bit for bit.
+template <int MODEL, class T, int BLOCK, bool AHEAD>
+__global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const long long n_iter, const unsigned epoch0,
+                                                         const int n_stage, const int prefetch) {
   __shared__ Iter it;
   __shared__ double red[32][NPART];
+  extern __shared__ __align__(16) unsigned char stage_raw[];   // n_stage x DrawSet::NV x BLOCK values of T
+  T* const stage = reinterpret_cast<T*>(stage_raw);
+  constexpr int TAILT = 128;                                   // the four warps of the theta tail
   copy_iter(&it, P.iter);
   __syncthreads();
+  // draws of the launch's first iteration: every thread stages (nothing to overlap with yet)
+  if (AHEAD) {
+    stage_draws<MODEL, T>(P, (uint32_t)it.t, stage, n_stage, (int)threadIdx.x, BLOCK);
+    __syncthreads();
+  }
   const int G = (int)gridDim.x;
   double cnt[2] = {0.0, 0.0};
 #ifdef HM_PHASE_TIMING
@@ -512,7 +630,8 @@ __global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const l
     long long last_ = clock64();
 #endif
     double part[NPART];
-    sweep<MODEL, T, false>(P, it, part);
+    const uint32_t t_next = (uint32_t)it.t + 1u;
+    sweep<MODEL, T, false, AHEAD>(P, it, part, stage, n_stage, prefetch != 0);
     HM_STAMP(0)
     cnt[0] += part[3]; cnt[1] += part[4];
     double dq[2] = {part[1], part[2]};
@@ -522,14 +641,33 @@ __global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const l
     const unsigned epoch = epoch0 + (unsigned)k;
     mbox_push<NVX>(mb, G, (int)blockIdx.x, epoch, dq, (int)threadIdx.x, (int)blockDim.x);
     HM_STAMP(1)
-    double tot[NPART] = {0.0, 0.0, 0.0, 0.0, 0.0};
-    if (threadIdx.x < 32) {
-      double t2[2] = {0.0, 0.0};
-      mbox_collect<NVX>(mb + (size_t)blockIdx.x * mbox_reader_words(G), G, epoch, t2);
-      tot[1] = t2[0]; tot[2] = t2[1];
+    // warps 0-3: collect + theta tail (the serial chain); the other warps meanwhile make the plate draws of the
+    // first n_stage steps of iteration t + 1, which depend on nothing but (seed, object, t + 1)
+    if (!AHEAD) {
+      double tot[NPART] = {0.0, 0.0, 0.0, 0.0, 0.0};
+      if (threadIdx.x < 32) {
+        double t2[2] = {0.0, 0.0};
+        mbox_collect<NVX>(mb + (size_t)blockIdx.x * mbox_reader_words(G), G, epoch, t2);
+        tot[1] = t2[0]; tot[2] = t2[1];
+      }
+      HM_STAMP(2)
+      tail_block(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, (int)(threadIdx.x >> 5), SyncAll());
+      HM_STAMP(3)
+      continue;
     }
-    HM_STAMP(2)
-    tail_block(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, (int)(threadIdx.x >> 5), SyncAll());
+    if (threadIdx.x < TAILT) {
+      double tot[NPART] = {0.0, 0.0, 0.0, 0.0, 0.0};
+      if (threadIdx.x < 32) {
+        double t2[2] = {0.0, 0.0};
+        mbox_collect<NVX>(mb + (size_t)blockIdx.x * mbox_reader_words(G), G, epoch, t2);
+        tot[1] = t2[0]; tot[2] = t2[1];
+      }
+      HM_STAMP(2)
+      tail_block(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, (int)(threadIdx.x >> 5), SyncNamed<1, TAILT>());
+    } else if (k + 1 < n_iter) {
+      stage_draws<MODEL, T>(P, t_next, stage, n_stage, (int)threadIdx.x - TAILT, BLOCK - TAILT);
+    }
+    __syncthreads();
     HM_STAMP(3)
   }
 #ifdef HM_PHASE_TIMING

@@ -246,6 +246,41 @@ def test_streaming_persistent_kernel_matches_oracle(model, astar, n, flags):
     assert stg["block_threads"] != 640
 
 
+@pytest.mark.parametrize("model,astar,n,precision", [(B.M_THINNED_SCHECHTER1D, 0.44, 200001, B.F64),
+                                                       (B.M_BINORMAL2D, 0.234, 200001, B.F64),
+                                                       (B.M_LINREG_ME1D, 0.44, 400003, B.F32_STATE_F64_REDUCE),
+                                                       (B.M_NORMAL3D_KNOWNCOV, 0.234, 160001, B.F64)],
+                         ids=["M1", "M2", "M3f32", "M5"])
+def test_staged_draws_and_prefetch_do_not_change_the_chain(model, astar, n, precision):
+    """k_persistent<AHEAD>: plate draws of the next iteration staged in shared memory during the exchange, next step's
+    columns prefetched into L2.  Whatever the number of staged steps (none, some, more than the sweep has), with or
+    without prefetch, the chain is the plain kernel's bit for bit; the plain kernel is checked against the oracle."""
+    iters, burn, thin = 40, 10, 5
+    variants = [B.flag_stage_steps(0) | B.FLAG_PREFETCH_OFF, B.flag_stage_steps(0) | B.FLAG_PREFETCH_ON,
+                B.flag_stage_steps(1) | B.FLAG_PREFETCH_OFF, B.flag_stage_steps(2) | B.FLAG_PREFETCH_ON,
+                B.flag_stage_steps(9) | B.FLAG_PREFETCH_ON, 0]
+    ref, inp, orc = None, None, None
+    for k, fl in enumerate(variants):
+        o, gpu, inp = make_pair(model, n, seed=77 + model, astar=astar, keep_moments=True, precision=precision,
+                                max_trace_rows=(iters - burn) // thin, flags=fl | B.FLAG_STREAMING_ONLY,
+                                block_threads=256, blocks_per_sm=1, inputs=inp, want_oracle=(k == 0))
+        gpu.run(iters, burn, thin, sync=True)
+        st, tr, mom = gpu.get_state(), gpu.get_theta_trace(), gpu.get_chi_moments()
+        assert gpu.get_stats()["grid_blocks"] * 256 * (2 if precision == B.F64 else 4) * 2 < n   # at least 3 steps
+        gpu.close()
+        if k == 0:
+            ref, orc = (st, tr, mom), o
+        else:
+            for key in ("chi", "L", "theta", "L_theta"):
+                assert np.array_equal(ref[0][key], st[key]), (key, hex(fl))
+            assert np.array_equal(ref[1], tr) and np.array_equal(ref[2][0], mom[0]) and np.array_equal(ref[2][1], mom[1])
+    if precision == B.F64:
+        orc.run(iters, burn, thin)
+        so = orc.get_state()
+        np.testing.assert_allclose(ref[0]["chi"], so["chi"], rtol=1e-9, atol=1e-9)
+        np.testing.assert_allclose(ref[1], orc.get_theta_trace(), rtol=1e-8, atol=1e-8)
+
+
 def test_resume_is_bit_exact():
     """Counter-based streams: run(70) + run(50) == run(120), and get_state/set_state round-trips."""
     _, g1, inp = make_pair(B.M_BINORMAL2D, 3000, seed=8, astar=0.234, max_trace_rows=120, want_oracle=False)
