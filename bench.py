@@ -38,9 +38,9 @@ ALG_BYTES = {"C0": (48, 32), "C1": (48, 32), "C2": (48, 32), "C3": (112, 64), "C
 MODES = {"host": 0, "graph": 1, "tail": 2}
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel PER GIBBS ITERATION, from the committed
 # `ncu --set full` captures (profiles/r01g_resident_C2_ncu.md: 14.59 MB + 0.111 MB over 300 iterations;
-# profiles/r01f_persistent_C4_ncu.md: 5.940 GB + 2.363 GB over 30 iterations); scaled to the K iterations one timed
+# profiles/r01i_persistent_C4_ncu.md: 5.972 GB + 2.372 GB over 30 iterations); scaled to the K iterations one timed
 # launch runs.  C2 keeps its state in shared memory, so its DRAM traffic is ~0.2 % of the algorithmic bytes.
-NCU_DRAM_BYTES_PER_ITER = {"C2": (14.590720e6 + 111.360e3) / 300, "C4": (5.940074e9 + 2.362765e9) / 30,
+NCU_DRAM_BYTES_PER_ITER = {"C2": (14.590720e6 + 111.360e3) / 300, "C4": (5.972273e9 + 2.372094e9) / 30,
                            "C5": (3.414528e6 + 126.720e3) / 300, "C6": (2.994176e6 + 19.968e3) / 300}
 
 
