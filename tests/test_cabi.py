@@ -73,6 +73,13 @@ def test_invalid_configs_are_refused(lib):
     # hooks: a negative prior precision or a negative freeze iteration is refused
     assert B.workspace_bytes(B.make_config(B.M_NORMAL1D, 10, prior_mean=[0.0, 0.0], prior_sd=[-1.0, 1.0])) == 0
     assert B.workspace_bytes(B.make_config(B.M_NORMAL1D, 10, adapt_until=-1)) == 0
+    # flags: the documented bits (streaming only, TMA staging, prefetch on / off, staged draw steps) pass; others do not
+    ok = B.FLAG_STREAMING_ONLY | B.FLAG_PREFETCH_ON | B.flag_stage_steps(3)
+    assert B.workspace_bytes(B.make_config(B.M_NORMAL1D, 10, flags=ok)) > 0
+    assert B.workspace_bytes(B.make_config(B.M_NORMAL1D, 10, flags=B.flag_stage_steps(0) | B.FLAG_PREFETCH_OFF)) > 0
+    assert B.workspace_bytes(B.make_config(B.M_NORMAL1D, 10, flags=1 << 16)) == 0
+    assert B.workspace_bytes(B.make_config(B.M_NORMAL1D, 10, flags=16)) == 0
+    assert B.flag_stage_steps(0) == 0x100 and B.flag_stage_steps(2) == 0x300
     cfg = B.make_config(B.M_NORMAL3D_KNOWNCOV, 10, precision=B.F32_STATE_F64_REDUCE)
     h = C.c_void_p()
     assert lib.cudahm_create(C.byref(cfg), None, 0, None, C.byref(h)) == B.E_UNSUPPORTED
