@@ -251,11 +251,15 @@ def test_streaming_persistent_kernel_matches_oracle(model, astar, n, flags):
                                                        (B.M_LINREG_ME1D, 0.44, 400003, B.F32_STATE_F64_REDUCE),
                                                        (B.M_NORMAL3D_KNOWNCOV, 0.234, 160001, B.F64)],
                          ids=["M1", "M2", "M3f32", "M5"])
-def test_staged_draws_and_prefetch_do_not_change_the_chain(model, astar, n, precision):
+@pytest.mark.parametrize("block", [256, 512, 1024])
+def test_staged_draws_and_prefetch_do_not_change_the_chain(model, astar, n, precision, block):
     """k_persistent<AHEAD>: plate draws of the next iteration staged in shared memory during the exchange, next step's
     columns prefetched into L2.  Whatever the number of staged steps (none, some, more than the sweep has), with or
     without prefetch, the chain is the plain kernel's bit for bit; the plain kernel is checked against the oracle."""
     iters, burn, thin = 40, 10, 5
+    n = n * (block // 256)                      # at least three steps per thread at every block size
+    if block == 1024 and model == B.M_NORMAL3D_KNOWNCOV:
+        pytest.skip("p = 3 at 64 registers per thread: not a configuration anything selects")
     variants = [B.flag_stage_steps(0) | B.FLAG_PREFETCH_OFF, B.flag_stage_steps(0) | B.FLAG_PREFETCH_ON,
                 B.flag_stage_steps(1) | B.FLAG_PREFETCH_OFF, B.flag_stage_steps(2) | B.FLAG_PREFETCH_ON,
                 B.flag_stage_steps(9) | B.FLAG_PREFETCH_ON, 0]
@@ -263,10 +267,11 @@ def test_staged_draws_and_prefetch_do_not_change_the_chain(model, astar, n, prec
     for k, fl in enumerate(variants):
         o, gpu, inp = make_pair(model, n, seed=77 + model, astar=astar, keep_moments=True, precision=precision,
                                 max_trace_rows=(iters - burn) // thin, flags=fl | B.FLAG_STREAMING_ONLY,
-                                block_threads=256, blocks_per_sm=1, inputs=inp, want_oracle=(k == 0))
+                                block_threads=block, blocks_per_sm=1, inputs=inp, want_oracle=(k == 0 and block == 256))
         gpu.run(iters, burn, thin, sync=True)
         st, tr, mom = gpu.get_state(), gpu.get_theta_trace(), gpu.get_chi_moments()
-        assert gpu.get_stats()["grid_blocks"] * 256 * (2 if precision == B.F64 else 4) * 2 < n   # at least 3 steps
+        assert gpu.get_stats()["block_threads"] == block
+        assert gpu.get_stats()["grid_blocks"] * block * (2 if precision == B.F64 else 4) * 2 < n   # at least 3 steps
         gpu.close()
         if k == 0:
             ref, orc = (st, tr, mom), o
@@ -274,7 +279,7 @@ def test_staged_draws_and_prefetch_do_not_change_the_chain(model, astar, n, prec
             for key in ("chi", "L", "theta", "L_theta"):
                 assert np.array_equal(ref[0][key], st[key]), (key, hex(fl))
             assert np.array_equal(ref[1], tr) and np.array_equal(ref[2][0], mom[0]) and np.array_equal(ref[2][1], mom[1])
-    if precision == B.F64:
+    if precision == B.F64 and orc is not None:
         orc.run(iters, burn, thin)
         so = orc.get_state()
         np.testing.assert_allclose(ref[0]["chi"], so["chi"], rtol=1e-9, atol=1e-9)
