@@ -246,6 +246,15 @@ def time_e2e(cfg_name, args, device, rank):
     return dict(sec=sec, n=n, iters=W + K, h2d=h2d, d2h=d2h)
 
 
+def kernel_label(st):
+    """Which persistent kernel a THETA_DEVICE_TAIL run launched (cudahm_get_stats says)."""
+    if st["block_threads"] == 640:
+        return "k_resident"
+    if st.get("stage_steps", 0) or st.get("l2_prefetch", 0):
+        return f"k_persistent<AHEAD> (staged draw steps {st['stage_steps']}, L2 prefetch {'on' if st['l2_prefetch'] else 'off'})"
+    return "k_persistent"
+
+
 def roofline_entry(cfg_name, c, n, K, W, ms, peak, peak_src, kernel=None):
     base, mom = ALG_BYTES[cfg_name]
     per_obj = base + (mom if c.keep_chi_moments else 0)     # the timed iterations are all past burn-in
@@ -457,7 +466,7 @@ def main():
         "gpu_launches": int(r["launches"]),
         "clocks": r["clocks"],
         "roofline": roofline_entry(args.config, c, n, K, W, r["ms"], peak, peak_src,
-                                   "k_resident" if r["stats"]["block_threads"] == 640 else "k_persistent"),
+                                   kernel_label(r["stats"]) if args.theta_mode == "tail" else "k_sweep"),
         "accept": {"chi": r["stats"]["chi_accepts"] / max(1, r["stats"]["chi_proposals"]),
                    "theta": r["stats"]["theta_accepts"] / max(1, r["stats"]["theta_proposals"])},
         "theta_mean": [float(x) for x in r["trace"].mean(0)] if len(r["trace"]) else None,
@@ -501,7 +510,7 @@ def extras(args, device, peak, peak_src, n):
         a = copy.copy(args)
         a.steps, a.warmup, a.n_objects = k, w, 0
         r = time_gpu(cfg_name, a, device, 0, 1, lambda: None, with_clocks=False)
-        kern = "k_resident" if r["stats"]["block_threads"] == 640 else "k_persistent"
+        kern = kernel_label(r["stats"])
         rf = roofline_entry(cfg_name, r["cfg"], r["n"], k, w, r["ms"], peak, peak_src, kern)
         side[cfg_name] = {"n_objects": r["n"], "steps": k, "warmup": w, "updates_per_s": r["n"] * k / (r["ms"] * 1e-3),
                           "gibbs_iters_per_s": k / (r["ms"] * 1e-3), "roofline": rf,

@@ -121,6 +121,8 @@ typedef struct {
   int64_t gpu_launches;          /* kernels launched by this handle so far                                  */
   int32_t grid_blocks, block_threads;   /* launch configuration of the sweep                               */
   double  last_run_ms;           /* device time of the last cudahm_run (CUDA events on the stream)          */
+  int32_t stage_steps;           /* streaming persistent kernel: steps of plate draws staged ahead per thread */
+  int32_t l2_prefetch;           /* ... 1: it prefetches the next step's columns into L2 (0 for the on-chip kernel) */
 } cudahm_stats;
 
 /* Per-iteration taps of cudahm_debug_step; HOST pointers, each may be NULL.  Values are widened to double. */

@@ -50,7 +50,8 @@ class Stats(C.Structure):
     _fields_ = [(k, C.c_int64) for k in ("iterations", "chi_accepts", "chi_proposals", "theta_accepts",
                                          "theta_proposals", "nonfinite", "moment_samples", "trace_rows",
                                          "gpu_launches")] + \
-               [("grid_blocks", C.c_int32), ("block_threads", C.c_int32), ("last_run_ms", C.c_double)]
+               [("grid_blocks", C.c_int32), ("block_threads", C.c_int32), ("last_run_ms", C.c_double),
+                ("stage_steps", C.c_int32), ("l2_prefetch", C.c_int32)]
 
 
 class Taps(C.Structure):

@@ -884,6 +884,8 @@ extern "C" int cudahm_get_stats(cudahm_sampler* s, cudahm_stats* out) {
   if (!s || !out) return fail(s, CUDAHM_E_INVALID, "get_stats: NULL argument");
   std::memset(out, 0, sizeof *out);
   out->grid_blocks = s->grid; out->block_threads = s->block; out->gpu_launches = s->launches;
+  const bool streaming_tail = s->cfg.theta_mode == CUDAHM_THETA_DEVICE_TAIL && !s->res_kernel && s->tma_stages == 0 && s->ahead;
+  out->stage_steps = streaming_tail ? s->n_stage : 0; out->l2_prefetch = streaming_tail ? s->prefetch : 0;
   if (!s->have_init) return CUDAHM_OK;
   int rc = fetch_iter(s); if (rc) return rc;
   const Iter& it = *s->h_iter;

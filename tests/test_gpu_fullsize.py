@@ -89,6 +89,7 @@ def test_c3_full_size_free_running():
     gpu.run(8, 0, 1, sync=True)
     st = gpu.get_stats()
     assert (st["grid_blocks"], st["block_threads"]) == (148, 512)
+    assert (st["stage_steps"], st["l2_prefetch"]) == (0, 0), "C3 (state + data inside L2, p = 2) keeps the plain variant"
     so, sg = orc.get_state(), gpu.get_state()
     np.testing.assert_allclose(gpu.get_theta_trace(), orc.get_theta_trace(), rtol=1e-9, atol=1e-9)
     np.testing.assert_allclose(sg["chi"], so["chi"], rtol=1e-9, atol=1e-9)
@@ -120,4 +121,5 @@ def test_c4_full_size_single_steps():
         np.testing.assert_allclose(sg["theta"], so["theta"], rtol=1e-6, atol=1e-6)
     stg = gpu.get_stats()
     assert (stg["grid_blocks"], stg["block_threads"]) == (148, 512)
+    assert (stg["stage_steps"], stg["l2_prefetch"]) == (2, 1), "C4 as benched: staged draws + L2 prefetch (DESIGN.md 8.7)"
     print(f"C4: {flips} near-tie accept flips in {2 * n} fp32 decisions")
