@@ -278,9 +278,9 @@ __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c
       }
     } else {
       const T s1 = T(1) + cc * cs * cs;
-      const T k00 = hm_sqrt(s1);
+      const T k00 = hm_sqrt_pos(s1);
       const T k10 = cc * cs * sn / k00;
-      const T k11 = hm_sqrt((T(1) + cc) / s1);
+      const T k11 = hm_sqrt_pos((T(1) + cc) / s1);
       ln[0] = l[0][v] * k00;
       ln[1] = l[1][v] * k00 + l[2][v] * k10;
       ln[2] = l[2][v] * k11;
