@@ -180,6 +180,19 @@ HM_HD double hm_sqrt_fast(double w) {
   return hm_fma(hm_fma(-g, g, w), h, g);                    // final correction
 }
 
+// sqrt(w) and 1/sqrt(w) together (the same Newton pair; 1/sqrt = 2 h after one more correction step), w > 0 normal
+HM_HD void hm_sqrt_rsqrt(double w, double* root, double* inv_root) {
+  const double y = hm_rsqrt_seed(w);
+  double g = w * y, h = 0.5 * y;
+  double r = hm_fma(-g, h, 0.5);
+  g = hm_fma(g, r, g); h = hm_fma(h, r, h);
+  r = hm_fma(-g, h, 0.5);
+  g = hm_fma(g, r, g); h = hm_fma(h, r, h);
+  r = hm_fma(-g, h, 0.5);
+  *root = hm_fma(hm_fma(-g, g, w), h, g);
+  *inv_root = 2.0 * hm_fma(h, r, h);
+}
+
 // exp / log of the theta tail: the specialised versions on the device (the tail is a serial chain on the critical
 // path of every iteration), libm on the host (THETA_HOST).
 HM_HD double hm_exp_any(double x) {

@@ -64,6 +64,8 @@ __device__ __forceinline__ float hm_sqrt(float x) { return sqrtf(x); }
 __device__ __forceinline__ double hm_rsqrt(double x) { return rsqrt(x); }
 __device__ __forceinline__ float hm_rsqrt(float x) { return rsqrtf(x); }
 __device__ __forceinline__ double hm_sqrt_pos(double x) { return hm_sqrt_fast(x); }
+__device__ __forceinline__ void hm_sqrt_both(double x, double* g, double* ig) { hm_sqrt_rsqrt(x, g, ig); }
+__device__ __forceinline__ void hm_sqrt_both(float x, float* g, float* ig) { *ig = rsqrtf(x); *g = x * *ig; }
 __device__ __forceinline__ float hm_sqrt_pos(float x) { return x * rsqrtf(x); }
 
 // Plate-level draws.  Objects draw in PAIRS m = i >> 1 so that one Philox call and one
@@ -278,9 +280,10 @@ __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c
       }
     } else {
       const T s1 = T(1) + cc * cs * cs;
-      const T k00 = hm_sqrt_pos(s1);
-      const T k10 = cc * cs * sn / k00;
-      const T k11 = hm_sqrt_pos((T(1) + cc) / s1);
+      T k00, ik00;
+      hm_sqrt_both(s1, &k00, &ik00);                       // sqrt(s1), 1/sqrt(s1): no division in the update
+      const T k10 = cc * cs * sn * ik00;
+      const T k11 = hm_sqrt_pos(T(1) + cc) * ik00;
       ln[0] = l[0][v] * k00;
       ln[1] = l[1][v] * k00 + l[2][v] * k10;
       ln[2] = l[2][v] * k11;
