@@ -77,6 +77,16 @@ def test_sqrt_fast(binary):
     assert np.mean(got == np.sqrt(w)) > 0.95          # almost always the correctly rounded root
 
 
+def test_sqrt_rsqrt_pair(binary):
+    """The p = 2 RAM update takes sqrt(s1) and 1/sqrt(s1) from one Newton pair (s1 = 1 + c u1^2 in (0.4, 2))."""
+    rng = np.random.default_rng(4)
+    w = np.concatenate([rng.uniform(0.4, 2.0, 4000), np.exp(rng.uniform(-20, 20, 2000)), [1.0, 4.0, 0.25, 2.0]])
+    root, inv = run(binary, "sqrt_both_root", w), run(binary, "sqrt_both_inv", w)
+    assert ulp_err(root, mpmath.sqrt, w) <= 1.0
+    assert ulp_err(inv, lambda x: 1 / mpmath.sqrt(x), w) <= 2.0
+    assert root[-4] == 1.0 and inv[-4] == 1.0 and root[-3] == 2.0 and inv[-3] == 0.5
+
+
 def test_u01_is_exact(binary):
     rng = np.random.default_rng(4)
     a = rng.integers(0, 2 ** 32, 5000, dtype=np.uint64)
