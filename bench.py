@@ -36,12 +36,14 @@ UNIT = "updates/s"
 ALG_BYTES = {"C0": (48, 32), "C1": (48, 32), "C2": (48, 32), "C3": (112, 64), "C4": (28, 32), "C5": (48, 32),
              "C6": (240, 96)}     # p = 3: chi 3 + L 6 doubles read and written, 3 data doubles read
 MODES = {"host": 0, "graph": 1, "tail": 2}
-# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel PER GIBBS ITERATION, from the committed
-# `ncu --set full` captures (profiles/r01g_resident_C2_ncu.md: 14.59 MB + 0.111 MB over 300 iterations;
-# profiles/r01i_persistent_C4_ncu.md: 5.972 GB + 2.372 GB over 30 iterations); scaled to the K iterations one timed
-# launch runs.  C2 keeps its state in shared memory, so its DRAM traffic is ~0.2 % of the algorithmic bytes.
-NCU_DRAM_BYTES_PER_ITER = {"C2": (14.590720e6 + 111.360e3) / 300, "C4": (5.972273e9 + 2.372094e9) / 30,
-                           "C5": (3.414528e6 + 126.720e3) / 300, "C6": (2.994176e6 + 19.968e3) / 300}
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel PER LAUNCH, from committed `ncu --set full` captures of
+# exactly the (config, warm-up, steps) named in the key; any other launch reports traffic = null.  Filled from profiles/.
+NCU_DRAM_BYTES_PER_LAUNCH = {}
+# warp-level instructions executed per 32 object-updates (ncu smsp__inst_executed.sum / (N K / 32)) and the share of them
+# on the fp64 pipe, per config, from the committed captures; None where no capture exists.  They give the two compute
+# floors reported beside the HBM one: issue slots (4 warp-instructions / clk / SM) and the fp64 pipe (64 lanes / clk / SM).
+NCU_WARP_INSTR_PER_32 = {"C2": (425, 0.37 * 4 * 32 / 64 / 0.61), "C3": (459, None), "C4": (165, None)}
+N_SMS, SM_CLOCK_HZ = 148, 1.965e9
 
 
 def workload_label(name):
@@ -50,6 +52,14 @@ def workload_label(name):
     if name == "C6":
         return "C6: the paper's normal-normal benchmark (PAPER.md section 3: 3-vector latents, N = 3e4); not a BASELINE.json config"
     return f"{name}: BASELINE.json configs[{int(name[1])}]"
+
+
+def config_entry(cfg_name, c, n, W):
+    """`config` of the JSON line: the same keys in the CUDA arm and in the --impl reference arm."""
+    return {"workload": workload_label(cfg_name), "n_objects": n, "burn_in": W, "thin": c.thin,
+            "chi_moments": bool(c.keep_chi_moments),
+            "model": ["normal1d", "thinned_schechter1d", "binormal2d", "linreg_me1d", "bb1_fluxnoise1d",
+                      "normal3d_knowncov", "normalpd_knowncov"][c.model]}
 
 
 def parse_args():
@@ -176,7 +186,7 @@ def make_gpu_sampler(c, n, inp, args, seed, max_trace_rows, device, cols=None):
     s.set_data(inp["cols"] if cols is None else cols)
     if inp["consts"] is not None:
         s.set_model_consts(inp["consts"])
-    s.set_init(inp["theta0"])
+    s.set_init(inp["theta0"], theta_chol0=make_theta_chol0(inp, n))
     return s
 
 
@@ -184,38 +194,86 @@ def trace_rows_needed(total_iters, burn_in, thin):
     return max(0, (total_iters - burn_in) // thin) + 1
 
 
-def time_gpu(cfg_name, args, device, rank, world, barrier, with_clocks=True):
-    """W burn-in iterations untimed, then exactly K iterations timed on the device (inputs resident in HBM)."""
+REPEATS = 5     # best and median of 5
+
+
+def make_theta_chol0(inp, n):
+    """The theta proposal factor the workload recipe supplies; None = the library default."""
+    f = inp.get("theta_chol0")
+    return None if f is None else np.asarray(f, dtype=np.float64)
+
+
+def time_gpu(cfg_name, args, device, rank, world, barrier, with_clocks=True, repeats=REPEATS):
+    """W burn-in iterations untimed, then `repeats` timed regions of EXACTLY K iterations each, back to back, each timed
+    on the device with CUDA events on the sampler's stream (inputs resident in HBM).  ms = the median region."""
     import torch
-    from paper_2105_08026_b200 import binding as B
     c, n, inp = make_workload(cfg_name, args.n_objects if cfg_name == args.config else 0, seed_offset=rank)
     W, K = args.warmup, args.steps
     dt = np.float64 if c.precision == synth.F64 else np.float32
     dev_cols = [torch.from_numpy(np.ascontiguousarray(col, dtype=dt)).to(device) for col in inp["cols"]]
-    s = make_gpu_sampler(c, n, inp, args, c.seed + rank, trace_rows_needed(W + K, W, c.thin), device, cols=dev_cols)
+    s = make_gpu_sampler(c, n, inp, args, c.seed + rank, trace_rows_needed(W + repeats * K, W, c.thin), device, cols=dev_cols)
     s.run(W, W, c.thin, sync=True)                      # burn-in = warm-up (adaptation, caches, clocks)
     l0 = s.get_stats()["gpu_launches"]
     stream = s.stream
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     clk = ClockSampler(torch.device(device).index or 0) if with_clocks else None
-    barrier()
-    torch.cuda.synchronize(device)
     if clk:
         clk.start()
-    with torch.cuda.stream(stream):
-        e0.record(stream)
-        s.run(K, W, c.thin)
-        e1.record(stream)
-    torch.cuda.synchronize(device)
+    times = []
+    for _ in range(repeats):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        torch.cuda.synchronize(device)
+        with torch.cuda.stream(stream):
+            e0.record(stream)
+            s.run(K, W, c.thin)
+            e1.record(stream)
+        torch.cuda.synchronize(device)
+        barrier()
+        times.append(e0.elapsed_time(e1))
     clocks = clk.stop() if clk else None
-    barrier()
-    ms = e0.elapsed_time(e1)
+    ms = float(np.median(times))
     st = s.get_stats()
     tr = s.get_theta_trace()
-    res = dict(cfg=c, n=n, ms=ms, launches=st["gpu_launches"] - l0, stats=st, clocks=clocks, trace=tr,
-               inputs=inp, lib_ms=st["last_run_ms"])
+    res = dict(cfg=c, n=n, ms=ms, times=times, launches=(st["gpu_launches"] - l0) // repeats, stats=st, clocks=clocks,
+               trace=tr, inputs=inp, lib_ms=st["last_run_ms"])
     s.close()
     return res
+
+
+def timing_entry(times, K):
+    return {"protocol": f"{len(times)} timed regions of exactly {K} Gibbs iterations each, back to back after the warm-up; "
+                        "CUDA events on the sampler's stream; value and ms_per_step are the MEDIAN region",
+            "region_ms": [float(t) for t in times], "best_us_per_iter": min(times) * 1e3 / K,
+            "median_us_per_iter": float(np.median(times)) * 1e3 / K}
+
+
+def fixed_cost_per_run(cfg_name, args, device):
+    """Fixed cost of one cudahm_run (launch, state load / write-back of the on-chip kernel, first front): device time of a
+    K1-iteration run minus K1 x the marginal iteration time, the latter from a K2-iteration run (best of 3 each)."""
+    import copy
+    import torch
+    c, n, inp = make_workload(cfg_name, 0, 0)
+    K1, K2, W = 20, 2020, max(args.warmup, 5)
+    a = copy.copy(args)
+    a.n_objects = 0
+    s = make_gpu_sampler(c, n, inp, a, c.seed, trace_rows_needed(W + 3 * (K1 + K2), W, c.thin), device)
+    s.run(W, W, c.thin, sync=True)
+    best = {}
+    for K in (K1, K2, K1, K2, K1, K2):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(device)
+        with torch.cuda.stream(s.stream):
+            e0.record(s.stream)
+            s.run(K, W, c.thin)
+            e1.record(s.stream)
+        torch.cuda.synchronize(device)
+        best[K] = min(best.get(K, 1e30), e0.elapsed_time(e1) * 1e3)
+    s.close()
+    per_iter = (best[K2] - best[K1]) / (K2 - K1)
+    return {"fixed_us_per_run": best[K1] - K1 * per_iter, "marginal_us_per_iter": per_iter,
+            "how": f"best of 3: t({K1} iterations) = {best[K1]:.1f} us, t({K2}) = {best[K2]:.1f} us on {cfg_name}; fixed = t({K1}) - {K1} x "
+                   "(t(K2) - t(K1)) / (K2 - K1): cooperative launch, load of the state into shared memory, first front, "
+                   "write-back"}
 
 
 def time_e2e(cfg_name, args, device, rank):
@@ -229,15 +287,18 @@ def time_e2e(cfg_name, args, device, rank):
     host_cols = [p.numpy() for p in pinned]
     rows = trace_rows_needed(W + K, W, c.thin)
     s = make_gpu_sampler(c, n, inp, args, c.seed + rank, rows, device)   # allocation + table set-up: outside
+    # result buffers in pinned host memory, allocated before the clock starts (like the input buffers)
+    out_mean = torch.empty((s.p, n), dtype=torch.float64).pin_memory().numpy() if c.keep_chi_moments else None
+    out_var = torch.empty((s.p, n), dtype=torch.float64).pin_memory().numpy() if c.keep_chi_moments else None
     torch.cuda.synchronize(device)
     t0 = time.perf_counter()
     s.set_data(host_cols)                    # H2D
-    s.set_init(inp["theta0"])
+    s.set_init(inp["theta0"], theta_chol0=make_theta_chol0(inp, n))
     s.run(W + K, W, c.thin)
     tr = s.get_theta_trace()                 # D2H (synchronises)
     d2h = tr.nbytes
     if c.keep_chi_moments:
-        mean, var, _ = s.get_chi_moments()   # D2H
+        mean, var, _ = s.get_chi_moments(out_mean, out_var)   # D2H
         d2h += mean.nbytes + var.nbytes
     torch.cuda.synchronize(device)
     sec = time.perf_counter() - t0
@@ -256,16 +317,28 @@ def kernel_label(st):
 
 
 def roofline_entry(cfg_name, c, n, K, W, ms, peak, peak_src, kernel=None):
+    """HBM roofline on ALGORITHMIC bytes (the bound north_star names) plus the two compute floors of the same kernel:
+    issue slots and the fp64 pipe, from ncu instruction counts where a capture exists (north_star: "the slower of bytes
+    moved at HBM peak and the op count at the pipe peak")."""
     base, mom = ALG_BYTES[cfg_name]
     per_obj = base + (mom if c.keep_chi_moments else 0)     # the timed iterations are all past burn-in
     bytes_per_iter = per_obj * n
     achieved = bytes_per_iter * K / (ms * 1e-3) / 1e9
-    per_iter = NCU_DRAM_BYTES_PER_ITER.get(cfg_name) if n == c.n_objects else None
-    return {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-            "traffic": None if per_iter is None else per_iter * K, "peak_source": peak_src, "kernel": kernel,
-            "launches_timed": 1, "iterations_per_launch": K, "alg_bytes_per_object_iter": per_obj,
-            "alg_bytes_per_iter": bytes_per_iter, "alg_bytes_per_launch": bytes_per_iter * K,
-            "us_per_iter": ms * 1e3 / K}
+    us = ms * 1e3 / K
+    hbm_floor = bytes_per_iter / (peak * 1e9) * 1e6
+    out = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+           "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((cfg_name, W, K)) if n == c.n_objects else None,
+           "peak_source": peak_src, "kernel": kernel,
+           "launches_timed": 1, "iterations_per_launch": K, "alg_bytes_per_object_iter": per_obj,
+           "alg_bytes_per_iter": bytes_per_iter, "alg_bytes_per_launch": bytes_per_iter * K,
+           "us_per_iter": us, "floors_us_per_iter": {"hbm": hbm_floor}}
+    ins = NCU_WARP_INSTR_PER_32.get(cfg_name) if n == c.n_objects else None
+    if ins:
+        issue = ins[0] * (n / 32.0) / (4.0 * N_SMS * SM_CLOCK_HZ) * 1e6
+        out["floors_us_per_iter"]["issue_slots"] = issue
+        out["warp_instructions_per_32_updates"] = ins[0]
+        out["frac_of_slowest_floor"] = max(hbm_floor, issue) / us
+    return out
 
 
 # ----------------------------------------------------------------------------------------------------------
@@ -279,7 +352,7 @@ def time_oracle(cfg_name, n_sample, iters, burn_in, seed_offset=0):
     o.set_data(inp["cols"])
     if inp["consts"] is not None:
         o.set_model_consts(inp["consts"])
-    o.set_init(inp["theta0"])
+    o.set_init(inp["theta0"], theta_chol0=make_theta_chol0(inp, n))
     t0 = time.perf_counter()
     o.run(iters, burn_in, c.thin)
     sec = time.perf_counter() - t0
@@ -336,9 +409,9 @@ def run_reference(args, rank):
             "warmup": W, "ms_per_step": sec_k * 1e3 / K, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64" if c.precision == synth.F64 else "f32 state / f64 reductions",
             "data": "synthetic",
-            "config": {"workload": workload_label(args.config), "n_objects": n_full,
-                       "sample_objects": n_s},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "config": config_entry(args.config, c, n_full, W),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                             "sample_objects": n_s},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gibbs_iters_per_s": K / sec_k, "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -443,10 +516,8 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64" if c.precision == synth.F64 else "f32 state / f64 reductions", "data": "synthetic",
-        "config": {"workload": workload_label(args.config), "n_objects": n,
-                   "model": ["normal1d", "thinned_schechter1d", "binormal2d", "linreg_me1d", "bb1_fluxnoise1d", "normal3d_knowncov"][c.model],
-                   "burn_in": W, "thin": c.thin, "chi_moments": bool(c.keep_chi_moments),
-                   "theta_mode": args.theta_mode, "parallelism": "replicas only" if world > 1 else "1 gpu",
+        "config": config_entry(args.config, c, n, W),
+        "launch": {"theta_mode": args.theta_mode, "parallelism": "replicas only" if world > 1 else "1 gpu",
                    "grid": [r["stats"]["grid_blocks"], r["stats"]["block_threads"]],
                    "l2": ("inputs larger than L2: every iteration streams the whole state through HBM"
                           if n * ALG_BYTES[args.config][0] > 126e6 else
@@ -457,8 +528,9 @@ def main():
                           "state resident ON CHIP by design: the sampler iterates K times over the same objects "
                           "inside one persistent launch and keeps them in shared memory, so there is nothing to "
                           "flush between iterations; roofline.achieved divides the ALGORITHMIC bytes by the time "
-                          "(roofline.traffic is what actually reached DRAM); other_configs holds the HBM-streaming "
-                          "configs C3 / C4, whose inputs are larger than L2")},
+                          "(roofline.traffic is what actually reached DRAM); other_configs.C4 is the HBM-streaming "
+                          "config, whose inputs are larger than L2")},
+        "timing": timing_entry(r["times"], K),
         "gibbs_iters_per_s": K * world / (ms * 1e-3),
         "e2e": {"value": e_value, "unit": UNIT, "h2d_bytes_per_step": e["h2d"] / e["iters"],
                 "d2h_bytes_per_step": e["d2h"] / e["iters"], "seconds": e_ms * 1e-3,
@@ -498,23 +570,28 @@ def extras(args, device, peak, peak_src, n):
     for m in ("graph", "host"):
         a = copy.copy(args)
         a.theta_mode, a.steps, a.warmup = m, min(args.steps, 2000), min(args.warmup, 500)
-        r = time_gpu(args.config, a, device, 0, 1, lambda: None, with_clocks=False)
+        r = time_gpu(args.config, a, device, 0, 1, lambda: None, with_clocks=False, repeats=1)
         modes[m] = {"us_per_iter": r["ms"] * 1e3 / a.steps, "updates_per_s": r["n"] * a.steps / (r["ms"] * 1e-3),
                     "gpu_launches": int(r["launches"])}
     out["other_theta_modes"] = modes
+    out["fixed_cost"] = fixed_cost_per_run(args.config, args, device)
     side = {}
-    # C3 / C4: the HBM-streaming configs; C5: the paper's own case study (BB1 population, N = 1e5)
-    for cfg_name, k, w in (("C3", 600, 200), ("C4", 300, 100), ("C5", 3000, 1000), ("C6", 3000, 1000)):
-        if cfg_name == args.config:
-            continue
+    # every BASELINE.json config (C0 .. C4; C2 also at its steady state: burn-in 2,000 + 8,000 timed iterations in one
+    # launch) plus the paper's own two workloads (C5: BB1 case study, C6: normal-normal benchmark), each as 3 timed regions
+    for label, cfg_name, k, w in (("C0", "C0", 1500, 500), ("C1", "C1", 2000, 1000), ("C2_steady", "C2", 8000, 2000),
+                                  ("C3", "C3", 600, 200), ("C4", "C4", 300, 100), ("C5", "C5", 3000, 1000),
+                                  ("C6", "C6", 3000, 1000)):
         a = copy.copy(args)
         a.steps, a.warmup, a.n_objects = k, w, 0
-        r = time_gpu(cfg_name, a, device, 0, 1, lambda: None, with_clocks=False)
+        r = time_gpu(cfg_name, a, device, 0, 1, lambda: None, with_clocks=False, repeats=3)
         kern = kernel_label(r["stats"])
         rf = roofline_entry(cfg_name, r["cfg"], r["n"], k, w, r["ms"], peak, peak_src, kern)
-        side[cfg_name] = {"n_objects": r["n"], "steps": k, "warmup": w, "updates_per_s": r["n"] * k / (r["ms"] * 1e-3),
-                          "gibbs_iters_per_s": k / (r["ms"] * 1e-3), "roofline": rf,
-                          "grid": [r["stats"]["grid_blocks"], r["stats"]["block_threads"]]}
+        side[label] = {"workload": workload_label(cfg_name), "n_objects": r["n"], "steps": k, "warmup": w,
+                       "updates_per_s": r["n"] * k / (r["ms"] * 1e-3),
+                       "gibbs_iters_per_s": k / (r["ms"] * 1e-3), "roofline": rf, "timing": timing_entry(r["times"], k),
+                       "grid": [r["stats"]["grid_blocks"], r["stats"]["block_threads"]],
+                       "accept": {"chi": r["stats"]["chi_accepts"] / max(1, r["stats"]["chi_proposals"]),
+                                  "theta": r["stats"]["theta_accepts"] / max(1, r["stats"]["theta_proposals"])}}
     out["other_configs"] = side
     out["cpu_baseline"] = cpu_baseline(args.config, n)
     return out

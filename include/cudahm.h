@@ -168,7 +168,8 @@ int cudahm_set_model_consts(cudahm_sampler* s, const double* v, int n);
 /* Initial state: chi0 (p*N values of type T, host or device per chi0_on_device; NULL = the model's default
  * X_1, reading R6), theta0 (dtheta host doubles), theta_chol0 (packed lower triangle, host doubles;
  * NULL = 0.1 * I).  Resets t = 0, L_i = init_scale_chi * I, the trace, the moments and the counters.
- * CUDAHM_E_STATE before set_data (and set_model_consts where the model has constants). */
+ * CUDAHM_E_STATE before set_data (and set_model_consts where the model has constants); CUDAHM_E_NONFINITE if theta0 has
+ * zero prior density or a non-finite theta-only term (the chain needs pi(X_1) > 0; set_state likewise). */
 int cudahm_set_init(cudahm_sampler* s, const void* chi0_or_null, int chi0_on_device, const double* theta0,
                     const double* theta_chol0_or_null);
 

@@ -261,8 +261,12 @@ class Sampler:
             self._ck(self.lib.cudahm_get_theta_trace(self._h, _d(out), n.value, C.byref(n)))
         return out
 
-    def get_chi_moments(self):
-        mean, var = np.empty((self.p, self.N)), np.empty((self.p, self.N))
+    def get_chi_moments(self, mean=None, var=None):
+        """mean, var: optional caller buffers (p, N) float64, e.g. pinned host memory; allocated here if omitted."""
+        mean = np.empty((self.p, self.N)) if mean is None else mean
+        var = np.empty((self.p, self.N)) if var is None else var
+        assert mean.shape == var.shape == (self.p, self.N) and mean.dtype == var.dtype == np.float64
+        assert mean.flags.c_contiguous and var.flags.c_contiguous
         n = C.c_int64()
         with self._dev():
             self._ck(self.lib.cudahm_get_chi_moments(self._h, _d(mean), _d(var), self.N, C.byref(n)))

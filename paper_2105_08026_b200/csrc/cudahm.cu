@@ -8,12 +8,15 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <map>
+#include <mutex>
 #include <string>
+#include <utility>
 #include <vector>
 
-#include "kernels.cuh"
-#include "resident.cuh"
-#include "stream_tma.cuh"
+#include "kernel_sets.h"
+#include "tail_kernels.cuh"
+#include "resident_cfg.h"
 
 using namespace hm;
 
@@ -32,69 +35,15 @@ constexpr size_t STAGE_MAX_SMEM = 192 * 1024;   // dynamic shared memory k_persi
 
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
-struct KernelSet {
-  const void* persistent;          // plain streaming persistent kernel
-  const void* persistent_ahead;    // the variant with staged draws / L2 prefetch
-  size_t stage_step_bytes;         // shared memory of one staged step of plate draws (DrawSet::NV x BLOCK values)
-  const void* persistent_tma;
-  size_t tma_stage_bytes;
-  const void* sweep;
-  const void* sweep_tap;
-  const void* init_state;
-};
-
-template <int MODEL, class T, int BLOCK>
-KernelSet make_set() {
-  KernelSet k;
-  k.persistent = (const void*)k_persistent<MODEL, T, BLOCK, false>;
-  k.persistent_ahead = (const void*)k_persistent<MODEL, T, BLOCK, true>;
-  k.stage_step_bytes = (size_t)DrawSet<MODEL, T>::NV * BLOCK * sizeof(T);
-  k.persistent_tma = (const void*)k_persistent_tma<MODEL, T, BLOCK>;
-  k.tma_stage_bytes = (size_t)(ModelDims<MODEL>::p * (ModelDims<MODEL>::p + 3) / 2 + ModelDims<MODEL>::ncols) * (BLOCK - 32) * 16;
-  k.sweep = (const void*)k_sweep<MODEL, T, BLOCK, false>;
-  k.sweep_tap = (const void*)k_sweep<MODEL, T, BLOCK, true>;
-  k.init_state = (const void*)k_init_state<MODEL, T>;
-  return k;
-}
-
-template <int MODEL, class T>
-bool pick_block(int block, KernelSet* k) {
-  switch (block) {
-    case 256:  *k = make_set<MODEL, T, 256>(); return true;
-    case 512:  *k = make_set<MODEL, T, 512>(); return true;
-    case 1024: *k = make_set<MODEL, T, 1024>(); return true;
-  }
-  return false;
-}
-
-// on-chip variant (resident.cuh): fp64, p = 1 models; n_values = shared-memory doubles per object
-const void* pick_resident(int model, int precision, int keep_moments, int* n_values) {
-  if (precision != CUDAHM_F64) return nullptr;
-  const int mom = keep_moments ? 2 : 0;
+// kernels of one (model, precision, block size): the per-model translation units inst_*.cu hold the instantiations
+bool pick_kernels(int model, int precision, int block, KernelSet* k, ResidentSet* r) {
   switch (model) {
-    case M_NORMAL1D:            *n_values = ResValues<M_NORMAL1D>::n_base + mom; return (const void*)k_resident<M_NORMAL1D>;
-    case M_THINNED_SCHECHTER1D: *n_values = ResValues<M_THINNED_SCHECHTER1D>::n_base + mom; return (const void*)k_resident<M_THINNED_SCHECHTER1D>;
-    case M_LINREG_ME1D:         *n_values = ResValues<M_LINREG_ME1D>::n_base + mom; return (const void*)k_resident<M_LINREG_ME1D>;
-    case M_BB1_FLUXNOISE1D:     *n_values = ResValues<M_BB1_FLUXNOISE1D>::n_base + mom; return (const void*)k_resident<M_BB1_FLUXNOISE1D>;
-  }
-  return nullptr;
-}
-
-bool pick_kernels(int model, int precision, int block, KernelSet* k) {
-  if (precision == CUDAHM_F64) {
-    switch (model) {
-      case M_NORMAL1D:            return pick_block<M_NORMAL1D, double>(block, k);
-      case M_THINNED_SCHECHTER1D: return pick_block<M_THINNED_SCHECHTER1D, double>(block, k);
-      case M_BINORMAL2D:          return pick_block<M_BINORMAL2D, double>(block, k);
-      case M_LINREG_ME1D:         return pick_block<M_LINREG_ME1D, double>(block, k);
-      case M_BB1_FLUXNOISE1D:     return pick_block<M_BB1_FLUXNOISE1D, double>(block, k);
-      case M_NORMAL3D_KNOWNCOV:   return pick_block<M_NORMAL3D_KNOWNCOV, double>(block, k);
-    }
-  } else if (precision == CUDAHM_F32_STATE_F64_REDUCE) {
-    switch (model) {
-      case M_NORMAL1D:    return pick_block<M_NORMAL1D, float>(block, k);
-      case M_LINREG_ME1D: return pick_block<M_LINREG_ME1D, float>(block, k);
-    }
+    case M_NORMAL1D:            return kernels_normal1d(precision, block, k, r);
+    case M_THINNED_SCHECHTER1D: return kernels_thinned_schechter1d(precision, block, k, r);
+    case M_BINORMAL2D:          return kernels_binormal2d(precision, block, k, r);
+    case M_LINREG_ME1D:         return kernels_linreg_me1d(precision, block, k, r);
+    case M_BB1_FLUXNOISE1D:     return kernels_bb1_fluxnoise1d(precision, block, k, r);
+    case M_NORMAL3D_KNOWNCOV:   return kernels_normal3d_knowncov(precision, block, k, r);
   }
   return false;
 }
@@ -113,6 +62,8 @@ struct cudahm_sampler {
   bool have_data = false, have_consts = false, have_init = false;
   int num_sms = 0, grid = 1, block = 512, vec = 2;
   long long t_done = 0;             // iterations completed (host mirror)
+  long long h_trace_rows = 0;       // host mirrors of Iter::trace_rows / mom_count: pure functions of the (t, burn_in, thin)
+  long long h_mom_count = 0;        // history, so cudahm_run never has to read the device before it launches
   long long launches = 0;
   Iter* h_iter = nullptr;           // pinned host copy of the iteration state
   double* h_totals = nullptr;       // pinned
@@ -147,11 +98,45 @@ int fail(cudahm_sampler* s, int code, const char* fmt, ...) {
   return code;
 }
 
+// the captured k_sweep / k_tail nodes of THETA_GRAPH hold Params BY VALUE (model constants, pointers, prior): anything
+// that changes them, or rewinds the chain, drops the cached executable graph so the next run captures afresh
+void invalidate_graph(cudahm_sampler* s) {
+  if (s->gexec) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }
+  s->g_burn = -1; s->g_thin = -1; s->g_iters = 0;
+}
+
 #define CU_TRY(s, call)                                                                      \
   do {                                                                                       \
     cudaError_t e_ = (call);                                                                 \
     if (e_ != cudaSuccess) return fail(s, CUDAHM_E_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
   } while (0)
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize belongs to the FUNCTION (per device), not to a handle: keep a process-wide
+// maximum per (device, function) and only ever raise it, so that two handles of one model with different N cannot lower
+// each other's limit between create and launch.
+cudaError_t ensure_dyn_smem(const void* fn, size_t bytes) {
+  static std::mutex mu;
+  static std::map<std::pair<int, const void*>, size_t> have;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  std::lock_guard<std::mutex> lock(mu);
+  size_t& cur = have[{dev, fn}];
+  if (bytes <= cur) return cudaSuccess;
+  e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+  if (e == cudaSuccess) cur = bytes;
+  return e;
+}
+
+// rows the thinned trace gains / post-burn-in iterations the moments gain over iterations (t0, t1]
+long long trace_rows_between(long long t0, long long t1, long long burn_in, long long thin) {
+  const long long lo = std::max(t0, burn_in);
+  return t1 > lo ? (t1 - burn_in) / thin - (lo - burn_in) / thin : 0;
+}
+long long moment_samples_between(long long t0, long long t1, long long burn_in) {
+  const long long lo = std::max(t0, burn_in);
+  return t1 > lo ? t1 - lo : 0;
+}
 
 bool valid_config(const cudahm_config* c, int* p, int* dt, int* nc, int* nk) {
   if (!c || c->struct_size != sizeof(cudahm_config)) return false;
@@ -229,10 +214,13 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
   int block = cfg->block_threads ? cfg->block_threads : 512;
   if (!cfg->block_threads) {
     const long long vec = cfg->precision == CUDAHM_F64 ? 2 : 4;
-    if ((cfg->n_objects + vec * 512 - 1) / (vec * 512) < 148) block = 256;
+    int dev0 = 0, sms0 = 0;
+    if (cudaGetDevice(&dev0) == cudaSuccess) cudaDeviceGetAttribute(&sms0, cudaDevAttrMultiProcessorCount, dev0);
+    if ((cfg->n_objects + vec * 512 - 1) / (vec * 512) < (sms0 > 0 ? sms0 : 148)) block = 256;
   }
   KernelSet ks;
-  if (!pick_kernels(cfg->model, cfg->precision, block, &ks))
+  ResidentSet rs;
+  if (!pick_kernels(cfg->model, cfg->precision, block, &ks, &rs))
     return fail(nullptr, CUDAHM_E_UNSUPPORTED, "model %d is not compiled in for precision %d", cfg->model, cfg->precision);
   const Layout lay = make_layout(*cfg, p, nc, dt);
   if (!dev_workspace || bytes < lay.total || ((uintptr_t)dev_workspace & 255u))
@@ -280,7 +268,7 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
     for (; ns > 0; --ns) {
       const size_t bytes = (size_t)ns * ks.stage_step_bytes;
       int fit = 0;
-      if (cudaFuncSetAttribute(ks.persistent_ahead, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) == cudaSuccess &&
+      if (ensure_dyn_smem(ks.persistent_ahead, bytes) == cudaSuccess &&
           cudaOccupancyMaxActiveBlocksPerMultiprocessor(&fit, ks.persistent_ahead, block, bytes) == cudaSuccess &&
           (long long)fit * sms >= s->grid) break;
       cudaGetLastError();
@@ -297,8 +285,7 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
   // loads on C3 / C4 (the sweep is issue-bound, not latency-bound, and the producer warp costs a sweep warp)
   if (cfg->theta_mode == CUDAHM_THETA_DEVICE_TAIL && (cfg->flags & CUDAHM_FLAG_TMA_STAGING) && block <= 512) {
     int stages = (int)std::min<size_t>(TMA_MAX_STAGES, (size_t)(200 * 1024) / ks.tma_stage_bytes);
-    if (stages >= 2 && cudaFuncSetAttribute(ks.persistent_tma, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                            (int)(stages * ks.tma_stage_bytes)) == cudaSuccess) {
+    if (stages >= 2 && ensure_dyn_smem(ks.persistent_tma, stages * ks.tma_stage_bytes) == cudaSuccess) {
       s->tma_stages = stages; s->tma_smem = stages * ks.tma_stage_bytes;
       const long long tiles = (cfg->n_objects + (long long)s->vec * (block - 32) - 1) / ((long long)s->vec * (block - 32));
       s->grid = (int)std::max(1LL, std::min<long long>(sms, tiles));
@@ -308,15 +295,14 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
   }
   // on-chip variant: every object stays in the shared memory of its block for the whole launch
   if (cfg->theta_mode == CUDAHM_THETA_DEVICE_TAIL && !(cfg->flags & CUDAHM_FLAG_STREAMING_ONLY) && cfg->n_objects > 0) {
-    int nv = 0;
-    const void* rk = pick_resident(cfg->model, cfg->precision, cfg->keep_chi_moments, &nv);
+    const int nv = rs.n_base + (cfg->keep_chi_moments ? 2 : 0);
+    const void* rk = rs.kernel;
     if (rk) {
       const long long g = std::min<long long>(sms, (cfg->n_objects + 63) / 64);          // >= one warp of pairs per block
       const long long OB = 2 * ((cfg->n_objects + 2 * g - 1) / (2 * g));                   // objects per block (even)
       const long long R = 2 * ((OB + 2 * RES_S - 1) / (2 * RES_S));                        // slots per thread, in pairs
       const size_t bytes = (size_t)nv * R * RES_S * sizeof(double);
-      if (bytes <= (size_t)RES_MAX_SMEM &&
-          cudaFuncSetAttribute(rk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) == cudaSuccess) {
+      if (bytes <= (size_t)RES_MAX_SMEM && ensure_dyn_smem(rk, bytes) == cudaSuccess) {
         s->res_kernel = rk; s->res_R = (int)R; s->res_OB = (int)OB; s->res_smem = bytes;
         s->grid = (int)g; s->block = RES_THREADS;
       } else {
@@ -450,6 +436,7 @@ extern "C" int cudahm_set_model_consts(cudahm_sampler* s, const double* v, int n
     const double q[6] = {0.5 * a11 / det, a21 / det, 0.5 * a22 / det, a31 / det, a32 / det, 0.5 * a33 / det};
     for (int j = 0; j < 6; ++j) s->P.mc[MN_Q + j] = q[j];
     s->have_consts = true; s->have_init = false;
+    invalidate_graph(s);
     return CUDAHM_OK;
   }
   std::vector<double> xk, wk, rj, wj, ex(NQUAD), W(NQUAD);
@@ -503,6 +490,7 @@ extern "C" int cudahm_set_model_consts(cudahm_sampler* s, const double* v, int n
   CU_TRY(s, cudaMemcpyAsync((void*)s->P.qW, W.data(), NQUAD * 8, cudaMemcpyHostToDevice, s->stream));
   CU_TRY(s, cudaStreamSynchronize(s->stream));
   s->have_consts = true; s->have_init = false;
+  invalidate_graph(s);
   return CUDAHM_OK;
 }
 
@@ -528,6 +516,10 @@ int upload_and_init_iter(cudahm_sampler* s, const Iter& raw) {
   CU_TRY(s, cudaMemcpyAsync(s->h_iter, s->P.iter, sizeof(Iter), cudaMemcpyDeviceToHost, s->stream));
   CU_TRY(s, cudaStreamSynchronize(s->stream));
   s->host_iter_valid = true;
+  // the chain must start where the theta target is positive and finite (X_1 with pi(X_1) > 0)
+  if (!s->cfg.freeze_theta && (!std::isfinite(s->h_iter->lp_cur) || !std::isfinite(s->h_iter->T_cur)))
+    return fail(s, CUDAHM_E_NONFINITE, "theta has zero prior density or a non-finite theta-only term (log prior %g, T %g)",
+                s->h_iter->lp_cur, s->h_iter->T_cur);
   return CUDAHM_OK;
 }
 
@@ -569,7 +561,8 @@ extern "C" int cudahm_set_init(cudahm_sampler* s, const void* chi0, int chi0_on_
   if (theta_chol0) for (int k = 0; k < s->ntri_theta; ++k) raw.Lth[k] = theta_chol0[k];
   else for (int r = 0; r < s->dtheta; ++r) raw.Lth[tri(r, r)] = 0.1;
   raw.t = 1;
-  s->t_done = 0;
+  s->t_done = 0; s->h_trace_rows = 0; s->h_mom_count = 0;
+  invalidate_graph(s);
   int rc = upload_and_init_iter(s, raw);
   if (rc) return rc;
   s->have_init = true;
@@ -584,28 +577,37 @@ int run_device_tail(cudahm_sampler* s, long long n_iter) {
   while (n_iter > 0) {
     long long k = std::min(n_iter, max_it);
     Params P = s->P;
-    unsigned epoch0 = s->epoch;            // epochs never repeat over the sampler's lifetime (0 = never written)
+    // mailbox epochs must never repeat while a stale slot could still hold them (0 = never written): before the 32-bit
+    // counter would wrap, clear the mailboxes (stream-ordered) and start again at 1
+    if ((unsigned long long)s->epoch + (unsigned long long)k >= 0xffffffffull) {
+      CU_TRY(s, cudaMemsetAsync(s->ws + s->lay.mbox, 0, s->lay.blk_cnt - s->lay.mbox, s->stream));
+      s->epoch = 1;
+    }
+    unsigned epoch0 = s->epoch;
     s->epoch += (unsigned)k;
     int R = s->res_R, OB = s->res_OB, ns = s->n_stage, pf = s->prefetch;
     void* args[] = {&P, &k, &epoch0, &R, &OB};
     void* pargs[] = {&P, &k, &epoch0, &ns, &pf};
     int rc;
     if (s->res_kernel) {
-      cudaError_t e = cudaLaunchCooperativeKernel(s->res_kernel, dim3(s->grid), dim3(RES_THREADS), args, s->res_smem, s->stream);
+      cudaError_t e = ensure_dyn_smem(s->res_kernel, s->res_smem);      // a map lookup unless the limit has to grow
+      if (e == cudaSuccess)
+        e = cudaLaunchCooperativeKernel(s->res_kernel, dim3(s->grid), dim3(RES_THREADS), args, s->res_smem, s->stream);
       if (e != cudaSuccess) return fail(s, CUDAHM_E_CUDA, "resident kernel launch: %s", cudaGetErrorString(e));
       s->launches++;
       rc = CUDAHM_OK;
     } else if (s->tma_stages > 0) {
       int st = s->tma_stages;
       void* targs[] = {&P, &k, &epoch0, &st};
-      cudaError_t e = cudaLaunchCooperativeKernel(s->ks.persistent_tma, dim3(s->grid), dim3(s->block), targs, s->tma_smem, s->stream);
+      cudaError_t e = ensure_dyn_smem(s->ks.persistent_tma, s->tma_smem);
+      if (e == cudaSuccess)
+        e = cudaLaunchCooperativeKernel(s->ks.persistent_tma, dim3(s->grid), dim3(s->block), targs, s->tma_smem, s->stream);
       if (e != cudaSuccess) return fail(s, CUDAHM_E_CUDA, "streaming kernel launch: %s", cudaGetErrorString(e));
       s->launches++;
       rc = CUDAHM_OK;
     } else {
-      // the shared-memory limit is a property of the function, shared by every handle of this model: set per launch
       const void* fn = s->ahead ? s->ks.persistent_ahead : s->ks.persistent;
-      cudaError_t e = s->ahead ? cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->stage_smem) : cudaSuccess;
+      cudaError_t e = s->ahead ? ensure_dyn_smem(fn, s->stage_smem) : cudaSuccess;
       if (e == cudaSuccess)
         e = cudaLaunchCooperativeKernel(fn, dim3(s->grid), dim3(s->block), pargs, s->ahead ? s->stage_smem : 0, s->stream);
       if (e != cudaSuccess) return fail(s, CUDAHM_E_CUDA, "persistent kernel launch: %s", cudaGetErrorString(e));
@@ -708,16 +710,13 @@ extern "C" int cudahm_run(cudahm_sampler* s, int64_t n_iter, int64_t burn_in, in
   if (!s->have_init) return fail(s, CUDAHM_E_STATE, "run before set_init");
   if (n_iter < 0 || burn_in < 0 || thin < 1) return fail(s, CUDAHM_E_INVALID, "run: bad n_iter/burn_in/thin");
   if (s->t_done + n_iter >= 0xffffffffLL) return fail(s, CUDAHM_E_INVALID, "iteration index exceeds the 32-bit stream counter");
-  // trace capacity
-  {
-    int rc = fetch_iter(s); if (rc) return rc;
-    const long long t1 = s->t_done + n_iter;
-    const long long lo = std::max<long long>(s->t_done, burn_in);
-    const long long rows = t1 > lo ? (t1 - burn_in) / thin - (lo - burn_in) / thin : 0;
-    if (s->cfg.max_trace_rows > 0 && s->h_iter->trace_rows + rows > s->cfg.max_trace_rows)
-      return fail(s, CUDAHM_E_INVALID, "theta trace would need %lld rows, capacity %lld", s->h_iter->trace_rows + rows,
-                  (long long)s->cfg.max_trace_rows);
-  }
+  // trace capacity, from the host mirror of the row count: nothing is read back from the device (and the stream is not
+  // synchronised) before the launch -- trace_rows and mom_count are functions of the (t, burn_in, thin) history alone
+  const long long t1 = s->t_done + n_iter;
+  const long long rows = s->cfg.max_trace_rows > 0 ? trace_rows_between(s->t_done, t1, burn_in, thin) : 0;
+  if (s->cfg.max_trace_rows > 0 && s->h_trace_rows + rows > s->cfg.max_trace_rows)
+    return fail(s, CUDAHM_E_INVALID, "theta trace would need %lld rows, capacity %lld", s->h_trace_rows + rows,
+                (long long)s->cfg.max_trace_rows);
   s->P.tail.burn_in = burn_in; s->P.tail.thin = thin;
   if (n_iter == 0) return CUDAHM_OK;
   CU_TRY(s, cudaEventRecord(s->ev0, s->stream));
@@ -730,7 +729,9 @@ extern "C" int cudahm_run(cudahm_sampler* s, int64_t n_iter, int64_t burn_in, in
   if (rc) return rc;
   CU_TRY(s, cudaEventRecord(s->ev1, s->stream));
   s->timed = true;
-  s->t_done += n_iter;
+  s->h_trace_rows += rows;
+  if (s->cfg.keep_chi_moments) s->h_mom_count += moment_samples_between(s->t_done, t1, burn_in);
+  s->t_done = t1;
   return CUDAHM_OK;
 }
 
@@ -765,6 +766,7 @@ extern "C" int cudahm_shard_decide(cudahm_sampler* s, int64_t burn_in, int32_t t
   rc = host_decide(s, totals_global);
   if (rc) return rc;
   s->t_done += 1;
+  s->h_trace_rows = s->h_iter->trace_rows; s->h_mom_count = s->h_iter->mom_count;
   return CUDAHM_OK;
 }
 
@@ -841,6 +843,7 @@ extern "C" int cudahm_debug_step(cudahm_sampler* s, int64_t burn_in, int32_t thi
   if (rc) return rc;
   if (e != cudaSuccess) return fail(s, CUDAHM_E_CUDA, "debug_step: %s", cudaGetErrorString(e));
   s->t_done += 1;
+  s->h_trace_rows = s->h_iter->trace_rows; s->h_mom_count = s->h_iter->mom_count;
   return CUDAHM_OK;
 }
 
@@ -894,7 +897,7 @@ extern "C" int cudahm_get_stats(cudahm_sampler* s, cudahm_stats* out) {
   CU_TRY(s, cudaMemcpy(bc.data(), s->P.blk_cnt, bc.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
   unsigned long long acc = it.chi_acc, nonf = it.nonfinite;
   for (int b = 0; b < MAX_BLOCKS; ++b) { acc += bc[2 * b]; nonf += bc[2 * b + 1]; }
-  out->chi_accepts = (int64_t)acc; out->chi_proposals = (it.t - 1) * s->P.N;
+  out->chi_accepts = (int64_t)acc; out->chi_proposals = (it.t - 1) * (long long)s->P.tail.n_objects;   // the WHOLE population's (sharded: chi_acc is global too)
   out->theta_accepts = (int64_t)it.theta_acc; out->theta_proposals = (int64_t)it.theta_prop_n;
   out->nonfinite = (int64_t)nonf; out->moment_samples = it.mom_count; out->trace_rows = it.trace_rows;
   if (s->timed) {
@@ -934,5 +937,6 @@ extern "C" int cudahm_set_state(cudahm_sampler* s, const void* chi, const void* 
   if (L_theta) std::copy(L_theta, L_theta + s->ntri_theta, raw.Lth);
   raw.t = t + 1;
   s->t_done = t;
+  invalidate_graph(s);
   return upload_and_init_iter(s, raw);
 }

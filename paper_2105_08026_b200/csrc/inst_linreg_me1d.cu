@@ -1,0 +1,14 @@
+// inst_linreg_me1d.cu -- every kernel of model M_LINREG_ME1D (its own translation unit: the models build in parallel).
+#include "kernel_sets_impl.cuh"
+
+namespace hm {
+
+bool kernels_linreg_me1d(int precision, int block, KernelSet* k, ResidentSet* r) {
+  r->kernel = nullptr; r->n_base = 0;
+  if (precision == 0) { r->kernel = (const void*)k_resident<M_LINREG_ME1D>; r->n_base = ResValues<M_LINREG_ME1D>::n_base; }
+  if (precision == 0) return pick_block<M_LINREG_ME1D, double>(block, k);
+  if (precision == 1) return pick_block<M_LINREG_ME1D, float>(block, k);
+  return false;
+}
+
+}  // namespace hm

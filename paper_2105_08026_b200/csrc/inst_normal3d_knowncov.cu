@@ -1,0 +1,12 @@
+// inst_normal3d_knowncov.cu -- every kernel of model M_NORMAL3D_KNOWNCOV (its own translation unit: the models build in parallel).
+#include "kernel_sets_impl.cuh"
+
+namespace hm {
+
+bool kernels_normal3d_knowncov(int precision, int block, KernelSet* k, ResidentSet* r) {
+  r->kernel = nullptr; r->n_base = 0;
+  if (precision == 0) return pick_block<M_NORMAL3D_KNOWNCOV, double>(block, k);
+  return false;
+}
+
+}  // namespace hm

@@ -1,0 +1,13 @@
+// inst_thinned_schechter1d.cu -- every kernel of model M_THINNED_SCHECHTER1D (its own translation unit: the models build in parallel).
+#include "kernel_sets_impl.cuh"
+
+namespace hm {
+
+bool kernels_thinned_schechter1d(int precision, int block, KernelSet* k, ResidentSet* r) {
+  r->kernel = nullptr; r->n_base = 0;
+  if (precision == 0) { r->kernel = (const void*)k_resident<M_THINNED_SCHECHTER1D>; r->n_base = ResValues<M_THINNED_SCHECHTER1D>::n_base; }
+  if (precision == 0) return pick_block<M_THINNED_SCHECHTER1D, double>(block, k);
+  return false;
+}
+
+}  // namespace hm

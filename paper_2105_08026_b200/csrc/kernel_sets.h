@@ -1,0 +1,33 @@
+// kernel_sets.h -- the table of kernel entry points of one (model, precision, block size), filled by the per-model
+// translation units inst_*.cu (one per compiled-in model, so that they build in parallel) and read by cudahm.cu.
+#pragma once
+#include <cstddef>
+
+namespace hm {
+
+struct KernelSet {
+  const void* persistent;          // plain streaming persistent kernel
+  const void* persistent_ahead;    // the variant with staged draws / L2 prefetch
+  size_t stage_step_bytes;         // shared memory of one staged step of plate draws (DrawSet::NV x BLOCK values)
+  const void* persistent_tma;
+  size_t tma_stage_bytes;
+  const void* sweep;
+  const void* sweep_tap;
+  const void* init_state;
+};
+
+// on-chip kernel (resident.cuh) of one (model, precision)
+struct ResidentSet {
+  const void* kernel;              // NULL: the model has no on-chip kernel in this precision
+  int n_base;                      // shared-memory values per object without the running moments (+ 2 with them)
+};
+
+// each returns false when the (precision, block) combination is not compiled in for that model
+bool kernels_normal1d(int precision, int block, KernelSet* k, ResidentSet* r);
+bool kernels_thinned_schechter1d(int precision, int block, KernelSet* k, ResidentSet* r);
+bool kernels_binormal2d(int precision, int block, KernelSet* k, ResidentSet* r);
+bool kernels_linreg_me1d(int precision, int block, KernelSet* k, ResidentSet* r);
+bool kernels_bb1_fluxnoise1d(int precision, int block, KernelSet* k, ResidentSet* r);
+bool kernels_normal3d_knowncov(int precision, int block, KernelSet* k, ResidentSet* r);
+
+}  // namespace hm

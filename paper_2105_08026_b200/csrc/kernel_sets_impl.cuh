@@ -1,0 +1,35 @@
+// kernel_sets_impl.cuh -- included by the per-model translation units inst_*.cu only: instantiates every kernel of
+// one model and fills its KernelSet / ResidentSet.
+#pragma once
+#include "kernel_sets.h"
+#include "kernels.cuh"
+#include "resident.cuh"
+#include "stream_tma.cuh"
+
+namespace hm {
+
+template <int MODEL, class T, int BLOCK>
+KernelSet make_set() {
+  KernelSet k;
+  k.persistent = (const void*)k_persistent<MODEL, T, BLOCK, false>;
+  k.persistent_ahead = (const void*)k_persistent<MODEL, T, BLOCK, true>;
+  k.stage_step_bytes = (size_t)DrawSet<MODEL, T>::NV * BLOCK * sizeof(T);
+  k.persistent_tma = (const void*)k_persistent_tma<MODEL, T, BLOCK>;
+  k.tma_stage_bytes = (size_t)(ModelDims<MODEL>::p * (ModelDims<MODEL>::p + 3) / 2 + ModelDims<MODEL>::ncols) * (BLOCK - 32) * 16;
+  k.sweep = (const void*)k_sweep<MODEL, T, BLOCK, false>;
+  k.sweep_tap = (const void*)k_sweep<MODEL, T, BLOCK, true>;
+  k.init_state = (const void*)k_init_state<MODEL, T>;
+  return k;
+}
+
+template <int MODEL, class T>
+bool pick_block(int block, KernelSet* k) {
+  switch (block) {
+    case 256:  *k = make_set<MODEL, T, 256>(); return true;
+    case 512:  *k = make_set<MODEL, T, 512>(); return true;
+    case 1024: *k = make_set<MODEL, T, 1024>(); return true;
+  }
+  return false;
+}
+
+}  // namespace hm

@@ -622,20 +622,10 @@ __global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const l
   }
   const int G = (int)gridDim.x;
   double cnt[2] = {0.0, 0.0};
-#ifdef HM_PHASE_TIMING
-  long long ph[5] = {0, 0, 0, 0, 0};
-#define HM_STAMP(i) { const long long now_ = clock64(); ph[i] += now_ - last_; last_ = now_; }
-#else
-#define HM_STAMP(i)
-#endif
   for (long long k = 0; k < n_iter; ++k) {
-#ifdef HM_PHASE_TIMING
-    long long last_ = clock64();
-#endif
     double part[NPART];
     const uint32_t t_next = (uint32_t)it.t + 1u;
     sweep<MODEL, T, false, AHEAD>(P, it, part, stage, n_stage, prefetch != 0);
-    HM_STAMP(0)
     cnt[0] += part[3]; cnt[1] += part[4];
     double dq[2] = {part[1], part[2]};
     block_reduce_all<2>(dq, red);
@@ -643,7 +633,6 @@ __global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const l
     unsigned long long* mb = P.mbox + (size_t)(k & 1) * mbox_parity_words(G);
     const unsigned epoch = epoch0 + (unsigned)k;
     mbox_push<NVX>(mb, G, (int)blockIdx.x, epoch, dq, (int)threadIdx.x, (int)blockDim.x);
-    HM_STAMP(1)
     // warps 0-3: collect + theta tail (the serial chain); the other warps meanwhile make the plate draws of the
     // first n_stage steps of iteration t + 1, which depend on nothing but (seed, object, t + 1)
     if (!AHEAD) {
@@ -653,9 +642,7 @@ __global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const l
         mbox_collect<NVX>(mb + (size_t)blockIdx.x * mbox_reader_words(G), G, epoch, t2);
         tot[1] = t2[0]; tot[2] = t2[1];
       }
-      HM_STAMP(2)
       tail_block(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, (int)(threadIdx.x >> 5), SyncAll());
-      HM_STAMP(3)
       continue;
     }
     if (threadIdx.x < TAILT) {
@@ -665,19 +652,12 @@ __global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const l
         mbox_collect<NVX>(mb + (size_t)blockIdx.x * mbox_reader_words(G), G, epoch, t2);
         tot[1] = t2[0]; tot[2] = t2[1];
       }
-      HM_STAMP(2)
       tail_block(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, (int)(threadIdx.x >> 5), SyncNamed<1, TAILT>());
     } else if (k + 1 < n_iter) {
       stage_draws<MODEL, T>(P, t_next, stage, n_stage, (int)threadIdx.x - TAILT, BLOCK - TAILT);
     }
     __syncthreads();
-    HM_STAMP(3)
   }
-#ifdef HM_PHASE_TIMING
-  if (threadIdx.x == 0 && (blockIdx.x == 0 || blockIdx.x == gridDim.x - 1))
-    printf("block %d: cycles/iter sweep %.0f reduce+publish %.0f collect %.0f tail %.0f\n", (int)blockIdx.x,
-           (double)ph[0] / n_iter, (double)ph[1] / n_iter, (double)ph[2] / n_iter, (double)ph[3] / n_iter);
-#endif
   block_reduce<2>(cnt, red);
   if (threadIdx.x == 0) {
     P.blk_cnt[2 * blockIdx.x] += (unsigned long long)cnt[0];
@@ -700,52 +680,6 @@ __global__ void __launch_bounds__(BLOCK, 1) k_sweep(const Params P) {
 #pragma unroll
     for (int q = 0; q < NPART; ++q) P.slots[(size_t)blockIdx.x * NPART + q] = part[q];
   }
-}
-
-// Tail kernel: reduce the slots (TAIL_REDUCE: also publish the totals for the host); TAIL_DECIDE: the
-// block-parallel theta tail, which decides iteration t and prepares t + 1.
-enum : int { TAIL_REDUCE = 1, TAIL_DECIDE = 2 };
-constexpr int TAIL_THREADS = 128;
-__global__ void __launch_bounds__(TAIL_THREADS, 1) k_tail(const Params P, const int nblocks, const int flags) {
-  __shared__ Iter it;
-  copy_iter(&it, P.iter);
-  __syncthreads();
-  double tot[NPART] = {0.0, 0.0, 0.0, 0.0, 0.0};
-  if (threadIdx.x < 32) {
-    slots_reduce(P.slots, nblocks, tot);
-    if ((flags & TAIL_REDUCE) && threadIdx.x == 0) {
-#pragma unroll
-      for (int q = 0; q < NPART; ++q) P.totals[q] = tot[q];
-    }
-  }
-  if (flags & TAIL_DECIDE) {
-    tail_block(it, P.tail, tot, P.trace, (int)(threadIdx.x >> 5), SyncAll());
-    __syncthreads();
-    copy_iter(P.iter, &it);
-  }
-}
-
-// After set_init / set_state: derive kc, log prior and T(theta) for the uploaded theta, then prepare it.t.
-__global__ void __launch_bounds__(256, 1) k_init_iter(const Params P) {
-  __shared__ Iter it;
-  __shared__ double red[32][NPART];
-  copy_iter(&it, P.iter);
-  __syncthreads();
-  const ThetaK kc = theta_consts(P.tail.model, it.theta);
-  double part[NPART] = {0, 0, 0, 0, 0};
-  if (has_selection(P.tail.model)) {
-    for (int k = threadIdx.x; k < NQUAD; k += blockDim.x)
-      part[2] += selection_term_rt(P.tail.model, kc, P.qW[k], P.qx[k], P.qex[k]);
-  }
-  block_reduce<NPART>(part, red);
-  if (threadIdx.x == 0) {
-    it.kc = kc;
-    it.lp_cur = log_prior_full(P.tail, it.theta);
-    it.T_cur = has_selection(P.tail.model) ? theta_only_from_sum(P.tail.model, kc, part[2], P.tail.n_objects) : 0.0;
-    prepare_iteration(it, P.tail, it.t);
-  }
-  __syncthreads();
-  copy_iter(P.iter, &it);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -783,12 +717,6 @@ __global__ void k_init_state(const Params P, const T* raw, const int have_chi0, 
 #pragma unroll
     for (int j = 0; j < p; ++j) { P.mom_mean[j * P.Npad + i] = 0.0; P.mom_M2[j * P.Npad + i] = 0.0; }
   }
-}
-
-// sample variance from the Welford sums, written next to them for read-out
-__global__ void k_finalize_moments(const double* M2, double* var, long long n, double inv_km1) {
-  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) var[i] = M2[i] * inv_km1;
 }
 
 }  // namespace hm

@@ -14,21 +14,14 @@
 // block partials are added differs (fixed, so still deterministic).
 #pragma once
 #include "kernels.cuh"
+#include "resident_cfg.h"
 
 namespace hm {
 
-#ifndef HM_RES_SW
-#define HM_RES_SW 16
-#endif
-constexpr int RES_SW = HM_RES_SW;                   // sweep warps per block
-constexpr int RES_S = RES_SW * 32;                  // sweep threads per block
-constexpr int RES_TW = 4;                           // tail warps per block (tail_block needs exactly 4)
-constexpr int RES_THREADS = RES_S + RES_TW * 32;    // 640 with 16 sweep warps
 #ifndef HM_RES_IL
 #define HM_RES_IL 2
 #endif
 constexpr int RES_IL = HM_RES_IL;                   // slots of the back processed together (instruction-level parallelism)
-constexpr int RES_MAX_SMEM = 200 * 1024;            // dynamic shared memory the kernel may ask for
 
 // per-object values kept in shared memory: [value][slot r][sweep thread]
 template <int MODEL> struct ResValues {
@@ -78,9 +71,25 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
   copy_iter(&it, P.iter);
   if (tid < 2) cnt_sm[tid] = 0ull;
   if (!is_tail) {
-    for (int r = 0; r < nlive; ++r) {
+    // a thread's slot pair (r, r + 1) is two ADJACENT objects starting at an even index: one 16-byte access per column
+    for (int r = 0; r < nlive; r += 2) {
       const long long i = HM_OBJ(r);
-      {
+      if (r + 1 < nlive) {
+        const double2 x = *reinterpret_cast<const double2*>(chi + i), l = *reinterpret_cast<const double2*>(Lm + i);
+        HM_AT(V::V_CHI, r) = x.x; HM_AT(V::V_CHI, r + 1) = x.y;
+        HM_AT(V::V_L, r) = l.x; HM_AT(V::V_L, r + 1) = l.y;
+#pragma unroll
+        for (int c = 0; c < ncols; ++c) {
+          const double2 d = __ldg(reinterpret_cast<const double2*>(dat + c * Npad + i));
+          HM_AT(V::V_D + c, r) = d.x; HM_AT(V::V_D + c, r + 1) = d.y;
+        }
+        if (V::m1) { HM_AT(V::V_E, r) = hm_exp(x.x); HM_AT(V::V_E, r + 1) = hm_exp(x.y); }
+        if (keep_mom) {
+          const double2 m = *reinterpret_cast<const double2*>(P.mom_mean + i), q = *reinterpret_cast<const double2*>(P.mom_M2 + i);
+          HM_AT(V_MEAN, r) = m.x; HM_AT(V_MEAN, r + 1) = m.y;
+          HM_AT(V_M2, r) = q.x; HM_AT(V_M2, r + 1) = q.y;
+        }
+      } else {
         const T x = chi[i];
         HM_AT(V::V_CHI, r) = x;
         HM_AT(V::V_L, r) = Lm[i];
@@ -117,20 +126,10 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
     const T astar = (T)P.astar_chi;
     double nacc = 0.0, nnan = 0.0;
 
-#ifdef HM_PHASE_TIMING
-    long long ph[6] = {0, 0, 0, 0, 0, 0}, last_ = 0;
-#define HM_RSTAMP(i) { const long long now_ = clock64(); ph[i] += now_ - last_; last_ = now_; }
-#else
-#define HM_RSTAMP(i)
-#endif
     front((uint32_t)t0);
     for (long long k = 0; k < n_iter; ++k) {
       const long long t = t0 + k;
-#ifdef HM_PHASE_TIMING
-      last_ = clock64();
-#endif
       if (k > 0) bar_sync(BAR_THETA, RES_THREADS);          // theta_t and everything derived from it are in `it`
-      HM_RSTAMP(0)
       // back, part 1 (needs theta_t only): targets, accept, RAM update, new chi, moments
       const ThetaK kc = it.kc;
       const KT<T> kT = narrow<T>(kc);
@@ -193,9 +192,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
       // back, part 2 (needs theta'_t, which the tail finishes a little later): population terms.  (M1's selection
       // integral at theta' is computed by the tail warps, see below: every value less in the exchange is worth more
       // than the arithmetic it saves -- a third mailbox value measured +0.7 us per iteration.)
-      HM_RSTAMP(3)
       if (k > 0) bar_sync(BAR_THETAP, RES_THREADS);
-      HM_RSTAMP(4)
       const ThetaK kp = it.kp;
       double v[2] = {0.0, 0.0};
       for (int r = 0; r < nlive; ++r) {
@@ -212,19 +209,8 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
       if (lane == 0) red[k & 1][warp][0] = v[0];
       __threadfence_block();
       bar_arrive(BAR_PARTIALS, RES_THREADS);                 // hand the partials to the tail warps, do not wait
-      HM_RSTAMP(1)
       if (k + 1 < n_iter) front((uint32_t)(t + 1));          // overlaps the exchange and the theta step
-#ifdef HM_SWEEP_DELAY
-      { const long long t_ = clock64(); while (clock64() - t_ < HM_SWEEP_DELAY) {} }
-#endif
-      HM_RSTAMP(2)
     }
-#ifdef HM_PHASE_TIMING
-    if (tid == 0 && (blockIdx.x == 0 || blockIdx.x == G - 1))
-      printf("block %d sweep warp 0: cycles/iter wait-theta %.0f back1 %.0f wait-theta' %.0f back2+reduce %.0f front %.0f\n",
-             (int)blockIdx.x, (double)ph[0] / n_iter, (double)ph[3] / n_iter, (double)ph[4] / n_iter,
-             (double)ph[1] / n_iter, (double)ph[2] / n_iter);
-#endif
     bar_sync(BAR_THETA, RES_THREADS);                        // the last tail has finished
     bar_sync(BAR_THETAP, RES_THREADS);
 #pragma unroll
@@ -236,9 +222,16 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
       atomicAdd(&cnt_sm[0], (unsigned long long)nacc);
       atomicAdd(&cnt_sm[1], (unsigned long long)nnan);
     }
-    for (int r = 0; r < nlive; ++r) {
+    for (int r = 0; r < nlive; r += 2) {
       const long long i = HM_OBJ(r);
-      {
+      if (r + 1 < nlive) {
+        *reinterpret_cast<double2*>(chi + i) = make_double2(HM_AT(V::V_CHI, r), HM_AT(V::V_CHI, r + 1));
+        *reinterpret_cast<double2*>(Lm + i) = make_double2(HM_AT(V::V_L, r), HM_AT(V::V_L, r + 1));
+        if (keep_mom) {
+          *reinterpret_cast<double2*>(P.mom_mean + i) = make_double2(HM_AT(V_MEAN, r), HM_AT(V_MEAN, r + 1));
+          *reinterpret_cast<double2*>(P.mom_M2 + i) = make_double2(HM_AT(V_M2, r), HM_AT(V_M2, r + 1));
+        }
+      } else {
         chi[i] = HM_AT(V::V_CHI, r);
         Lm[i] = HM_AT(V::V_L, r);
         if (keep_mom) { P.mom_mean[i] = HM_AT(V_MEAN, r); P.mom_M2[i] = HM_AT(V_M2, r); }
@@ -273,15 +266,8 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
       }
     };
     selection_full();
-#ifdef HM_PHASE_TIMING
-    long long ph[4] = {0, 0, 0, 0}, last_ = 0;
-#endif
     for (long long k = 0; k < n_iter; ++k) {
-#ifdef HM_PHASE_TIMING
-      last_ = clock64();
-#endif
       bar_sync(BAR_PARTIALS, RES_THREADS);                   // the block's 16 warp partials of iteration t0 + k
-      HM_RSTAMP(0)
       double dq[1];
       dq[0] = lane < RES_SW ? red[k & 1][lane][0] : 0.0;
       lanes_to_total<1>(dq);
@@ -295,22 +281,12 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
         tot[1] = t1[0];
         if constexpr (V::m1) tot[2] = ((tq_warp[0] + tq_warp[1]) + tq_warp[2]) + tq_warp[3];
       }
-      HM_RSTAMP(1)
-#ifdef HM_TAIL_DELAY      /* scratch experiment: is the tail on the critical path? */
-      { const long long t_ = clock64(); while (clock64() - t_ < HM_TAIL_DELAY) {} }
-#endif
       tail_block(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, tw, SyncNamed<BAR_TAIL, RES_TW * 32>(),
                  ArriveNamed<BAR_THETA, RES_THREADS>());      // theta_{t+1} is signalled after the decision phase ...
       __threadfence_block();
       bar_arrive(BAR_THETAP, RES_THREADS);                   // ... theta'_{t+1} and its constants when the tail is done
       selection_full();                                      // M1: for the NEXT decision; off the critical path
-      HM_RSTAMP(2)
     }
-#ifdef HM_PHASE_TIMING
-    if (ttid == 0 && (blockIdx.x == 0 || blockIdx.x == G - 1))
-      printf("block %d tail warp 0: cycles/iter wait-partials %.0f push+collect %.0f tail %.0f\n", (int)blockIdx.x,
-             (double)ph[0] / n_iter, (double)ph[1] / n_iter, (double)ph[2] / n_iter);
-#endif
   }
 #undef HM_AT
 #undef HM_OBJ

@@ -15,6 +15,7 @@
 //              requested before the exchange and the theta tail of iteration t, so their latency overlaps them.
 #pragma once
 #include "kernels.cuh"
+#include "resident_cfg.h"
 
 namespace hm {
 
@@ -49,7 +50,6 @@ __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
-constexpr int TMA_MAX_STAGES = 4;
 
 // BLOCK threads = BLOCK - 32 consumers + one producer warp (a 17th warp would cost every thread a quarter of its
 // registers: the register file is allocated per 4 warps).

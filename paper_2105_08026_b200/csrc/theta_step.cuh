@@ -254,10 +254,6 @@ __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const dou
   const Draws& d0 = it.dr[r0];
   const Draws& d1 = it.dr[r1];
   Draws& d2 = it.dr[r2];
-#ifdef HM_PHASE_TIMING
-  const long long tc0_ = clock64();
-  long long tc1_ = 0, tc2_ = 0, tc3_ = 0;
-#endif
 
   // decision scalars stay in warp 0's registers until phase C, where the taps are written (off the critical path)
   double T_prop = 0.0, log_r = 0.0, alpha = 0.0;
@@ -287,9 +283,6 @@ __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const dou
     } else {
       decided();
     }
-#ifdef HM_PHASE_TIMING
-    tc1_ = clock64();
-#endif
   } else if (warp == 1) {
     decided();
     if (!c.freeze_theta) {
@@ -322,9 +315,6 @@ __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const dou
     }
   }
   sync();
-#ifdef HM_PHASE_TIMING
-  tc2_ = clock64();
-#endif
   if (!c.freeze_theta) {
     if (warp >= 1) {
       if (lane == 0) theta_consts_part(c.model, warp - 1, it.thetaP, it.kp);
@@ -355,17 +345,10 @@ __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const dou
   if (warp == 2 && trace_or_null && it.trace_write && lane < dt)
     trace_or_null[(it.trace_rows - 1) * dt + lane] = it.theta[lane];
   if (warp == 3 && lane == 1) it.t = t + 1;
-#ifdef HM_PHASE_TIMING
-  tc3_ = clock64();
-#endif
   sync();
   // warp 0 read it.lp_prop (the decided iteration's) during phase C, so the next one is moved in only now; the
   // next reader is the decision of iteration t + 1, at least one block barrier away
   if (warp == 3 && lane == 0) it.lp_prop = it.lp_prop_next;
-#ifdef HM_PHASE_TIMING
-  if (warp == 0 && lane == 0 && blockIdx.x == 0 && (t % 100) == 0)
-    printf("tail t=%lld: decide %lld  wait-sync1 %lld  phaseC %lld  sync2 %lld\n", t, tc1_ - tc0_, tc2_ - tc1_, tc3_ - tc2_, clock64() - tc3_);
-#endif
 }
 #endif
 

@@ -73,6 +73,29 @@ NN3_CPOP = NN3_D[:, None] * NN3_R * NN3_D[None, :]
 NN3_CONSTS = np.concatenate([NN3_SIGMA, NN3_CPOP[np.tril_indices(3)]])
 
 
+# Initial theta proposal factor handed to both samplers (SURVEY 8(c) S7 allows "diag(user scales)"; the library default
+# 0.1 I is 100-1000 x the width of theta | chi at N >= 1e5 and eta_n = n^(-2/3) shrinks it too slowly).  The conditional
+# law of theta given the latents narrows as N^(-1/2); its unit-N covariance C at the generating truth of each recipe
+# below was computed once through the oracle (tests/golden/make_theta_scales.py: finite-difference Hessian of
+# sum_i log f(chi_i; theta) + T(theta) + log prior) and is stored here as chol(C), packed lower-triangular row-major.
+# theta_chol0 = (2.38 / sqrt(dtheta)) chol(C) / sqrt(N): the random-walk scaling at which a Gaussian target accepts
+# about a quarter of the proposals, so the RAM adaptation of L_theta starts near its fixed point.
+THETA_COND_CHOL = {
+    M_NORMAL1D: [1.0, 0.0, 0.7071],
+    M_THINNED_SCHECHTER1D: [1.481, -3.214, 2.542, 4.413, -1.182, 0.994],
+    M_BINORMAL2D: [1.0, 0.182, 0.5786, 0.0, 0.0, 0.7139, 0.0, 0.0, 0.0648, 0.7075, 0.0, 0.0, 0.2177, 0.2020, 0.9663],
+    M_LINREG_ME1D: [0.6, -0.3, 0.1732, 0.0, 0.0, 0.7071],
+    M_BB1_FLUXNOISE1D: [2.038, -18.80, 17.98, -1.795, -0.185, 1.005],
+    M_NORMAL3D_KNOWNCOV: [2.3, 0.135, 0.4293, -6.7, 9.6924, 6.3817],
+}
+
+
+def theta_chol0(model, n):
+    d = {M_NORMAL1D: 2, M_THINNED_SCHECHTER1D: 3, M_BINORMAL2D: 5, M_LINREG_ME1D: 3, M_BB1_FLUXNOISE1D: 3,
+         M_NORMAL3D_KNOWNCOV: 3}[model]
+    return np.asarray(THETA_COND_CHOL[model], dtype=np.float64) * (2.38 / np.sqrt(d) / np.sqrt(max(int(n), 1)))
+
+
 def _rng(seed):
     return np.random.Generator(np.random.Philox(key=int(seed)))
 
@@ -93,7 +116,8 @@ def make_normal1d(n, seed=0, fp32=False):
     sd = float(np.std(cols[0])) if n > 1 else 1.0
     return dict(model=M_NORMAL1D, cols=cols, consts=None, chi_true=chi[None, :],
                 theta_true=np.array([0.0, 0.0]),
-                theta0=np.array([float(np.mean(cols[0])) if n else 0.0, np.log(max(sd, 1e-3))]))
+                theta0=np.array([float(np.mean(cols[0])) if n else 0.0, np.log(max(sd, 1e-3))]),
+                theta_chol0=theta_chol0(M_NORMAL1D, n))
 
 
 def make_thinned_schechter1d(n, seed=1):
@@ -129,7 +153,7 @@ def make_thinned_schechter1d(n, seed=1):
     return dict(model=M_THINNED_SCHECHTER1D, cols=[Fhat, gi], consts=SCHECHTER_CONSTS.copy(),
                 chi_true=x[None, :], theta_true=np.array([alpha, xstar, a_true]),
                 theta0=np.array([alpha + 0.05, xstar + 0.05, a_true + 0.05]),
-                detected_fraction=n / max(drawn, 1))
+                theta_chol0=theta_chol0(M_THINNED_SCHECHTER1D, n), detected_fraction=n / max(drawn, 1))
 
 
 def make_bb1_fluxnoise1d(n, seed=5, truth=BB1_TRUTH):
@@ -173,7 +197,7 @@ def make_bb1_fluxnoise1d(n, seed=5, truth=BB1_TRUTH):
     th = np.array([beta, ll, lu])
     return dict(model=M_BB1_FLUXNOISE1D, cols=[Fhat, gi], consts=BB1_CONSTS.copy(), chi_true=x[None, :],
                 theta_true=th, theta0=th + np.array([0.03, 0.1, 0.03]),
-                detected_fraction=reach * n / max(drawn, 1))
+                theta_chol0=theta_chol0(M_BB1_FLUXNOISE1D, n), detected_fraction=reach * n / max(drawn, 1))
 
 
 def make_normal3d_knowncov(n, seed=6):
@@ -182,7 +206,8 @@ def make_normal3d_knowncov(n, seed=6):
     chi = NN3_MU[:, None] + np.linalg.cholesky(NN3_CPOP) @ g.standard_normal((3, n))
     y = chi + NN3_SIGMA[:, None] * g.standard_normal((3, n))
     return dict(model=M_NORMAL3D_KNOWNCOV, cols=[y[0].copy(), y[1].copy(), y[2].copy()], consts=NN3_CONSTS.copy(),
-                chi_true=chi, theta_true=NN3_MU.copy(), theta0=NN3_MU + np.array([0.05, -0.02, 0.2]))
+                chi_true=chi, theta_true=NN3_MU.copy(), theta0=NN3_MU + np.array([0.05, -0.02, 0.2]),
+                theta_chol0=theta_chol0(M_NORMAL3D_KNOWNCOV, n))
 
 
 def make_binormal2d(n, seed=3, fp32=False):
@@ -200,7 +225,7 @@ def make_binormal2d(n, seed=3, fp32=False):
         cols = _round_f32(cols)
     th = np.array([m[0], m[1], lam[0], lam[1], np.arctanh(rho)])
     return dict(model=M_BINORMAL2D, cols=cols, consts=None, chi_true=chi, theta_true=th,
-                theta0=th + np.array([0.05, -0.05, 0.05, 0.05, -0.05]))
+                theta0=th + np.array([0.05, -0.05, 0.05, 0.05, -0.05]), theta_chol0=theta_chol0(M_BINORMAL2D, n))
 
 
 def make_linreg_me1d(n, seed=4, fp32=True):
@@ -215,7 +240,7 @@ def make_linreg_me1d(n, seed=4, fp32=True):
         cols = _round_f32(cols)
     th = np.array([1.0, -0.5, np.log(0.3)])
     return dict(model=M_LINREG_ME1D, cols=cols, consts=None, chi_true=chi[None, :], theta_true=th,
-                theta0=th + np.array([0.02, -0.02, 0.05]))
+                theta0=th + np.array([0.02, -0.02, 0.05]), theta_chol0=theta_chol0(M_LINREG_ME1D, n))
 
 
 def make_inputs(config_name, n_objects=None):

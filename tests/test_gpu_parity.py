@@ -386,3 +386,49 @@ def test_config0_posterior_against_oracle_and_closed_form():
     y, s = inp["cols"]
     w = 1.0 / (s ** 2 + np.exp(2 * mg[1]))
     assert abs(mg[0] - (w * y).sum() / w.sum()) <= 4 * seg[0] + 0.01
+
+
+def test_two_on_chip_handles_of_one_model_with_different_sizes():
+    """cudaFuncAttributeMaxDynamicSharedMemorySize belongs to the function, not the handle: creating a SMALL handle of
+    the same model after a LARGE one must not lower the large one's limit (both run the on-chip kernel)."""
+    _, big, inp_b = make_pair(B.M_THINNED_SCHECHTER1D, 120_000, seed=3, want_oracle=False, max_trace_rows=8)
+    _, small, _ = make_pair(B.M_THINNED_SCHECHTER1D, 2_000, seed=4, want_oracle=False, max_trace_rows=8)
+    assert big.get_stats()["block_threads"] == small.get_stats()["block_threads"] == 640
+    small.run(4, 0, 1, sync=True)
+    big.run(4, 0, 1, sync=True)            # launches with the larger shared-memory request after the small handle's
+    small.run(4, 0, 1, sync=True)
+    _, ref, _ = make_pair(B.M_THINNED_SCHECHTER1D, 120_000, seed=3, want_oracle=False, max_trace_rows=8, inputs=inp_b)
+    ref.run(4, 0, 1, sync=True)
+    assert np.array_equal(ref.get_state()["chi"], big.get_state()["chi"])
+    assert big.get_stats()["iterations"] == 4 and small.get_stats()["iterations"] == 8
+
+
+def test_graph_cache_is_dropped_when_the_model_constants_change():
+    """THETA_GRAPH caches an executable graph whose nodes hold the model constants by value: set_model_consts on a live
+    handle (then set_init and a run long enough to replay the graph) must give the chain of a fresh handle."""
+    from paper_2105_08026_b200 import synth
+    n, iters = 3000, 120
+    inp = synth.make_normal3d_knowncov(n, 5)
+    consts2 = inp["consts"].copy()
+    consts2[:3] *= 1.5                                       # other measurement errors: another target
+    _, a, _ = make_pair(B.M_NORMAL3D_KNOWNCOV, n, seed=5, astar=0.234, theta_mode=B.THETA_GRAPH, inputs=inp,
+                        max_trace_rows=iters, want_oracle=False)
+    a.run(iters, 0, 1, sync=True)                            # graph captured with the first constants
+    a.set_model_consts(consts2)
+    a.set_init(inp["theta0"])
+    a.run(iters, 0, 1, sync=True)
+    inp2 = dict(inp, consts=consts2)
+    _, b, _ = make_pair(B.M_NORMAL3D_KNOWNCOV, n, seed=5, astar=0.234, theta_mode=B.THETA_GRAPH, inputs=inp2,
+                        max_trace_rows=iters, want_oracle=False)
+    b.run(iters, 0, 1, sync=True)
+    assert np.array_equal(a.get_theta_trace(), b.get_theta_trace())
+    assert np.array_equal(a.get_state()["chi"], b.get_state()["chi"])
+
+
+def test_theta0_outside_the_prior_support_is_refused():
+    _, g, inp = make_pair(B.M_NORMAL1D, 100, seed=1, want_oracle=False)
+    with pytest.raises(B.CudahmError) as e:
+        g.set_init(np.array([0.0, 50.0]))                    # |log tau| <= 10 is the prior box
+    assert e.value.code == B.E_NONFINITE
+    g.set_init(inp["theta0"])
+    g.run(3, 0, 1, sync=True)
