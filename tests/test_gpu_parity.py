@@ -28,10 +28,10 @@ IDS = ["M0-f64", "M1-f64", "M2-f64", "M3-f64", "M0-f32", "M3-f32", "M4-f64", "M5
 @pytest.mark.parametrize("model,precision,astar,n", CASES, ids=IDS)
 def test_single_step_fed_state(model, precision, astar, n):
     """One iteration from identical state: every tap of SURVEY 8(c) protocol (i)."""
-    orc, gpu, _ = make_pair(model, n, seed=11 + model, precision=precision, astar=astar, block_threads=256)
+    orc, gpu, inp = make_pair(model, n, seed=11 + model, precision=precision, astar=astar, block_threads=256)
     st = sync_gpu_to_oracle(orc, gpu)
     to, tg = orc.step(NO_TRACE, 1, taps=True), gpu.debug_step(NO_TRACE, 1)
-    nm = compare_step(to, tg, precision, st, what=f"model {model}")
+    nm = compare_step(to, tg, precision, st, what=f"model {model}", ctx=dict(model=model, inputs=inp, astar=astar))
     compare_theta_step(to, tg, what=f"model {model}")
     assert nm == 0 or precision != B.F64, "an fp64 near tie in the very first step is (almost surely) a bug"
     if nm == 0:
@@ -43,12 +43,13 @@ def test_lockstep_trajectory(model, precision, astar, n):
     """Protocol (ii): lock-step for 60 iterations with taps; accept sequences identical outside the tie band;
     the GPU is re-fed the oracle's state after every iteration in fp32 (per-decision disagreement is expected
     there) and only after a counted in-band divergence in fp64."""
-    orc, gpu, _ = make_pair(model, n, seed=21 + model, precision=precision, astar=astar, block_threads=256)
+    orc, gpu, inp = make_pair(model, n, seed=21 + model, precision=precision, astar=astar, block_threads=256)
     ties = 0
+    ctx = dict(model=model, inputs=inp, astar=astar)
     st = sync_gpu_to_oracle(orc, gpu)
     for it in range(60):
         to, tg = orc.step(NO_TRACE, 1, taps=True), gpu.debug_step(NO_TRACE, 1)
-        nm = compare_step(to, tg, precision, st, what=f"model {model} it {it}")
+        nm = compare_step(to, tg, precision, st, what=f"model {model} it {it}", ctx=ctx)
         compare_theta_step(to, tg, what=f"model {model} it {it}", rel=1e-9 if precision == B.F64 else 1e-6)
         ties += nm
         if precision == B.F64 and nm == 0 and to["accepted_theta"] == tg["accepted_theta"]:
@@ -312,11 +313,11 @@ def test_resume_is_bit_exact():
 @pytest.mark.parametrize("precision", [B.F64, B.F32_STATE_F64_REDUCE], ids=["f64", "f32"])
 def test_ragged_and_degenerate_sizes(n, precision):
     """Empty, single-object and ragged-tail populations (vector tails, partial warps)."""
-    orc, gpu, _ = make_pair(B.M_NORMAL1D, n, seed=3, precision=precision, astar=0.44, max_trace_rows=16)
+    orc, gpu, inp = make_pair(B.M_NORMAL1D, n, seed=3, precision=precision, astar=0.44, max_trace_rows=16)
     if n > 0:
         st = sync_gpu_to_oracle(orc, gpu)
         to, tg = orc.step(taps=True), gpu.debug_step()
-        compare_step(to, tg, precision, st, what=f"N={n}")
+        compare_step(to, tg, precision, st, what=f"N={n}", ctx=dict(model=B.M_NORMAL1D, inputs=inp, astar=0.44))
         sync_gpu_to_oracle(orc, gpu)
     gpu.run(8, 0, 1, sync=True)
     orc.run(8, 0, 1)
@@ -328,10 +329,10 @@ def test_ragged_and_degenerate_sizes(n, precision):
 @pytest.mark.parametrize("n", [1, 2, 3, 5, 63, 65, 513])
 def test_ragged_sizes_p3(n):
     """The p = 3 path (general rank-one update, two Box-Muller pairs per object) on ragged and tiny populations."""
-    orc, gpu, _ = make_pair(B.M_NORMAL3D_KNOWNCOV, n, seed=4, astar=0.234, max_trace_rows=16)
+    orc, gpu, inp = make_pair(B.M_NORMAL3D_KNOWNCOV, n, seed=4, astar=0.234, max_trace_rows=16)
     st = sync_gpu_to_oracle(orc, gpu)
     to, tg = orc.step(taps=True), gpu.debug_step()
-    compare_step(to, tg, B.F64, st, what=f"N={n}")
+    compare_step(to, tg, B.F64, st, what=f"N={n}", ctx=dict(model=B.M_NORMAL3D_KNOWNCOV, inputs=inp, astar=0.234))
     sync_gpu_to_oracle(orc, gpu)
     gpu.run(8, 0, 1, sync=True)
     orc.run(8, 0, 1)

@@ -215,16 +215,13 @@ def test_plate_stationary_law_bb1_against_grid():
     assert chain.min() >= c[2] and chain.max() <= c[3]
 
 
-def test_theta_posterior_bb1_against_eq_4_3_grid():
+def check_bb1_posterior(inp, tr, grid=(41, 81, 41)):
     """The (beta, ln l, ln u) chain against a direct grid of the paper's likelihood, Eq. 4.3-4.4:
     L(theta) = prod_i [int dx rho(x; theta) l_i(x)] / I(theta)^N, times the prior of Eq. 5.5 -- written here in numpy
     from the equations with its own quadratures (trapezoid in x, Gauss-Legendre in ln r)."""
-    n, burn, T = 100, 8000, 100000
-    s, inp = _sampler(n, 41, truth=(-1.3, np.log(0.3), 0.0))
     c = inp["consts"]
-    s.run(burn + T, burn_in=burn)
-    tr = s.get_theta_trace()
     Fh, g = inp["cols"]
+    n = Fh.size
     # G(x) on the test's own grid
     qr, wq = np.polynomial.legendre.leggauss(400)
     a_, b_ = np.log(c[4]), np.log(c[5])
@@ -239,9 +236,9 @@ def test_theta_posterior_bb1_against_eq_4_3_grid():
     sg = np.sqrt(c[0] ** 2 + (c[1] * F) ** 2)
     lik = np.exp(stats.norm.logpdf(Fh[:, None], F, sg) - stats.norm.logpdf(0.0, 0.0, c[0])) * dloc
     lo, hi = tr.min(0), tr.max(0)
-    be = np.linspace(max(lo[0] - 0.1, -1.999), min(hi[0] + 0.1, -1e-3), 41)
-    ll = np.linspace(lo[1] - 1.0, hi[1] + 0.3, 81)
-    lu = np.linspace(lo[2] - 0.2, hi[2] + 0.3, 41)
+    be = np.linspace(max(lo[0] - 0.1, -1.999), min(hi[0] + 0.1, -1e-3), grid[0])
+    ll = np.linspace(lo[1] - 1.0, hi[1] + 0.3, grid[1])
+    lu = np.linspace(lo[2] - 0.2, hi[2] + 0.3, grid[2])
     Lg, Ll = np.exp(xg), np.exp(loc)
     num = np.einsum("ik,aik,bik,cik->abci", lik, np.exp((be[:, None, None] + 1) * loc[None]),
                     -np.expm1(-Ll[None] / np.exp(ll)[:, None, None]), np.exp(-Ll[None] / np.exp(lu)[:, None, None]),
@@ -265,3 +262,10 @@ def test_theta_posterior_bb1_against_eq_4_3_grid():
         assert (wk[0] < 2e-3 * wk.max() or k == 1 or ax[0] <= -1.99) and wk[-1] < 2e-3 * wk.max(), "grid too narrow"
         assert abs(mean[k] - m) <= 4 * mse[k] + 0.02 * sd, f"theta[{k}] mean {mean[k]} vs grid {m} (sd {sd}, mcse {mse[k]})"
         assert abs(var[k] - sd ** 2) <= 4 * vse[k] + 0.06 * sd ** 2, f"theta[{k}] var {var[k]} vs grid {sd ** 2}"
+
+
+def test_theta_posterior_bb1_against_eq_4_3_grid():
+    n, burn, T = 100, 8000, 100000
+    s, inp = _sampler(n, 41, truth=(-1.3, np.log(0.3), 0.0))
+    s.run(burn + T, burn_in=burn)
+    check_bb1_posterior(inp, s.get_theta_trace())

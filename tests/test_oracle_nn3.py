@@ -81,15 +81,10 @@ def test_plate_stationary_law_is_the_conjugate_normal():
     assert np.all(np.abs(k / k.mean(1, keepdims=True) - 1) < 0.5)
 
 
-def test_theta_posterior_is_the_closed_form():
+def check_nn3_posterior(inp, tr):
     """mu | y ~ N(ybar, (C_pop + diag sigma_j^2)/N) with the uniform hyperprior of PAPER.md:166."""
-    n, burn, T = 30, 20000, 150000
-    inp = synth.make_normal3d_knowncov(n, seed=52)
-    s = O.Sampler(M5, n, seed=52, target_accept_chi=0.234)
-    s.set_data(inp["cols"]); s.set_model_consts(inp["consts"]); s.set_init(inp["theta0"])
-    s.run(burn + T, burn_in=burn)
-    tr = s.get_theta_trace()
     y = np.array(inp["cols"])
+    n = y.shape[1]
     S = (synth.NN3_CPOP + np.diag(synth.NN3_SIGMA ** 2)) / n
     mean, mse, var, vse = mean_and_var_with_mcse(tr)
     sd = np.sqrt(np.diag(S))
@@ -98,3 +93,12 @@ def test_theta_posterior_is_the_closed_form():
     cr = (tr[:, 0] - y[0].mean()) * (tr[:, 2] - y[2].mean())
     cm, cse, _, _ = mean_and_var_with_mcse(cr)
     assert abs(cm[0] - S[0, 2]) <= 4 * cse[0] + 0.03 * sd[0] * sd[2]
+
+
+def test_theta_posterior_is_the_closed_form():
+    n, burn, T = 30, 20000, 150000
+    inp = synth.make_normal3d_knowncov(n, seed=52)
+    s = O.Sampler(M5, n, seed=52, target_accept_chi=0.234)
+    s.set_data(inp["cols"]); s.set_model_consts(inp["consts"]); s.set_init(inp["theta0"])
+    s.run(burn + T, burn_in=burn)
+    check_nn3_posterior(inp, s.get_theta_trace())

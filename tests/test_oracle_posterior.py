@@ -154,8 +154,23 @@ def _grid_moments(logpost, axes):
     return np.array(means), np.array(sds)
 
 
-def test_theta_posterior_normal1d_against_marginal_grid():
+def check_normal1d_posterior(inp, tr):
     """P9: integrating chi out, y_i ~ N(mu, s_i^2 + tau^2); exact 2-D grid over (mu, log tau), flat prior."""
+    y, sig = inp["cols"]
+    m0, s0 = tr.mean(0), tr.std(0)
+    mu = np.linspace(m0[0] - 7 * s0[0], m0[0] + 7 * s0[0], 301); lam = np.linspace(m0[1] - 7 * s0[1], m0[1] + 7 * s0[1], 301)
+    lp = np.zeros((mu.size, lam.size))
+    for lo in range(0, y.size, 64):
+        yy, ss = y[lo:lo + 64], sig[lo:lo + 64]
+        V = ss[None, None, :] ** 2 + np.exp(2 * lam)[None, :, None]
+        lp += (-0.5 * np.log(V) - 0.5 * (yy[None, None, :] - mu[:, None, None]) ** 2 / V).sum(-1)
+    gm, gs = _grid_moments(lp, [mu, lam])
+    mean, mse, var, vse = mean_and_var_with_mcse(tr)
+    _assert_within(mean, mse, gm, floor=1e-3 * gs.max(), what="theta mean")
+    _assert_within(var, vse, gs ** 2, floor=1e-3 * gs.max() ** 2, what="theta variance")
+
+
+def test_theta_posterior_normal1d_against_marginal_grid():
     n, burn, T = 200, 4000, 50000
     inp = synth.make_normal1d(n, seed=35)
     s = O.Sampler(0, n, seed=35, target_accept_chi=0.44, target_accept_theta=0.234)
@@ -163,50 +178,42 @@ def test_theta_posterior_normal1d_against_marginal_grid():
     s.run(burn + T, burn_in=burn, thin=1)
     tr = s.get_theta_trace()
     assert tr.shape == (T, 2)
-    y, sig = inp["cols"]
-    mu = np.linspace(-0.6, 0.6, 401); lam = np.linspace(-1.0, 0.6, 401)
-    V = sig[None, None, :] ** 2 + np.exp(2 * lam)[None, :, None]
-    lp = (-0.5 * np.log(V) - 0.5 * (y[None, None, :] - mu[:, None, None]) ** 2 / V).sum(-1)
-    gm, gs = _grid_moments(lp, [mu, lam])
-    mean, mse, var, vse = mean_and_var_with_mcse(tr)
-    _assert_within(mean, mse, gm, floor=1e-4, what="theta mean")
-    _assert_within(var, vse, gs ** 2, floor=1e-3 * gs.max() ** 2, what="theta variance")
+    check_normal1d_posterior(inp, tr)
     st = s.get_stats()
     assert 0.1 < st["theta_accepts"] / st["theta_proposals"] < 0.4      # RAM on theta homes in on 0.234
 
 
+def check_linreg_posterior(inp, tr, npts=81):
+    """P12 (M3): y_i ~ N(a + b z_i, s_i^2 + tau^2); exact 3-D grid."""
+    y, sig, z = inp["cols"]
+    m0, s0 = tr.mean(0), tr.std(0)
+    axes = [np.linspace(m0[k] - 6 * s0[k], m0[k] + 6 * s0[k], npts) for k in range(3)]
+    A, Bm, Lm = np.meshgrid(*axes, indexing="ij")
+    e2 = np.exp(2 * Lm)
+    lp = np.zeros_like(A)
+    for i in range(y.size):
+        V = sig[i] ** 2 + e2
+        lp += -0.5 * np.log(V) - 0.5 * (y[i] - A - Bm * z[i]) ** 2 / V
+    gm, gs = _grid_moments(lp, axes)
+    mean, mse, var, vse = mean_and_var_with_mcse(tr)
+    _assert_within(mean, mse, gm, floor=2e-3 * gs.max(), what="theta mean")
+    _assert_within(var, vse, gs ** 2, floor=2e-3 * gs.max() ** 2, what="theta variance")
+
+
 @pytest.mark.parametrize("prec", [O.F64, O.F32_STATE_F64_REDUCE])
 def test_theta_posterior_linreg_against_marginal_grid(prec):
-    """P12 (M3): y_i ~ N(a + b z_i, s_i^2 + tau^2); exact 3-D grid; both precisions of the oracle."""
+    """Both precisions of the oracle."""
     n, burn, T = 150, 5000, 50000
     inp = synth.make_linreg_me1d(n, seed=36, fp32=True)
     s = O.Sampler(3, n, seed=36, precision=prec, target_accept_chi=0.44)
     s.set_data(inp["cols"]); s.set_init(inp["theta0"])
     s.run(burn + T, burn_in=burn)
-    tr = s.get_theta_trace()
-    y, sig, z = inp["cols"]
-    m0, s0 = tr.mean(0), tr.std(0)
-    axes = [np.linspace(m0[k] - 6 * s0[k], m0[k] + 6 * s0[k], 81) for k in range(3)]
-    A, B, Lm = np.meshgrid(*axes, indexing="ij")
-    lp = np.zeros_like(A)
-    for i in range(n):
-        V = sig[i] ** 2 + np.exp(2 * Lm)
-        lp += -0.5 * np.log(V) - 0.5 * (y[i] - A - B * z[i]) ** 2 / V
-    gm, gs = _grid_moments(lp, axes)
-    mean, mse, var, vse = mean_and_var_with_mcse(tr)
-    _assert_within(mean, mse, gm, floor=2e-4, what="theta mean")
-    _assert_within(var, vse, gs ** 2, floor=2e-3 * gs.max() ** 2, what="theta variance")
+    check_linreg_posterior(inp, s.get_theta_trace())
 
 
-def test_theta_posterior_binormal_against_independent_sampler():
+def check_binormal_posterior(inp, tr, n_ref=60000):
     """P12 (M2): plain random-walk MH (numpy) on the closed-form MARGINAL likelihood
     y_i ~ N2(m, Sigma_pop + diag(s_i^2)) -- a different algorithm on a different (chi-free) target."""
-    n, burn, T = 200, 6000, 50000
-    inp = synth.make_binormal2d(n, seed=37)
-    s = O.Sampler(2, n, seed=37, target_accept_chi=0.234)
-    s.set_data(inp["cols"]); s.set_init(inp["theta0"])
-    s.run(burn + T, burn_in=burn)
-    tr = s.get_theta_trace()
     y1, y2, s1, s2 = inp["cols"]
 
     def marg(th):
@@ -219,35 +226,38 @@ def test_theta_posterior_binormal_against_independent_sampler():
     g = np.random.default_rng(0)
     step = np.linalg.cholesky(np.cov(tr.T) * (2.38 ** 2 / 5))
     cur = tr.mean(0); lc = marg(cur)
-    ref = np.empty((60000, 5))
+    ref = np.empty((n_ref, 5))
     for t in range(ref.shape[0]):
         prop = cur + step @ g.normal(size=5)
         lpn = marg(prop)
         if np.log(g.uniform()) < lpn - lc:
             cur, lc = prop, lpn
         ref[t] = cur
-    ref = ref[5000:]
+    ref = ref[n_ref // 12:]
     m1, e1, v1, ve1 = mean_and_var_with_mcse(tr)
     m2, e2, v2, ve2 = mean_and_var_with_mcse(ref)
-    _assert_within(m1, np.hypot(e1, e2), m2, floor=2e-4, what="theta mean")
+    _assert_within(m1, np.hypot(e1, e2), m2, floor=2e-3 * np.sqrt(v2.max()), what="theta mean")
     _assert_within(v1, np.hypot(ve1, ve2), v2, floor=2e-3 * v2.max(), what="theta variance")
 
 
-def test_theta_posterior_schechter_against_eq_4_3():
+def test_theta_posterior_binormal_against_independent_sampler():
+    n, burn, T = 200, 6000, 50000
+    inp = synth.make_binormal2d(n, seed=37)
+    s = O.Sampler(2, n, seed=37, target_accept_chi=0.234)
+    s.set_data(inp["cols"]); s.set_init(inp["theta0"])
+    s.run(burn + T, burn_in=burn)
+    check_binormal_posterior(inp, s.get_theta_trace())
+
+
+def check_schechter_posterior(inp, tr, theta_only, ngrid=61, nloc=801):
     """P11: marginalising the log-flat amplitude out of the Poisson form gives the paper's likelihood
     L(zeta) = prod_i int dx mu(x, r_i; zeta) l_i(x), mu = phi h / int int eta h phi (Eq. 4.3-4.4).
     The (alpha, x*) marginals of the 3-parameter chain must match a direct grid of that expression, written
-    here in numpy from the equations (its own quadrature, its own densities)."""
-    n, burn, T = 120, 6000, 60000
-    inp = synth.make_thinned_schechter1d(n, seed=38)
+    here in numpy from the equations (its own quadrature, its own densities).  theta_only = the oracle's T(theta)."""
     c = inp["consts"]
     F_lim, sigF, x_lo, x_hi, r_min, r_max = c
-    s = O.Sampler(1, n, seed=38, target_accept_chi=0.44)
-    s.set_data(inp["cols"]); s.set_model_consts(c); s.set_init(inp["theta0"])
-    s.run(burn + T, burn_in=burn)
-    tr = s.get_theta_trace()
     Fh, g = inp["cols"]
-
+    n = Fh.size
     # selection integral on the test's own tensor grid (trapezoid in x on a fine grid, Gauss-Legendre in r)
     xr, wr = np.polynomial.legendre.leggauss(200)
     r = 0.5 * (r_max - r_min) * xr + 0.5 * (r_max + r_min); w_r = 0.5 * (r_max - r_min) * wr
@@ -257,20 +267,21 @@ def test_theta_posterior_schechter_against_eq_4_3():
     # per-object local grids around the flux estimate
     xc = np.log(Fh / g)
     half = 12 * sigF / Fh + 1e-3
-    loc = xc[:, None] + half[:, None] * np.linspace(-1, 1, 801)[None, :]
+    loc = xc[:, None] + half[:, None] * np.linspace(-1, 1, nloc)[None, :]
     loc = np.clip(loc, x_lo, x_hi)
     lik = np.exp(stats.norm.logpdf(Fh[:, None], g[:, None] * np.exp(loc), sigF) - stats.norm.logpdf(0, 0, sigF))
     dloc = np.gradient(loc, axis=1)
+    likd = lik * dloc
+    eloc = np.exp(loc)
 
     m0, s0 = tr[:, :2].mean(0), tr[:, :2].std(0)
-    al = np.linspace(max(m0[0] - 5 * s0[0], -1.999), min(m0[0] + 5 * s0[0], -1e-3), 61)
-    xs = np.linspace(m0[1] - 5 * s0[1], m0[1] + 5 * s0[1], 61)
+    al = np.linspace(max(m0[0] - 5 * s0[0], -1.999), min(m0[0] + 5 * s0[0], -1e-3), ngrid)
+    xs = np.linspace(m0[1] - 5 * s0[1], m0[1] + 5 * s0[1], ngrid)
     lp = np.empty((al.size, xs.size))
     for i, a_ in enumerate(al):
         for j, x_ in enumerate(xs):
-            phi = lambda x: np.exp((a_ + 1) * (x - x_) - np.exp(x - x_))
-            I = np.trapezoid(phi(xg) * G, xg)
-            num = (phi(loc) * lik * dloc).sum(1)
+            I = np.trapezoid(np.exp((a_ + 1) * (xg - x_) - np.exp(xg - x_)) * G, xg)
+            num = (np.exp((a_ + 1) * (loc - x_) - eloc * np.exp(-x_)) * likd).sum(1)
             lp[i, j] = np.log(num).sum() - n * np.log(I) - np.log(1 + a_ * a_)
     gm, gs = _grid_moments(lp, [al, xs])
     mean, mse, var, vse = mean_and_var_with_mcse(tr[:, :2])
@@ -278,9 +289,18 @@ def test_theta_posterior_schechter_against_eq_4_3():
     _assert_within(var, vse, gs ** 2, floor=0.02 * gs.max() ** 2, what="(alpha, x*) variance")
     # P10: given (alpha, x*), A ~ Gamma(N, rate I): E[a | rest] = digamma(N) - log I  => check the chain average
     from scipy.special import digamma
-    I_chain = np.array([-s.theta_only([t_[0], t_[1], 0.0]) for t_ in tr[::50]])
+    I_chain = np.array([-theta_only([t_[0], t_[1], 0.0]) for t_ in tr[::50]])
     want = (digamma(n) - np.log(I_chain)).mean()
-    assert tr[:, 2].mean() == pytest.approx(want, abs=4 * mcse_batch_means(tr[:, 2])[0] + 5e-3)
+    assert tr[:, 2].mean() == pytest.approx(want, abs=4 * mcse_batch_means(tr[:, 2])[0] + 5e-3 * tr[:, 2].std())
+
+
+def test_theta_posterior_schechter_against_eq_4_3():
+    n, burn, T = 120, 6000, 60000
+    inp = synth.make_thinned_schechter1d(n, seed=38)
+    s = O.Sampler(1, n, seed=38, target_accept_chi=0.44)
+    s.set_data(inp["cols"]); s.set_model_consts(inp["consts"]); s.set_init(inp["theta0"])
+    s.run(burn + T, burn_in=burn)
+    check_schechter_posterior(inp, s.get_theta_trace(), s.theta_only)
 
 
 def test_trace_thinning_and_resume_bookkeeping():
@@ -336,3 +356,39 @@ def test_population_sums_in_taps():
     chi = s.get_state()["chi"][0]
     i = 11
     assert tp["b"][i] == O.logpop(1, [chi[i]], [0, 0], tp["theta_prop"], inp["consts"])
+
+
+def test_plate_tails_beyond_4_sigma_follow_the_normal_law_on_the_32_bit_grid():
+    """DESIGN.md reading R23: the fp64 p = 1 plate draws are built from 32-bit uniforms (normals on a 2^-32 grid, radius
+    capped at sqrt(66 ln 2) = 6.76, accept uniforms >= 2^-33).  A Metropolis chain with a symmetric proposal has the target
+    as its stationary law whatever the proposal's tails are, so the grid must not show in the chain's OWN tails: with
+    theta frozen, chi_i | theta, y_i is N(m_i, v_i) in closed form (P6) and the frequency of |chi_i - m_i| > 4 sqrt(v_i)
+    over 2e5 iterations per object must be 2 Phi(-4) = 6.334e-5.  128 independent objects; the standard error of the
+    pooled frequency is taken ACROSS objects (the chains are autocorrelated, so a plain binomial SE would be too small;
+    it is asserted that the across-object SE is not below the binomial one)."""
+    n, burn, T = 128, 2000, 200_000
+    inp = synth.make_normal1d(n, seed=41)
+    theta = np.array([-0.1, 0.15])
+    s = O.Sampler(0, n, seed=41, target_accept_chi=0.44, freeze_theta=True)
+    s.set_data(inp["cols"]); s.set_init(theta)
+    s.run(burn)
+    y, sig = inp["cols"]
+    tau = np.exp(theta[1])
+    v2 = 1 / (1 / sig ** 2 + 1 / tau ** 2)
+    m = (y / sig ** 2 + theta[0] / tau ** 2) * v2
+    sd = np.sqrt(v2)
+    counts = np.zeros(n)
+    counts3 = np.zeros(n)
+    for _ in range(T):
+        s.step()
+        z = np.abs(s.get_state()["chi"][0] - m) / sd
+        counts += z > 4.0
+        counts3 += z > 3.0
+    for k, cnt in ((4.0, counts), (3.0, counts3)):
+        p_true = 2 * stats.norm.sf(k)
+        freq = cnt / T
+        se_across = freq.std(ddof=1) / np.sqrt(n)
+        se_binom = np.sqrt(p_true / (n * T))
+        assert se_across >= 0.9 * se_binom
+        assert abs(freq.mean() - p_true) <= 4 * se_across, f"|z| > {k}: {freq.mean():.3e} against {p_true:.3e} +- {se_across:.1e}"
+        assert se_across < 0.1 * p_true            # the test has the power to see a 40 % distortion of the tail
