@@ -10,7 +10,7 @@ import numpy as np
 from . import build as _build
 
 M_NORMAL1D, M_THINNED_SCHECHTER1D, M_BINORMAL2D, M_LINREG_ME1D, M_BB1_FLUXNOISE1D = 0, 1, 2, 3, 4
-M_NORMAL3D_KNOWNCOV = 5
+M_NORMAL3D_KNOWNCOV, M_NORMAL4D_KNOWNCOV, M_NORMAL5D_KNOWNCOV, M_NORMAL6D_KNOWNCOV = 5, 6, 7, 8
 F64, F32_STATE_F64_REDUCE = 0, 1
 KIND_PLATE, KIND_THETA = 0, 1
 
@@ -25,7 +25,8 @@ class Config(C.Structure):
                 ("init_scale_chi", C.c_double), ("freeze_theta", C.c_int32),
                 ("keep_chi_moments", C.c_int32), ("adapt_until", C.c_int64),
                 ("prior_mean", C.c_double * 8), ("prior_isd", C.c_double * 8),
-                ("object_offset", C.c_int64), ("n_objects_total", C.c_int64)]
+                ("object_offset", C.c_int64), ("n_objects_total", C.c_int64),
+                ("per_object_counter", C.c_int32), ("pad_", C.c_int32)]
 
 
 class Taps(C.Structure):
@@ -56,6 +57,9 @@ def lib():
         L.oracle_set_data.argtypes = [C.c_void_p, C.POINTER(_dp), C.c_int]
         L.oracle_set_model_consts.argtypes = [C.c_void_p, _dp, C.c_int]
         L.oracle_set_init.argtypes = [C.c_void_p, _dp, _dp, _dp]
+        L.oracle_set_update_mask.argtypes = [C.c_void_p, C.POINTER(C.c_uint8)]
+        L.oracle_get_counters.argtypes = [C.c_void_p, C.POINTER(C.c_uint32)]
+        L.oracle_set_counters.argtypes = [C.c_void_p, C.POINTER(C.c_uint32)]
         L.oracle_run.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_int32]
         L.oracle_step.argtypes = [C.c_void_p, C.c_int64, C.c_int32, C.POINTER(Taps)]
         L.oracle_shard_sweep.argtypes = [C.c_void_p, C.c_int64, C.c_int32, _dp]
@@ -133,7 +137,7 @@ class Sampler:
     def __init__(self, model, n_objects, seed=0, precision=F64, target_accept_chi=0.4,
                  target_accept_theta=0.234, eta_exponent=2.0 / 3.0, init_scale_chi=1.0,
                  freeze_theta=False, keep_chi_moments=False, adapt_until=0, prior_mean=None, prior_sd=None,
-                 object_offset=0, n_objects_total=0):
+                 object_offset=0, n_objects_total=0, per_object_counter=False):
         self.dims = model_dims(model)
         self.N = int(n_objects)
         self.p, self.dtheta = self.dims["p"], self.dims["dtheta"]
@@ -146,6 +150,7 @@ class Sampler:
                 self.cfg.prior_mean[j] = float(m)
                 self.cfg.prior_isd[j] = 0.0 if not np.isfinite(sd) else 1.0 / float(sd)
         self.cfg.object_offset, self.cfg.n_objects_total = int(object_offset), int(n_objects_total)
+        self.cfg.per_object_counter = int(per_object_counter)
         self._h = C.c_void_p()
         _check(lib().oracle_create(C.byref(self.cfg), C.byref(self._h)), "create")
 
@@ -169,6 +174,25 @@ class Sampler:
     def set_model_consts(self, v):
         v = _arr(v)
         _check(lib().oracle_set_model_consts(self._h, _d(v), v.size), "set_model_consts")
+
+    def set_update_mask(self, mask):
+        """mask: N bytes (1 = update, 0 = hold fixed) or None (update everything)."""
+        if mask is None:
+            _check(lib().oracle_set_update_mask(self._h, None), "set_update_mask")
+            return
+        m = np.ascontiguousarray(np.asarray(mask, dtype=np.uint8))
+        assert m.shape == (self.N,)
+        _check(lib().oracle_set_update_mask(self._h, m.ctypes.data_as(C.POINTER(C.c_uint8))), "set_update_mask")
+
+    def get_counters(self):
+        out = np.empty(self.N, dtype=np.uint32)
+        _check(lib().oracle_get_counters(self._h, out.ctypes.data_as(C.POINTER(C.c_uint32))), "get_counters")
+        return out
+
+    def set_counters(self, c):
+        c = np.ascontiguousarray(np.asarray(c, dtype=np.uint32))
+        assert c.shape == (self.N,)
+        _check(lib().oracle_set_counters(self._h, c.ctypes.data_as(C.POINTER(C.c_uint32))), "set_counters")
 
     def set_init(self, theta0, chi0=None, theta_chol0=None):
         th = _arr(theta0)

@@ -13,7 +13,15 @@
 namespace oracle {
 
 enum Model { M_NORMAL1D = 0, M_THINNED_SCHECHTER1D = 1, M_BINORMAL2D = 2, M_LINREG_ME1D = 3, M_BB1_FLUXNOISE1D = 4,
-             M_NORMAL3D_KNOWNCOV = 5 };
+             M_NORMAL3D_KNOWNCOV = 5,
+             // the same normal-normal model for p-vector latents, p = 4, 5, 6 (RAM of Eq. 2.6 is stated for any dimension,
+             // PAPER.md:129-140; section 3 is its p = 3 instance): chi ~ N_p(mu, C_pop), y_j ~ N(chi_j, sigma_j^2)
+             M_NORMAL4D_KNOWNCOV = 6, M_NORMAL5D_KNOWNCOV = 7, M_NORMAL6D_KNOWNCOV = 8 };
+
+// latent dimension of the normal-normal family (0 for the other models)
+inline int normal_family_p(int model) {
+  return (model >= M_NORMAL3D_KNOWNCOV && model <= M_NORMAL6D_KNOWNCOV) ? model - M_NORMAL3D_KNOWNCOV + 3 : 0;
+}
 
 struct Dims { int p, dtheta, n_cols, n_consts; };
 inline bool model_dims(int model, Dims* d) {
@@ -24,6 +32,9 @@ inline bool model_dims(int model, Dims* d) {
     case M_LINREG_ME1D:         *d = {1, 3, 3, 0}; return true;   // cols y, sigma, z;       theta (a, b, log tau)
     case M_BB1_FLUXNOISE1D:     *d = {1, 3, 2, 7}; return true;   // cols Fhat, g=1/(4 pi r^2); theta (beta, ln l, ln u)
     case M_NORMAL3D_KNOWNCOV:   *d = {3, 3, 3, 9}; return true;   // cols y1, y2, y3;        theta = mu (3)
+    case M_NORMAL4D_KNOWNCOV:   *d = {4, 4, 4, 14}; return true;  // cols y1..y4;  theta = mu;  consts sigma_1..4, C_pop (10)
+    case M_NORMAL5D_KNOWNCOV:   *d = {5, 5, 5, 20}; return true;
+    case M_NORMAL6D_KNOWNCOV:   *d = {6, 6, 6, 27}; return true;
   }
   return false;
 }
@@ -34,9 +45,10 @@ enum { C_FLIM = 0, C_SIGF = 1, C_XLO = 2, C_XHI = 3, C_RMIN = 4, C_RMAX = 5 };
 // r_min, r_max, F_th}; x_lo .. r_max sit at the same indices as in M1
 enum { B_SIG0 = 0, B_ANOISE = 1, B_FTH = 6 };
 
-// consts of M5 (the normal-normal benchmark of PAPER.md:146-166, Eq. 3.1-3.4): {sigma_1, sigma_2, sigma_3, then the
-// packed lower triangle of C_pop: C11, C21, C22, C31, C32, C33}; C_pop and sigma_j are KNOWN, theta = mu
-enum { N3_SIG = 0, N3_COV = 3 };
+// consts of the normal-normal family (the benchmark of PAPER.md:146-166, Eq. 3.1-3.4, for p = 3 .. 6): {sigma_1 .. sigma_p,
+// then the packed lower triangle of C_pop row-major: C11, C21, C22, C31, ...}; C_pop and sigma_j are KNOWN, theta = mu
+// (PAPER.md:166).  The covariance block starts at index p.
+enum { N3_SIG = 0 };
 
 // log C(beta, u, l), the BB1 normaliser of PAPER.md:429 (Eq. C.3):
 //   C = 1 / (Gamma(beta+1) (1 - (1 + u/l)^-(beta+1)))   (beta > -2, beta != -1),     C = 1/log(1 + u/l)  (beta = -1).
@@ -67,9 +79,11 @@ inline T loglik(int model, const T* chi, const T* d, const T* consts) {
       const T r1 = d[0] - chi[0], r2 = d[1] - chi[1];
       return -T(0.5) * ((r1 * r1) / (d[2] * d[2]) + (r2 * r2) / (d[3] * d[3]));
     }
-    case M_NORMAL3D_KNOWNCOV: {                 // y_ij ~ N(chi_ij, sigma_j^2), j = 1..3   (Eq. 3.2, sigma_j of :164)
+    case M_NORMAL3D_KNOWNCOV: case M_NORMAL4D_KNOWNCOV: case M_NORMAL5D_KNOWNCOV: case M_NORMAL6D_KNOWNCOV: {
+      // y_ij ~ N(chi_ij, sigma_j^2), j = 1..p   (Eq. 3.2, sigma_j of :164)
+      const int np = normal_family_p(model);
       T s = T(0);
-      for (int j = 0; j < 3; ++j) { const T r = d[j] - chi[j]; s += (r * r) / (consts[N3_SIG + j] * consts[N3_SIG + j]); }
+      for (int j = 0; j < np; ++j) { const T r = d[j] - chi[j]; s += (r * r) / (consts[N3_SIG + j] * consts[N3_SIG + j]); }
       return -T(0.5) * s;
     }
     case M_BB1_FLUXNOISE1D: {
@@ -109,19 +123,20 @@ inline T logpop(int model, const T* chi, const T* d, const T* th, const T* const
       const T rho = std::tanh(th[4]);
       return -th[2] - th[3] + std::log(ch) - ch * ch * (u1 * u1 - T(2) * rho * u1 * u2 + u2 * u2) / T(2);
     }
-    case M_NORMAL3D_KNOWNCOV: {
+    case M_NORMAL3D_KNOWNCOV: case M_NORMAL4D_KNOWNCOV: case M_NORMAL5D_KNOWNCOV: case M_NORMAL6D_KNOWNCOV: {
       // chi ~ N(mu, C_pop) (Eq. 3.1), C_pop known: log f = -1/2 (chi - mu)^T C_pop^-1 (chi - mu) + const.
       // Plain route: factor C_pop = G G^T (Cholesky), solve G w = chi - mu, then -1/2 w^T w.
-      T G[3][3] = {};
-      const T* Cp = consts + N3_COV;
-      for (int r = 0; r < 3; ++r)
+      const int np = normal_family_p(model);
+      T G[6][6] = {};
+      const T* Cp = consts + np;
+      for (int r = 0; r < np; ++r)
         for (int k = 0; k <= r; ++k) {
           T a = Cp[r * (r + 1) / 2 + k];
           for (int m = 0; m < k; ++m) a -= G[r][m] * G[k][m];
           G[r][k] = (r == k) ? std::sqrt(a) : a / G[k][k];
         }
-      T w[3], q = T(0);
-      for (int r = 0; r < 3; ++r) {
+      T w[6], q = T(0);
+      for (int r = 0; r < np; ++r) {
         T a = chi[r] - th[r];
         for (int m = 0; m < r; ++m) a -= G[r][m] * w[m];
         w[r] = a / G[r][r];
@@ -161,8 +176,10 @@ inline double logprior(int model, const double* th) {
     case M_THINNED_SCHECHTER1D:
       if (!(th[0] > -2.0 && th[0] < 0.0 && std::fabs(th[1]) <= 20.0 && std::fabs(th[2]) <= 50.0)) return ninf;
       return -std::log(1.0 + th[0] * th[0]);
-    case M_NORMAL3D_KNOWNCOV:                   // "uniform hyperpriors", on a wide box so they are proper
-      if (!(std::fabs(th[0]) <= 1e3 && std::fabs(th[1]) <= 1e3 && std::fabs(th[2]) <= 1e3)) return ninf;
+    case M_NORMAL3D_KNOWNCOV: case M_NORMAL4D_KNOWNCOV: case M_NORMAL5D_KNOWNCOV: case M_NORMAL6D_KNOWNCOV:
+      // "uniform hyperpriors", on a wide box so they are proper
+      for (int j = 0; j < normal_family_p(model); ++j)
+        if (!(std::fabs(th[j]) <= 1e3)) return ninf;
       return 0.0;
     case M_BB1_FLUXNOISE1D:
       // PAPER.md:277-290 (Eq. 5.3-5.5): truncated Cauchy in beta on (-2, 0), log-flat in u, flat in l on l < u

@@ -31,7 +31,9 @@ enum { ORACLE_OK = 0, ORACLE_E_INVALID = -1, ORACLE_E_STATE = -2, ORACLE_E_UNSUP
 /* models: */
 enum { ORACLE_M_NORMAL1D = 0, ORACLE_M_THINNED_SCHECHTER1D = 1, ORACLE_M_BINORMAL2D = 2, ORACLE_M_LINREG_ME1D = 3,
        ORACLE_M_BB1_FLUXNOISE1D = 4, /* the paper's case study: BB1 population, flux-dependent noise */
-       ORACLE_M_NORMAL3D_KNOWNCOV = 5 /* the normal-normal benchmark: 3-vector latents, known C_pop */ };
+       ORACLE_M_NORMAL3D_KNOWNCOV = 5, /* the normal-normal benchmark: 3-vector latents, known C_pop */
+       /* the same model for p = 4, 5, 6 (RAM for general dimension, Eq. 2.6) */
+       ORACLE_M_NORMAL4D_KNOWNCOV = 6, ORACLE_M_NORMAL5D_KNOWNCOV = 7, ORACLE_M_NORMAL6D_KNOWNCOV = 8 };
 enum { ORACLE_F64 = 0, ORACLE_F32_STATE_F64_REDUCE = 1 };
 /* Philox stream kinds */
 enum { ORACLE_KIND_PLATE = 0, ORACLE_KIND_THETA = 1 };
@@ -55,6 +57,11 @@ typedef struct {
   /* sharded populations: this sampler owns objects [object_offset, object_offset + n_objects) of
    * n_objects_total (0 = n_objects); object_offset even (objects draw in pairs) */
   int64_t  object_offset, n_objects_total;
+  /* frozen members (properties "which should be held fixed over the course of posterior simulation"):
+   * 1 = eta_n of object i uses its OWN update count, n_i = (updates of object i so far) + 2, instead of the global
+   * n = t + 1; identical as long as every object is updated in every iteration (reading R3) */
+  int32_t  per_object_counter;
+  int32_t  pad_;
 } oracle_config;
 
 /* Per-iteration taps (all optional: a NULL member is skipped).  Per-object arrays have N entries
@@ -92,6 +99,14 @@ int  oracle_create(const oracle_config* cfg, oracle_sampler** out);
 void oracle_destroy(oracle_sampler* s);
 int  oracle_set_data(oracle_sampler* s, const double* const* cols, int n_cols);
 int  oracle_set_model_consts(oracle_sampler* s, const double* v, int n);
+/* Per-object update mask, N bytes: 1 = object i takes RAM steps 1-3 as usual, 0 = object i is held
+ * fixed (chi_i, L_i and its update count untouched, no draws consumed) but still contributes log f(chi_i; theta) and
+ * log f(chi_i; theta') to the population sums.  NULL = update everything (the default).  May be changed between
+ * iterations.  Taps of a held object: chi_prop = chi, pi_prop = pi_cur, alpha = 0, u = 1, accepted = 0, L_new = L. */
+int  oracle_set_update_mask(oracle_sampler* s, const uint8_t* mask_or_null);
+/* per-object update counts (N values); set_init zeroes them, set_state(t) sets them all to t */
+int  oracle_get_counters(oracle_sampler* s, uint32_t* out);
+int  oracle_set_counters(oracle_sampler* s, const uint32_t* in);
 int  oracle_set_init(oracle_sampler* s, const double* chi0_or_null, const double* theta0,
                      const double* theta_chol0_or_null);
 int  oracle_run(oracle_sampler* s, int64_t n_iter, int64_t burn_in, int32_t thin);

@@ -63,6 +63,14 @@ struct Base {
   std::vector<double> trace;         // rows of dtheta
   std::vector<double> mom_mean, mom_M2;
   int64_t mom_count = 0;
+  std::vector<uint8_t> mask;         // empty = every object is updated (held-fixed members)
+  std::vector<uint32_t> counters;    // RAM updates each object has taken so far
+  int64_t n_active() const {
+    if (mask.empty()) return cfg.n_objects;
+    int64_t k = 0;
+    for (uint8_t m : mask) k += m ? 1 : 0;
+    return k;
+  }
   oracle_stats stats{};
   virtual int set_data(const double* const* cols, int n_cols) = 0;
   virtual int set_init(const double* chi0, const double* theta0, const double* chol0) = 0;
@@ -127,6 +135,7 @@ struct Impl : Base {
     if (chol0) std::copy(chol0, chol0 + ntri(dt), Ltheta.begin());
     else for (int r = 0; r < dt; ++r) Ltheta[tri(r, r)] = 0.1;
     t = 0; trace.clear(); mom_count = 0;
+    counters.assign((size_t)N, 0u);
     mom_mean.assign((size_t)p * N, 0.0); mom_M2.assign((size_t)p * N, 0.0);
     stats = oracle_stats{};
     have_init = true;
@@ -149,6 +158,7 @@ struct Impl : Base {
     if (th) std::copy(th, th + dims.dtheta, theta.begin());
     if (lth) std::copy(lth, lth + ntri(dims.dtheta), Ltheta.begin());
     t = tt;
+    counters.assign((size_t)cfg.n_objects, (uint32_t)tt);   // as if every object had been updated in every iteration
     return ORACLE_OK;
   }
 
@@ -203,6 +213,42 @@ struct Impl : Base {
       for (int j = 0; j < p; ++j) x[j] = chi[(size_t)j * N + i];
       for (int k = 0; k < nt; ++k) l[k] = L[(size_t)k * N + i];
       for (int c = 0; c < nc; ++c) d[c] = data[(size_t)c * N + i];
+      if (!mask.empty() && !mask[(size_t)i]) {
+        // a member held fixed: no RAM step, but it stays in the population sums
+        double xd[8], dd[16];
+        for (int j = 0; j < p; ++j) xd[j] = (double)x[j];
+        for (int c = 0; c < nc; ++c) dd[c] = (double)d[c];
+        const double a = logpop<double>(model, xd, dd, theta.data(), cD);
+        const double b = logpop<double>(model, xd, dd, thp_, cD);
+        S += (long double)a;
+        Delta += (long double)(b - a);
+        if (taps) {
+          const T pc = loglik<T>(model, x, d, cT) + logpop<T>(model, x, d, thT, cT);
+          if (taps->chi_prop) for (int j = 0; j < p; ++j) taps->chi_prop[(size_t)j * N + i] = (double)x[j];
+          if (taps->pi_cur) taps->pi_cur[i] = (double)pc;
+          if (taps->pi_prop) taps->pi_prop[i] = (double)pc;
+          if (taps->alpha) taps->alpha[i] = 0.0;
+          if (taps->u) taps->u[i] = 1.0;
+          if (taps->accepted) taps->accepted[i] = 0;
+          if (taps->L_new) for (int k = 0; k < nt; ++k) taps->L_new[(size_t)k * N + i] = (double)l[k];
+          if (taps->a) taps->a[i] = a;
+          if (taps->b) taps->b[i] = b;
+        }
+        if (cfg.keep_chi_moments && (t + 1) > burn_in) {
+          const double k1 = (double)(mom_count + 1);
+          for (int j = 0; j < p; ++j) {
+            const size_t q = (size_t)j * N + i;
+            const double dl = xd[j] - mom_mean[q];
+            mom_mean[q] += dl / k1;
+            mom_M2[q] += dl * (xd[j] - mom_mean[q]);
+          }
+        }
+        continue;
+      }
+      // eta_n of THIS object: its own update count when asked for (n_i = count + 2: the first update is n = 2)
+      double eta_i = eta;
+      if (cfg.per_object_counter && eta != 0.0) eta_i = std::pow((double)counters[(size_t)i] + 2.0, -cfg.eta_exponent);
+      counters[(size_t)i] += 1u;
       if (sizeof(T) == 8) {
         double zz[8] = {}, uu = 0;
         plate_draws_f64(cfg.seed, (uint64_t)(cfg.object_offset + i), tcur, p, zz, &uu);
@@ -232,7 +278,7 @@ struct Impl : Base {
       if (acc) { for (int j = 0; j < p; ++j) x[j] = y[j]; n_acc++; }
       // step 3: S_n = chol(S (I + eta (alpha - alpha_*) U U^T/||U||^2) S^T)
       T lnew[36];
-      ram_update<T>(p, l, z, (T)eta * (alpha - (T)cfg.target_accept_chi), lnew);
+      ram_update<T>(p, l, z, (T)eta_i * (alpha - (T)cfg.target_accept_chi), lnew);
       for (int j = 0; j < p; ++j) chi[(size_t)j * N + i] = x[j];
       for (int k = 0; k < nt; ++k) L[(size_t)k * N + i] = lnew[k];
       // population terms at the new chi, fp64 (log-posterior with the updated parameters)
@@ -283,7 +329,7 @@ struct Impl : Base {
     const double S = tot[0], Delta = tot[1];
     stats.chi_accepts += (int64_t)tot[3];
     stats.nonfinite += (int64_t)tot[4];
-    stats.chi_proposals += cfg.n_objects_total ? cfg.n_objects_total : cfg.n_objects;
+    stats.chi_proposals += mask.empty() ? (cfg.n_objects_total ? cfg.n_objects_total : cfg.n_objects) : n_active();
 
     // O5-O7: theta decision and RAM update of L_theta
     double T_cur = 0, T_prop = 0, lp_cur = 0, lp_prop = 0, log_r = 0, alpha_th = 0, u_th = 0;
@@ -383,6 +429,27 @@ int oracle_set_model_consts(oracle_sampler* s, const double* v, int n) {
   if (b->cfg.model == M_THINNED_SCHECHTER1D) b->table.build(b->consts.data());
   if (b->cfg.model == M_BB1_FLUXNOISE1D) b->table.build_bb1(b->consts.data());
   b->have_consts = true;
+  return ORACLE_OK;
+}
+
+int oracle_set_update_mask(oracle_sampler* s, const uint8_t* mask) {
+  if (!s) return ORACLE_E_INVALID;
+  Base* b = s->impl.get();
+  if (mask && b->cfg.n_objects_total != 0 && b->cfg.n_objects_total != b->cfg.n_objects) return ORACLE_E_UNSUPPORTED;
+  if (mask) b->mask.assign(mask, mask + b->cfg.n_objects);
+  else b->mask.clear();
+  return ORACLE_OK;
+}
+int oracle_get_counters(oracle_sampler* s, uint32_t* out) {
+  if (!s || !out) return ORACLE_E_INVALID;
+  if (!s->impl->have_init) return ORACLE_E_STATE;
+  std::copy(s->impl->counters.begin(), s->impl->counters.end(), out);
+  return ORACLE_OK;
+}
+int oracle_set_counters(oracle_sampler* s, const uint32_t* in) {
+  if (!s || !in) return ORACLE_E_INVALID;
+  if (!s->impl->have_init) return ORACLE_E_STATE;
+  s->impl->counters.assign(in, in + s->impl->cfg.n_objects);
   return ORACLE_OK;
 }
 

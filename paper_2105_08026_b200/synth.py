@@ -13,6 +13,7 @@ from dataclasses import dataclass
 import numpy as np
 
 M_NORMAL1D, M_THINNED_SCHECHTER1D, M_BINORMAL2D, M_LINREG_ME1D, M_BB1_FLUXNOISE1D, M_NORMAL3D_KNOWNCOV = 0, 1, 2, 3, 4, 5
+M_NORMAL4D_KNOWNCOV, M_NORMAL5D_KNOWNCOV, M_NORMAL6D_KNOWNCOV = 6, 7, 8
 F64, F32_STATE_F64_REDUCE = 0, 1
 
 
@@ -94,6 +95,33 @@ def theta_chol0(model, n):
     d = {M_NORMAL1D: 2, M_THINNED_SCHECHTER1D: 3, M_BINORMAL2D: 5, M_LINREG_ME1D: 3, M_BB1_FLUXNOISE1D: 3,
          M_NORMAL3D_KNOWNCOV: 3}[model]
     return np.asarray(THETA_COND_CHOL[model], dtype=np.float64) * (2.38 / np.sqrt(d) / np.sqrt(max(int(n), 1)))
+
+
+# the normal-normal model for p = 4, 5, 6 (RAM for general dimension): the paper's
+# three components (Eq. 3.3-3.4) followed by up to three more; R is the leading p x p block of a fixed positive definite
+# correlation matrix whose leading 3 x 3 block is the paper's Eq. 3.4
+NNP_MU = np.array([1.2, -0.4, 3.4, 0.7, -2.1, 5.0])
+NNP_D = np.array([2.3, 0.45, 13.4, 1.1, 0.8, 3.2])
+NNP_SIGMA = np.array([1.2, 0.4, 0.24, 0.6, 0.3, 1.5])
+NNP_R = np.array([[1.0, 0.3, -0.5, 0.2, -0.1, 0.15],
+                  [0.3, 1.0, 0.54, -0.25, 0.2, 0.1],
+                  [-0.5, 0.54, 1.0, -0.3, 0.1, -0.2],
+                  [0.2, -0.25, -0.3, 1.0, 0.35, -0.15],
+                  [-0.1, 0.2, 0.1, 0.35, 1.0, 0.25],
+                  [0.15, 0.1, -0.2, -0.15, 0.25, 1.0]])
+
+
+def nnp_model(p):
+    return {3: M_NORMAL3D_KNOWNCOV, 4: M_NORMAL4D_KNOWNCOV, 5: M_NORMAL5D_KNOWNCOV, 6: M_NORMAL6D_KNOWNCOV}[int(p)]
+
+
+def nnp_cpop(p):
+    return NNP_D[:p, None] * NNP_R[:p, :p] * NNP_D[None, :p]
+
+
+def nnp_consts(p):
+    """{sigma_1 .. sigma_p, packed lower triangle of C_pop}"""
+    return np.concatenate([NNP_SIGMA[:p], nnp_cpop(p)[np.tril_indices(p)]])
 
 
 def _rng(seed):
@@ -208,6 +236,19 @@ def make_normal3d_knowncov(n, seed=6):
     return dict(model=M_NORMAL3D_KNOWNCOV, cols=[y[0].copy(), y[1].copy(), y[2].copy()], consts=NN3_CONSTS.copy(),
                 chi_true=chi, theta_true=NN3_MU.copy(), theta0=NN3_MU + np.array([0.05, -0.02, 0.2]),
                 theta_chol0=theta_chol0(M_NORMAL3D_KNOWNCOV, n))
+
+
+def make_normalpd_knowncov(n, seed=7, p=4):
+    """The normal-normal model with p-vector latents, p = 3 .. 6: chi_i ~ N_p(mu, C_pop), y_ij = chi_ij + sigma_j eps."""
+    g = _rng(seed)
+    C = nnp_cpop(p)
+    chi = NNP_MU[:p, None] + np.linalg.cholesky(C) @ g.standard_normal((p, n))
+    y = chi + NNP_SIGMA[:p, None] * g.standard_normal((p, n))
+    # theta | chi ~ N(chibar, C_pop / N): the proposal factor of the recipe (see THETA_COND_CHOL)
+    chol0 = np.linalg.cholesky(C)[np.tril_indices(p)] * (2.38 / np.sqrt(p) / np.sqrt(max(int(n), 1)))
+    return dict(model=nnp_model(p), cols=[y[j].copy() for j in range(p)], consts=nnp_consts(p), chi_true=chi,
+                theta_true=NNP_MU[:p].copy(), theta0=NNP_MU[:p] + 0.05 * NNP_D[:p] * np.array([1, -1, 1, -1, 1, -1])[:p],
+                theta_chol0=chol0)
 
 
 def make_binormal2d(n, seed=3, fp32=False):
