@@ -54,7 +54,10 @@ enum { CUDAHM_M_NORMAL1D = 0,            /* (1, 2, {y, sigma}, 0)            the
        CUDAHM_M_BB1_FLUXNOISE1D = 4,     /* (1, 3, {Fhat, g=1/(4 pi r^2)}, 7) theta = (beta, log l, log u)       */
        /* the normal-normal benchmark (Eq. 3.1-3.4): chi_i ~ N3(mu, C_pop), y_ij ~ N(chi_ij, sigma_j^2),
         * C_pop and sigma_j known, uniform hyperprior; p = 3 RAM with the general rank-one Cholesky update            */
-       CUDAHM_M_NORMAL3D_KNOWNCOV = 5 }; /* (3, 3, {y1, y2, y3}, 9)          theta = mu                         */
+       CUDAHM_M_NORMAL3D_KNOWNCOV = 5,   /* (3, 3, {y1, y2, y3}, 9)          theta = mu                         */
+       /* the same normal-normal model with p-vector latents, p = 4, 5, 6: RAM for general dimension (Eq. 2.6, PAPER.md:129-140,
+        * is stated for any p; section 3 is its p = 3 instance).  (p, p, {y1..yp}, p + p(p+1)/2), theta = mu.  F64 only, 256-thread blocks */
+       CUDAHM_M_NORMAL4D_KNOWNCOV = 6, CUDAHM_M_NORMAL5D_KNOWNCOV = 7, CUDAHM_M_NORMAL6D_KNOWNCOV = 8 };
 enum { CUDAHM_F64 = 0, CUDAHM_F32_STATE_F64_REDUCE = 1 };
 /* where the theta Metropolis-Hastings step runs (PAPER.md:142 puts it on the host) */
 enum { CUDAHM_THETA_HOST = 0,         /* one sweep launch + one sync per iteration; theta step in host C++     */
@@ -162,7 +165,8 @@ int cudahm_set_data(cudahm_sampler* s, const void* const* cols, int n_cols, int 
 /* Model constants (host doubles).  THINNED_SCHECHTER1D: {F_lim, sigma_F, x_lo, x_hi, r_min, r_max};
  * BB1_FLUXNOISE1D: {sigma_0, alpha, x_lo, x_hi, r_min, r_max, F_th} (Eq. 5.8-5.10); both build the 1,024-point
  * selection-integral table (Eq. 4.4 denominator).  NORMAL3D_KNOWNCOV: {sigma_1, sigma_2, sigma_3, C11, C21,
- * C22, C31, C32, C33} (packed lower triangle of C_pop, Eq. 3.3).  Other models take n = 0. */
+ * C22, C31, C32, C33} (packed lower triangle of C_pop, Eq. 3.3); NORMAL4D .. 6D likewise: {sigma_1..p, packed lower triangle
+ * of C_pop row-major}; CUDAHM_E_INVALID unless sigma_j > 0 and C_pop is positive definite.  Other models take n = 0. */
 int cudahm_set_model_consts(cudahm_sampler* s, const double* v, int n);
 
 /* Initial state: chi0 (p*N values of type T, host or device per chi0_on_device; NULL = the model's default

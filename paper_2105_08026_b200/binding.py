@@ -14,6 +14,7 @@ LIB_PATH = os.path.join(HERE, "libcudahm.so")
 
 OK, E_INVALID, E_STATE, E_CUDA, E_WORKSPACE, E_UNSUPPORTED, E_NONFINITE = 0, -1, -2, -3, -4, -5, -6
 M_NORMAL1D, M_THINNED_SCHECHTER1D, M_BINORMAL2D, M_LINREG_ME1D, M_BB1_FLUXNOISE1D, M_NORMAL3D_KNOWNCOV = 0, 1, 2, 3, 4, 5
+M_NORMAL4D_KNOWNCOV, M_NORMAL5D_KNOWNCOV, M_NORMAL6D_KNOWNCOV = 6, 7, 8
 F64, F32_STATE_F64_REDUCE = 0, 1
 THETA_HOST, THETA_GRAPH, THETA_DEVICE_TAIL = 0, 1, 2
 FLAG_STREAMING_ONLY, FLAG_TMA_STAGING = 1, 2

@@ -44,6 +44,9 @@ bool pick_kernels(int model, int precision, int block, KernelSet* k, ResidentSet
     case M_LINREG_ME1D:         return kernels_linreg_me1d(precision, block, k, r);
     case M_BB1_FLUXNOISE1D:     return kernels_bb1_fluxnoise1d(precision, block, k, r);
     case M_NORMAL3D_KNOWNCOV:   return kernels_normal3d_knowncov(precision, block, k, r);
+    case M_NORMAL4D_KNOWNCOV:   return kernels_normal4d_knowncov(precision, block, k, r);
+    case M_NORMAL5D_KNOWNCOV:   return kernels_normal5d_knowncov(precision, block, k, r);
+    case M_NORMAL6D_KNOWNCOV:   return kernels_normal6d_knowncov(precision, block, k, r);
   }
   return false;
 }
@@ -212,7 +215,8 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
   // default block: 512 threads; a population too small to give every SM a 512-thread block of 16-byte vectors takes
   // 256-thread blocks instead (twice the SMs at work: the small configs are latency-bound, not bandwidth-bound)
   int block = cfg->block_threads ? cfg->block_threads : 512;
-  if (!cfg->block_threads) {
+  if (!cfg->block_threads && p >= 4) block = 256;     // two objects of p (p + 5) / 2 doubles each per thread: 255 registers
+  else if (!cfg->block_threads) {
     const long long vec = cfg->precision == CUDAHM_F64 ? 2 : 4;
     int dev0 = 0, sms0 = 0;
     if (cudaGetDevice(&dev0) == cudaSuccess) cudaDeviceGetAttribute(&sms0, cudaDevAttrMultiProcessorCount, dev0);
@@ -283,7 +287,7 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
   }
   // HBM-streaming variant with TMA-staged loads (stream_tma.cuh), opt-in: measured 10-30 % slower than plain vector
   // loads on C3 / C4 (the sweep is issue-bound, not latency-bound, and the producer warp costs a sweep warp)
-  if (cfg->theta_mode == CUDAHM_THETA_DEVICE_TAIL && (cfg->flags & CUDAHM_FLAG_TMA_STAGING) && block <= 512) {
+  if (cfg->theta_mode == CUDAHM_THETA_DEVICE_TAIL && (cfg->flags & CUDAHM_FLAG_TMA_STAGING) && block <= 512 && ks.persistent_tma) {
     int stages = (int)std::min<size_t>(TMA_MAX_STAGES, (size_t)(200 * 1024) / ks.tma_stage_bytes);
     if (stages >= 2 && ensure_dyn_smem(ks.persistent_tma, stages * ks.tma_stage_bytes) == cudaSuccess) {
       s->tma_stages = stages; s->tma_smem = stages * ks.tma_stage_bytes;
@@ -423,18 +427,36 @@ extern "C" int cudahm_set_model_consts(cudahm_sampler* s, const double* v, int n
   if (!s) return fail(s, CUDAHM_E_INVALID, "NULL handle");
   if (n != s->nconsts || (n > 0 && !v)) return fail(s, CUDAHM_E_INVALID, "model takes %d constants, got %d", s->nconsts, n);
   if (n == 0) { s->have_consts = true; return CUDAHM_OK; }
-  if (s->cfg.model == M_NORMAL3D_KNOWNCOV) {
-    // NORMAL3D_KNOWNCOV: {sigma_1..3, packed lower triangle of C_pop} (Eq. 3.3-3.4).  The kernels take
-    // h_j = 1/(2 sigma_j^2) and Q = packed lower triangle of C_pop^-1 with the diagonal halved (adjugate / determinant).
-    const double c11 = v[3], c21 = v[4], c22 = v[5], c31 = v[6], c32 = v[7], c33 = v[8];
-    const double a11 = c22 * c33 - c32 * c32, a21 = c31 * c32 - c21 * c33, a31 = c21 * c32 - c31 * c22;
-    const double a22 = c11 * c33 - c31 * c31, a32 = c31 * c21 - c11 * c32, a33 = c11 * c22 - c21 * c21;
-    const double det = c11 * a11 + c21 * a21 + c31 * a31;
-    if (!(v[0] > 0.0 && v[1] > 0.0 && v[2] > 0.0 && c11 > 0.0 && a33 > 0.0 && det > 0.0))
-      return fail(s, CUDAHM_E_INVALID, "model constants out of range (sigma_j > 0, C_pop positive definite)");
-    for (int j = 0; j < 3; ++j) s->P.mc[MN_H + j] = 0.5 / (v[j] * v[j]);
-    const double q[6] = {0.5 * a11 / det, a21 / det, 0.5 * a22 / det, a31 / det, a32 / det, 0.5 * a33 / det};
-    for (int j = 0; j < 6; ++j) s->P.mc[MN_Q + j] = q[j];
+  if (normal_family_p(s->cfg.model) > 0) {
+    // normal-normal family: {sigma_1..p, packed lower triangle of C_pop} (Eq. 3.3-3.4).  The kernels take
+    // h_j = 1/(2 sigma_j^2) and Q = packed lower triangle of C_pop^-1 with the diagonal halved.  C_pop^-1 = G^-T G^-1 from
+    // the Cholesky factor G of C_pop (long double; C_pop must be positive definite).
+    const int np = normal_family_p(s->cfg.model);
+    long double G[6][6] = {}, Gi[6][6] = {};
+    const double* Cp = v + np;
+    bool ok = true;
+    for (int j = 0; j < np; ++j) ok = ok && v[j] > 0.0 && std::isfinite(v[j]);
+    for (int r = 0; r < np && ok; ++r)
+      for (int k = 0; k <= r; ++k) {
+        long double a = Cp[r * (r + 1) / 2 + k];
+        for (int m = 0; m < k; ++m) a -= G[r][m] * G[k][m];
+        if (r == k) { ok = ok && a > 0.0L; G[r][r] = ok ? sqrtl(a) : 1.0L; }
+        else G[r][k] = a / G[k][k];
+      }
+    if (!ok) return fail(s, CUDAHM_E_INVALID, "model constants out of range (sigma_j > 0, C_pop positive definite)");
+    for (int c = 0; c < np; ++c)                       // Gi = G^-1 (lower triangular), column by column
+      for (int r = c; r < np; ++r) {
+        long double a = (r == c) ? 1.0L : 0.0L;
+        for (int m = c; m < r; ++m) a -= G[r][m] * Gi[m][c];
+        Gi[r][c] = a / G[r][r];
+      }
+    for (int j = 0; j < np; ++j) s->P.mc[MN_H + j] = 0.5 / (v[j] * v[j]);
+    for (int r = 0; r < np; ++r)
+      for (int c = 0; c <= r; ++c) {
+        long double a = 0.0L;                          // (C^-1)_rc = sum_m Gi[m][r] Gi[m][c], m >= r
+        for (int m = r; m < np; ++m) a += Gi[m][r] * Gi[m][c];
+        s->P.mc[np + r * (r + 1) / 2 + c] = (double)(r == c ? 0.5L * a : a);
+      }
     s->have_consts = true; s->have_init = false;
     invalidate_graph(s);
     return CUDAHM_OK;

@@ -1,0 +1,15 @@
+// inst_normal5d_knowncov.cu -- every kernel of model M_NORMAL5D_KNOWNCOV (its own translation unit: the models build in parallel).
+// p = 5: a thread holds two objects of p (p + 5) / 2 doubles each, so only the 256-thread block (255 registers) is built,
+// and the TMA-staged variant (one stage of its ring would not fit twice in shared memory) is not.
+#include "kernel_sets_impl.cuh"
+
+namespace hm {
+
+bool kernels_normal5d_knowncov(int precision, int block, KernelSet* k, ResidentSet* r) {
+  r->kernel = nullptr; r->n_base = 0;
+  if (precision != 0 || block != 256) return false;
+  *k = make_set<M_NORMAL5D_KNOWNCOV, double, 256, false>();
+  return true;
+}
+
+}  // namespace hm

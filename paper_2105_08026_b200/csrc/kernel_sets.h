@@ -29,5 +29,8 @@ bool kernels_binormal2d(int precision, int block, KernelSet* k, ResidentSet* r);
 bool kernels_linreg_me1d(int precision, int block, KernelSet* k, ResidentSet* r);
 bool kernels_bb1_fluxnoise1d(int precision, int block, KernelSet* k, ResidentSet* r);
 bool kernels_normal3d_knowncov(int precision, int block, KernelSet* k, ResidentSet* r);
+bool kernels_normal4d_knowncov(int precision, int block, KernelSet* k, ResidentSet* r);   // p >= 4: 256-thread blocks only
+bool kernels_normal5d_knowncov(int precision, int block, KernelSet* k, ResidentSet* r);
+bool kernels_normal6d_knowncov(int precision, int block, KernelSet* k, ResidentSet* r);
 
 }  // namespace hm

@@ -8,13 +8,14 @@
 
 namespace hm {
 
-template <int MODEL, class T, int BLOCK>
+template <int MODEL, class T, int BLOCK, bool WITH_TMA = true>
 KernelSet make_set() {
   KernelSet k;
   k.persistent = (const void*)k_persistent<MODEL, T, BLOCK, false>;
   k.persistent_ahead = (const void*)k_persistent<MODEL, T, BLOCK, true>;
   k.stage_step_bytes = (size_t)DrawSet<MODEL, T>::NV * BLOCK * sizeof(T);
-  k.persistent_tma = (const void*)k_persistent_tma<MODEL, T, BLOCK>;
+  k.persistent_tma = nullptr;
+  if constexpr (WITH_TMA) k.persistent_tma = (const void*)k_persistent_tma<MODEL, T, BLOCK>;
   k.tma_stage_bytes = (size_t)(ModelDims<MODEL>::p * (ModelDims<MODEL>::p + 3) / 2 + ModelDims<MODEL>::ncols) * (BLOCK - 32) * 16;
   k.sweep = (const void*)k_sweep<MODEL, T, BLOCK, false>;
   k.sweep_tap = (const void*)k_sweep<MODEL, T, BLOCK, true>;

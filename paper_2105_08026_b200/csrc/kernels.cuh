@@ -38,6 +38,9 @@ struct Params {
   double astar_chi;
   int max_blocks, pad_;
   long long obj_offset;          // global index of object 0 (sharded populations; even): keys the plate Philox streams
+  // frozen members, read by the HOLD kernel variants only
+  const unsigned char* mask;     // [Npad] 1 = update object i, 0 = hold it fixed; NULL = update everything
+  unsigned* cnt;                 // [Npad] RAM updates object i has taken (eta_n from the object's own count); NULL = global n
   TailCfg tail;
   DevTaps taps;
 };
@@ -76,7 +79,7 @@ __device__ __forceinline__ float hm_sqrt_pos(float x) { return x * rsqrtf(x); }
 //                normals: per object, draw 1 of object i; z = rad*(cs, sn), unit vector (cs, sn).
 //   fp32  p = 1: one call per pair (draw 0 of pair m): x -> u1, y -> u2, cos / sin branch, accept uniforms z / w.
 // i0 is the even object of the pair.  z[h][k]: normal k of object i0 + h.
-//         p = 3 normals:   per object, draws 1 and 2 of object i: (z0, z1) and (z2, -).
+//         p >= 3 normals:  per object, draws 1 + k of object i give (z_2k, z_2k+1), k = 0 .. ceil(p/2) - 1.
 template <int P, int ZD>
 __device__ __forceinline__ void pair_draws(unsigned long long seed, long long i0, uint32_t t, double (*z)[ZD], double* cs,
                                            double* sn, double* u) {
@@ -100,13 +103,19 @@ __device__ __forceinline__ void pair_draws(unsigned long long seed, long long i0
       const double rad = hm_sqrt_fast(-2.0 * hm_log_unit(u1));
       sincospi(2.0 * u2, &sn[h], &cs[h]);
       z[h][0] = rad * cs[h]; z[h][1] = rad * sn[h];
-      if constexpr (P == 3) {
-        static_assert(P < 3 || ZD >= 3, "z needs room for the third normal");
-        const U4 b2 = stream(seed, KIND_PLATE, (uint64_t)(i0 + h), t, 2u);
-        const double v1 = u01(b2.x, b2.y), v2 = u01(b2.z, b2.w);
-        double s2_, c2_;
-        sincospi(2.0 * v2, &s2_, &c2_);
-        z[h][2] = hm_sqrt_fast(-2.0 * hm_log_unit(v1)) * c2_;
+      if constexpr (P >= 3) {
+        // general p: Box-Muller pair k of object i comes from draw 1 + k (z_{2k}, z_{2k+1}); an odd p drops the last sine
+        static_assert(P < 3 || ZD >= P, "z needs room for all p normals");
+#pragma unroll
+        for (int k = 1; 2 * k < P; ++k) {
+          const U4 b2 = stream(seed, KIND_PLATE, (uint64_t)(i0 + h), t, 1u + (uint32_t)k);
+          const double v1 = u01(b2.x, b2.y), v2 = u01(b2.z, b2.w);
+          const double rad2 = hm_sqrt_fast(-2.0 * hm_log_unit(v1));
+          double s2_, c2_;
+          sincospi(2.0 * v2, &s2_, &c2_);
+          z[h][2 * k] = rad2 * c2_;
+          if (2 * k + 1 < P) z[h][2 * k + 1] = rad2 * s2_;
+        }
       }
     }
   }
@@ -205,7 +214,10 @@ template <int MODEL, class T> struct DrawSet {
   }
 };
 
-template <int MODEL, class T, bool TAP>
+// HOLD: the variant for frozen members.  An object whose mask byte is 0 takes no RAM step (chi, L and its
+// update count stay bit for bit; its draws are made and discarded, the streams being counter-based) but still contributes
+// a_i, b_i; with a per-object counter eta_n comes from the object's own update count n_i = count + 2.
+template <int MODEL, class T, bool TAP, bool HOLD = false>
 __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c, const long long base,
                                            T (*x)[VecOf<T>::n], T (*l)[VecOf<T>::n], const T (*d)[VecOf<T>::n], double* sum,
                                            const DrawSet<MODEL, T>* staged = nullptr) {
@@ -220,6 +232,17 @@ __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c
   for (int v = 0; v < VEC; ++v) {
     const long long i = base + v;
     const bool live = i < P.N;
+    bool upd = true;
+    T eta_v = c.eta;
+    if constexpr (HOLD) {
+      if (live && P.mask) upd = P.mask[i] != 0;
+      if (live && upd && P.cnt) {
+        const unsigned n_i = P.cnt[i];
+        P.cnt[i] = n_i + 1u;
+        // the common case (updated in every iteration so far) reuses the iteration's eta; same function, same argument
+        if (c.eta != T(0) && n_i + 1u != c.t) eta_v = (T)pow((double)n_i + 2.0, -P.tail.eta_exp);
+      }
+    }
     T xi[p], di[ncols];
     const T cs = csv[v], sn = snv[v], u = uu[v];
     const T* z = zz[v];
@@ -244,12 +267,12 @@ __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c
     const bool bad = diff != diff;
     const T la = bad ? T(-INFINITY) : (diff < T(0) ? diff : T(0));
     const T alpha = hm_exp_nonpos(la);
-    const bool acc = u < alpha;
+    const bool acc = HOLD ? (upd && u < alpha) : (u < alpha);
     const typename PL::Pt qn = acc ? qp : qc;
 #pragma unroll
     for (int j = 0; j < p; ++j) x[j][v] = acc ? yi[j] : xi[j];
     // step 3: L <- L chol(I + c uu^T), u = z/|z| = (cs, sn)
-    const T cc = c.eta * (alpha - c.astar);
+    const T cc = eta_v * (alpha - c.astar);
     T ln[ntri];
     if constexpr (p == 1) {
       ln[0] = l[0][v] * hm_sqrt_pos(T(1) + cc);
@@ -291,10 +314,14 @@ __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c
     // population terms at the new chi, fp64
     const double a = PL::pop(qn, di, c.kc, P.mc), b = PL::pop(qn, di, c.kp, P.mc);
     if (live) {
+      if constexpr (HOLD) {
+#pragma unroll
+        for (int k = 0; k < ntri; ++k) ln[k] = upd ? ln[k] : l[k][v];
+      }
 #pragma unroll
       for (int k = 0; k < ntri; ++k) l[k][v] = ln[k];
       sum[0] += a; sum[1] += b - a;
-      sum[2] += acc ? 1.0 : 0.0; sum[3] += bad ? 1.0 : 0.0;
+      sum[2] += acc ? 1.0 : 0.0; sum[3] += (bad && upd) ? 1.0 : 0.0;
       if (c.do_mom) {
 #pragma unroll
         for (int j = 0; j < p; ++j) {
@@ -310,11 +337,11 @@ __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c
       if (TAP) {
         const DevTaps& tp = P.taps;
 #pragma unroll
-        for (int j = 0; j < p; ++j) if (tp.chi_prop) tp.chi_prop[j * P.N + i] = (double)yi[j];
+        for (int j = 0; j < p; ++j) if (tp.chi_prop) tp.chi_prop[j * P.N + i] = (double)(upd ? yi[j] : xi[j]);
         if (tp.pi_cur) tp.pi_cur[i] = (double)pc + tp.shift_c;
-        if (tp.pi_prop) tp.pi_prop[i] = (double)pp + tp.shift_c;
-        if (tp.alpha) tp.alpha[i] = (double)alpha;
-        if (tp.u) tp.u[i] = (double)u;
+        if (tp.pi_prop) tp.pi_prop[i] = (double)(upd ? pp : pc) + tp.shift_c;
+        if (tp.alpha) tp.alpha[i] = upd ? (double)alpha : 0.0;
+        if (tp.u) tp.u[i] = upd ? (double)u : 1.0;
         if (tp.accepted) tp.accepted[i] = acc ? 1 : 0;
 #pragma unroll
         for (int k = 0; k < ntri; ++k) if (tp.L_new) tp.L_new[k * P.N + i] = (double)ln[k];
@@ -340,7 +367,7 @@ __device__ __forceinline__ double selection_slice(const Params& P, const ThetaK&
 }
 
 // one step of the sweep: load the thread's VEC objects, update, store
-template <int MODEL, class T, bool TAP>
+template <int MODEL, class T, bool TAP, bool HOLD = false>
 __device__ __forceinline__ void sweep_step(const Params& P, const SweepCtx<T>& c, const long long base, double* acc,
                                            const DrawSet<MODEL, T>* staged) {
   constexpr int p = ModelDims<MODEL>::p, ntri = p * (p + 1) / 2, ncols = ModelDims<MODEL>::ncols;
@@ -356,7 +383,7 @@ __device__ __forceinline__ void sweep_step(const Params& P, const SweepCtx<T>& c
   for (int k = 0; k < ntri; ++k) ld_vec<T>(Lm + k * Npad + base, l[k], false);
 #pragma unroll
   for (int cc = 0; cc < ncols; ++cc) ld_vec<T>(dat + cc * Npad + base, d[cc], true);
-  update_vec<MODEL, T, TAP>(P, c, base, x, l, d, acc, staged);
+  update_vec<MODEL, T, TAP, HOLD>(P, c, base, x, l, d, acc, staged);
 #pragma unroll
   for (int j = 0; j < p; ++j) st_vec(chi + j * Npad + base, x[j]);
 #pragma unroll
@@ -386,7 +413,7 @@ __device__ __forceinline__ void prefetch_step(const Params& P, const long long b
 
 // part[NPART] receives this thread's partial sums in ascending object order.  stage / n_stage: the plate draws of
 // the thread's first n_stage steps, made ahead by stage_draws (k_persistent); the same values bit for bit.
-template <int MODEL, class T, bool TAP, bool AHEAD = false>
+template <int MODEL, class T, bool TAP, bool AHEAD = false, bool HOLD = false>
 __device__ __forceinline__ void sweep(const Params& P, const Iter& it, double* part, const T* stage = nullptr,
                                       const int n_stage = 0, const bool prefetch = false) {
   constexpr int VEC = VecOf<T>::n;
@@ -412,7 +439,7 @@ __device__ __forceinline__ void sweep(const Params& P, const Iter& it, double* p
       sweep_step<MODEL, T, TAP>(P, c, base, acc, nullptr);
     }
   } else {
-    for (; base < N; base += stride) sweep_step<MODEL, T, TAP>(P, c, base, acc, nullptr);
+    for (; base < N; base += stride) sweep_step<MODEL, T, TAP, HOLD>(P, c, base, acc, nullptr);
   }
   part[0] = acc[0]; part[1] = acc[1]; part[2] = selection_slice<MODEL>(P, c.kp, (int)blockDim.x); part[3] = acc[2]; part[4] = acc[3];
 }

@@ -16,14 +16,18 @@
 namespace hm {
 
 enum : int { M_NORMAL1D = 0, M_THINNED_SCHECHTER1D = 1, M_BINORMAL2D = 2, M_LINREG_ME1D = 3, M_BB1_FLUXNOISE1D = 4,
-             M_NORMAL3D_KNOWNCOV = 5 };
+             M_NORMAL3D_KNOWNCOV = 5, M_NORMAL4D_KNOWNCOV = 6, M_NORMAL5D_KNOWNCOV = 7, M_NORMAL6D_KNOWNCOV = 8 };
+// latent dimension of the normal-normal family (PAPER.md:146-166 for p = 3; Eq. 2.6 holds for any p), 0 for the others
+HM_HD constexpr int normal_family_p(int model) {
+  return (model >= M_NORMAL3D_KNOWNCOV && model <= M_NORMAL6D_KNOWNCOV) ? model - M_NORMAL3D_KNOWNCOV + 3 : 0;
+}
 enum : int { MC_FLIM = 0, MC_SIGF = 1, MC_XLO = 2, MC_XHI = 3, MC_RMIN = 4, MC_RMAX = 5, MC_INV2S2 = 6 };
 // M4 keeps sigma_0^2 and alpha^2 (Eq. 5.8) where M1 keeps F_lim and sigma_F; the threshold goes to slot 6
 enum : int { MB_S0SQ = 0, MB_A2 = 1, MB_FTH = 6 };
-// M5: h_j = 1/(2 sigma_j^2) (3), then Q = the packed lower triangle of C_pop^-1 with the diagonal halved (6), so that
-// -1/2 e^T C_pop^-1 e = -(Q0 e1^2 + Q1 e2 e1 + Q2 e2^2 + Q3 e3 e1 + Q4 e3 e2 + Q5 e3^2)
-enum : int { MN_H = 0, MN_Q = 3 };
-constexpr int MC_N = 10;      // model-constant slots
+// normal-normal family (p = 3 .. 6): h_j = 1/(2 sigma_j^2) (p values), then Q = the packed lower triangle of C_pop^-1 with
+// the diagonal halved (p (p + 1) / 2 values, starting at slot p), so that -1/2 e^T C_pop^-1 e = -sum_i e_i sum_{j<=i} Q_ij e_j
+enum : int { MN_H = 0 };
+constexpr int MC_N = 27;      // model-constant slots (p = 6: 6 + 21)
 constexpr int NQUAD = 1024;   // selection-integral nodes (BASELINE.json configs[1])
 
 template <int MODEL> struct ModelDims;
@@ -33,6 +37,9 @@ template <> struct ModelDims<M_BINORMAL2D>          { static constexpr int p = 2
 template <> struct ModelDims<M_LINREG_ME1D>         { static constexpr int p = 1, dtheta = 3, ncols = 3, nconsts = 0; };
 template <> struct ModelDims<M_BB1_FLUXNOISE1D>     { static constexpr int p = 1, dtheta = 3, ncols = 2, nconsts = 7; };
 template <> struct ModelDims<M_NORMAL3D_KNOWNCOV>   { static constexpr int p = 3, dtheta = 3, ncols = 3, nconsts = 9; };
+template <> struct ModelDims<M_NORMAL4D_KNOWNCOV>   { static constexpr int p = 4, dtheta = 4, ncols = 4, nconsts = 14; };
+template <> struct ModelDims<M_NORMAL5D_KNOWNCOV>   { static constexpr int p = 5, dtheta = 5, ncols = 5, nconsts = 20; };
+template <> struct ModelDims<M_NORMAL6D_KNOWNCOV>   { static constexpr int p = 6, dtheta = 6, ncols = 6, nconsts = 27; };
 
 // models whose likelihood carries a theta-only selection term (the denominator of Eq. 4.4) summed over
 // the NQUAD nodes, whose latent is x = ln L with flux columns (Fhat, g = 1/(4 pi r^2)) and a bounded support
@@ -45,7 +52,10 @@ inline bool model_dims(int model, int* p, int* dtheta, int* ncols, int* nconsts)
     case M_BINORMAL2D:          *p = 2; *dtheta = 5; *ncols = 4; *nconsts = 0; return true;
     case M_LINREG_ME1D:         *p = 1; *dtheta = 3; *ncols = 3; *nconsts = 0; return true;
     case M_BB1_FLUXNOISE1D:     *p = 1; *dtheta = 3; *ncols = 2; *nconsts = 7; return true;
-    case M_NORMAL3D_KNOWNCOV:   *p = 3; *dtheta = 3; *ncols = 3; *nconsts = 9; return true;
+    case M_NORMAL3D_KNOWNCOV: case M_NORMAL4D_KNOWNCOV: case M_NORMAL5D_KNOWNCOV: case M_NORMAL6D_KNOWNCOV: {
+      const int np = normal_family_p(model);
+      *p = np; *dtheta = np; *ncols = np; *nconsts = np + np * (np + 1) / 2; return true;
+    }
   }
   return false;
 }
@@ -72,8 +82,9 @@ HM_HD void theta_consts_part(int model, int part, const double* th, ThetaK& k) {
       if (part == 1) { const double ch = cosh(th[4]); k.v[4] = -th[2] - th[3] + log(ch); k.v[5] = 0.5 * ch * ch; }
       if (part == 2) k.v[6] = tanh(th[4]);
       break;
-    case M_NORMAL3D_KNOWNCOV:   // theta = mu; C_pop is a known model constant
-      if (part == 0) { k.v[0] = th[0]; k.v[1] = th[1]; k.v[2] = th[2]; }
+    case M_NORMAL3D_KNOWNCOV: case M_NORMAL4D_KNOWNCOV: case M_NORMAL5D_KNOWNCOV: case M_NORMAL6D_KNOWNCOV:
+      // theta = mu; C_pop is a known model constant
+      if (part == 0) { for (int j = 0; j < normal_family_p(model); ++j) k.v[j] = th[j]; }
       break;
     case M_BB1_FLUXNOISE1D:
       // (beta, ln l, ln u): f = log C + (beta+1)(x - ln u) + log(1 - e^(-L/l)) - L/u   (Eq. 5.1 in x = ln L).
@@ -120,8 +131,12 @@ HM_HD double log_prior(int model, const double* th) {
     case M_THINNED_SCHECHTER1D:
       return (th[0] > -2.0 && th[0] < 0.0 && fabs(th[1]) <= 20.0 && fabs(th[2]) <= 50.0)
                  ? -hm_log_any_pos(1.0 + th[0] * th[0]) : ninf;
-    case M_NORMAL3D_KNOWNCOV:   // "uniform hyperpriors" on a wide box
-      return (fabs(th[0]) <= 1e3 && fabs(th[1]) <= 1e3 && fabs(th[2]) <= 1e3) ? 0.0 : ninf;
+    case M_NORMAL3D_KNOWNCOV: case M_NORMAL4D_KNOWNCOV: case M_NORMAL5D_KNOWNCOV: case M_NORMAL6D_KNOWNCOV: {
+      // "uniform hyperpriors" on a wide box
+      bool in = true;
+      for (int j = 0; j < normal_family_p(model); ++j) in = in && fabs(th[j]) <= 1e3;
+      return in ? 0.0 : ninf;
+    }
     case M_BB1_FLUXNOISE1D:     // Eq. 5.5 as a density in (beta, ln l, ln u): l / (u (1 + beta^2)), l < u
       return (th[0] > -2.0 && th[0] < 0.0 && th[1] < th[2] && fabs(th[1]) <= 30.0 && fabs(th[2]) <= 30.0)
                  ? th[1] - th[2] - hm_log_any_pos(1.0 + th[0] * th[0]) : ninf;
@@ -236,23 +251,45 @@ template <class T> struct Plate<M_BB1_FLUXNOISE1D, T> {
   }
 };
 
-// M5, the normal-normal benchmark: chi ~ N3(mu, C_pop), y_j ~ N(chi_j, sigma_j^2), C_pop and sigma_j known.
-template <class T> struct Plate<M_NORMAL3D_KNOWNCOV, T> {
-  struct Pt { T x1, x2, x3; };
-  __device__ __forceinline__ static Pt point(const T* chi) { return Pt{chi[0], chi[1], chi[2]}; }
+// The normal-normal family (PAPER.md:146-166 is p = 3): chi ~ N_p(mu, C_pop), y_j ~ N(chi_j, sigma_j^2), C_pop and sigma_j known.
+template <int P, class T> struct PlateNormalP {
+  struct Pt { T x[P]; };
+  __device__ __forceinline__ static Pt point(const T* chi) {
+    Pt q;
+#pragma unroll
+    for (int j = 0; j < P; ++j) q.x[j] = chi[j];
+    return q;
+  }
+  // sum_i e_i sum_{j<=i} Q_ij e_j with Q the packed lower triangle (diagonal halved)
   template <class R>
-  __device__ __forceinline__ static R quad(R e1, R e2, R e3, const R* Q) {
-    return e1 * (Q[0] * e1) + e2 * (Q[1] * e1 + Q[2] * e2) + e3 * (Q[3] * e1 + Q[4] * e2 + Q[5] * e3);
+  __device__ __forceinline__ static R quad(const R* e, const R* Q) {
+    R s = R(0);
+#pragma unroll
+    for (int i = 0; i < P; ++i) {
+      R a = R(0);
+#pragma unroll
+      for (int j = 0; j <= i; ++j) a += Q[i * (i + 1) / 2 + j] * e[j];
+      s += e[i] * a;
+    }
+    return s;
   }
   __device__ __forceinline__ static T target(const Pt& q, const T* d, const KT<T>& k, const T* mc) {
-    const T r1 = d[0] - q.x1, r2 = d[1] - q.x2, r3 = d[2] - q.x3;
-    return -(r1 * r1) * mc[MN_H] - (r2 * r2) * mc[MN_H + 1] - (r3 * r3) * mc[MN_H + 2] -
-           quad<T>(q.x1 - k.v[0], q.x2 - k.v[1], q.x3 - k.v[2], mc + MN_Q);
+    T s = T(0), e[P];
+#pragma unroll
+    for (int j = 0; j < P; ++j) { const T r = d[j] - q.x[j]; s -= (r * r) * mc[MN_H + j]; e[j] = q.x[j] - k.v[j]; }
+    return s - quad<T>(e, mc + P);
   }
   __device__ __forceinline__ static double pop(const Pt& q, const T*, const ThetaK& k, const double* mc) {
-    return -quad<double>((double)q.x1 - k.v[0], (double)q.x2 - k.v[1], (double)q.x3 - k.v[2], mc + MN_Q);
+    double e[P];
+#pragma unroll
+    for (int j = 0; j < P; ++j) e[j] = (double)q.x[j] - k.v[j];
+    return -quad<double>(e, mc + P);
   }
 };
+template <class T> struct Plate<M_NORMAL3D_KNOWNCOV, T> : PlateNormalP<3, T> {};
+template <class T> struct Plate<M_NORMAL4D_KNOWNCOV, T> : PlateNormalP<4, T> {};
+template <class T> struct Plate<M_NORMAL5D_KNOWNCOV, T> : PlateNormalP<5, T> {};
+template <class T> struct Plate<M_NORMAL6D_KNOWNCOV, T> : PlateNormalP<6, T> {};
 
 // one node of the selection sum: W_k rho(x_k; theta) from the node's x_k and e^(x_k)
 template <int MODEL>

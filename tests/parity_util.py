@@ -38,7 +38,7 @@ def make_pair(model, n, seed, precision=B.F64, theta_mode=B.THETA_DEVICE_TAIL, a
         kw = dict(fp32=True) if (precision == B.F32_STATE_F64_REDUCE and model in (0, 3)) else {}
         if model == 3 and precision == B.F64:
             kw = dict(fp32=False)
-        inputs = maker(n, seed, **kw) if maker else synth.make_normalpd_knowncov(n, seed, **extra.pop("maker_kw", {}))
+        inputs = maker(n, seed, **kw) if maker else synth.make_normalpd_knowncov(n, seed, p=model - 2)
     th0 = inputs["theta0"] if theta0 is None else theta0
     orc = None
     if want_oracle:

@@ -21,8 +21,11 @@ CASES = [
     (B.M_LINREG_ME1D, B.F32_STATE_F64_REDUCE, 0.44, 10007),
     (B.M_BB1_FLUXNOISE1D, B.F64, 0.44, 4099),
     (B.M_NORMAL3D_KNOWNCOV, B.F64, 0.234, 3003),
+    (B.M_NORMAL4D_KNOWNCOV, B.F64, 0.234, 2051),
+    (B.M_NORMAL5D_KNOWNCOV, B.F64, 0.234, 1031),
+    (B.M_NORMAL6D_KNOWNCOV, B.F64, 0.234, 1543),
 ]
-IDS = ["M0-f64", "M1-f64", "M2-f64", "M3-f64", "M0-f32", "M3-f32", "M4-f64", "M5-f64"]
+IDS = ["M0-f64", "M1-f64", "M2-f64", "M3-f64", "M0-f32", "M3-f32", "M4-f64", "M5-f64", "p4-f64", "p5-f64", "p6-f64"]
 
 
 @pytest.mark.parametrize("model,precision,astar,n", CASES, ids=IDS)
@@ -73,8 +76,9 @@ def test_lockstep_trajectory(model, precision, astar, n):
 @pytest.mark.parametrize("mode", [B.THETA_HOST, B.THETA_GRAPH, B.THETA_DEVICE_TAIL], ids=["host", "graph", "tail"])
 @pytest.mark.parametrize("model,astar,n", [(B.M_NORMAL1D, 0.44, 1000), (B.M_THINNED_SCHECHTER1D, 0.44, 3000),
                                              (B.M_BINORMAL2D, 0.234, 2000), (B.M_BB1_FLUXNOISE1D, 0.44, 3000),
-                                             (B.M_NORMAL3D_KNOWNCOV, 0.234, 2001)],
-                         ids=["M0", "M1", "M2", "M4", "M5"])
+                                             (B.M_NORMAL3D_KNOWNCOV, 0.234, 2001), (B.M_NORMAL4D_KNOWNCOV, 0.234, 1501),
+                                             (B.M_NORMAL5D_KNOWNCOV, 0.234, 1201), (B.M_NORMAL6D_KNOWNCOV, 0.234, 1001)],
+                         ids=["M0", "M1", "M2", "M4", "M5", "p4", "p5", "p6"])
 def test_free_running_matches_oracle(model, astar, n, mode):
     """cudahm_run (no taps, no resync) for 120 iterations in every theta mode against oracle_run: same theta
     trace, same chi / L, same moments, same counters.  (~1e5 decisions at ~1e-9 tie probability each.)"""
@@ -326,13 +330,15 @@ def test_ragged_and_degenerate_sizes(n, precision):
     assert gpu.get_stats()["iterations"] == orc.get_stats()["iterations"]
 
 
+@pytest.mark.parametrize("model", [B.M_NORMAL3D_KNOWNCOV, B.M_NORMAL4D_KNOWNCOV, B.M_NORMAL5D_KNOWNCOV, B.M_NORMAL6D_KNOWNCOV],
+                         ids=["p3", "p4", "p5", "p6"])
 @pytest.mark.parametrize("n", [1, 2, 3, 5, 63, 65, 513])
-def test_ragged_sizes_p3(n):
-    """The p = 3 path (general rank-one update, two Box-Muller pairs per object) on ragged and tiny populations."""
-    orc, gpu, inp = make_pair(B.M_NORMAL3D_KNOWNCOV, n, seed=4, astar=0.234, max_trace_rows=16)
+def test_ragged_sizes_p3(n, model):
+    """The p >= 3 path (general rank-one update, ceil(p/2) Box-Muller pairs per object) on ragged and tiny populations."""
+    orc, gpu, inp = make_pair(model, n, seed=4, astar=0.234, max_trace_rows=16)
     st = sync_gpu_to_oracle(orc, gpu)
     to, tg = orc.step(taps=True), gpu.debug_step()
-    compare_step(to, tg, B.F64, st, what=f"N={n}", ctx=dict(model=B.M_NORMAL3D_KNOWNCOV, inputs=inp, astar=0.234))
+    compare_step(to, tg, B.F64, st, what=f"N={n}", ctx=dict(model=model, inputs=inp, astar=0.234))
     sync_gpu_to_oracle(orc, gpu)
     gpu.run(8, 0, 1, sync=True)
     orc.run(8, 0, 1)

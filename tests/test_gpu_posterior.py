@@ -11,6 +11,7 @@ from paper_2105_08026_b200 import binding as B
 from paper_2105_08026_b200 import synth
 from test_oracle_bb1 import check_bb1_posterior
 from test_oracle_nn3 import check_nn3_posterior
+from test_oracle_nnp import check_nnp_posterior
 from test_oracle_posterior import (check_binormal_posterior, check_linreg_posterior, check_normal1d_posterior,
                                    check_schechter_posterior)
 
@@ -71,3 +72,10 @@ def test_m5_theta_posterior_on_the_gpu():
     n = 20000
     inp = synth.make_normal3d_knowncov(n, seed=152)
     check_nn3_posterior(inp, _gpu_chain(B.M_NORMAL3D_KNOWNCOV, inp, n, 152, 5000, 40000, 0.234))
+
+
+@pytest.mark.parametrize("p", [4, 5, 6])
+def test_normal_family_theta_posterior_on_the_gpu(p):
+    n = 20000
+    inp = synth.make_normalpd_knowncov(n, seed=160 + p, p=p)
+    check_nnp_posterior(inp, _gpu_chain(synth.nnp_model(p), inp, n, 160 + p, 8000, 40000, 0.234), p)

@@ -14,10 +14,11 @@ from parity_util import compare_step  # noqa: E402
 
 CASES = [(0, 0, 0.44, synth.make_normal1d, {}), (1, 0, 0.44, synth.make_thinned_schechter1d, {}),
          (2, 0, 0.234, synth.make_binormal2d, {}), (3, 1, 0.44, synth.make_linreg_me1d, dict(fp32=True)),
-         (4, 0, 0.44, synth.make_bb1_fluxnoise1d, {}), (5, 0, 0.234, synth.make_normal3d_knowncov, {})]
+         (4, 0, 0.44, synth.make_bb1_fluxnoise1d, {}), (5, 0, 0.234, synth.make_normal3d_knowncov, {}),
+         (8, 0, 0.234, synth.make_normalpd_knowncov, dict(p=6))]
 
 
-@pytest.mark.parametrize("model,precision,astar,maker,kw", CASES, ids=["M0", "M1", "M2", "M3f32", "M4", "M5"])
+@pytest.mark.parametrize("model,precision,astar,maker,kw", CASES, ids=["M0", "M1", "M2", "M3f32", "M4", "M5", "p6"])
 def test_oracle_against_itself_and_perturbed_taps(model, precision, astar, maker, kw):
     n = 257
     inp = maker(n, 5, **kw)
