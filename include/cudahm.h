@@ -110,6 +110,12 @@ typedef struct {
    * objects [object_offset, object_offset + n_objects) of a population of n_objects_total                          */
   int64_t  object_offset;        /* even, >= 0: global index of this handle's first object (keys its Philox streams) */
   int64_t  n_objects_total;      /* 0 = n_objects (not sharded)                                                    */
+  /* frozen members (member properties "which should be held fixed over the course of posterior
+   * simulation").  Either switch selects the HOLD variants of the streaming kernels (not the on-chip kernel, no staged
+   * draws / TMA); as-built extra state: 1 byte (mask) and 4 bytes (counter) per object, read and written every iteration. */
+  int32_t  update_mask;          /* 1: reserve a per-object update mask (cudahm_set_update_mask); all ones until set    */
+  int32_t  per_object_counter;   /* 1: eta_n of object i uses ITS OWN update count, n_i = count_i + 2, instead of the
+                                    global n = t + 1 (identical while every object is updated in every iteration)  */
 } cudahm_config;
 
 typedef struct {
@@ -176,6 +182,17 @@ int cudahm_set_model_consts(cudahm_sampler* s, const double* v, int n);
  * zero prior density or a non-finite theta-only term (the chain needs pi(X_1) > 0; set_state likewise). */
 int cudahm_set_init(cudahm_sampler* s, const void* chi0_or_null, int chi0_on_device, const double* theta0,
                     const double* theta_chol0_or_null);
+
+/* Per-object update mask (needs cfg.update_mask): N bytes, host or device; 1 = object i takes RAM steps 1-3 as usual,
+ * 0 = object i is held fixed -- chi_i, L_i and its update count stay bit for bit -- but still contributes log f(chi_i; theta)
+ * and log f(chi_i; theta') to the population sums.  NULL = update everything again.  May be changed between runs; copied.
+ * Taps of a held object: chi_prop = chi, pi_prop = pi_cur, alpha = 0, u = 1, accepted = 0, L_new = L.  chi_proposals counts
+ * updated objects only.  CUDAHM_E_STATE without cfg.update_mask, CUDAHM_E_UNSUPPORTED on a sharded handle. */
+int cudahm_set_update_mask(cudahm_sampler* s, const uint8_t* mask_or_null, int mask_on_device);
+/* Per-object update counts (needs cfg.per_object_counter), N host values.  set_init zeroes them, set_state(t) sets them
+ * all to t (as if every object had been updated in every iteration so far); set_counters overrides. */
+int cudahm_get_counters(cudahm_sampler* s, uint32_t* out);
+int cudahm_set_counters(cudahm_sampler* s, const uint32_t* in);
 
 /* Run n_iter more Gibbs iterations (resumable: continues from the current iteration index t).  Moments are
  * accumulated for t > burn_in, the trace takes theta whenever t > burn_in and (t - burn_in) % thin == 0.

@@ -137,7 +137,7 @@ class Sampler:
     def __init__(self, model, n_objects, seed=0, precision=F64, target_accept_chi=0.4,
                  target_accept_theta=0.234, eta_exponent=2.0 / 3.0, init_scale_chi=1.0,
                  freeze_theta=False, keep_chi_moments=False, adapt_until=0, prior_mean=None, prior_sd=None,
-                 object_offset=0, n_objects_total=0, per_object_counter=False):
+                 object_offset=0, n_objects_total=0, per_object_counter=False, update_mask=False):
         self.dims = model_dims(model)
         self.N = int(n_objects)
         self.p, self.dtheta = self.dims["p"], self.dims["dtheta"]

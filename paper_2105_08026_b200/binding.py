@@ -29,7 +29,8 @@ FLOOR_LAUNCH, FLOOR_GRAPH, FLOOR_GRID_BARRIER, FLOOR_HOST_SYNC = 0, 1, 2, 3
 EXPORTS = ["cudahm_model_dims", "cudahm_workspace_bytes", "cudahm_create", "cudahm_destroy", "cudahm_set_data",
            "cudahm_set_model_consts", "cudahm_set_init", "cudahm_run", "cudahm_debug_step",
            "cudahm_get_theta_trace", "cudahm_get_chi_moments", "cudahm_get_stats", "cudahm_get_state",
-           "cudahm_set_state", "cudahm_sync", "cudahm_last_error", "cudahm_shard_sweep", "cudahm_shard_decide", "cudahm_probe_floor", "cudahm_probe_fma_peak"]
+           "cudahm_set_state", "cudahm_sync", "cudahm_last_error", "cudahm_shard_sweep", "cudahm_shard_decide", "cudahm_set_update_mask", "cudahm_get_counters", "cudahm_set_counters",
+           "cudahm_probe_floor", "cudahm_probe_fma_peak"]
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int32)
@@ -44,7 +45,8 @@ class Config(C.Structure):
                 ("block_threads", C.c_int32), ("blocks_per_sm", C.c_int32), ("flags", C.c_int32),
                 ("max_trace_rows", C.c_int64), ("adapt_until", C.c_int64),
                 ("prior_mean", C.c_double * 8), ("prior_isd", C.c_double * 8),
-                ("object_offset", C.c_int64), ("n_objects_total", C.c_int64)]
+                ("object_offset", C.c_int64), ("n_objects_total", C.c_int64),
+                ("update_mask", C.c_int32), ("per_object_counter", C.c_int32)]
 
 
 class Stats(C.Structure):
@@ -95,6 +97,9 @@ def load():
     L.cudahm_set_state.argtypes = [vp, vp, vp, _dp, _dp, C.c_int64]
     L.cudahm_shard_sweep.argtypes = [vp, C.c_int64, C.c_int32, _dp]
     L.cudahm_shard_decide.argtypes = [vp, C.c_int64, C.c_int32, _dp]
+    L.cudahm_set_update_mask.argtypes = [vp, vp, C.c_int]
+    L.cudahm_get_counters.argtypes = [vp, vp]
+    L.cudahm_set_counters.argtypes = [vp, vp]
     L.cudahm_sync.argtypes = [vp]
     L.cudahm_last_error.argtypes = [vp]
     L.cudahm_last_error.restype = C.c_char_p
@@ -125,7 +130,8 @@ def model_dims(model):
 def make_config(model, n_objects, seed=0, precision=F64, theta_mode=THETA_DEVICE_TAIL, target_accept_chi=0.4,
                 target_accept_theta=0.234, eta_exponent=2.0 / 3.0, init_scale_chi=1.0, freeze_theta=False,
                 keep_chi_moments=False, max_trace_rows=0, block_threads=0, blocks_per_sm=0, flags=0, adapt_until=0,
-                prior_mean=None, prior_sd=None, object_offset=0, n_objects_total=0):
+                prior_mean=None, prior_sd=None, object_offset=0, n_objects_total=0, update_mask=False,
+                per_object_counter=False):
     d = model_dims(model)
     cfg = Config(C.sizeof(Config), model, precision, theta_mode, int(n_objects), d["p"], d["dtheta"], d["n_cols"],
                   int(freeze_theta), seed, target_accept_chi, target_accept_theta, eta_exponent, init_scale_chi,
@@ -135,6 +141,7 @@ def make_config(model, n_objects, seed=0, precision=F64, theta_mode=THETA_DEVICE
             cfg.prior_mean[j] = float(m)
             cfg.prior_isd[j] = 0.0 if not np.isfinite(sd) else 1.0 / float(sd)
     cfg.object_offset, cfg.n_objects_total = int(object_offset), int(n_objects_total)
+    cfg.update_mask, cfg.per_object_counter = int(update_mask), int(per_object_counter)
     return cfg
 
 
@@ -213,6 +220,33 @@ class Sampler:
         with self._dev():
             self._ck(self.lib.cudahm_set_init(self._h, None if c0 is None else C.c_void_p(c0.ctypes.data), 0,
                                               _d(th), _d(l0)))
+
+    def set_update_mask(self, mask):
+        """mask: N bytes (1 = update, 0 = hold fixed), host array or CUDA uint8 tensor; None = update everything."""
+        torch = self._torch
+        with self._dev():
+            if mask is None:
+                self._ck(self.lib.cudahm_set_update_mask(self._h, None, 0))
+            elif isinstance(mask, torch.Tensor) and mask.is_cuda:
+                m = mask.contiguous()
+                assert m.dtype == torch.uint8 and m.numel() == self.N
+                self._ck(self.lib.cudahm_set_update_mask(self._h, C.c_void_p(m.data_ptr()), 1))
+            else:
+                m = np.ascontiguousarray(np.asarray(mask, dtype=np.uint8))
+                assert m.shape == (self.N,)
+                self._ck(self.lib.cudahm_set_update_mask(self._h, C.c_void_p(m.ctypes.data), 0))
+
+    def get_counters(self):
+        out = np.empty(self.N, dtype=np.uint32)
+        with self._dev():
+            self._ck(self.lib.cudahm_get_counters(self._h, C.c_void_p(out.ctypes.data)))
+        return out
+
+    def set_counters(self, c):
+        c = np.ascontiguousarray(np.asarray(c, dtype=np.uint32))
+        assert c.shape == (self.N,)
+        with self._dev():
+            self._ck(self.lib.cudahm_set_counters(self._h, C.c_void_p(c.ctypes.data)))
 
     def run(self, n_iter, burn_in=0, thin=1, sync=False):
         with self._dev():

@@ -25,7 +25,7 @@ namespace {
 thread_local std::string g_err;
 
 struct Layout {
-  size_t chi, L, data, mom_mean, mom_M2, mom_var, slots, mbox, blk_cnt, iter, trace, totals, qx, qex, qW, total;
+  size_t chi, L, data, mom_mean, mom_M2, mom_var, slots, mbox, blk_cnt, iter, trace, totals, qx, qex, qW, mask, cnt, total;
 };
 
 constexpr int MAX_BLOCKS = 148 * 8 * 2;   // upper bound on the grid (slots capacity)
@@ -65,6 +65,9 @@ struct cudahm_sampler {
   bool have_data = false, have_consts = false, have_init = false;
   int num_sms = 0, grid = 1, block = 512, vec = 2;
   long long t_done = 0;             // iterations completed (host mirror)
+  bool hold = false;                // frozen-member kernel variants (update mask and / or per-object counter)
+  long long n_active = 0;           // objects the mask lets update (N without a mask)
+  long long h_proposals = 0;        // plate proposals made so far (host mirror: iterations x updated objects)
   long long h_trace_rows = 0;       // host mirrors of Iter::trace_rows / mom_count: pure functions of the (t, burn_in, thin)
   long long h_mom_count = 0;        // history, so cudahm_run never has to read the device before it launches
   long long launches = 0;
@@ -156,6 +159,7 @@ bool valid_config(const cudahm_config* c, int* p, int* dt, int* nc, int* nk) {
     return false;
   if (c->blocks_per_sm < 0 || c->adapt_until < 0) return false;
   if (c->object_offset < 0 || (c->object_offset & 1) || c->n_objects_total < 0) return false;
+  if ((c->update_mask | c->per_object_counter) & ~1) return false;
   if (c->n_objects_total != 0 && c->object_offset + c->n_objects > c->n_objects_total) return false;
   for (int j = 0; j < 8; ++j)
     if (!(c->prior_isd[j] >= 0.0) || !std::isfinite(c->prior_isd[j]) || !std::isfinite(c->prior_mean[j])) return false;
@@ -181,6 +185,8 @@ Layout make_layout(const cudahm_config& c, int p, int ncols, int dtheta) {
   l.trace = take((size_t)c.max_trace_rows * dtheta * 8);
   l.totals = take(NPART * 8);
   l.qx = take(NQUAD * 8); l.qex = take(NQUAD * 8); l.qW = take(NQUAD * 8);
+  l.mask = take(c.update_mask ? Npad : 0);
+  l.cnt = take(c.per_object_counter ? Npad * 4 : 0);
   l.total = o;
   return l;
 }
@@ -222,6 +228,8 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
     if (cudaGetDevice(&dev0) == cudaSuccess) cudaDeviceGetAttribute(&sms0, cudaDevAttrMultiProcessorCount, dev0);
     if ((cfg->n_objects + vec * 512 - 1) / (vec * 512) < (sms0 > 0 ? sms0 : 148)) block = 256;
   }
+  if (cfg->update_mask && cfg->n_objects_total != 0 && cfg->n_objects_total != cfg->n_objects)
+    return fail(nullptr, CUDAHM_E_UNSUPPORTED, "an update mask on a sharded handle is not supported");
   KernelSet ks;
   ResidentSet rs;
   if (!pick_kernels(cfg->model, cfg->precision, block, &ks, &rs))
@@ -242,6 +250,8 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
   s->vec = cfg->precision == CUDAHM_F64 ? 2 : 4;
   s->num_sms = sms; s->block = block;
   s->have_consts = (nk == 0);
+  s->hold = cfg->update_mask || cfg->per_object_counter;
+  s->n_active = cfg->n_objects_total ? cfg->n_objects_total : cfg->n_objects;
 
   int per_sm = 0;
   cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ks.persistent, block, 0);
@@ -259,7 +269,7 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
   //     theta step of iteration t are in flight (they depend on (seed, object, t) only) and wait in shared memory.
   //     Measured gains: p = 1 out of L2 -13 %, C6 (p = 3, one step) -10 %, C4 -0.5 %; C3 (p = 2: the fp64 draws of
   //     one step take the idle warps as long as the whole exchange) loses 5 % to the plain kernel, which it keeps.
-  if (cfg->theta_mode == CUDAHM_THETA_DEVICE_TAIL && cfg->n_objects > 0) {
+  if (cfg->theta_mode == CUDAHM_THETA_DEVICE_TAIL && cfg->n_objects > 0 && !s->hold) {
     int l2 = 0;
     cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev);
     const size_t set_bytes = (size_t)(p + p * (p + 1) / 2 + nc) * (size_t)cfg->n_objects * s->tsize;
@@ -287,7 +297,7 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
   }
   // HBM-streaming variant with TMA-staged loads (stream_tma.cuh), opt-in: measured 10-30 % slower than plain vector
   // loads on C3 / C4 (the sweep is issue-bound, not latency-bound, and the producer warp costs a sweep warp)
-  if (cfg->theta_mode == CUDAHM_THETA_DEVICE_TAIL && (cfg->flags & CUDAHM_FLAG_TMA_STAGING) && block <= 512 && ks.persistent_tma) {
+  if (cfg->theta_mode == CUDAHM_THETA_DEVICE_TAIL && (cfg->flags & CUDAHM_FLAG_TMA_STAGING) && block <= 512 && ks.persistent_tma && !s->hold) {
     int stages = (int)std::min<size_t>(TMA_MAX_STAGES, (size_t)(200 * 1024) / ks.tma_stage_bytes);
     if (stages >= 2 && ensure_dyn_smem(ks.persistent_tma, stages * ks.tma_stage_bytes) == cudaSuccess) {
       s->tma_stages = stages; s->tma_smem = stages * ks.tma_stage_bytes;
@@ -298,7 +308,7 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
     }
   }
   // on-chip variant: every object stays in the shared memory of its block for the whole launch
-  if (cfg->theta_mode == CUDAHM_THETA_DEVICE_TAIL && !(cfg->flags & CUDAHM_FLAG_STREAMING_ONLY) && cfg->n_objects > 0) {
+  if (cfg->theta_mode == CUDAHM_THETA_DEVICE_TAIL && !(cfg->flags & CUDAHM_FLAG_STREAMING_ONLY) && cfg->n_objects > 0 && !s->hold) {
     const int nv = rs.n_base + (cfg->keep_chi_moments ? 2 : 0);
     const void* rk = rs.kernel;
     if (rk) {
@@ -331,10 +341,13 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
                    cfg->target_accept_theta, cfg->eta_exponent, 0, cfg->max_trace_rows, 1, 0,
                    (double)(cfg->n_objects_total ? cfg->n_objects_total : cfg->n_objects), cfg->adapt_until, {}, {}};
   P.obj_offset = cfg->object_offset;
+  P.mask = cfg->update_mask ? (const unsigned char*)(s->ws + lay.mask) : nullptr;
+  P.cnt = cfg->per_object_counter ? (unsigned*)(s->ws + lay.cnt) : nullptr;
   for (int j = 0; j < MAXD; ++j) { P.tail.prior_mean[j] = cfg->prior_mean[j]; P.tail.prior_isd[j] = cfg->prior_isd[j]; }
   P.taps = DevTaps{};
 
   if (cudaMemsetAsync(s->ws, 0, lay.total, s->stream) != cudaSuccess ||
+      (cfg->update_mask && cudaMemsetAsync(s->ws + lay.mask, 1, (size_t)P.Npad, s->stream) != cudaSuccess) ||
       cudaHostAlloc((void**)&s->h_iter, sizeof(Iter), cudaHostAllocDefault) != cudaSuccess ||
       cudaHostAlloc((void**)&s->h_totals, NPART * sizeof(double), cudaHostAllocDefault) != cudaSuccess ||
       cudaEventCreate(&s->ev0) != cudaSuccess || cudaEventCreate(&s->ev1) != cudaSuccess) {
@@ -583,7 +596,7 @@ extern "C" int cudahm_set_init(cudahm_sampler* s, const void* chi0, int chi0_on_
   if (theta_chol0) for (int k = 0; k < s->ntri_theta; ++k) raw.Lth[k] = theta_chol0[k];
   else for (int r = 0; r < s->dtheta; ++r) raw.Lth[tri(r, r)] = 0.1;
   raw.t = 1;
-  s->t_done = 0; s->h_trace_rows = 0; s->h_mom_count = 0;
+  s->t_done = 0; s->h_trace_rows = 0; s->h_mom_count = 0; s->h_proposals = 0;
   invalidate_graph(s);
   int rc = upload_and_init_iter(s, raw);
   if (rc) return rc;
@@ -628,7 +641,7 @@ int run_device_tail(cudahm_sampler* s, long long n_iter) {
       s->launches++;
       rc = CUDAHM_OK;
     } else {
-      const void* fn = s->ahead ? s->ks.persistent_ahead : s->ks.persistent;
+      const void* fn = s->hold ? s->ks.persistent_hold : s->ahead ? s->ks.persistent_ahead : s->ks.persistent;
       cudaError_t e = s->ahead ? ensure_dyn_smem(fn, s->stage_smem) : cudaSuccess;
       if (e == cudaSuccess)
         e = cudaLaunchCooperativeKernel(fn, dim3(s->grid), dim3(s->block), pargs, s->ahead ? s->stage_smem : 0, s->stream);
@@ -645,7 +658,7 @@ int run_device_tail(cudahm_sampler* s, long long n_iter) {
 int enqueue_graph_iteration(cudahm_sampler* s) {
   Params P = s->P;
   void* a1[] = {&P};
-  int rc = launch(s, s->ks.sweep, s->sweep_grid, s->sweep_block, a1, false);
+  int rc = launch(s, s->hold ? s->ks.sweep_hold : s->ks.sweep, s->sweep_grid, s->sweep_block, a1, false);
   if (rc) return rc;
   int nb = s->sweep_grid, flags = TAIL_DECIDE;
   void* a2[] = {&P, &nb, &flags};
@@ -694,7 +707,7 @@ int run_graph(cudahm_sampler* s, long long n_iter) {
 int host_sweep(cudahm_sampler* s) {          // -> s->h_totals = {S, Delta, Tq, n_accept, n_nonfinite} of this handle
   Params P = s->P;
   void* a1[] = {&P};
-  int rc = launch(s, s->ks.sweep, s->sweep_grid, s->sweep_block, a1, false);
+  int rc = launch(s, s->hold ? s->ks.sweep_hold : s->ks.sweep, s->sweep_grid, s->sweep_block, a1, false);
   if (rc) return rc;
   int nb = s->sweep_grid, flags = TAIL_REDUCE;
   void* a2[] = {&P, &nb, &flags};
@@ -727,6 +740,50 @@ int run_host(cudahm_sampler* s, long long n_iter) {
 
 }  // namespace
 
+extern "C" int cudahm_set_update_mask(cudahm_sampler* s, const uint8_t* mask, int mask_on_device) {
+  if (!s) return fail(s, CUDAHM_E_INVALID, "NULL handle");
+  if (!s->cfg.update_mask) return fail(s, CUDAHM_E_STATE, "set_update_mask needs cudahm_config.update_mask = 1");
+  const size_t N = (size_t)s->P.N;
+  unsigned char* dst = (unsigned char*)(s->ws + s->lay.mask);
+  if (!mask) {
+    CU_TRY(s, cudaMemsetAsync(dst, 1, (size_t)s->P.Npad, s->stream));
+    s->n_active = (long long)N;
+    return CUDAHM_OK;
+  }
+  std::vector<unsigned char> h(N);
+  if (mask_on_device) {
+    if (N) CU_TRY(s, cudaMemcpyAsync(dst, mask, N, cudaMemcpyDeviceToDevice, s->stream));
+    if (N) CU_TRY(s, cudaMemcpyAsync(h.data(), mask, N, cudaMemcpyDeviceToHost, s->stream));
+    CU_TRY(s, cudaStreamSynchronize(s->stream));
+  } else {
+    std::copy(mask, mask + N, h.begin());
+    if (N) CU_TRY(s, cudaMemcpyAsync(dst, h.data(), N, cudaMemcpyHostToDevice, s->stream));
+    CU_TRY(s, cudaStreamSynchronize(s->stream));      // h goes out of scope; the caller may free its buffer
+  }
+  long long k = 0;
+  for (unsigned char m : h) k += m ? 1 : 0;
+  s->n_active = k;
+  return CUDAHM_OK;
+}
+
+extern "C" int cudahm_get_counters(cudahm_sampler* s, uint32_t* out) {
+  if (!s || !out) return fail(s, CUDAHM_E_INVALID, "get_counters: NULL argument");
+  if (!s->P.cnt) return fail(s, CUDAHM_E_STATE, "get_counters needs cudahm_config.per_object_counter = 1");
+  if (!s->have_init) return fail(s, CUDAHM_E_STATE, "get_counters before set_init");
+  CU_TRY(s, cudaStreamSynchronize(s->stream));
+  if (s->P.N) CU_TRY(s, cudaMemcpy(out, s->P.cnt, (size_t)s->P.N * 4, cudaMemcpyDeviceToHost));
+  return CUDAHM_OK;
+}
+
+extern "C" int cudahm_set_counters(cudahm_sampler* s, const uint32_t* in) {
+  if (!s || !in) return fail(s, CUDAHM_E_INVALID, "set_counters: NULL argument");
+  if (!s->P.cnt) return fail(s, CUDAHM_E_STATE, "set_counters needs cudahm_config.per_object_counter = 1");
+  if (!s->have_init) return fail(s, CUDAHM_E_STATE, "set_counters before set_init");
+  CU_TRY(s, cudaStreamSynchronize(s->stream));
+  if (s->P.N) CU_TRY(s, cudaMemcpy(s->P.cnt, in, (size_t)s->P.N * 4, cudaMemcpyHostToDevice));
+  return CUDAHM_OK;
+}
+
 extern "C" int cudahm_run(cudahm_sampler* s, int64_t n_iter, int64_t burn_in, int32_t thin) {
   if (!s) return fail(s, CUDAHM_E_INVALID, "NULL handle");
   if (!s->have_init) return fail(s, CUDAHM_E_STATE, "run before set_init");
@@ -753,6 +810,7 @@ extern "C" int cudahm_run(cudahm_sampler* s, int64_t n_iter, int64_t burn_in, in
   s->timed = true;
   s->h_trace_rows += rows;
   if (s->cfg.keep_chi_moments) s->h_mom_count += moment_samples_between(s->t_done, t1, burn_in);
+  s->h_proposals += n_iter * s->n_active;
   s->t_done = t1;
   return CUDAHM_OK;
 }
@@ -788,6 +846,7 @@ extern "C" int cudahm_shard_decide(cudahm_sampler* s, int64_t burn_in, int32_t t
   rc = host_decide(s, totals_global);
   if (rc) return rc;
   s->t_done += 1;
+  s->h_proposals += s->n_active;
   s->h_trace_rows = s->h_iter->trace_rows; s->h_mom_count = s->h_iter->mom_count;
   return CUDAHM_OK;
 }
@@ -837,7 +896,7 @@ extern "C" int cudahm_debug_step(cudahm_sampler* s, int64_t burn_in, int32_t thi
   P.taps.shift_c = lc; P.taps.shift_p = lcp;
   const bool prop_in_support = s->h_iter->lp_prop != -INFINITY;
   void* a1[] = {&P};
-  rc = launch(s, s->ks.sweep_tap, s->sweep_grid, s->sweep_block, a1, false);
+  rc = launch(s, s->hold ? s->ks.sweep_tap_hold : s->ks.sweep_tap, s->sweep_grid, s->sweep_block, a1, false);
   int nb = s->sweep_grid, flags = TAIL_REDUCE | TAIL_DECIDE;     // the device tail decides t and prepares t + 1
   void* a2[] = {&P, &nb, &flags};
   if (!rc) rc = launch(s, (const void*)k_tail, 1, TAIL_THREADS, a2, false);
@@ -865,6 +924,7 @@ extern "C" int cudahm_debug_step(cudahm_sampler* s, int64_t burn_in, int32_t thi
   if (rc) return rc;
   if (e != cudaSuccess) return fail(s, CUDAHM_E_CUDA, "debug_step: %s", cudaGetErrorString(e));
   s->t_done += 1;
+  s->h_proposals += s->n_active;
   s->h_trace_rows = s->h_iter->trace_rows; s->h_mom_count = s->h_iter->mom_count;
   return CUDAHM_OK;
 }
@@ -919,7 +979,7 @@ extern "C" int cudahm_get_stats(cudahm_sampler* s, cudahm_stats* out) {
   CU_TRY(s, cudaMemcpy(bc.data(), s->P.blk_cnt, bc.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
   unsigned long long acc = it.chi_acc, nonf = it.nonfinite;
   for (int b = 0; b < MAX_BLOCKS; ++b) { acc += bc[2 * b]; nonf += bc[2 * b + 1]; }
-  out->chi_accepts = (int64_t)acc; out->chi_proposals = (it.t - 1) * (long long)s->P.tail.n_objects;   // the WHOLE population's (sharded: chi_acc is global too)
+  out->chi_accepts = (int64_t)acc; out->chi_proposals = s->h_proposals;   // iterations x updated objects of the WHOLE population (sharded: chi_acc is global too)
   out->theta_accepts = (int64_t)it.theta_acc; out->theta_proposals = (int64_t)it.theta_prop_n;
   out->nonfinite = (int64_t)nonf; out->moment_samples = it.mom_count; out->trace_rows = it.trace_rows;
   if (s->timed) {
@@ -959,6 +1019,12 @@ extern "C" int cudahm_set_state(cudahm_sampler* s, const void* chi, const void* 
   if (L_theta) std::copy(L_theta, L_theta + s->ntri_theta, raw.Lth);
   raw.t = t + 1;
   s->t_done = t;
+  s->h_proposals = t * (long long)s->P.tail.n_objects;
+  if (s->P.cnt && N > 0) {       // as if every object had been updated in every iteration so far
+    k_fill_u32<<<(unsigned)((N + 255) / 256), 256, 0, s->stream>>>(s->P.cnt, (long long)N, (unsigned)t);
+    s->launches++;
+    CU_TRY(s, cudaGetLastError());
+  }
   invalidate_graph(s);
   return upload_and_init_iter(s, raw);
 }

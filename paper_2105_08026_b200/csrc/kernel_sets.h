@@ -14,6 +14,10 @@ struct KernelSet {
   const void* sweep;
   const void* sweep_tap;
   const void* init_state;
+  // the frozen-member variants (update mask / per-object counter)
+  const void* persistent_hold;
+  const void* sweep_hold;
+  const void* sweep_tap_hold;
 };
 
 // on-chip kernel (resident.cuh) of one (model, precision)

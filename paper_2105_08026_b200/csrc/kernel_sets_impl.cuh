@@ -11,8 +11,11 @@ namespace hm {
 template <int MODEL, class T, int BLOCK, bool WITH_TMA = true>
 KernelSet make_set() {
   KernelSet k;
-  k.persistent = (const void*)k_persistent<MODEL, T, BLOCK, false>;
-  k.persistent_ahead = (const void*)k_persistent<MODEL, T, BLOCK, true>;
+  k.persistent = (const void*)k_persistent<MODEL, T, BLOCK, PK_PLAIN>;
+  k.persistent_ahead = (const void*)k_persistent<MODEL, T, BLOCK, PK_AHEAD>;
+  k.persistent_hold = (const void*)k_persistent<MODEL, T, BLOCK, PK_HOLD>;
+  k.sweep_hold = (const void*)k_sweep<MODEL, T, BLOCK, false, true>;
+  k.sweep_tap_hold = (const void*)k_sweep<MODEL, T, BLOCK, true, true>;
   k.stage_step_bytes = (size_t)DrawSet<MODEL, T>::NV * BLOCK * sizeof(T);
   k.persistent_tma = nullptr;
   if constexpr (WITH_TMA) k.persistent_tma = (const void*)k_persistent_tma<MODEL, T, BLOCK>;

@@ -632,9 +632,11 @@ static_assert(sizeof(Iter) % sizeof(double) == 0, "Iter is copied as doubles");
 // AHEAD: the variant that works ahead of the exchange -- plate draws of the next iteration staged in shared memory by
 // the warps that do not run the theta tail, next step's columns prefetched into L2.  The plain variant
 // is kept for the populations that gain nothing from either (p = 2 out of L2: C3).  Same chain bit for bit.
-template <int MODEL, class T, int BLOCK, bool AHEAD>
+enum : int { PK_PLAIN = 0, PK_AHEAD = 1, PK_HOLD = 2 };   // PK_HOLD: the plain kernel with the frozen-member hooks of update_vec
+template <int MODEL, class T, int BLOCK, int VARIANT>
 __global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const long long n_iter, const unsigned epoch0,
                                                          const int n_stage, const int prefetch) {
+  constexpr bool AHEAD = VARIANT == PK_AHEAD, HOLD = VARIANT == PK_HOLD;
   __shared__ Iter it;
   __shared__ double red[32][NPART];
   extern __shared__ __align__(16) unsigned char stage_raw[];   // n_stage x DrawSet::NV x BLOCK values of T
@@ -652,7 +654,7 @@ __global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const l
   for (long long k = 0; k < n_iter; ++k) {
     double part[NPART];
     const uint32_t t_next = (uint32_t)it.t + 1u;
-    sweep<MODEL, T, false, AHEAD>(P, it, part, stage, n_stage, prefetch != 0);
+    sweep<MODEL, T, false, AHEAD, HOLD>(P, it, part, stage, n_stage, prefetch != 0);
     cnt[0] += part[3]; cnt[1] += part[4];
     double dq[2] = {part[1], part[2]};
     block_reduce_all<2>(dq, red);
@@ -694,14 +696,14 @@ __global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const l
 }
 
 // One sweep as its own launch (THETA_GRAPH, THETA_HOST, debug_step).  Same grid, same maps, same order.
-template <int MODEL, class T, int BLOCK, bool TAP>
+template <int MODEL, class T, int BLOCK, bool TAP, bool HOLD = false>
 __global__ void __launch_bounds__(BLOCK, 1) k_sweep(const Params P) {
   __shared__ Iter it;
   __shared__ double red[32][NPART];
   copy_iter(&it, P.iter);
   __syncthreads();
   double part[NPART];
-  sweep<MODEL, T, TAP>(P, it, part);
+  sweep<MODEL, T, TAP, false, HOLD>(P, it, part);
   block_reduce<NPART>(part, red);
   if (threadIdx.x == 0) {
 #pragma unroll
@@ -744,6 +746,7 @@ __global__ void k_init_state(const Params P, const T* raw, const int have_chi0, 
 #pragma unroll
     for (int j = 0; j < p; ++j) { P.mom_mean[j * P.Npad + i] = 0.0; P.mom_M2[j * P.Npad + i] = 0.0; }
   }
+  if (P.cnt) P.cnt[i] = 0u;
 }
 
 }  // namespace hm

@@ -51,6 +51,11 @@ __global__ void __launch_bounds__(256, 1) k_init_iter(const Params P) {
   copy_iter(P.iter, &it);
 }
 
+__global__ void k_fill_u32(unsigned* v, long long n, unsigned value) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) v[i] = value;
+}
+
 // sample variance from the Welford sums, written next to them for read-out
 __global__ void k_finalize_moments(const double* M2, double* var, long long n, double inv_km1) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;

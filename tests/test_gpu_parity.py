@@ -439,3 +439,98 @@ def test_theta0_outside_the_prior_support_is_refused():
     assert e.value.code == B.E_NONFINITE
     g.set_init(inp["theta0"])
     g.run(3, 0, 1, sync=True)
+
+
+@pytest.mark.parametrize("mode", [B.THETA_HOST, B.THETA_GRAPH, B.THETA_DEVICE_TAIL], ids=["host", "graph", "tail"])
+@pytest.mark.parametrize("model,astar,n,precision", [(B.M_NORMAL1D, 0.44, 3001, B.F64), (B.M_BINORMAL2D, 0.234, 2501, B.F64),
+                                                       (B.M_LINREG_ME1D, 0.44, 4099, B.F32_STATE_F64_REDUCE)],
+                         ids=["M0", "M2", "M3f32"])
+def test_update_mask_and_per_object_counter_match_oracle(model, astar, n, precision, mode):
+    """Frozen members: a third of the objects held fixed for 60 iterations, then
+    released (their own update counts lag, so their eta_n is larger), 60 more; free-running against the oracle in every theta
+    driver.  Held objects keep chi and L bit for bit, stay in the population sums, and consume no proposals."""
+    K1, K2, burn, thin = 60, 60, 20, 5
+    orc, gpu, inp = make_pair(model, n, seed=91 + model, astar=astar, precision=precision, theta_mode=mode, keep_moments=True,
+                              max_trace_rows=(K1 + K2 - burn) // thin, update_mask=True, per_object_counter=True)
+    mask = (np.arange(n) % 3 != 1).astype(np.uint8)
+    held = mask == 0
+    s0 = gpu.get_state()
+    orc.set_update_mask(mask)
+    gpu.set_update_mask(mask)
+    if precision == B.F64:
+        orc.run(K1, burn, thin)
+        gpu.run(K1, burn, thin, sync=True)
+    else:                               # fp32: lock-step from the oracle's state (near-tie flips are expected, see C4)
+        for _ in range(K1):
+            st = sync_gpu_to_oracle(orc, gpu)
+            orc.set_counters(orc.get_counters()); gpu.set_counters(orc.get_counters())
+            orc.run(1, burn, thin); gpu.run(1, burn, thin, sync=True)
+    s1, o1 = gpu.get_state(), orc.get_state()
+    assert np.array_equal(s1["chi"][:, held], s0["chi"][:, held]) and np.array_equal(s1["L"][:, held], s0["L"][:, held])
+    assert np.array_equal(gpu.get_counters(), orc.get_counters())
+    assert np.array_equal(gpu.get_counters(), np.where(held, 0, K1).astype(np.uint32))
+    if precision == B.F64:
+        np.testing.assert_allclose(s1["chi"], o1["chi"], rtol=1e-9, atol=1e-9)
+        np.testing.assert_allclose(s1["L"], o1["L"], rtol=1e-9)
+        assert gpu.get_stats()["chi_proposals"] == orc.get_stats()["chi_proposals"] == K1 * int(mask.sum())
+        assert gpu.get_stats()["chi_accepts"] == orc.get_stats()["chi_accepts"]
+    # a tapped step with the mask on: held objects report the documented taps and stay in S and Delta
+    st = sync_gpu_to_oracle(orc, gpu)
+    gpu.set_counters(orc.get_counters())
+    to, tg = orc.step(NO_TRACE, 1, taps=True), gpu.debug_step(NO_TRACE, 1)
+    for k in ("chi_prop", "L_new"):
+        assert np.array_equal(tg[k][:, held], st[k.replace("chi_prop", "chi").replace("L_new", "L")][:, held])
+    assert np.all(tg["alpha"][held] == 0) and np.all(tg["u"][held] == 1) and np.all(tg["accepted"][held] == 0)
+    assert np.array_equal(tg["pi_prop"][held], tg["pi_cur"][held])
+    tol = 1e-12 if precision == B.F64 else 1e-5
+    assert np.all(np.abs(tg["a"][held] - to["a"][held]) <= 1e-12 * np.maximum(1.0, np.abs(to["a"][held])))
+    assert np.array_equal(tg["u"][~held], to["u"][~held])
+    assert np.all(np.abs(tg["pi_cur"] - to["pi_cur"]) <= tol * np.maximum(1.0, np.abs(to["pi_cur"])))
+    import math
+    assert abs(tg["S"] - math.fsum(tg["a"])) <= 1e-10 * max(1.0, abs(tg["S"]))
+    # release: the held objects now adapt with eta from their OWN count (1 -> n = 2 ...), the others with theirs
+    sync_gpu_to_oracle(orc, gpu)
+    gpu.set_counters(orc.get_counters())
+    orc.set_update_mask(None); gpu.set_update_mask(None)
+    if precision == B.F64:
+        orc.run(K2 - 1, burn, thin)
+        gpu.run(K2 - 1, burn, thin, sync=True)
+        s2, o2 = gpu.get_state(), orc.get_state()
+        np.testing.assert_allclose(s2["chi"], o2["chi"], rtol=1e-9, atol=1e-9)
+        np.testing.assert_allclose(s2["L"], o2["L"], rtol=1e-9)
+        np.testing.assert_allclose(gpu.get_theta_trace(), orc.get_theta_trace(), rtol=1e-8, atol=1e-8)
+        mo, _, ko = orc.get_chi_moments()
+        mg, _, kg = gpu.get_chi_moments()
+        assert kg == ko
+        np.testing.assert_allclose(mg, mo, rtol=1e-10, atol=1e-10)
+    else:
+        orc.run(1, burn, thin); gpu.run(1, burn, thin, sync=True)
+        s2, o2 = gpu.get_state(), orc.get_state()
+        same = np.abs(s2["chi"][0] - o2["chi"][0]) <= 2e-5 * np.maximum(1.0, np.abs(o2["chi"][0]))
+        assert (~same).sum() <= 3
+        np.testing.assert_allclose(s2["L"][0][same], o2["L"][0][same], rtol=2e-5)
+    assert np.array_equal(gpu.get_counters(), orc.get_counters())
+    assert np.all(s2["L"][:, held] != s1["L"][:, held])
+    assert gpu.get_stats()["block_threads"] != 640
+
+
+def test_mask_calls_need_the_config_switches():
+    _, g, _ = make_pair(B.M_NORMAL1D, 100, seed=1, want_oracle=False)
+    with pytest.raises(B.CudahmError) as e:
+        g.set_update_mask(np.ones(100, np.uint8))
+    assert e.value.code == B.E_STATE
+    with pytest.raises(B.CudahmError):
+        g.get_counters()
+    # an all-ones mask + counter on the HOLD kernels is the plain chain bit for bit
+    _, a, inp = make_pair(B.M_BINORMAL2D, 3000, seed=8, astar=0.234, max_trace_rows=50, want_oracle=False, flags=B.FLAG_STREAMING_ONLY)
+    _, b, _ = make_pair(B.M_BINORMAL2D, 3000, seed=8, astar=0.234, max_trace_rows=60, want_oracle=False, inputs=inp,
+                        update_mask=True, per_object_counter=True)
+    a.run(50, 0, 1, sync=True); b.run(50, 0, 1, sync=True)
+    for k in ("chi", "L", "theta", "L_theta"):
+        assert np.array_equal(a.get_state()[k], b.get_state()[k]), k
+    assert np.array_equal(a.get_theta_trace(), b.get_theta_trace())
+    mask_dev = __import__("torch").ones(3000, dtype=__import__("torch").uint8, device="cuda")
+    mask_dev[::2] = 0
+    b.set_update_mask(mask_dev)
+    b.run(3, 0, 1, sync=True)
+    assert b.get_stats()["chi_proposals"] == 50 * 3000 + 3 * 1500
