@@ -443,7 +443,7 @@ def run_sharded(args, device, rank, world, dist, barrier, peak, peak_src):
     if inp["consts"] is not None:
         s.set_model_consts(inp["consts"])
     s.set_init(th0)
-    drv = sharded.DistributedShard(s, dist, device) if world > 1 else sharded.LocalShards([s])
+    drv = sharded.DistributedShard(s, dist, device) if world > 1 else sharded.LocalShards([s], device=True)
     drv.run(W, W, c.thin)
     l0 = s.get_stats()["gpu_launches"]
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -465,7 +465,7 @@ def run_sharded(args, device, rank, world, dist, barrier, peak, peak_src):
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64" if c.precision == synth.F64 else "f32 state / f64 reductions", "data": "synthetic",
             "config": {"workload": workload_label(args.config), "n_objects_per_gpu": n, "n_objects_total": world * n,
-                       "parallelism": f"one chain sharded by object range over {world} gpu(s); all-gather of 5 doubles per rank and iteration",
+                       "parallelism": f"one chain sharded by object range over {world} gpu(s); one device-side all-gather of 5 doubles per rank and iteration, one 40-byte-per-rank read-back",
                        "theta_mode": "host", "grid": [st["grid_blocks"], st["block_threads"]]},
             "gibbs_iters_per_s": K / (ms * 1e-3), "gpu_launches": int(st["gpu_launches"] - l0), "roofline": rf,
             "accept": {"chi": st["chi_accepts"] / max(1, st["chi_proposals"]),

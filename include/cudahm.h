@@ -212,6 +212,16 @@ int cudahm_run(cudahm_sampler* s, int64_t n_iter, int64_t burn_in, int32_t thin)
  * A handle with object_offset = 0 and n_objects_total = n_objects reproduces cudahm_run(THETA_HOST) bit for bit. */
 int cudahm_shard_sweep(cudahm_sampler* s, int64_t burn_in, int32_t thin, double* totals);
 int cudahm_shard_decide(cudahm_sampler* s, int64_t burn_in, int32_t thin, const double* totals_global);
+/* The fixed-order (rank-order) sum of the shards' totals: out[5] = {sum S, sum Delta, Tq of rank 0, sum n_accept,
+ * sum n_nonfinite} from totals_by_rank[n_ranks][5] (host doubles).  Pure host arithmetic, no device needed: every rank
+ * that calls it on the same gathered array holds the same bits. */
+int cudahm_shard_combine(const double* totals_by_rank, int n_ranks, double* out);
+/* The same two halves without a host bounce between them, for an exchange that runs on the device (NCCL all-gather on the
+ * sampler's stream): shard_sweep_device leaves this shard's five totals in the caller's DEVICE buffer totals_dev[5]
+ * (enqueued, no synchronisation); shard_decide_gathered takes the DEVICE array gathered_dev[n_ranks][5] in rank order,
+ * reads it back once (40 n_ranks bytes), combines it with cudahm_shard_combine's rule and takes the theta step. */
+int cudahm_shard_sweep_device(cudahm_sampler* s, int64_t burn_in, int32_t thin, void* totals_dev);
+int cudahm_shard_decide_gathered(cudahm_sampler* s, int64_t burn_in, int32_t thin, const void* gathered_dev, int n_ranks);
 
 /* One iteration through the non-persistent sweep + tail kernels with per-object taps (test instrument). */
 int cudahm_debug_step(cudahm_sampler* s, int64_t burn_in, int32_t thin, cudahm_taps* taps);

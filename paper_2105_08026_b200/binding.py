@@ -29,7 +29,8 @@ FLOOR_LAUNCH, FLOOR_GRAPH, FLOOR_GRID_BARRIER, FLOOR_HOST_SYNC = 0, 1, 2, 3
 EXPORTS = ["cudahm_model_dims", "cudahm_workspace_bytes", "cudahm_create", "cudahm_destroy", "cudahm_set_data",
            "cudahm_set_model_consts", "cudahm_set_init", "cudahm_run", "cudahm_debug_step",
            "cudahm_get_theta_trace", "cudahm_get_chi_moments", "cudahm_get_stats", "cudahm_get_state",
-           "cudahm_set_state", "cudahm_sync", "cudahm_last_error", "cudahm_shard_sweep", "cudahm_shard_decide", "cudahm_set_update_mask", "cudahm_get_counters", "cudahm_set_counters",
+           "cudahm_set_state", "cudahm_sync", "cudahm_last_error", "cudahm_shard_sweep", "cudahm_shard_decide", "cudahm_shard_combine", "cudahm_shard_sweep_device",
+           "cudahm_shard_decide_gathered", "cudahm_set_update_mask", "cudahm_get_counters", "cudahm_set_counters",
            "cudahm_probe_floor", "cudahm_probe_fma_peak"]
 
 _dp = C.POINTER(C.c_double)
@@ -97,6 +98,9 @@ def load():
     L.cudahm_set_state.argtypes = [vp, vp, vp, _dp, _dp, C.c_int64]
     L.cudahm_shard_sweep.argtypes = [vp, C.c_int64, C.c_int32, _dp]
     L.cudahm_shard_decide.argtypes = [vp, C.c_int64, C.c_int32, _dp]
+    L.cudahm_shard_combine.argtypes = [_dp, C.c_int, _dp]
+    L.cudahm_shard_sweep_device.argtypes = [vp, C.c_int64, C.c_int32, vp]
+    L.cudahm_shard_decide_gathered.argtypes = [vp, C.c_int64, C.c_int32, vp, C.c_int]
     L.cudahm_set_update_mask.argtypes = [vp, vp, C.c_int]
     L.cudahm_get_counters.argtypes = [vp, vp]
     L.cudahm_set_counters.argtypes = [vp, vp]
@@ -143,6 +147,16 @@ def make_config(model, n_objects, seed=0, precision=F64, theta_mode=THETA_DEVICE
     cfg.object_offset, cfg.n_objects_total = int(object_offset), int(n_objects_total)
     cfg.update_mask, cfg.per_object_counter = int(update_mask), int(per_object_counter)
     return cfg
+
+
+def shard_combine(totals_by_rank):
+    """cudahm_shard_combine: the rank-order sum of the shards' totals (n_ranks x 5 host doubles -> 5); no device needed."""
+    t = np.ascontiguousarray(np.asarray(totals_by_rank, dtype=np.float64).reshape(-1, 5))
+    out = np.empty(5)
+    rc = load().cudahm_shard_combine(_d(t), t.shape[0], _d(out))
+    if rc:
+        raise CudahmError(rc, load().cudahm_last_error(None).decode())
+    return out
 
 
 def workspace_bytes(cfg):
@@ -270,6 +284,16 @@ class Sampler:
         tot = np.ascontiguousarray(totals_global, dtype=np.float64)
         with self._dev():
             self._ck(self.lib.cudahm_shard_decide(self._h, burn_in, thin, _d(tot)))
+
+    def shard_sweep_device(self, totals_dev_ptr, burn_in=0, thin=1):
+        """One sweep over this handle's objects; its five totals are left in the DEVICE buffer at totals_dev_ptr."""
+        with self._dev():
+            self._ck(self.lib.cudahm_shard_sweep_device(self._h, burn_in, thin, C.c_void_p(int(totals_dev_ptr))))
+
+    def shard_decide_gathered(self, gathered_dev_ptr, n_ranks, burn_in=0, thin=1):
+        """The theta step from the DEVICE array gathered[n_ranks][5] (rank order), combined inside the library."""
+        with self._dev():
+            self._ck(self.lib.cudahm_shard_decide_gathered(self._h, burn_in, thin, C.c_void_p(int(gathered_dev_ptr)), int(n_ranks)))
 
     def debug_step(self, burn_in=0, thin=1):
         N, p = self.N, self.p

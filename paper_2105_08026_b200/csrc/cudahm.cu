@@ -704,7 +704,7 @@ int run_graph(cudahm_sampler* s, long long n_iter) {
 
 // THETA_HOST (the paper's split): sweep + reduction on the device, theta step in host C++.
 // Two halves, so that a sharded population can put its exchange between them (cudahm_shard_sweep / _decide).
-int host_sweep(cudahm_sampler* s) {          // -> s->h_totals = {S, Delta, Tq, n_accept, n_nonfinite} of this handle
+int host_sweep(cudahm_sampler* s, void* totals_dev = nullptr) {   // -> s->h_totals = {S, Delta, Tq, n_accept, n_nonfinite} of this handle
   Params P = s->P;
   void* a1[] = {&P};
   int rc = launch(s, s->hold ? s->ks.sweep_hold : s->ks.sweep, s->sweep_grid, s->sweep_block, a1, false);
@@ -713,6 +713,10 @@ int host_sweep(cudahm_sampler* s) {          // -> s->h_totals = {S, Delta, Tq, 
   void* a2[] = {&P, &nb, &flags};
   rc = launch(s, (const void*)k_tail, 1, TAIL_THREADS, a2, false);
   if (rc) return rc;
+  if (totals_dev) {                            // the exchange runs on the device: leave the totals there, do not wait
+    CU_TRY(s, cudaMemcpyAsync(totals_dev, s->P.totals, NPART * sizeof(double), cudaMemcpyDeviceToDevice, s->stream));
+    return CUDAHM_OK;
+  }
   CU_TRY(s, cudaMemcpyAsync(s->h_totals, s->P.totals, NPART * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
   CU_TRY(s, cudaStreamSynchronize(s->stream));
   return CUDAHM_OK;
@@ -835,6 +839,33 @@ extern "C" int cudahm_shard_sweep(cudahm_sampler* s, int64_t burn_in, int32_t th
   if (rc) return rc;
   for (int q = 0; q < NPART; ++q) totals[q] = s->h_totals[q];
   return CUDAHM_OK;
+}
+
+extern "C" int cudahm_shard_combine(const double* totals_by_rank, int n_ranks, double* out) {
+  if (!totals_by_rank || !out || n_ranks < 1) return fail(nullptr, CUDAHM_E_INVALID, "shard_combine: bad argument");
+  for (int q = 0; q < NPART; ++q) out[q] = totals_by_rank[q];
+  for (int r = 1; r < n_ranks; ++r)                     // rank order; Tq (slot 2) is computed in full by every shard
+    for (int q = 0; q < NPART; ++q)
+      if (q != 2) out[q] += totals_by_rank[(size_t)r * NPART + q];
+  return CUDAHM_OK;
+}
+
+extern "C" int cudahm_shard_sweep_device(cudahm_sampler* s, int64_t burn_in, int32_t thin, void* totals_dev) {
+  int rc = shard_check(s, burn_in, thin, totals_dev);
+  if (rc) return rc;
+  return host_sweep(s, totals_dev);
+}
+
+extern "C" int cudahm_shard_decide(cudahm_sampler* s, int64_t burn_in, int32_t thin, const double* totals_global);
+extern "C" int cudahm_shard_decide_gathered(cudahm_sampler* s, int64_t burn_in, int32_t thin, const void* gathered_dev,
+                                            int n_ranks) {
+  if (!s || !gathered_dev || n_ranks < 1 || n_ranks > 4096) return fail(s, CUDAHM_E_INVALID, "shard_decide_gathered: bad argument");
+  std::vector<double> all((size_t)n_ranks * NPART);
+  CU_TRY(s, cudaMemcpyAsync(all.data(), gathered_dev, all.size() * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+  CU_TRY(s, cudaStreamSynchronize(s->stream));
+  double tot[NPART];
+  cudahm_shard_combine(all.data(), n_ranks, tot);
+  return cudahm_shard_decide(s, burn_in, thin, tot);
 }
 
 extern "C" int cudahm_shard_decide(cudahm_sampler* s, int64_t burn_in, int32_t thin, const double* totals_global) {

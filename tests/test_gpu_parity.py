@@ -142,7 +142,8 @@ def test_user_prior_and_adaptation_freeze_match_oracle(model, astar, n, flags, m
 
 @pytest.mark.parametrize("model,astar,n", [(B.M_THINNED_SCHECHTER1D, 0.44, 4001), (B.M_BINORMAL2D, 0.234, 3000),
                                              (B.M_BB1_FLUXNOISE1D, 0.44, 2500)], ids=["M1", "M2", "M4"])
-def test_sharded_population_matches_oracle(model, astar, n):
+@pytest.mark.parametrize("on_device", [False, True], ids=["host-exchange", "device-exchange"])
+def test_sharded_population_matches_oracle(model, astar, n, on_device):
     """the population split by object range over THREE handles (here on one GPU, launched one after the
     other), theta replicated, the shards' totals summed in rank order between the sweep and the theta step
     (cudahm_shard_sweep / cudahm_shard_decide) -- against the UNSHARDED oracle chain."""
@@ -159,7 +160,7 @@ def test_sharded_population_matches_oracle(model, astar, n):
             g.set_model_consts(inp["consts"])
         g.set_init(inp["theta0"])
         parts.append(g)
-    sharded.LocalShards(parts).run(iters, burn, thin)
+    sharded.LocalShards(parts, device=on_device).run(iters, burn, thin)
     for g in parts:
         np.testing.assert_allclose(g.get_theta_trace(), orc.get_theta_trace(), rtol=1e-8, atol=1e-8)
         assert np.array_equal(g.get_theta_trace(), parts[0].get_theta_trace())
