@@ -671,7 +671,7 @@ __global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const l
         mbox_collect<NVX>(mb + (size_t)blockIdx.x * mbox_reader_words(G), G, epoch, t2);
         tot[1] = t2[0]; tot[2] = t2[1];
       }
-      tail_block(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, (int)(threadIdx.x >> 5), SyncAll());
+      tail_block<MODEL>(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, (int)(threadIdx.x >> 5), SyncAll());
       continue;
     }
     if (threadIdx.x < TAILT) {
@@ -681,7 +681,7 @@ __global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const l
         mbox_collect<NVX>(mb + (size_t)blockIdx.x * mbox_reader_words(G), G, epoch, t2);
         tot[1] = t2[0]; tot[2] = t2[1];
       }
-      tail_block(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, (int)(threadIdx.x >> 5), SyncNamed<1, TAILT>());
+      tail_block<MODEL>(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, (int)(threadIdx.x >> 5), SyncNamed<1, TAILT>());
     } else if (k + 1 < n_iter) {
       stage_draws<MODEL, T>(P, t_next, stage, n_stage, (int)threadIdx.x - TAILT, BLOCK - TAILT);
     }

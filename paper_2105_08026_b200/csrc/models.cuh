@@ -84,7 +84,7 @@ HM_HD void theta_consts_part(int model, int part, const double* th, ThetaK& k) {
       break;
     case M_NORMAL3D_KNOWNCOV: case M_NORMAL4D_KNOWNCOV: case M_NORMAL5D_KNOWNCOV: case M_NORMAL6D_KNOWNCOV:
       // theta = mu; C_pop is a known model constant
-      if (part == 0) { for (int j = 0; j < normal_family_p(model); ++j) k.v[j] = th[j]; }
+      if (part == 0) { k.v[0] = th[0]; k.v[1] = th[1]; k.v[2] = th[2]; if (model >= M_NORMAL4D_KNOWNCOV) k.v[3] = th[3]; if (model >= M_NORMAL5D_KNOWNCOV) k.v[4] = th[4]; if (model >= M_NORMAL6D_KNOWNCOV) k.v[5] = th[5]; }
       break;
     case M_BB1_FLUXNOISE1D:
       // (beta, ln l, ln u): f = log C + (beta+1)(x - ln u) + log(1 - e^(-L/l)) - L/u   (Eq. 5.1 in x = ln L).
@@ -133,8 +133,10 @@ HM_HD double log_prior(int model, const double* th) {
                  ? -hm_log_any_pos(1.0 + th[0] * th[0]) : ninf;
     case M_NORMAL3D_KNOWNCOV: case M_NORMAL4D_KNOWNCOV: case M_NORMAL5D_KNOWNCOV: case M_NORMAL6D_KNOWNCOV: {
       // "uniform hyperpriors" on a wide box
-      bool in = true;
-      for (int j = 0; j < normal_family_p(model); ++j) in = in && fabs(th[j]) <= 1e3;
+      bool in = fabs(th[0]) <= 1e3 && fabs(th[1]) <= 1e3 && fabs(th[2]) <= 1e3;
+      if (model >= M_NORMAL4D_KNOWNCOV) in = in && fabs(th[3]) <= 1e3;
+      if (model >= M_NORMAL5D_KNOWNCOV) in = in && fabs(th[4]) <= 1e3;
+      if (model >= M_NORMAL6D_KNOWNCOV) in = in && fabs(th[5]) <= 1e3;
       return in ? 0.0 : ninf;
     }
     case M_BB1_FLUXNOISE1D:     // Eq. 5.5 as a density in (beta, ln l, ln u): l / (u (1 + beta^2)), l < u

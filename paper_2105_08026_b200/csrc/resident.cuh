@@ -281,7 +281,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
         tot[1] = t1[0];
         if constexpr (V::m1) tot[2] = ((tq_warp[0] + tq_warp[1]) + tq_warp[2]) + tq_warp[3];
       }
-      tail_block(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, tw, SyncNamed<BAR_TAIL, RES_TW * 32>(),
+      tail_block<MODEL>(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, tw, SyncNamed<BAR_TAIL, RES_TW * 32>(),
                  ArriveNamed<BAR_THETA, RES_THREADS>());      // theta_{t+1} is signalled after the decision phase ...
       __threadfence_block();
       bar_arrive(BAR_THETAP, RES_THREADS);                   // ... theta'_{t+1} and its constants when the tail is done

@@ -154,7 +154,7 @@ __global__ void __launch_bounds__(BLOCK_ALL, 1) k_persistent_tma(const Params P,
       mbox_collect<NVX>(mb + (size_t)blockIdx.x * mbox_reader_words(G), G, epoch, t2);
       tot[1] = t2[0]; tot[2] = t2[1];
     }
-    tail_block(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, tid >> 5, SyncAll());
+    tail_block<MODEL>(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, tid >> 5, SyncAll());
   }
   block_reduce_all<2>(cnt, red);
   if (tid == 0) {

@@ -61,14 +61,15 @@ HM_HD double eta_of(const TailCfg& c, long long t) {
   return pow((double)(t + 1), -c.eta_exp);
 }
 // log prior = the model's default (uniform on a box; models.cuh) + the user's normal factors
-HM_HD double log_prior_full(const TailCfg& c, const double* th) {
-  double s = log_prior(c.model, th);
+HM_HD double log_prior_full(const TailCfg& c, const double* th, int model) {
+  double s = log_prior(model, th);
   for (int j = 0; j < c.dtheta; ++j) {
     const double r = (th[j] - c.prior_mean[j]) * c.prior_isd[j];
     s += -0.5 * r * r;
   }
   return s;
 }
+HM_HD double log_prior_full(const TailCfg& c, const double* th) { return log_prior_full(c, th, c.model); }
 
 HM_HD int tri(int r, int c) { return r * (r + 1) / 2 + c; }
 HM_HD int tri_row(int e) { int r = 0; while ((r + 1) * (r + 2) / 2 <= e) ++r; return r; }
@@ -149,14 +150,15 @@ HM_HD void prepare_iteration(Iter& it, const TailCfg& c, long long t) {
 // inside the near-tie band (1e-9) in which BASELINE.json allows accept sequences to differ.  alpha itself (the
 // RAM update needs it) is computed by the caller afterwards.
 HM_HD void decide_scalars(const Iter& it, const TailCfg& c, const Draws& d, double Delta, double tq, double* T_prop,
-                          double* log_r, double* la, int* acc) {
+                          double* log_r, double* la, int* acc, int model = -1) {
+  if (model < 0) model = c.model;
   *T_prop = 0.0;
   if (it.lp_prop == -INFINITY) {
     *log_r = -INFINITY; *la = -INFINITY;
   } else {
     // M1: T(theta') = -A' sum_k W_k phi(x_k; theta'): minus the expected detected count (Eq. 4.4 denominator)
     // M4: T(theta') = -N log sum_k W_k rho(x_k; theta')   (Eq. 4.3-4.4)
-    *T_prop = theta_only_from_sum(c.model, it.kp, tq, c.n_objects);
+    *T_prop = theta_only_from_sum(model, it.kp, tq, c.n_objects);
     *log_r = Delta + (*T_prop - it.T_cur) + (it.lp_prop - it.lp_cur);
     *la = (*log_r != *log_r) ? -INFINITY : fmin(0.0, *log_r);
   }
@@ -244,10 +246,13 @@ struct ArriveNamed {
 // `decided` is called once by every thread of the four warps as soon as what the next sweep's targets need is
 // final: kc (theta_{t+1}'s constants: the accept decision only, NOT the RAM update of L_theta), the moments count
 // and eta of iteration t + 1.  theta', kp, the prior, L_theta and W are final only when tail_block returns.
-template <class Sync, class Decided = NoSignal>
+// MODEL: the compiled-in model of the calling kernel (the persistent kernels know it at compile time, which collapses the
+// model switches of the tail -- the serial chain every iteration waits for); -1: taken from c.model at run time (k_tail).
+template <int MODEL = -1, class Sync, class Decided = NoSignal>
 __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const double* tot, double* trace_or_null,
                                            const int warp, const Sync sync, const Decided decided = Decided()) {
   const int lane = threadIdx.x & 31;
+  const int model = MODEL >= 0 ? MODEL : c.model;
   const int dt = c.dtheta, nt = dt * (dt + 1) / 2;
   const long long t = it.t;
   const int r0 = (int)(t % 3), r1 = r0 == 2 ? 0 : r0 + 1, r2 = r1 == 2 ? 0 : r1 + 1;
@@ -261,7 +266,7 @@ __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const dou
   if (warp == 0) {
     if (!c.freeze_theta) {
       double la;
-      decide_scalars(it, c, d0, tot[1], tot[2], &T_prop, &log_r, &la, &acc);
+      decide_scalars(it, c, d0, tot[1], tot[2], &T_prop, &log_r, &la, &acc, model);
       const double kpv = lane < 8 ? it.kp.v[lane] : 0.0;
       if (lane < 8 && acc) it.kc.v[lane] = kpv;          // theta_{t+1}'s constants: all the next sweep's targets need
       decided();
@@ -317,12 +322,12 @@ __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const dou
   sync();
   if (!c.freeze_theta) {
     if (warp >= 1) {
-      if (lane == 0) theta_consts_part(c.model, warp - 1, it.thetaP, it.kp);
+      if (lane == 0) theta_consts_part(model, warp - 1, it.thetaP, it.kp);
       if (warp == 1 && lane >= 1 && lane <= nt) {
         const int e = lane - 1, ei = tri_row(e), ej = e - ei * (ei + 1) / 2;
         it.W[e] = make_W_entry(it, d1, ei, ej);
       }
-      if (warp == 3 && lane == 0) it.lp_prop_next = log_prior_full(c, it.thetaP);
+      if (warp == 3 && lane == 0) it.lp_prop_next = log_prior_full(c, it.thetaP, model);
     } else if (lane == 0) {               // warp 0: taps and acceptance bookkeeping of the decision just taken
       it.T_cur_used = it.T_cur; it.lp_cur_used = it.lp_cur;
       it.T_prop = T_prop; it.log_r = log_r; it.alpha_theta = alpha; it.u_theta = d0.u;
