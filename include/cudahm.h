@@ -77,6 +77,9 @@ enum { CUDAHM_FLAG_STREAMING_ONLY = 1,
  * one, by default when state + data exceed the L2 cache (they then stream from HBM every iteration); these two force it */
 #define CUDAHM_FLAG_PREFETCH_OFF 4
 #define CUDAHM_FLAG_PREFETCH_ON 8
+/* bracket every cudahm_run with a pair of CUDA events so that cudahm_stats.last_run_ms is filled.  Off by default: the two
+ * event records cost about 5 us of device front-end time per run, as much as one Gibbs iteration at N = 3e5. */
+#define CUDAHM_FLAG_TIME_RUNS 16
 #define CUDAHM_FLAG_STAGE_STEPS_MASK 0xff00
 #define CUDAHM_FLAG_STAGE_STEPS(n) ((((n) + 1) << 8) & CUDAHM_FLAG_STAGE_STEPS_MASK)
 
@@ -129,7 +132,7 @@ typedef struct {
   int64_t trace_rows;
   int64_t gpu_launches;          /* kernels launched by this handle so far                                  */
   int32_t grid_blocks, block_threads;   /* launch configuration of the sweep                               */
-  double  last_run_ms;           /* device time of the last cudahm_run (CUDA events on the stream)          */
+  double  last_run_ms;           /* device time of the last cudahm_run (needs CUDAHM_FLAG_TIME_RUNS; else 0)  */
   int32_t stage_steps;           /* streaming persistent kernel: steps of plate draws staged ahead per thread */
   int32_t l2_prefetch;           /* ... 1: it prefetches the next step's columns into L2 (0 for the on-chip kernel) */
 } cudahm_stats;

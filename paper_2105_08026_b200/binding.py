@@ -18,7 +18,7 @@ M_NORMAL4D_KNOWNCOV, M_NORMAL5D_KNOWNCOV, M_NORMAL6D_KNOWNCOV = 6, 7, 8
 F64, F32_STATE_F64_REDUCE = 0, 1
 THETA_HOST, THETA_GRAPH, THETA_DEVICE_TAIL = 0, 1, 2
 FLAG_STREAMING_ONLY, FLAG_TMA_STAGING = 1, 2
-FLAG_PREFETCH_OFF, FLAG_PREFETCH_ON = 4, 8
+FLAG_PREFETCH_OFF, FLAG_PREFETCH_ON, FLAG_TIME_RUNS = 4, 8, 16
 
 
 def flag_stage_steps(n):

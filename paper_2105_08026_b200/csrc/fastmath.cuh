@@ -69,16 +69,32 @@ struct hm_d2 { double hi, lo; };
 #ifdef __CUDACC__
 __device__ const hm_d2 hm_exp2_tab_dev[64] = {HM_EXP2_TABLE};
 #endif
+// Where the polynomial coefficients of exp / log come from on the device.  As literals they reach the fp64 pipe through
+// uniform registers, two UMOV per coefficient and use (44 of the 425 warp-instructions per 32 updates of the C2 kernel);
+// from the constant bank one LDCU.128 brings two of them.  Which is faster depends on the kernel: measured -2 to -3.5 % on
+// the streaming p = 2 kernel (C3), +1.4 % on C2, within noise elsewhere -- so a translation unit opts in with
+// HM_CONST_BANK_COEFFS (inst_binormal2d.cu does).
+#if defined(__CUDACC__) && defined(HM_CONST_BANK_COEFFS)
+__constant__ double hm_kc[24] = {HM_64_LN2, -HM_LN2_64_HI, -HM_LN2_64_LO, 1.3888888888888889e-03, 8.3333333333333332e-03,
+  4.1666666666666664e-02, 1.6666666666666666e-01, 0.0,
+  1.0 / 23.0, 1.0 / 21.0, 1.0 / 19.0, 1.0 / 17.0, 1.0 / 15.0, 1.0 / 13.0, 1.0 / 11.0, 1.0 / 9.0, 1.0 / 7.0, 1.0 / 5.0, 1.0 / 3.0,
+  6.93147180369123816490e-01, 1.90821492927058770002e-10, 0.0, 0.0, 0.0};
+#endif
+#if defined(__CUDA_ARCH__) && defined(HM_CONST_BANK_COEFFS)
+#define HM_KC(i, lit) hm_kc[i]
+#else
+#define HM_KC(i, lit) (lit)
+#endif
 static const hm_d2 hm_exp2_tab_host[64] = {HM_EXP2_TABLE};
 
 // hm_exp_core: NO argument check -- finite garbage (or inf / NaN) outside [-708, 709]; for callers that discard the
 // result there anyway (a proposal outside the model's support, alpha of a log ratio below -708).
 HM_HD double hm_exp_core(double x) {
   const double SHIFT = 6755399441055744.0;                 // 1.5 * 2^52: adding it rounds to the nearest integer
-  const double t = hm_fma(x, HM_64_LN2, SHIFT);
+  const double t = hm_fma(x, HM_KC(0, HM_64_LN2), SHIFT);
   const double nf = t - SHIFT;
-  double r = hm_fma(nf, -HM_LN2_64_HI, x);                 // HM_LN2_64_HI has 32 significant bits: exact product
-  r = hm_fma(nf, -HM_LN2_64_LO, r);
+  double r = hm_fma(nf, HM_KC(1, -HM_LN2_64_HI), x);       // HM_LN2_64_HI has 32 significant bits: exact product
+  r = hm_fma(nf, HM_KC(2, -HM_LN2_64_LO), r);
   const int n = (int)(uint32_t)(hm_d2bits(t) & 0xffffffffull);   // the integer sits in the low word of t
   const int j = n & 63, k = n >> 6;
 #ifdef __CUDA_ARCH__
@@ -87,10 +103,10 @@ HM_HD double hm_exp_core(double x) {
 #else
   const double thi = hm_exp2_tab_host[j].hi, tlo = hm_exp2_tab_host[j].lo;
 #endif
-  double p = 1.3888888888888889e-03;                       // 1/6!
-  p = hm_fma(p, r, 8.3333333333333332e-03);                // 1/5!
-  p = hm_fma(p, r, 4.1666666666666664e-02);                // 1/4!
-  p = hm_fma(p, r, 1.6666666666666666e-01);                // 1/3!
+  double p = HM_KC(3, 1.3888888888888889e-03);             // 1/6!
+  p = hm_fma(p, r, HM_KC(4, 8.3333333333333332e-03));      // 1/5!
+  p = hm_fma(p, r, HM_KC(5, 4.1666666666666664e-02));      // 1/4!
+  p = hm_fma(p, r, HM_KC(6, 1.6666666666666666e-01));      // 1/3!
   p = hm_fma(p, r, 0.5);
   p = p * r;
   p = hm_fma(p, r, r);                                     // e^r - 1
@@ -149,22 +165,22 @@ HM_HD double hm_log_pos(double u) {
   double s = f * rc;
   s = hm_fma(hm_fma(-s, a, f), rc, s);                      // one correction: s = f/a to ~0.5 ulp
   const double s2 = s * s;
-  double p = 1.0 / 23.0;
-  p = hm_fma(p, s2, 1.0 / 21.0);
-  p = hm_fma(p, s2, 1.0 / 19.0);
-  p = hm_fma(p, s2, 1.0 / 17.0);
-  p = hm_fma(p, s2, 1.0 / 15.0);
-  p = hm_fma(p, s2, 1.0 / 13.0);
-  p = hm_fma(p, s2, 1.0 / 11.0);
-  p = hm_fma(p, s2, 1.0 / 9.0);
-  p = hm_fma(p, s2, 1.0 / 7.0);
-  p = hm_fma(p, s2, 1.0 / 5.0);
-  p = hm_fma(p, s2, 1.0 / 3.0);
+  double p = HM_KC(8, 1.0 / 23.0);
+  p = hm_fma(p, s2, HM_KC(9, 1.0 / 21.0));
+  p = hm_fma(p, s2, HM_KC(10, 1.0 / 19.0));
+  p = hm_fma(p, s2, HM_KC(11, 1.0 / 17.0));
+  p = hm_fma(p, s2, HM_KC(12, 1.0 / 15.0));
+  p = hm_fma(p, s2, HM_KC(13, 1.0 / 13.0));
+  p = hm_fma(p, s2, HM_KC(14, 1.0 / 11.0));
+  p = hm_fma(p, s2, HM_KC(15, 1.0 / 9.0));
+  p = hm_fma(p, s2, HM_KC(16, 1.0 / 7.0));
+  p = hm_fma(p, s2, HM_KC(17, 1.0 / 5.0));
+  p = hm_fma(p, s2, HM_KC(18, 1.0 / 3.0));
   p = p * s2;                                               // atanh(s)/s - 1
   const double two_s = s + s;
   const double lm = hm_fma(two_s, p, two_s);                // ln m
   const double ed = (double)e;
-  return hm_fma(ed, 6.93147180369123816490e-01, hm_fma(ed, 1.90821492927058770002e-10, lm));
+  return hm_fma(ed, HM_KC(19, 6.93147180369123816490e-01), hm_fma(ed, HM_KC(20, 1.90821492927058770002e-10), lm));
 }
 
 HM_HD double hm_log_unit(double u) { return hm_log_pos(u); }   // u in [2^-53, 1)

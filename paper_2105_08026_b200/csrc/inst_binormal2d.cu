@@ -1,4 +1,6 @@
 // inst_binormal2d.cu -- every kernel of model M_BINORMAL2D (its own translation unit: the models build in parallel).
+// exp / log coefficients from the constant bank in this translation unit (fastmath.cuh: measured faster for this model)
+#define HM_CONST_BANK_COEFFS 1
 #include "kernel_sets_impl.cuh"
 
 namespace hm {

@@ -31,6 +31,13 @@ template <int MODEL> struct ResValues {
   static constexpr int n_base = 4 + ncols + (m1 ? 2 : 0);   // + 2 (mean, M2) when moments are kept
 };
 
+// 8-byte asynchronous copy global -> shared (LDGSTS); completion per thread with cp_async_wait_all
+__device__ __forceinline__ void cp_async8(double* dst_smem, const double* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
 __device__ __forceinline__ void bar_sync(const int id, const int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 __device__ __forceinline__ void bar_arrive(const int id, const int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 enum : int { BAR_PARTIALS = 1, BAR_THETA = 2, BAR_TAIL = 3, BAR_THETAP = 4 };
@@ -71,33 +78,34 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
   copy_iter(&it, P.iter);
   if (tid < 2) cnt_sm[tid] = 0ull;
   if (!is_tail) {
-    // a thread's slot pair (r, r + 1) is two ADJACENT objects starting at an even index: one 16-byte access per column
-    for (int r = 0; r < nlive; r += 2) {
+    // The state comes on chip with asynchronous 8-byte copies (cp.async: global -> shared without passing through
+    // registers; a thread's slot pair is two adjacent objects, so a warp still reads whole 512-byte runs per column) ...
+    for (int r = 0; r < nlive; ++r) {
       const long long i = HM_OBJ(r);
-      if (r + 1 < nlive) {
-        const double2 x = *reinterpret_cast<const double2*>(chi + i), l = *reinterpret_cast<const double2*>(Lm + i);
-        HM_AT(V::V_CHI, r) = x.x; HM_AT(V::V_CHI, r + 1) = x.y;
-        HM_AT(V::V_L, r) = l.x; HM_AT(V::V_L, r + 1) = l.y;
+      cp_async8(&HM_AT(V::V_CHI, r), chi + i);
+      cp_async8(&HM_AT(V::V_L, r), Lm + i);
 #pragma unroll
-        for (int c = 0; c < ncols; ++c) {
-          const double2 d = __ldg(reinterpret_cast<const double2*>(dat + c * Npad + i));
-          HM_AT(V::V_D + c, r) = d.x; HM_AT(V::V_D + c, r + 1) = d.y;
-        }
-        if (V::m1) { HM_AT(V::V_E, r) = hm_exp(x.x); HM_AT(V::V_E, r + 1) = hm_exp(x.y); }
-        if (keep_mom) {
-          const double2 m = *reinterpret_cast<const double2*>(P.mom_mean + i), q = *reinterpret_cast<const double2*>(P.mom_M2 + i);
-          HM_AT(V_MEAN, r) = m.x; HM_AT(V_MEAN, r + 1) = m.y;
-          HM_AT(V_M2, r) = q.x; HM_AT(V_M2, r + 1) = q.y;
-        }
-      } else {
-        const T x = chi[i];
-        HM_AT(V::V_CHI, r) = x;
-        HM_AT(V::V_L, r) = Lm[i];
+      for (int c = 0; c < ncols; ++c) cp_async8(&HM_AT(V::V_D + c, r), dat + c * Npad + i);
+      if (keep_mom) { cp_async8(&HM_AT(V_MEAN, r), P.mom_mean + i); cp_async8(&HM_AT(V_M2, r), P.mom_M2 + i); }
+    }
+    cp_async_commit();
+    // ... and while they are in flight the thread makes the plate draws of the launch's first front, which depend on
+    // (seed, object, t) only (the normal is parked in the chi' slot)
+    const uint32_t t_first = (uint32_t)P.iter->t;
+    for (int r = 0; r < nlive; r += 2) {
+      T z[2][2], cs[2], sn[2], u[2];
+      pair_draws<1>(P.tail.seed, P.obj_offset + HM_OBJ(r), t_first, z, cs, sn, u);
 #pragma unroll
-        for (int c = 0; c < ncols; ++c) HM_AT(V::V_D + c, r) = __ldg(dat + c * Npad + i);
-        if (V::m1) HM_AT(V::V_E, r) = hm_exp(x);
-        if (keep_mom) { HM_AT(V_MEAN, r) = P.mom_mean[i]; HM_AT(V_M2, r) = P.mom_M2[i]; }
+      for (int h = 0; h < 2; ++h) {
+        if (r + h < nlive) { HM_AT(V::V_XP, r + h) = z[h][0]; HM_AT(V::V_U, r + h) = u[h]; }
       }
+    }
+    cp_async_wait_all();
+    for (int r = 0; r < nlive; ++r) {                        // the rest of the first front: chi' = chi + L z, e^chi, e^chi'
+      const T x = HM_AT(V::V_CHI, r);
+      const T xp = x + HM_AT(V::V_L, r) * HM_AT(V::V_XP, r);
+      HM_AT(V::V_XP, r) = xp;
+      if (V::m1) { HM_AT(V::V_E, r) = hm_exp(x); HM_AT(V::V_EP, r) = hm_exp_point(xp); }
     }
   }
   __syncthreads();
@@ -126,7 +134,6 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
     const T astar = (T)P.astar_chi;
     double nacc = 0.0, nnan = 0.0;
 
-    front((uint32_t)t0);
     for (long long k = 0; k < n_iter; ++k) {
       const long long t = t0 + k;
       if (k > 0) bar_sync(BAR_THETA, RES_THREADS);          // theta_t and everything derived from it are in `it`
