@@ -311,6 +311,8 @@ def kernel_label(st):
     """Which persistent kernel a THETA_DEVICE_TAIL run launched (cudahm_get_stats says)."""
     if st["block_threads"] == 640:
         return "k_resident"
+    if st["block_threads"] == 384:
+        return "k_resident_gen"
     if st.get("stage_steps", 0) or st.get("l2_prefetch", 0):
         return f"k_persistent<AHEAD> (staged draw steps {st['stage_steps']}, L2 prefetch {'on' if st['l2_prefetch'] else 'off'})"
     return "k_persistent"
@@ -524,7 +526,7 @@ def main():
                           "streaming persistent kernel on a working set SMALLER than L2 (the sampler iterates over the "
                           "same objects inside one launch, so there is nothing to flush between iterations): the state "
                           "is served from L2, roofline.achieved divides the ALGORITHMIC bytes by the time"
-                          if r["stats"]["block_threads"] != 640 else
+                          if r["stats"]["block_threads"] not in (640, 384) else
                           "state resident ON CHIP by design: the sampler iterates K times over the same objects "
                           "inside one persistent launch and keeps them in shared memory, so there is nothing to "
                           "flush between iterations; roofline.achieved divides the ALGORITHMIC bytes by the time "

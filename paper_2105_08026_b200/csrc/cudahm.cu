@@ -78,7 +78,7 @@ struct cudahm_sampler {
   bool timed = false;
   unsigned epoch = 1;               // next mailbox epoch of the persistent kernel
   const void* res_kernel = nullptr; // on-chip persistent kernel (resident.cuh) when the population fits, else NULL
-  int res_R = 0, res_OB = 0; size_t res_smem = 0;
+  int res_R = 0, res_OB = 0, res_threads = 0; size_t res_smem = 0;
   int sweep_grid = 1, sweep_block = 512;   // launch shape of k_sweep (THETA_GRAPH / HOST / debug_step)
   int tma_stages = 0; size_t tma_smem = 0;   // > 0: the streaming persistent kernel is k_persistent_tma
   bool ahead = false;                        // run k_persistent<.., AHEAD = true>
@@ -322,7 +322,20 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
       const size_t bytes = (size_t)nv * R * RES_S * sizeof(double);
       if (bytes <= (size_t)RES_MAX_SMEM && ensure_dyn_smem(rk, bytes) == cudaSuccess) {
         s->res_kernel = rk; s->res_R = (int)R; s->res_OB = (int)OB; s->res_smem = bytes;
-        s->grid = (int)g; s->block = RES_THREADS;
+        s->grid = (int)g; s->block = RES_THREADS; s->res_threads = RES_THREADS;
+      } else {
+        cudaGetLastError();
+      }
+    } else if (rs.gen_kernel) {
+      // the general on-chip kernel: groups of `vec` adjacent objects per thread, 256 sweep threads per block
+      const long long vec = rs.gen_vec;
+      const long long g = std::min<long long>(sms, (cfg->n_objects + vec * 32 - 1) / (vec * 32));     // >= one warp of groups per block
+      const long long OB = vec * ((cfg->n_objects + vec * g - 1) / (vec * g));                        // objects per block
+      const long long R = vec * ((OB + vec * RG_S - 1) / (vec * RG_S));                               // slots per thread
+      const size_t bytes = (size_t)rs.gen_values * R * RG_S * s->tsize;
+      if (bytes <= (size_t)RES_MAX_SMEM && ensure_dyn_smem(rs.gen_kernel, bytes) == cudaSuccess) {
+        s->res_kernel = rs.gen_kernel; s->res_R = (int)R; s->res_OB = (int)OB; s->res_smem = bytes;
+        s->grid = (int)g; s->block = RG_THREADS; s->res_threads = RG_THREADS;
       } else {
         cudaGetLastError();
       }
@@ -665,7 +678,7 @@ int run_device_tail(cudahm_sampler* s, long long n_iter) {
     if (s->res_kernel) {
       cudaError_t e = ensure_dyn_smem(s->res_kernel, s->res_smem);      // a map lookup unless the limit has to grow
       if (e == cudaSuccess)
-        e = launch_persistent(s, s->res_kernel, s->grid, RES_THREADS, args, s->res_smem);
+        e = launch_persistent(s, s->res_kernel, s->grid, s->res_threads, args, s->res_smem);
       if (e != cudaSuccess) return fail(s, CUDAHM_E_CUDA, "resident kernel launch: %s", cudaGetErrorString(e));
       s->launches++;
       rc = CUDAHM_OK;

@@ -24,6 +24,10 @@ struct KernelSet {
 struct ResidentSet {
   const void* kernel;              // NULL: the model has no on-chip kernel in this precision
   int n_base;                      // shared-memory values per object without the running moments (+ 2 with them)
+  // the general on-chip kernel (resident_gen.cuh; p >= 2, fp32 state): entry point, values of T per object, objects per
+  // thread group (16 bytes of T)
+  const void* gen_kernel;
+  int gen_values, gen_vec;
 };
 
 // each returns false when the (precision, block) combination is not compiled in for that model

@@ -4,6 +4,7 @@
 #include "kernel_sets.h"
 #include "kernels.cuh"
 #include "resident.cuh"
+#include "resident_gen.cuh"
 #include "stream_tma.cuh"
 
 namespace hm {
@@ -24,6 +25,13 @@ KernelSet make_set() {
   k.sweep_tap = (const void*)k_sweep<MODEL, T, BLOCK, true>;
   k.init_state = (const void*)k_init_state<MODEL, T>;
   return k;
+}
+
+template <int MODEL, class T>
+void set_resident_gen(ResidentSet* r) {
+  r->gen_kernel = (const void*)k_resident_gen<MODEL, T>;
+  r->gen_values = ResGenValues<MODEL, T>::n_values;
+  r->gen_vec = VecOf<T>::n;
 }
 
 template <int MODEL, class T>

@@ -69,10 +69,11 @@ def test_c5_full_size_free_running():
 
 def test_c6_full_size_free_running():
     """C6, the normal-normal benchmark at the paper's largest population (N = 3e4, p = 3) in the
-    streaming persistent kernel; 40 iterations."""
+    general on-chip kernel (resident_gen.cuh: 148 x 384); 40 iterations."""
     c, orc, gpu = _pair("C6")
     orc.run(40, 0, 1)
     gpu.run(40, 0, 1, sync=True)
+    assert gpu.get_stats()["block_threads"] == 384, "C6 must run the general on-chip kernel"
     so, sg = orc.get_state(), gpu.get_state()
     np.testing.assert_allclose(gpu.get_theta_trace(), orc.get_theta_trace(), rtol=1e-9, atol=1e-9)
     np.testing.assert_allclose(sg["chi"], so["chi"], rtol=1e-9, atol=1e-9)

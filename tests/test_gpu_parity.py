@@ -535,3 +535,32 @@ def test_mask_calls_need_the_config_switches():
     b.set_update_mask(mask_dev)
     b.run(3, 0, 1, sync=True)
     assert b.get_stats()["chi_proposals"] == 50 * 3000 + 3 * 1500
+
+
+@pytest.mark.parametrize("model,precision,astar,n", [(B.M_BINORMAL2D, B.F64, 0.234, 150_001), (B.M_NORMAL3D_KNOWNCOV, B.F64, 0.234, 30_000),
+                                                       (B.M_NORMAL6D_KNOWNCOV, B.F64, 0.234, 9_001),
+                                                       (B.M_LINREG_ME1D, B.F32_STATE_F64_REDUCE, 0.44, 400_003)],
+                         ids=["M2", "M5", "p6", "M3f32"])
+def test_general_on_chip_kernel_is_the_streaming_chain(model, precision, astar, n):
+    """resident_gen.cuh keeps p >= 2 and fp32 populations in shared memory and runs update_vec itself from there: per object
+    the same arithmetic as the streaming kernel, so chi / L / moments agree to the rounding of the (differently ordered)
+    population sums, over several slots per thread and a ragged tail."""
+    iters, burn, thin = 60, 10, 5
+    out, inp = [], None
+    for flags in (0, B.FLAG_STREAMING_ONLY):
+        _, g, inp = make_pair(model, n, seed=55 + model, precision=precision, astar=astar, keep_moments=True,
+                              max_trace_rows=(iters - burn) // thin, want_oracle=False, flags=flags, inputs=inp)
+        g.run(iters, burn, thin, sync=True)
+        st = g.get_state()
+        out.append((st["chi"], st["L"], g.get_theta_trace(), g.get_chi_moments()[0], g.get_stats()))
+        g.close()
+    assert out[0][4]["block_threads"] == 384 and out[1][4]["block_threads"] != 384
+    if precision == B.F64:
+        np.testing.assert_allclose(out[0][2], out[1][2], rtol=1e-9, atol=1e-10)
+        np.testing.assert_allclose(out[0][0], out[1][0], rtol=1e-9, atol=1e-10)
+        np.testing.assert_allclose(out[0][1], out[1][1], rtol=1e-9, atol=1e-12)
+        np.testing.assert_allclose(out[0][3], out[1][3], rtol=1e-10, atol=1e-10)
+        assert out[0][4]["chi_accepts"] == out[1][4]["chi_accepts"]
+    else:      # fp32: theta differs by the rounding of the sums, which flips a few near-tie decisions over 60 iterations
+        np.testing.assert_allclose(out[0][2], out[1][2], rtol=1e-4, atol=1e-4)
+        assert abs(out[0][4]["chi_accepts"] - out[1][4]["chi_accepts"]) <= 1e-4 * iters * n
