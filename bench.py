@@ -36,13 +36,17 @@ UNIT = "updates/s"
 ALG_BYTES = {"C0": (48, 32), "C1": (48, 32), "C2": (48, 32), "C3": (112, 64), "C4": (28, 32), "C5": (48, 32),
              "C6": (240, 96)}     # p = 3: chi 3 + L 6 doubles read and written, 3 data doubles read
 MODES = {"host": 0, "graph": 1, "tail": 2}
-# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel PER LAUNCH, from committed `ncu --set full` captures of
-# exactly the (config, warm-up, steps) named in the key; any other launch reports traffic = null.  Filled from profiles/.
-NCU_DRAM_BYTES_PER_LAUNCH = {}
-# warp-level instructions executed per 32 object-updates (ncu smsp__inst_executed.sum / (N K / 32)) and the share of them
-# on the fp64 pipe, per config, from the committed captures; None where no capture exists.  They give the two compute
-# floors reported beside the HBM one: issue slots (4 warp-instructions / clk / SM) and the fp64 pipe (64 lanes / clk / SM).
-NCU_WARP_INSTR_PER_32 = {"C2": (425, 0.37 * 4 * 32 / 64 / 0.61), "C3": (459, None), "C4": (165, None)}
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel PER LAUNCH of K iterations, as (bytes per launch that do
+# not depend on K, bytes per iteration), from the committed `ncu --set full` captures under profiles/ (r02_*_ncu.md):
+#   C2  on-chip kernel: 14.69 MB at K = 20 (the driver's launch) and 14.66 MB at K = 300 -- the state load; nothing per iteration
+#   C3  streaming kernel, 60 iterations: 586.4 MB = 9.77 MB per iteration (the 104 MB working set is served from L2: hit rate 93 %)
+#   C4  streaming kernel, 30 iterations: 8,333.8 MB = 277.8 MB per iteration (= the algorithmic 280 MB: nothing is re-read)
+#   C6  general on-chip kernel, 300 iterations: 3.12 MB, taken as the per-launch state load
+# A config without a capture reports traffic = null.
+NCU_DRAM_BYTES = {"C2": (14.68e6, 0.0), "C3": (0.0, 586.41e6 / 60), "C4": (0.0, 8333.78e6 / 30), "C6": (3.12e6, 0.0)}
+# warp-level instructions executed per 32 object-updates (smsp__inst_executed.sum / (N K / 32)) and fp64-pipe activity from
+# the same captures.  They give the compute floor reported beside the HBM one: issue slots (4 warp-instructions / clk / SM).
+NCU_WARP_INSTR_PER_32 = {"C2": (420, 38.0), "C3": (433, 39.6), "C4": (162, 14.2), "C6": (1366, None)}
 N_SMS, SM_CLOCK_HZ = 148, 1.965e9
 
 
@@ -329,7 +333,8 @@ def roofline_entry(cfg_name, c, n, K, W, ms, peak, peak_src, kernel=None):
     us = ms * 1e3 / K
     hbm_floor = bytes_per_iter / (peak * 1e9) * 1e6
     out = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-           "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((cfg_name, W, K)) if n == c.n_objects else None,
+           "traffic": (NCU_DRAM_BYTES[cfg_name][0] + NCU_DRAM_BYTES[cfg_name][1] * K)
+                      if (n == c.n_objects and cfg_name in NCU_DRAM_BYTES) else None,
            "peak_source": peak_src, "kernel": kernel,
            "launches_timed": 1, "iterations_per_launch": K, "alg_bytes_per_object_iter": per_obj,
            "alg_bytes_per_iter": bytes_per_iter, "alg_bytes_per_launch": bytes_per_iter * K,
@@ -339,6 +344,7 @@ def roofline_entry(cfg_name, c, n, K, W, ms, peak, peak_src, kernel=None):
         issue = ins[0] * (n / 32.0) / (4.0 * N_SMS * SM_CLOCK_HZ) * 1e6
         out["floors_us_per_iter"]["issue_slots"] = issue
         out["warp_instructions_per_32_updates"] = ins[0]
+        out["fp64_pipe_active_pct_ncu"] = ins[1]
         out["frac_of_slowest_floor"] = max(hbm_floor, issue) / us
     return out
 
