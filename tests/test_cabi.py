@@ -78,7 +78,7 @@ def test_invalid_configs_are_refused(lib):
     assert B.workspace_bytes(B.make_config(B.M_NORMAL1D, 10, flags=ok)) > 0
     assert B.workspace_bytes(B.make_config(B.M_NORMAL1D, 10, flags=B.flag_stage_steps(0) | B.FLAG_PREFETCH_OFF)) > 0
     assert B.workspace_bytes(B.make_config(B.M_NORMAL1D, 10, flags=1 << 16)) == 0
-    assert B.workspace_bytes(B.make_config(B.M_NORMAL1D, 10, flags=16)) == 0
+    assert B.workspace_bytes(B.make_config(B.M_NORMAL1D, 10, flags=1 << 20)) == 0
     assert B.flag_stage_steps(0) == 0x100 and B.flag_stage_steps(2) == 0x300
     cfg = B.make_config(B.M_NORMAL3D_KNOWNCOV, 10, precision=B.F32_STATE_F64_REDUCE)
     h = C.c_void_p()
