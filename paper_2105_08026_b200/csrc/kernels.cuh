@@ -664,16 +664,6 @@ __global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const l
     mbox_push<NVX>(mb, G, (int)blockIdx.x, epoch, dq, (int)threadIdx.x, (int)blockDim.x);
     // warps 0-3: collect + theta tail (the serial chain); the other warps meanwhile make the plate draws of the
     // first n_stage steps of iteration t + 1, which depend on nothing but (seed, object, t + 1)
-    if (!AHEAD) {
-      double tot[NPART] = {0.0, 0.0, 0.0, 0.0, 0.0};
-      if (threadIdx.x < 32) {
-        double t2[2] = {0.0, 0.0};
-        mbox_collect<NVX>(mb + (size_t)blockIdx.x * mbox_reader_words(G), G, epoch, t2);
-        tot[1] = t2[0]; tot[2] = t2[1];
-      }
-      tail_block<MODEL>(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, (int)(threadIdx.x >> 5), SyncAll());
-      continue;
-    }
     if (threadIdx.x < TAILT) {
       double tot[NPART] = {0.0, 0.0, 0.0, 0.0, 0.0};
       if (threadIdx.x < 32) {
@@ -682,10 +672,10 @@ __global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const l
         tot[1] = t2[0]; tot[2] = t2[1];
       }
       tail_block<MODEL>(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, (int)(threadIdx.x >> 5), SyncNamed<1, TAILT>());
-    } else if (k + 1 < n_iter) {
+    } else if (AHEAD && k + 1 < n_iter) {
       stage_draws<MODEL, T>(P, t_next, stage, n_stage, (int)threadIdx.x - TAILT, BLOCK - TAILT);
     }
-    __syncthreads();
+    __syncthreads();                    // the plain variant's other warps wait here: only warps 0-3 run the tail
   }
   block_reduce<2>(cnt, red);
   if (threadIdx.x == 0) {
