@@ -339,7 +339,12 @@ struct Impl : Base {
       lp_cur = logprior(model, theta.data()) + user_prior(theta.data());
       lp_prop = logprior(model, thp) + user_prior(thp);
       double la_th;
-      if (lp_prop == ninf) { log_r = ninf; la_th = ninf; T_prop = 0; }
+      // Eq. 4.3 divides by I(theta')^N: where the selection integral is not a positive normal number the likelihood is
+      // undefined and the proposal is rejected like one outside the prior's support (reading R26)
+      bool undefined = false;
+      if (model == M_BB1_FLUXNOISE1D && lp_prop != ninf)
+        undefined = !(table.bb1_integral(thp, consts.data()) >= std::numeric_limits<double>::min());
+      if (lp_prop == ninf || undefined) { log_r = ninf; la_th = ninf; T_prop = 0; }
       else {
         T_prop = theta_only(thp);
         log_r = (double)Delta + (T_prop - T_cur) + (lp_prop - lp_cur);

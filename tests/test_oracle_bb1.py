@@ -269,3 +269,24 @@ def test_theta_posterior_bb1_against_eq_4_3_grid():
     s, inp = _sampler(n, 41, truth=(-1.3, np.log(0.3), 0.0))
     s.run(burn + T, burn_in=burn)
     check_bb1_posterior(inp, s.get_theta_trace())
+
+
+def test_a_proposal_with_vanishing_selection_integral_is_rejected():
+    """DESIGN.md reading R26: Eq. 4.3 divides by I(theta')^N.  Inside the prior box I(theta') underflows to 0 once e^(-L/u)
+    does for every node (ln u below about -20 with x_lo = ln 1e-5); such a proposal is rejected (alpha = 0), exactly like one
+    outside the prior's support -- it is NOT accepted on log r = -N log 0 = +inf."""
+    n = 60
+    s, inp = _sampler(n, 43)
+    st = s.get_state()
+    theta = np.array([st["theta"][0], -29.0, st["theta"][2]])   # l tiny, so that l < u' holds far down in ln u'
+    chol = np.array([1e-3, 0.0, 1e-3, 0.0, 0.0, 12.0])          # a theta proposal that jumps far in ln u
+    hit = 0
+    for t in range(600):
+        s.set_state(st["chi"], st["L"], theta, chol, t)
+        tp = s.step(taps=True)
+        th = tp["theta_prop"]
+        if np.isfinite(tp["lp_prop"]) and th[2] < -21.0:
+            assert s.theta_only(th) == np.inf                   # -N log I with I = 0
+            assert tp["accepted_theta"] == 0 and tp["alpha_theta"] == 0.0 and tp["T_prop"] == 0.0 and tp["log_r"] == -np.inf
+            hit += 1
+    assert hit >= 8, hit
