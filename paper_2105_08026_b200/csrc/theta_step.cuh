@@ -153,7 +153,10 @@ HM_HD void decide_scalars(const Iter& it, const TailCfg& c, const Draws& d, doub
                           double* log_r, double* la, int* acc, int model = -1) {
   if (model < 0) model = c.model;
   *T_prop = 0.0;
-  if (it.lp_prop == -INFINITY) {
+  // M4: Eq. 4.3 divides by I(theta')^N; a selection sum that is not a positive normal number leaves the likelihood undefined
+  // and the proposal is rejected like one outside the prior's support (reading R26; hm_log_pos needs a normal input)
+  const bool undefined = model == M_BB1_FLUXNOISE1D && !(tq >= 2.2250738585072014e-308);
+  if (it.lp_prop == -INFINITY || undefined) {
     *log_r = -INFINITY; *la = -INFINITY;
   } else {
     // M1: T(theta') = -A' sum_k W_k phi(x_k; theta'): minus the expected detected count (Eq. 4.4 denominator)

@@ -564,3 +564,32 @@ def test_general_on_chip_kernel_is_the_streaming_chain(model, precision, astar, 
     else:      # fp32: theta differs by the rounding of the sums, which flips a few near-tie decisions over 60 iterations
         np.testing.assert_allclose(out[0][2], out[1][2], rtol=1e-4, atol=1e-4)
         assert abs(out[0][4]["chi_accepts"] - out[1][4]["chi_accepts"]) <= 1e-4 * iters * n
+
+
+@pytest.mark.parametrize("mode", [B.THETA_HOST, B.THETA_DEVICE_TAIL], ids=["host", "device"])
+def test_m4_proposal_with_vanishing_selection_integral_is_rejected(mode):
+    """DESIGN.md reading R26 on the GPU, device tail (k_tail through debug_step) and host tail (THETA_HOST run): a theta'
+    inside the prior box whose selection sum underflows to 0 is rejected, as in the oracle -- not accepted on -N log 0."""
+    n = 60
+    orc, gpu, inp = make_pair(B.M_BB1_FLUXNOISE1D, n, seed=43, theta_mode=mode, max_trace_rows=0)
+    st = orc.get_state()
+    theta = np.array([st["theta"][0], -29.0, st["theta"][2]])
+    chol = np.array([1e-3, 0.0, 1e-3, 0.0, 0.0, 12.0])
+    hit = 0
+    for t in range(400):
+        orc.set_state(st["chi"], st["L"], theta, chol, t)
+        gpu.set_state(st["chi"], st["L"], theta, chol, t)
+        to = orc.step(NO_TRACE, 1, taps=True)
+        if mode == B.THETA_HOST:
+            gpu.run(1, NO_TRACE, 1, sync=True)
+            acc_g = int(not np.array_equal(gpu.get_state()["theta"], theta))
+        else:
+            tg = gpu.debug_step(NO_TRACE, 1)
+            acc_g = tg["accepted_theta"]
+            np.testing.assert_allclose(tg["theta_prop"], to["theta_prop"], rtol=1e-9, atol=1e-9)
+        if np.isfinite(to["lp_prop"]) and to["theta_prop"][2] < -21.0:
+            assert to["accepted_theta"] == 0 and acc_g == 0
+            hit += 1
+        elif abs(to["log_r"]) > 1e-6 or not np.isfinite(to["log_r"]):
+            assert acc_g == to["accepted_theta"]
+    assert hit >= 5, hit
