@@ -135,6 +135,8 @@ typedef struct {
   double  last_run_ms;           /* device time of the last cudahm_run (needs CUDAHM_FLAG_TIME_RUNS; else 0)  */
   int32_t stage_steps;           /* streaming persistent kernel: steps of plate draws staged ahead per thread */
   int32_t l2_prefetch;           /* ... 1: it prefetches the next step's columns into L2 (0 for the on-chip kernel) */
+  int32_t dedicated_tail;        /* 1: the streaming kernel with dedicated tail warps (k_persistent_dt) runs             */
+  int32_t pad_;
 } cudahm_stats;
 
 /* Per-iteration taps of cudahm_debug_step; HOST pointers, each may be NULL.  Values are widened to double. */

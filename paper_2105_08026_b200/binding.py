@@ -55,7 +55,7 @@ class Stats(C.Structure):
                                          "theta_proposals", "nonfinite", "moment_samples", "trace_rows",
                                          "gpu_launches")] + \
                [("grid_blocks", C.c_int32), ("block_threads", C.c_int32), ("last_run_ms", C.c_double),
-                ("stage_steps", C.c_int32), ("l2_prefetch", C.c_int32)]
+                ("stage_steps", C.c_int32), ("l2_prefetch", C.c_int32), ("dedicated_tail", C.c_int32), ("pad_", C.c_int32)]
 
 
 class Taps(C.Structure):

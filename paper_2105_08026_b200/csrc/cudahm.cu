@@ -82,6 +82,7 @@ struct cudahm_sampler {
   int sweep_grid = 1, sweep_block = 512;   // launch shape of k_sweep (THETA_GRAPH / HOST / debug_step)
   int tma_stages = 0; size_t tma_smem = 0;   // > 0: the streaming persistent kernel is k_persistent_tma
   bool ahead = false;                        // run k_persistent<.., AHEAD = true>
+  bool dt = false;                           // run k_persistent_dt (dedicated tail warps)
   int prefetch = 0;                          // ... with L2 prefetch of the next step's columns
   int n_stage = 0; size_t stage_smem = 0;    // k_persistent: steps of plate draws staged in shared memory ahead of the sweep
   double h_lp_prop_before = 0.0;    // log prior at theta' of the iteration debug_step is about to decide
@@ -299,6 +300,22 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
           (long long)fit * sms < s->grid) { cudaGetLastError(); s->ahead = false; s->n_stage = 0; s->stage_smem = 0; s->prefetch = 0; }
     }
   }
+  // dedicated tail warps (k_persistent_dt) where the model's translation unit built them and nothing else was asked for:
+  // default block size, no staged draws / prefetch chosen above, no TMA staging, no frozen-member hooks
+  if (cfg->theta_mode == CUDAHM_THETA_DEVICE_TAIL && cfg->n_objects > 0 && ks.persistent_dt && !cfg->block_threads && !s->hold &&
+      !s->ahead && !(cfg->flags & (CUDAHM_FLAG_TMA_STAGING | CUDAHM_FLAG_STAGE_STEPS_MASK | CUDAHM_FLAG_PREFETCH_ON))) {
+    const long long per = (long long)s->vec * ks.dt_sweep_threads;
+    s->dt = true;
+    s->grid = (int)std::max(1LL, std::min<long long>(sms, (cfg->n_objects + per - 1) / per));
+    s->block = ks.dt_sweep_threads + 128;
+    s->sweep_grid = s->grid; s->sweep_block = ks.dt_sweep_threads;      // k_sweep at the same thread -> object map
+    // own-thread staged draws: steps of plate draws made while the thread waits for the theta decision
+    const long long steps = (cfg->n_objects + per * s->grid - 1) / (per * s->grid);
+    long long ns = 2;                     // measured on C3: 0 -> 22.4, 1 -> 22.3, 2 -> 22.0, 3 -> 22.2, 4 -> 22.6 us per iteration
+    ns = std::min<long long>(std::min(ns, steps), (long long)(STAGE_MAX_SMEM / (ks.stage_step_bytes * ks.dt_sweep_threads / block)));
+    s->n_stage = (int)ns; s->stage_smem = (size_t)ns * (ks.stage_step_bytes * ks.dt_sweep_threads / block);
+    if (ensure_dyn_smem(ks.persistent_dt, s->stage_smem) != cudaSuccess) { cudaGetLastError(); s->n_stage = 0; s->stage_smem = 0; }
+  }
   // HBM-streaming variant with TMA-staged loads (stream_tma.cuh), opt-in: measured 10-30 % slower than plain vector
   // loads on C3 / C4 (the sweep is issue-bound, not latency-bound, and the producer warp costs a sweep warp)
   if (cfg->theta_mode == CUDAHM_THETA_DEVICE_TAIL && (cfg->flags & CUDAHM_FLAG_TMA_STAGING) && block <= 512 && ks.persistent_tma && !s->hold) {
@@ -322,7 +339,7 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
       const size_t bytes = (size_t)nv * R * RES_S * sizeof(double);
       if (bytes <= (size_t)RES_MAX_SMEM && ensure_dyn_smem(rk, bytes) == cudaSuccess) {
         s->res_kernel = rk; s->res_R = (int)R; s->res_OB = (int)OB; s->res_smem = bytes;
-        s->grid = (int)g; s->block = RES_THREADS; s->res_threads = RES_THREADS;
+        s->grid = (int)g; s->block = RES_THREADS; s->res_threads = RES_THREADS; s->dt = false;
       } else {
         cudaGetLastError();
       }
@@ -335,7 +352,7 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
       const size_t bytes = (size_t)rs.gen_values * R * RG_S * s->tsize;
       if (bytes <= (size_t)RES_MAX_SMEM && ensure_dyn_smem(rs.gen_kernel, bytes) == cudaSuccess) {
         s->res_kernel = rs.gen_kernel; s->res_R = (int)R; s->res_OB = (int)OB; s->res_smem = bytes;
-        s->grid = (int)g; s->block = RG_THREADS; s->res_threads = RG_THREADS;
+        s->grid = (int)g; s->block = RG_THREADS; s->res_threads = RG_THREADS; s->dt = false;
       } else {
         cudaGetLastError();
       }
@@ -691,6 +708,12 @@ int run_device_tail(cudahm_sampler* s, long long n_iter) {
       if (e != cudaSuccess) return fail(s, CUDAHM_E_CUDA, "streaming kernel launch: %s", cudaGetErrorString(e));
       s->launches++;
       rc = CUDAHM_OK;
+    } else if (s->dt) {
+      void* dargs[] = {&P, &k, &epoch0, &ns, &pf};
+      cudaError_t e = launch_persistent(s, s->ks.persistent_dt, s->grid, s->block, dargs, s->stage_smem);
+      if (e != cudaSuccess) return fail(s, CUDAHM_E_CUDA, "streaming kernel launch: %s", cudaGetErrorString(e));
+      s->launches++;
+      rc = CUDAHM_OK;
     } else {
       const void* fn = s->hold ? s->ks.persistent_hold : s->ahead ? s->ks.persistent_ahead : s->ks.persistent;
       cudaError_t e = s->ahead ? ensure_dyn_smem(fn, s->stage_smem) : cudaSuccess;
@@ -709,7 +732,7 @@ int run_device_tail(cudahm_sampler* s, long long n_iter) {
 int enqueue_graph_iteration(cudahm_sampler* s) {
   Params P = s->P;
   void* a1[] = {&P};
-  int rc = launch(s, s->hold ? s->ks.sweep_hold : s->ks.sweep, s->sweep_grid, s->sweep_block, a1, false);
+  int rc = launch(s, s->hold ? s->ks.sweep_hold : s->dt ? s->ks.sweep_dt : s->ks.sweep, s->sweep_grid, s->sweep_block, a1, false);
   if (rc) return rc;
   int nb = s->sweep_grid, flags = TAIL_DECIDE;
   void* a2[] = {&P, &nb, &flags};
@@ -758,7 +781,7 @@ int run_graph(cudahm_sampler* s, long long n_iter) {
 int host_sweep(cudahm_sampler* s, void* totals_dev = nullptr) {   // -> s->h_totals = {S, Delta, Tq, n_accept, n_nonfinite} of this handle
   Params P = s->P;
   void* a1[] = {&P};
-  int rc = launch(s, s->hold ? s->ks.sweep_hold : s->ks.sweep, s->sweep_grid, s->sweep_block, a1, false);
+  int rc = launch(s, s->hold ? s->ks.sweep_hold : s->dt ? s->ks.sweep_dt : s->ks.sweep, s->sweep_grid, s->sweep_block, a1, false);
   if (rc) return rc;
   int nb = s->sweep_grid, flags = TAIL_REDUCE;
   void* a2[] = {&P, &nb, &flags};
@@ -979,7 +1002,7 @@ extern "C" int cudahm_debug_step(cudahm_sampler* s, int64_t burn_in, int32_t thi
   P.taps.shift_c = lc; P.taps.shift_p = lcp;
   const bool prop_in_support = s->h_iter->lp_prop != -INFINITY;
   void* a1[] = {&P};
-  rc = launch(s, s->hold ? s->ks.sweep_tap_hold : s->ks.sweep_tap, s->sweep_grid, s->sweep_block, a1, false);
+  rc = launch(s, s->hold ? s->ks.sweep_tap_hold : s->dt ? s->ks.sweep_tap_dt : s->ks.sweep_tap, s->sweep_grid, s->sweep_block, a1, false);
   int nb = s->sweep_grid, flags = TAIL_REDUCE | TAIL_DECIDE;     // the device tail decides t and prepares t + 1
   void* a2[] = {&P, &nb, &flags};
   if (!rc) rc = launch(s, (const void*)k_tail, 1, TAIL_THREADS, a2, false);
@@ -1052,7 +1075,8 @@ extern "C" int cudahm_get_stats(cudahm_sampler* s, cudahm_stats* out) {
   if (!s || !out) return fail(s, CUDAHM_E_INVALID, "get_stats: NULL argument");
   std::memset(out, 0, sizeof *out);
   out->grid_blocks = s->grid; out->block_threads = s->block; out->gpu_launches = s->launches;
-  const bool streaming_tail = s->cfg.theta_mode == CUDAHM_THETA_DEVICE_TAIL && !s->res_kernel && s->tma_stages == 0 && s->ahead;
+  const bool streaming_tail = s->cfg.theta_mode == CUDAHM_THETA_DEVICE_TAIL && !s->res_kernel && s->tma_stages == 0 && (s->ahead || s->dt);
+  out->dedicated_tail = (s->dt && !s->res_kernel) ? 1 : 0;
   out->stage_steps = streaming_tail ? s->n_stage : 0; out->l2_prefetch = streaming_tail ? s->prefetch : 0;
   if (!s->have_init) return CUDAHM_OK;
   int rc = fetch_iter(s); if (rc) return rc;

@@ -18,6 +18,11 @@ struct KernelSet {
   const void* persistent_hold;
   const void* sweep_hold;
   const void* sweep_tap_hold;
+  // streaming kernel with dedicated tail warps (k_persistent_dt) and its sweep threads per block; NULL where not built
+  const void* persistent_dt;
+  int dt_sweep_threads;
+  const void* sweep_dt;          // k_sweep / tapped k_sweep at the same thread -> object map
+  const void* sweep_tap_dt;
 };
 
 // on-chip kernel (resident.cuh) of one (model, precision)

@@ -45,6 +45,11 @@ struct Params {
   DevTaps taps;
 };
 
+// named barriers of the kernels with dedicated tail warps (resident.cuh, resident_gen.cuh, k_persistent_dt)
+__device__ __forceinline__ void bar_sync(const int id, const int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void bar_arrive(const int id, const int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+enum : int { BAR_PARTIALS = 1, BAR_THETA = 2, BAR_TAIL = 3, BAR_THETAP = 4 };
+
 template <class T> struct VecOf;
 template <> struct VecOf<double> { using type = double2; static constexpr int n = 2; };
 template <> struct VecOf<float>  { using type = float4;  static constexpr int n = 4; };
@@ -162,15 +167,16 @@ template <class T> struct SweepCtx {
   double inv_k;
 };
 template <class T>
-__device__ __forceinline__ SweepCtx<T> make_ctx(const Params& P, const Iter& it) {
+__device__ __forceinline__ SweepCtx<T> make_ctx(const Params& P, const Iter& it, const long long t_or_neg = -1) {
   SweepCtx<T> c;
-  c.t = (uint32_t)it.t;
+  const long long t_it = t_or_neg >= 0 ? t_or_neg : it.t;       // (a kernel that starts before the tail has bumped it.t passes t)
+  c.t = (uint32_t)t_it;
   c.kc = it.kc; c.kp = it.kp;
   c.kT = narrow<T>(c.kc);
 #pragma unroll
   for (int j = 0; j < MC_N; ++j) c.mcT[j] = (T)P.mc[j];
-  c.eta = (T)it.dr[it.t % 3].eta; c.astar = (T)P.astar_chi;
-  c.do_mom = P.tail.keep_moments && it.t > P.tail.burn_in;
+  c.eta = (T)it.dr[t_it % 3].eta; c.astar = (T)P.astar_chi;
+  c.do_mom = P.tail.keep_moments && t_it > P.tail.burn_in;
   c.inv_k = 1.0 / (double)(it.mom_count + 1);
   return c;
 }
@@ -217,10 +223,17 @@ template <int MODEL, class T> struct DrawSet {
 // HOLD: the variant for frozen members.  An object whose mask byte is 0 takes no RAM step (chi, L and its
 // update count stay bit for bit; its draws are made and discarded, the streams being counter-based) but still contributes
 // a_i, b_i; with a per-object counter eta_n comes from the object's own update count n_i = count + 2.
-template <int MODEL, class T, bool TAP, bool HOLD = false>
+// LateKp (k_persistent_dt): theta' and its constants are still being derived by the tail warps when the sweep of the next
+// iteration starts; the population term at theta' reads them from shared memory, after a one-off wait per iteration.
+struct LateKp {
+  const ThetaK* kp;      // it.kp in shared memory
+  int* wait;             // != 0: sync on BAR_THETAP (n threads) before the first use, then cleared
+  int n;
+};
+template <int MODEL, class T, bool TAP, bool HOLD = false, bool LATE = false>
 __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c, const long long base,
                                            T (*x)[VecOf<T>::n], T (*l)[VecOf<T>::n], const T (*d)[VecOf<T>::n], double* sum,
-                                           const DrawSet<MODEL, T>* staged = nullptr) {
+                                           const DrawSet<MODEL, T>* staged = nullptr, const LateKp* late = nullptr) {
   constexpr int p = ModelDims<MODEL>::p, ntri = p * (p + 1) / 2, ncols = ModelDims<MODEL>::ncols;
   constexpr int VEC = VecOf<T>::n;
   DrawSet<MODEL, T> ds_;
@@ -312,7 +325,10 @@ __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c
       ln[2] = l[2][v] * k11;
     }
     // population terms at the new chi, fp64
-    const double a = PL::pop(qn, di, c.kc, P.mc), b = PL::pop(qn, di, c.kp, P.mc);
+    if constexpr (LATE) {
+      if (*late->wait) { bar_sync(BAR_THETAP, late->n); *late->wait = 0; }
+    }
+    const double a = PL::pop(qn, di, c.kc, P.mc), b = PL::pop(qn, di, LATE ? *late->kp : c.kp, P.mc);
     if (live) {
       if constexpr (HOLD) {
 #pragma unroll
@@ -367,9 +383,9 @@ __device__ __forceinline__ double selection_slice(const Params& P, const ThetaK&
 }
 
 // one step of the sweep: load the thread's VEC objects, update, store
-template <int MODEL, class T, bool TAP, bool HOLD = false>
+template <int MODEL, class T, bool TAP, bool HOLD = false, bool LATE = false>
 __device__ __forceinline__ void sweep_step(const Params& P, const SweepCtx<T>& c, const long long base, double* acc,
-                                           const DrawSet<MODEL, T>* staged) {
+                                           const DrawSet<MODEL, T>* staged, const LateKp* late = nullptr) {
   constexpr int p = ModelDims<MODEL>::p, ntri = p * (p + 1) / 2, ncols = ModelDims<MODEL>::ncols;
   constexpr int VEC = VecOf<T>::n;
   const long long Npad = P.Npad;
@@ -383,7 +399,7 @@ __device__ __forceinline__ void sweep_step(const Params& P, const SweepCtx<T>& c
   for (int k = 0; k < ntri; ++k) ld_vec<T>(Lm + k * Npad + base, l[k], false);
 #pragma unroll
   for (int cc = 0; cc < ncols; ++cc) ld_vec<T>(dat + cc * Npad + base, d[cc], true);
-  update_vec<MODEL, T, TAP, HOLD>(P, c, base, x, l, d, acc, staged);
+  update_vec<MODEL, T, TAP, HOLD, LATE>(P, c, base, x, l, d, acc, staged, late);
 #pragma unroll
   for (int j = 0; j < p; ++j) st_vec(chi + j * Npad + base, x[j]);
 #pragma unroll
@@ -681,6 +697,112 @@ __global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const l
   if (threadIdx.x == 0) {
     P.blk_cnt[2 * blockIdx.x] += (unsigned long long)cnt[0];
     P.blk_cnt[2 * blockIdx.x + 1] += (unsigned long long)cnt[1];
+  }
+  if (blockIdx.x == 0) copy_iter(P.iter, &it);
+}
+
+// The streaming kernel with DEDICATED tail warps: SWEEP sweep threads + 4 tail warps per block.
+// The sweep warps hand their partials over and wait only for the DECISION of the theta step (theta_{t+1} and its constants);
+// the rest of the tail -- RAM update of L_theta, theta', its constants, prior, W: ~4,000 cycles -- runs on the tail warps
+// while the sweep warps already load, draw, propose and decide the first objects of iteration t + 1; the population term at
+// theta' waits once per iteration for the tail to finish (LateKp).  Worth it where fewer sweep warps with more registers are
+// as fast as 16 (p = 2 in fp64: the sweep is latency-bound); same per-object arithmetic, its own (fixed) summation order.
+constexpr int DT_TAIL = 128;
+template <int MODEL, class T, int SWEEP>
+__global__ void __launch_bounds__(SWEEP + DT_TAIL, 1) k_persistent_dt(const Params P, const long long n_iter, const unsigned epoch0,
+                                                                      const int n_stage, const int prefetch) {
+  constexpr int VEC = VecOf<T>::n, THREADS = SWEEP + DT_TAIL, SW = SWEEP / 32, NV = DrawSet<MODEL, T>::NV;
+  // a sweep thread makes the plate draws of its OWN first n_stage steps of iteration t + 1 while it waits for the decision of
+  // iteration t (they depend on (seed, object, t + 1) only) and parks them in shared memory: [step][value][thread]
+  extern __shared__ __align__(16) unsigned char stage_raw[];
+  T* const stage = reinterpret_cast<T*>(stage_raw) + threadIdx.x;
+  __shared__ Iter it;
+  __shared__ double red[2][SW];
+  __shared__ unsigned long long cnt_sm[2];
+  const int tid = (int)threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int G = (int)gridDim.x;
+  copy_iter(&it, P.iter);
+  if (tid < 2) cnt_sm[tid] = 0ull;
+  __syncthreads();
+  const long long t0 = it.t;
+  if (tid < SWEEP) {
+    const long long N = P.N;
+    const long long stride = (long long)VEC * G * SWEEP;
+    const long long first = (long long)VEC * ((long long)blockIdx.x * SWEEP + tid);
+    double nacc = 0.0, nnan = 0.0;
+    auto stage_own = [&](const uint32_t t) {
+      long long base = first;
+      for (int s = 0; s < n_stage && base < N; ++s, base += stride) {
+        DrawSet<MODEL, T> ds;
+        ds.make(P, base, t);
+        ds.put(stage + (size_t)s * NV * SWEEP, SWEEP);
+      }
+    };
+    stage_own((uint32_t)t0);
+    for (long long k = 0; k < n_iter; ++k) {
+      if (k > 0) bar_sync(BAR_THETA, THREADS);               // the decision of iteration t - 1 is taken: kc, eta, moment count
+      const SweepCtx<T> c = make_ctx<T>(P, it, t0 + k);      // (its kp is not used: LateKp)
+      int wait = k > 0 ? 1 : 0;
+      const LateKp late{&it.kp, &wait, THREADS};
+      double acc[4] = {0.0, 0.0, 0.0, 0.0};
+      long long base = first;
+      for (int s = 0; s < n_stage && base < N; ++s, base += stride) {
+        if (prefetch) prefetch_step<MODEL, T>(P, base + stride < N ? base + stride : first);
+        DrawSet<MODEL, T> ds;
+        ds.get(stage + (size_t)s * NV * SWEEP, SWEEP);
+        sweep_step<MODEL, T, false, false, true>(P, c, base, acc, &ds, &late);
+      }
+      for (; base < N; base += stride) {
+        if (prefetch) prefetch_step<MODEL, T>(P, base + stride < N ? base + stride : first);
+        sweep_step<MODEL, T, false, false, true>(P, c, base, acc, nullptr, &late);
+      }
+      if (wait) bar_sync(BAR_THETAP, THREADS);               // a thread without objects still takes part in the barrier
+      nacc += acc[2]; nnan += acc[3];
+      double v = acc[1];
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+      if (lane == 0) red[k & 1][warp] = v;
+      __threadfence_block();
+      bar_arrive(BAR_PARTIALS, THREADS);
+      if (k + 1 < n_iter) stage_own((uint32_t)(t0 + k + 1));
+    }
+    bar_sync(BAR_THETA, THREADS);
+    bar_sync(BAR_THETAP, THREADS);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      nacc += __shfl_down_sync(0xffffffffu, nacc, o);
+      nnan += __shfl_down_sync(0xffffffffu, nnan, o);
+    }
+    if (lane == 0) {
+      atomicAdd(&cnt_sm[0], (unsigned long long)nacc);
+      atomicAdd(&cnt_sm[1], (unsigned long long)nnan);
+    }
+  } else {
+    const int tw = warp - SW, ttid = tid - SWEEP;
+    for (long long k = 0; k < n_iter; ++k) {
+      bar_sync(BAR_PARTIALS, THREADS);
+      double dq[1];
+      dq[0] = lane < SW ? red[k & 1][lane] : 0.0;
+      lanes_to_total<1>(dq);
+      unsigned long long* mb = P.mbox + (size_t)(k & 1) * mbox_parity_words(G);
+      const unsigned epoch = epoch0 + (unsigned)k;
+      mbox_push<1>(mb, G, (int)blockIdx.x, epoch, dq, ttid, DT_TAIL);
+      double tot[NPART] = {0.0, 0.0, 0.0, 0.0, 0.0};
+      if (tw == 0) {
+        double t1[1];
+        mbox_collect<1>(mb + (size_t)blockIdx.x * mbox_reader_words(G), G, epoch, t1);
+        tot[1] = t1[0];
+      }
+      tail_block<MODEL>(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, tw, SyncNamed<BAR_TAIL, DT_TAIL>(),
+                        ArriveNamed<BAR_THETA, THREADS>());
+      __threadfence_block();
+      bar_arrive(BAR_THETAP, THREADS);
+    }
+  }
+  __syncthreads();
+  if (tid == 0) {
+    P.blk_cnt[2 * blockIdx.x] += cnt_sm[0];
+    P.blk_cnt[2 * blockIdx.x + 1] += cnt_sm[1];
   }
   if (blockIdx.x == 0) copy_iter(P.iter, &it);
 }

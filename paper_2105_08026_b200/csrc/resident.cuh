@@ -38,9 +38,6 @@ __device__ __forceinline__ void cp_async8(double* dst_smem, const double* src) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
-__device__ __forceinline__ void bar_sync(const int id, const int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
-__device__ __forceinline__ void bar_arrive(const int id, const int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
-enum : int { BAR_PARTIALS = 1, BAR_THETA = 2, BAR_TAIL = 3, BAR_THETAP = 4 };
 
 template <int MODEL>
 __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, const long long n_iter, const unsigned epoch0,

@@ -84,13 +84,13 @@ def test_c6_full_size_free_running():
 
 
 def test_c3_full_size_free_running():
-    """C3 as benched: N = 1e6, 2-D latent, streaming persistent kernel (148 x 512); 8 iterations."""
+    """C3 as benched: N = 1e6, 2-D latent, streaming kernel with dedicated tail warps (148 x (384 + 128)); 8 iterations."""
     c, orc, gpu = _pair("C3")
     orc.run(8, 0, 1)
     gpu.run(8, 0, 1, sync=True)
     st = gpu.get_stats()
     assert (st["grid_blocks"], st["block_threads"]) == (148, 512)
-    assert (st["stage_steps"], st["l2_prefetch"]) == (0, 0), "C3 (state + data inside L2, p = 2) keeps the plain variant"
+    assert (st["dedicated_tail"], st["stage_steps"], st["l2_prefetch"]) == (1, 2, 0), "C3 as benched: k_persistent_dt (DESIGN.md 8.7b)"
     so, sg = orc.get_state(), gpu.get_state()
     np.testing.assert_allclose(gpu.get_theta_trace(), orc.get_theta_trace(), rtol=1e-9, atol=1e-9)
     np.testing.assert_allclose(sg["chi"], so["chi"], rtol=1e-9, atol=1e-9)
