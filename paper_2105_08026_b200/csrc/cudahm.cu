@@ -375,6 +375,7 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
                    cfg->target_accept_theta, cfg->eta_exponent, 0, cfg->max_trace_rows, 1, 0,
                    (double)(cfg->n_objects_total ? cfg->n_objects_total : cfg->n_objects), cfg->adapt_until, {}, {}};
   P.obj_offset = cfg->object_offset;
+  P.rk = make_round_keys(cfg->seed);
   P.mask = cfg->update_mask ? (const unsigned char*)(s->ws + lay.mask) : nullptr;
   P.cnt = cfg->per_object_counter ? (unsigned*)(s->ws + lay.cnt) : nullptr;
   for (int j = 0; j < MAXD; ++j) { P.tail.prior_mean[j] = cfg->prior_mean[j]; P.tail.prior_isd[j] = cfg->prior_isd[j]; }

@@ -43,6 +43,7 @@ struct Params {
   unsigned* cnt;                 // [Npad] RAM updates object i has taken (eta_n from the object's own count); NULL = global n
   TailCfg tail;
   DevTaps taps;
+  RoundKeys rk;                  // Philox round keys of tail.seed (philox.cuh)
 };
 
 // named barriers of the kernels with dedicated tail warps (resident.cuh, resident_gen.cuh, k_persistent_dt)
@@ -85,8 +86,8 @@ __device__ __forceinline__ float hm_sqrt_pos(float x) { return x * rsqrtf(x); }
 //   fp32  p = 1: one call per pair (draw 0 of pair m): x -> u1, y -> u2, cos / sin branch, accept uniforms z / w.
 // i0 is the even object of the pair.  z[h][k]: normal k of object i0 + h.
 //         p >= 3 normals:  per object, draws 1 + k of object i give (z_2k, z_2k+1), k = 0 .. ceil(p/2) - 1.
-template <int P, int ZD>
-__device__ __forceinline__ void pair_draws(unsigned long long seed, long long i0, uint32_t t, double (*z)[ZD], double* cs,
+template <int P, int ZD, class KEY>
+__device__ __forceinline__ void pair_draws(const KEY& seed, long long i0, uint32_t t, double (*z)[ZD], double* cs,
                                            double* sn, double* u) {
   const uint64_t m = (uint64_t)i0 >> 1;
   const U4 a = stream(seed, KIND_PLATE, m, t, 0u);
@@ -125,8 +126,8 @@ __device__ __forceinline__ void pair_draws(unsigned long long seed, long long i0
     }
   }
 }
-template <int P, int ZD>
-__device__ __forceinline__ void pair_draws(unsigned long long seed, long long i0, uint32_t t, float (*z)[ZD], float* cs,
+template <int P, int ZD, class KEY>
+__device__ __forceinline__ void pair_draws(const KEY& seed, long long i0, uint32_t t, float (*z)[ZD], float* cs,
                                            float* sn, float* u) {
   static_assert(P <= 2, "fp32 state: p <= 2");
   if (P == 1) {
@@ -192,8 +193,13 @@ template <int MODEL, class T> struct DrawSet {
   static constexpr int NZ = p, NU = (p == 2 ? 2 : 0), NV = VEC * (NZ + NU + 1);
   T zz[VEC][ZD], csv[VEC], snv[VEC], uu[VEC];
   __device__ __forceinline__ void make(const Params& P, const long long base, const uint32_t t) {
+    // KEY of the plate streams: the seed (fp64 kernels) or its ready-made round keys (fp32 kernels: philox.cuh; measured
+    // -1.4 % on C4, while the fp64 kernels, bound by their fp64 chains, gain nothing or lose to the changed schedule)
 #pragma unroll
-    for (int v = 0; v < VEC; v += 2) pair_draws<p>(P.tail.seed, P.obj_offset + base + v, t, &zz[v], &csv[v], &snv[v], &uu[v]);
+    for (int v = 0; v < VEC; v += 2) {
+      if constexpr (sizeof(T) == 4) pair_draws<p, ZD>(P.rk, P.obj_offset + base + v, t, &zz[v], &csv[v], &snv[v], &uu[v]);
+      else pair_draws<p, ZD>((uint64_t)P.tail.seed, P.obj_offset + base + v, t, &zz[v], &csv[v], &snv[v], &uu[v]);
+    }
   }
   // staged layout: value q of thread-slot j at st[q * stride + j] (unit stride across a warp: conflict-free)
   __device__ __forceinline__ void put(T* st, const int stride) const {

@@ -37,6 +37,31 @@ HM_HD U4 philox4x32_10(U4 c, uint32_t k0, uint32_t k1) {
   return c;
 }
 
+// The key schedule (a Weyl sequence of the seed) is the same for every call: the sweep takes the 10 round keys ready-made
+// from the kernel parameters (constant bank operands of the XORs) instead of bumping the key twice per round and call --
+// 20 integer adds less per Philox call, about 6 % of the instructions of the fp32 kernel.  Same words bit for bit.
+struct RoundKeys { uint32_t k0[10], k1[10]; };
+HM_HD RoundKeys make_round_keys(uint64_t seed) {
+  RoundKeys rk;
+  uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+  for (int r = 0; r < 10; ++r) { rk.k0[r] = k0; rk.k1[r] = k1; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
+  return rk;
+}
+HM_HD U4 philox4x32_10(U4 c, const RoundKeys& rk) {
+  constexpr uint32_t PM0 = 0xD2511F53u, PM1 = 0xCD9E8D57u;
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint32_t h0 = mulhi32(PM0, c.x), l0 = PM0 * c.x;
+    const uint32_t h1 = mulhi32(PM1, c.z), l1 = PM1 * c.z;
+    c = U4{h1 ^ c.y ^ rk.k0[r], l1, h0 ^ c.w ^ rk.k1[r], l0};
+  }
+  return c;
+}
+HM_HD U4 stream(const RoundKeys& rk, int kind, uint64_t obj, uint32_t t, uint32_t d) {
+  U4 c{(uint32_t)obj, ((uint32_t)kind << 24) | ((uint32_t)(obj >> 32) & 0xffffffu), t, d};
+  return philox4x32_10(c, rk);
+}
+
 // counter = (object lo, kind<<24 | object bits 32..55, iteration, draw); key = seed words
 HM_HD U4 stream(uint64_t seed, int kind, uint64_t obj, uint32_t t, uint32_t d) {
   U4 c{(uint32_t)obj, ((uint32_t)kind << 24) | ((uint32_t)(obj >> 32) & 0xffffffu), t, d};

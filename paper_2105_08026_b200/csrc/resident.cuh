@@ -91,7 +91,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
     const uint32_t t_first = (uint32_t)P.iter->t;
     for (int r = 0; r < nlive; r += 2) {
       T z[2][2], cs[2], sn[2], u[2];
-      pair_draws<1>(P.tail.seed, P.obj_offset + HM_OBJ(r), t_first, z, cs, sn, u);
+      pair_draws<1, 2>((uint64_t)P.tail.seed, P.obj_offset + HM_OBJ(r), t_first, z, cs, sn, u);
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
         if (r + h < nlive) { HM_AT(V::V_XP, r + h) = z[h][0]; HM_AT(V::V_U, r + h) = u[h]; }
@@ -113,7 +113,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
     auto front = [&](const uint32_t t) {
       for (int r = 0; r < nlive; r += 2) {
         T z[2][2], cs[2], sn[2], u[2];
-        pair_draws<1>(P.tail.seed, P.obj_offset + HM_OBJ(r), t, z, cs, sn, u);
+        pair_draws<1, 2>((uint64_t)P.tail.seed, P.obj_offset + HM_OBJ(r), t, z, cs, sn, u);
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
           if (r + h < nlive) {
