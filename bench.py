@@ -208,6 +208,17 @@ def make_theta_chol0(inp, n):
     return None if f is None else np.asarray(f, dtype=np.float64)
 
 
+def warm_up(s, W, thin):
+    """The W untimed warm-up iterations, as three cudahm_run calls (W - 2, 1, 1) where W allows: the library submits a
+    handle's first persistent launch directly, builds its one-node graph at the second and pays the graph's first in-place
+    parameter update at the third -- the timed regions then see the steady launch path."""
+    parts = [W - 2, 1, 1] if W >= 3 else [W]
+    for k in parts:
+        if k > 0:
+            s.run(k, W, thin)
+    s.sync()
+
+
 def time_gpu(cfg_name, args, device, rank, world, barrier, with_clocks=True, repeats=REPEATS):
     """W burn-in iterations untimed, then `repeats` timed regions of EXACTLY K iterations each, back to back, each timed
     on the device with CUDA events on the sampler's stream (inputs resident in HBM).  ms = the median region."""
@@ -217,7 +228,7 @@ def time_gpu(cfg_name, args, device, rank, world, barrier, with_clocks=True, rep
     dt = np.float64 if c.precision == synth.F64 else np.float32
     dev_cols = [torch.from_numpy(np.ascontiguousarray(col, dtype=dt)).to(device) for col in inp["cols"]]
     s = make_gpu_sampler(c, n, inp, args, c.seed + rank, trace_rows_needed(W + repeats * K, W, c.thin), device, cols=dev_cols)
-    s.run(W, W, c.thin, sync=True)                      # burn-in = warm-up (adaptation, caches, clocks)
+    warm_up(s, W, c.thin)                               # burn-in = warm-up (adaptation, caches, clocks, launch path)
     l0 = s.get_stats()["gpu_launches"]
     stream = s.stream
     clk = ClockSampler(torch.device(device).index or 0) if with_clocks else None
@@ -262,7 +273,7 @@ def fixed_cost_per_run(cfg_name, args, device):
     a = copy.copy(args)
     a.n_objects = 0
     s = make_gpu_sampler(c, n, inp, a, c.seed, trace_rows_needed(W + 3 * (K1 + K2), W, c.thin), device)
-    s.run(W, W, c.thin, sync=True)
+    warm_up(s, W, c.thin)
     best = {}
     for K in (K1, K2, K1, K2, K1, K2):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)

@@ -91,6 +91,7 @@ struct cudahm_sampler {
   cudaGraphNode_t pg_node = nullptr;
   const void* pg_fn = nullptr;
   bool pg_broken = false;
+  long long pg_launches = 0;
   cudaGraphExec_t gexec = nullptr;
   long long g_burn = -1; int g_thin = -1; int g_iters = 0;
   std::string err;
@@ -646,7 +647,9 @@ namespace {
 // place: measured 1.5-2 us less launch latency per cudahm_run than cudaLaunchCooperativeKernel.  Falls
 // back to the direct launch for good if any graph call fails.
 cudaError_t launch_persistent(cudahm_sampler* s, const void* fn, int grid, int block, void** args, size_t smem) {
-  if (!s->pg_broken) {
+  // the first launch of a handle goes out directly: building the graph costs ~100 us of host time, which a caller who runs
+  // the whole chain in one cudahm_run should not pay before its kernel starts
+  if (!s->pg_broken && s->pg_launches++ > 0) {
     cudaKernelNodeParams kp{};
     kp.func = const_cast<void*>(fn); kp.gridDim = dim3(grid); kp.blockDim = dim3(block); kp.sharedMemBytes = (unsigned)smem;
     kp.kernelParams = args; kp.extra = nullptr;
@@ -1039,10 +1042,10 @@ extern "C" int cudahm_debug_step(cudahm_sampler* s, int64_t burn_in, int32_t thi
 extern "C" int cudahm_get_theta_trace(cudahm_sampler* s, double* out, int64_t cap_rows, int64_t* n_rows) {
   if (!s || !n_rows) return fail(s, CUDAHM_E_INVALID, "get_theta_trace: NULL argument");
   if (!s->have_init) return fail(s, CUDAHM_E_STATE, "get_theta_trace before set_init");
+  if (!out) { *n_rows = s->h_trace_rows; return CUDAHM_OK; }      // the count is mirrored on the host: no synchronisation
   int rc = fetch_iter(s); if (rc) return rc;
   const long long rows = s->h_iter->trace_rows;
   *n_rows = rows;
-  if (!out) return CUDAHM_OK;
   if (cap_rows < rows) return fail(s, CUDAHM_E_INVALID, "trace has %lld rows, capacity %lld", rows, (long long)cap_rows);
   if (rows > 0) CU_TRY(s, cudaMemcpy(out, s->P.trace, (size_t)rows * s->dtheta * 8, cudaMemcpyDeviceToHost));
   return CUDAHM_OK;
