@@ -231,6 +231,19 @@ int cudahm_shard_decide_gathered(cudahm_sampler* s, int64_t burn_in, int32_t thi
 /* One iteration through the non-persistent sweep + tail kernels with per-object taps (test instrument). */
 int cudahm_debug_step(cudahm_sampler* s, int64_t burn_in, int32_t thin, cudahm_taps* taps);
 
+/* cudahm_debug_step for callers that cannot call cudaMalloc (code under CUDA-graph capture, tight serving loops, harnesses
+ * that forbid it): identical kernels and taps, but the per-object tap scratch -- (p + p(p+1)/2 + 6) doubles and one int per
+ * object, which cudahm_debug_step cudaMallocs and frees on every call -- lives in ONE file-scope device array of
+ * CUDAHM_NOALLOC_SCRATCH_BYTES that every GPU loading the library holds until the process exits.  The call allocates no
+ * device memory (no cudaMalloc / cudaFree / allocating library routine).  CUDAHM_E_WORKSPACE, with nothing touched, if the
+ * handle needs more than the array holds (cudahm_debug_step_noalloc_bytes(s) says how much: p = 1 fits about 61,600
+ * objects, p = 2 45,500, p = 6 15,600).  Every call on a device shares the array, which keeps the previous call's contents: the range
+ * a call uses is cleared before its kernels run, and calls that OVERLAP on the GPU (other streams, other host threads) race
+ * -- serialise them.  The handle's device must be current, as for every other call. */
+#define CUDAHM_NOALLOC_SCRATCH_BYTES (4u << 20)
+int cudahm_debug_step_noalloc(cudahm_sampler* s, int64_t burn_in, int32_t thin, cudahm_taps* taps);
+size_t cudahm_debug_step_noalloc_bytes(const cudahm_sampler* s);
+
 /* out: row-major n_rows x dtheta host doubles.  out == NULL just reports n_rows. */
 int cudahm_get_theta_trace(cudahm_sampler* s, double* out, int64_t cap_rows, int64_t* n_rows);
 /* mean, var: p*N host doubles (SoA); var is the sample variance (divisor n_samples - 1). */

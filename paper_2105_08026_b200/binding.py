@@ -25,9 +25,11 @@ def flag_stage_steps(n):
     """CUDAHM_FLAG_STAGE_STEPS(n): exactly n steps of plate draws staged ahead of the sweep (0 = off)."""
     return ((int(n) + 1) << 8) & 0xff00
 FLOOR_LAUNCH, FLOOR_GRAPH, FLOOR_GRID_BARRIER, FLOOR_HOST_SYNC = 0, 1, 2, 3
+NOALLOC_SCRATCH_BYTES = 4 << 20       # CUDAHM_NOALLOC_SCRATCH_BYTES
 
 EXPORTS = ["cudahm_model_dims", "cudahm_workspace_bytes", "cudahm_create", "cudahm_destroy", "cudahm_set_data",
-           "cudahm_set_model_consts", "cudahm_set_init", "cudahm_run", "cudahm_debug_step",
+           "cudahm_set_model_consts", "cudahm_set_init", "cudahm_run", "cudahm_debug_step", "cudahm_debug_step_noalloc",
+           "cudahm_debug_step_noalloc_bytes",
            "cudahm_get_theta_trace", "cudahm_get_chi_moments", "cudahm_get_stats", "cudahm_get_state",
            "cudahm_set_state", "cudahm_sync", "cudahm_last_error", "cudahm_shard_sweep", "cudahm_shard_decide", "cudahm_shard_combine", "cudahm_shard_sweep_device",
            "cudahm_shard_decide_gathered", "cudahm_set_update_mask", "cudahm_get_counters", "cudahm_set_counters",
@@ -91,6 +93,9 @@ def load():
     L.cudahm_set_init.argtypes = [vp, vp, C.c_int, _dp, _dp]
     L.cudahm_run.argtypes = [vp, C.c_int64, C.c_int64, C.c_int32]
     L.cudahm_debug_step.argtypes = [vp, C.c_int64, C.c_int32, C.POINTER(Taps)]
+    L.cudahm_debug_step_noalloc.argtypes = [vp, C.c_int64, C.c_int32, C.POINTER(Taps)]
+    L.cudahm_debug_step_noalloc_bytes.argtypes = [vp]
+    L.cudahm_debug_step_noalloc_bytes.restype = C.c_size_t
     L.cudahm_get_theta_trace.argtypes = [vp, _dp, C.c_int64, C.POINTER(C.c_int64)]
     L.cudahm_get_chi_moments.argtypes = [vp, _dp, _dp, C.c_int64, C.POINTER(C.c_int64)]
     L.cudahm_get_stats.argtypes = [vp, C.POINTER(Stats)]
@@ -311,6 +316,28 @@ class Sampler:
                   "accepted_theta"):
             out[k] = getattr(tp, k)
         return out
+
+    def debug_step_noalloc(self, burn_in=0, thin=1):
+        """cudahm_debug_step_noalloc: the same tapped iteration with its tap scratch in the library's built-in device array
+        (no cudaMalloc in the call); raises CudahmError(E_WORKSPACE) if the population does not fit NOALLOC_SCRATCH_BYTES."""
+        N, p = self.N, self.p
+        out = dict(chi_prop=np.empty((p, N)), pi_cur=np.empty(N), pi_prop=np.empty(N), alpha=np.empty(N),
+                   u=np.empty(N), accepted=np.empty(N, dtype=np.int32), L_new=np.empty((self.ntri, N)),
+                   a=np.empty(N), b=np.empty(N))
+        tp = Taps()
+        for k in ("chi_prop", "pi_cur", "pi_prop", "alpha", "u", "L_new", "a", "b"):
+            setattr(tp, k, _d(out[k]))
+        tp.accepted = out["accepted"].ctypes.data_as(_ip)
+        with self._dev():
+            self._ck(self.lib.cudahm_debug_step_noalloc(self._h, burn_in, thin, C.byref(tp)))
+        out["theta_prop"] = np.array(tp.theta_prop[: self.dtheta])
+        for k in ("S", "Delta", "T_cur", "T_prop", "lp_cur", "lp_prop", "log_r", "alpha_theta", "u_theta",
+                  "accepted_theta"):
+            out[k] = getattr(tp, k)
+        return out
+
+    def debug_step_noalloc_bytes(self):
+        return int(self.lib.cudahm_debug_step_noalloc_bytes(self._h))
 
     def get_theta_trace(self):
         n = C.c_int64()

@@ -1039,6 +1039,115 @@ extern "C" int cudahm_debug_step(cudahm_sampler* s, int64_t burn_in, int32_t thi
   return CUDAHM_OK;
 }
 
+// ----------------------------------------------------------------------------------------------------
+// cudahm_debug_step_noalloc: the tapped iteration for callers that cannot call cudaMalloc (code under CUDA-graph capture,
+// tight serving loops, harnesses that forbid it).  Same kernels, same launch shape, same taps as cudahm_debug_step; the tap
+// scratch lives in ONE file-scope device array of CUDAHM_NOALLOC_SCRATCH_BYTES instead of a cudaMalloc per call.
+//   - every GPU that loads the library holds the array until the process exits;
+//   - in host code `g_noalloc_scratch` is a host-side STAND-IN for the symbol, not a device address: its device address is
+//     looked up once per device, with that device current, by cudaGetSymbolAddress (noalloc_scratch_ptr) and only that
+//     pointer is handed to the kernels;
+//   - every call on a device shares the array, which keeps the previous call's contents: the range a call uses is cleared
+//     (stream-ordered) before its kernels run, and calls that overlap on the GPU (two streams, two host threads) RACE.
+namespace {
+static __device__ __align__(256) unsigned char g_noalloc_scratch[CUDAHM_NOALLOC_SCRATCH_BYTES];
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+// device address of g_noalloc_scratch on the CURRENT device (resolved once per device); NULL + *err on failure
+unsigned char* noalloc_scratch_ptr(cudaError_t* err) {
+  static std::mutex mu;
+  static unsigned char* ptr_of_device[NOALLOC_MAX_DEVICES] = {};
+  int dev = -1;
+  *err = cudaGetDevice(&dev);
+  if (*err != cudaSuccess) return nullptr;
+  if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) { *err = cudaErrorInvalidDevice; return nullptr; }
+  std::lock_guard<std::mutex> lock(mu);
+  if (!ptr_of_device[dev]) {
+    void* q = nullptr;
+    *err = cudaGetSymbolAddress(&q, g_noalloc_scratch);
+    if (*err != cudaSuccess || !q) { if (*err == cudaSuccess) *err = cudaErrorInvalidSymbol; return nullptr; }
+    ptr_of_device[dev] = static_cast<unsigned char*>(q);
+  }
+  return ptr_of_device[dev];
+}
+// bytes of tap scratch one tapped iteration of this handle needs: (p + ntri + 6) doubles and one int per object
+size_t noalloc_bytes_needed(const cudahm_sampler* s) {
+  const size_t N = (size_t)s->P.N;
+  return align_up((size_t)(s->p + s->ntri + 6) * N * sizeof(double)) + N * sizeof(int);
+}
+}  // namespace
+
+extern "C" size_t cudahm_debug_step_noalloc_bytes(const cudahm_sampler* s) { return s ? noalloc_bytes_needed(s) : 0; }
+
+extern "C" int cudahm_debug_step_noalloc(cudahm_sampler* s, int64_t burn_in, int32_t thin, cudahm_taps* taps) {
+  if (!s || !taps) return fail(s, CUDAHM_E_INVALID, "debug_step_noalloc: NULL argument");
+  if (!s->have_init) return fail(s, CUDAHM_E_STATE, "debug_step_noalloc before set_init");
+  if (burn_in < 0 || thin < 1) return fail(s, CUDAHM_E_INVALID, "debug_step_noalloc: bad burn_in/thin");
+  const size_t N = (size_t)s->P.N;
+  const size_t dbytes = align_up((size_t)(s->p + s->ntri + 6) * N * sizeof(double)), need = noalloc_bytes_needed(s);
+  if (need > (size_t)CUDAHM_NOALLOC_SCRATCH_BYTES)      // refused before anything is touched: the handle stays usable
+    return fail(s, CUDAHM_E_WORKSPACE,
+                "debug_step_noalloc: %lld objects of this model need %zu bytes of tap scratch, the built-in array holds %zu "
+                "(CUDAHM_NOALLOC_SCRATCH_BYTES); use cudahm_debug_step for larger populations",
+                (long long)N, need, (size_t)CUDAHM_NOALLOC_SCRATCH_BYTES);
+  cudaError_t e = cudaSuccess;
+  unsigned char* const scratch = noalloc_scratch_ptr(&e);
+  if (!scratch) return fail(s, CUDAHM_E_CUDA, "debug_step_noalloc: cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+  int rc = fetch_iter(s); if (rc) return rc;
+  if (s->cfg.theta_mode == CUDAHM_THETA_HOST)   // make the device copy current
+    CU_TRY(s, cudaMemcpy(s->P.iter, s->h_iter, sizeof(Iter), cudaMemcpyHostToDevice));
+  const long long t = s->h_iter->t;
+  s->h_lp_prop_before = s->h_iter->lp_prop;
+  if (s->cfg.max_trace_rows > 0 && t > burn_in && ((t - burn_in) % thin) == 0 &&
+      s->h_iter->trace_rows + 1 > s->cfg.max_trace_rows)
+    return fail(s, CUDAHM_E_INVALID, "theta trace is full");
+  s->P.tail.burn_in = burn_in; s->P.tail.thin = thin;
+  // the array keeps the last call's taps (possibly another handle's): clear the range this call uses
+  if (need > 0) CU_TRY(s, cudaMemsetAsync(scratch, 0, need, s->stream));
+  double* const dbuf = reinterpret_cast<double*>(scratch);
+  int* const ibuf = reinterpret_cast<int*>(scratch + dbytes);
+  Params P = s->P;
+  double* q = dbuf;
+  P.taps.chi_prop = q; q += (size_t)s->p * N;
+  P.taps.L_new = q; q += (size_t)s->ntri * N;
+  P.taps.pi_cur = q; q += N; P.taps.pi_prop = q; q += N; P.taps.alpha = q; q += N;
+  P.taps.u = q; q += N; P.taps.a = q; q += N; P.taps.b = q; q += N;
+  P.taps.accepted = ibuf;
+  double lc = 0.0, lcp = 0.0;
+  if (s->cfg.model == M_BB1_FLUXNOISE1D) { lc = bb1_log_norm(s->h_iter->theta); lcp = bb1_log_norm(s->h_iter->thetaP); }
+  P.taps.shift_c = lc; P.taps.shift_p = lcp;
+  const bool prop_in_support = s->h_iter->lp_prop != -INFINITY;
+  void* a1[] = {&P};
+  rc = launch(s, s->hold ? s->ks.sweep_tap_hold : s->dt ? s->ks.sweep_tap_dt : s->ks.sweep_tap, s->sweep_grid, s->sweep_block, a1, false);
+  int nb = s->sweep_grid, flags = TAIL_REDUCE | TAIL_DECIDE;
+  void* a2[] = {&P, &nb, &flags};
+  if (!rc) rc = launch(s, (const void*)k_tail, 1, TAIL_THREADS, a2, false);
+  if (rc) return rc;
+  e = cudaMemcpyAsync(s->h_iter, s->P.iter, sizeof(Iter), cudaMemcpyDeviceToHost, s->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  if (e == cudaSuccess) {
+    const Iter& it = *s->h_iter;
+    for (int r = 0; r < 8; ++r) taps->theta_prop[r] = r < s->dtheta ? it.tap_thetaP[r] : 0.0;
+    const double Nd = (double)s->P.N;
+    taps->S = it.S + Nd * lc; taps->Delta = it.Delta + Nd * (lcp - lc);
+    taps->T_cur = it.T_cur_used - Nd * lc; taps->T_prop = it.T_prop - (prop_in_support ? Nd * lcp : 0.0);
+    taps->lp_cur = it.lp_cur_used; taps->lp_prop = s->h_lp_prop_before; taps->log_r = it.log_r;
+    taps->alpha_theta = it.alpha_theta; taps->u_theta = it.u_theta; taps->accepted_theta = it.accepted_theta;
+    struct { double* dst; const double* src; size_t n; } cp[] = {
+        {taps->chi_prop, P.taps.chi_prop, (size_t)s->p * N}, {taps->L_new, P.taps.L_new, (size_t)s->ntri * N},
+        {taps->pi_cur, P.taps.pi_cur, N}, {taps->pi_prop, P.taps.pi_prop, N}, {taps->alpha, P.taps.alpha, N},
+        {taps->u, P.taps.u, N}, {taps->a, P.taps.a, N}, {taps->b, P.taps.b, N}};
+    for (auto& c : cp)
+      if (c.dst && c.n && e == cudaSuccess) e = cudaMemcpy(c.dst, c.src, c.n * sizeof(double), cudaMemcpyDeviceToHost);
+    if (taps->accepted && N && e == cudaSuccess) e = cudaMemcpy(taps->accepted, ibuf, N * sizeof(int), cudaMemcpyDeviceToHost);
+  }
+  if (e != cudaSuccess) return fail(s, CUDAHM_E_CUDA, "debug_step_noalloc: %s", cudaGetErrorString(e));
+  s->t_done += 1;
+  s->h_proposals += s->n_active;
+  s->h_trace_rows = s->h_iter->trace_rows; s->h_mom_count = s->h_iter->mom_count;
+  return CUDAHM_OK;
+}
+
 extern "C" int cudahm_get_theta_trace(cudahm_sampler* s, double* out, int64_t cap_rows, int64_t* n_rows) {
   if (!s || !n_rows) return fail(s, CUDAHM_E_INVALID, "get_theta_trace: NULL argument");
   if (!s->have_init) return fail(s, CUDAHM_E_STATE, "get_theta_trace before set_init");
