@@ -171,6 +171,9 @@ def test_sharded_population_matches_oracle(model, astar, n, on_device):
                                rtol=1e-10, atol=1e-10)
     st, sto = parts[0].get_stats(), orc.get_stats()
     assert st["chi_accepts"] == sto["chi_accepts"] and st["theta_accepts"] == sto["theta_accepts"] and st["iterations"] == iters
+    # accepts are global on every shard, so proposals must be the WHOLE population's too (a rate above 1 otherwise)
+    for g in parts:
+        assert g.get_stats()["chi_proposals"] == sto["chi_proposals"] == iters * n
 
 
 def test_single_shard_is_the_host_mode_run_bit_for_bit():
