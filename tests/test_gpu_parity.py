@@ -596,3 +596,41 @@ def test_m4_proposal_with_vanishing_selection_integral_is_rejected(mode):
         elif abs(to["log_r"]) > 1e-6 or not np.isfinite(to["log_r"]):
             assert acc_g == to["accepted_theta"]
     assert hit >= 5, hit
+
+
+@pytest.mark.parametrize("mode", [B.THETA_HOST, B.THETA_GRAPH, B.THETA_DEVICE_TAIL], ids=["host", "graph", "tail"])
+def test_trace_and_moment_counts_across_split_runs_crossing_burn_in(mode):
+    """cudahm_run checks the trace capacity from HOST mirrors of the row and moment counts (no device read-back before the
+    launch): split runs that cross burn-in with thinning, a zero-length run and a tapped step in between must leave the
+    same counts, trace and moments as the oracle; a run that would overflow the trace is refused with nothing launched."""
+    n, burn, thin = 1500, 20, 7
+    chunks = [7, 1, 13, 0, 29, 50]                      # 100 iterations: rows at t = 27, 34, ..., 97 -> 11
+    rows_total = (sum(chunks) + 1 - burn) // thin        # + 1: the tapped step below
+    orc, gpu, _ = make_pair(B.M_NORMAL1D, n, seed=61, theta_mode=mode, keep_moments=True, max_trace_rows=rows_total)
+    done = 0
+    for k, c in enumerate(chunks):
+        orc.run(c, burn, thin)
+        gpu.run(c, burn, thin, sync=True)
+        done += c
+        if k == 2:                                       # a tapped step through the other kernels, in between
+            orc.step(burn, thin)
+            gpu.debug_step(burn, thin)
+            done += 1
+        sg, so = gpu.get_stats(), orc.get_stats()
+        for key in ("iterations", "trace_rows", "moment_samples"):
+            assert sg[key] == so[key], (key, k)
+        assert sg["trace_rows"] == max(0, (done - burn) // thin) and sg["moment_samples"] == max(0, done - burn)
+    assert gpu.get_theta_trace().shape == (rows_total, 2)
+    np.testing.assert_allclose(gpu.get_theta_trace(), orc.get_theta_trace(), rtol=1e-8, atol=1e-8)
+    mg, vg, kg = gpu.get_chi_moments()
+    mo, vo, ko = orc.get_chi_moments()
+    assert kg == ko == done - burn
+    np.testing.assert_allclose(mg, mo, rtol=1e-10, atol=1e-10)
+    before = gpu.get_state()
+    with pytest.raises(B.CudahmError) as e:              # 7 more iterations would add a 12th row
+        gpu.run(7, burn, thin)
+    assert e.value.code == B.E_INVALID and "trace" in str(e.value)
+    after = gpu.get_state()
+    assert after["t"] == before["t"] and np.array_equal(after["chi"], before["chi"])
+    gpu.run(2, burn, thin, sync=True)                    # still room for iterations that add no row (t = 103 < 104)
+    assert gpu.get_stats()["trace_rows"] == rows_total
