@@ -338,6 +338,7 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
       const long long OB = 2 * ((cfg->n_objects + 2 * g - 1) / (2 * g));                   // objects per block (even)
       const long long R = 2 * ((OB + 2 * RES_S - 1) / (2 * RES_S));                        // slots per thread, in pairs
       const size_t bytes = (size_t)nv * R * RES_S * sizeof(double);
+      if (R <= 2 && rs.kernel_sel_sweep) rk = rs.kernel_sel_sweep;      // short sweep: selection sum on the sweep warps
       if (bytes <= (size_t)RES_MAX_SMEM && ensure_dyn_smem(rk, bytes) == cudaSuccess) {
         s->res_kernel = rk; s->res_R = (int)R; s->res_OB = (int)OB; s->res_smem = bytes;
         s->grid = (int)g; s->block = RES_THREADS; s->res_threads = RES_THREADS; s->dt = false;

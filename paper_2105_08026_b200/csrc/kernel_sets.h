@@ -29,6 +29,7 @@ struct KernelSet {
 struct ResidentSet {
   const void* kernel;              // NULL: the model has no on-chip kernel in this precision
   int n_base;                      // shared-memory values per object without the running moments (+ 2 with them)
+  const void* kernel_sel_sweep;    // variant whose sweep warps compute the selection sum (few slots per thread); may be NULL
   // the general on-chip kernel (resident_gen.cuh; p >= 2, fp32 state): entry point, values of T per object, objects per
   // thread group (16 bytes of T)
   const void* gen_kernel;

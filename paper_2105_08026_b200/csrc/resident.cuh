@@ -39,7 +39,12 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 
-template <int MODEL>
+// SEL_SWEEP (M1 with few slots per thread, e.g. C1): the selection sum at theta' is computed by the 512 SWEEP threads, two
+// nodes each, right after theta' arrives, and handed to the tail warps with the Delta partials -- instead of by the 128 tail
+// threads after the theta tail, where a short sweep leaves it on the critical path (C1: 4.80 -> 4.5 us per iteration).  A
+// variant of its own because the default kernel's code generation must not move (C2 loses 0.1 us to a run-time switch), and
+// not used for M4, whose node term (exp and expm1) is long enough to cost the sweep warps more than it saves the tail.
+template <int MODEL, bool SEL_SWEEP = false>
 __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, const long long n_iter, const unsigned epoch0,
                                                              const int R, const int OB) {
   using T = double;
@@ -48,7 +53,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
   constexpr int ncols = V::ncols;
   extern __shared__ double sm[];
   __shared__ Iter it;
-  __shared__ double red[2][RES_SW][1];
+  __shared__ double red[2][RES_SW][SEL_SWEEP ? 2 : 1];   // per sweep warp: Delta partial (and selection-sum partial)
   __shared__ unsigned long long cnt_sm[2];
   __shared__ double qtab[V::m1 ? 3 : 1][V::m1 ? NQUAD : 1];   // M1: quadrature weights W_k, nodes x_k, e^{x_k}
   __shared__ double tq_warp[RES_TW];     // M1: the tail warps' partial sums of the selection integral at theta'
@@ -74,6 +79,10 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
 
   copy_iter(&it, P.iter);
   if (tid < 2) cnt_sm[tid] = 0ull;
+  if constexpr (SEL_SWEEP) {
+    static_assert(!SEL_SWEEP || V::m1, "SEL_SWEEP is for the models with a selection sum");
+    for (int q = tid; q < NQUAD; q += RES_THREADS) { qtab[0][q] = P.qW[q]; qtab[1][q] = P.qx[q]; qtab[2][q] = P.qex[q]; }
+  }
   if (!is_tail) {
     // The state comes on chip with asynchronous 8-byte copies (cp.async: global -> shared without passing through
     // registers; a thread's slot pair is two adjacent objects, so a warp still reads whole 512-byte runs per column) ...
@@ -208,6 +217,19 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
         if constexpr (V::m1) qn = typename PL::Pt{xn, HM_AT(V::V_E, r)}; else qn = PL::point(&xn);
         v[0] += PL::pop(qn, di, kp, P.mc) - PL::pop(qn, di, kc, P.mc);
       }
+      if constexpr (SEL_SWEEP) {
+        static_assert(NQUAD % RES_S == 0, "quadrature nodes must divide over the sweep threads");
+        if (!P.tail.freeze_theta) {
+#pragma unroll
+          for (int m = 0; m < NQUAD / RES_S; ++m) {
+            const int q = tid + m * RES_S;
+            v[1] += selection_term<MODEL>(kp, qtab[0][q], qtab[1][q], qtab[2][q]);
+          }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[1] += __shfl_down_sync(0xffffffffu, v[1], o);
+        if (lane == 0) red[k & 1][warp][SEL_SWEEP ? 1 : 0] = v[1];
+      }
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) v[0] += __shfl_down_sync(0xffffffffu, v[0], o);
       if (lane == 0) red[k & 1][warp][0] = v[0];
@@ -249,7 +271,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
     // exchanged.  Node tables in shared memory (24 KB), loaded once per launch.
     constexpr int QPT = NQUAD / (RES_TW * 32);
     static_assert(NQUAD % (RES_TW * 32) == 0, "quadrature nodes must divide over the tail threads");
-    if constexpr (V::m1) {
+    if constexpr (V::m1 && !SEL_SWEEP) {
       for (int q = ttid; q < NQUAD; q += RES_TW * 32) { qtab[0][q] = P.qW[q]; qtab[1][q] = P.qx[q]; qtab[2][q] = P.qex[q]; }
     }
     auto selection_full = [&]() {
@@ -269,12 +291,17 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
         bar_sync(BAR_TAIL, RES_TW * 32);
       }
     };
-    selection_full();
+    if constexpr (!SEL_SWEEP) selection_full();
     for (long long k = 0; k < n_iter; ++k) {
       bar_sync(BAR_PARTIALS, RES_THREADS);                   // the block's 16 warp partials of iteration t0 + k
       double dq[1];
       dq[0] = lane < RES_SW ? red[k & 1][lane][0] : 0.0;
       lanes_to_total<1>(dq);
+      double tq[1] = {0.0};
+      if constexpr (SEL_SWEEP) {                             // the sweep warps' partials of the selection sum, same fixed order
+        tq[0] = lane < RES_SW ? red[k & 1][lane][SEL_SWEEP ? 1 : 0] : 0.0;
+        lanes_to_total<1>(tq);
+      }
       unsigned long long* mb = P.mbox + (size_t)(k & 1) * mbox_parity_words(G);
       const unsigned epoch = epoch0 + (unsigned)k;
       mbox_push<1>(mb, G, (int)blockIdx.x, epoch, dq, ttid, RES_TW * 32);
@@ -283,13 +310,14 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
         double t1[1];
         mbox_collect<1>(mb + (size_t)blockIdx.x * mbox_reader_words(G), G, epoch, t1);
         tot[1] = t1[0];
-        if constexpr (V::m1) tot[2] = ((tq_warp[0] + tq_warp[1]) + tq_warp[2]) + tq_warp[3];
+        if constexpr (SEL_SWEEP) tot[2] = tq[0];
+        else if constexpr (V::m1) tot[2] = ((tq_warp[0] + tq_warp[1]) + tq_warp[2]) + tq_warp[3];
       }
       tail_block<MODEL>(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, tw, SyncNamed<BAR_TAIL, RES_TW * 32>(),
                  ArriveNamed<BAR_THETA, RES_THREADS>());      // theta_{t+1} is signalled after the decision phase ...
       __threadfence_block();
       bar_arrive(BAR_THETAP, RES_THREADS);                   // ... theta'_{t+1} and its constants when the tail is done
-      selection_full();                                      // M1: for the NEXT decision; off the critical path
+      if constexpr (!SEL_SWEEP) selection_full();            // M1: for the NEXT decision; off the critical path
     }
   }
 #undef HM_AT
