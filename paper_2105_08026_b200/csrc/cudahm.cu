@@ -346,14 +346,17 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
         cudaGetLastError();
       }
     } else if (rs.gen_kernel) {
-      // the general on-chip kernel: groups of `vec` adjacent objects per thread, 256 sweep threads per block
-      const long long vec = rs.gen_vec;
+      // the general on-chip kernel: groups of `vec` adjacent objects per thread, 256 sweep threads per block; ONE object per
+      // thread where that still covers the population (all sweep warps busy, half the serial work per thread)
+      const bool one = rs.gen_kernel_v1 && cfg->n_objects <= (long long)sms * RG_S;
+      const void* gk = one ? rs.gen_kernel_v1 : rs.gen_kernel;
+      const long long vec = one ? 1 : rs.gen_vec;
       const long long g = std::min<long long>(sms, (cfg->n_objects + vec * 32 - 1) / (vec * 32));     // >= one warp of groups per block
       const long long OB = vec * ((cfg->n_objects + vec * g - 1) / (vec * g));                        // objects per block
       const long long R = vec * ((OB + vec * RG_S - 1) / (vec * RG_S));                               // slots per thread
       const size_t bytes = (size_t)rs.gen_values * R * RG_S * s->tsize;
-      if (bytes <= (size_t)RES_MAX_SMEM && ensure_dyn_smem(rs.gen_kernel, bytes) == cudaSuccess) {
-        s->res_kernel = rs.gen_kernel; s->res_R = (int)R; s->res_OB = (int)OB; s->res_smem = bytes;
+      if (bytes <= (size_t)RES_MAX_SMEM && ensure_dyn_smem(gk, bytes) == cudaSuccess) {
+        s->res_kernel = gk; s->res_R = (int)R; s->res_OB = (int)OB; s->res_smem = bytes;
         s->grid = (int)g; s->block = RG_THREADS; s->res_threads = RG_THREADS; s->dt = false;
       } else {
         cudaGetLastError();

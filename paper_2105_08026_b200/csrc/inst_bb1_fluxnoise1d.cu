@@ -4,7 +4,7 @@
 namespace hm {
 
 bool kernels_bb1_fluxnoise1d(int precision, int block, KernelSet* k, ResidentSet* r) {
-  r->kernel = nullptr; r->kernel_sel_sweep = nullptr; r->n_base = 0; r->gen_kernel = nullptr; r->gen_values = 0; r->gen_vec = 0;
+  r->kernel = nullptr; r->kernel_sel_sweep = nullptr; r->n_base = 0; r->gen_kernel = nullptr; r->gen_kernel_v1 = nullptr; r->gen_values = 0; r->gen_vec = 0;
   if (precision == 0) { r->kernel = (const void*)k_resident<M_BB1_FLUXNOISE1D>; r->n_base = ResValues<M_BB1_FLUXNOISE1D>::n_base; }
   if (precision == 0) return pick_block<M_BB1_FLUXNOISE1D, double>(block, k);
   return false;

@@ -6,7 +6,7 @@
 namespace hm {
 
 bool kernels_normal6d_knowncov(int precision, int block, KernelSet* k, ResidentSet* r) {
-  r->kernel = nullptr; r->kernel_sel_sweep = nullptr; r->n_base = 0; r->gen_kernel = nullptr; r->gen_values = 0; r->gen_vec = 0;
+  r->kernel = nullptr; r->kernel_sel_sweep = nullptr; r->n_base = 0; r->gen_kernel = nullptr; r->gen_kernel_v1 = nullptr; r->gen_values = 0; r->gen_vec = 0;
   if (precision != 0 || block != 256) return false;
   set_resident_gen<M_NORMAL6D_KNOWNCOV, double>(r);
   *k = make_set<M_NORMAL6D_KNOWNCOV, double, 256, false>();

@@ -34,6 +34,7 @@ struct ResidentSet {
   // thread group (16 bytes of T)
   const void* gen_kernel;
   int gen_values, gen_vec;
+  const void* gen_kernel_v1;       // the same kernel with ONE object per thread (fp64, p >= 2; small populations); may be NULL
 };
 
 // each returns false when the (precision, block) combination is not compiled in for that model

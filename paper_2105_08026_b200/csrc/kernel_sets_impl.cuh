@@ -33,6 +33,11 @@ void set_resident_gen(ResidentSet* r) {
   r->gen_kernel = (const void*)k_resident_gen<MODEL, T>;
   r->gen_values = ResGenValues<MODEL, T>::n_values;
   r->gen_vec = VecOf<T>::n;
+  r->gen_kernel_v1 = nullptr;
+  if constexpr (sizeof(T) == 8 && ModelDims<MODEL>::p >= 2) {
+    static_assert(ResGenValues<MODEL, T, 1>::n_values == ResGenValues<MODEL, T>::n_values, "same shared-memory values per object");
+    r->gen_kernel_v1 = (const void*)k_resident_gen<MODEL, T, 1>;
+  }
 }
 
 template <int MODEL, class T>

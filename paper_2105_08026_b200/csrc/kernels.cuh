@@ -184,21 +184,49 @@ __device__ __forceinline__ SweepCtx<T> make_ctx(const Params& P, const Iter& it,
 
 // RAM steps 1-3 + population terms + moments for the VEC objects base .. base+VEC-1 held in x, l (updated in
 // place; the caller stores them) and d.  acc = {S, Delta, n_accept, n_nonfinite} of this thread.
+// The draws of ONE object (fp64, p >= 2), for the one-object-per-thread map of k_resident_gen: the accept uniform from its
+// half of the pair's draw 0, its own normals from draws 1 + k -- the same words and values as pair_draws gives that object.
+template <int P, int ZD, class KEY>
+__device__ __forceinline__ void single_draws(const KEY& seed, long long i, uint32_t t, double* z, double* cs, double* sn, double* u) {
+  static_assert(P >= 2 && ZD >= P, "single-object draws exist for p >= 2 (for p = 1 a pair shares one Box-Muller evaluation)");
+  const U4 a = stream(seed, KIND_PLATE, (uint64_t)i >> 1, t, 0u);
+  *u = (i & 1) ? u01(a.z, a.w) : u01(a.x, a.y);
+  const U4 b = stream(seed, KIND_PLATE, (uint64_t)i, t, 1u);
+  const double u1 = u01(b.x, b.y), u2 = u01(b.z, b.w);
+  const double rad = hm_sqrt_fast(-2.0 * hm_log_unit(u1));
+  sincospi(2.0 * u2, sn, cs);
+  z[0] = rad * *cs; z[1] = rad * *sn;
+#pragma unroll
+  for (int k = 1; 2 * k < P; ++k) {
+    const U4 b2 = stream(seed, KIND_PLATE, (uint64_t)i, t, 1u + (uint32_t)k);
+    const double v1 = u01(b2.x, b2.y), v2 = u01(b2.z, b2.w);
+    const double rad2 = hm_sqrt_fast(-2.0 * hm_log_unit(v1));
+    double s2_, c2_;
+    sincospi(2.0 * v2, &s2_, &c2_);
+    z[2 * k] = rad2 * c2_;
+    if (2 * k + 1 < P) z[2 * k + 1] = rad2 * s2_;
+  }
+}
+
 // The plate draws of the VEC objects one thread owns at one step (theta- and chi-independent: a function of
 // (seed, object, t) only, so they can be made ahead of the sweep -- k_persistent stages them in shared memory
 // while the exchange and the theta step are in flight).
-template <int MODEL, class T> struct DrawSet {
-  static constexpr int p = ModelDims<MODEL>::p, VEC = VecOf<T>::n, ZD = p < 2 ? 2 : p;
+template <int MODEL, class T, int VEC_ = VecOf<T>::n> struct DrawSet {
+  static constexpr int p = ModelDims<MODEL>::p, VEC = VEC_, ZD = p < 2 ? 2 : p;
   // values kept per object when staged: the p normals, the unit vector (p = 2 only) and the accept uniform
   static constexpr int NZ = p, NU = (p == 2 ? 2 : 0), NV = VEC * (NZ + NU + 1);
   T zz[VEC][ZD], csv[VEC], snv[VEC], uu[VEC];
   __device__ __forceinline__ void make(const Params& P, const long long base, const uint32_t t) {
     // KEY of the plate streams: the seed (fp64 kernels) or its ready-made round keys (fp32 kernels: philox.cuh; measured
     // -1.4 % on C4, while the fp64 kernels, bound by their fp64 chains, gain nothing or lose to the changed schedule)
+    if constexpr (VEC == 1) {                 // one object per thread (k_resident_gen, small p >= 2 populations in fp64)
+      single_draws<p, ZD>((uint64_t)P.tail.seed, P.obj_offset + base, t, zz[0], &csv[0], &snv[0], &uu[0]);
+    } else {
 #pragma unroll
-    for (int v = 0; v < VEC; v += 2) {
-      if constexpr (sizeof(T) == 4) pair_draws<p, ZD>(P.rk, P.obj_offset + base + v, t, &zz[v], &csv[v], &snv[v], &uu[v]);
-      else pair_draws<p, ZD>((uint64_t)P.tail.seed, P.obj_offset + base + v, t, &zz[v], &csv[v], &snv[v], &uu[v]);
+      for (int v = 0; v < VEC; v += 2) {
+        if constexpr (sizeof(T) == 4) pair_draws<p, ZD>(P.rk, P.obj_offset + base + v, t, &zz[v], &csv[v], &snv[v], &uu[v]);
+        else pair_draws<p, ZD>((uint64_t)P.tail.seed, P.obj_offset + base + v, t, &zz[v], &csv[v], &snv[v], &uu[v]);
+      }
     }
   }
   // staged layout: value q of thread-slot j at st[q * stride + j] (unit stride across a warp: conflict-free)
@@ -236,16 +264,16 @@ struct LateKp {
   int* wait;             // != 0: sync on BAR_THETAP (n threads) before the first use, then cleared
   int n;
 };
-template <int MODEL, class T, bool TAP, bool HOLD = false, bool LATE = false>
+template <int MODEL, class T, bool TAP, bool HOLD = false, bool LATE = false, int VEC_ = VecOf<T>::n>
 __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c, const long long base,
-                                           T (*x)[VecOf<T>::n], T (*l)[VecOf<T>::n], const T (*d)[VecOf<T>::n], double* sum,
-                                           const DrawSet<MODEL, T>* staged = nullptr, const LateKp* late = nullptr) {
+                                           T (*x)[VEC_], T (*l)[VEC_], const T (*d)[VEC_], double* sum,
+                                           const DrawSet<MODEL, T, VEC_>* staged = nullptr, const LateKp* late = nullptr) {
   constexpr int p = ModelDims<MODEL>::p, ntri = p * (p + 1) / 2, ncols = ModelDims<MODEL>::ncols;
-  constexpr int VEC = VecOf<T>::n;
-  DrawSet<MODEL, T> ds_;
+  constexpr int VEC = VEC_;
+  DrawSet<MODEL, T, VEC_> ds_;
   if (!staged) ds_.make(P, base, c.t);
-  const DrawSet<MODEL, T>& ds = staged ? *staged : ds_;
-  const T (*zz)[DrawSet<MODEL, T>::ZD] = ds.zz;
+  const DrawSet<MODEL, T, VEC_>& ds = staged ? *staged : ds_;
+  const T (*zz)[DrawSet<MODEL, T, VEC_>::ZD] = ds.zz;
   const T* csv = ds.csv; const T* snv = ds.snv; const T* uu = ds.uu;
 #pragma unroll
   for (int v = 0; v < VEC; ++v) {
@@ -749,6 +777,9 @@ __global__ void __launch_bounds__(SWEEP + DT_TAIL, 1) k_persistent_dt(const Para
       if (k > 0) bar_sync(BAR_THETA, THREADS);               // the decision of iteration t - 1 is taken: kc, eta, moment count
       const SweepCtx<T> c = make_ctx<T>(P, it, t0 + k);      // (its kp is not used: LateKp)
       int wait = k > 0 ? 1 : 0;
+      // the late wait inside update_vec is a block barrier and needs the warp converged there: a warp whose lanes do not ALL
+      // own a first-step object (the ragged end of a small population) waits up front instead -- warp-uniform either way
+      if (wait && !__all_sync(0xffffffffu, first < N)) { bar_sync(BAR_THETAP, THREADS); wait = 0; }
       const LateKp late{&it.kp, &wait, THREADS};
       double acc[4] = {0.0, 0.0, 0.0, 0.0};
       long long base = first;
@@ -762,7 +793,7 @@ __global__ void __launch_bounds__(SWEEP + DT_TAIL, 1) k_persistent_dt(const Para
         if (prefetch) prefetch_step<MODEL, T>(P, base + stride < N ? base + stride : first);
         sweep_step<MODEL, T, false, false, true>(P, c, base, acc, nullptr, &late);
       }
-      if (wait) bar_sync(BAR_THETAP, THREADS);               // a thread without objects still takes part in the barrier
+      if (wait) bar_sync(BAR_THETAP, THREADS);               // (not reached with wait set: kept as a guard)
       nacc += acc[2]; nnan += acc[3];
       double v = acc[1];
 #pragma unroll

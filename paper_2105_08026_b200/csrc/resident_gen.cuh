@@ -5,7 +5,8 @@
 // Same idea as k_resident: a population that fits in shared memory stays there for the whole launch (chi, L, data columns:
 // HBM / L2 are touched at launch start and end only), the theta-independent plate draws of iteration t + 1 are made while
 // the exchange and the theta step of iteration t are in flight, and 4 dedicated warps run the exchange and the theta tail.
-// The per-object arithmetic is update_vec itself (kernels.cuh), fed from shared memory and from draws staged there, so the
+// The per-object arithmetic is update_vec itself (kernels.cuh), fed from shared memory and from draws staged there (it starts at
+// the theta DECISION and reads theta' late, like k_persistent_dt), so the
 // chain is the streaming kernels' to the last bit of every object; only the order in which block partials are added differs
 // (fixed, so still deterministic).  The running chi moments stay in global memory (they are touched once per iteration).
 #pragma once
@@ -14,18 +15,33 @@
 namespace hm {
 
 // shared-memory values of T per object: the state and data columns plus the staged draws of one iteration
-template <int MODEL, class T> struct ResGenValues {
+template <int MODEL, class T, int VEC_ = VecOf<T>::n> struct ResGenValues {
   static constexpr int p = ModelDims<MODEL>::p, ntri = p * (p + 1) / 2, ncols = ModelDims<MODEL>::ncols;
-  static constexpr int VEC = VecOf<T>::n, NV = DrawSet<MODEL, T>::NV;
+  static constexpr int VEC = VEC_, NV = DrawSet<MODEL, T, VEC_>::NV;
   static constexpr int n_state = p + ntri + ncols;
   static constexpr int n_values = n_state + NV / VEC;
 };
 
-template <int MODEL, class T>
+// one group of VEC adjacent objects of a column: a 16-byte access for the full vector, a scalar one for VEC = 1
+template <class T, int VEC>
+__device__ __forceinline__ void rg_load(const T* q, T* out, bool ro) {
+  if constexpr (VEC == VecOf<T>::n) ld_vec<T>(q, out, ro);
+  else { static_assert(VEC == 1, "VEC is 1 or a full 16-byte vector"); out[0] = ro ? __ldg(q) : *q; }
+}
+template <class T, int VEC>
+__device__ __forceinline__ void rg_store(T* q, const T* v) {
+  if constexpr (VEC == VecOf<T>::n) st_vec(q, v);
+  else *q = v[0];
+}
+
+// VEC_: objects per thread group.  The full 16-byte vector by default; 1 for populations of at most one object per sweep
+// thread (N <= blocks x 256: C6), where an object PAIR per thread would leave half the sweep warps idle and every busy
+// thread with twice the serial work (C6: update ~6,000 + draws ~3,600 cycles per iteration on 4 of 8 warps).
+template <int MODEL, class T, int VEC_ = VecOf<T>::n>
 __global__ void __launch_bounds__(RG_THREADS, 1) k_resident_gen(const Params P, const long long n_iter, const unsigned epoch0,
                                                                 const int R, const int OB) {
-  using V = ResGenValues<MODEL, T>;
-  using DS = DrawSet<MODEL, T>;
+  using V = ResGenValues<MODEL, T, VEC_>;
+  using DS = DrawSet<MODEL, T, VEC_>;
   constexpr int p = V::p, ntri = V::ntri, ncols = V::ncols, VEC = V::VEC, NV = V::NV;
   extern __shared__ __align__(16) unsigned char sm_raw[];
   T* const sm = reinterpret_cast<T*>(sm_raw);
@@ -59,19 +75,19 @@ __global__ void __launch_bounds__(RG_THREADS, 1) k_resident_gen(const Params P, 
       T tmp[VEC];
 #pragma unroll
       for (int j = 0; j < p; ++j) {
-        ld_vec<T>(chi + j * Npad + base, tmp, false);
+        rg_load<T, VEC>(chi + j * Npad + base, tmp, false);
 #pragma unroll
         for (int v = 0; v < VEC; ++v) HM_GAT(j, g * VEC + v) = tmp[v];
       }
 #pragma unroll
       for (int k = 0; k < ntri; ++k) {
-        ld_vec<T>(Lm + k * Npad + base, tmp, false);
+        rg_load<T, VEC>(Lm + k * Npad + base, tmp, false);
 #pragma unroll
         for (int v = 0; v < VEC; ++v) HM_GAT(p + k, g * VEC + v) = tmp[v];
       }
 #pragma unroll
       for (int c = 0; c < ncols; ++c) {
-        ld_vec<T>(dat + c * Npad + base, tmp, true);
+        rg_load<T, VEC>(dat + c * Npad + base, tmp, true);
 #pragma unroll
         for (int v = 0; v < VEC; ++v) HM_GAT(p + ntri + c, g * VEC + v) = tmp[v];
       }
@@ -86,12 +102,21 @@ __global__ void __launch_bounds__(RG_THREADS, 1) k_resident_gen(const Params P, 
   if (!is_tail) {
     double nacc = 0.0, nnan = 0.0;
     for (long long k = 0; k < n_iter; ++k) {
-      if (k > 0) bar_sync(BAR_THETAP, RG_THREADS);            // the tail of iteration t - 1 is done: `it` holds iteration t
-      const SweepCtx<T> c = make_ctx<T>(P, it);
+      // the update starts as soon as the DECISION of iteration t - 1 is taken (theta_t's constants, eta, the moment count
+      // are final then); theta'_t and its constants, which the tail warps are still deriving (~3,500 cycles), are needed only
+      // by the population term at the end of the first object's update, which waits for them once (LateKp)
+      if (k > 0) bar_sync(BAR_THETA, RG_THREADS);
+      const SweepCtx<T> c = make_ctx<T>(P, it, t0 + k);
+      int wait = k > 0 ? 1 : 0;
+      const LateKp late{&it.kp, &wait, RG_THREADS};
       double acc[4] = {0.0, 0.0, 0.0, 0.0};
       for (int g = 0; g < ngroups; ++g) {
-        const long long base = HM_GOBJ(g);
-        if (base >= obj_end) break;
+        // The one-off wait for theta' sits inside update_vec and is a block barrier: a warp must reach it CONVERGED.  So the
+        // loop runs while ANY lane of the warp owns group g, and a lane that does not runs the update in lockstep on a
+        // non-live dummy (base beyond N: nothing accumulated or stored; every access stays in its own shared-memory slots).
+        const bool mine = HM_GOBJ(g) < obj_end;
+        if (!__any_sync(0xffffffffu, mine)) break;
+        const long long base = mine ? HM_GOBJ(g) : Npad + VEC;
         T x[p][VEC], l[ntri][VEC], d[ncols][VEC];
 #pragma unroll
         for (int v = 0; v < VEC; ++v) {
@@ -104,7 +129,8 @@ __global__ void __launch_bounds__(RG_THREADS, 1) k_resident_gen(const Params P, 
         }
         DS ds;
         ds.get(dr_my + (size_t)g * NV * RG_S, RG_S);
-        update_vec<MODEL, T, false>(P, c, base, x, l, d, acc, &ds);
+        update_vec<MODEL, T, false, false, true, VEC>(P, c, base, x, l, d, acc, &ds, &late);
+        if (mine) {
 #pragma unroll
         for (int v = 0; v < VEC; ++v) {
 #pragma unroll
@@ -112,7 +138,9 @@ __global__ void __launch_bounds__(RG_THREADS, 1) k_resident_gen(const Params P, 
 #pragma unroll
           for (int q = 0; q < ntri; ++q) HM_GAT(p + q, g * VEC + v) = l[q][v];
         }
+        }
       }
+      if (wait) bar_sync(BAR_THETAP, RG_THREADS);             // a WARP without objects still takes part in the barrier (warp-uniform)
       nacc += acc[2]; nnan += acc[3];
       double v = acc[1];
 #pragma unroll
@@ -131,7 +159,8 @@ __global__ void __launch_bounds__(RG_THREADS, 1) k_resident_gen(const Params P, 
         }
       }
     }
-    bar_sync(BAR_THETAP, RG_THREADS);                         // the last tail has finished
+    bar_sync(BAR_THETA, RG_THREADS);                          // the last tail has finished
+    bar_sync(BAR_THETAP, RG_THREADS);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
       nacc += __shfl_down_sync(0xffffffffu, nacc, o);
@@ -149,13 +178,13 @@ __global__ void __launch_bounds__(RG_THREADS, 1) k_resident_gen(const Params P, 
       for (int j = 0; j < p; ++j) {
 #pragma unroll
         for (int v = 0; v < VEC; ++v) tmp[v] = HM_GAT(j, g * VEC + v);
-        st_vec(chi + j * Npad + base, tmp);
+        rg_store<T, VEC>(chi + j * Npad + base, tmp);
       }
 #pragma unroll
       for (int q = 0; q < ntri; ++q) {
 #pragma unroll
         for (int v = 0; v < VEC; ++v) tmp[v] = HM_GAT(p + q, g * VEC + v);
-        st_vec(Lm + q * Npad + base, tmp);
+        rg_store<T, VEC>(Lm + q * Npad + base, tmp);
       }
     }
   } else {
@@ -174,9 +203,10 @@ __global__ void __launch_bounds__(RG_THREADS, 1) k_resident_gen(const Params P, 
         mbox_collect<1>(mb + (size_t)blockIdx.x * mbox_reader_words(G), G, epoch, t1);
         tot[1] = t1[0];
       }
-      tail_block<MODEL>(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, tw, SyncNamed<BAR_TAIL, RG_TW * 32>());
+      tail_block<MODEL>(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, tw, SyncNamed<BAR_TAIL, RG_TW * 32>(),
+                        ArriveNamed<BAR_THETA, RG_THREADS>());   // theta_{t+1} is signalled after the decision phase ...
       __threadfence_block();
-      bar_arrive(BAR_THETAP, RG_THREADS);
+      bar_arrive(BAR_THETAP, RG_THREADS);                     // ... theta'_{t+1} and its constants when the tail is done
     }
   }
 #undef HM_GAT

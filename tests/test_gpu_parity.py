@@ -634,3 +634,23 @@ def test_trace_and_moment_counts_across_split_runs_crossing_burn_in(mode):
     assert after["t"] == before["t"] and np.array_equal(after["chi"], before["chi"])
     gpu.run(2, burn, thin, sync=True)                    # still room for iterations that add no row (t = 103 < 104)
     assert gpu.get_stats()["trace_rows"] == rows_total
+
+
+@pytest.mark.parametrize("n", [150_529, 200_001])
+def test_dedicated_tail_kernel_at_its_smallest_populations(n):
+    """k_persistent_dt (M2, default block size, streaming forced) at the smallest population cudahm_create gives it (below
+    150,529 objects -- fewer than 148 blocks of 512 x 2 -- the default block is 256 threads and the plain kernel runs) and with a ragged second step: the one-off wait
+    for theta' is a block barrier inside the update and must be reached warp-uniformly.  Free-running against the oracle."""
+    iters, burn, thin = 30, 10, 5
+    orc, gpu, _ = make_pair(B.M_BINORMAL2D, n, seed=47, astar=0.234, keep_moments=True, max_trace_rows=(iters - burn) // thin,
+                            flags=B.FLAG_STREAMING_ONLY)
+    assert gpu.get_stats()["dedicated_tail"] == 1
+    _, small, _ = make_pair(B.M_BINORMAL2D, n - 2, seed=47, astar=0.234, want_oracle=False, flags=B.FLAG_STREAMING_ONLY)
+    assert small.get_stats()["dedicated_tail"] == (1 if n - 2 >= 150_529 else 0)
+    orc.run(iters, burn, thin)
+    gpu.run(iters, burn, thin, sync=True)
+    so, sg = orc.get_state(), gpu.get_state()
+    np.testing.assert_allclose(gpu.get_theta_trace(), orc.get_theta_trace(), rtol=1e-8, atol=1e-8)
+    np.testing.assert_allclose(sg["chi"], so["chi"], rtol=1e-9, atol=1e-9)
+    np.testing.assert_allclose(sg["L"], so["L"], rtol=1e-9, atol=1e-12)
+    assert gpu.get_stats()["chi_accepts"] == orc.get_stats()["chi_accepts"]
