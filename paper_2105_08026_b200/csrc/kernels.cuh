@@ -799,7 +799,7 @@ __global__ void __launch_bounds__(SWEEP + DT_TAIL, 1) k_persistent_dt(const Para
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
       if (lane == 0) red[k & 1][warp] = v;
-      __threadfence_block();
+      // (no fence needed: when the barrier completes, bar.arrive has ordered this thread's prior shared-memory writes for its participants)
       bar_arrive(BAR_PARTIALS, THREADS);
       if (k + 1 < n_iter) stage_own((uint32_t)(t0 + k + 1));
     }
@@ -832,7 +832,7 @@ __global__ void __launch_bounds__(SWEEP + DT_TAIL, 1) k_persistent_dt(const Para
       }
       tail_block<MODEL>(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, tw, SyncNamed<BAR_TAIL, DT_TAIL>(),
                         ArriveNamed<BAR_THETA, THREADS>());
-      __threadfence_block();
+      // (no fence needed: when the barrier completes, bar.arrive has ordered this thread's prior shared-memory writes for its participants)
       bar_arrive(BAR_THETAP, THREADS);
     }
   }

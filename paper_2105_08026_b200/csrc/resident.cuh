@@ -233,7 +233,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) v[0] += __shfl_down_sync(0xffffffffu, v[0], o);
       if (lane == 0) red[k & 1][warp][0] = v[0];
-      __threadfence_block();
+      // (no fence needed: when the barrier completes, bar.arrive has ordered this thread's prior shared-memory writes for its participants)
       bar_arrive(BAR_PARTIALS, RES_THREADS);                 // hand the partials to the tail warps, do not wait
       if (k + 1 < n_iter) front((uint32_t)(t + 1));          // overlaps the exchange and the theta step
     }
@@ -315,7 +315,7 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
       }
       tail_block<MODEL>(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, tw, SyncNamed<BAR_TAIL, RES_TW * 32>(),
                  ArriveNamed<BAR_THETA, RES_THREADS>());      // theta_{t+1} is signalled after the decision phase ...
-      __threadfence_block();
+      // (no fence needed: when the barrier completes, bar.arrive has ordered this thread's prior shared-memory writes for its participants)
       bar_arrive(BAR_THETAP, RES_THREADS);                   // ... theta'_{t+1} and its constants when the tail is done
       if constexpr (!SEL_SWEEP) selection_full();            // M1: for the NEXT decision; off the critical path
     }

@@ -146,7 +146,7 @@ __global__ void __launch_bounds__(RG_THREADS, 1) k_resident_gen(const Params P, 
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
       if (lane == 0) red[k & 1][warp] = v;
-      __threadfence_block();
+      // (no fence needed: when the barrier completes, bar.arrive has ordered this thread's prior shared-memory writes for its participants)
       bar_arrive(BAR_PARTIALS, RG_THREADS);                   // hand the partials to the tail warps, do not wait
       if (k + 1 < n_iter) {                                   // the draws of iteration t + 1: overlaps the exchange and the theta step
         const uint32_t tn = (uint32_t)(t0 + k + 1);
@@ -205,7 +205,7 @@ __global__ void __launch_bounds__(RG_THREADS, 1) k_resident_gen(const Params P, 
       }
       tail_block<MODEL>(it, P.tail, tot, blockIdx.x == 0 ? P.trace : nullptr, tw, SyncNamed<BAR_TAIL, RG_TW * 32>(),
                         ArriveNamed<BAR_THETA, RG_THREADS>());   // theta_{t+1} is signalled after the decision phase ...
-      __threadfence_block();
+      // (no fence needed: when the barrier completes, bar.arrive has ordered this thread's prior shared-memory writes for its participants)
       bar_arrive(BAR_THETAP, RG_THREADS);                     // ... theta'_{t+1} and its constants when the tail is done
     }
   }

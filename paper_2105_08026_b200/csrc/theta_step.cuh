@@ -241,7 +241,7 @@ struct NoSignal { __device__ __forceinline__ void operator()() const {} };
 template <int ID, int THREADS>
 struct ArriveNamed {
   __device__ __forceinline__ void operator()() const {
-    __threadfence_block();
+    // (no fence needed: when the barrier completes, bar.arrive has ordered this thread's prior shared-memory writes for its participants)
     asm volatile("bar.arrive %0, %1;" ::"n"(ID), "n"(THREADS) : "memory");
   }
 };
