@@ -176,9 +176,9 @@ __device__ __forceinline__ SweepCtx<T> make_ctx(const Params& P, const Iter& it,
   c.kT = narrow<T>(c.kc);
 #pragma unroll
   for (int j = 0; j < MC_N; ++j) c.mcT[j] = (T)P.mc[j];
-  c.eta = (T)it.dr[t_it % 3].eta; c.astar = (T)P.astar_chi;
+  c.eta = (T)it.dr[slot3(t_it)].eta; c.astar = (T)P.astar_chi;
   c.do_mom = P.tail.keep_moments && t_it > P.tail.burn_in;
-  c.inv_k = 1.0 / (double)(it.mom_count + 1);
+  c.inv_k = it.inv_k;
   return c;
 }
 

@@ -146,9 +146,9 @@ __global__ void __launch_bounds__(RES_THREADS, 1) k_resident(const Params P, con
       // back, part 1 (needs theta_t only): targets, accept, RAM update, new chi, moments
       const ThetaK kc = it.kc;
       const KT<T> kT = narrow<T>(kc);
-      const T eta = (T)it.dr[t % 3].eta;
+      const T eta = (T)it.dr[slot3(t)].eta;
       const bool do_mom = keep_mom && t > P.tail.burn_in;
-      const double inv_k = 1.0 / (double)(it.mom_count + 1);
+      const double inv_k = it.inv_k;
       // RES_IL slots at a time in straight-line code: the back sits on the critical path of the iteration (the
       // exchange cannot start before it ends) and one slot is a single dependent chain of fp64 operations, so with
       // 4 warps per scheduler it is latency-bound; independent slots interleave.  A slot past nlive repeats the

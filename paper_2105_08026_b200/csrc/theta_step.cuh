@@ -36,6 +36,7 @@ struct Iter {
   ThetaK kc, kp;                      // theta-derived constants at theta / theta'
   double T_cur, lp_cur, lp_prop;      // theta-only term and log prior at theta; log prior at theta'
   double lp_prop_next;                // staging slot of the block-parallel tail
+  double inv_k;                       // 1 / (mom_count + 1) of the PREPARED iteration (Welford step of the running chi moments)
   // taps of the last decision (debug_step / host mode read them)
   double S, Delta, T_prop, log_r, alpha_theta, u_theta, T_cur_used, lp_cur_used, tap_thetaP[MAXD];
   long long t;                        // the PREPARED iteration (1-based): t-1 iterations are complete
@@ -70,6 +71,9 @@ HM_HD double log_prior_full(const TailCfg& c, const double* th, int model) {
   return s;
 }
 HM_HD double log_prior_full(const TailCfg& c, const double* th) { return log_prior_full(c, th, c.model); }
+
+// ring slot of iteration t (t < 2^32 is checked by cudahm_run): a 32-bit modulo by a constant, not the 64-bit software routine
+HM_HD int slot3(long long t) { return (int)((unsigned)t % 3u); }
 
 HM_HD int tri(int r, int c) { return r * (r + 1) / 2 + c; }
 HM_HD int tri_row(int e) { int r = 0; while ((r + 1) * (r + 2) / 2 <= e) ++r; return r; }
@@ -127,9 +131,10 @@ HM_HD double propose_entry(const Iter& it, const Draws& d, int r) {
 // drawn BEFORE the sweep so one pass evaluates f at theta and theta' (reading R7).
 HM_HD void prepare_iteration(Iter& it, const TailCfg& c, long long t) {
   it.t = t;
-  Draws& d = it.dr[t % 3];
+  Draws& d = it.dr[slot3(t)];
   make_draws(d, c, t);
-  make_draws(it.dr[(t + 1) % 3], c, t + 1);
+  make_draws(it.dr[slot3(t + 1)], c, t + 1);
+  it.inv_k = 1.0 / (double)(it.mom_count + 1);
   if (!c.freeze_theta) {
     for (int r = 0; r < c.dtheta; ++r) it.thetaP[r] = propose_entry(it, d, r);
     for (int i = 0; i < c.dtheta; ++i)
@@ -178,6 +183,7 @@ HM_HD void decide_counters(Iter& it, double S, double Delta, double nacc, double
 // ... and the moments count / trace row of iteration it.t (independent of the decision)
 HM_HD void decide_schedule(Iter& it, const TailCfg& c) {
   if (c.keep_moments && it.t > c.burn_in) it.mom_count += 1;
+  it.inv_k = 1.0 / (double)(it.mom_count + 1);      // for the sweep of iteration t + 1: one division here instead of one per thread
   it.trace_write = 0;
   if (it.t > c.burn_in && ((it.t - c.burn_in) % c.thin) == 0 && it.trace_rows < c.max_trace_rows) {
     it.trace_rows += 1;
@@ -188,7 +194,7 @@ HM_HD void decide_schedule(Iter& it, const TailCfg& c) {
 // (a) serial: the theta decision of iteration it.t from the reduced sweep totals {S, Delta, Tq, nacc, nnan}.
 // Sets it.trace_write when the (new) theta has to be appended to the thinned trace at row it.trace_rows - 1.
 HM_HD void tail_decide(Iter& it, const TailCfg& c, const double* tot) {
-  const Draws& d = it.dr[it.t % 3];
+  const Draws& d = it.dr[slot3(it.t)];
   it.accepted_theta = 0;
   it.T_prop = 0.0; it.log_r = 0.0; it.alpha_theta = 0.0; it.u_theta = 0.0;
   it.T_cur_used = it.T_cur; it.lp_cur_used = it.lp_cur;
@@ -258,7 +264,7 @@ __device__ __forceinline__ void tail_block(Iter& it, const TailCfg& c, const dou
   const int model = MODEL >= 0 ? MODEL : c.model;
   const int dt = c.dtheta, nt = dt * (dt + 1) / 2;
   const long long t = it.t;
-  const int r0 = (int)(t % 3), r1 = r0 == 2 ? 0 : r0 + 1, r2 = r1 == 2 ? 0 : r1 + 1;
+  const int r0 = slot3(t), r1 = r0 == 2 ? 0 : r0 + 1, r2 = r1 == 2 ? 0 : r1 + 1;
   const Draws& d0 = it.dr[r0];
   const Draws& d1 = it.dr[r1];
   Draws& d2 = it.dr[r2];
