@@ -136,7 +136,8 @@ typedef struct {
   int32_t stage_steps;           /* streaming persistent kernel: steps of plate draws staged ahead per thread */
   int32_t l2_prefetch;           /* ... 1: it prefetches the next step's columns into L2 (0 for the on-chip kernel) */
   int32_t dedicated_tail;        /* 1: the streaming kernel with dedicated tail warps (k_persistent_dt) runs             */
-  int32_t pad_;
+  int32_t graph_launches;        /* persistent-kernel launches submitted through the handle's one-node CUDA graph (every
+                                    cudahm_run in THETA_DEVICE_TAIL mode after the handle's first; 0 = direct launches only) */
 } cudahm_stats;
 
 /* Per-iteration taps of cudahm_debug_step; HOST pointers, each may be NULL.  Values are widened to double. */
@@ -201,7 +202,11 @@ int cudahm_set_counters(cudahm_sampler* s, const uint32_t* in);
 
 /* Run n_iter more Gibbs iterations (resumable: continues from the current iteration index t).  Moments are
  * accumulated for t > burn_in, the trace takes theta whenever t > burn_in and (t - burn_in) % thin == 0.
- * CUDAHM_E_INVALID if the trace would overflow max_trace_rows (max_trace_rows == 0 keeps no trace at all). */
+ * CUDAHM_E_INVALID if the trace would overflow max_trace_rows (max_trace_rows == 0 keeps no trace at all).
+ * Asynchronous: the work is queued on the handle's stream, nothing is read back.  May be called with any device current
+ * (the device that was current at cudahm_create is made current for the duration of the call); every other call expects
+ * the handle's device to be current.  In THETA_DEVICE_TAIL mode a handle's first run is submitted as a direct cooperative
+ * launch, later ones through a one-node CUDA graph whose parameters are updated in place (cudahm_stats.graph_launches). */
 int cudahm_run(cudahm_sampler* s, int64_t n_iter, int64_t burn_in, int32_t thin);
 
 /* Sharded populations: objects are conditionally independent given theta (Eq. 2.4), so a

@@ -57,7 +57,7 @@ class Stats(C.Structure):
                                          "theta_proposals", "nonfinite", "moment_samples", "trace_rows",
                                          "gpu_launches")] + \
                [("grid_blocks", C.c_int32), ("block_threads", C.c_int32), ("last_run_ms", C.c_double),
-                ("stage_steps", C.c_int32), ("l2_prefetch", C.c_int32), ("dedicated_tail", C.c_int32), ("pad_", C.c_int32)]
+                ("stage_steps", C.c_int32), ("l2_prefetch", C.c_int32), ("dedicated_tail", C.c_int32), ("graph_launches", C.c_int32)]
 
 
 class Taps(C.Structure):
@@ -192,6 +192,7 @@ class Sampler:
                                         C.c_void_p(self.stream.cuda_stream), C.byref(self._h))
         if rc:
             raise CudahmError(rc, self.lib.cudahm_last_error(None).decode())
+        self._run = self.lib.cudahm_run
 
     def _ck(self, rc):
         if rc:
@@ -268,10 +269,13 @@ class Sampler:
             self._ck(self.lib.cudahm_set_counters(self._h, C.c_void_p(c.ctypes.data)))
 
     def run(self, n_iter, burn_in=0, thin=1, sync=False):
-        with self._dev():
-            self._ck(self.lib.cudahm_run(self._h, n_iter, burn_in, thin))
-            if sync:
-                self._ck(self.lib.cudahm_sync(self._h))
+        # no torch device context here: cudahm_run makes the handle's device current itself, and the context manager's
+        # two device switches are 3 us of host time between the caller's stream position and the launch
+        rc = self._run(self._h, n_iter, burn_in, thin)
+        if rc:
+            self._ck(rc)
+        if sync:
+            self.sync()
 
     def sync(self):
         with self._dev():

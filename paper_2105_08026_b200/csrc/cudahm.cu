@@ -88,7 +88,10 @@ struct cudahm_sampler {
   double h_lp_prop_before = 0.0;    // log prior at theta' of the iteration debug_step is about to decide
   // CUDA-graph cache (THETA_GRAPH)
   cudaGraphExec_t pg_exec = nullptr;          // one-node graph of the persistent kernel (launch_persistent)
+  cudaGraph_t pg_graph = nullptr;             // ... the graph pg_node lives in: kept as long as pg_exec (the in-place update names the node)
   cudaGraphNode_t pg_node = nullptr;
+  int pg_graph_launches = 0;                  // launches that went out through pg_exec (cudahm_stats.graph_launches)
+  int device = 0;                             // the device that was current at cudahm_create (owns workspace and stream)
   const void* pg_fn = nullptr;
   bool pg_broken = false;
   long long pg_launches = 0;
@@ -112,6 +115,12 @@ int fail(cudahm_sampler* s, int code, const char* fmt, ...) {
 
 // the captured k_sweep / k_tail nodes of THETA_GRAPH hold Params BY VALUE (model constants, pointers, prior): anything
 // that changes them, or rewinds the chain, drops the cached executable graph so the next run captures afresh
+void drop_persistent_graph(cudahm_sampler* s) {
+  if (s->pg_exec) { cudaGraphExecDestroy(s->pg_exec); s->pg_exec = nullptr; }
+  if (s->pg_graph) { cudaGraphDestroy(s->pg_graph); s->pg_graph = nullptr; }
+  s->pg_node = nullptr; s->pg_fn = nullptr;
+}
+
 void invalidate_graph(cudahm_sampler* s) {
   if (s->gexec) { cudaGraphExecDestroy(s->gexec); s->gexec = nullptr; }
   s->g_burn = -1; s->g_thin = -1; s->g_iters = 0;
@@ -250,7 +259,7 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
   if (!coop) return fail(nullptr, CUDAHM_E_CUDA, "device does not support cooperative launches");
 
   cudahm_sampler* s = new cudahm_sampler();
-  s->cfg = *cfg; s->lay = lay; s->ks = ks; s->stream = (cudaStream_t)cuda_stream; s->ws = (char*)dev_workspace;
+  s->cfg = *cfg; s->lay = lay; s->ks = ks; s->stream = (cudaStream_t)cuda_stream; s->ws = (char*)dev_workspace; s->device = dev;
   s->p = p; s->dtheta = dt; s->ncols = nc; s->nconsts = nk; s->ntri = p * (p + 1) / 2; s->ntri_theta = dt * (dt + 1) / 2;
   s->tsize = cfg->precision == CUDAHM_F64 ? 8 : 4;
   s->vec = cfg->precision == CUDAHM_F64 ? 2 : 4;
@@ -404,7 +413,7 @@ extern "C" void cudahm_destroy(cudahm_sampler* s) {
   if (!s) return;
   cudaStreamSynchronize(s->stream);
   if (s->gexec) cudaGraphExecDestroy(s->gexec);
-  if (s->pg_exec) cudaGraphExecDestroy(s->pg_exec);
+  drop_persistent_graph(s);
   if (s->h_iter) cudaFreeHost(s->h_iter);
   if (s->h_totals) cudaFreeHost(s->h_totals);
   if (s->ev0) cudaEventDestroy(s->ev0);
@@ -648,8 +657,10 @@ extern "C" int cudahm_set_init(cudahm_sampler* s, const void* chi0, int chi0_on_
 namespace {
 
 // One cooperative launch of a persistent kernel, submitted as a one-node CUDA graph whose kernel parameters are updated in
-// place: measured 1.5-2 us less launch latency per cudahm_run than cudaLaunchCooperativeKernel.  Falls
-// back to the direct launch for good if any graph call fails.
+// place: 2.3 us of host time per call (update 0.7 + launch 1.6) against 7.0 us for cudaLaunchCooperativeKernel, and on an
+// idle stream the GPU waits for exactly that time.  The graph is kept as long as its executable:
+// the in-place update names the NODE, which dies with the graph.  Falls back to the direct launch for good if any graph
+// call fails; cudahm_stats.graph_launches tells which path a handle is on.
 cudaError_t launch_persistent(cudahm_sampler* s, const void* fn, int grid, int block, void** args, size_t smem) {
   // the first launch of a handle goes out directly: building the graph costs ~100 us of host time, which a caller who runs
   // the whole chain in one cudahm_run should not pay before its kernel starts
@@ -659,24 +670,22 @@ cudaError_t launch_persistent(cudahm_sampler* s, const void* fn, int grid, int b
     kp.kernelParams = args; kp.extra = nullptr;
     cudaError_t e = cudaSuccess;
     if (!s->pg_exec || s->pg_fn != fn) {
-      if (s->pg_exec) { cudaGraphExecDestroy(s->pg_exec); s->pg_exec = nullptr; }
-      cudaGraph_t g = nullptr;
-      e = cudaGraphCreate(&g, 0);
-      if (e == cudaSuccess) e = cudaGraphAddKernelNode(&s->pg_node, g, nullptr, 0, &kp);
+      drop_persistent_graph(s);
+      e = cudaGraphCreate(&s->pg_graph, 0);
+      if (e == cudaSuccess) e = cudaGraphAddKernelNode(&s->pg_node, s->pg_graph, nullptr, 0, &kp);
       cudaKernelNodeAttrValue av{};
       av.cooperative = 1;
       if (e == cudaSuccess) e = cudaGraphKernelNodeSetAttribute(s->pg_node, cudaKernelNodeAttributeCooperative, &av);
-      if (e == cudaSuccess) e = cudaGraphInstantiate(&s->pg_exec, g, 0);
+      if (e == cudaSuccess) e = cudaGraphInstantiate(&s->pg_exec, s->pg_graph, 0);
       if (e == cudaSuccess) e = cudaGraphExecKernelNodeSetParams(s->pg_exec, s->pg_node, &kp);   // pays the lazy set-up of the update path now
-      if (g) cudaGraphDestroy(g);
       s->pg_fn = fn;
     } else {
       e = cudaGraphExecKernelNodeSetParams(s->pg_exec, s->pg_node, &kp);
     }
     if (e == cudaSuccess) e = cudaGraphLaunch(s->pg_exec, s->stream);
-    if (e == cudaSuccess) return e;
+    if (e == cudaSuccess) { s->pg_graph_launches++; return e; }
     cudaGetLastError();
-    if (s->pg_exec) { cudaGraphExecDestroy(s->pg_exec); s->pg_exec = nullptr; }
+    drop_persistent_graph(s);
     s->pg_broken = true;
   }
   return cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(block), args, smem, s->stream);
@@ -884,6 +893,13 @@ extern "C" int cudahm_run(cudahm_sampler* s, int64_t n_iter, int64_t burn_in, in
                 (long long)s->cfg.max_trace_rows);
   s->P.tail.burn_in = burn_in; s->P.tail.thin = thin;
   if (n_iter == 0) return CUDAHM_OK;
+  // the one call that may be made with any device current (a caller in a loop over handles need not switch): the handle's
+  // device is made current for the duration of the call if it is not already
+  struct DeviceScope {
+    int prev = -1; bool switched = false;
+    explicit DeviceScope(int want) { if (cudaGetDevice(&prev) == cudaSuccess && prev != want) switched = cudaSetDevice(want) == cudaSuccess; }
+    ~DeviceScope() { if (switched) cudaSetDevice(prev); }
+  } scope(s->device);
   const bool time_it = (s->cfg.flags & CUDAHM_FLAG_TIME_RUNS) != 0;
   if (time_it) CU_TRY(s, cudaEventRecord(s->ev0, s->stream));
   int rc;
@@ -1194,6 +1210,7 @@ extern "C" int cudahm_get_stats(cudahm_sampler* s, cudahm_stats* out) {
   out->grid_blocks = s->grid; out->block_threads = s->block; out->gpu_launches = s->launches;
   const bool streaming_tail = s->cfg.theta_mode == CUDAHM_THETA_DEVICE_TAIL && !s->res_kernel && s->tma_stages == 0 && (s->ahead || s->dt);
   out->dedicated_tail = (s->dt && !s->res_kernel) ? 1 : 0;
+  out->graph_launches = s->pg_graph_launches;
   out->stage_steps = streaming_tail ? s->n_stage : 0; out->l2_prefetch = streaming_tail ? s->prefetch : 0;
   if (!s->have_init) return CUDAHM_OK;
   int rc = fetch_iter(s); if (rc) return rc;

@@ -64,6 +64,10 @@ def test_long_chain_is_split_invariant(name, n_over, iters, block):
     if block is not None:
         assert a["stats"]["block_threads"] == block, "the case no longer reaches the kernel variant it names"
     assert a["stats"]["dedicated_tail"] == int(name == "C3" and not n_over)
+    # launch path: a handle's first persistent launch is direct, every later one goes through its one-node
+    # graph with the parameters updated in place -- a graph call that fails makes the handle fall back to direct launches
+    # for good, silently but for this count
+    assert a["stats"]["graph_launches"] == 0 and b["stats"]["graph_launches"] == len(cuts) - 1
     assert a["state"]["t"] == b["state"]["t"] == total
     for key in ("chi", "L", "theta", "L_theta"):
         assert np.isfinite(a["state"][key]).all()
