@@ -249,7 +249,10 @@ int cudahm_debug_step(cudahm_sampler* s, int64_t burn_in, int32_t thin, cudahm_t
 int cudahm_debug_step_noalloc(cudahm_sampler* s, int64_t burn_in, int32_t thin, cudahm_taps* taps);
 size_t cudahm_debug_step_noalloc_bytes(const cudahm_sampler* s);
 
-/* out: row-major n_rows x dtheta host doubles.  out == NULL just reports n_rows. */
+/* Results.  Both calls queue their transfers on the handle's stream behind the runs already submitted and synchronise that
+ * stream once before they return; the row / sample counts come from host-side mirrors (functions of the (t, burn_in, thin)
+ * history), so nothing else is read back.  Host buffers may be pageable or pinned (pinned ones move at PCIe speed).
+ * out: row-major n_rows x dtheta host doubles.  out == NULL just reports n_rows, without synchronising. */
 int cudahm_get_theta_trace(cudahm_sampler* s, double* out, int64_t cap_rows, int64_t* n_rows);
 /* mean, var: p*N host doubles (SoA); var is the sample variance (divisor n_samples - 1). */
 int cudahm_get_chi_moments(cudahm_sampler* s, double* mean, double* var, int64_t cap_objects, int64_t* n_samples);

@@ -1171,12 +1171,14 @@ extern "C" int cudahm_debug_step_noalloc(cudahm_sampler* s, int64_t burn_in, int
 extern "C" int cudahm_get_theta_trace(cudahm_sampler* s, double* out, int64_t cap_rows, int64_t* n_rows) {
   if (!s || !n_rows) return fail(s, CUDAHM_E_INVALID, "get_theta_trace: NULL argument");
   if (!s->have_init) return fail(s, CUDAHM_E_STATE, "get_theta_trace before set_init");
-  if (!out) { *n_rows = s->h_trace_rows; return CUDAHM_OK; }      // the count is mirrored on the host: no synchronisation
-  int rc = fetch_iter(s); if (rc) return rc;
-  const long long rows = s->h_iter->trace_rows;
+  // the count is mirrored on the host (a function of the (t, burn_in, thin) history): the query needs no synchronisation,
+  // and the copy is ONE stream-ordered transfer followed by one synchronise -- no read-back of the iteration record first
+  const long long rows = s->h_trace_rows;
   *n_rows = rows;
+  if (!out) return CUDAHM_OK;
   if (cap_rows < rows) return fail(s, CUDAHM_E_INVALID, "trace has %lld rows, capacity %lld", rows, (long long)cap_rows);
-  if (rows > 0) CU_TRY(s, cudaMemcpy(out, s->P.trace, (size_t)rows * s->dtheta * 8, cudaMemcpyDeviceToHost));
+  if (rows > 0) CU_TRY(s, cudaMemcpyAsync(out, s->P.trace, (size_t)rows * s->dtheta * 8, cudaMemcpyDeviceToHost, s->stream));
+  CU_TRY(s, cudaStreamSynchronize(s->stream));
   return CUDAHM_OK;
 }
 
@@ -1184,8 +1186,9 @@ extern "C" int cudahm_get_chi_moments(cudahm_sampler* s, double* mean, double* v
   if (!s || !n_samples) return fail(s, CUDAHM_E_INVALID, "get_chi_moments: NULL argument");
   if (!s->have_init) return fail(s, CUDAHM_E_STATE, "get_chi_moments before set_init");
   if (!s->cfg.keep_chi_moments) return fail(s, CUDAHM_E_STATE, "keep_chi_moments was not set");
-  int rc = fetch_iter(s); if (rc) return rc;
-  const long long cnt = s->h_iter->mom_count, N = s->P.N, Npad = s->P.Npad;
+  // the sample count is mirrored on the host; the finalising kernel and every transfer are queued on the handle's stream
+  // and synchronised ONCE (with pinned destinations the two arrays move back to back at PCIe speed)
+  const long long cnt = s->h_mom_count, N = s->P.N, Npad = s->P.Npad;
   *n_samples = cnt;
   if (cap_objects < N) return fail(s, CUDAHM_E_INVALID, "moments need room for %lld objects", N);
   double* dvar = (double*)(s->ws + s->lay.mom_var);
@@ -1195,12 +1198,12 @@ extern "C" int cudahm_get_chi_moments(cudahm_sampler* s, double* mean, double* v
     k_finalize_moments<<<(unsigned)((n + 255) / 256), 256, 0, s->stream>>>(s->P.mom_M2, dvar, n, inv);
     s->launches++;
     CU_TRY(s, cudaGetLastError());
-    CU_TRY(s, cudaStreamSynchronize(s->stream));
   }
-  for (int j = 0; j < s->p && N > 0; ++j) {
-    if (mean) CU_TRY(s, cudaMemcpy(mean + (size_t)j * N, s->P.mom_mean + (size_t)j * Npad, (size_t)N * 8, cudaMemcpyDeviceToHost));
-    if (var) CU_TRY(s, cudaMemcpy(var + (size_t)j * N, dvar + (size_t)j * Npad, (size_t)N * 8, cudaMemcpyDeviceToHost));
-  }
+  for (int j = 0; j < s->p && N > 0; ++j)       // the means first: their transfer does not wait for the kernel's result
+    if (mean) CU_TRY(s, cudaMemcpyAsync(mean + (size_t)j * N, s->P.mom_mean + (size_t)j * Npad, (size_t)N * 8, cudaMemcpyDeviceToHost, s->stream));
+  for (int j = 0; j < s->p && N > 0; ++j)
+    if (var) CU_TRY(s, cudaMemcpyAsync(var + (size_t)j * N, dvar + (size_t)j * Npad, (size_t)N * 8, cudaMemcpyDeviceToHost, s->stream));
+  CU_TRY(s, cudaStreamSynchronize(s->stream));
   return CUDAHM_OK;
 }
 
