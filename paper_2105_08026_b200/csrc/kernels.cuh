@@ -254,6 +254,28 @@ template <int MODEL, class T, int VEC_ = VecOf<T>::n> struct DrawSet {
   }
 };
 
+// Running moments of object i's new chi (Welford; PAPER.md:337-341 reports posterior means and standard deviations of the
+// member properties): mean += (x - mean)/k, M2 += (x - mean_old)(x - mean_new), with 1/k from the tail (Iter::inv_k).
+template <int p, class T, int VEC>
+__device__ __forceinline__ void moments_update(const Params& P, const SweepCtx<T>& c, const long long i, const T (*x)[VEC], const int v) {
+#pragma unroll
+  for (int j = 0; j < p; ++j) {
+    const long long q = j * P.Npad + i;
+    const double xv = (double)x[j][v];
+    const double m0 = P.mom_mean[q];
+    const double dl = xv - m0;
+    const double m1 = m0 + dl * c.inv_k;
+    P.mom_mean[q] = m1;
+    P.mom_M2[q] += dl * (xv - m1);
+  }
+}
+// Where the update sits.  Inside the per-object loop the compiler turns `if (do_mom)` into predication, so a run WITHOUT
+// moments still issues the 14 instructions per object and component, predicated off: 9 % of the issue slots of the fp32
+// kernel (ncu, C4), which is issue-bound -- there the update of all of a thread's objects sits behind ONE warp-uniform
+// branch after the loop (C4 60.0 -> 57.2 us, same-box A/B).  The fp64 kernels are latency-bound, the slots are free, and
+// the p = 2 kernel at its 128-register cap spills more with the late placement (C3 21.9 -> 22.25 us): they keep it inside.
+template <class T> struct MomentsAfterLoop { static constexpr bool value = sizeof(T) == 4; };
+
 // HOLD: the variant for frozen members.  An object whose mask byte is 0 takes no RAM step (chi, L and its
 // update count stay bit for bit; its draws are made and discarded, the streams being counter-based) but still contributes
 // a_i, b_i; with a per-object counter eta_n comes from the object's own update count n_i = count + 2.
@@ -372,17 +394,8 @@ __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c
       for (int k = 0; k < ntri; ++k) l[k][v] = ln[k];
       sum[0] += a; sum[1] += b - a;
       sum[2] += acc ? 1.0 : 0.0; sum[3] += (bad && upd) ? 1.0 : 0.0;
-      if (c.do_mom) {
-#pragma unroll
-        for (int j = 0; j < p; ++j) {
-          const long long q = j * P.Npad + i;
-          const double xv = (double)x[j][v];
-          const double m0 = P.mom_mean[q];
-          const double dl = xv - m0;
-          const double m1 = m0 + dl * c.inv_k;
-          P.mom_mean[q] = m1;
-          P.mom_M2[q] += dl * (xv - m1);
-        }
+      if constexpr (!MomentsAfterLoop<T>::value) {
+        if (c.do_mom) moments_update<p, T, VEC>(P, c, i, x, v);
       }
       if (TAP) {
         const DevTaps& tp = P.taps;
@@ -401,6 +414,13 @@ __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c
     } else {
 #pragma unroll
       for (int j = 0; j < p; ++j) x[j][v] = xi[j];
+    }
+  }
+  if constexpr (MomentsAfterLoop<T>::value) {
+    if (c.do_mom) {
+#pragma unroll
+      for (int v = 0; v < VEC; ++v)
+        if (base + v < P.N) moments_update<p, T, VEC>(P, c, base + v, x, v);
     }
   }
 }
