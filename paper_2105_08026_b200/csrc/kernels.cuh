@@ -71,11 +71,15 @@ __device__ __forceinline__ double hm_sqrt(double x) { return sqrt(x); }
 __device__ __forceinline__ float hm_sqrt(float x) { return sqrtf(x); }
 // sqrt of a positive normal number as x * rsqrt(x) (<= 2 ulp): the RAM scale factor sqrt(1 + c), 1 + c in (0.4, 2)
 __device__ __forceinline__ double hm_rsqrt(double x) { return rsqrt(x); }
-__device__ __forceinline__ float hm_rsqrt(float x) { return rsqrtf(x); }
+// fp32: the hardware reciprocal square root on a NORMAL positive argument.  rsqrtf() wraps the same MUFU.RSQ in a subnormal
+// pre-scale and post-scale (a compare and two multiplies, issued predicated off on every call); every argument here is
+// normal -- -2 ln u1 >= 1.19e-7 for u1 <= 1 - 2^-24, 1 + c >= 1 - alpha*, |z|^2 and s_j s_j+1 of such terms -- so the .ftz
+// form returns the same bits without them (a subnormal argument would flush to zero and return +inf).
+__device__ __forceinline__ float hm_rsqrt(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ double hm_sqrt_pos(double x) { return hm_sqrt_fast(x); }
 __device__ __forceinline__ void hm_sqrt_both(double x, double* g, double* ig) { hm_sqrt_rsqrt(x, g, ig); }
-__device__ __forceinline__ void hm_sqrt_both(float x, float* g, float* ig) { *ig = rsqrtf(x); *g = x * *ig; }
-__device__ __forceinline__ float hm_sqrt_pos(float x) { return x * rsqrtf(x); }
+__device__ __forceinline__ void hm_sqrt_both(float x, float* g, float* ig) { *ig = hm_rsqrt(x); *g = x * *ig; }
+__device__ __forceinline__ float hm_sqrt_pos(float x) { return x * hm_rsqrt(x); }
 
 // Plate-level draws.  Objects draw in PAIRS m = i >> 1 so that one Philox call and one
 // Box-Muller evaluation serve two objects (both Box-Muller branches are independent N(0,1); nothing is wasted):
