@@ -47,7 +47,7 @@ MODES = {"host": 0, "graph": 1, "tail": 2}
 NCU_DRAM_BYTES = {"C2": (14.65e6, 0.0), "C3": (0.0, 313.93e6 / 60), "C4": (0.0, 8333.34e6 / 30), "C6": (3.13e6, 0.0)}
 # warp-level instructions executed per 32 object-updates (smsp__inst_executed.sum / (N K / 32)) and fp64-pipe activity from
 # the same captures.  They give the compute floor reported beside the HBM one: issue slots (4 warp-instructions / clk / SM).
-NCU_WARP_INSTR_PER_32 = {"C2": (409, 38.7), "C3": (442, 42.8), "C4": (145, 11.7), "C6": (1311, 15.4)}
+NCU_WARP_INSTR_PER_32 = {"C2": (409, 38.7), "C3": (442, 42.8), "C4": (138, 12.0), "C6": (1311, 15.4)}
 N_SMS, SM_CLOCK_HZ = 148, 1.965e9
 
 
