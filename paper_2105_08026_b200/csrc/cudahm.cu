@@ -324,7 +324,9 @@ extern "C" int cudahm_create(const cudahm_config* cfg, void* dev_workspace, size
     long long ns = 2;                     // measured on C3: 0 -> 22.4, 1 -> 22.3, 2 -> 22.0, 3 -> 22.2, 4 -> 22.6 us per iteration
     ns = std::min<long long>(std::min(ns, steps), (long long)(STAGE_MAX_SMEM / (ks.stage_step_bytes * ks.dt_sweep_threads / block)));
     s->n_stage = (int)ns; s->stage_smem = (size_t)ns * (ks.stage_step_bytes * ks.dt_sweep_threads / block);
-    if (ensure_dyn_smem(ks.persistent_dt, s->stage_smem) != cudaSuccess) { cudaGetLastError(); s->n_stage = 0; s->stage_smem = 0; }
+    // a handle that keeps no running moments runs the instantiation compiled without them (kernels.cuh, NO_MOM)
+    if (!cfg->keep_chi_moments && ks.persistent_dt_nomom) s->ks.persistent_dt = ks.persistent_dt_nomom;
+    if (ensure_dyn_smem(s->ks.persistent_dt, s->stage_smem) != cudaSuccess) { cudaGetLastError(); s->n_stage = 0; s->stage_smem = 0; }
   }
   // HBM-streaming variant with TMA-staged loads (stream_tma.cuh), opt-in: measured 10-30 % slower than plain vector
   // loads on C3 / C4 (the sweep is issue-bound, not latency-bound, and the producer warp costs a sweep warp)

@@ -12,6 +12,7 @@ bool kernels_binormal2d(int precision, int block, KernelSet* k, ResidentSet* r) 
     if (!pick_block<M_BINORMAL2D, double>(block, k)) return false;
     if (block == 512) {     // p = 2 in fp64: 12 sweep warps with 170 registers are as fast as 16 with 128, which leaves room for tail warps
       k->persistent_dt = (const void*)k_persistent_dt<M_BINORMAL2D, double, 384>;
+      k->persistent_dt_nomom = (const void*)k_persistent_dt<M_BINORMAL2D, double, 384, true>;
       k->dt_sweep_threads = 384;
       k->sweep_dt = (const void*)k_sweep<M_BINORMAL2D, double, 384, false>;
       k->sweep_tap_dt = (const void*)k_sweep<M_BINORMAL2D, double, 384, true>;

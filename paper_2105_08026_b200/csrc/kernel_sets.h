@@ -20,6 +20,7 @@ struct KernelSet {
   const void* sweep_tap_hold;
   // streaming kernel with dedicated tail warps (k_persistent_dt) and its sweep threads per block; NULL where not built
   const void* persistent_dt;
+  const void* persistent_dt_nomom;   // ... compiled without the running-moments update (handles with keep_chi_moments = 0)
   int dt_sweep_threads;
   const void* sweep_dt;          // k_sweep / tapped k_sweep at the same thread -> object map
   const void* sweep_tap_dt;

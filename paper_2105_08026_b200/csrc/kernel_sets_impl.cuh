@@ -17,7 +17,7 @@ KernelSet make_set() {
   k.persistent_hold = (const void*)k_persistent<MODEL, T, BLOCK, PK_HOLD>;
   k.sweep_hold = (const void*)k_sweep<MODEL, T, BLOCK, false, true>;
   k.sweep_tap_hold = (const void*)k_sweep<MODEL, T, BLOCK, true, true>;
-  k.persistent_dt = nullptr; k.dt_sweep_threads = 0; k.sweep_dt = nullptr; k.sweep_tap_dt = nullptr;
+  k.persistent_dt = nullptr; k.persistent_dt_nomom = nullptr; k.dt_sweep_threads = 0; k.sweep_dt = nullptr; k.sweep_tap_dt = nullptr;
   k.stage_step_bytes = (size_t)DrawSet<MODEL, T>::NV * BLOCK * sizeof(T);
   k.persistent_tma = nullptr;
   if constexpr (WITH_TMA) k.persistent_tma = (const void*)k_persistent_tma<MODEL, T, BLOCK>;

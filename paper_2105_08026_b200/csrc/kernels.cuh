@@ -290,7 +290,7 @@ struct LateKp {
   int* wait;             // != 0: sync on BAR_THETAP (n threads) before the first use, then cleared
   int n;
 };
-template <int MODEL, class T, bool TAP, bool HOLD = false, bool LATE = false, int VEC_ = VecOf<T>::n>
+template <int MODEL, class T, bool TAP, bool HOLD = false, bool LATE = false, int VEC_ = VecOf<T>::n, bool NO_MOM = false>
 __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c, const long long base,
                                            T (*x)[VEC_], T (*l)[VEC_], const T (*d)[VEC_], double* sum,
                                            const DrawSet<MODEL, T, VEC_>* staged = nullptr, const LateKp* late = nullptr) {
@@ -398,7 +398,7 @@ __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c
       for (int k = 0; k < ntri; ++k) l[k][v] = ln[k];
       sum[0] += a; sum[1] += b - a;
       sum[2] += acc ? 1.0 : 0.0; sum[3] += (bad && upd) ? 1.0 : 0.0;
-      if constexpr (!MomentsAfterLoop<T>::value) {
+      if constexpr (!MomentsAfterLoop<T>::value && !NO_MOM) {
         if (c.do_mom) moments_update<p, T, VEC>(P, c, i, x, v);
       }
       if (TAP) {
@@ -420,7 +420,7 @@ __device__ __forceinline__ void update_vec(const Params& P, const SweepCtx<T>& c
       for (int j = 0; j < p; ++j) x[j][v] = xi[j];
     }
   }
-  if constexpr (MomentsAfterLoop<T>::value) {
+  if constexpr (MomentsAfterLoop<T>::value && !NO_MOM) {
     if (c.do_mom) {
 #pragma unroll
       for (int v = 0; v < VEC; ++v)
@@ -441,7 +441,7 @@ __device__ __forceinline__ double selection_slice(const Params& P, const ThetaK&
 }
 
 // one step of the sweep: load the thread's VEC objects, update, store
-template <int MODEL, class T, bool TAP, bool HOLD = false, bool LATE = false>
+template <int MODEL, class T, bool TAP, bool HOLD = false, bool LATE = false, bool NO_MOM = false>
 __device__ __forceinline__ void sweep_step(const Params& P, const SweepCtx<T>& c, const long long base, double* acc,
                                            const DrawSet<MODEL, T>* staged, const LateKp* late = nullptr) {
   constexpr int p = ModelDims<MODEL>::p, ntri = p * (p + 1) / 2, ncols = ModelDims<MODEL>::ncols;
@@ -457,7 +457,7 @@ __device__ __forceinline__ void sweep_step(const Params& P, const SweepCtx<T>& c
   for (int k = 0; k < ntri; ++k) ld_vec<T>(Lm + k * Npad + base, l[k], false);
 #pragma unroll
   for (int cc = 0; cc < ncols; ++cc) ld_vec<T>(dat + cc * Npad + base, d[cc], true);
-  update_vec<MODEL, T, TAP, HOLD, LATE>(P, c, base, x, l, d, acc, staged, late);
+  update_vec<MODEL, T, TAP, HOLD, LATE, VecOf<T>::n, NO_MOM>(P, c, base, x, l, d, acc, staged, late);
 #pragma unroll
   for (int j = 0; j < p; ++j) st_vec(chi + j * Npad + base, x[j]);
 #pragma unroll
@@ -765,8 +765,10 @@ __global__ void __launch_bounds__(BLOCK, 1) k_persistent(const Params P, const l
 // while the sweep warps already load, draw, propose and decide the first objects of iteration t + 1; the population term at
 // theta' waits once per iteration for the tail to finish (LateKp).  Worth it where fewer sweep warps with more registers are
 // as fast as 16 (p = 2 in fp64: the sweep is latency-bound); same per-object arithmetic, its own (fixed) summation order.
+// NO_MOM: the instantiation for handles that keep no running moments (cfg.keep_chi_moments = 0).  As a run-time flag the
+// Welford update stays in the code, predicated off, and holds address registers in a kernel that sits at its register cap.
 constexpr int DT_TAIL = 128;
-template <int MODEL, class T, int SWEEP>
+template <int MODEL, class T, int SWEEP, bool NO_MOM = false>
 __global__ void __launch_bounds__(SWEEP + DT_TAIL, 1) k_persistent_dt(const Params P, const long long n_iter, const unsigned epoch0,
                                                                       const int n_stage, const int prefetch) {
   constexpr int VEC = VecOf<T>::n, THREADS = SWEEP + DT_TAIL, SW = SWEEP / 32, NV = DrawSet<MODEL, T>::NV;
@@ -811,11 +813,11 @@ __global__ void __launch_bounds__(SWEEP + DT_TAIL, 1) k_persistent_dt(const Para
         if (prefetch) prefetch_step<MODEL, T>(P, base + stride < N ? base + stride : first);
         DrawSet<MODEL, T> ds;
         ds.get(stage + (size_t)s * NV * SWEEP, SWEEP);
-        sweep_step<MODEL, T, false, false, true>(P, c, base, acc, &ds, &late);
+        sweep_step<MODEL, T, false, false, true, NO_MOM>(P, c, base, acc, &ds, &late);
       }
       for (; base < N; base += stride) {
         if (prefetch) prefetch_step<MODEL, T>(P, base + stride < N ? base + stride : first);
-        sweep_step<MODEL, T, false, false, true>(P, c, base, acc, nullptr, &late);
+        sweep_step<MODEL, T, false, false, true, NO_MOM>(P, c, base, acc, nullptr, &late);
       }
       if (wait) bar_sync(BAR_THETAP, THREADS);               // (not reached with wait set: kept as a guard)
       nacc += acc[2]; nnan += acc[3];
