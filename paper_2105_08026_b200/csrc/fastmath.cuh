@@ -71,9 +71,11 @@ __device__ const hm_d2 hm_exp2_tab_dev[64] = {HM_EXP2_TABLE};
 #endif
 // Where the polynomial coefficients of exp / log come from on the device.  As literals they reach the fp64 pipe through
 // uniform registers, two UMOV per coefficient and use (44 of the 425 warp-instructions per 32 updates of the C2 kernel);
-// from the constant bank one LDCU.128 brings two of them.  Which is faster depends on the kernel: measured -2 to -3.5 % on
-// the streaming p = 2 kernel (C3), +1.4 % on C2, within noise elsewhere -- so a translation unit opts in with
-// HM_CONST_BANK_COEFFS (inst_binormal2d.cu does).
+// from the constant bank one LDCU.128 brings two of them (sm_100a's DFMA takes a register or a uniform register, never a
+// c[bank][offset] operand: probed).  Fewer issue slots, but a constant-cache latency in front of the dependent chain, so
+// which is faster depends on the kernel: measured -2 to -3.5 % on the streaming p = 2 kernel (C3), -1.9 % on C1
+// (k_resident<M1, SEL_SWEEP>), -0.6 % on C0, +0.3 % on C2, +1.3 % on C6, noise on C5 -- so a translation unit opts in with
+// HM_CONST_BANK_COEFFS (inst_binormal2d.cu and inst_thinned_schechter1d_selsweep.cu do).
 #if defined(__CUDACC__) && defined(HM_CONST_BANK_COEFFS)
 __constant__ double hm_kc[24] = {HM_64_LN2, -HM_LN2_64_HI, -HM_LN2_64_LO, 1.3888888888888889e-03, 8.3333333333333332e-03,
   4.1666666666666664e-02, 1.6666666666666666e-01, 0.0,
