@@ -654,3 +654,39 @@ def test_dedicated_tail_kernel_at_its_smallest_populations(n):
     np.testing.assert_allclose(sg["chi"], so["chi"], rtol=1e-9, atol=1e-9)
     np.testing.assert_allclose(sg["L"], so["L"], rtol=1e-9, atol=1e-12)
     assert gpu.get_stats()["chi_accepts"] == orc.get_stats()["chi_accepts"]
+
+
+@pytest.mark.parametrize("model,precision,n,streaming", [
+    (B.M_LINREG_ME1D, B.F32_STATE_F64_REDUCE, 400_001, True),     # fp32 streaming kernel, three ragged steps per thread
+    (B.M_LINREG_ME1D, B.F32_STATE_F64_REDUCE, 50_001, False),     # fp32 state in the general on-chip kernel
+    (B.M_NORMAL1D, B.F32_STATE_F64_REDUCE, 400_001, True),
+    (B.M_BINORMAL2D, B.F64, 200_001, True),                       # fp64 streaming kernel (update inside the per-object loop)
+], ids=["M3f32-stream", "M3f32-onchip", "M0f32-stream", "M2f64-stream"])
+def test_moments_are_the_welford_moments_of_the_gpu_chain(model, precision, n, streaming):
+    """The running chi moments against the definition (PAPER.md:337-341 reports posterior means and standard deviations of
+    the member properties; Welford: mean_k = mean_{k-1} + (x - mean_{k-1}) / k, M2 += (x - mean_{k-1})(x - mean_k)),
+    recomputed on the host in fp64 from the chi the GPU chain itself visits -- one iteration per call, chi read back after
+    each.  Independent of fp32 near-tie decisions (the chain is the GPU's own), so it pins the accumulation exactly:
+    the fp32 kernels update the moments after the per-object loop (kernels.cuh, MomentsAfterLoop), the fp64 ones inside."""
+    burn, post = 3, 9
+    _, gpu, _ = make_pair(model, n, seed=123 + model, precision=precision, astar=0.44 if model != B.M_BINORMAL2D else 0.234,
+                          keep_moments=True, want_oracle=False, flags=B.FLAG_STREAMING_ONLY if streaming else 0,
+                          block_threads=256 if streaming else 0, blocks_per_sm=1 if streaming else 0)
+    p = gpu.p
+    mean, m2 = np.zeros((p, n)), np.zeros((p, n))
+    for t in range(1, burn + post + 1):
+        gpu.run(1, burn, 1, sync=True)
+        if t > burn:
+            x = gpu.get_state()["chi"]                 # float64 view of the (fp32 or fp64) state: exact
+            k = t - burn
+            d = x - mean
+            mean = mean + d * (1.0 / k)
+            m2 = m2 + d * (x - mean)
+    st = gpu.get_stats()
+    assert st["block_threads"] == (256 if streaming else 384)
+    mg, vg, kg = gpu.get_chi_moments()
+    assert kg == post
+    # a fused multiply-add on the device against two roundings here: a few ulp of the mean, relative to the spread for M2
+    np.testing.assert_allclose(mg, mean, rtol=1e-13, atol=1e-13)
+    np.testing.assert_allclose(vg, m2 / (post - 1), rtol=1e-11, atol=1e-14)
+    assert (vg > 0).mean() > 0.1                       # objects moved (p = 2 accepts few proposals this early): not a 0 = 0 check
