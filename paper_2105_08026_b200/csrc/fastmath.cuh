@@ -221,6 +221,49 @@ HM_HD double hm_exp_any(double x) {
   return std::exp(x);
 #endif
 }
+// sin(2 pi u), cos(2 pi u) for u in [0, 1]: the Box-Muller angle of the plate draws (u on the sampler's 2^-32 or 2^-53
+// grids, but any double in range works).  64 u is exact; adding 1.5 * 2^52 rounds it to the nearest integer n (low word
+// of the sum) and d = 64 u - n in [-1/2, 1/2] is exact, so the angle is 2 pi n / 64 + phi with phi = d pi / 32,
+// |phi| <= pi / 64 = 0.0491.  T[n & 63] = (S, C) = (sin, cos)(2 pi n / 64) from a 64-entry table (1 KB, stays in L1), rounded
+// to nearest and EXACTLY 0 / +-1 at the quarter turns, so that near the zeros of sin and cos the result is C sin(phi)
+// (resp. -S sin(phi)) with full relative accuracy.  sin(phi) by its Taylor polynomial through phi^9 (truncation
+// phi^10 / 11! < 3e-21 relative), cos(phi) - 1 through phi^8 (phi^10 / 10! < 3e-20), then
+//   sin = S + (S (cos phi - 1) + C sin phi),  cos = C + (C (cos phi - 1) - S sin phi).
+// Error: half an ulp of the table entry, half an ulp of the last sum, and the roundings of the small bracket: <= 2 ulp,
+// pinned in tests/test_fastmath_host.py against mpmath.  Half the instructions of the library sincospi on this argument
+// range (26 + 11 fp64 immediates against 38 + 15), and a dependent chain of 4 DFMA instead of 7.
+#include "sincos_table.inc"
+#ifdef __CUDACC__
+__device__ const hm_d2 hm_sincos64_tab_dev[64] = {HM_SINCOS64_TABLE};
+#endif
+static const hm_d2 hm_sincos64_tab_host[64] = {HM_SINCOS64_TABLE};
+HM_HD void hm_sincos2pi(double u, double* s, double* c) {
+  const double SHIFT = 6755399441055744.0;                 // 1.5 * 2^52
+  const double t = hm_fma(u, 64.0, SHIFT);                 // n = rint(64 u) in the low word
+  const double d = hm_fma(u, 64.0, -(t - SHIFT));          // 64 u - n, exact
+  const int j = (int)(uint32_t)(hm_d2bits(t) & 63ull);
+#ifdef __CUDA_ARCH__
+  const double2 tj = __ldg(reinterpret_cast<const double2*>(hm_sincos64_tab_dev) + j);
+  const double S = tj.x, C = tj.y;
+#else
+  const double S = hm_sincos64_tab_host[j].hi, C = hm_sincos64_tab_host[j].lo;
+#endif
+  const double phi = d * HM_PI_32;
+  const double p2 = phi * phi;
+  double sp = 2.7557319223985893e-06;                      // 1/9!
+  sp = hm_fma(sp, p2, -1.9841269841269841e-04);            // -1/7!
+  sp = hm_fma(sp, p2, 8.3333333333333332e-03);             // 1/5!
+  sp = hm_fma(sp, p2, -1.6666666666666666e-01);            // -1/3!
+  const double sphi = hm_fma(sp * p2, phi, phi);           // sin(phi)
+  double cp = 2.4801587301587302e-05;                      // 1/8!
+  cp = hm_fma(cp, p2, -1.3888888888888889e-03);            // -1/6!
+  cp = hm_fma(cp, p2, 4.1666666666666664e-02);             // 1/4!
+  cp = hm_fma(cp, p2, -0.5);
+  const double cm = cp * p2;                               // cos(phi) - 1
+  *s = S + hm_fma(S, cm, C * sphi);
+  *c = C + hm_fma(C, cm, -(S * sphi));
+}
+
 HM_HD double hm_log_any_pos(double x) {
 #ifdef __CUDA_ARCH__
   return hm_log_pos(x);

@@ -100,7 +100,7 @@ __device__ __forceinline__ void pair_draws(const KEY& seed, long long i0, uint32
     u[0] = u01_32(a.z); u[1] = u01_32(a.w);
     const double rad = hm_sqrt_fast(-2.0 * hm_log_unit(u1));
     double s_, c_;
-    sincospi(2.0 * u2, &s_, &c_);
+    hm_sincos2pi(u2, &s_, &c_);
     z[0][0] = rad * c_; z[1][0] = rad * s_;
     z[0][1] = 0.0; z[1][1] = 0.0;
     cs[0] = cs[1] = 0.0; sn[0] = sn[1] = 0.0;      // the unit vector is not needed for p = 1
@@ -111,7 +111,7 @@ __device__ __forceinline__ void pair_draws(const KEY& seed, long long i0, uint32
       const U4 b = stream(seed, KIND_PLATE, (uint64_t)(i0 + h), t, 1u);
       const double u1 = u01(b.x, b.y), u2 = u01(b.z, b.w);
       const double rad = hm_sqrt_fast(-2.0 * hm_log_unit(u1));
-      sincospi(2.0 * u2, &sn[h], &cs[h]);
+      hm_sincos2pi(u2, &sn[h], &cs[h]);
       z[h][0] = rad * cs[h]; z[h][1] = rad * sn[h];
       if constexpr (P >= 3) {
         // general p: Box-Muller pair k of object i comes from draw 1 + k (z_{2k}, z_{2k+1}); an odd p drops the last sine
@@ -122,7 +122,7 @@ __device__ __forceinline__ void pair_draws(const KEY& seed, long long i0, uint32
           const double v1 = u01(b2.x, b2.y), v2 = u01(b2.z, b2.w);
           const double rad2 = hm_sqrt_fast(-2.0 * hm_log_unit(v1));
           double s2_, c2_;
-          sincospi(2.0 * v2, &s2_, &c2_);
+          hm_sincos2pi(v2, &s2_, &c2_);
           z[h][2 * k] = rad2 * c2_;
           if (2 * k + 1 < P) z[h][2 * k + 1] = rad2 * s2_;
         }
@@ -198,7 +198,7 @@ __device__ __forceinline__ void single_draws(const KEY& seed, long long i, uint3
   const U4 b = stream(seed, KIND_PLATE, (uint64_t)i, t, 1u);
   const double u1 = u01(b.x, b.y), u2 = u01(b.z, b.w);
   const double rad = hm_sqrt_fast(-2.0 * hm_log_unit(u1));
-  sincospi(2.0 * u2, sn, cs);
+  hm_sincos2pi(u2, sn, cs);
   z[0] = rad * *cs; z[1] = rad * *sn;
 #pragma unroll
   for (int k = 1; 2 * k < P; ++k) {
@@ -206,7 +206,7 @@ __device__ __forceinline__ void single_draws(const KEY& seed, long long i, uint3
     const double v1 = u01(b2.x, b2.y), v2 = u01(b2.z, b2.w);
     const double rad2 = hm_sqrt_fast(-2.0 * hm_log_unit(v1));
     double s2_, c2_;
-    sincospi(2.0 * v2, &s2_, &c2_);
+    hm_sincos2pi(v2, &s2_, &c2_);
     z[2 * k] = rad2 * c2_;
     if (2 * k + 1 < P) z[2 * k + 1] = rad2 * s2_;
   }

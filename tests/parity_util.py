@@ -7,7 +7,7 @@ Tolerances (DESIGN.md section 14 derives every one that is not north_star's own 
   fed state    every GPU tap is ALSO compared with the oracle's primitive evaluated at the GPU's own upstream taps
                (the oracle's log-densities at the GPU's chi', the closed form / defining identity of the RAM update at the
                GPU's alpha), so each stage is held to north_star's figure on identical inputs and no tolerance has to
-               absorb the propagated few-ulp difference of the normals (device log / sqrt / sincospi against glibc's).
+               absorb the propagated few-ulp difference of the normals (device log / sqrt / sin-cos of fastmath.cuh against glibc's).
   propagated   the direct GPU-vs-oracle comparisons downstream of the normals use bounds computed from the measured
                upstream differences (first-order error propagation), not fixed multipliers.
 """

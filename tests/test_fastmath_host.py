@@ -108,3 +108,40 @@ def test_u01_32_is_exact(binary):
     got = run(binary, "u32", w.view(np.float64))
     assert np.array_equal(got, (w.astype(np.float64) + 0.5) * 2.0 ** -32)
     assert got.min() == 2.0 ** -33 and got.max() == 1 - 2.0 ** -33
+
+
+def _angle_grid_points():
+    rng = np.random.default_rng(8)
+    w = rng.integers(0, 2 ** 32, 5000).astype(np.float64)
+    near = []
+    for z in (0, 2 ** 30, 2 ** 31, 3 * 2 ** 30, 2 ** 32):                    # the zeros of sin and cos on the 32-bit grid
+        near += [z + o for o in range(-6, 6) if 0 <= z + o < 2 ** 32]
+    for n in range(0, 64, 3):                                                # both sides of every third table boundary
+        near += [n * 2 ** 26 + 2 ** 25 + o for o in (-2, -1, 0, 1)]
+    u32 = (np.concatenate([w, np.array(near, dtype=np.float64)]) + 0.5) * 2.0 ** -32      # exactly the p = 1 uniforms
+    k = rng.integers(0, 2 ** 52, 3000).astype(np.float64)
+    k = np.concatenate([k, [0.0, 1.0, 2.0 ** 52 - 1, 2.0 ** 50, 2.0 ** 50 - 1, 2.0 ** 51, 2.0 ** 51 - 1]])
+    u52 = (k + 0.5) * 2.0 ** -52                                             # exactly the p >= 2 uniforms
+    return np.concatenate([u32, u52])
+
+
+def test_sincos2pi_within_2_ulp_on_the_draw_grids(binary):
+    """hm_sincos2pi(u) = (sin, cos)(2 pi u), the Box-Muller angle: <= 2 ulp of the RESULT everywhere on the two grids the
+    sampler draws from, the neighbourhoods of the zeros included (the table entries there are exactly 0 and +-1)."""
+    u = _angle_grid_points()
+    two_pi = lambda x: 2 * mpmath.pi * x
+    sn, cs = run(binary, "sin2pi", u), run(binary, "cos2pi", u)
+    es, ec = ulp_err(sn, lambda x: mpmath.sin(two_pi(x)), u), ulp_err(cs, lambda x: mpmath.cos(two_pi(x)), u)
+    assert es <= 2.0 and ec <= 2.0, (es, ec)
+    # the identity the sampler relies on (a unit vector): to a few ulp
+    assert np.abs(sn * sn + cs * cs - 1.0).max() < 1e-15
+
+
+def test_sincos2pi_exact_at_the_quarter_turns(binary):
+    u = np.array([0.0, 0.25, 0.5, 0.75, 1.0])
+    assert np.array_equal(run(binary, "sin2pi", u), [0.0, 1.0, 0.0, -1.0, 0.0])
+    assert np.array_equal(run(binary, "cos2pi", u), [1.0, 0.0, -1.0, 0.0, 1.0])
+    # odd / even symmetry about the half turn, bit for bit (the reduction is symmetric: d -> -d, the table is antisymmetric)
+    v = (np.arange(1, 4000, 7, dtype=np.float64) + 0.5) * 2.0 ** -32
+    assert np.array_equal(run(binary, "sin2pi", 1.0 - v), -run(binary, "sin2pi", v))
+    assert np.array_equal(run(binary, "cos2pi", 1.0 - v), run(binary, "cos2pi", v))
