@@ -23,6 +23,16 @@ int cudahm_probe_floor(void* cuda_stream, int kind, int n_iter, int grid_blocks,
 /* Register-resident FMA throughput of the plain ALU pipes, in tera-FMA/s: dtype 0 = fp64 (DFMA), 1 = fp32 (FFMA). */
 int cudahm_probe_fma_peak(void* cuda_stream, int dtype, double* tera_fma_per_s);
 
+/* The device builds of the elementary functions of csrc/fastmath.cuh, evaluated on the GPU: y[i] = fn(x[i]) for n HOST
+ * doubles (copied in and out on `stream`, which is synchronised before the call returns).  The sampler's kernels call these
+ * very functions; tests/test_gpu_fastmath.py holds their device results to the bounds the host builds are pinned to
+ * (the device seeds its reciprocal and reciprocal square root with MUFU instructions the host cannot reproduce).
+ * CUDAHM_MATH_SIN2PI / COS2PI: hm_sincos2pi (the Box-Muller angle, x in [0, 1]); SQRT_BOTH_*: the two results of
+ * hm_sqrt_rsqrt.  Returns 0 or a negative CUDAHM_E_* code. */
+enum { CUDAHM_MATH_EXP = 0, CUDAHM_MATH_EXPM1_NONPOS = 1, CUDAHM_MATH_LOG = 2, CUDAHM_MATH_SQRT = 3, CUDAHM_MATH_SQRT_BOTH_ROOT = 4,
+       CUDAHM_MATH_SQRT_BOTH_INV = 5, CUDAHM_MATH_SIN2PI = 6, CUDAHM_MATH_COS2PI = 7 };
+int cudahm_probe_math(void* cuda_stream, int fn, const double* x_host, double* y_host, long long n);
+
 #ifdef __cplusplus
 }
 #endif

@@ -33,7 +33,7 @@ EXPORTS = ["cudahm_model_dims", "cudahm_workspace_bytes", "cudahm_create", "cuda
            "cudahm_get_theta_trace", "cudahm_get_chi_moments", "cudahm_get_stats", "cudahm_get_state",
            "cudahm_set_state", "cudahm_sync", "cudahm_last_error", "cudahm_shard_sweep", "cudahm_shard_decide", "cudahm_shard_combine", "cudahm_shard_sweep_device",
            "cudahm_shard_decide_gathered", "cudahm_set_update_mask", "cudahm_get_counters", "cudahm_set_counters",
-           "cudahm_probe_floor", "cudahm_probe_fma_peak"]
+           "cudahm_probe_floor", "cudahm_probe_fma_peak", "cudahm_probe_math"]
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int32)
@@ -114,6 +114,7 @@ def load():
     L.cudahm_last_error.restype = C.c_char_p
     L.cudahm_probe_floor.argtypes = [vp, C.c_int, C.c_int, C.c_int, C.c_int, _dp]
     L.cudahm_probe_fma_peak.argtypes = [vp, C.c_int, _dp]
+    L.cudahm_probe_math.argtypes = [vp, C.c_int, _dp, _dp, C.c_longlong]
     _lib = L
     return L
 
@@ -405,3 +406,19 @@ def probe_fma_peak(dtype, stream=None):
     if rc:
         raise CudahmError(rc, "probe_fma_peak failed")
     return out.value
+
+
+# cudahm_probe.h: CUDAHM_MATH_*
+MATH_EXP, MATH_EXPM1_NONPOS, MATH_LOG, MATH_SQRT, MATH_SQRT_BOTH_ROOT, MATH_SQRT_BOTH_INV, MATH_SIN2PI, MATH_COS2PI = range(8)
+
+
+def probe_math(fn, x, stream=None):
+    """y = fn(x) evaluated by the DEVICE build of csrc/fastmath.cuh (cudahm_probe_math); x: float64 array."""
+    import torch
+    st = stream if stream is not None else torch.cuda.current_stream()
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    y = np.empty_like(x)
+    rc = load().cudahm_probe_math(C.c_void_p(st.cuda_stream), int(fn), _d(x), _d(y), x.size)
+    if rc:
+        raise CudahmError(rc, "probe_math failed")
+    return y

@@ -1,5 +1,6 @@
 // probe.cu -- launch / sync / barrier floors and ALU-pipe peaks (include/cudahm_probe.h).
 #include "cudahm_probe.h"
+#include "fastmath.cuh"
 
 #include <cuda_runtime.h>
 #include <vector>
@@ -130,5 +131,43 @@ done:
   if (out) cudaFree(out);
   if (e0) cudaEventDestroy(e0);
   if (e1) cudaEventDestroy(e1);
+  return rc;
+}
+
+namespace {
+__global__ void k_probe_math(const int fn, const double* __restrict__ x, double* __restrict__ y, const long long n) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double v = x[i];
+  double r = 0.0, q = 0.0;
+  switch (fn) {
+    case CUDAHM_MATH_EXP: r = hm::hm_exp_fast(v); break;
+    case CUDAHM_MATH_EXPM1_NONPOS: r = hm::hm_expm1_nonpos(v); break;
+    case CUDAHM_MATH_LOG: r = hm::hm_log_pos(v); break;
+    case CUDAHM_MATH_SQRT: r = hm::hm_sqrt_fast(v); break;
+    case CUDAHM_MATH_SQRT_BOTH_ROOT: hm::hm_sqrt_rsqrt(v, &r, &q); break;
+    case CUDAHM_MATH_SQRT_BOTH_INV: hm::hm_sqrt_rsqrt(v, &q, &r); break;
+    case CUDAHM_MATH_SIN2PI: hm::hm_sincos2pi(v, &r, &q); break;
+    default: hm::hm_sincos2pi(v, &q, &r); break;
+  }
+  y[i] = r;
+}
+}  // namespace
+
+extern "C" int cudahm_probe_math(void* cuda_stream, int fn, const double* x_host, double* y_host, long long n) {
+  if (!x_host || !y_host || n < 0 || fn < CUDAHM_MATH_EXP || fn > CUDAHM_MATH_COS2PI) return -1;
+  if (n == 0) return 0;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int rc = 0;
+  double *x = nullptr, *y = nullptr;
+  PR_TRY(cudaMalloc(&x, (size_t)n * 8)); PR_TRY(cudaMalloc(&y, (size_t)n * 8));
+  PR_TRY(cudaMemcpyAsync(x, x_host, (size_t)n * 8, cudaMemcpyHostToDevice, st));
+  k_probe_math<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(fn, x, y, n);
+  PR_TRY(cudaGetLastError());
+  PR_TRY(cudaMemcpyAsync(y_host, y, (size_t)n * 8, cudaMemcpyDeviceToHost, st));
+  PR_TRY(cudaStreamSynchronize(st));
+done:
+  if (x) cudaFree(x);
+  if (y) cudaFree(y);
   return rc;
 }
