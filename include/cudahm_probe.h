@@ -30,7 +30,9 @@ int cudahm_probe_fma_peak(void* cuda_stream, int dtype, double* tera_fma_per_s);
  * CUDAHM_MATH_SIN2PI / COS2PI: hm_sincos2pi (the Box-Muller angle, x in [0, 1]); SQRT_BOTH_*: the two results of
  * hm_sqrt_rsqrt.  Returns 0 or a negative CUDAHM_E_* code. */
 enum { CUDAHM_MATH_EXP = 0, CUDAHM_MATH_EXPM1_NONPOS = 1, CUDAHM_MATH_LOG = 2, CUDAHM_MATH_SQRT = 3, CUDAHM_MATH_SQRT_BOTH_ROOT = 4,
-       CUDAHM_MATH_SQRT_BOTH_INV = 5, CUDAHM_MATH_SIN2PI = 6, CUDAHM_MATH_COS2PI = 7 };
+       CUDAHM_MATH_SQRT_BOTH_INV = 5, CUDAHM_MATH_SIN2PI = 6, CUDAHM_MATH_COS2PI = 7,
+       /* LOG .. SQRT_BOTH_INV above are the one-Newton-step variants; these are the two-step ones (fastmath.cuh, HM_NEWTON_STEPS) */
+       CUDAHM_MATH_LOG_2 = 8, CUDAHM_MATH_SQRT_2 = 9, CUDAHM_MATH_SQRT_BOTH_ROOT_2 = 10, CUDAHM_MATH_SQRT_BOTH_INV_2 = 11 };
 int cudahm_probe_math(void* cuda_stream, int fn, const double* x_host, double* y_host, long long n);
 
 #ifdef __cplusplus

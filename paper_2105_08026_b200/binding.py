@@ -410,6 +410,7 @@ def probe_fma_peak(dtype, stream=None):
 
 # cudahm_probe.h: CUDAHM_MATH_*
 MATH_EXP, MATH_EXPM1_NONPOS, MATH_LOG, MATH_SQRT, MATH_SQRT_BOTH_ROOT, MATH_SQRT_BOTH_INV, MATH_SIN2PI, MATH_COS2PI = range(8)
+MATH_LOG_2, MATH_SQRT_2, MATH_SQRT_BOTH_ROOT_2, MATH_SQRT_BOTH_INV_2 = range(8, 12)   # the two-Newton-step variants
 
 
 def probe_math(fn, x, stream=None):

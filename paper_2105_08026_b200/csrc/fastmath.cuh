@@ -44,19 +44,23 @@ HM_HD double hm_fma(double a, double b, double c) {
 #endif
 }
 
-// 2^-23-accurate seeds (one MUFU each on the device)
+// Seeds with about 20 good bits (one MUFU each on the device: the instruction works on the upper 32-bit word of its
+// argument and returns a result whose lower word is zero).  The host build imitates the WORST such seed -- the exact value
+// with its lower word cleared -- so that the host pins cover what the device may return; tests/test_gpu_fastmath.py
+// holds the device build itself to the same pins.  One Newton step takes 2^-20 to 2^-40, and every user below ends with a
+// correction step that squares the residual once more (2^-80): a second Newton step would buy nothing.
 HM_HD double hm_rcp_seed(double a) {
 #ifdef __CUDA_ARCH__
   double r; asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a)); return r;
 #else
-  return (double)(1.0f / (float)a);
+  return hm_bits2d(hm_d2bits(1.0 / a) & 0xffffffff00000000ull);
 #endif
 }
 HM_HD double hm_rsqrt_seed(double a) {
 #ifdef __CUDA_ARCH__
   double r; asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a)); return r;
 #else
-  return (double)(1.0f / std::sqrt((float)a));
+  return hm_bits2d(hm_d2bits(1.0 / std::sqrt(a)) & 0xffffffff00000000ull);
 #endif
 }
 
@@ -152,7 +156,15 @@ HM_HD double hm_exp_fast(double x) {
 
 // ln u for positive normal u: u = 2^e m, m in [sqrt(1/2), sqrt 2); ln m = 2 atanh(s), s = (m-1)/(m+1), |s| <= 0.1716,
 // atanh series to s^23 (truncation 6e-19 relative); the quotient by a Newton-refined reciprocal.
-HM_HD double hm_log_pos(double u) {
+// NEWTON: Newton steps on the seed before the correcting step (1 is enough, see hm_rcp_seed; 2 is the former code, kept
+// because the on-chip p = 1 kernel is FASTER with it: C2 +0.6 %, C1 / C0 +0.5 % with one step -- code generation, the
+// kernel is not issue-bound -- while the p = 2 streaming kernel gains 3.2 %).  A translation unit chooses with
+// HM_NEWTON_STEPS (default 1); both variants are pinned on the host and on the device.
+#ifndef HM_NEWTON_STEPS
+#define HM_NEWTON_STEPS 1
+#endif
+template <int NEWTON>
+HM_HD double hm_log_pos_n(double u) {
   uint64_t b = hm_d2bits(u);
   int e = (int)(b >> 52) - 1023;
   b = (b & 0x000fffffffffffffull) | 0x3ff0000000000000ull;
@@ -160,12 +172,13 @@ HM_HD double hm_log_pos(double u) {
   if (m > 1.4142135623730951) { m *= 0.5; e += 1; }
   const double a = m + 1.0, f = m - 1.0;
   double rc = hm_rcp_seed(a);
-  double err = hm_fma(-a, rc, 1.0);
-  rc = hm_fma(rc, err, rc);
-  err = hm_fma(-a, rc, 1.0);
-  rc = hm_fma(rc, err, rc);
+#pragma unroll
+  for (int it = 0; it < NEWTON; ++it) {                     // 1/a to 2^-40 (2^-80)
+    const double err = hm_fma(-a, rc, 1.0);
+    rc = hm_fma(rc, err, rc);
+  }
   double s = f * rc;
-  s = hm_fma(hm_fma(-s, a, f), rc, s);                      // one correction: s = f/a to ~0.5 ulp
+  s = hm_fma(hm_fma(-s, a, f), rc, s);                      // the correction squares the residual: s = f/a to ~0.5 ulp
   const double s2 = s * s;
   double p = HM_KC(8, 1.0 / 23.0);
   p = hm_fma(p, s2, HM_KC(9, 1.0 / 21.0));
@@ -185,31 +198,39 @@ HM_HD double hm_log_pos(double u) {
   return hm_fma(ed, HM_KC(19, 6.93147180369123816490e-01), hm_fma(ed, HM_KC(20, 1.90821492927058770002e-10), lm));
 }
 
+HM_HD double hm_log_pos(double u) { return hm_log_pos_n<HM_NEWTON_STEPS>(u); }
 HM_HD double hm_log_unit(double u) { return hm_log_pos(u); }   // u in [2^-53, 1)
 
 // sqrt(w), w > 0 normal: Newton on (g, h) = (sqrt w, 1/(2 sqrt w)) from a 2^-23 reciprocal-root seed.
-HM_HD double hm_sqrt_fast(double w) {
+template <int NEWTON>
+HM_HD double hm_sqrt_fast_n(double w) {
   const double y = hm_rsqrt_seed(w);
   double g = w * y, h = 0.5 * y;
-  double r = hm_fma(-g, h, 0.5);
-  g = hm_fma(g, r, g); h = hm_fma(h, r, h);
-  r = hm_fma(-g, h, 0.5);
-  g = hm_fma(g, r, g); h = hm_fma(h, r, h);
-  return hm_fma(hm_fma(-g, g, w), h, g);                    // final correction
+#pragma unroll
+  for (int it = 0; it < NEWTON; ++it) {                     // (g, h) to 2^-40 (2^-80)
+    const double r = hm_fma(-g, h, 0.5);
+    g = hm_fma(g, r, g); h = hm_fma(h, r, h);
+  }
+  return hm_fma(hm_fma(-g, g, w), h, g);                    // final correction: g + (w - g^2) h, residual squared
 }
+HM_HD double hm_sqrt_fast(double w) { return hm_sqrt_fast_n<HM_NEWTON_STEPS>(w); }
 
 // sqrt(w) and 1/sqrt(w) together (the same Newton pair; 1/sqrt = 2 h after one more correction step), w > 0 normal
-HM_HD void hm_sqrt_rsqrt(double w, double* root, double* inv_root) {
+template <int NEWTON>
+HM_HD void hm_sqrt_rsqrt_n(double w, double* root, double* inv_root) {
   const double y = hm_rsqrt_seed(w);
   double g = w * y, h = 0.5 * y;
-  double r = hm_fma(-g, h, 0.5);
-  g = hm_fma(g, r, g); h = hm_fma(h, r, h);
-  r = hm_fma(-g, h, 0.5);
-  g = hm_fma(g, r, g); h = hm_fma(h, r, h);
+  double r;
+#pragma unroll
+  for (int it = 0; it < NEWTON; ++it) {                     // (g, h) to 2^-40 (2^-80)
+    r = hm_fma(-g, h, 0.5);
+    g = hm_fma(g, r, g); h = hm_fma(h, r, h);
+  }
   r = hm_fma(-g, h, 0.5);
   *root = hm_fma(hm_fma(-g, g, w), h, g);
   *inv_root = 2.0 * hm_fma(h, r, h);
 }
+HM_HD void hm_sqrt_rsqrt(double w, double* root, double* inv_root) { hm_sqrt_rsqrt_n<HM_NEWTON_STEPS>(w, root, inv_root); }
 
 // exp / log of the theta tail: the specialised versions on the device (the tail is a serial chain on the critical
 // path of every iteration), libm on the host (THETA_HOST).

@@ -1,4 +1,6 @@
 // inst_normal1d.cu -- every kernel of model M_NORMAL1D (its own translation unit: the models build in parallel).
+// two Newton steps in log / sqrt (fastmath.cuh, HM_NEWTON_STEPS): measured faster for the on-chip p = 1 kernel of this model
+#define HM_NEWTON_STEPS 2
 #include "kernel_sets_impl.cuh"
 
 namespace hm {

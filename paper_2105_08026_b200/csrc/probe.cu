@@ -143,10 +143,14 @@ __global__ void k_probe_math(const int fn, const double* __restrict__ x, double*
   switch (fn) {
     case CUDAHM_MATH_EXP: r = hm::hm_exp_fast(v); break;
     case CUDAHM_MATH_EXPM1_NONPOS: r = hm::hm_expm1_nonpos(v); break;
-    case CUDAHM_MATH_LOG: r = hm::hm_log_pos(v); break;
-    case CUDAHM_MATH_SQRT: r = hm::hm_sqrt_fast(v); break;
-    case CUDAHM_MATH_SQRT_BOTH_ROOT: hm::hm_sqrt_rsqrt(v, &r, &q); break;
-    case CUDAHM_MATH_SQRT_BOTH_INV: hm::hm_sqrt_rsqrt(v, &q, &r); break;
+    case CUDAHM_MATH_LOG: r = hm::hm_log_pos_n<1>(v); break;
+    case CUDAHM_MATH_SQRT: r = hm::hm_sqrt_fast_n<1>(v); break;
+    case CUDAHM_MATH_SQRT_BOTH_ROOT: hm::hm_sqrt_rsqrt_n<1>(v, &r, &q); break;
+    case CUDAHM_MATH_SQRT_BOTH_INV: hm::hm_sqrt_rsqrt_n<1>(v, &q, &r); break;
+    case CUDAHM_MATH_LOG_2: r = hm::hm_log_pos_n<2>(v); break;
+    case CUDAHM_MATH_SQRT_2: r = hm::hm_sqrt_fast_n<2>(v); break;
+    case CUDAHM_MATH_SQRT_BOTH_ROOT_2: hm::hm_sqrt_rsqrt_n<2>(v, &r, &q); break;
+    case CUDAHM_MATH_SQRT_BOTH_INV_2: hm::hm_sqrt_rsqrt_n<2>(v, &q, &r); break;
     case CUDAHM_MATH_SIN2PI: hm::hm_sincos2pi(v, &r, &q); break;
     default: hm::hm_sincos2pi(v, &q, &r); break;
   }
@@ -155,7 +159,7 @@ __global__ void k_probe_math(const int fn, const double* __restrict__ x, double*
 }  // namespace
 
 extern "C" int cudahm_probe_math(void* cuda_stream, int fn, const double* x_host, double* y_host, long long n) {
-  if (!x_host || !y_host || n < 0 || fn < CUDAHM_MATH_EXP || fn > CUDAHM_MATH_COS2PI) return -1;
+  if (!x_host || !y_host || n < 0 || fn < CUDAHM_MATH_EXP || fn > CUDAHM_MATH_SQRT_BOTH_INV_2) return -1;
   if (n == 0) return 0;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   int rc = 0;

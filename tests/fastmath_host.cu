@@ -1,5 +1,5 @@
 // Host build of paper_2105_08026_b200/csrc/fastmath.cuh and philox.cuh::u01 for tests/test_fastmath_host.py.
-// usage: fastmath_host <exp|expm1|log|sqrt|sqrt_both_root|sqrt_both_inv|sin2pi|cos2pi|u01|u32> < binary doubles (u01: pairs of uint32 packed in uint64) > binary doubles
+// usage: fastmath_host <exp|expm1|log[2]|sqrt[2]|sqrt_both_root[2]|sqrt_both_inv[2]|sin2pi|cos2pi|u01|u32> (a trailing 2: the two-Newton-step variant) < binary doubles (u01: pairs of uint32 packed in uint64) > binary doubles
 #include <cstdio>
 #include <cstring>
 #include <vector>
@@ -15,11 +15,15 @@ int main(int argc, char** argv) {
   std::vector<double> out(in.size());
   for (size_t i = 0; i < in.size(); ++i) {
     if (!strcmp(argv[1], "exp")) out[i] = hm::hm_exp_fast(in[i]);
-    else if (!strcmp(argv[1], "log")) out[i] = hm::hm_log_pos(in[i]);
+    else if (!strcmp(argv[1], "log")) out[i] = hm::hm_log_pos_n<1>(in[i]);
+    else if (!strcmp(argv[1], "log2")) out[i] = hm::hm_log_pos_n<2>(in[i]);
     else if (!strcmp(argv[1], "expm1")) out[i] = hm::hm_expm1_nonpos(in[i]);
-    else if (!strcmp(argv[1], "sqrt")) out[i] = hm::hm_sqrt_fast(in[i]);
-    else if (!strcmp(argv[1], "sqrt_both_root")) { double g, ig; hm::hm_sqrt_rsqrt(in[i], &g, &ig); out[i] = g; }
-    else if (!strcmp(argv[1], "sqrt_both_inv")) { double g, ig; hm::hm_sqrt_rsqrt(in[i], &g, &ig); out[i] = ig; }
+    else if (!strcmp(argv[1], "sqrt")) out[i] = hm::hm_sqrt_fast_n<1>(in[i]);
+    else if (!strcmp(argv[1], "sqrt2")) out[i] = hm::hm_sqrt_fast_n<2>(in[i]);
+    else if (!strcmp(argv[1], "sqrt_both_root")) { double g, ig; hm::hm_sqrt_rsqrt_n<1>(in[i], &g, &ig); out[i] = g; }
+    else if (!strcmp(argv[1], "sqrt_both_inv")) { double g, ig; hm::hm_sqrt_rsqrt_n<1>(in[i], &g, &ig); out[i] = ig; }
+    else if (!strcmp(argv[1], "sqrt_both_root2")) { double g, ig; hm::hm_sqrt_rsqrt_n<2>(in[i], &g, &ig); out[i] = g; }
+    else if (!strcmp(argv[1], "sqrt_both_inv2")) { double g, ig; hm::hm_sqrt_rsqrt_n<2>(in[i], &g, &ig); out[i] = ig; }
     else if (!strcmp(argv[1], "sin2pi")) { double sn, cs; hm::hm_sincos2pi(in[i], &sn, &cs); out[i] = sn; }
     else if (!strcmp(argv[1], "cos2pi")) { double sn, cs; hm::hm_sincos2pi(in[i], &sn, &cs); out[i] = cs; }
     else if (!strcmp(argv[1], "u01")) { uint64_t w; memcpy(&w, &in[i], 8); out[i] = hm::u01((uint32_t)(w >> 32), (uint32_t)w); }

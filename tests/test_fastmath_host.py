@@ -63,29 +63,35 @@ def test_expm1_nonpos(binary):
     assert run(binary, "expm1", np.array([-1e4, -np.inf]))[0] == -1.0
 
 
-def test_log_pos(binary):
+STEPS = pytest.mark.parametrize("steps", ["", "2"], ids=["newton1", "newton2"])   # fastmath.cuh: HM_NEWTON_STEPS variants
+
+
+@STEPS
+def test_log_pos(binary, steps):
     rng = np.random.default_rng(2)
     k = rng.integers(0, 2 ** 52, 4000)
     u = (k + 0.5) * 2.0 ** -52                       # exactly the uniforms the sampler draws
     u = np.concatenate([u, [2.0 ** -53, 1 - 2.0 ** -53, 0.5, 0.70710678118654752, 0.7071067811865476, 0.25],
                         np.exp(-rng.uniform(0, 36, 2000)), rng.uniform(1.0, 5.0, 1000), [1.0, 2.0, 1e300, 3e-308]])
-    got = run(binary, "log", u)
+    got = run(binary, "log" + steps, u)
     assert ulp_err(got, mpmath.log, u) <= 2.0       # worst case: e ln2 and ln m of opposite sign near m = sqrt 2
 
 
-def test_sqrt_fast(binary):
+@STEPS
+def test_sqrt_fast(binary, steps):
     rng = np.random.default_rng(3)
     w = np.concatenate([np.exp(rng.uniform(-36, 5, 4000)), rng.uniform(0.4, 2.0, 2000), [1.0, 4.0, 2.0, 73.5]])
-    got = run(binary, "sqrt", w)
+    got = run(binary, "sqrt" + steps, w)
     assert ulp_err(got, mpmath.sqrt, w) <= 1.0
     assert np.mean(got == np.sqrt(w)) > 0.95          # almost always the correctly rounded root
 
 
-def test_sqrt_rsqrt_pair(binary):
+@STEPS
+def test_sqrt_rsqrt_pair(binary, steps):
     """The p = 2 RAM update takes sqrt(s1) and 1/sqrt(s1) from one Newton pair (s1 = 1 + c u1^2 in (0.4, 2))."""
     rng = np.random.default_rng(4)
     w = np.concatenate([rng.uniform(0.4, 2.0, 4000), np.exp(rng.uniform(-20, 20, 2000)), [1.0, 4.0, 0.25, 2.0]])
-    root, inv = run(binary, "sqrt_both_root", w), run(binary, "sqrt_both_inv", w)
+    root, inv = run(binary, "sqrt_both_root" + steps, w), run(binary, "sqrt_both_inv" + steps, w)
     assert ulp_err(root, mpmath.sqrt, w) <= 1.0
     assert ulp_err(inv, lambda x: 1 / mpmath.sqrt(x), w) <= 2.0
     assert root[-4] == 1.0 and inv[-4] == 1.0 and root[-3] == 2.0 and inv[-3] == 0.5
