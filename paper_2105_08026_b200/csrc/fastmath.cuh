@@ -69,6 +69,7 @@ HM_HD double hm_rsqrt_seed(double a) {
 // (truncation 3e-20).  The result is scaled by 2^k through the exponent field (normal for x in [-708, 709]).
 // Half the polynomial of a table-free version, and -- what matters more here -- half the fp64 immediates.
 #include "exp_table.inc"
+#include "log_coeffs.inc"
 struct hm_d2 { double hi, lo; };
 #ifdef __CUDACC__
 __device__ const hm_d2 hm_exp2_tab_dev[64] = {HM_EXP2_TABLE};
@@ -83,7 +84,7 @@ __device__ const hm_d2 hm_exp2_tab_dev[64] = {HM_EXP2_TABLE};
 #if defined(__CUDACC__) && defined(HM_CONST_BANK_COEFFS)
 __constant__ double hm_kc[24] = {HM_64_LN2, -HM_LN2_64_HI, -HM_LN2_64_LO, 1.3888888888888889e-03, 8.3333333333333332e-03,
   4.1666666666666664e-02, 1.6666666666666666e-01, 0.0,
-  1.0 / 23.0, 1.0 / 21.0, 1.0 / 19.0, 1.0 / 17.0, 1.0 / 15.0, 1.0 / 13.0, 1.0 / 11.0, 1.0 / 9.0, 1.0 / 7.0, 1.0 / 5.0, 1.0 / 3.0,
+  HM_LOG_P7, HM_LOG_P6, HM_LOG_P5, HM_LOG_P4, HM_LOG_P3, HM_LOG_P2, HM_LOG_P1, 0.0, 0.0, 0.0, 0.0,
   6.93147180369123816490e-01, 1.90821492927058770002e-10, 0.0, 0.0, 0.0};
 #endif
 #if defined(__CUDA_ARCH__) && defined(HM_CONST_BANK_COEFFS)
@@ -155,7 +156,8 @@ HM_HD double hm_exp_fast(double x) {
 }
 
 // ln u for positive normal u: u = 2^e m, m in [sqrt(1/2), sqrt 2); ln m = 2 atanh(s), s = (m-1)/(m+1), |s| <= 0.1716,
-// atanh series to s^23 (truncation 6e-19 relative); the quotient by a Newton-refined reciprocal.
+// atanh(s)/s - 1 by 7 near-minimax coefficients in s^2 (log_coeffs.inc; the Taylor series needed 11 for the same 5e-18:
+// 4 fewer DFMA on the serial chain and 8 fewer immediate moves per call); the quotient by a Newton-refined reciprocal.
 // NEWTON: Newton steps on the seed before the correcting step (1 is enough, see hm_rcp_seed; 2 is the former code, kept
 // because the on-chip p = 1 kernel is FASTER with it: C2 +0.6 %, C1 / C0 +0.5 % with one step -- code generation, the
 // kernel is not issue-bound -- while the p = 2 streaming kernel gains 3.2 %).  A translation unit chooses with
@@ -180,17 +182,13 @@ HM_HD double hm_log_pos_n(double u) {
   double s = f * rc;
   s = hm_fma(hm_fma(-s, a, f), rc, s);                      // the correction squares the residual: s = f/a to ~0.5 ulp
   const double s2 = s * s;
-  double p = HM_KC(8, 1.0 / 23.0);
-  p = hm_fma(p, s2, HM_KC(9, 1.0 / 21.0));
-  p = hm_fma(p, s2, HM_KC(10, 1.0 / 19.0));
-  p = hm_fma(p, s2, HM_KC(11, 1.0 / 17.0));
-  p = hm_fma(p, s2, HM_KC(12, 1.0 / 15.0));
-  p = hm_fma(p, s2, HM_KC(13, 1.0 / 13.0));
-  p = hm_fma(p, s2, HM_KC(14, 1.0 / 11.0));
-  p = hm_fma(p, s2, HM_KC(15, 1.0 / 9.0));
-  p = hm_fma(p, s2, HM_KC(16, 1.0 / 7.0));
-  p = hm_fma(p, s2, HM_KC(17, 1.0 / 5.0));
-  p = hm_fma(p, s2, HM_KC(18, 1.0 / 3.0));
+  double p = HM_KC(8, HM_LOG_P7);                           // 7 near-minimax coefficients (gen_log_coeffs.py): 4.7e-18
+  p = hm_fma(p, s2, HM_KC(9, HM_LOG_P6));
+  p = hm_fma(p, s2, HM_KC(10, HM_LOG_P5));
+  p = hm_fma(p, s2, HM_KC(11, HM_LOG_P4));
+  p = hm_fma(p, s2, HM_KC(12, HM_LOG_P3));
+  p = hm_fma(p, s2, HM_KC(13, HM_LOG_P2));
+  p = hm_fma(p, s2, HM_KC(14, HM_LOG_P1));
   p = p * s2;                                               // atanh(s)/s - 1
   const double two_s = s + s;
   const double lm = hm_fma(two_s, p, two_s);                // ln m
