@@ -82,8 +82,8 @@ __device__ const hm_d2 hm_exp2_tab_dev[64] = {HM_EXP2_TABLE};
 // (k_resident<M1, SEL_SWEEP>), -0.6 % on C0, +0.3 % on C2, +1.3 % on C6, noise on C5 -- so a translation unit opts in with
 // HM_CONST_BANK_COEFFS (inst_binormal2d.cu and inst_thinned_schechter1d_selsweep.cu do).
 #if defined(__CUDACC__) && defined(HM_CONST_BANK_COEFFS)
-__constant__ double hm_kc[24] = {HM_64_LN2, -HM_LN2_64_HI, -HM_LN2_64_LO, 1.3888888888888889e-03, 8.3333333333333332e-03,
-  4.1666666666666664e-02, 1.6666666666666666e-01, 0.0,
+__constant__ double hm_kc[24] = {HM_64_LN2, -HM_LN2_64_HI, -HM_LN2_64_LO, HM_EXP_Q3, HM_EXP_Q2,
+  HM_EXP_Q1, HM_EXP_Q0, 0.0,
   HM_LOG_P7, HM_LOG_P6, HM_LOG_P5, HM_LOG_P4, HM_LOG_P3, HM_LOG_P2, HM_LOG_P1, 0.0, 0.0, 0.0, 0.0,
   6.93147180369123816490e-01, 1.90821492927058770002e-10, 0.0, 0.0, 0.0};
 #endif
@@ -110,11 +110,10 @@ HM_HD double hm_exp_core(double x) {
 #else
   const double thi = hm_exp2_tab_host[j].hi, tlo = hm_exp2_tab_host[j].lo;
 #endif
-  double p = HM_KC(3, 1.3888888888888889e-03);             // 1/6!
-  p = hm_fma(p, r, HM_KC(4, 8.3333333333333332e-03));      // 1/5!
-  p = hm_fma(p, r, HM_KC(5, 4.1666666666666664e-02));      // 1/4!
-  p = hm_fma(p, r, HM_KC(6, 1.6666666666666666e-01));      // 1/3!
-  p = hm_fma(p, r, 0.5);
+  double p = HM_KC(3, HM_EXP_Q3);                          // 4 near-minimax coefficients (gen_exp_table.py; absolute error
+  p = hm_fma(p, r, HM_KC(4, HM_EXP_Q2));                   // 4.4e-18 on e^r - 1: 0.04 ulp of the e^r it becomes; the Taylor
+  p = hm_fma(p, r, HM_KC(5, HM_EXP_Q1));                   // polynomial took 5) -- NOT for hm_expm1_nonpos below, which needs
+  p = hm_fma(p, r, HM_KC(6, HM_EXP_Q0));                   // relative accuracy at small |x| and keeps the Taylor form
   p = p * r;
   p = hm_fma(p, r, r);                                     // e^r - 1
   const double y = thi + hm_fma(thi, p, tlo);              // T[j] e^r
