@@ -38,16 +38,16 @@ ALG_BYTES = {"C0": (48, 32), "C1": (48, 32), "C2": (48, 32), "C3": (112, 64), "C
 MODES = {"host": 0, "graph": 1, "tail": 2}
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel PER LAUNCH of K iterations, as (bytes per launch that do
 # not depend on K, bytes per iteration), from the committed `ncu --set full` captures under profiles/ (r02_*_ncu.md):
-#   C2  on-chip kernel: 14.62 MB at K = 20 (the driver's launch) and 14.70 MB at K = 300 -- the state load; nothing per iteration
-#   C3  streaming kernel (dedicated tail warps), 60 iterations: 320.5 MB = 5.3 MB per iteration (the 104 MB working set is
-#       served from L2: hit rate 96 %)
-#   C4  streaming kernel, 30 iterations: 8,345.4 MB = 278.2 MB per iteration (= the algorithmic 280 MB: nothing is re-read)
-#   C6  general on-chip kernel, 300 iterations: 3.17 MB, taken as the per-launch state load
+#   C2  on-chip kernel: 14.63 MB at K = 20 (the driver's launch) and 14.72 MB at K = 300 -- the state load; nothing per iteration
+#   C3  streaming kernel (dedicated tail warps), 60 iterations: 220.1 MB = 3.7 MB per iteration (the 104 MB working set is
+#       served from L2: hit rate 96 %; 3.7-5.6 MB per iteration from capture to capture)
+#   C4  streaming kernel, 30 iterations: 8,335.9 MB = 277.9 MB per iteration (= the algorithmic 280 MB: nothing is re-read)
+#   C6  general on-chip kernel, 300 iterations: 3.25 MB, taken as the per-launch state load
 # A config without a capture reports traffic = null.
-NCU_DRAM_BYTES = {"C2": (14.62e6, 0.0), "C3": (0.0, 320.50e6 / 60), "C4": (0.0, 8345.40e6 / 30), "C6": (3.17e6, 0.0)}
+NCU_DRAM_BYTES = {"C2": (14.63e6, 0.0), "C3": (0.0, 220.09e6 / 60), "C4": (0.0, 8335.89e6 / 30), "C6": (3.25e6, 0.0)}
 # warp-level instructions executed per 32 object-updates (smsp__inst_executed.sum / (N K / 32)) and fp64-pipe activity from
 # the same captures.  They give the compute floor reported beside the HBM one: issue slots (4 warp-instructions / clk / SM).
-NCU_WARP_INSTR_PER_32 = {"C2": (388, 38.5), "C3": (394, 42.0), "C4": (138, 12.0), "C6": (1224, 14.9)}
+NCU_WARP_INSTR_PER_32 = {"C2": (389, 37.6), "C3": (392, 42.3), "C4": (138, 12.0), "C6": (1223, 14.9)}
 N_SMS, SM_CLOCK_HZ = 148, 1.965e9
 
 
